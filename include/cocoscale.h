@@ -1,0 +1,228 @@
+/*
+ * cocoscale.h -- C ABI of the B200-native replicated decoder-layer hot path of CoCoScale
+ * (arxiv/paper_2607_04181, "layer-wise scaling"; PAPER.md = the paper text as surveyed).
+ *
+ * What this library is: the forward of ONE hot decoder layer over a decode batch that is split
+ * across that layer's replicas (section 3.1), on ONE GPU, where a replica is an
+ * extra byte copy of the layer's weights held in reclaimed HBM; plus creating / retiring such
+ * replicas without ever re-capturing the CUDA Graph that replays the forward (the paper
+ * re-captures when the configuration vector v changes; here a device-resident
+ * replica table is read by the kernels instead).
+ *
+ * Layer arithmetic (BASELINE.json north_star; the paper gives none):  RMSNorm -> QKV projection
+ * -> RoPE (rotate-half, position seq_len-1) -> KV append -> paged GQA decode attention
+ * -> O projection + residual -> RMSNorm -> SwiGLU MLP -> down projection + residual.
+ * bf16 storage, fp32 accumulation.  Readings of every point the paper leaves open: DESIGN.md.
+ *
+ * Conventions
+ *   - All pointers named *_dev / documented "device" are device memory of the context's GPU;
+ *     everything else is host memory.  The library never takes ownership of caller memory.
+ *   - `stream` arguments are a `cudaStream_t` passed as `void*` (NULL = legacy default stream).
+ *   - Every call returns a cc_status; on failure cc_last_error() (thread-local) says why.
+ *     No exception or abort crosses this boundary.
+ *   - One control thread per cc_ctx.  cc_forward only ENQUEUES work (no allocation, no
+ *     synchronisation, no host read of device data) and is safe inside stream capture.
+ *   - Caller-owned buffers handed to cc_forward (hidden, KV pools, block table, seq_lens,
+ *     replica_assign) must keep their addresses while a captured graph that contains the call is
+ *     alive ("tensor memory addresses remain constant across iterations").
+ *   - There is no CPU fallback: without a usable CUDA device every compute entry point fails
+ *     with CC_ERR_CUDA.
+ */
+#ifndef COCOSCALE_H_
+#define COCOSCALE_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+#if defined(__GNUC__)
+#pragma GCC visibility push(default)   /* the library is built with -fvisibility=hidden */
+#endif
+
+#define CC_MAX_REPLICAS 4   /* P_max = 4 */
+#define CC_PAGE_SIZE 16     /* tokens per KV page (BASELINE.json configs) */
+#define CC_MAX_LAYERS 128   /* rows of the device replica table per context */
+
+typedef enum {
+    CC_OK = 0,
+    CC_ERR_INVALID = 1,  /* bad argument / unsupported shape                                  */
+    CC_ERR_NO_SLOT = 2,  /* no donated range can hold another replica (infeasible Delta_res,  */
+                         /* PAPER.md:320-323)                                                 */
+    CC_ERR_CUDA = 3,     /* a CUDA call failed, or no device                                  */
+    CC_ERR_BUSY = 4,     /* range still holds a live slot / replica still copying             */
+    CC_ERR_STATE = 5     /* e.g. releasing replica 0 or a replica that is not live            */
+} cc_status;
+
+/* Bits of the sticky device error word (cc_poll_device_error). Set by kernels on contract
+ * violations that are only visible on the device inside a graph; never a fault. */
+#define CC_DEVERR_BAD_REPLICA 1u   /* replica_assign[b] not an active replica: row ran on replica 0 */
+#define CC_DEVERR_BAD_PAGE 2u      /* block-table entry < 0 or >= n_pages inside seq_len: row skipped */
+#define CC_DEVERR_BAD_SEQLEN 4u    /* seq_len > max_position or needs > max_blocks_per_seq: row skipped */
+#define CC_DEVERR_HANG 8u          /* reserved: an internal wait gave up (the kernel traps instead)       */
+
+typedef struct cc_ctx cc_ctx;     /* device, side stream, donated ranges, replica table, error word */
+typedef struct cc_layer cc_layer; /* one decoder layer: slot 0 blob, replica slots, workspace        */
+
+typedef struct {
+    int32_t hidden;              /* d; multiple of 64                                           */
+    int32_t n_q_heads;           /* Hq                                                          */
+    int32_t n_kv_heads;          /* Hkv; Hq % Hkv == 0 and Hq / Hkv <= 8                        */
+    int32_t head_dim;            /* Dh: 64 or 128                                               */
+    int32_t ffn;                 /* F (SwiGLU width)                                            */
+    float rms_eps;
+    float rope_base;
+    int32_t page_size;           /* must be CC_PAGE_SIZE                                        */
+    int32_t max_batch;           /* rows per cc_forward call, 1..256                            */
+    int32_t max_blocks_per_seq;  /* row width of the block table                                */
+    int32_t max_position;        /* largest seq_len accepted (RoPE table rows)                  */
+} cc_layer_desc;
+
+/* bf16, DEVICE, each matrix [out][in] row-major (y = W x), gains [hidden].
+ * wq [Hq*Dh][d], wk/wv [Hkv*Dh][d], wo [d][Hq*Dh], wgate/wup [F][d], wdown [d][F]. */
+typedef struct {
+    const void *g1, *wq, *wk, *wv, *wo, *g2, *wgate, *wup, *wdown;
+} cc_layer_weights;
+
+/* Paged KV cache of this layer (caller-owned, DEVICE).
+ * k_pool / v_pool: bf16 [n_pages][n_kv_heads][CC_PAGE_SIZE][head_dim]; K is stored post-RoPE.
+ * block_table: int32 [max_batch][max_blocks_per_seq]; entry j of row b is the page holding
+ * tokens [16j, 16j+16) of request b; padding = -1 (never dereferenced below seq_len). The caller
+ * has already placed the page that holds position seq_len-1. */
+typedef struct {
+    void *k_pool;
+    void *v_pool;
+    const int32_t *block_table;
+    int32_t n_pages;
+} cc_kv_pages;
+
+/* ---- context ------------------------------------------------------------------------------ */
+cc_status cc_ctx_create(int device, cc_ctx **out);
+cc_status cc_ctx_destroy(cc_ctx *ctx); /* all layers must have been destroyed */
+
+/* "Reclaimed HBM": lend [dev_base, dev_base+bytes) (device memory the caller keeps owning) as
+ * replica slot space.  Trimmed to 1024-byte boundaries.  CC_ERR_INVALID if it overlaps a range
+ * already donated.  cc_ctx_reclaim takes it back; CC_ERR_BUSY while any live slot lies in it. */
+cc_status cc_ctx_donate(cc_ctx *ctx, void *dev_base, size_t bytes);
+cc_status cc_ctx_reclaim(cc_ctx *ctx, void *dev_base);
+
+/* Chunk size of the replica copy ("fine-grained chunked transfer"); one kernel
+ * launch per chunk on the context's side stream.  Default 32 MiB; multiple of 1 MiB. */
+cc_status cc_ctx_set_copy_chunk(cc_ctx *ctx, size_t chunk_bytes);
+
+/* Programmatic dependent launch between the kernels of one cc_forward (default on; the
+ * environment variable CC_PDL=0 turns it off at cc_ctx_create).  A launch attribute only: the
+ * kernels and their results are the same either way. */
+cc_status cc_ctx_set_pdl(cc_ctx *ctx, int enabled);
+
+/* Sticky device error word (CC_DEVERR_* bits); reading clears it. Synchronises the device. */
+cc_status cc_poll_device_error(cc_ctx *ctx, uint32_t *bits);
+
+/* ---- layer lifecycle ------------------------------------------------------------------------ */
+/* Re-packs the nine weight tensors into one library-owned blob ("slot 0": tcgen05 operand tile
+ * images + gains), allocates the layer's workspace and its replica-table row.  Everything the
+ * layer will ever need is allocated here (PAPER.md:393 persistent pool); later calls allocate
+ * nothing on the device.  Synchronous. */
+cc_status cc_create_layer(cc_ctx *ctx, const cc_layer_desc *desc, const cc_layer_weights *weights_dev,
+                          cc_layer **out);
+cc_status cc_destroy_layer(cc_layer *layer);
+
+/* Bytes of one replica slot of this layer (= bytes cc_scale_layer copies per new replica). */
+cc_status cc_layer_blob_bytes(const cc_layer *layer, size_t *bytes);
+
+/* Set the TARGET replica count, 1..CC_MAX_REPLICAS (a replica is a copy of the
+ * layer's weights).  Growing: takes the lowest free slot(s) from the donated ranges and enqueues
+ * the chunked in-HBM copy of slot 0 on the side stream; returns at once (CC_ERR_NO_SLOT if no
+ * range fits; nothing changes then).  Shrinking: marks the highest-numbered live replicas for
+ * retirement.  Nothing becomes visible to cc_forward until cc_commit. */
+cc_status cc_scale_layer(cc_layer *layer, int n_replicas);
+
+/* Publish: makes `stream` wait for the finished copies, then enqueues the replica-table update
+ * (new rows / retired rows) on `stream`, so that forwards enqueued or replayed on `stream`
+ * AFTER this call see the new replica set and earlier ones the old.  Retired slots return to
+ * the allocator once the work enqueued before the flip has finished (checked lazily by later
+ * calls).  Never captures or re-captures anything; must be called outside stream capture.
+ * No-op when nothing is pending. */
+cc_status cc_commit(cc_layer *layer, void *stream);
+
+/* Retire one live replica (1..CC_MAX_REPLICAS-1); takes effect at the next cc_commit.
+ * CC_ERR_STATE for replica 0 or a replica that is not live / already retiring. */
+cc_status cc_release_replica(cc_layer *layer, int replica);
+
+/* n_active: replicas visible to forwards enqueued now; n_pending: copies enqueued by
+ * cc_scale_layer and not yet committed. Either pointer may be NULL. */
+cc_status cc_query(cc_layer *layer, int *n_active, int *n_pending);
+
+/* Device address and size of replica r's blob (for byte-exact checks of the copy). */
+cc_status cc_replica_blob(cc_layer *layer, int replica, const void **blob_dev, size_t *bytes);
+
+/* ---- the hot path --------------------------------------------------------------------------- */
+/* One decode step of the layer over `batch` rows (batch <= max_batch), in place on hidden_dev.
+ *   hidden_dev      bf16 [batch][hidden], DEVICE; row b is replaced by the layer's output for
+ *                   request b (original request order: PAPER.md:101 gather + concat).
+ *   kv              see cc_kv_pages; the step appends request b's new K/V at position
+ *                   seq_lens[b]-1 and attends over positions [0, seq_lens[b]).
+ *   seq_lens_dev    int32 [batch], DEVICE: tokens attended INCLUDING the one being decoded.
+ *                   seq_lens[b] <= 0 marks a padding row: left untouched, no KV write.
+ *   replica_assign_dev  int32 [batch], DEVICE: which replica's weights serve row b
+ *                   (PAPER.md:93 sub-batches; any assignment, any group sizes including 0).
+ * Rows are grouped by replica on the device; each group streams ITS replica's weight slot, read
+ * through the device replica table, so a graph captured around this call keeps working across
+ * cc_commit.  Results are bit-identical for any assignment and replica count. */
+cc_status cc_forward(cc_layer *layer, void *hidden_dev, const cc_kv_pages *kv, const int32_t *seq_lens_dev,
+                     const int32_t *replica_assign_dev, int batch, void *stream);
+
+/* Same step with HOST buffers for the per-step inputs (pinned memory recommended): copies
+ * hidden, block table, seq_lens and replica_assign to library-owned device staging, runs
+ * cc_forward, copies hidden back and synchronises `stream`.  The KV pools stay on the device
+ * (they are state, like the weights).  block_table_host is [batch][max_blocks_per_seq]. */
+cc_status cc_forward_host(cc_layer *layer, void *hidden_host, void *k_pool_dev, void *v_pool_dev,
+                          int32_t n_pages, const int32_t *block_table_host, const int32_t *seq_lens_host,
+                          const int32_t *replica_assign_host, int batch, void *stream);
+
+/* Kernel launches one cc_forward enqueues (for launch accounting). */
+cc_status cc_forward_launch_count(const cc_layer *layer, int *n);
+
+/* The vectorised chunked copy kernel on its own: dst/src DEVICE, 32-byte aligned (256-bit
+ * accesses), bytes % 16 == 0, else CC_ERR_INVALID; chunk_bytes = 0 uses the context's chunk size.
+ * Enqueue-only on `stream`. */
+cc_status cc_replica_copy(cc_ctx *ctx, void *dst_dev, const void *src_dev, size_t bytes, size_t chunk_bytes,
+                          void *stream);
+
+/* ---- stage taps (tests only; reads the workspace left by the last cc_forward) ---------------- */
+typedef enum {
+    CC_TAP_X = 0,   /* [batch][hidden]      input RMSNorm output (bf16 operand, widened)        */
+    CC_TAP_Q = 1,   /* [batch][Hq*Dh]       q after RoPE (fp32)                                 */
+    CC_TAP_O = 2,   /* [batch][Hq*Dh]       attention output (bf16 operand, widened)            */
+    CC_TAP_H1 = 3,  /* [batch][hidden]      hidden + O-projection (fp32)                        */
+    CC_TAP_Y = 4,   /* [batch][hidden]      post-attention RMSNorm output (bf16 operand)        */
+    CC_TAP_A = 5    /* [batch][ffn]         silu(gate)*up (bf16 operand)                        */
+} cc_tap;
+/* out_host: fp32 [batch][dim] in ORIGINAL row order; padding rows are zero. Synchronous. */
+cc_status cc_debug_tap(cc_layer *layer, cc_tap which, float *out_host, int batch);
+/* perm_host[pos] (int32, length >= max_batch + 64): original row at grouped position pos or -1;
+ * counts_host[CC_MAX_REPLICAS]: rows per replica group, from the last cc_forward. Synchronous. */
+cc_status cc_debug_grouping(cc_layer *layer, int32_t *perm_host, int32_t *counts_host, int32_t *n_pos);
+
+/* ---- host-only slot allocator (the same code cc_ctx uses; exposed so it can be tested without
+ * a GPU).  Addresses are plain integers here. ---------------------------------------------------- */
+typedef struct cc_slotalloc cc_slotalloc;
+cc_slotalloc *cc_slotalloc_create(void);
+void cc_slotalloc_destroy(cc_slotalloc *a);
+cc_status cc_slotalloc_donate(cc_slotalloc *a, uint64_t base, uint64_t bytes);
+cc_status cc_slotalloc_reclaim(cc_slotalloc *a, uint64_t base);
+cc_status cc_slotalloc_alloc(cc_slotalloc *a, uint64_t bytes, uint64_t *addr); /* lowest address that fits */
+cc_status cc_slotalloc_free(cc_slotalloc *a, uint64_t addr);
+uint64_t cc_slotalloc_free_bytes(const cc_slotalloc *a);
+
+const char *cc_last_error(void);
+const char *cc_version(void);
+
+#if defined(__GNUC__)
+#pragma GCC visibility pop
+#endif
+#ifdef __cplusplus
+}
+#endif
+#endif /* COCOSCALE_H_ */

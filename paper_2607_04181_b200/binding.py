@@ -1,0 +1,265 @@
+"""Thin ctypes binding over libcocoscale.so -- same names as include/cocoscale.h, argument
+marshalling only (every step of the hot path runs in the CUDA kernels behind the C ABI).
+
+Device pointers may be given as torch CUDA tensors (their data_ptr() is passed), as ints, or as
+None (NULL); host buffers as numpy arrays / torch CPU tensors.  Streams are passed as the raw
+`cudaStream_t` integer (torch.cuda.Stream.cuda_stream) or None for the legacy default stream.
+Every call raises CcError when the library returns a non-zero cc_status.  There is no CPU
+fallback: if the library cannot be loaded, importing this module raises.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+import numpy as np
+
+from . import build as _build
+
+CC_MAX_REPLICAS = 4
+CC_PAGE_SIZE = 16
+CC_MAX_LAYERS = 128
+CC_OK, CC_ERR_INVALID, CC_ERR_NO_SLOT, CC_ERR_CUDA, CC_ERR_BUSY, CC_ERR_STATE = range(6)
+STATUS_NAMES = ("CC_OK", "CC_ERR_INVALID", "CC_ERR_NO_SLOT", "CC_ERR_CUDA", "CC_ERR_BUSY", "CC_ERR_STATE")
+CC_DEVERR_BAD_REPLICA, CC_DEVERR_BAD_PAGE, CC_DEVERR_BAD_SEQLEN, CC_DEVERR_HANG = 1, 2, 4, 8
+CC_TAP_X, CC_TAP_Q, CC_TAP_O, CC_TAP_H1, CC_TAP_Y, CC_TAP_A = range(6)
+
+# every function include/cocoscale.h declares (checked against the header by tests/test_cabi.py)
+EXPORTS = (
+    "cc_ctx_create", "cc_ctx_destroy", "cc_ctx_donate", "cc_ctx_reclaim", "cc_ctx_set_copy_chunk",
+    "cc_ctx_set_pdl", "cc_poll_device_error", "cc_create_layer", "cc_destroy_layer", "cc_layer_blob_bytes",
+    "cc_scale_layer", "cc_commit", "cc_release_replica", "cc_query", "cc_replica_blob", "cc_forward",
+    "cc_forward_host", "cc_forward_launch_count", "cc_replica_copy", "cc_debug_tap", "cc_debug_grouping",
+    "cc_slotalloc_create", "cc_slotalloc_destroy", "cc_slotalloc_donate", "cc_slotalloc_reclaim",
+    "cc_slotalloc_alloc", "cc_slotalloc_free", "cc_slotalloc_free_bytes", "cc_last_error", "cc_version",
+)
+
+
+class CcError(RuntimeError):
+    def __init__(self, status: int, message: str):
+        super().__init__(f"{STATUS_NAMES[status] if 0 <= status < len(STATUS_NAMES) else status}: {message}")
+        self.status = status
+
+
+class cc_layer_desc(C.Structure):
+    _fields_ = [("hidden", C.c_int32), ("n_q_heads", C.c_int32), ("n_kv_heads", C.c_int32),
+                ("head_dim", C.c_int32), ("ffn", C.c_int32), ("rms_eps", C.c_float), ("rope_base", C.c_float),
+                ("page_size", C.c_int32), ("max_batch", C.c_int32), ("max_blocks_per_seq", C.c_int32),
+                ("max_position", C.c_int32)]
+
+
+class cc_layer_weights(C.Structure):
+    _fields_ = [(n, C.c_void_p) for n in ("g1", "wq", "wk", "wv", "wo", "g2", "wgate", "wup", "wdown")]
+
+
+class cc_kv_pages(C.Structure):
+    _fields_ = [("k_pool", C.c_void_p), ("v_pool", C.c_void_p), ("block_table", C.c_void_p), ("n_pages", C.c_int32)]
+
+
+def _load() -> C.CDLL:
+    path = _build.LIB
+    if _build.needs_build():
+        try:
+            _build.build()
+        except Exception as e:  # no nvcc and no prebuilt library: fail loudly, never fall back
+            if not os.path.exists(path):
+                raise ImportError(f"libcocoscale.so is missing and could not be built: {e}") from e
+    return C.CDLL(path)
+
+
+_lib = _load()
+_lib.cc_last_error.restype = C.c_char_p
+_lib.cc_version.restype = C.c_char_p
+_lib.cc_slotalloc_create.restype = C.c_void_p
+_lib.cc_slotalloc_free_bytes.restype = C.c_uint64
+_lib.cc_slotalloc_free_bytes.argtypes = [C.c_void_p]
+_lib.cc_slotalloc_destroy.argtypes = [C.c_void_p]
+_lib.cc_slotalloc_destroy.restype = None
+
+
+def library_path() -> str:
+    return _build.LIB
+
+
+def _ptr(x) -> C.c_void_p:
+    if x is None:
+        return C.c_void_p(0)
+    if isinstance(x, int):
+        return C.c_void_p(x)
+    if hasattr(x, "data_ptr"):
+        return C.c_void_p(x.data_ptr())
+    if isinstance(x, np.ndarray):
+        assert x.flags["C_CONTIGUOUS"]
+        return C.c_void_p(x.ctypes.data)
+    if isinstance(x, C.c_void_p):
+        return x
+    raise TypeError(f"cannot pass {type(x)} as a pointer")
+
+
+def _stream(s) -> C.c_void_p:
+    if s is None:
+        return C.c_void_p(0)
+    if hasattr(s, "cuda_stream"):
+        return C.c_void_p(s.cuda_stream)
+    return C.c_void_p(int(s))
+
+
+def _check(status: int) -> None:
+    if status != CC_OK:
+        raise CcError(status, cc_last_error())
+
+
+def cc_last_error() -> str:
+    return (_lib.cc_last_error() or b"").decode()
+
+
+def cc_version() -> str:
+    return _lib.cc_version().decode()
+
+
+# ---- context ---------------------------------------------------------------------------------
+def cc_ctx_create(device: int = 0) -> C.c_void_p:
+    out = C.c_void_p()
+    _check(_lib.cc_ctx_create(C.c_int(device), C.byref(out)))
+    return out
+
+
+def cc_ctx_destroy(ctx) -> None:
+    _check(_lib.cc_ctx_destroy(ctx))
+
+
+def cc_ctx_donate(ctx, dev_base, nbytes: int) -> None:
+    _check(_lib.cc_ctx_donate(ctx, _ptr(dev_base), C.c_size_t(nbytes)))
+
+
+def cc_ctx_reclaim(ctx, dev_base) -> None:
+    _check(_lib.cc_ctx_reclaim(ctx, _ptr(dev_base)))
+
+
+def cc_ctx_set_copy_chunk(ctx, chunk_bytes: int) -> None:
+    _check(_lib.cc_ctx_set_copy_chunk(ctx, C.c_size_t(chunk_bytes)))
+
+
+def cc_ctx_set_pdl(ctx, enabled: bool) -> None:
+    _check(_lib.cc_ctx_set_pdl(ctx, C.c_int(1 if enabled else 0)))
+
+
+def cc_poll_device_error(ctx) -> int:
+    bits = C.c_uint32()
+    _check(_lib.cc_poll_device_error(ctx, C.byref(bits)))
+    return bits.value
+
+
+# ---- layer lifecycle ---------------------------------------------------------------------------
+def cc_create_layer(ctx, desc: cc_layer_desc, weights: dict) -> C.c_void_p:
+    """`weights`: name -> device tensor / pointer for g1 wq wk wv wo g2 wgate wup wdown (bf16)."""
+    w = cc_layer_weights(*[_ptr(weights[n[0]]) for n in cc_layer_weights._fields_])
+    out = C.c_void_p()
+    _check(_lib.cc_create_layer(ctx, C.byref(desc), C.byref(w), C.byref(out)))
+    return out
+
+
+def cc_destroy_layer(layer) -> None:
+    _check(_lib.cc_destroy_layer(layer))
+
+
+def cc_layer_blob_bytes(layer) -> int:
+    n = C.c_size_t()
+    _check(_lib.cc_layer_blob_bytes(layer, C.byref(n)))
+    return n.value
+
+
+def cc_scale_layer(layer, n_replicas: int) -> None:
+    _check(_lib.cc_scale_layer(layer, C.c_int(n_replicas)))
+
+
+def cc_commit(layer, stream=None) -> None:
+    _check(_lib.cc_commit(layer, _stream(stream)))
+
+
+def cc_release_replica(layer, replica: int) -> None:
+    _check(_lib.cc_release_replica(layer, C.c_int(replica)))
+
+
+def cc_query(layer):
+    a, p = C.c_int(), C.c_int()
+    _check(_lib.cc_query(layer, C.byref(a), C.byref(p)))
+    return a.value, p.value
+
+
+def cc_replica_blob(layer, replica: int):
+    ptr, n = C.c_void_p(), C.c_size_t()
+    _check(_lib.cc_replica_blob(layer, C.c_int(replica), C.byref(ptr), C.byref(n)))
+    return ptr.value, n.value
+
+
+# ---- hot path ----------------------------------------------------------------------------------
+def cc_forward(layer, hidden, k_pool, v_pool, block_table, n_pages: int, seq_lens, replica_assign, batch: int,
+               stream=None) -> None:
+    kv = cc_kv_pages(_ptr(k_pool), _ptr(v_pool), _ptr(block_table), C.c_int32(n_pages))
+    _check(_lib.cc_forward(layer, _ptr(hidden), C.byref(kv), _ptr(seq_lens), _ptr(replica_assign), C.c_int(batch),
+                           _stream(stream)))
+
+
+def cc_forward_host(layer, hidden_host, k_pool, v_pool, n_pages: int, block_table_host, seq_lens_host,
+                    replica_assign_host, batch: int, stream=None) -> None:
+    _check(_lib.cc_forward_host(layer, _ptr(hidden_host), _ptr(k_pool), _ptr(v_pool), C.c_int32(n_pages),
+                                _ptr(block_table_host), _ptr(seq_lens_host), _ptr(replica_assign_host),
+                                C.c_int(batch), _stream(stream)))
+
+
+def cc_forward_launch_count(layer) -> int:
+    n = C.c_int()
+    _check(_lib.cc_forward_launch_count(layer, C.byref(n)))
+    return n.value
+
+
+def cc_replica_copy(ctx, dst, src, nbytes: int, chunk_bytes: int = 0, stream=None) -> None:
+    _check(_lib.cc_replica_copy(ctx, _ptr(dst), _ptr(src), C.c_size_t(nbytes), C.c_size_t(chunk_bytes),
+                                _stream(stream)))
+
+
+# ---- stage taps (tests) ------------------------------------------------------------------------
+def cc_debug_tap(layer, which: int, batch: int, dim: int) -> np.ndarray:
+    out = np.zeros((batch, dim), dtype=np.float32)
+    _check(_lib.cc_debug_tap(layer, C.c_int(which), _ptr(out), C.c_int(batch)))
+    return out
+
+
+def cc_debug_grouping(layer, max_batch: int):
+    perm = np.full(max_batch + 80, -1, dtype=np.int32)
+    counts = np.zeros(CC_MAX_REPLICAS, dtype=np.int32)
+    n_pos = C.c_int32()
+    _check(_lib.cc_debug_grouping(layer, _ptr(perm), _ptr(counts), C.byref(n_pos)))
+    return perm[:n_pos.value].copy(), counts, n_pos.value
+
+
+# ---- host-only slot allocator --------------------------------------------------------------------
+def cc_slotalloc_create() -> C.c_void_p:
+    return C.c_void_p(_lib.cc_slotalloc_create())
+
+
+def cc_slotalloc_destroy(a) -> None:
+    _lib.cc_slotalloc_destroy(a)
+
+
+def cc_slotalloc_donate(a, base: int, nbytes: int) -> int:
+    return _lib.cc_slotalloc_donate(a, C.c_uint64(base), C.c_uint64(nbytes))
+
+
+def cc_slotalloc_reclaim(a, base: int) -> int:
+    return _lib.cc_slotalloc_reclaim(a, C.c_uint64(base))
+
+
+def cc_slotalloc_alloc(a, nbytes: int):
+    addr = C.c_uint64()
+    st = _lib.cc_slotalloc_alloc(a, C.c_uint64(nbytes), C.byref(addr))
+    return st, (addr.value if st == CC_OK else None)
+
+
+def cc_slotalloc_free(a, addr: int) -> int:
+    return _lib.cc_slotalloc_free(a, C.c_uint64(addr))
+
+
+def cc_slotalloc_free_bytes(a) -> int:
+    return int(_lib.cc_slotalloc_free_bytes(a))

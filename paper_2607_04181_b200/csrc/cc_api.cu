@@ -1,0 +1,741 @@
+// cc_api.cu -- host side of libcocoscale: the C ABI of include/cocoscale.h (product code).
+// Context, weight-slot allocator over donated ("reclaimed") HBM, replica state machine, device
+// replica table, chunked side-stream replica copy, and the enqueue-only forward chain.
+#include "../../include/cocoscale.h"
+#include "cc_kernels.h"
+
+#include <cmath>
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+#include <map>
+#include <new>
+#include <string>
+#include <vector>
+
+cudaError_t cc_gemm_configure();
+cudaError_t cc_attn_configure();
+cudaError_t cc_rowwise_configure(int max_d);
+
+namespace {
+
+thread_local std::string g_err;
+
+cc_status fail(cc_status st, const char* fmt, ...) {
+    char buf[512];
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(buf, sizeof buf, fmt, ap);
+    va_end(ap);
+    g_err = buf;
+    return st;
+}
+#define CC_CUDA(expr)                                                                              \
+    do {                                                                                           \
+        cudaError_t e_ = (expr);                                                                   \
+        if (e_ != cudaSuccess) return fail(CC_ERR_CUDA, "%s: %s", #expr, cudaGetErrorString(e_)); \
+    } while (0)
+
+constexpr uint64_t kSlotAlign = 1024;
+inline uint64_t up(uint64_t x, uint64_t a) { return (x + a - 1) / a * a; }
+
+}  // namespace
+
+// ---- slot allocator (host only; also exported for CPU tests) ------------------------------------
+// Address-ordered: donated ranges keyed by the base the caller passed, live allocations in one
+// ordered map.  alloc = first fit inside each range, lowest address over all ranges.
+struct cc_slotalloc {
+    struct Range { uint64_t key, lo, hi; };
+    std::vector<Range> ranges;
+    std::map<uint64_t, uint64_t> live;   // addr -> size (rounded up to kSlotAlign)
+};
+
+extern "C" {
+
+cc_slotalloc* cc_slotalloc_create(void) { return new (std::nothrow) cc_slotalloc(); }
+void cc_slotalloc_destroy(cc_slotalloc* a) { delete a; }
+
+cc_status cc_slotalloc_donate(cc_slotalloc* a, uint64_t base, uint64_t bytes) {
+    if (!a) return fail(CC_ERR_INVALID, "null allocator");
+    const uint64_t lo = up(base, kSlotAlign), hi = (base + bytes) / kSlotAlign * kSlotAlign;
+    if (hi <= lo) return fail(CC_ERR_INVALID, "donated range is empty after trimming to %llu-byte boundaries",
+                              (unsigned long long)kSlotAlign);
+    for (const auto& r : a->ranges)
+        if (r.key == base || (lo < r.hi && r.lo < hi)) return fail(CC_ERR_INVALID, "range overlaps a donated range");
+    a->ranges.push_back({base, lo, hi});
+    return CC_OK;
+}
+
+cc_status cc_slotalloc_reclaim(cc_slotalloc* a, uint64_t base) {
+    if (!a) return fail(CC_ERR_INVALID, "null allocator");
+    for (size_t i = 0; i < a->ranges.size(); ++i) {
+        if (a->ranges[i].key != base) continue;
+        const auto& r = a->ranges[i];
+        auto it = a->live.lower_bound(r.lo);
+        if (it != a->live.end() && it->first < r.hi) return fail(CC_ERR_BUSY, "range still holds a live slot");
+        a->ranges.erase(a->ranges.begin() + i);
+        return CC_OK;
+    }
+    return fail(CC_ERR_INVALID, "range was not donated");
+}
+
+cc_status cc_slotalloc_alloc(cc_slotalloc* a, uint64_t bytes, uint64_t* addr) {
+    if (!a || !addr) return fail(CC_ERR_INVALID, "null argument");
+    const uint64_t size = up(bytes ? bytes : 1, kSlotAlign);
+    bool found = false;
+    uint64_t best = 0;
+    for (const auto& r : a->ranges) {
+        uint64_t cur = r.lo;   // walk the gaps between live allocations of this range
+        for (auto it = a->live.lower_bound(r.lo); it != a->live.end() && it->first < r.hi; ++it) {
+            if (it->first >= cur + size) break;
+            cur = it->first + it->second;
+        }
+        if (cur + size <= r.hi && (!found || cur < best)) {
+            found = true;
+            best = cur;
+        }
+    }
+    if (!found) return fail(CC_ERR_NO_SLOT, "no donated range can hold %llu bytes", (unsigned long long)size);
+    a->live[best] = size;
+    *addr = best;
+    return CC_OK;
+}
+
+cc_status cc_slotalloc_free(cc_slotalloc* a, uint64_t addr) {
+    if (!a) return fail(CC_ERR_INVALID, "null allocator");
+    if (!a->live.erase(addr)) return fail(CC_ERR_INVALID, "address is not a live slot");
+    return CC_OK;
+}
+
+uint64_t cc_slotalloc_free_bytes(const cc_slotalloc* a) {
+    if (!a) return 0;
+    uint64_t tot = 0;
+    for (const auto& r : a->ranges) tot += r.hi - r.lo;
+    for (const auto& kv : a->live) tot -= kv.second;
+    return tot;
+}
+
+const char* cc_last_error(void) { return g_err.c_str(); }
+const char* cc_version(void) { return "cocoscale-b200 0.1 (sm_100a)"; }
+
+}  // extern "C"
+
+// ---- context ----------------------------------------------------------------------------------
+namespace {
+enum RepState { REP_EMPTY = 0, REP_COPYING = 1, REP_LIVE = 2, REP_RETIRING = 3 };
+struct Replica {
+    int state = REP_EMPTY;
+    uint8_t* blob = nullptr;
+    cudaEvent_t copied = nullptr;   // recorded on the side stream after the last chunk
+    bool published = false;         // named in the device table row
+};
+struct Zombie {                     // a retired slot waiting for its last reader
+    uint64_t addr;
+    cudaEvent_t after_flip;
+};
+}  // namespace
+
+struct cc_ctx {
+    int device = 0, n_sms = 0;
+    cudaStream_t side = nullptr;
+    cc_slotalloc* slots = nullptr;
+    CcLayerTable* table_dev = nullptr;   // [CC_MAX_LAYERS], fixed address for the life of the context
+    uint32_t* err_dev = nullptr;
+    size_t chunk = (size_t)32 << 20;
+    bool row_used[CC_MAX_LAYERS] = {};
+    int n_layers = 0;
+    bool pdl = true;
+    std::vector<Zombie> zombies;
+};
+
+struct cc_layer {
+    cc_ctx* ctx = nullptr;
+    int row = -1;
+    cc_layer_desc desc{};
+    CcDims D{};
+    CcWork W{};
+    size_t blob_bytes = 0;
+    uint8_t* blob0 = nullptr;
+    uint8_t* work_base = nullptr;
+    Replica rep[CC_MAX_REPLICAS];
+    CcLayerTable host_row{};
+    // staging for cc_forward_host
+    __nv_bfloat16* st_hidden = nullptr;
+    int* st_bt = nullptr;
+    int* st_sl = nullptr;
+    int* st_ra = nullptr;
+    int last_batch = 0;
+};
+
+namespace {
+
+void reap_zombies(cc_ctx* ctx, bool block) {
+    for (size_t i = 0; i < ctx->zombies.size();) {
+        Zombie& z = ctx->zombies[i];
+        cudaError_t e = block ? cudaEventSynchronize(z.after_flip) : cudaEventQuery(z.after_flip);
+        if (e == cudaSuccess) {
+            cc_slotalloc_free(ctx->slots, z.addr);
+            cudaEventDestroy(z.after_flip);
+            ctx->zombies.erase(ctx->zombies.begin() + i);
+        } else {
+            if (e != cudaErrorNotReady) cudaGetLastError();
+            ++i;
+        }
+    }
+}
+
+cc_status set_device(cc_ctx* ctx) {
+    CC_CUDA(cudaSetDevice(ctx->device));
+    return CC_OK;
+}
+
+cc_status launch_chunked_copy(cc_ctx* ctx, void* dst, const void* src, size_t bytes, size_t chunk, cudaStream_t st) {
+    if (chunk == 0) chunk = ctx->chunk;
+    for (size_t off = 0; off < bytes; off += chunk) {
+        const size_t n = bytes - off < chunk ? bytes - off : chunk;
+        CC_CUDA(cc_launch_copy((uint8_t*)dst + off, (const uint8_t*)src + off, n, ctx->n_sms, st));
+    }
+    return CC_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+cc_status cc_ctx_create(int device, cc_ctx** out) {
+    if (!out) return fail(CC_ERR_INVALID, "out is null");
+    *out = nullptr;
+    int n_dev = 0;
+    if (cudaGetDeviceCount(&n_dev) != cudaSuccess || n_dev == 0) {
+        cudaGetLastError();
+        return fail(CC_ERR_CUDA, "no CUDA device (this library has no CPU fallback)");
+    }
+    if (device < 0 || device >= n_dev) return fail(CC_ERR_INVALID, "device %d out of range", device);
+    cudaDeviceProp prop;
+    CC_CUDA(cudaGetDeviceProperties(&prop, device));
+    if (prop.major != 10) return fail(CC_ERR_CUDA, "device is sm_%d%d; this library is sm_100a only", prop.major, prop.minor);
+    cc_ctx* ctx = new (std::nothrow) cc_ctx();
+    if (!ctx) return fail(CC_ERR_INVALID, "out of host memory");
+    ctx->device = device;
+    ctx->n_sms = prop.multiProcessorCount;
+    CC_CUDA(cudaSetDevice(device));
+    CC_CUDA(cudaStreamCreateWithFlags(&ctx->side, cudaStreamNonBlocking));
+    CC_CUDA(cudaMalloc(&ctx->table_dev, sizeof(CcLayerTable) * CC_MAX_LAYERS));
+    CC_CUDA(cudaMemset(ctx->table_dev, 0, sizeof(CcLayerTable) * CC_MAX_LAYERS));
+    CC_CUDA(cudaMalloc(&ctx->err_dev, 256));
+    CC_CUDA(cudaMemset(ctx->err_dev, 0, 256));
+    CC_CUDA(cc_gemm_configure());
+    CC_CUDA(cc_attn_configure());
+    CC_CUDA(cc_rowwise_configure(0));
+    ctx->slots = cc_slotalloc_create();
+    const char* env = getenv("CC_PDL");
+    if (env && env[0] == '0') ctx->pdl = false;
+    *out = ctx;
+    return CC_OK;
+}
+
+cc_status cc_ctx_destroy(cc_ctx* ctx) {
+    if (!ctx) return CC_OK;
+    if (ctx->n_layers) return fail(CC_ERR_BUSY, "%d layer(s) still alive", ctx->n_layers);
+    cudaSetDevice(ctx->device);
+    cudaDeviceSynchronize();
+    reap_zombies(ctx, true);
+    cudaStreamDestroy(ctx->side);
+    cudaFree(ctx->table_dev);
+    cudaFree(ctx->err_dev);
+    cc_slotalloc_destroy(ctx->slots);
+    delete ctx;
+    return CC_OK;
+}
+
+cc_status cc_ctx_donate(cc_ctx* ctx, void* dev_base, size_t bytes) {
+    if (!ctx || !dev_base) return fail(CC_ERR_INVALID, "null argument");
+    return cc_slotalloc_donate(ctx->slots, (uint64_t)(uintptr_t)dev_base, bytes);
+}
+
+cc_status cc_ctx_reclaim(cc_ctx* ctx, void* dev_base) {
+    if (!ctx) return fail(CC_ERR_INVALID, "null context");
+    reap_zombies(ctx, false);
+    cc_status st = cc_slotalloc_reclaim(ctx->slots, (uint64_t)(uintptr_t)dev_base);
+    if (st == CC_ERR_BUSY && !ctx->zombies.empty()) {   // retired slots whose last reader is still running
+        reap_zombies(ctx, true);
+        st = cc_slotalloc_reclaim(ctx->slots, (uint64_t)(uintptr_t)dev_base);
+    }
+    return st;
+}
+
+cc_status cc_ctx_set_copy_chunk(cc_ctx* ctx, size_t chunk_bytes) {
+    if (!ctx) return fail(CC_ERR_INVALID, "null context");
+    if (chunk_bytes == 0 || chunk_bytes % ((size_t)1 << 20)) return fail(CC_ERR_INVALID, "chunk must be a multiple of 1 MiB");
+    ctx->chunk = chunk_bytes;
+    return CC_OK;
+}
+
+cc_status cc_ctx_set_pdl(cc_ctx* ctx, int enabled) {
+    if (!ctx) return fail(CC_ERR_INVALID, "null context");
+    ctx->pdl = enabled != 0;
+    return CC_OK;
+}
+
+cc_status cc_poll_device_error(cc_ctx* ctx, uint32_t* bits) {
+    if (!ctx || !bits) return fail(CC_ERR_INVALID, "null argument");
+    CC_CUDA(cudaSetDevice(ctx->device));
+    CC_CUDA(cudaDeviceSynchronize());
+    CC_CUDA(cudaMemcpy(bits, ctx->err_dev, 4, cudaMemcpyDeviceToHost));
+    CC_CUDA(cudaMemset(ctx->err_dev, 0, 4));
+    return CC_OK;
+}
+
+cc_status cc_replica_copy(cc_ctx* ctx, void* dst_dev, const void* src_dev, size_t bytes, size_t chunk_bytes,
+                          void* stream) {
+    if (!ctx || !dst_dev || !src_dev) return fail(CC_ERR_INVALID, "null argument");
+    if ((((uintptr_t)dst_dev | (uintptr_t)src_dev) & 31) || (bytes & 15))
+        return fail(CC_ERR_INVALID, "pointers must be 32-byte aligned and the size a multiple of 16");
+    if (set_device(ctx) != CC_OK) return CC_ERR_CUDA;
+    return launch_chunked_copy(ctx, dst_dev, src_dev, bytes, chunk_bytes, (cudaStream_t)stream);
+}
+
+}  // extern "C"
+
+// ---- layer lifecycle ----------------------------------------------------------------------------
+namespace {
+
+CcGemmGeo make_geo(int n_out, int k_in, int n_sms, size_t w_off) {
+    CcGemmGeo g{};
+    g.T = (n_out + CC_TILE_N - 1) / CC_TILE_N;
+    g.KB = (k_in + CC_TILE_K - 1) / CC_TILE_K;
+    const long long atoms = (long long)g.T * g.KB;
+    g.P = atoms < n_sms ? (int)atoms : n_sms;   // no empty range => every piece slot is written
+    g.w_off = w_off;
+    return g;
+}
+size_t geo_bytes(const CcGemmGeo& g) { return (size_t)g.T * g.KB * CC_A_TILE_BYTES; }
+
+struct Carver {   // bump allocator over one cudaMalloc
+    size_t off = 0;
+    size_t take(size_t bytes, size_t align = 1024) {
+        off = (off + align - 1) / align * align;
+        const size_t r = off;
+        off += bytes;
+        return r;
+    }
+};
+
+void destroy_layer_memory(cc_layer* L) {
+    cudaFree(L->blob0);
+    cudaFree(L->work_base);
+}
+
+}  // namespace
+
+extern "C" {
+
+cc_status cc_create_layer(cc_ctx* ctx, const cc_layer_desc* desc, const cc_layer_weights* w, cc_layer** out) {
+    if (!ctx || !desc || !w || !out) return fail(CC_ERR_INVALID, "null argument");
+    *out = nullptr;
+    const cc_layer_desc& d = *desc;
+    if (d.hidden <= 0 || d.hidden % 64) return fail(CC_ERR_INVALID, "hidden must be a positive multiple of 64");
+    if (d.head_dim != 64 && d.head_dim != 128) return fail(CC_ERR_INVALID, "head_dim must be 64 or 128");
+    if (d.n_kv_heads <= 0 || d.n_q_heads <= 0 || d.n_q_heads % d.n_kv_heads || d.n_q_heads / d.n_kv_heads > 8)
+        return fail(CC_ERR_INVALID, "need n_q_heads %% n_kv_heads == 0 and a GQA group of at most 8");
+    if (d.ffn <= 0 || d.ffn % 8) return fail(CC_ERR_INVALID, "ffn must be a positive multiple of 8");
+    if (d.page_size != CC_PAGE_SIZE) return fail(CC_ERR_INVALID, "page_size must be %d", CC_PAGE_SIZE);
+    if (d.max_batch < 1 || d.max_batch > 256) return fail(CC_ERR_INVALID, "max_batch must be in 1..256");
+    if (d.max_blocks_per_seq < 1 || d.max_position < 1) return fail(CC_ERR_INVALID, "max_blocks_per_seq / max_position must be >= 1");
+    if (!(d.rms_eps > 0.f) || !(d.rope_base > 1.f)) return fail(CC_ERR_INVALID, "bad rms_eps / rope_base");
+    const void* ptrs[9] = {w->g1, w->wq, w->wk, w->wv, w->wo, w->g2, w->wgate, w->wup, w->wdown};
+    for (const void* p : ptrs)
+        if (!p || ((uintptr_t)p & 15)) return fail(CC_ERR_INVALID, "weight pointers must be non-null and 16-byte aligned");
+    int row = -1;
+    for (int i = 0; i < CC_MAX_LAYERS; ++i)
+        if (!ctx->row_used[i]) { row = i; break; }
+    if (row < 0) return fail(CC_ERR_INVALID, "context already holds %d layers", CC_MAX_LAYERS);
+    CC_CUDA(cudaSetDevice(ctx->device));
+
+    cc_layer* L = new (std::nothrow) cc_layer();
+    if (!L) return fail(CC_ERR_INVALID, "out of host memory");
+    L->ctx = ctx;
+    L->row = row;
+    L->desc = d;
+    CcDims& D = L->D;
+    D.d = d.hidden; D.Hq = d.n_q_heads; D.Hkv = d.n_kv_heads; D.Dh = d.head_dim; D.G = D.Hq / D.Hkv; D.F = d.ffn;
+    D.QD = D.Hq * D.Dh; D.KD = D.Hkv * D.Dh;
+    D.max_batch = d.max_batch; D.max_blocks = d.max_blocks_per_seq; D.max_position = d.max_position;
+    D.Mpad = (d.max_batch + 15) / 16 * 16 + 16 * CC_MAXR;
+    D.eps = d.rms_eps;
+    D.qk_scale_log2 = (float)(1.4426950408889634 / std::sqrt((double)D.Dh));
+    // blob layout: [QKV tiles][O tiles][gate/up tiles][down tiles][g1][g2]
+    Carver blob;
+    D.qkv = make_geo(D.QD + 2 * D.KD, D.d, ctx->n_sms, 0);
+    D.qkv.w_off = blob.take(geo_bytes(D.qkv));
+    D.o = make_geo(D.d, D.QD, ctx->n_sms, 0);
+    D.o.w_off = blob.take(geo_bytes(D.o));
+    D.gu = make_geo(2 * D.F, D.d, ctx->n_sms, 0);
+    D.gu.w_off = blob.take(geo_bytes(D.gu));
+    D.dn = make_geo(D.d, D.F, ctx->n_sms, 0);
+    D.dn.w_off = blob.take(geo_bytes(D.dn));
+    D.off_g1 = blob.take((size_t)D.d * 2);
+    D.off_g2 = blob.take((size_t)D.d * 2);
+    L->blob_bytes = blob.take(0);
+
+    // workspace
+    CcWork& W = L->W;
+    W.nch_max = (d.max_position + CC_ATTN_CHUNK - 1) / CC_ATTN_CHUNK;
+    Carver ws;
+    const size_t Mp = (size_t)D.Mpad;
+    const size_t o_sched = ws.take(sizeof(CcSched));
+    const size_t o_perm = ws.take(Mp * 4);
+    const size_t o_items = ws.take((size_t)d.max_batch * W.nch_max * sizeof(int2));
+    const size_t o_x = ws.take((size_t)D.qkv.KB * Mp * 128);
+    const size_t o_o = ws.take((size_t)D.o.KB * Mp * 128);
+    const size_t o_y = ws.take((size_t)D.gu.KB * Mp * 128);
+    const size_t o_a = ws.take((size_t)D.dn.KB * Mp * 128);
+    auto part_bytes = [&](const CcGemmGeo& g) { return (size_t)(g.P + g.T) * Mp * 128 * 4; };
+    const size_t o_pq = ws.take(part_bytes(D.qkv));
+    const size_t o_po = ws.take(part_bytes(D.o));
+    const size_t o_pg = ws.take(part_bytes(D.gu));
+    const size_t o_pd = ws.take(part_bytes(D.dn));
+    const size_t o_qrot = ws.take(Mp * D.QD * 4);
+    const size_t o_h1 = ws.take(Mp * D.d * 4);
+    const size_t o_atto = ws.take(Mp * D.Hq * W.nch_max * D.Dh * 4);
+    const size_t o_attml = ws.take(Mp * D.Hq * W.nch_max * sizeof(float2));
+    const size_t o_rope = ws.take((size_t)d.max_position * (D.Dh / 2) * sizeof(float2));
+    const size_t o_sth = ws.take((size_t)d.max_batch * D.d * 2);
+    const size_t o_stbt = ws.take((size_t)d.max_batch * d.max_blocks_per_seq * 4);
+    const size_t o_stsl = ws.take((size_t)d.max_batch * 4);
+    const size_t o_stra = ws.take((size_t)d.max_batch * 4);
+    const size_t ws_bytes = ws.take(0);
+
+    cudaError_t e = cudaMalloc(&L->blob0, L->blob_bytes);
+    if (e == cudaSuccess) e = cudaMalloc(&L->work_base, ws_bytes);
+    if (e == cudaSuccess) e = cudaMemset(L->work_base, 0, ws_bytes);
+    if (e == cudaSuccess) e = cudaMemset(L->blob0, 0, L->blob_bytes);
+    if (e != cudaSuccess) {
+        destroy_layer_memory(L);
+        delete L;
+        cudaGetLastError();
+        return fail(CC_ERR_CUDA, "device allocation of %zu + %zu bytes failed: %s", L->blob_bytes, ws_bytes, cudaGetErrorString(e));
+    }
+    uint8_t* wb = L->work_base;
+    W.sched = (CcSched*)(wb + o_sched); W.perm = (int*)(wb + o_perm); W.items = (int2*)(wb + o_items);
+    W.x_act = wb + o_x; W.o_act = wb + o_o; W.y_act = wb + o_y; W.a_act = wb + o_a;
+    W.qkv_part = (float*)(wb + o_pq); W.o_part = (float*)(wb + o_po); W.gu_part = (float*)(wb + o_pg);
+    W.d_part = (float*)(wb + o_pd);
+    W.q_rot = (float*)(wb + o_qrot); W.h1 = (float*)(wb + o_h1);
+    W.att_o = (float*)(wb + o_atto); W.att_ml = (float2*)(wb + o_attml);
+    W.rope_cs = (const float2*)(wb + o_rope);
+    W.err = ctx->err_dev;
+    L->st_hidden = (__nv_bfloat16*)(wb + o_sth); L->st_bt = (int*)(wb + o_stbt);
+    L->st_sl = (int*)(wb + o_stsl); L->st_ra = (int*)(wb + o_stra);
+
+    // RoPE table in fp64 on the host: angle = p * base^(-2i/Dh)  (rotate-half pairing, reading 4)
+    {
+        const int half = D.Dh / 2;
+        std::vector<float2> tab((size_t)d.max_position * half);
+        for (int i = 0; i < half; ++i) {
+            const double inv_freq = std::pow((double)d.rope_base, -2.0 * i / D.Dh);
+            for (int p = 0; p < d.max_position; ++p) {
+                const double th = (double)p * inv_freq;
+                tab[(size_t)p * half + i] = make_float2((float)std::cos(th), (float)std::sin(th));
+            }
+        }
+        e = cudaMemcpy(wb + o_rope, tab.data(), tab.size() * sizeof(float2), cudaMemcpyHostToDevice);
+    }
+    // one-time re-pack of the nine tensors into the blob (tcgen05 operand tile images + gains)
+    typedef const __nv_bfloat16* bp;
+    if (e == cudaSuccess)
+        e = cc_launch_pack(L->blob0 + D.qkv.w_off, (bp)w->wq, (bp)w->wk, (bp)w->wv, D.QD, D.KD, D.KD, 0, D.d, D.qkv.T,
+                           D.qkv.KB, 0);
+    if (e == cudaSuccess)
+        e = cc_launch_pack(L->blob0 + D.o.w_off, (bp)w->wo, nullptr, nullptr, D.d, 0, 0, 0, D.QD, D.o.T, D.o.KB, 0);
+    if (e == cudaSuccess)
+        e = cc_launch_pack(L->blob0 + D.gu.w_off, (bp)w->wgate, (bp)w->wup, nullptr, D.F, D.F, 0, 1, D.d, D.gu.T,
+                           D.gu.KB, 0);
+    if (e == cudaSuccess)
+        e = cc_launch_pack(L->blob0 + D.dn.w_off, (bp)w->wdown, nullptr, nullptr, D.d, 0, 0, 0, D.F, D.dn.T, D.dn.KB, 0);
+    if (e == cudaSuccess) e = cudaMemcpy(L->blob0 + D.off_g1, w->g1, (size_t)D.d * 2, cudaMemcpyDeviceToDevice);
+    if (e == cudaSuccess) e = cudaMemcpy(L->blob0 + D.off_g2, w->g2, (size_t)D.d * 2, cudaMemcpyDeviceToDevice);
+    L->rep[0].state = REP_LIVE;
+    L->rep[0].blob = L->blob0;
+    L->rep[0].published = true;
+    L->host_row = CcLayerTable{};
+    L->host_row.rep[0].blob = L->blob0;
+    L->host_row.active_mask = 1u;
+    if (e == cudaSuccess)
+        e = cudaMemcpy(ctx->table_dev + row, &L->host_row, sizeof(CcLayerTable), cudaMemcpyHostToDevice);
+    if (e == cudaSuccess) e = cudaDeviceSynchronize();
+    if (e != cudaSuccess) {
+        destroy_layer_memory(L);
+        delete L;
+        cudaGetLastError();
+        return fail(CC_ERR_CUDA, "cc_create_layer: %s", cudaGetErrorString(e));
+    }
+    ctx->row_used[row] = true;
+    ctx->n_layers++;
+    *out = L;
+    return CC_OK;
+}
+
+cc_status cc_destroy_layer(cc_layer* L) {
+    if (!L) return CC_OK;
+    cc_ctx* ctx = L->ctx;
+    cudaSetDevice(ctx->device);
+    cudaDeviceSynchronize();
+    for (int r = 1; r < CC_MAX_REPLICAS; ++r) {
+        if (L->rep[r].state != REP_EMPTY) cc_slotalloc_free(ctx->slots, (uint64_t)(uintptr_t)L->rep[r].blob);
+        if (L->rep[r].copied) cudaEventDestroy(L->rep[r].copied);
+    }
+    reap_zombies(ctx, true);
+    CcLayerTable zero{};
+    cudaMemcpy(ctx->table_dev + L->row, &zero, sizeof zero, cudaMemcpyHostToDevice);
+    destroy_layer_memory(L);
+    ctx->row_used[L->row] = false;
+    ctx->n_layers--;
+    delete L;
+    return CC_OK;
+}
+
+cc_status cc_layer_blob_bytes(const cc_layer* L, size_t* bytes) {
+    if (!L || !bytes) return fail(CC_ERR_INVALID, "null argument");
+    *bytes = L->blob_bytes;
+    return CC_OK;
+}
+
+}  // extern "C"
+
+// ---- scaling: create / publish / retire replicas ------------------
+extern "C" {
+
+cc_status cc_scale_layer(cc_layer* L, int n_replicas) {
+    if (!L) return fail(CC_ERR_INVALID, "null layer");
+    if (n_replicas < 1 || n_replicas > CC_MAX_REPLICAS) return fail(CC_ERR_INVALID, "n_replicas must be in 1..%d", CC_MAX_REPLICAS);
+    cc_ctx* ctx = L->ctx;
+    CC_CUDA(cudaSetDevice(ctx->device));
+    reap_zombies(ctx, false);
+    int cur = 0;
+    for (int r = 0; r < CC_MAX_REPLICAS; ++r) cur += (L->rep[r].state == REP_LIVE || L->rep[r].state == REP_COPYING);
+    if (n_replicas > cur) {
+        // take every slot first so that a failure changes nothing
+        int want = n_replicas - cur, got = 0, idx[CC_MAX_REPLICAS];
+        uint64_t addr[CC_MAX_REPLICAS];
+        for (int r = 1; r < CC_MAX_REPLICAS && got < want; ++r) {
+            if (L->rep[r].state != REP_EMPTY) continue;
+            if (cc_slotalloc_alloc(ctx->slots, L->blob_bytes, &addr[got]) != CC_OK) break;
+            idx[got++] = r;
+        }
+        if (got < want) {
+            for (int i = 0; i < got; ++i) cc_slotalloc_free(ctx->slots, addr[i]);
+            return fail(CC_ERR_NO_SLOT, "no free slot of %zu bytes for replica %d of this layer (free: %llu bytes)",
+                        L->blob_bytes, cur + got, (unsigned long long)cc_slotalloc_free_bytes(ctx->slots));
+        }
+        for (int i = 0; i < got; ++i) {
+            Replica& R = L->rep[idx[i]];
+            R.blob = (uint8_t*)(uintptr_t)addr[i];
+            R.state = REP_COPYING;
+            R.published = false;
+            if (!R.copied) CC_CUDA(cudaEventCreateWithFlags(&R.copied, cudaEventDisableTiming));
+            cc_status st = launch_chunked_copy(ctx, R.blob, L->blob0, L->blob_bytes, 0, ctx->side);
+            if (st != CC_OK) return st;
+            CC_CUDA(cudaEventRecord(R.copied, ctx->side));
+        }
+    } else if (n_replicas < cur) {
+        int drop = cur - n_replicas;
+        for (int r = CC_MAX_REPLICAS - 1; r >= 1 && drop > 0; --r) {
+            if (L->rep[r].state == REP_LIVE || L->rep[r].state == REP_COPYING) {
+                L->rep[r].state = REP_RETIRING;
+                --drop;
+            }
+        }
+    }
+    return CC_OK;
+}
+
+cc_status cc_release_replica(cc_layer* L, int replica) {
+    if (!L) return fail(CC_ERR_INVALID, "null layer");
+    if (replica < 0 || replica >= CC_MAX_REPLICAS) return fail(CC_ERR_INVALID, "replica index out of range");
+    if (replica == 0) return fail(CC_ERR_STATE, "replica 0 (the layer itself) cannot be released");
+    if (L->rep[replica].state != REP_LIVE) return fail(CC_ERR_STATE, "replica %d is not live", replica);
+    L->rep[replica].state = REP_RETIRING;
+    return CC_OK;
+}
+
+cc_status cc_commit(cc_layer* L, void* stream) {
+    if (!L) return fail(CC_ERR_INVALID, "null layer");
+    cc_ctx* ctx = L->ctx;
+    cudaStream_t st = (cudaStream_t)stream;
+    CC_CUDA(cudaSetDevice(ctx->device));
+    reap_zombies(ctx, false);
+    bool pending = false;
+    for (int r = 1; r < CC_MAX_REPLICAS; ++r) pending |= (L->rep[r].state == REP_COPYING || L->rep[r].state == REP_RETIRING);
+    if (!pending) return CC_OK;
+    std::vector<uint64_t> retired;
+    for (int r = 1; r < CC_MAX_REPLICAS; ++r) {
+        Replica& R = L->rep[r];
+        if (R.state == REP_COPYING) {
+            CC_CUDA(cudaStreamWaitEvent(st, R.copied, 0));    // two-phase publish: visible only once copied
+            R.state = REP_LIVE;
+            R.published = true;
+        } else if (R.state == REP_RETIRING) {
+            CC_CUDA(cudaStreamWaitEvent(st, R.copied, 0));    // a retired copy may still be in flight
+            retired.push_back((uint64_t)(uintptr_t)R.blob);
+            R.state = REP_EMPTY;
+            R.published = false;
+            R.blob = nullptr;
+        }
+    }
+    CcLayerTable row{};
+    for (int r = 0; r < CC_MAX_REPLICAS; ++r) {
+        if (L->rep[r].state == REP_LIVE) {
+            row.rep[r].blob = L->rep[r].blob;
+            row.active_mask |= 1u << r;
+        }
+    }
+    L->host_row = row;
+    CC_CUDA(cc_launch_publish(ctx->table_dev + L->row, row, st));
+    for (uint64_t a : retired) {
+        Zombie z{a, nullptr};
+        CC_CUDA(cudaEventCreateWithFlags(&z.after_flip, cudaEventDisableTiming));
+        CC_CUDA(cudaEventRecord(z.after_flip, st));           // everything enqueued before the flip has run
+        ctx->zombies.push_back(z);
+    }
+    return CC_OK;
+}
+
+cc_status cc_query(cc_layer* L, int* n_active, int* n_pending) {
+    if (!L) return fail(CC_ERR_INVALID, "null layer");
+    int a = 0, p = 0;
+    for (int r = 0; r < CC_MAX_REPLICAS; ++r) {
+        a += (L->host_row.active_mask >> r) & 1u;
+        p += (L->rep[r].state == REP_COPYING);
+    }
+    if (n_active) *n_active = a;
+    if (n_pending) *n_pending = p;
+    return CC_OK;
+}
+
+cc_status cc_replica_blob(cc_layer* L, int replica, const void** blob_dev, size_t* bytes) {
+    if (!L || !blob_dev || !bytes) return fail(CC_ERR_INVALID, "null argument");
+    if (replica < 0 || replica >= CC_MAX_REPLICAS) return fail(CC_ERR_INVALID, "replica index out of range");
+    if (L->rep[replica].state == REP_EMPTY) return fail(CC_ERR_STATE, "replica %d holds no slot", replica);
+    *blob_dev = L->rep[replica].blob;
+    *bytes = L->blob_bytes;
+    return CC_OK;
+}
+
+}  // extern "C"
+
+// ---- the hot path -------------------------------------------------------------------------------
+namespace {
+constexpr int kForwardLaunches = 12;
+
+cudaError_t enqueue_forward(cc_layer* L, __nv_bfloat16* hidden, const CcKv& kv, const int* seq_lens, const int* assign,
+                            int batch, cudaStream_t st) {
+    cc_ctx* ctx = L->ctx;
+    const CcDims& D = L->D;
+    const CcWork& W = L->W;
+    const CcLayerTable* tab = ctx->table_dev + L->row;
+    CcLaunch Ln{st, ctx->n_sms, ctx->pdl};
+    cudaError_t e;
+    // a0 grouping | a1 norm | a2 QKV | a3+a4 RoPE + append | a5 attention (+ combine) | a6 O |
+    // a6+a7 residual + norm | a8 gate/up | a8 SwiGLU | a9 down | a9 residual, original row order
+    if ((e = cc_launch_group(assign, seq_lens, batch, D, tab, W, Ln)) != cudaSuccess) return e;
+    if ((e = cc_launch_rmsnorm_in(hidden, D, tab, W, Ln)) != cudaSuccess) return e;
+    if ((e = cc_launch_gemm(0, D, tab, W, Ln)) != cudaSuccess) return e;
+    if ((e = cc_launch_rope_append(seq_lens, kv, D, W, Ln)) != cudaSuccess) return e;
+    if ((e = cc_launch_attention(seq_lens, kv, D, W, Ln)) != cudaSuccess) return e;
+    if ((e = cc_launch_attn_combine(seq_lens, D, W, Ln)) != cudaSuccess) return e;
+    if ((e = cc_launch_gemm(1, D, tab, W, Ln)) != cudaSuccess) return e;
+    if ((e = cc_launch_resid_norm(hidden, D, tab, W, Ln)) != cudaSuccess) return e;
+    if ((e = cc_launch_gemm(2, D, tab, W, Ln)) != cudaSuccess) return e;
+    if ((e = cc_launch_swiglu(D, W, Ln)) != cudaSuccess) return e;
+    if ((e = cc_launch_gemm(3, D, tab, W, Ln)) != cudaSuccess) return e;
+    return cc_launch_final(hidden, D, W, Ln);
+}
+}  // namespace
+
+extern "C" {
+
+cc_status cc_forward(cc_layer* L, void* hidden_dev, const cc_kv_pages* kv, const int32_t* seq_lens_dev,
+                     const int32_t* replica_assign_dev, int batch, void* stream) {
+    if (!L || !hidden_dev || !kv || !seq_lens_dev || !replica_assign_dev) return fail(CC_ERR_INVALID, "null argument");
+    if (batch < 1 || batch > L->desc.max_batch) return fail(CC_ERR_INVALID, "batch %d outside 1..max_batch=%d", batch, L->desc.max_batch);
+    if (!kv->k_pool || !kv->v_pool || !kv->block_table || kv->n_pages < 1) return fail(CC_ERR_INVALID, "bad cc_kv_pages");
+    if (((uintptr_t)hidden_dev | (uintptr_t)kv->k_pool | (uintptr_t)kv->v_pool) & 15)
+        return fail(CC_ERR_INVALID, "hidden and KV pools must be 16-byte aligned");
+    CcKv k{(__nv_bfloat16*)kv->k_pool, (__nv_bfloat16*)kv->v_pool, kv->block_table, kv->n_pages};
+    cudaError_t e = enqueue_forward(L, (__nv_bfloat16*)hidden_dev, k, seq_lens_dev, replica_assign_dev, batch,
+                                    (cudaStream_t)stream);
+    if (e != cudaSuccess) return fail(CC_ERR_CUDA, "cc_forward launch: %s", cudaGetErrorString(e));
+    L->last_batch = batch;
+    return CC_OK;
+}
+
+cc_status cc_forward_host(cc_layer* L, void* hidden_host, void* k_pool_dev, void* v_pool_dev, int32_t n_pages,
+                          const int32_t* block_table_host, const int32_t* seq_lens_host,
+                          const int32_t* replica_assign_host, int batch, void* stream) {
+    if (!L || !hidden_host || !block_table_host || !seq_lens_host || !replica_assign_host)
+        return fail(CC_ERR_INVALID, "null argument");
+    if (batch < 1 || batch > L->desc.max_batch) return fail(CC_ERR_INVALID, "batch %d outside 1..max_batch=%d", batch, L->desc.max_batch);
+    cudaStream_t st = (cudaStream_t)stream;
+    CC_CUDA(cudaSetDevice(L->ctx->device));
+    const size_t hb = (size_t)batch * L->D.d * 2, bb = (size_t)batch * L->desc.max_blocks_per_seq * 4;
+    CC_CUDA(cudaMemcpyAsync(L->st_hidden, hidden_host, hb, cudaMemcpyHostToDevice, st));
+    CC_CUDA(cudaMemcpyAsync(L->st_bt, block_table_host, bb, cudaMemcpyHostToDevice, st));
+    CC_CUDA(cudaMemcpyAsync(L->st_sl, seq_lens_host, (size_t)batch * 4, cudaMemcpyHostToDevice, st));
+    CC_CUDA(cudaMemcpyAsync(L->st_ra, replica_assign_host, (size_t)batch * 4, cudaMemcpyHostToDevice, st));
+    cc_kv_pages kv{k_pool_dev, v_pool_dev, L->st_bt, n_pages};
+    cc_status s = cc_forward(L, L->st_hidden, &kv, L->st_sl, L->st_ra, batch, stream);
+    if (s != CC_OK) return s;
+    CC_CUDA(cudaMemcpyAsync(hidden_host, L->st_hidden, hb, cudaMemcpyDeviceToHost, st));
+    CC_CUDA(cudaStreamSynchronize(st));
+    return CC_OK;
+}
+
+cc_status cc_forward_launch_count(const cc_layer* L, int* n) {
+    if (!L || !n) return fail(CC_ERR_INVALID, "null argument");
+    *n = kForwardLaunches;
+    return CC_OK;
+}
+
+// ---- stage taps (tests only) ----------------------------------------------------------------------
+cc_status cc_debug_tap(cc_layer* L, cc_tap which, float* out_host, int batch) {
+    if (!L || !out_host) return fail(CC_ERR_INVALID, "null argument");
+    if (batch < 1 || batch > L->desc.max_batch) return fail(CC_ERR_INVALID, "bad batch");
+    const CcDims& D = L->D;
+    const void* src;
+    int kind, dim;
+    switch (which) {
+        case CC_TAP_X: src = L->W.x_act; kind = 0; dim = D.d; break;
+        case CC_TAP_Q: src = L->W.q_rot; kind = 1; dim = D.QD; break;
+        case CC_TAP_O: src = L->W.o_act; kind = 0; dim = D.QD; break;
+        case CC_TAP_H1: src = L->W.h1; kind = 1; dim = D.d; break;
+        case CC_TAP_Y: src = L->W.y_act; kind = 0; dim = D.d; break;
+        case CC_TAP_A: src = L->W.a_act; kind = 0; dim = D.F; break;
+        default: return fail(CC_ERR_INVALID, "unknown tap");
+    }
+    CC_CUDA(cudaSetDevice(L->ctx->device));
+    CC_CUDA(cudaDeviceSynchronize());
+    float* tmp = nullptr;
+    const size_t bytes = (size_t)batch * dim * 4;
+    CC_CUDA(cudaMalloc(&tmp, bytes));
+    cudaError_t e = cudaMemset(tmp, 0, bytes);
+    if (e == cudaSuccess) e = cc_launch_tap(src, kind, dim, D, L->W, tmp, batch, 0);
+    if (e == cudaSuccess) e = cudaMemcpy(out_host, tmp, bytes, cudaMemcpyDeviceToHost);
+    cudaFree(tmp);
+    if (e != cudaSuccess) return fail(CC_ERR_CUDA, "cc_debug_tap: %s", cudaGetErrorString(e));
+    return CC_OK;
+}
+
+cc_status cc_debug_grouping(cc_layer* L, int32_t* perm_host, int32_t* counts_host, int32_t* n_pos) {
+    if (!L || !perm_host || !counts_host || !n_pos) return fail(CC_ERR_INVALID, "null argument");
+    CC_CUDA(cudaSetDevice(L->ctx->device));
+    CC_CUDA(cudaDeviceSynchronize());
+    CcSched s;
+    CC_CUDA(cudaMemcpy(&s, L->W.sched, sizeof s, cudaMemcpyDeviceToHost));
+    CC_CUDA(cudaMemcpy(perm_host, L->W.perm, (size_t)L->D.Mpad * 4, cudaMemcpyDeviceToHost));
+    for (int r = 0; r < CC_MAX_REPLICAS; ++r) counts_host[r] = s.cnt[r];
+    *n_pos = s.n_pos;
+    return CC_OK;
+}
+
+}  // extern "C"

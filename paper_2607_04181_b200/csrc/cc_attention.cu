@@ -1,0 +1,267 @@
+// cc_attention.cu -- paged GQA decode attention, split-KV (the KV cache
+// partitioning the paper relies on: PAPER.md:103, 391, 476).
+//
+// HBM-bound: every cached K/V byte of a request is read exactly once per step.  Work item =
+// (grouped row, kv head, chunk of 256 tokens = 16 pages); the G query heads that share the kv
+// head are the (zero-padded) 16 rows of an mma.sync m16n8k16 tile, so one KV read serves the
+// whole GQA group.  This is a memory kernel with M <= 8 real rows: the legacy warp-level
+// tensor path is ample here (tcgen05 needs M >= 64), the design effort goes into the stream:
+//   * each warp owns 4 of the chunk's 16 pages (w, w+4, w+8, w+12) and a private ring of
+//     cp.async stages (one stage = one K page + one V page = 2 x 16 x Dh bf16), so loads of the
+//     next pages -- and of the next work item -- are in flight while a page is being used;
+//   * pages land in smem XOR-swizzled at 16-byte granularity, so the ldmatrix reads of the
+//     K (B operand of q.K^T) and V (transposed B operand of p.V) fragments are conflict-free;
+//   * softmax is online per warp (running max / sum in log2 units, fp32), the 4 warps of a CTA
+//     are merged in fixed order through smem, chunks are merged in fixed order by
+//     k_attn_combine.  The chunking depends on seq_len only => bit-identical across replicas.
+#include "cc_kernels.h"
+
+namespace {
+
+constexpr int kAttnWarps = 4;
+constexpr int kAttnThreads = kAttnWarps * 32;
+constexpr int kAttnStages = 3;
+constexpr int kPagesPerChunk = CC_ATTN_CHUNK / CC_PAGE;       // 16
+constexpr int kSlotsPerItem = kPagesPerChunk / kAttnWarps;    // 4 page slots per warp per item
+
+template <int DH>
+struct AttnCfg {
+    static constexpr int kRowBytes = DH * 2;
+    static constexpr int kPageBytes = CC_PAGE * kRowBytes;     // one K (or V) page of one kv head
+    static constexpr int kStageBytes = 2 * kPageBytes;
+    static constexpr int kChunksPerRow = DH / 8;               // 16-byte chunks per token row
+    static constexpr int kMergeStride = DH + 2;                // floats per (warp, head): o[DH], m, l
+    static size_t smem_bytes(int G) {
+        return (size_t)kAttnWarps * kAttnStages * kStageBytes + (size_t)kAttnWarps * G * kMergeStride * 4;
+    }
+};
+
+struct ItemMeta {
+    int pos, chunk, b, s;     // s <= 0 marks "no item"
+};
+
+template <int DH>
+__global__ void __launch_bounds__(kAttnThreads, 2)
+k_attn(const int* __restrict__ seq_lens, CcKv kv, CcDims D, CcWork W) {
+    using C = AttnCfg<DH>;
+    extern __shared__ __align__(1024) uint8_t smem_raw[];
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int g = lane >> 2, t4 = lane & 3;
+    uint8_t* ring = smem_raw + (size_t)warp * kAttnStages * C::kStageBytes;
+    float* merge = reinterpret_cast<float*>(smem_raw + (size_t)kAttnWarps * kAttnStages * C::kStageBytes);
+    const uint32_t ring_u32 = smem_u32(ring);
+
+    pdl_launch_dependents();
+    pdl_wait();
+
+    const int G = D.G, Hkv = D.Hkv;
+    const int n_items = W.sched->n_items * Hkv;
+    const int my_items = ((int)blockIdx.x < n_items) ? (n_items - 1 - (int)blockIdx.x) / (int)gridDim.x + 1 : 0;
+    const int n_slots = my_items * kSlotsPerItem;
+
+    // ---- producer side: issue the cp.async copies of page slot k of this warp -------------------
+    ItemMeta pm = {0, 0, 0, 0};
+    int p_hk = 0, p_item = -1, p_page_id = 0;      // p_page_id: lane l < 16 holds page id l of the chunk
+    auto prefetch = [&](int k) {
+        const int it = k / kSlotsPerItem, i = k % kSlotsPerItem;
+        if (it != p_item) {
+            p_item = it;
+            const int j = (int)blockIdx.x + it * (int)gridDim.x;
+            const int base = j / Hkv;
+            p_hk = j - base * Hkv;
+            const int2 rec = W.items[base];
+            pm.pos = rec.x;
+            pm.chunk = rec.y;
+            pm.b = W.perm[rec.x];
+            pm.s = seq_lens[pm.b];
+            const int n_row_pages = (pm.s + CC_PAGE - 1) / CC_PAGE;
+            const int pg = pm.chunk * kPagesPerChunk + (lane & 15);
+            int id = 0;
+            if (pg < n_row_pages) {
+                id = kv.block_table[(size_t)pm.b * D.max_blocks + pg];
+                if (id < 0 || id >= kv.n_pages) {
+                    atomicOr(W.err, CC_DEVERR_BAD_PAGE);
+                    id = 0;
+                }
+            }
+            p_page_id = id;
+        }
+        const int pl = warp + i * kAttnWarps;                       // page within the chunk
+        const int tok0 = pm.chunk * CC_ATTN_CHUNK + pl * CC_PAGE;   // first token of the page
+        const int page = __shfl_sync(0xffffffffu, p_page_id, pl);
+        if (tok0 < pm.s) {
+            const int valid = min(CC_PAGE, pm.s - tok0);
+            const size_t src_off = ((size_t)page * Hkv + p_hk) * (size_t)(CC_PAGE * DH);
+            const __nv_bfloat16* ksrc = kv.k_pool + src_off;
+            const __nv_bfloat16* vsrc = kv.v_pool + src_off;
+            const uint32_t dstK = ring_u32 + (uint32_t)(k % kAttnStages) * C::kStageBytes;
+            const uint32_t dstV = dstK + C::kPageBytes;
+#pragma unroll
+            for (int q = lane; q < CC_PAGE * C::kChunksPerRow; q += 32) {
+                const int tok = q / C::kChunksPerRow, ch = q % C::kChunksPerRow;
+                const uint32_t off = (uint32_t)tok * C::kRowBytes + (uint32_t)((ch ^ (tok & 7)) << 4);
+                const uint32_t sz = tok < valid ? 16u : 0u;        // rows past seq_len are zero-filled
+                asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;" ::"r"(dstK + off),
+                             "l"(ksrc + tok * DH + ch * 8), "r"(sz)
+                             : "memory");
+                asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;" ::"r"(dstV + off),
+                             "l"(vsrc + tok * DH + ch * 8), "r"(sz)
+                             : "memory");
+            }
+        }
+    };
+
+    for (int k = 0; k < kAttnStages - 1; ++k) {
+        if (k < n_slots) prefetch(k);
+        cp_async_commit();
+    }
+
+    // ---- consumer state ----------------------------------------------------------------------
+    ItemMeta cm = {0, 0, 0, 0};
+    int c_hk = 0;
+    uint32_t qa0[DH / 16], qa2[DH / 16];   // Q fragments (rows g < G), scaled by log2(e)/sqrt(Dh)
+    float o[DH / 8][4];
+    float m_run = -INFINITY, l_run = 0.f;
+
+    for (int k = 0; k < n_slots; ++k) {
+        const int it = k / kSlotsPerItem, i = k % kSlotsPerItem;
+        if (k + kAttnStages - 1 < n_slots) prefetch(k + kAttnStages - 1);
+        cp_async_commit();
+
+        if (i == 0) {   // new item: metadata, Q fragments, reset the running softmax state
+            const int j = (int)blockIdx.x + it * (int)gridDim.x;
+            const int base = j / Hkv;
+            c_hk = j - base * Hkv;
+            const int2 rec = W.items[base];
+            cm.pos = rec.x;
+            cm.chunk = rec.y;
+            cm.b = W.perm[rec.x];
+            cm.s = seq_lens[cm.b];
+            const float* qrow = W.q_rot + (size_t)cm.pos * D.QD + (size_t)(c_hk * G + g) * DH;
+#pragma unroll
+            for (int ks = 0; ks < DH / 16; ++ks) {
+                float2 x0 = make_float2(0.f, 0.f), x1 = make_float2(0.f, 0.f);
+                if (g < G) {
+                    x0 = *reinterpret_cast<const float2*>(qrow + ks * 16 + 2 * t4);
+                    x1 = *reinterpret_cast<const float2*>(qrow + ks * 16 + 8 + 2 * t4);
+                }
+                qa0[ks] = pack_bf16(x0.x * D.qk_scale_log2, x0.y * D.qk_scale_log2);
+                qa2[ks] = pack_bf16(x1.x * D.qk_scale_log2, x1.y * D.qk_scale_log2);
+            }
+#pragma unroll
+            for (int nt = 0; nt < DH / 8; ++nt) o[nt][0] = o[nt][1] = o[nt][2] = o[nt][3] = 0.f;
+            m_run = -INFINITY;
+            l_run = 0.f;
+        }
+
+        cp_async_wait<kAttnStages - 1>();
+        __syncwarp();
+
+        const int pl = warp + i * kAttnWarps;
+        const int tok0 = cm.chunk * CC_ATTN_CHUNK + pl * CC_PAGE;
+        if (tok0 < cm.s) {
+            const int valid = min(CC_PAGE, cm.s - tok0);
+            const uint32_t sK = ring_u32 + (uint32_t)(k % kAttnStages) * C::kStageBytes;
+            const uint32_t sV = sK + C::kPageBytes;
+            // ---- scores: S[16 x 16] = Q[16 x DH] . K^T
+            float s0[4] = {0.f, 0.f, 0.f, 0.f}, s1[4] = {0.f, 0.f, 0.f, 0.f};
+            {
+                const int mi = lane >> 3, rr = lane & 7;
+                const int tok = ((mi >> 1) << 3) + rr;
+                const uint32_t rowaddr = sK + (uint32_t)tok * C::kRowBytes;
+#pragma unroll
+                for (int ks = 0; ks < DH / 16; ++ks) {
+                    const int ch = ks * 2 + (mi & 1);
+                    uint32_t r0, r1, r2, r3;
+                    ldsm_x4(rowaddr + (uint32_t)((ch ^ (tok & 7)) << 4), r0, r1, r2, r3);
+                    mma_bf16_16816(s0, qa0[ks], 0u, qa2[ks], 0u, r0, r1);
+                    mma_bf16_16816(s1, qa0[ks], 0u, qa2[ks], 0u, r2, r3);
+                }
+            }
+            // ---- online softmax on row g (tokens 2t,2t+1 and 8+2t,8+2t+1 of the page)
+            const int c0 = 2 * t4;
+            float v00 = (c0 < valid) ? s0[0] : -INFINITY, v01 = (c0 + 1 < valid) ? s0[1] : -INFINITY;
+            float v10 = (c0 + 8 < valid) ? s1[0] : -INFINITY, v11 = (c0 + 9 < valid) ? s1[1] : -INFINITY;
+            float pmax = fmaxf(fmaxf(v00, v01), fmaxf(v10, v11));
+            pmax = fmaxf(pmax, __shfl_xor_sync(0xffffffffu, pmax, 1));
+            pmax = fmaxf(pmax, __shfl_xor_sync(0xffffffffu, pmax, 2));
+            const float m_new = fmaxf(m_run, pmax);        // finite: token 0 of the page is valid
+            const float alpha = exp2f(m_run - m_new);
+            const float p00 = exp2f(v00 - m_new), p01 = exp2f(v01 - m_new);
+            const float p10 = exp2f(v10 - m_new), p11 = exp2f(v11 - m_new);
+            l_run = l_run * alpha + ((p00 + p01) + (p10 + p11));
+            m_run = m_new;
+            const uint32_t pa0 = pack_bf16(p00, p01), pa2 = pack_bf16(p10, p11);
+            // ---- O[16 x DH] = alpha * O + P[16 x 16] . V[16 x DH]
+            {
+                const int mi = lane >> 3, rr = lane & 7;
+                const int tok = ((mi & 1) << 3) + rr;
+                const uint32_t rowaddr = sV + (uint32_t)tok * C::kRowBytes;
+#pragma unroll
+                for (int jn = 0; jn < DH / 16; ++jn) {
+                    const int ch = jn * 2 + (mi >> 1);
+                    uint32_t r0, r1, r2, r3;
+                    ldsm_x4_trans(rowaddr + (uint32_t)((ch ^ (tok & 7)) << 4), r0, r1, r2, r3);
+                    o[2 * jn][0] *= alpha; o[2 * jn][1] *= alpha;
+                    o[2 * jn + 1][0] *= alpha; o[2 * jn + 1][1] *= alpha;
+                    mma_bf16_16816(o[2 * jn], pa0, 0u, pa2, 0u, r0, r1);
+                    mma_bf16_16816(o[2 * jn + 1], pa0, 0u, pa2, 0u, r2, r3);
+                }
+            }
+        }
+        __syncwarp();   // all lanes are done with this stage before a later prefetch overwrites it
+
+        if (i == kSlotsPerItem - 1) {
+            // ---- merge the 4 warps of the CTA in fixed order, write the chunk partial
+            float l_tot = l_run;
+            l_tot += __shfl_xor_sync(0xffffffffu, l_tot, 1);
+            l_tot += __shfl_xor_sync(0xffffffffu, l_tot, 2);
+            if (g < G) {
+                float* mrow = merge + (size_t)(warp * G + g) * C::kMergeStride;
+#pragma unroll
+                for (int nt = 0; nt < DH / 8; ++nt)
+                    *reinterpret_cast<float2*>(mrow + nt * 8 + 2 * t4) = make_float2(o[nt][0], o[nt][1]);
+                if (t4 == 0) {
+                    mrow[DH] = m_run;
+                    mrow[DH + 1] = l_tot;
+                }
+            }
+            __syncthreads();
+            for (int e = threadIdx.x; e < G * DH; e += kAttnThreads) {
+                const int hg = e / DH, dim = e - hg * DH;
+                float M = -INFINITY;
+#pragma unroll
+                for (int w = 0; w < kAttnWarps; ++w) M = fmaxf(M, merge[(size_t)(w * G + hg) * C::kMergeStride + DH]);
+                float acc = 0.f, L = 0.f;
+#pragma unroll
+                for (int w = 0; w < kAttnWarps; ++w) {
+                    const float* mr = merge + (size_t)(w * G + hg) * C::kMergeStride;
+                    const float sc = exp2f(mr[DH] - M);
+                    acc += sc * mr[dim];
+                    L += sc * mr[DH + 1];
+                }
+                const size_t row = ((size_t)cm.pos * D.Hq + (size_t)(c_hk * G + hg)) * W.nch_max + cm.chunk;
+                W.att_o[row * DH + dim] = acc;
+                if (dim == 0) W.att_ml[row] = make_float2(M, L);
+            }
+            __syncthreads();   // merge buffer is reused by the next item
+        }
+    }
+    cp_async_wait<0>();
+}
+
+}  // namespace
+
+cudaError_t cc_attn_configure() {
+    cudaError_t e = cudaFuncSetAttribute(k_attn<128>, cudaFuncAttributeMaxDynamicSharedMemorySize, 112 * 1024);
+    if (e != cudaSuccess) return e;
+    return cudaFuncSetAttribute(k_attn<64>, cudaFuncAttributeMaxDynamicSharedMemorySize, 112 * 1024);
+}
+
+cudaError_t cc_launch_attention(const int* seq_lens, const CcKv& kv, const CcDims& D, const CcWork& W,
+                                const CcLaunch& L) {
+    const dim3 grid(2 * L.n_sms), block(kAttnThreads);
+    if (D.Dh == 128)
+        return cc_launch_kernel(k_attn<128>, grid, block, AttnCfg<128>::smem_bytes(D.G), L, seq_lens, kv, D, W);
+    return cc_launch_kernel(k_attn<64>, grid, block, AttnCfg<64>::smem_bytes(D.G), L, seq_lens, kv, D, W);
+}

@@ -1,0 +1,250 @@
+// cc_common.cuh -- device-side structures and sm_100a PTX wrappers shared by the kernels of
+// libcocoscale.  (Product code; shares nothing with oracle/.)
+#pragma once
+#include <cuda_runtime.h>
+#include <cuda_bf16.h>
+#include <stdint.h>
+
+#define CC_MAXR 4              // CC_MAX_REPLICAS
+#define CC_PAGE 16             // tokens per KV page
+#define CC_TILE_N 128          // weight rows per GEMM tile (UMMA M)
+#define CC_TILE_K 64           // K elements per pipeline stage (one 128B-swizzle atom of bf16)
+#define CC_A_TILE_BYTES (CC_TILE_N * CC_TILE_K * 2)   // 16 KiB packed weight tile
+#define CC_ROW_ALIGN 16        // group offsets are multiples of this (UMMA N granularity)
+#define CC_ATTN_CHUNK 256      // tokens per split-KV work item (a function of nothing but this)
+
+#define CC_DEVERR_BAD_REPLICA 1u
+#define CC_DEVERR_BAD_PAGE 2u
+#define CC_DEVERR_BAD_SEQLEN 4u
+#define CC_DEVERR_HANG 8u         // an mbarrier wait gave up (kernel bug); the kernel trapped
+
+// ---- device replica table -----------------------------------------
+// One row per layer, at a fixed device address for the life of the context.  Kernels read the
+// weight-blob base of replica r from here at run time, so a captured graph survives flips.
+struct CcReplicaRow {
+    const uint8_t* blob;   // packed weight blob of replica r (slot base), or nullptr
+};
+struct CcLayerTable {
+    CcReplicaRow rep[CC_MAXR];
+    uint32_t active_mask;  // bit r set <=> replica r may be named by replica_assign
+    uint32_t pad_[3];
+};
+
+// Geometry of one weight-streaming GEMM (swap-AB: the packed weight tile is the UMMA A operand,
+// M = 128 output features; the activations are the B operand, N = rows of one replica group).
+// The (tile, k-block) "atoms" of 16 KiB are numbered tile-major and cut into P contiguous
+// ranges, range i owned by CTA i.  P and the cut points depend on the layer shape and the SM
+// count only -- never on the batch split -- so every output element is summed in one fixed
+// order whatever the replica count (PAPER.md:385 bit-wise consistency).
+struct CcGemmGeo {
+    int T;        // tiles of 128 output features
+    int KB;       // k-blocks of 64 per tile
+    int P;        // CTAs (ranges)
+    int pad_;
+    size_t w_off; // byte offset of the packed matrix inside a replica blob
+};
+// Range of CTA i: atoms [cc_range_begin(i), cc_range_begin(i+1)).
+__host__ __device__ __forceinline__ long long cc_range_begin(const CcGemmGeo& g, int i) {
+    return (long long)i * g.T * g.KB / g.P;
+}
+// CTA whose range holds atom a (inverse of cc_range_begin).
+__host__ __device__ __forceinline__ int cc_range_of_atom(const CcGemmGeo& g, long long a) {
+    return (int)(((a + 1) * g.P - 1) / ((long long)g.T * g.KB));
+}
+// A "piece" is the part of one tile that one CTA accumulated; piece id = CTA + tile (unique and
+// increasing along the atom axis).  Partial sums live at part[piece][pos][128] fp32.
+__host__ __device__ __forceinline__ void cc_tile_pieces(const CcGemmGeo& g, int t, int& first, int& last) {
+    first = cc_range_of_atom(g, (long long)t * g.KB) + t;
+    last = cc_range_of_atom(g, (long long)(t + 1) * g.KB - 1) + t;
+}
+
+// Static per-layer geometry, passed to kernels by value.
+struct CcDims {
+    int d, Hq, Hkv, Dh, G, F;
+    int QD, KD;                 // Hq*Dh, Hkv*Dh
+    int Mpad;                   // rows of every grouped workspace buffer (multiple of 16)
+    int max_batch, max_blocks, max_position;
+    float eps;
+    float qk_scale_log2;        // log2(e) / sqrt(Dh)
+    CcGemmGeo qkv, o, gu, dn;   // the four projections
+    size_t off_g1, off_g2;      // gains inside the blob (bf16 [d])
+};
+
+// Per-forward schedule, rebuilt on the device by k_group every step (row a0).
+struct CcSched {
+    int cnt[CC_MAXR];      // rows in replica group r
+    int goff[CC_MAXR];     // first grouped position of group r (multiple of 16)
+    int n_pos;             // grouped positions in use (end of the last group, multiple of 16)
+    int n_items;           // attention work items (pos, chunk); x Hkv inside the kernel
+    int nmax;              // largest padded group size (UMMA N of the widest group)
+    int pad_[5];
+};
+
+// ---- small helpers -----------------------------------------------------------------------
+__device__ __forceinline__ float bf16lo(uint32_t w) { return __uint_as_float(w << 16); }
+__device__ __forceinline__ float bf16hi(uint32_t w) { return __uint_as_float(w & 0xffff0000u); }
+__device__ __forceinline__ uint32_t pack_bf16(float lo, float hi) {
+    __nv_bfloat162 v = __floats2bfloat162_rn(lo, hi);   // .x = lo (low 16 bits)
+    return *reinterpret_cast<uint32_t*>(&v);
+}
+__device__ __forceinline__ uint32_t smem_u32(const void* p) {
+    return static_cast<uint32_t>(__cvta_generic_to_shared(p));
+}
+// Byte offset of element (row, k) inside a packed activation buffer [K/64][Mpad][64] whose
+// 128-byte rows are stored in the 128B-swizzle pattern (16-byte chunk c of row r at c ^ (r & 7)).
+__device__ __forceinline__ size_t act_chunk_off(int row, int k, int Mpad) {
+    int kb = k >> 6, c = (k >> 3) & 7;
+    return ((size_t)kb * Mpad + row) * 128 + (size_t)((c ^ (row & 7)) << 4);
+}
+
+// ---- mbarrier / bulk-copy / TMA ----------------------------------------------------------
+__device__ __forceinline__ void mbar_init(uint64_t* bar, uint32_t count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count));
+}
+__device__ __forceinline__ void fence_mbar_init() {
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+}
+__device__ __forceinline__ void fence_proxy_async_smem() {
+    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(uint64_t* bar, uint32_t bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes)
+                 : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(uint64_t* bar) {
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ bool mbar_try_wait(uint64_t* bar, uint32_t parity) {
+    uint32_t ok;
+    asm volatile(
+        "{\n\t.reg .pred p;\n\t"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
+        "selp.u32 %0, 1, 0, p;\n\t}"
+        : "=r"(ok)
+        : "r"(smem_u32(bar)), "r"(parity)
+        : "memory");
+    return ok != 0;
+}
+// Bounded wait: try_wait suspends in hardware for a while per call, so this limit is seconds of
+// real time; a kernel bug then traps (CUDA error at the next sync) instead of hanging the GPU.
+__device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
+    uint32_t spins = 0;
+    while (!mbar_try_wait(bar, parity)) {
+        if (++spins > (1u << 26)) __trap();
+    }
+}
+// Programmatic dependent launch: wait for the preceding kernel's memory / let the next one start.
+__device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+__device__ __forceinline__ void pdl_launch_dependents() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+// cp.async (LDGSTS) 16 bytes, L2 only.
+__device__ __forceinline__ void cp_async16(uint32_t dst_smem, const void* src) {
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(dst_smem), "l"(src) : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+template <int N>
+__device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
+// 1-D bulk copy global -> shared (TMA engine, no descriptor); completes `bytes` on the mbarrier.
+__device__ __forceinline__ void bulk_g2s(void* dst_smem, const void* src_gmem, uint32_t bytes, uint64_t* bar) {
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(
+                     smem_u32(dst_smem)),
+                 "l"(src_gmem), "r"(bytes), "r"(smem_u32(bar))
+                 : "memory");
+}
+__device__ __forceinline__ void bulk_g2s_hint(void* dst_smem, const void* src_gmem, uint32_t bytes, uint64_t* bar,
+                                              uint64_t policy) {
+    asm volatile(
+        "cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes.L2::cache_hint [%0], [%1], %2, [%3], %4;" ::
+            "r"(smem_u32(dst_smem)),
+        "l"(src_gmem), "r"(bytes), "r"(smem_u32(bar)), "l"(policy)
+        : "memory");
+}
+__device__ __forceinline__ uint64_t policy_evict_first() {
+    uint64_t p;
+    asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(p));
+    return p;
+}
+__device__ __forceinline__ uint64_t policy_evict_last() {
+    uint64_t p;
+    asm volatile("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;" : "=l"(p));
+    return p;
+}
+// ---- tcgen05 / TMEM --------------------------------------------------------------------------
+template <int kCols>
+__device__ __forceinline__ void tmem_alloc(uint32_t* dst_smem) {   // one full warp
+    asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(dst_smem)),
+                 "n"(kCols)
+                 : "memory");
+    asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+}
+template <int kCols>
+__device__ __forceinline__ void tmem_dealloc(uint32_t taddr) {     // the same warp
+    asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(taddr), "n"(kCols) : "memory");
+}
+__device__ __forceinline__ void tc_fence_before() { asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory"); }
+__device__ __forceinline__ void tc_fence_after() { asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory"); }
+// D[tmem] (+)= A[smem desc] * B[smem desc]; bf16 x bf16 -> fp32; issued by ONE thread.
+__device__ __forceinline__ void umma_bf16(uint32_t d_tmem, uint64_t a_desc, uint64_t b_desc, uint32_t idesc,
+                                          uint32_t accumulate) {
+    asm volatile(
+        "{\n\t.reg .pred p;\n\t"
+        "setp.ne.b32 p, %4, 0;\n\t"
+        "tcgen05.mma.cta_group::1.kind::f16 [%0], %1, %2, %3, p;\n\t}" ::"r"(d_tmem),
+        "l"(a_desc), "l"(b_desc), "r"(idesc), "r"(accumulate)
+        : "memory");
+}
+// mbarrier arrive once all previously issued tcgen05.mma of this thread have completed.
+__device__ __forceinline__ void umma_commit(uint64_t* bar) {
+    asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(smem_u32(bar))
+                 : "memory");
+}
+// TMEM -> registers: this warp's 32 lanes x 16 consecutive fp32 columns.
+__device__ __forceinline__ void tmem_ld_32x32b_x16(uint32_t taddr, uint32_t (&r)[16]) {
+    asm volatile(
+        "tcgen05.ld.sync.aligned.32x32b.x16.b32 "
+        "{%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15}, [%16];"
+        : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7]), "=r"(r[8]),
+          "=r"(r[9]), "=r"(r[10]), "=r"(r[11]), "=r"(r[12]), "=r"(r[13]), "=r"(r[14]), "=r"(r[15])
+        : "r"(taddr)
+        : "memory");
+}
+__device__ __forceinline__ void tmem_ld_wait() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
+
+// Shared-memory matrix descriptor: K-major operand, 128B swizzle, rows of 128 bytes, 8-row
+// groups 1024 bytes apart (SBO), descriptor version 1 (sm_100).  Tile base must be 1024-aligned;
+// advancing K by 16 bf16 inside the swizzle atom adds 32 bytes to the start address.
+__device__ __forceinline__ uint64_t umma_desc_sw128(uint32_t smem_addr) {
+    uint64_t d = 0;
+    d |= (uint64_t)((smem_addr & 0x3FFFFu) >> 4);   // start address  [0,14)
+    d |= (uint64_t)1 << 16;                          // LBO (unused for swizzled K-major) [16,30)
+    d |= (uint64_t)(1024 >> 4) << 32;                // SBO = 1024 B   [32,46)
+    d |= (uint64_t)1 << 46;                          // version = 1    [46,48)
+    d |= (uint64_t)2 << 61;                          // SWIZZLE_128B   [61,64)
+    return d;
+}
+// Instruction descriptor, kind::f16: D = fp32, A = B = bf16, both K-major, M = 128, N = n.
+__device__ __forceinline__ uint32_t umma_idesc_bf16_m128(uint32_t n) {
+    return (1u << 4) | (1u << 7) | (1u << 10) | ((n >> 3) << 17) | ((128u >> 4) << 24);
+}
+
+// ---- legacy tensor path used by decode attention (HBM-bound, tiny M): mma.sync + ldmatrix ----
+__device__ __forceinline__ void ldsm_x4(uint32_t addr, uint32_t& r0, uint32_t& r1, uint32_t& r2, uint32_t& r3) {
+    asm volatile("ldmatrix.sync.aligned.m8n8.x4.shared.b16 {%0,%1,%2,%3}, [%4];"
+                 : "=r"(r0), "=r"(r1), "=r"(r2), "=r"(r3)
+                 : "r"(addr));
+}
+__device__ __forceinline__ void ldsm_x4_trans(uint32_t addr, uint32_t& r0, uint32_t& r1, uint32_t& r2, uint32_t& r3) {
+    asm volatile("ldmatrix.sync.aligned.m8n8.x4.trans.shared.b16 {%0,%1,%2,%3}, [%4];"
+                 : "=r"(r0), "=r"(r1), "=r"(r2), "=r"(r3)
+                 : "r"(addr));
+}
+// D(16x8, fp32) += A(16x16, bf16, row) * B(16x8, bf16, col)
+__device__ __forceinline__ void mma_bf16_16816(float (&c)[4], uint32_t a0, uint32_t a1, uint32_t a2, uint32_t a3,
+                                               uint32_t b0, uint32_t b1) {
+    asm volatile(
+        "mma.sync.aligned.m16n8k16.row.col.f32.bf16.bf16.f32 {%0,%1,%2,%3}, {%4,%5,%6,%7}, {%8,%9}, {%0,%1,%2,%3};"
+        : "+f"(c[0]), "+f"(c[1]), "+f"(c[2]), "+f"(c[3])
+        : "r"(a0), "r"(a1), "r"(a2), "r"(a3), "r"(b0), "r"(b1));
+}
+__device__ __forceinline__ void named_bar_sync(int id, int nthreads) {
+    asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(nthreads) : "memory");
+}

@@ -1,0 +1,201 @@
+// cc_gemm.cu -- the weight-streaming projection GEMM of the replicated decoder layer (sm_100a).
+//
+// SURVEY.md 8(a) rows a2 (QKV), a6 (O), a8 (gate/up), a9 (down); replica indirection row a10.
+// Decode is HBM-bound: every weight byte is read once per replica group, so the kernel is built
+// around the weight stream, not around the MMA:
+//   * swap-AB: the packed weight tile (128 output features x 64 k, a 16 KiB pre-swizzled image
+//     made once at cc_create_layer) is the tcgen05 A operand (M = 128); the activations of one
+//     replica group (n rows, n = multiple of 16, <= 256) are the B operand (N = n).  The fp32
+//     accumulator D[128][n] lives in TMEM (n columns), double-buffered.
+//   * one persistent CTA per SM, stream-K: the (tile, k-block) atoms are cut into P contiguous
+//     ranges fixed by the layer shape (cc_common.cuh); CTA i streams range i of EVERY active
+//     replica's blob, whose base it reads from the device replica table at run time
+//     (PAPER.md:391-393 re-captures a graph when the replica set changes; here nothing does).
+//   * warp 0 = producer: 1-D bulk copies (TMA engine, no tensor map) of 16 KiB weight atoms and
+//     of the matching activation slab into a ring of smem stages guarded by mbarriers;
+//     warp 1 = MMA issuer (one elected thread, 4 x tcgen05.mma K=16 per atom, tcgen05.commit
+//     frees the stage); warps 2..5 = epilogue (tcgen05.ld -> fp32 partials in global memory).
+//   * a tile's partial sums ("pieces") are added up in fixed order by the next kernel of the
+//     chain, which also applies the fused epilogue (RoPE, residual + RMSNorm, SwiGLU, ...).
+#include "cc_kernels.h"
+
+namespace {
+
+constexpr int kGemmThreads = 192;
+constexpr int kMaxStages = 12;
+constexpr int kGemmSmem = 200 * 1024;     // dynamic shared memory per CTA
+constexpr int kTmemCols = 512;            // two accumulators of up to 256 columns
+
+struct GemmSmemHdr {                      // lives at the start of dynamic smem
+    uint64_t full[kMaxStages];
+    uint64_t empty[kMaxStages];
+    uint64_t tmem_full[2];
+    uint64_t tmem_empty[2];
+    uint32_t tmem_base;
+    int cnt[CC_MAXR];
+    int goff[CC_MAXR];
+    const uint8_t* blob[CC_MAXR];
+};
+
+__global__ void __launch_bounds__(kGemmThreads, 1)
+k_gemm(CcGemmGeo G, const uint8_t* __restrict__ act, float* __restrict__ part, int Mpad,
+       const CcLayerTable* __restrict__ tab, const CcSched* __restrict__ sched) {
+    extern __shared__ __align__(1024) uint8_t smem_raw[];
+    GemmSmemHdr* H = reinterpret_cast<GemmSmemHdr*>(smem_raw);
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+
+    // ---- one-time setup (independent of the previous kernel: overlaps its tail under PDL) ----
+    if (threadIdx.x == 0) {
+        for (int i = 0; i < kMaxStages; ++i) {
+            mbar_init(&H->full[i], 1);
+            mbar_init(&H->empty[i], 1);
+        }
+        for (int i = 0; i < 2; ++i) {
+            mbar_init(&H->tmem_full[i], 1);
+            mbar_init(&H->tmem_empty[i], 4);
+        }
+        fence_mbar_init();
+    }
+    if (warp == 1) tmem_alloc<kTmemCols>(&H->tmem_base);
+    pdl_launch_dependents();
+    pdl_wait();
+    if (threadIdx.x < CC_MAXR) {
+        H->cnt[threadIdx.x] = sched->cnt[threadIdx.x];
+        H->goff[threadIdx.x] = sched->goff[threadIdx.x];
+        H->blob[threadIdx.x] = tab->rep[threadIdx.x].blob;
+    }
+    tc_fence_before();
+    __syncthreads();
+    tc_fence_after();
+
+    const int nmax = sched->nmax;
+    const uint32_t act_bytes_max = (uint32_t)((nmax * 128 + 1023) & ~1023);
+    const uint32_t stage_bytes = CC_A_TILE_BYTES + act_bytes_max;
+    uint8_t* stage0 = smem_raw + 1024;                      // header occupies the first KiB
+    int n_stages = (kGemmSmem - 1024) / (int)stage_bytes;
+    if (n_stages > kMaxStages) n_stages = kMaxStages;
+
+    const long long a_begin = cc_range_begin(G, blockIdx.x), a_end = cc_range_begin(G, blockIdx.x + 1);
+    const uint32_t tmem_base = H->tmem_base;
+
+    if (nmax > 0 && a_begin < a_end) {
+        if (warp == 0) {
+            // ===================== producer =====================
+            if (lane == 0) {
+                const uint64_t pol_w = policy_evict_first();
+                int stage = 0;
+                uint32_t ph = 0;
+                for (int r = 0; r < CC_MAXR; ++r) {
+                    const int cnt = H->cnt[r];
+                    if (cnt == 0) continue;
+                    const uint32_t n = (uint32_t)((cnt + 15) & ~15);
+                    const uint8_t* wsrc = H->blob[r] + G.w_off;
+                    const int goff = H->goff[r];
+                    for (long long a = a_begin; a < a_end; ++a) {
+                        const int kb = (int)(a % G.KB);
+                        mbar_wait(&H->empty[stage], ph ^ 1);
+                        uint8_t* sW = stage0 + (size_t)stage * stage_bytes;
+                        mbar_expect_tx(&H->full[stage], CC_A_TILE_BYTES + n * 128);
+                        bulk_g2s_hint(sW, wsrc + (size_t)a * CC_A_TILE_BYTES, CC_A_TILE_BYTES, &H->full[stage], pol_w);
+                        bulk_g2s(sW + CC_A_TILE_BYTES, act + ((size_t)kb * Mpad + goff) * 128, n * 128, &H->full[stage]);
+                        if (++stage == n_stages) { stage = 0; ph ^= 1; }
+                    }
+                }
+            }
+        } else if (warp == 1) {
+            // ===================== MMA issuer =====================
+            if (lane == 0) {
+                int stage = 0;
+                uint32_t ph = 0;
+                uint32_t pc = 0;   // pieces started so far
+                for (int r = 0; r < CC_MAXR; ++r) {
+                    const int cnt = H->cnt[r];
+                    if (cnt == 0) continue;
+                    const uint32_t n = (uint32_t)((cnt + 15) & ~15);
+                    const uint32_t idesc = umma_idesc_bf16_m128(n);
+                    for (long long a = a_begin; a < a_end; ++a) {
+                        const int kb = (int)(a % G.KB);
+                        const bool first = (a == a_begin) || kb == 0;
+                        const bool last = (a == a_end - 1) || kb == G.KB - 1;
+                        const uint32_t buf = pc & 1;
+                        if (first) {
+                            mbar_wait(&H->tmem_empty[buf], ((pc >> 1) & 1) ^ 1);
+                            tc_fence_after();
+                        }
+                        mbar_wait(&H->full[stage], ph);
+                        tc_fence_after();
+                        const uint32_t sW = smem_u32(stage0 + (size_t)stage * stage_bytes);
+                        const uint64_t da = umma_desc_sw128(sW), db = umma_desc_sw128(sW + CC_A_TILE_BYTES);
+                        const uint32_t d_tmem = tmem_base + buf * 256;
+#pragma unroll
+                        for (int k = 0; k < CC_TILE_K / 16; ++k)
+                            umma_bf16(d_tmem, da + 2 * k, db + 2 * k, idesc, (first && k == 0) ? 0u : 1u);
+                        umma_commit(&H->empty[stage]);
+                        if (last) {
+                            umma_commit(&H->tmem_full[buf]);
+                            ++pc;
+                        }
+                        if (++stage == n_stages) { stage = 0; ph ^= 1; }
+                    }
+                }
+            }
+        } else {
+            // ===================== epilogue: TMEM -> fp32 partial pieces =====================
+            const int q = warp & 3;                          // TMEM lane quarter this warp may read
+            const int f = q * 32 + lane;                     // output feature within the tile
+            uint32_t pc = 0;
+            for (int r = 0; r < CC_MAXR; ++r) {
+                const int cnt = H->cnt[r];
+                if (cnt == 0) continue;
+                const int n = (cnt + 15) & ~15;
+                const int goff = H->goff[r];
+                long long a = a_begin;
+                while (a < a_end) {
+                    const int t = (int)(a / G.KB);
+                    long long a_next = (long long)(t + 1) * G.KB;
+                    if (a_next > a_end) a_next = a_end;
+                    const uint32_t buf = pc & 1;
+                    mbar_wait(&H->tmem_full[buf], (pc >> 1) & 1);
+                    tc_fence_after();
+                    float* dst = part + ((size_t)(blockIdx.x + t) * Mpad + goff) * 128 + f;
+                    for (int c = 0; c < n; c += 16) {
+                        uint32_t v[16];
+                        tmem_ld_32x32b_x16(tmem_base + ((uint32_t)(q * 32) << 16) + buf * 256 + c, v);
+                        tmem_ld_wait();
+#pragma unroll
+                        for (int j = 0; j < 16; ++j)
+                            if (c + j < cnt) dst[(size_t)(c + j) * 128] = __uint_as_float(v[j]);
+                    }
+                    tc_fence_before();
+                    __syncwarp();
+                    if (lane == 0) mbar_arrive(&H->tmem_empty[buf]);
+                    ++pc;
+                    a = a_next;
+                }
+            }
+        }
+    }
+    tc_fence_before();
+    __syncthreads();
+    if (warp == 1) tmem_dealloc<kTmemCols>(tmem_base);
+}
+
+}  // namespace
+
+cudaError_t cc_gemm_configure() {
+    return cudaFuncSetAttribute(k_gemm, cudaFuncAttributeMaxDynamicSharedMemorySize, kGemmSmem);
+}
+
+cudaError_t cc_launch_gemm(int which, const CcDims& D, const CcLayerTable* tab, const CcWork& W, const CcLaunch& L) {
+    const CcGemmGeo* G;
+    const uint8_t* act;
+    float* part;
+    switch (which) {
+        case 0: G = &D.qkv; act = W.x_act; part = W.qkv_part; break;
+        case 1: G = &D.o; act = W.o_act; part = W.o_part; break;
+        case 2: G = &D.gu; act = W.y_act; part = W.gu_part; break;
+        default: G = &D.dn; act = W.a_act; part = W.d_part; break;
+    }
+    return cc_launch_kernel(k_gemm, dim3(G->P), dim3(kGemmThreads), (size_t)kGemmSmem, L, *G, act, part, D.Mpad, tab,
+                            W.sched);
+}

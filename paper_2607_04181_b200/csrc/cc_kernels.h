@@ -1,0 +1,84 @@
+// cc_kernels.h -- host-callable launchers of the sm_100a kernels (product code).
+#pragma once
+#include "cc_common.cuh"
+
+// Device workspace of one layer (allocated once at cc_create_layer; PAPER.md:393 persistent pool).
+struct CcWork {
+    CcSched* sched;
+    int* perm;           // [Mpad] original row at grouped position, or -1
+    int2* items;         // attention work items (pos, chunk), at most max_batch * nch_max
+    uint8_t* x_act;      // packed bf16 GEMM operands, [K/64][Mpad][128 B swizzled]
+    uint8_t* o_act;
+    uint8_t* y_act;
+    uint8_t* a_act;
+    float* qkv_part;     // stream-K partial sums, [P + T][Mpad][128] fp32 (piece-major)
+    float* o_part;
+    float* gu_part;
+    float* d_part;
+    float* q_rot;        // [Mpad][Hq*Dh] fp32, q after RoPE
+    float* h1;           // [Mpad][d]     fp32, hidden + O projection
+    float* att_o;        // [Mpad*Hq][nch_max][Dh] fp32 un-normalised chunk outputs
+    float2* att_ml;      // [Mpad*Hq][nch_max] (max in log2 units, sum)
+    const float2* rope_cs;  // [max_position][Dh/2] (cos, sin), built in fp64 on the host
+    uint32_t* err;       // sticky device error word (context-owned)
+    int nch_max;
+};
+
+struct CcKv {
+    __nv_bfloat16* k_pool;
+    __nv_bfloat16* v_pool;
+    const int* block_table;
+    int n_pages;
+};
+
+// Launch options shared by the forward chain.
+struct CcLaunch {
+    cudaStream_t st;
+    int n_sms;
+    bool pdl;            // programmatic dependent launch between the kernels of the chain
+};
+
+cudaError_t cc_kernels_configure();   // sets max dynamic smem attributes once per process/device
+
+cudaError_t cc_launch_group(const int* assign, const int* seq_lens, int batch, const CcDims& D,
+                            const CcLayerTable* tab, const CcWork& W, const CcLaunch& L);
+cudaError_t cc_launch_rmsnorm_in(const __nv_bfloat16* hidden, const CcDims& D, const CcLayerTable* tab,
+                                 const CcWork& W, const CcLaunch& L);
+// which: 0 = QKV, 1 = O, 2 = gate/up, 3 = down
+cudaError_t cc_launch_gemm(int which, const CcDims& D, const CcLayerTable* tab, const CcWork& W, const CcLaunch& L);
+cudaError_t cc_launch_rope_append(const int* seq_lens, const CcKv& kv, const CcDims& D, const CcWork& W,
+                                  const CcLaunch& L);
+cudaError_t cc_launch_attention(const int* seq_lens, const CcKv& kv, const CcDims& D, const CcWork& W,
+                                const CcLaunch& L);
+cudaError_t cc_launch_attn_combine(const int* seq_lens, const CcDims& D, const CcWork& W, const CcLaunch& L);
+cudaError_t cc_launch_resid_norm(const __nv_bfloat16* hidden, const CcDims& D, const CcLayerTable* tab,
+                                 const CcWork& W, const CcLaunch& L);
+cudaError_t cc_launch_swiglu(const CcDims& D, const CcWork& W, const CcLaunch& L);
+cudaError_t cc_launch_final(__nv_bfloat16* hidden, const CcDims& D, const CcWork& W, const CcLaunch& L);
+
+cudaError_t cc_launch_copy(void* dst, const void* src, size_t bytes, int n_sms, cudaStream_t st);
+cudaError_t cc_launch_publish(CcLayerTable* row_dev, const CcLayerTable& value, cudaStream_t st);
+// mode 0: rows of src0, then src1, then src2 (concatenated); mode 1: rows alternate src0[j], src1[j].
+cudaError_t cc_launch_pack(uint8_t* dst, const __nv_bfloat16* src0, const __nv_bfloat16* src1,
+                           const __nv_bfloat16* src2, int rows0, int rows1, int rows2, int mode, int K, int n_tiles,
+                           int k_blocks, cudaStream_t st);
+// which: 0 = packed act buffer (bf16, K = dim), 1 = fp32 row buffer [Mpad][dim]
+cudaError_t cc_launch_tap(const void* src, int which, int dim, const CcDims& D, const CcWork& W, float* out_dev,
+                          int batch, cudaStream_t st);
+
+// Generic launcher: plain <<<>>> semantics, plus the PDL attribute when asked for.
+template <typename... KArgs, typename... Args>
+static inline cudaError_t cc_launch_kernel(void (*kern)(KArgs...), dim3 grid, dim3 block, size_t smem,
+                                           const CcLaunch& L, Args&&... args) {
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = grid;
+    cfg.blockDim = block;
+    cfg.dynamicSmemBytes = smem;
+    cfg.stream = L.st;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = L.pdl ? 1 : 0;
+    return cudaLaunchKernelEx(&cfg, kern, KArgs(args)...);
+}

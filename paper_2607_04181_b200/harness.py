@@ -1,0 +1,113 @@
+"""Plumbing shared by tests/, bench.py and __graft_entry__.smoke(): moves the seeded inputs of
+`inputs.py` into torch CUDA tensors and drives the C ABI through `binding`.  No arithmetic of the
+method lives here -- torch is used for device memory, streams and CUDA graphs only.
+"""
+from __future__ import annotations
+
+import numpy as np
+import torch
+
+from . import binding as B
+from . import inputs as I
+
+
+def _dev_u16(a: np.ndarray, device) -> torch.Tensor:
+    """uint16 bf16 bit patterns -> torch bf16 tensor on the device (bit-exact)."""
+    t = torch.from_numpy(np.ascontiguousarray(a).view(np.int16))
+    return t.to(device).view(torch.bfloat16)
+
+
+def _host_u16(t: torch.Tensor) -> np.ndarray:
+    return t.detach().cpu().contiguous().view(torch.int16).numpy().view(np.uint16).copy()
+
+
+def make_desc(shape: I.LayerShape, max_batch: int, max_blocks: int | None = None,
+              max_position: int | None = None) -> B.cc_layer_desc:
+    mb = shape.max_blocks if max_blocks is None else max_blocks
+    mp = mb * shape.page if max_position is None else max_position
+    return B.cc_layer_desc(shape.hidden, shape.n_q_heads, shape.n_kv_heads, shape.head_dim, shape.ffn,
+                           shape.rms_eps, shape.rope_base, shape.page, max_batch, mb, mp)
+
+
+class DeviceStep:
+    """One batch of step inputs resident in HBM."""
+
+    def __init__(self, st: I.StepInputs, assign: np.ndarray, device="cuda:0"):
+        self.device = device
+        self.batch = st.hidden.shape[0]
+        self.n_pages = st.n_pages
+        self.hidden = _dev_u16(st.hidden, device)
+        self.k_pool = _dev_u16(st.k_pool, device)
+        self.v_pool = _dev_u16(st.v_pool, device)
+        self.block_table = torch.from_numpy(st.block_table).to(device)
+        self.seq_lens = torch.from_numpy(st.seq_lens).to(device)
+        self.assign = torch.from_numpy(np.ascontiguousarray(assign, dtype=np.int32)).to(device)
+
+    def reset(self, st: I.StepInputs) -> None:
+        """Re-upload hidden and the KV pools (both are modified in place by a step)."""
+        self.hidden.copy_(_dev_u16(st.hidden, self.device))
+        self.k_pool.copy_(_dev_u16(st.k_pool, self.device))
+        self.v_pool.copy_(_dev_u16(st.v_pool, self.device))
+
+    def set_assign(self, assign: np.ndarray) -> None:
+        self.assign.copy_(torch.from_numpy(np.ascontiguousarray(assign, dtype=np.int32)))
+
+    def out_bits(self) -> np.ndarray:
+        return _host_u16(self.hidden)
+
+    def pools_bits(self):
+        return _host_u16(self.k_pool), _host_u16(self.v_pool)
+
+
+class Session:
+    """Context + one layer + a donated arena for replica slots."""
+
+    def __init__(self, shape: I.LayerShape, weights: dict, max_batch: int, n_slots: int = I.MAX_REPLICAS - 1,
+                 device_index: int = 0, max_blocks: int | None = None, max_position: int | None = None):
+        self.shape = shape
+        self.device = f"cuda:{device_index}"
+        torch.cuda.set_device(device_index)
+        self.ctx = B.cc_ctx_create(device_index)
+        self.desc = make_desc(shape, max_batch, max_blocks, max_position)
+        wdev = {k: _dev_u16(v, self.device) for k, v in weights.items()}
+        self.layer = B.cc_create_layer(self.ctx, self.desc, wdev)
+        del wdev                                   # the library keeps its own packed copy (slot 0)
+        self.blob_bytes = B.cc_layer_blob_bytes(self.layer)
+        self.arena = None
+        if n_slots > 0:
+            slot = (self.blob_bytes + 1023) // 1024 * 1024
+            self.arena = torch.empty(n_slots * slot + 2048, dtype=torch.uint8, device=self.device)
+            B.cc_ctx_donate(self.ctx, self.arena, self.arena.numel())
+
+    def forward(self, step: DeviceStep, stream=None) -> None:
+        B.cc_forward(self.layer, step.hidden, step.k_pool, step.v_pool, step.block_table, step.n_pages,
+                     step.seq_lens, step.assign, step.batch, stream)
+
+    def scale(self, n: int, stream=None) -> None:
+        """cc_scale_layer + cc_commit on `stream` (default: torch's current stream)."""
+        B.cc_scale_layer(self.layer, n)
+        B.cc_commit(self.layer, torch.cuda.current_stream() if stream is None else stream)
+
+    def tap(self, which: int, batch: int) -> np.ndarray:
+        dims = {B.CC_TAP_X: self.shape.hidden, B.CC_TAP_Q: self.shape.q_dim, B.CC_TAP_O: self.shape.q_dim,
+                B.CC_TAP_H1: self.shape.hidden, B.CC_TAP_Y: self.shape.hidden, B.CC_TAP_A: self.shape.ffn}
+        return B.cc_debug_tap(self.layer, which, batch, dims[which])
+
+    def close(self) -> None:
+        if self.layer is not None:
+            torch.cuda.synchronize()
+            B.cc_destroy_layer(self.layer)
+            self.layer = None
+        if self.ctx is not None:
+            if self.arena is not None:
+                B.cc_ctx_reclaim(self.ctx, self.arena)
+            B.cc_ctx_destroy(self.ctx)
+            self.ctx = None
+        self.arena = None
+
+    def __enter__(self):
+        return self
+
+    def __exit__(self, *exc):
+        self.close()
+        return False
