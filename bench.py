@@ -1,0 +1,392 @@
+#!/usr/bin/env python
+"""bench.py -- replicated decode-layer throughput on B200 (BASELINE.json metric).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--replicas R] [--impl reference]
+
+A "step" is one pass of the whole hot path (cc_forward: grouping, RMSNorm, QKV GEMM, RoPE + KV
+append, paged GQA decode attention, O GEMM, RMSNorm, gate/up GEMM + SwiGLU, down GEMM, residual)
+over one decode batch of BASELINE.json configs[1]: the Llama-3-8B-shaped layer, batch 64, contexts
+U{512..2048} in shuffled 16-token pages, the batch split evenly over R replicas of the layer
+(default R = 2).  Inputs are seeded and synthetic (inputs.py) and resident in HBM before the timed
+region; each step streams R x 436 MB of weights + ~335 MB of KV, far more than the 126 MB L2, so
+consecutive steps cannot hit in cache.  Prints ONE JSON line.
+
+N > 1 (torchrun): the path does not shard -- "replicas only": every rank runs its own independent
+batch on its own GPU, no data-path collective; value = all ranks' tokens / max-over-ranks time.
+
+--impl reference times the CPU oracle (oracle/, as it stands) on a bounded sample of the same
+workload; it is a deliberately slow baseline, not the target.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "replicated decode-layer tokens/s"
+UNIT = "tokens/s"
+REF_ROWS_PER_STEP = 4       # --impl reference: rows of the batch the oracle computes per step
+CPU_BASELINE_ROWS = 32      # cpu_baseline leg of the default arm (about 10 s of CPU work)
+FALLBACK_HBM_GBS = 6650.0   # /opt/skills/guides/B200_PROFILING.md, used only if MEASURED_PEAKS.json is absent
+
+
+def parse_args():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=200)
+    ap.add_argument("--warmup", type=int, default=20)
+    ap.add_argument("--replicas", type=int, default=2, choices=[1, 2, 3, 4])
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    return ap.parse_args()
+
+
+def measured_peak():
+    try:
+        with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as f:
+            return float(json.load(f)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs, read+write copy)"
+    except Exception:
+        return FALLBACK_HBM_GBS, "fallback (B200_PROFILING.md)"
+
+
+# ---------------------------------------------------------------------------------------------
+# clocks during the timed region (NVML, polled from a thread)
+# ---------------------------------------------------------------------------------------------
+_REASONS = {0x4: "sw_power_cap", 0x8: "hw_slowdown", 0x20: "sw_thermal_slowdown", 0x40: "hw_thermal_slowdown",
+            0x80: "hw_power_brake_slowdown", 0x2: "applications_clocks_setting", 0x10: "sync_boost"}
+
+
+class ClockSampler:
+    def __init__(self, torch_device_index: int):
+        self.samples, self.reasons, self.max_mhz, self.ok = [], set(), None, False
+        self._stop = threading.Event()
+        try:
+            import pynvml
+            import torch
+            pynvml.nvmlInit()
+            try:
+                uuid = str(torch.cuda.get_device_properties(torch_device_index).uuid)
+                self.h = pynvml.nvmlDeviceGetHandleByUUID(("GPU-" + uuid) if not uuid.startswith("GPU-") else uuid)
+            except Exception:
+                self.h = pynvml.nvmlDeviceGetHandleByIndex(torch_device_index)
+            self.nv = pynvml
+            self.max_mhz = float(pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM))
+            self.ok = True
+        except Exception:
+            self.ok = False
+        self.t = threading.Thread(target=self._run, daemon=True)
+
+    def _run(self):
+        while not self._stop.is_set():
+            try:
+                self.samples.append(float(self.nv.nvmlDeviceGetClockInfo(self.h, self.nv.NVML_CLOCK_SM)))
+                try:
+                    bits = int(self.nv.nvmlDeviceGetCurrentClocksEventReasons(self.h))
+                except Exception:
+                    bits = int(self.nv.nvmlDeviceGetCurrentClocksThrottleReasons(self.h))
+                for b, name in _REASONS.items():
+                    if bits & b:
+                        self.reasons.add(name)
+            except Exception:
+                pass
+            time.sleep(0.004)
+
+    def start(self):
+        if self.ok:
+            self.t.start()
+
+    def stop(self):
+        self._stop.set()
+        if self.ok:
+            self.t.join(timeout=2)
+        med = float(np.median(self.samples)) if self.samples else None
+        return {"sm_mhz": med, "sm_max_mhz": self.max_mhz, "reasons": sorted(self.reasons), "samples": len(self.samples)}
+
+
+# ---------------------------------------------------------------------------------------------
+# algorithmic bytes; bookkeeping only
+# ---------------------------------------------------------------------------------------------
+def stage_bytes(shape, seq_lens, n_groups: int) -> dict:
+    d, F, QD, KD = shape.hidden, shape.ffn, shape.q_dim, shape.kv_dim
+    B = int((seq_lens > 0).sum())
+    tok = int(seq_lens[seq_lens > 0].sum())                     # tokens attended, including the new one
+    return {
+        "gemm_qkv": n_groups * (QD + 2 * KD) * d * 2 + B * d * 2,
+        "attention": tok * 2 * KD * 2 + B * QD * 4,
+        "gemm_o": n_groups * d * QD * 2 + B * QD * 2,
+        "gemm_gate_up": n_groups * 2 * F * d * 2 + B * d * 2,
+        "gemm_down": n_groups * d * F * 2 + B * F * 2,
+    }
+
+
+# ---------------------------------------------------------------------------------------------
+# the reference arm: the CPU oracle on a bounded sample
+# ---------------------------------------------------------------------------------------------
+def time_oracle(shape, w, st, rows: int, steps: int, warmup: int):
+    import oracle
+    sub = slice(0, rows)
+    assign = np.zeros(rows, np.int32)
+
+    def one():
+        oracle.layer_forward(shape, w, st.hidden[sub], st.k_pool, st.v_pool, st.block_table[sub], st.seq_lens[sub],
+                             assign, 1)
+    for _ in range(warmup):
+        one()
+    t0 = time.perf_counter()
+    for _ in range(steps):
+        one()
+    dt = time.perf_counter() - t0
+    return rows * steps / dt, dt / steps, oracle.num_threads()
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return 0
+    from paper_2607_04181_b200 import inputs as I
+    shape = I.CFG2
+    w = I.make_weights(shape, 1002)
+    st = I.make_step_inputs(shape, 2002, 3002)
+    tps, s_per_step, cores = time_oracle(shape, w, st, REF_ROWS_PER_STEP, args.steps, args.warmup)
+    sample = (f"{REF_ROWS_PER_STEP} of the 64 rows of the cfg2 decode batch per step (full contexts, full layer), "
+              f"oracle/cc_oracle.c as it stands, OpenMP over {cores} threads")
+    line = {
+        "impl": "reference", "metric": METRIC, "value": tps, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": s_per_step * 1e3, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+        "config": {"workload": "cfg2: Llama-3-8B-shaped decoder layer, decode batch 64, contexts U{512..2048}, "
+                               "16-token pages, shuffled block tables", "sample": sample},
+        "cpu_baseline": {"value": tps, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+        "e2e": {"value": tps, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line), flush=True)
+    return 0
+
+
+# ---------------------------------------------------------------------------------------------
+# our arm
+# ---------------------------------------------------------------------------------------------
+def run_ours(args):
+    import torch
+    import torch.distributed as dist
+
+    from paper_2607_04181_b200 import binding as B
+    from paper_2607_04181_b200 import inputs as I
+    from paper_2607_04181_b200.harness import DeviceStep, Session
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the library has no CPU fallback")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device(f"cuda:{local}"))
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    shape, R, K, W = I.CFG2, args.replicas, args.steps, max(args.warmup, 3)
+    batch = shape.batch
+    w = I.make_weights(shape, 1002)
+    st = I.make_step_inputs(shape, 2002 + 10 * rank, 3002 + 10 * rank)     # every rank its own batch
+    assign = I.even_split(batch, R)
+    S = Session(shape, w, max_batch=batch, n_slots=3, device_index=local)
+    S.scale(R)
+    step = DeviceStep(st, assign, device=f"cuda:{local}")
+    stream = torch.cuda.current_stream()
+    for _ in range(3):
+        S.forward(step)
+    torch.cuda.synchronize()
+    graph = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(graph):
+        S.forward(step, torch.cuda.current_stream())
+    n_launch = B.cc_forward_launch_count(S.layer)
+
+    # ---- device-resident timed region: K graph replays ------------------------------------------
+    for _ in range(W):
+        graph.replay()
+    sampler = ClockSampler(local)
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    sampler.start()
+    ev0.record()
+    for _ in range(K):
+        graph.replay()
+    ev1.record()
+    barrier()
+    ms_total = ev0.elapsed_time(ev1)
+    # the timed region is short (K x ~0.2 ms): keep the same load running for ~1 s so that the NVML
+    # poll sees clocks and throttle reasons under this load (not part of any reported time)
+    t_end = time.perf_counter() + max(0.0, 1.0 - ms_total / 1e3)
+    while time.perf_counter() < t_end:
+        for _ in range(50):
+            graph.replay()
+        torch.cuda.synchronize()
+    clocks = sampler.stop()
+    if world > 1:
+        t = torch.tensor([ms_total], device=f"cuda:{local}")
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms_total = float(t.item())
+    ms_step = ms_total / K
+    value = world * batch * K / (ms_total / 1e3)
+    assert B.cc_poll_device_error(S.ctx) == 0
+
+    # ---- per-kernel roofline: the same step launched kernel by kernel with events between ---------
+    peak, peak_src = measured_peak()
+    n_prof = min(K, 50)
+    stage_ms = np.zeros(n_launch, dtype=np.float64)
+    for _ in range(3):
+        B.cc_forward_profiled(S.layer, step.hidden, step.k_pool, step.v_pool, step.block_table, step.n_pages,
+                              step.seq_lens, step.assign, batch, stream)
+    for _ in range(n_prof):
+        stage_ms += B.cc_forward_profiled(S.layer, step.hidden, step.k_pool, step.v_pool, step.block_table,
+                                          step.n_pages, step.seq_lens, step.assign, batch, stream)
+    stage_ms /= n_prof
+    sb = stage_bytes(shape, st.seq_lens, R)
+    stages = {}
+    for i, name in enumerate(B.STAGE_NAMES):
+        e = {"ms": round(float(stage_ms[i]), 5)}
+        if name in sb:
+            e["bytes"] = sb[name]
+            e["GBps"] = round(sb[name] / (stage_ms[i] * 1e-3) / 1e9, 1)
+            e["frac"] = round(e["GBps"] / peak, 4)
+        stages[name] = e
+    dom = max(sb, key=sb.get)
+    dom_ms = float(stage_ms[B.STAGE_NAMES.index(dom)])
+    achieved = sb[dom] / (dom_ms * 1e-3) / 1e9
+    roofline = {"bound": "hbm", "kernel": dom, "achieved": round(achieved, 1), "peak": peak, "unit": "GB/s",
+                "frac": round(achieved / peak, 4), "traffic": None, "peak_source": peak_src,
+                "kernel_ms": round(dom_ms, 5), "algorithmic_bytes": sb[dom],
+                "how": f"mean of {n_prof} launches, CUDA events around the kernel on its stream (cc_forward_profiled)"}
+    alg_bytes = I.forward_algorithmic_bytes(shape, st.seq_lens, R)
+    step_gbps = alg_bytes / (ms_step * 1e-3) / 1e9
+
+    # ---- other replica counts (outside the timed region; context for the headline) -------------------
+    by_r = {}
+    for r in (1, 2, 4):
+        S.scale(r)
+        step.set_assign(I.even_split(batch, r))
+        for _ in range(5):
+            graph.replay()
+        a, b_ = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record()
+        for _ in range(50):
+            graph.replay()
+        b_.record()
+        torch.cuda.synchronize()
+        ms = a.elapsed_time(b_) / 50
+        ab = I.forward_algorithmic_bytes(shape, st.seq_lens, r)
+        by_r[str(r)] = {"tokens_per_s": round(batch / (ms * 1e-3), 1), "ms_per_step": round(ms, 5),
+                        "algorithmic_GBps": round(ab / (ms * 1e-3) / 1e9, 1),
+                        "frac_of_peak": round(ab / (ms * 1e-3) / 1e9 / peak, 4)}
+    S.scale(R)
+    step.set_assign(assign)
+    torch.cuda.synchronize()
+
+    # ---- end to end through the C ABI with HOST buffers (pinned): H2D + step + D2H inside the timing ----
+    h_hidden = torch.from_numpy(st.hidden.view(np.int16).copy()).pin_memory()
+    h_bt = torch.from_numpy(st.block_table.copy()).pin_memory()
+    h_sl = torch.from_numpy(st.seq_lens.copy()).pin_memory()
+    h_ra = torch.from_numpy(assign.copy()).pin_memory()
+    for _ in range(W):
+        B.cc_forward_host(S.layer, h_hidden, step.k_pool, step.v_pool, step.n_pages, h_bt, h_sl, h_ra, batch, stream)
+    barrier()
+    t0 = time.perf_counter()
+    for _ in range(K):
+        B.cc_forward_host(S.layer, h_hidden, step.k_pool, step.v_pool, step.n_pages, h_bt, h_sl, h_ra, batch, stream)
+    torch.cuda.synchronize()
+    e2e_s = time.perf_counter() - t0
+    if world > 1:
+        t = torch.tensor([e2e_s], device=f"cuda:{local}")
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        e2e_s = float(t.item())
+    h2d = h_hidden.numel() * 2 + h_bt.numel() * 4 + h_sl.numel() * 4 + h_ra.numel() * 4
+    e2e = {"value": world * batch * K / e2e_s, "unit": UNIT, "h2d_bytes_per_step": int(h2d),
+           "d2h_bytes_per_step": int(h_hidden.numel() * 2), "ms_per_step": e2e_s / K * 1e3,
+           "api": "cc_forward_host (pinned host hidden/block_table/seq_lens/replica_assign in, hidden out; "
+                  "KV pools and weights are device-resident state)"}
+
+    # ---- replica creation: cc_scale_layer (chunked copy on the side stream) -> cc_commit (visible) ----
+    copy_ms = []
+    S.scale(1)
+    torch.cuda.synchronize()
+    for _ in range(8):
+        a, b_ = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record()
+        B.cc_scale_layer(S.layer, 2)
+        B.cc_commit(S.layer, stream)              # stream waits for the copy, then the table flip
+        b_.record()
+        torch.cuda.synchronize()
+        copy_ms.append(a.elapsed_time(b_))
+        S.scale(1)
+        torch.cuda.synchronize()
+    cms = float(np.median(copy_ms[2:]))
+    blob = S.blob_bytes
+    replica_copy = {"blob_bytes": blob, "ms_call_to_visible": round(cms, 4),
+                    "GBps_read_plus_write": round(2 * blob / (cms * 1e-3) / 1e9, 1),
+                    "GBps_payload": round(blob / (cms * 1e-3) / 1e9, 1),
+                    "frac_of_copy_peak": round(2 * blob / (cms * 1e-3) / 1e9 / peak, 4),
+                    "graph_recaptures": 0}
+
+    # ---- the oracle on this box's host cores, bounded sample (rank 0, N = 1) --------------------------
+    cpu = None
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        tps, s_per_step, cores = time_oracle(shape, w, st, CPU_BASELINE_ROWS, 1, 0)
+        cpu = {"value": tps, "unit": UNIT, "cores": cores, "kind": "oracle",
+               "sample": f"first {CPU_BASELINE_ROWS} of the 64 rows of the same cfg2 batch, one full layer step, "
+                         f"{s_per_step:.1f} s of oracle/cc_oracle.c (OpenMP)"}
+    S.close()
+
+    if rank == 0:
+        line = {
+            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
+            "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "bf16", "data": "synthetic",
+            "config": {"workload": "cfg2 (BASELINE.json configs[1]): Llama-3-8B-shaped decoder layer, hidden 4096, "
+                                   "32 q / 8 kv heads x 128, FFN 14336, decode batch 64, contexts U{512..2048}, "
+                                   "16-token pages, shuffled block tables",
+                       "replicas": R, "batch_split": np.bincount(assign, minlength=R).tolist(),
+                       "launch": "one CUDA graph of cc_forward, replayed; PDL between its kernels",
+                       "l2": "inputs larger than L2: each step streams R x 436 MB weights + 335 MB KV (L2 = 126 MB)",
+                       "parallelism": "replicas only (one independent batch per GPU)" if world > 1 else "single GPU"},
+            "clocks": clocks,
+            "e2e": e2e,
+            "gpu_launches": n_launch * K,
+            "roofline": roofline,
+            "step_roofline": {"algorithmic_bytes": alg_bytes, "achieved_GBps": round(step_gbps, 1),
+                              "frac_of_measured_peak": round(step_gbps / peak, 4),
+                              "frac_of_8TBps": round(step_gbps / 8000.0, 4)},
+            "stages": stages,
+            "by_replicas": by_r,
+            "replica_copy": replica_copy,
+            "cpu_baseline": cpu,
+        }
+        print(json.dumps(line), flush=True)
+    if world > 1:
+        dist.barrier()
+        dist.destroy_process_group()
+    return 0
+
+
+def main():
+    args = parse_args()
+    if args.impl == "reference":
+        return run_reference(args)
+    return run_ours(args)
+
+
+if __name__ == "__main__":
+    sys.exit(main())

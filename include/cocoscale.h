@@ -66,7 +66,7 @@ typedef struct cc_ctx cc_ctx;     /* device, side stream, donated ranges, replic
 typedef struct cc_layer cc_layer; /* one decoder layer: slot 0 blob, replica slots, workspace        */
 
 typedef struct {
-    int32_t hidden;              /* d; multiple of 64                                           */
+    int32_t hidden;              /* d; multiple of 64, at most 8192                             */
     int32_t n_q_heads;           /* Hq                                                          */
     int32_t n_kv_heads;          /* Hkv; Hq % Hkv == 0 and Hq / Hkv <= 8                        */
     int32_t head_dim;            /* Dh: 64 or 128                                               */
@@ -181,6 +181,15 @@ cc_status cc_forward_host(cc_layer *layer, void *hidden_host, void *k_pool_dev, 
                           int32_t n_pages, const int32_t *block_table_host, const int32_t *seq_lens_host,
                           const int32_t *replica_assign_host, int batch, void *stream);
 
+/* The same step, launched kernel by kernel with a CUDA event between consecutive kernels (so
+ * without programmatic dependent launch), synchronised; stage_ms_host[i] (host, fp32
+ * [cc_forward_launch_count]) receives the device time of kernel i in milliseconds, in launch
+ * order: grouping, input norm, QKV GEMM, RoPE+append, attention, chunk merge, O GEMM,
+ * residual+norm, gate/up GEMM, SwiGLU, down GEMM, residual/write-back.  For per-kernel roofline
+ * accounting; not capture-safe. */
+cc_status cc_forward_profiled(cc_layer *layer, void *hidden_dev, const cc_kv_pages *kv, const int32_t *seq_lens_dev,
+                              const int32_t *replica_assign_dev, int batch, void *stream, float *stage_ms_host);
+
 /* Kernel launches one cc_forward enqueues (for launch accounting). */
 cc_status cc_forward_launch_count(const cc_layer *layer, int *n);
 
@@ -192,12 +201,12 @@ cc_status cc_replica_copy(cc_ctx *ctx, void *dst_dev, const void *src_dev, size_
 
 /* ---- stage taps (tests only; reads the workspace left by the last cc_forward) ---------------- */
 typedef enum {
-    CC_TAP_X = 0,   /* [batch][hidden]      input RMSNorm output (bf16 operand, widened)        */
+    CC_TAP_X = 0,   /* [batch][hidden]      input RMSNorm output (GEMM operand: bf16 hi + lo)   */
     CC_TAP_Q = 1,   /* [batch][Hq*Dh]       q after RoPE (fp32)                                 */
-    CC_TAP_O = 2,   /* [batch][Hq*Dh]       attention output (bf16 operand, widened)            */
+    CC_TAP_O = 2,   /* [batch][Hq*Dh]       attention output (GEMM operand: one bf16 plane)     */
     CC_TAP_H1 = 3,  /* [batch][hidden]      hidden + O-projection (fp32)                        */
-    CC_TAP_Y = 4,   /* [batch][hidden]      post-attention RMSNorm output (bf16 operand)        */
-    CC_TAP_A = 5    /* [batch][ffn]         silu(gate)*up (bf16 operand)                        */
+    CC_TAP_Y = 4,   /* [batch][hidden]      post-attention RMSNorm output (bf16 hi + lo)        */
+    CC_TAP_A = 5    /* [batch][ffn]         silu(gate)*up (bf16 hi + lo)                        */
 } cc_tap;
 /* out_host: fp32 [batch][dim] in ORIGINAL row order; padding rows are zero. Synchronous. */
 cc_status cc_debug_tap(cc_layer *layer, cc_tap which, float *out_host, int batch);

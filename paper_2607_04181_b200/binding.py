@@ -29,7 +29,7 @@ EXPORTS = (
     "cc_ctx_create", "cc_ctx_destroy", "cc_ctx_donate", "cc_ctx_reclaim", "cc_ctx_set_copy_chunk",
     "cc_ctx_set_pdl", "cc_poll_device_error", "cc_create_layer", "cc_destroy_layer", "cc_layer_blob_bytes",
     "cc_scale_layer", "cc_commit", "cc_release_replica", "cc_query", "cc_replica_blob", "cc_forward",
-    "cc_forward_host", "cc_forward_launch_count", "cc_replica_copy", "cc_debug_tap", "cc_debug_grouping",
+    "cc_forward_host", "cc_forward_profiled", "cc_forward_launch_count", "cc_replica_copy", "cc_debug_tap", "cc_debug_grouping",
     "cc_slotalloc_create", "cc_slotalloc_destroy", "cc_slotalloc_donate", "cc_slotalloc_reclaim",
     "cc_slotalloc_alloc", "cc_slotalloc_free", "cc_slotalloc_free_bytes", "cc_last_error", "cc_version",
 )
@@ -206,6 +206,19 @@ def cc_forward_host(layer, hidden_host, k_pool, v_pool, n_pages: int, block_tabl
     _check(_lib.cc_forward_host(layer, _ptr(hidden_host), _ptr(k_pool), _ptr(v_pool), C.c_int32(n_pages),
                                 _ptr(block_table_host), _ptr(seq_lens_host), _ptr(replica_assign_host),
                                 C.c_int(batch), _stream(stream)))
+
+
+STAGE_NAMES = ("group", "rmsnorm_in", "gemm_qkv", "rope_append", "attention", "attn_combine", "gemm_o",
+               "resid_norm", "gemm_gate_up", "swiglu", "gemm_down", "final")
+
+
+def cc_forward_profiled(layer, hidden, k_pool, v_pool, block_table, n_pages: int, seq_lens, replica_assign,
+                        batch: int, stream=None) -> np.ndarray:
+    kv = cc_kv_pages(_ptr(k_pool), _ptr(v_pool), _ptr(block_table), C.c_int32(n_pages))
+    ms = np.zeros(len(STAGE_NAMES), dtype=np.float32)
+    _check(_lib.cc_forward_profiled(layer, _ptr(hidden), C.byref(kv), _ptr(seq_lens), _ptr(replica_assign),
+                                    C.c_int(batch), _stream(stream), _ptr(ms)))
+    return ms
 
 
 def cc_forward_launch_count(layer) -> int:

@@ -15,7 +15,6 @@
 
 cudaError_t cc_gemm_configure();
 cudaError_t cc_attn_configure();
-cudaError_t cc_rowwise_configure(int max_d);
 
 namespace {
 
@@ -226,7 +225,6 @@ cc_status cc_ctx_create(int device, cc_ctx** out) {
     CC_CUDA(cudaMemset(ctx->err_dev, 0, 256));
     CC_CUDA(cc_gemm_configure());
     CC_CUDA(cc_attn_configure());
-    CC_CUDA(cc_rowwise_configure(0));
     ctx->slots = cc_slotalloc_create();
     const char* env = getenv("CC_PDL");
     if (env && env[0] == '0') ctx->pdl = false;
@@ -334,7 +332,8 @@ cc_status cc_create_layer(cc_ctx* ctx, const cc_layer_desc* desc, const cc_layer
     if (!ctx || !desc || !w || !out) return fail(CC_ERR_INVALID, "null argument");
     *out = nullptr;
     const cc_layer_desc& d = *desc;
-    if (d.hidden <= 0 || d.hidden % 64) return fail(CC_ERR_INVALID, "hidden must be a positive multiple of 64");
+    if (d.hidden <= 0 || d.hidden % 64 || d.hidden > cc_max_hidden())
+        return fail(CC_ERR_INVALID, "hidden must be a positive multiple of 64, at most %d", cc_max_hidden());
     if (d.head_dim != 64 && d.head_dim != 128) return fail(CC_ERR_INVALID, "head_dim must be 64 or 128");
     if (d.n_kv_heads <= 0 || d.n_q_heads <= 0 || d.n_q_heads % d.n_kv_heads || d.n_q_heads / d.n_kv_heads > 8)
         return fail(CC_ERR_INVALID, "need n_q_heads %% n_kv_heads == 0 and a GQA group of at most 8");
@@ -386,10 +385,10 @@ cc_status cc_create_layer(cc_ctx* ctx, const cc_layer_desc* desc, const cc_layer
     const size_t o_sched = ws.take(sizeof(CcSched));
     const size_t o_perm = ws.take(Mp * 4);
     const size_t o_items = ws.take((size_t)d.max_batch * W.nch_max * sizeof(int2));
-    const size_t o_x = ws.take((size_t)D.qkv.KB * Mp * 128);
+    const size_t o_x = ws.take((size_t)2 * D.qkv.KB * Mp * 128);   // hi + lo planes
     const size_t o_o = ws.take((size_t)D.o.KB * Mp * 128);
-    const size_t o_y = ws.take((size_t)D.gu.KB * Mp * 128);
-    const size_t o_a = ws.take((size_t)D.dn.KB * Mp * 128);
+    const size_t o_y = ws.take((size_t)2 * D.gu.KB * Mp * 128);
+    const size_t o_a = ws.take((size_t)2 * D.dn.KB * Mp * 128);
     auto part_bytes = [&](const CcGemmGeo& g) { return (size_t)(g.P + g.T) * Mp * 128 * 4; };
     const size_t o_pq = ws.take(part_bytes(D.qkv));
     const size_t o_po = ws.take(part_bytes(D.o));
@@ -629,27 +628,34 @@ namespace {
 constexpr int kForwardLaunches = 12;
 
 cudaError_t enqueue_forward(cc_layer* L, __nv_bfloat16* hidden, const CcKv& kv, const int* seq_lens, const int* assign,
-                            int batch, cudaStream_t st) {
+                            int batch, cudaStream_t st, cudaEvent_t* ev = nullptr) {
     cc_ctx* ctx = L->ctx;
     const CcDims& D = L->D;
     const CcWork& W = L->W;
     const CcLayerTable* tab = ctx->table_dev + L->row;
-    CcLaunch Ln{st, ctx->n_sms, ctx->pdl};
-    cudaError_t e;
-    // a0 grouping | a1 norm | a2 QKV | a3+a4 RoPE + append | a5 attention (+ combine) | a6 O |
+    CcLaunch Ln{st, ctx->n_sms, ctx->pdl && ev == nullptr};
+    cudaError_t e = cudaSuccess;
+    // a0 grouping | a1 norm | a2 QKV | a3+a4 RoPE + append | a5 attention | a5 chunk merge | a6 O |
     // a6+a7 residual + norm | a8 gate/up | a8 SwiGLU | a9 down | a9 residual, original row order
-    if ((e = cc_launch_group(assign, seq_lens, batch, D, tab, W, Ln)) != cudaSuccess) return e;
-    if ((e = cc_launch_rmsnorm_in(hidden, D, tab, W, Ln)) != cudaSuccess) return e;
-    if ((e = cc_launch_gemm(0, D, tab, W, Ln)) != cudaSuccess) return e;
-    if ((e = cc_launch_rope_append(seq_lens, kv, D, W, Ln)) != cudaSuccess) return e;
-    if ((e = cc_launch_attention(seq_lens, kv, D, W, Ln)) != cudaSuccess) return e;
-    if ((e = cc_launch_attn_combine(seq_lens, D, W, Ln)) != cudaSuccess) return e;
-    if ((e = cc_launch_gemm(1, D, tab, W, Ln)) != cudaSuccess) return e;
-    if ((e = cc_launch_resid_norm(hidden, D, tab, W, Ln)) != cudaSuccess) return e;
-    if ((e = cc_launch_gemm(2, D, tab, W, Ln)) != cudaSuccess) return e;
-    if ((e = cc_launch_swiglu(D, W, Ln)) != cudaSuccess) return e;
-    if ((e = cc_launch_gemm(3, D, tab, W, Ln)) != cudaSuccess) return e;
-    return cc_launch_final(hidden, D, W, Ln);
+    for (int stage = 0; stage < kForwardLaunches && e == cudaSuccess; ++stage) {
+        if (ev && (e = cudaEventRecord(ev[stage], st)) != cudaSuccess) break;
+        switch (stage) {
+            case 0: e = cc_launch_group(assign, seq_lens, batch, D, tab, W, Ln); break;
+            case 1: e = cc_launch_rmsnorm_in(hidden, D, tab, W, Ln); break;
+            case 2: e = cc_launch_gemm(0, D, tab, W, Ln); break;
+            case 3: e = cc_launch_rope_append(seq_lens, kv, D, W, Ln); break;
+            case 4: e = cc_launch_attention(seq_lens, kv, D, W, Ln); break;
+            case 5: e = cc_launch_attn_combine(seq_lens, D, W, Ln); break;
+            case 6: e = cc_launch_gemm(1, D, tab, W, Ln); break;
+            case 7: e = cc_launch_resid_norm(hidden, D, tab, W, Ln); break;
+            case 8: e = cc_launch_gemm(2, D, tab, W, Ln); break;
+            case 9: e = cc_launch_swiglu(D, W, Ln); break;
+            case 10: e = cc_launch_gemm(3, D, tab, W, Ln); break;
+            default: e = cc_launch_final(hidden, D, W, Ln); break;
+        }
+    }
+    if (ev && e == cudaSuccess) e = cudaEventRecord(ev[kForwardLaunches], st);
+    return e;
 }
 }  // namespace
 
@@ -691,6 +697,24 @@ cc_status cc_forward_host(cc_layer* L, void* hidden_host, void* k_pool_dev, void
     return CC_OK;
 }
 
+cc_status cc_forward_profiled(cc_layer* L, void* hidden_dev, const cc_kv_pages* kv, const int32_t* seq_lens_dev,
+                              const int32_t* replica_assign_dev, int batch, void* stream, float* stage_ms_host) {
+    if (!L || !hidden_dev || !kv || !seq_lens_dev || !replica_assign_dev || !stage_ms_host)
+        return fail(CC_ERR_INVALID, "null argument");
+    if (batch < 1 || batch > L->desc.max_batch) return fail(CC_ERR_INVALID, "batch %d outside 1..max_batch=%d", batch, L->desc.max_batch);
+    CC_CUDA(cudaSetDevice(L->ctx->device));
+    cudaEvent_t ev[kForwardLaunches + 1];
+    for (auto& x : ev) CC_CUDA(cudaEventCreate(&x));
+    CcKv k{(__nv_bfloat16*)kv->k_pool, (__nv_bfloat16*)kv->v_pool, kv->block_table, kv->n_pages};
+    cudaError_t e = enqueue_forward(L, (__nv_bfloat16*)hidden_dev, k, seq_lens_dev, replica_assign_dev, batch,
+                                    (cudaStream_t)stream, ev);
+    if (e == cudaSuccess) e = cudaStreamSynchronize((cudaStream_t)stream);
+    for (int i = 0; i < kForwardLaunches && e == cudaSuccess; ++i) e = cudaEventElapsedTime(&stage_ms_host[i], ev[i], ev[i + 1]);
+    for (auto& x : ev) cudaEventDestroy(x);
+    if (e != cudaSuccess) return fail(CC_ERR_CUDA, "cc_forward_profiled: %s", cudaGetErrorString(e));
+    return CC_OK;
+}
+
 cc_status cc_forward_launch_count(const cc_layer* L, int* n) {
     if (!L || !n) return fail(CC_ERR_INVALID, "null argument");
     *n = kForwardLaunches;
@@ -704,13 +728,15 @@ cc_status cc_debug_tap(cc_layer* L, cc_tap which, float* out_host, int batch) {
     const CcDims& D = L->D;
     const void* src;
     int kind, dim;
+    size_t plane = 0;
+    const size_t Mp128 = (size_t)D.Mpad * 128;
     switch (which) {
-        case CC_TAP_X: src = L->W.x_act; kind = 0; dim = D.d; break;
+        case CC_TAP_X: src = L->W.x_act; kind = 2; dim = D.d; plane = D.qkv.KB * Mp128; break;
         case CC_TAP_Q: src = L->W.q_rot; kind = 1; dim = D.QD; break;
         case CC_TAP_O: src = L->W.o_act; kind = 0; dim = D.QD; break;
         case CC_TAP_H1: src = L->W.h1; kind = 1; dim = D.d; break;
-        case CC_TAP_Y: src = L->W.y_act; kind = 0; dim = D.d; break;
-        case CC_TAP_A: src = L->W.a_act; kind = 0; dim = D.F; break;
+        case CC_TAP_Y: src = L->W.y_act; kind = 2; dim = D.d; plane = D.gu.KB * Mp128; break;
+        case CC_TAP_A: src = L->W.a_act; kind = 2; dim = D.F; plane = D.dn.KB * Mp128; break;
         default: return fail(CC_ERR_INVALID, "unknown tap");
     }
     CC_CUDA(cudaSetDevice(L->ctx->device));
@@ -719,7 +745,7 @@ cc_status cc_debug_tap(cc_layer* L, cc_tap which, float* out_host, int batch) {
     const size_t bytes = (size_t)batch * dim * 4;
     CC_CUDA(cudaMalloc(&tmp, bytes));
     cudaError_t e = cudaMemset(tmp, 0, bytes);
-    if (e == cudaSuccess) e = cc_launch_tap(src, kind, dim, D, L->W, tmp, batch, 0);
+    if (e == cudaSuccess) e = cc_launch_tap(src, kind, dim, plane, D, L->W, tmp, batch, 0);
     if (e == cudaSuccess) e = cudaMemcpy(out_host, tmp, bytes, cudaMemcpyDeviceToHost);
     cudaFree(tmp);
     if (e != cudaSuccess) return fail(CC_ERR_CUDA, "cc_debug_tap: %s", cudaGetErrorString(e));

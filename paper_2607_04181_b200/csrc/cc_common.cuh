@@ -221,7 +221,9 @@ __device__ __forceinline__ uint64_t umma_desc_sw128(uint32_t smem_addr) {
     d |= (uint64_t)2 << 61;                          // SWIZZLE_128B   [61,64)
     return d;
 }
-// Instruction descriptor, kind::f16: D = fp32, A = B = bf16, both K-major, M = 128, N = n.
+// Instruction descriptor, kind::f16: D = fp32 (bits 4-5 = 1), A = B = bf16 (bits 7-9 = 10-12 = 1;
+// mixing bf16 with fp16 operands raises an illegal-instruction fault on sm_100a), both K-major,
+// N >> 3 at bit 17, M >> 4 at bit 24.
 __device__ __forceinline__ uint32_t umma_idesc_bf16_m128(uint32_t n) {
     return (1u << 4) | (1u << 7) | (1u << 10) | ((n >> 3) << 17) | ((128u >> 4) << 24);
 }

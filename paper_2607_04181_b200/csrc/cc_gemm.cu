@@ -5,8 +5,9 @@
 // around the weight stream, not around the MMA:
 //   * swap-AB: the packed weight tile (128 output features x 64 k, a 16 KiB pre-swizzled image
 //     made once at cc_create_layer) is the tcgen05 A operand (M = 128); the activations of one
-//     replica group (n rows, n = multiple of 16, <= 256) are the B operand (N = n).  The fp32
-//     accumulator D[128][n] lives in TMEM (n columns), double-buffered.
+//     replica group (n rows, n = multiple of 16, <= 256) are the B operand (N = n), held as two
+//     bf16 planes hi + lo that are both multiplied into the same accumulator (cc_rowwise.cu).
+//     The fp32 accumulator D[128][n] lives in TMEM (n columns), double-buffered.
 //   * one persistent CTA per SM, stream-K: the (tile, k-block) atoms are cut into P contiguous
 //     ranges fixed by the layer shape (cc_common.cuh); CTA i streams range i of EVERY active
 //     replica's blob, whose base it reads from the device replica table at run time
@@ -38,7 +39,7 @@ struct GemmSmemHdr {                      // lives at the start of dynamic smem
 };
 
 __global__ void __launch_bounds__(kGemmThreads, 1)
-k_gemm(CcGemmGeo G, const uint8_t* __restrict__ act, float* __restrict__ part, int Mpad,
+k_gemm(CcGemmGeo G, const uint8_t* __restrict__ act, int planes, float* __restrict__ part, int Mpad,
        const CcLayerTable* __restrict__ tab, const CcSched* __restrict__ sched) {
     extern __shared__ __align__(1024) uint8_t smem_raw[];
     GemmSmemHdr* H = reinterpret_cast<GemmSmemHdr*>(smem_raw);
@@ -70,7 +71,8 @@ k_gemm(CcGemmGeo G, const uint8_t* __restrict__ act, float* __restrict__ part, i
 
     const int nmax = sched->nmax;
     const uint32_t act_bytes_max = (uint32_t)((nmax * 128 + 1023) & ~1023);
-    const uint32_t stage_bytes = CC_A_TILE_BYTES + act_bytes_max;
+    const uint32_t stage_bytes = CC_A_TILE_BYTES + (uint32_t)planes * act_bytes_max;
+    const size_t plane_stride = (size_t)G.KB * Mpad * 128;   // bytes between the hi and lo operand planes
     uint8_t* stage0 = smem_raw + 1024;                      // header occupies the first KiB
     int n_stages = (kGemmSmem - 1024) / (int)stage_bytes;
     if (n_stages > kMaxStages) n_stages = kMaxStages;
@@ -95,9 +97,12 @@ k_gemm(CcGemmGeo G, const uint8_t* __restrict__ act, float* __restrict__ part, i
                         const int kb = (int)(a % G.KB);
                         mbar_wait(&H->empty[stage], ph ^ 1);
                         uint8_t* sW = stage0 + (size_t)stage * stage_bytes;
-                        mbar_expect_tx(&H->full[stage], CC_A_TILE_BYTES + n * 128);
+                        mbar_expect_tx(&H->full[stage], CC_A_TILE_BYTES + (uint32_t)planes * n * 128);
                         bulk_g2s_hint(sW, wsrc + (size_t)a * CC_A_TILE_BYTES, CC_A_TILE_BYTES, &H->full[stage], pol_w);
-                        bulk_g2s(sW + CC_A_TILE_BYTES, act + ((size_t)kb * Mpad + goff) * 128, n * 128, &H->full[stage]);
+                        const uint8_t* asrc = act + ((size_t)kb * Mpad + goff) * 128;
+                        for (int pl = 0; pl < planes; ++pl)
+                            bulk_g2s(sW + CC_A_TILE_BYTES + pl * act_bytes_max, asrc + pl * plane_stride, n * 128,
+                                     &H->full[stage]);
                         if (++stage == n_stages) { stage = 0; ph ^= 1; }
                     }
                 }
@@ -126,10 +131,13 @@ k_gemm(CcGemmGeo G, const uint8_t* __restrict__ act, float* __restrict__ part, i
                         tc_fence_after();
                         const uint32_t sW = smem_u32(stage0 + (size_t)stage * stage_bytes);
                         const uint64_t da = umma_desc_sw128(sW), db = umma_desc_sw128(sW + CC_A_TILE_BYTES);
+                        const uint64_t dlo = act_bytes_max >> 4;   // descriptor step from the hi to the lo plane
                         const uint32_t d_tmem = tmem_base + buf * 256;
 #pragma unroll
-                        for (int k = 0; k < CC_TILE_K / 16; ++k)
+                        for (int k = 0; k < CC_TILE_K / 16; ++k) {
                             umma_bf16(d_tmem, da + 2 * k, db + 2 * k, idesc, (first && k == 0) ? 0u : 1u);
+                            if (planes == 2) umma_bf16(d_tmem, da + 2 * k, db + dlo + 2 * k, idesc, 1u);
+                        }
                         umma_commit(&H->empty[stage]);
                         if (last) {
                             umma_commit(&H->tmem_full[buf]);
@@ -190,12 +198,13 @@ cudaError_t cc_launch_gemm(int which, const CcDims& D, const CcLayerTable* tab, 
     const CcGemmGeo* G;
     const uint8_t* act;
     float* part;
+    int planes = 2;   // hi + lo activation planes; the O projection's input needs one
     switch (which) {
         case 0: G = &D.qkv; act = W.x_act; part = W.qkv_part; break;
-        case 1: G = &D.o; act = W.o_act; part = W.o_part; break;
+        case 1: G = &D.o; act = W.o_act; part = W.o_part; planes = 1; break;
         case 2: G = &D.gu; act = W.y_act; part = W.gu_part; break;
         default: G = &D.dn; act = W.a_act; part = W.d_part; break;
     }
-    return cc_launch_kernel(k_gemm, dim3(G->P), dim3(kGemmThreads), (size_t)kGemmSmem, L, *G, act, part, D.Mpad, tab,
-                            W.sched);
+    return cc_launch_kernel(k_gemm, dim3(G->P), dim3(kGemmThreads), (size_t)kGemmSmem, L, *G, act, planes, part, D.Mpad,
+                            tab, W.sched);
 }

@@ -1,360 +1,13 @@
-// cc_kernels.cu -- the memory-bound kernels of the replicated decoder layer (sm_100a).
-//   k_group        a0   micro-batch grouping + attention work list (device-built, graph-safe)
-//   k_rmsnorm_in   a1   input RMSNorm -> packed bf16 GEMM operand
-//   k_rope_append  a3+a4  stream-K piece reduce of QKV, RoPE, KV append into the paged cache
-//   k_attn_combine a5   fixed-order merge of split-KV partials -> packed bf16 operand
-//   k_resid_norm   a6+a7  split-K reduce of O-proj + residual, RMSNorm -> packed operand
-//   k_swiglu       a8   split-K reduce of gate/up, silu(gate)*up -> packed operand
-//   k_final        a9   split-K reduce of down + residual, rows back in request order
-//   k_copy         a11  vectorised replica copy      k_publish  a12  replica-table flip
-//   k_pack              one-time re-pack of [out][in] weights into tcgen05 operand tile images
-// Every reduction order is a function of the layer shape only (never of the batch split), which
-// is what makes outputs bit-identical across replica counts.
+// cc_kernels.cu -- replica creation kernels (sm_100a):
+//   k_copy     a11  vectorised replica copy (256-bit accesses, streaming hints)
+//   k_publish  a12  replica-table flip
+//   k_pack          one-time re-pack of [out][in] weights into tcgen05 operand tile images
 #include "cc_kernels.h"
 
 namespace {
 
-constexpr int kRowThreads = 256;
-
-__device__ __forceinline__ int replica_of_pos(const CcSched* s, int pos) {
-    int r = 0;
-#pragma unroll
-    for (int i = 1; i < CC_MAXR; ++i)
-        if (s->cnt[i] > 0 && pos >= s->goff[i]) r = i;
-    return r;
-}
-
-// Sum of the stream-K partials of output column `col` for grouped row `pos`, pieces in
-// increasing order (a fixed order: the pieces of a tile depend on the layer shape only).
-__device__ __forceinline__ float reduce_pieces(const float* __restrict__ part, const CcGemmGeo& g, int Mpad, int pos,
-                                               int col) {
-    const int t = col >> 7, f = col & 127;
-    int p0, p1;
-    cc_tile_pieces(g, t, p0, p1);
-    float acc = 0.f;
-    for (int p = p0; p <= p1; ++p) acc += part[((size_t)p * Mpad + pos) * 128 + f];
-    return acc;
-}
-
-__device__ __forceinline__ float block_sum(float v, float* red) {
-#pragma unroll
-    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
-    int w = threadIdx.x >> 5, l = threadIdx.x & 31;
-    __syncthreads();
-    if (l == 0) red[w] = v;
-    __syncthreads();
-    float t = 0.f;
-    int nw = blockDim.x >> 5;
-    for (int i = 0; i < nw; ++i) t += red[i];   // same order in every thread
-    return t;
-}
-
 // ---------------------------------------------------------------------------------------------
-// a0: grouping.  One block; thread b owns row b.  Stable partition by replica,
-// groups start at multiples of 16 rows; builds the split-KV work list (pos, chunk).
-// ---------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(256) k_group(const int* __restrict__ assign, const int* __restrict__ seq_lens,
-                                               int batch, CcDims D, const CcLayerTable* __restrict__ tab, CcWork W) {
-    __shared__ int s_rep[256], s_nch[256], s_pos[256], s_cnt[CC_MAXR], s_goff[CC_MAXR + 1];
-    const int b = threadIdx.x;
-    pdl_launch_dependents();
-    pdl_wait();
-    const uint32_t mask = tab->active_mask;
-    int rep = -1, nch = 0;
-    if (b < batch) {
-        int s = seq_lens[b];
-        if (s > 0) {
-            if (s > D.max_position || (s + CC_PAGE - 1) / CC_PAGE > D.max_blocks) {
-                atomicOr(W.err, CC_DEVERR_BAD_SEQLEN);
-            } else {
-                rep = assign[b];
-                if (rep < 0 || rep >= CC_MAXR || !((mask >> rep) & 1u)) {
-                    atomicOr(W.err, CC_DEVERR_BAD_REPLICA);
-                    rep = 0;
-                }
-                nch = (s + CC_ATTN_CHUNK - 1) / CC_ATTN_CHUNK;
-            }
-        }
-    }
-    s_rep[b] = rep;
-    s_nch[b] = nch;
-    for (int i = b; i < D.Mpad; i += blockDim.x) W.perm[i] = -1;
-    __syncthreads();
-    if (b < CC_MAXR) {
-        int c = 0;
-        for (int i = 0; i < batch; ++i) c += (s_rep[i] == b);
-        s_cnt[b] = c;
-    }
-    __syncthreads();
-    if (b == 0) {
-        int off = 0;
-        for (int r = 0; r < CC_MAXR; ++r) {
-            s_goff[r] = off;
-            off += (s_cnt[r] + CC_ROW_ALIGN - 1) / CC_ROW_ALIGN * CC_ROW_ALIGN;
-        }
-        s_goff[CC_MAXR] = off;
-    }
-    __syncthreads();
-    int pos = -1;
-    if (rep >= 0) {
-        int rank = 0;
-        for (int i = 0; i < b; ++i) rank += (s_rep[i] == rep);
-        pos = s_goff[rep] + rank;
-        W.perm[pos] = b;
-    }
-    s_pos[b] = pos;
-    __syncthreads();
-    int total = 0, mine = 0;
-    for (int i = 0; i < batch; ++i) {
-        int p = s_pos[i];
-        if (p >= 0) {
-            total += s_nch[i];
-            if (pos >= 0 && p < pos) mine += s_nch[i];
-        }
-    }
-    if (pos >= 0)
-        for (int c = 0; c < nch; ++c) W.items[mine + c] = make_int2(pos, c);
-    if (b == 0) {
-        for (int r = 0; r < CC_MAXR; ++r) {
-            W.sched->cnt[r] = s_cnt[r];
-            W.sched->goff[r] = s_goff[r];
-        }
-        int nmax = 0;
-        for (int r = 0; r < CC_MAXR; ++r) nmax = max(nmax, (s_cnt[r] + CC_ROW_ALIGN - 1) / CC_ROW_ALIGN * CC_ROW_ALIGN);
-        W.sched->n_pos = s_goff[CC_MAXR];
-        W.sched->n_items = total;
-        W.sched->nmax = nmax;
-    }
-}
-
-// ---------------------------------------------------------------------------------------------
-// a1: x = h * rsqrt(mean(h^2) + eps) * g1  ->  packed bf16 operand.  One block per position.
-// ---------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(kRowThreads) k_rmsnorm_in(const __nv_bfloat16* __restrict__ hidden, CcDims D,
-                                                            const CcLayerTable* __restrict__ tab, CcWork W) {
-    __shared__ float red[kRowThreads / 32];
-    const int pos = blockIdx.x;
-    pdl_launch_dependents();
-    pdl_wait();
-    if (pos >= W.sched->n_pos) return;
-    const int b = W.perm[pos];
-    if (b < 0) return;
-    const int r = replica_of_pos(W.sched, pos);
-    const uint4* g = reinterpret_cast<const uint4*>(tab->rep[r].blob + D.off_g1);
-    const uint4* row = reinterpret_cast<const uint4*>(hidden + (size_t)b * D.d);
-    const int nchunk = D.d >> 3;
-    float ss = 0.f;
-    for (int c = threadIdx.x; c < nchunk; c += kRowThreads) {
-        uint4 v = row[c];
-        uint32_t w[4] = {v.x, v.y, v.z, v.w};
-#pragma unroll
-        for (int i = 0; i < 4; ++i) {
-            float a = bf16lo(w[i]), bb = bf16hi(w[i]);
-            ss += a * a + bb * bb;
-        }
-    }
-    ss = block_sum(ss, red);
-    const float inv = rsqrtf(ss / (float)D.d + D.eps);
-    for (int c = threadIdx.x; c < nchunk; c += kRowThreads) {
-        uint4 v = row[c], gv = g[c];
-        uint32_t w[4] = {v.x, v.y, v.z, v.w}, gw[4] = {gv.x, gv.y, gv.z, gv.w}, o[4];
-#pragma unroll
-        for (int i = 0; i < 4; ++i)
-            o[i] = pack_bf16(bf16lo(w[i]) * inv * bf16lo(gw[i]), bf16hi(w[i]) * inv * bf16hi(gw[i]));
-        *reinterpret_cast<uint4*>(W.x_act + act_chunk_off(pos, c << 3, D.Mpad)) = make_uint4(o[0], o[1], o[2], o[3]);
-    }
-}
-
-// ---------------------------------------------------------------------------------------------
-// a3 + a4: reduce the QKV split-K partials (fixed order), rotate q and k at position s-1
-// (rotate-half pairs (i, i+Dh/2), cos/sin from the fp64-built table), keep q in fp32, store
-// bf16(k), bf16(v) into the page slot of position s-1 (PAPER.md:103 local append).
-// ---------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(kRowThreads) k_rope_append(const int* __restrict__ seq_lens, CcKv kv, CcDims D,
-                                                             CcWork W) {
-    const int pos = blockIdx.x;
-    pdl_launch_dependents();
-    pdl_wait();
-    if (pos >= W.sched->n_pos) return;
-    const int b = W.perm[pos];
-    if (b < 0) return;
-    const int s = seq_lens[b], p = s - 1;
-    const int half = D.Dh >> 1;
-    const float2* cs = W.rope_cs + (size_t)p * half;
-    int page = kv.block_table[(size_t)b * D.max_blocks + p / CC_PAGE];
-    const bool page_ok = page >= 0 && page < kv.n_pages;
-    if (!page_ok && threadIdx.x == 0) atomicOr(W.err, CC_DEVERR_BAD_PAGE);
-    const int slot = p % CC_PAGE;
-    // q and k pairs
-    const int n_rot = (D.Hq + D.Hkv) * half;
-    for (int idx = threadIdx.x; idx < n_rot; idx += kRowThreads) {
-        const int h = idx / half, i = idx - h * half;
-        const int col = h * D.Dh + i;   // q heads then k heads are contiguous in the QKV output
-        const float a = reduce_pieces(W.qkv_part, D.qkv, D.Mpad, pos, col);
-        const float bb = reduce_pieces(W.qkv_part, D.qkv, D.Mpad, pos, col + half);
-        const float2 c = cs[i];
-        const float ra = a * c.x - bb * c.y, rb = bb * c.x + a * c.y;
-        if (h < D.Hq) {
-            W.q_rot[(size_t)pos * D.QD + col] = ra;
-            W.q_rot[(size_t)pos * D.QD + col + half] = rb;
-        } else if (page_ok) {
-            const int hk = h - D.Hq;
-            __nv_bfloat16* dst = kv.k_pool + (((size_t)page * D.Hkv + hk) * CC_PAGE + slot) * D.Dh;
-            dst[i] = __float2bfloat16_rn(ra);
-            dst[i + half] = __float2bfloat16_rn(rb);
-        }
-    }
-    if (page_ok) {
-        for (int idx = threadIdx.x; idx < D.KD; idx += kRowThreads) {
-            const int col = D.QD + D.KD + idx;
-            const float a = reduce_pieces(W.qkv_part, D.qkv, D.Mpad, pos, col);
-            const int hk = idx / D.Dh, i = idx - hk * D.Dh;
-            kv.v_pool[(((size_t)page * D.Hkv + hk) * CC_PAGE + slot) * D.Dh + i] = __float2bfloat16_rn(a);
-        }
-    }
-}
-
-// ---------------------------------------------------------------------------------------------
-// a5 (second half): merge the split-KV partials of one row in chunk order -> bf16 operand.
-// The number of chunks depends on seq_len only.
-// ---------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(kRowThreads) k_attn_combine(const int* __restrict__ seq_lens, CcDims D, CcWork W) {
-    const int pos = blockIdx.x;
-    pdl_launch_dependents();
-    pdl_wait();
-    if (pos >= W.sched->n_pos) return;
-    const int b = W.perm[pos];
-    if (b < 0) return;
-    const int nch = (seq_lens[b] + CC_ATTN_CHUNK - 1) / CC_ATTN_CHUNK;
-    for (int idx = threadIdx.x; idx < D.QD / 2; idx += kRowThreads) {
-        const int e = idx * 2, hq = e / D.Dh, dim = e - hq * D.Dh;
-        const size_t row = ((size_t)pos * D.Hq + hq) * W.nch_max;
-        float M = -INFINITY;
-        for (int c = 0; c < nch; ++c) M = fmaxf(M, W.att_ml[row + c].x);
-        float L = 0.f, a0 = 0.f, a1 = 0.f;
-        for (int c = 0; c < nch; ++c) {
-            const float2 ml = W.att_ml[row + c];
-            const float w = exp2f(ml.x - M);
-            const float2 o = *reinterpret_cast<const float2*>(W.att_o + (row + c) * D.Dh + dim);
-            L += w * ml.y;
-            a0 += w * o.x;
-            a1 += w * o.y;
-        }
-        const float inv = 1.f / L;
-        uint8_t* dst = W.o_act + act_chunk_off(pos, e, D.Mpad) + (e & 7) * 2;
-        *reinterpret_cast<uint32_t*>(dst) = pack_bf16(a0 * inv, a1 * inv);
-    }
-}
-
-// ---------------------------------------------------------------------------------------------
-// a6 (reduce + residual) and a7 (RMSNorm): h1 = h + sum_s part_s ; y = rmsnorm(h1) * g2.
-// ---------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(kRowThreads) k_resid_norm(const __nv_bfloat16* __restrict__ hidden, CcDims D,
-                                                            const CcLayerTable* __restrict__ tab, CcWork W) {
-    extern __shared__ float s_row[];
-    __shared__ float red[kRowThreads / 32];
-    const int pos = blockIdx.x;
-    pdl_launch_dependents();
-    pdl_wait();
-    if (pos >= W.sched->n_pos) return;
-    const int b = W.perm[pos];
-    if (b < 0) return;
-    const int r = replica_of_pos(W.sched, pos);
-    const __nv_bfloat16* g = reinterpret_cast<const __nv_bfloat16*>(tab->rep[r].blob + D.off_g2);
-    float ss = 0.f;
-    for (int i = threadIdx.x; i < D.d; i += kRowThreads) {
-        const float acc = reduce_pieces(W.o_part, D.o, D.Mpad, pos, i);
-        const float v = __bfloat162float(hidden[(size_t)b * D.d + i]) + acc;
-        s_row[i] = v;
-        W.h1[(size_t)pos * D.d + i] = v;
-        ss += v * v;
-    }
-    ss = block_sum(ss, red);
-    const float inv = rsqrtf(ss / (float)D.d + D.eps);
-    for (int c = threadIdx.x; c < (D.d >> 3); c += kRowThreads) {
-        uint32_t o[4];
-#pragma unroll
-        for (int i = 0; i < 4; ++i) {
-            const int k = (c << 3) + 2 * i;
-            o[i] = pack_bf16(s_row[k] * inv * __bfloat162float(g[k]), s_row[k + 1] * inv * __bfloat162float(g[k + 1]));
-        }
-        *reinterpret_cast<uint4*>(W.y_act + act_chunk_off(pos, c << 3, D.Mpad)) = make_uint4(o[0], o[1], o[2], o[3]);
-    }
-}
-
-// ---------------------------------------------------------------------------------------------
-// a8: a_j = silu(gate_j) * up_j with gate_j, up_j at interleaved columns 2j, 2j+1 of the
-// gate/up GEMM output (split-K partials reduced here in fixed order).
-// ---------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(kRowThreads) k_swiglu(CcDims D, CcWork W) {
-    const int pos = blockIdx.y;
-    pdl_launch_dependents();
-    pdl_wait();
-    if (pos >= W.sched->n_pos) return;
-    if (W.perm[pos] < 0) return;
-    const int c = blockIdx.x * kRowThreads + threadIdx.x;   // 16-byte chunk of 8 outputs = 16 GEMM columns
-    const int fpad = D.gu.T * 64;                           // padded SwiGLU width
-    if (c * 8 >= fpad) return;
-    const int col0 = c * 16, t = col0 >> 7, f0 = col0 & 127;
-    int p0, p1;
-    cc_tile_pieces(D.gu, t, p0, p1);
-    float v[16];
-#pragma unroll
-    for (int i = 0; i < 16; ++i) v[i] = 0.f;
-    for (int p = p0; p <= p1; ++p) {
-        const float4* p4 = reinterpret_cast<const float4*>(W.gu_part + ((size_t)p * D.Mpad + pos) * 128 + f0);
-#pragma unroll
-        for (int i = 0; i < 4; ++i) {
-            const float4 q = p4[i];
-            v[4 * i] += q.x; v[4 * i + 1] += q.y; v[4 * i + 2] += q.z; v[4 * i + 3] += q.w;
-        }
-    }
-    uint32_t o[4];
-#pragma unroll
-    for (int i = 0; i < 4; ++i) {
-        const float g0 = v[4 * i], u0 = v[4 * i + 1], g1 = v[4 * i + 2], u1 = v[4 * i + 3];
-        const float a0 = g0 / (1.f + __expf(-g0)) * u0;
-        const float a1 = g1 / (1.f + __expf(-g1)) * u1;
-        o[i] = pack_bf16(a0, a1);
-    }
-    *reinterpret_cast<uint4*>(W.a_act + act_chunk_off(pos, c << 3, D.Mpad)) = make_uint4(o[0], o[1], o[2], o[3]);
-}
-
-// ---------------------------------------------------------------------------------------------
-// a9 (reduce + residual): out[b] = bf16(h1 + sum of pieces), written to row b = original order
-// (PAPER.md:101 gather + concat along batch).
-// ---------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(kRowThreads) k_final(__nv_bfloat16* __restrict__ hidden, CcDims D, CcWork W) {
-    const int pos = blockIdx.y;
-    pdl_launch_dependents();
-    pdl_wait();
-    if (pos >= W.sched->n_pos) return;
-    const int b = W.perm[pos];
-    if (b < 0) return;
-    const int c = blockIdx.x * kRowThreads + threadIdx.x;
-    if (c * 8 >= D.d) return;
-    const int col0 = c * 8, t = col0 >> 7, f0 = col0 & 127;
-    int p0, p1;
-    cc_tile_pieces(D.dn, t, p0, p1);
-    const float4* h4 = reinterpret_cast<const float4*>(W.h1 + (size_t)pos * D.d + col0);
-    float4 x0 = h4[0], x1 = h4[1];
-    float v[8] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
-    for (int p = p0; p <= p1; ++p) {
-        const float4* p4 = reinterpret_cast<const float4*>(W.d_part + ((size_t)p * D.Mpad + pos) * 128 + f0);
-        const float4 t0 = p4[0], t1 = p4[1];
-        v[0] += t0.x; v[1] += t0.y; v[2] += t0.z; v[3] += t0.w;
-        v[4] += t1.x; v[5] += t1.y; v[6] += t1.z; v[7] += t1.w;
-    }
-    uint4 o;
-    o.x = pack_bf16(x0.x + v[0], x0.y + v[1]);
-    o.y = pack_bf16(x0.z + v[2], x0.w + v[3]);
-    o.z = pack_bf16(x1.x + v[4], x1.y + v[5]);
-    o.w = pack_bf16(x1.z + v[6], x1.w + v[7]);
-    *reinterpret_cast<uint4*>(hidden + (size_t)b * D.d + col0) = o;
-}
-
-// ---------------------------------------------------------------------------------------------
-// a11: vectorised copy, 8 x 16 B in flight per thread, streaming cache hints.
+// a11: vectorised copy, 4 x 32 B in flight per thread, streaming cache hints.
 // ---------------------------------------------------------------------------------------------
 constexpr int kCopyThreads = 512;
 constexpr int kCopyUnroll = 4;
@@ -427,61 +80,8 @@ __global__ void __launch_bounds__(256) k_pack(uint8_t* __restrict__ dst, const _
     }
 }
 
-// Test tap: widen a workspace buffer to fp32 [batch][dim] in original row order.
-__global__ void __launch_bounds__(256) k_tap(const void* __restrict__ src, int which, int dim, CcDims D, CcWork W,
-                                             float* __restrict__ out, int batch) {
-    const int pos = blockIdx.x;
-    if (pos >= W.sched->n_pos) return;
-    const int b = W.perm[pos];
-    if (b < 0 || b >= batch) return;
-    for (int k = threadIdx.x; k < dim; k += blockDim.x) {
-        float v;
-        if (which == 0) {
-            const uint8_t* p = reinterpret_cast<const uint8_t*>(src) + act_chunk_off(pos, k, D.Mpad) + (k & 7) * 2;
-            v = __bfloat162float(*reinterpret_cast<const __nv_bfloat16*>(p));
-        } else {
-            v = reinterpret_cast<const float*>(src)[(size_t)pos * dim + k];
-        }
-        out[(size_t)b * dim + k] = v;
-    }
-}
-
 }  // namespace
 
-// ---- launchers ---------------------------------------------------------------------------------
-cudaError_t cc_launch_group(const int* assign, const int* seq_lens, int batch, const CcDims& D,
-                            const CcLayerTable* tab, const CcWork& W, const CcLaunch& L) {
-    return cc_launch_kernel(k_group, dim3(1), dim3(256), 0, L, assign, seq_lens, batch, D, tab, W);
-}
-cudaError_t cc_launch_rmsnorm_in(const __nv_bfloat16* hidden, const CcDims& D, const CcLayerTable* tab,
-                                 const CcWork& W, const CcLaunch& L) {
-    return cc_launch_kernel(k_rmsnorm_in, dim3(D.Mpad), dim3(kRowThreads), 0, L, hidden, D, tab, W);
-}
-cudaError_t cc_launch_rope_append(const int* seq_lens, const CcKv& kv, const CcDims& D, const CcWork& W,
-                                  const CcLaunch& L) {
-    return cc_launch_kernel(k_rope_append, dim3(D.Mpad), dim3(kRowThreads), 0, L, seq_lens, kv, D, W);
-}
-cudaError_t cc_launch_attn_combine(const int* seq_lens, const CcDims& D, const CcWork& W, const CcLaunch& L) {
-    return cc_launch_kernel(k_attn_combine, dim3(D.Mpad), dim3(kRowThreads), 0, L, seq_lens, D, W);
-}
-cudaError_t cc_launch_resid_norm(const __nv_bfloat16* hidden, const CcDims& D, const CcLayerTable* tab,
-                                 const CcWork& W, const CcLaunch& L) {
-    return cc_launch_kernel(k_resid_norm, dim3(D.Mpad), dim3(kRowThreads), (size_t)D.d * sizeof(float), L, hidden, D,
-                            tab, W);
-}
-cudaError_t cc_launch_swiglu(const CcDims& D, const CcWork& W, const CcLaunch& L) {
-    const int chunks = (D.gu.T * 64) / 8;
-    dim3 grid((chunks + kRowThreads - 1) / kRowThreads, D.Mpad);
-    return cc_launch_kernel(k_swiglu, grid, dim3(kRowThreads), 0, L, D, W);
-}
-cudaError_t cc_launch_final(__nv_bfloat16* hidden, const CcDims& D, const CcWork& W, const CcLaunch& L) {
-    const int chunks = D.d / 8;
-    dim3 grid((chunks + kRowThreads - 1) / kRowThreads, D.Mpad);
-    return cc_launch_kernel(k_final, grid, dim3(kRowThreads), 0, L, hidden, D, W);
-}
-cudaError_t cc_rowwise_configure(int max_d) {
-    return cudaFuncSetAttribute(k_resid_norm, cudaFuncAttributeMaxDynamicSharedMemorySize, 96 * 1024);
-}
 cudaError_t cc_launch_copy(void* dst, const void* src, size_t bytes, int n_sms, cudaStream_t st) {
     if (bytes == 0) return cudaSuccess;
     if (((((uintptr_t)dst) | ((uintptr_t)src)) & 31) || (bytes & 15)) return cudaErrorInvalidValue;
@@ -504,10 +104,5 @@ cudaError_t cc_launch_pack(uint8_t* dst, const __nv_bfloat16* src0, const __nv_b
                            const __nv_bfloat16* src2, int rows0, int rows1, int rows2, int mode, int K, int n_tiles,
                            int k_blocks, cudaStream_t st) {
     k_pack<<<1184, 256, 0, st>>>(dst, src0, src1, src2, rows0, rows1, rows2, mode, K, n_tiles, k_blocks);
-    return cudaGetLastError();
-}
-cudaError_t cc_launch_tap(const void* src, int which, int dim, const CcDims& D, const CcWork& W, float* out_dev,
-                          int batch, cudaStream_t st) {
-    k_tap<<<D.Mpad, 256, 0, st>>>(src, which, dim, D, W, out_dev, batch);
     return cudaGetLastError();
 }

@@ -7,8 +7,8 @@ struct CcWork {
     CcSched* sched;
     int* perm;           // [Mpad] original row at grouped position, or -1
     int2* items;         // attention work items (pos, chunk), at most max_batch * nch_max
-    uint8_t* x_act;      // packed bf16 GEMM operands, [K/64][Mpad][128 B swizzled]
-    uint8_t* o_act;
+    uint8_t* x_act;      // packed bf16 GEMM operands, [plane hi|lo][K/64][Mpad][128 B swizzled]
+    uint8_t* o_act;      // (one plane)
     uint8_t* y_act;
     uint8_t* a_act;
     float* qkv_part;     // stream-K partial sums, [P + T][Mpad][128] fp32 (piece-major)
@@ -38,7 +38,6 @@ struct CcLaunch {
     bool pdl;            // programmatic dependent launch between the kernels of the chain
 };
 
-cudaError_t cc_kernels_configure();   // sets max dynamic smem attributes once per process/device
 
 cudaError_t cc_launch_group(const int* assign, const int* seq_lens, int batch, const CcDims& D,
                             const CcLayerTable* tab, const CcWork& W, const CcLaunch& L);
@@ -62,9 +61,10 @@ cudaError_t cc_launch_publish(CcLayerTable* row_dev, const CcLayerTable& value, 
 cudaError_t cc_launch_pack(uint8_t* dst, const __nv_bfloat16* src0, const __nv_bfloat16* src1,
                            const __nv_bfloat16* src2, int rows0, int rows1, int rows2, int mode, int K, int n_tiles,
                            int k_blocks, cudaStream_t st);
-// which: 0 = packed act buffer (bf16, K = dim), 1 = fp32 row buffer [Mpad][dim]
-cudaError_t cc_launch_tap(const void* src, int which, int dim, const CcDims& D, const CcWork& W, float* out_dev,
-                          int batch, cudaStream_t st);
+// which: 0 = one packed bf16 plane (K = dim), 1 = fp32 row buffer [Mpad][dim], 2 = hi + lo planes
+cudaError_t cc_launch_tap(const void* src, int which, int dim, size_t plane, const CcDims& D, const CcWork& W,
+                          float* out_dev, int batch, cudaStream_t st);
+int cc_max_hidden();
 
 // Generic launcher: plain <<<>>> semantics, plus the PDL attribute when asked for.
 template <typename... KArgs, typename... Args>

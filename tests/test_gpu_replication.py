@@ -1,0 +1,252 @@
+"""GPU tests of the replication mechanics: bit-identity across replica counts, the
+byte-exact chunked replica copy, one CUDA graph surviving scale-up and
+scale-down without recapture (north_star; the paper re-captures), the two-phase
+publish / retire state machine and the sticky device error word."""
+import numpy as np
+import pytest
+import torch
+
+import oracle
+from paper_2607_04181_b200 import inputs as I
+
+pytestmark = pytest.mark.gpu
+
+MID = I.LayerShape("mid", 512, 8, 2, 128, 1408, 1e-5, 500000.0, 21, 200, 700)
+
+
+def _binding():
+    from paper_2607_04181_b200 import binding as B
+    from paper_2607_04181_b200.harness import DeviceStep, Session
+    return B, DeviceStep, Session
+
+
+def _read_device(ptr: int, nbytes: int) -> np.ndarray:
+    """Raw device memory -> host bytes (torch has no public raw-pointer tensor; use cudart)."""
+    out = np.empty(nbytes, dtype=np.uint8)
+    from cuda.bindings import runtime as cudart  # cuda-python, in the image
+    (err,) = cudart.cudaMemcpy(out.ctypes.data, ptr, nbytes, cudart.cudaMemcpyKind.cudaMemcpyDeviceToHost)
+    assert int(err) == 0, err
+    return out
+
+
+@pytest.mark.parametrize("shape,batch,seeds", [(I.CFG1, 4, (1001, 2001, 3001)), (MID, 21, (1007, 2007, 3007))])
+def test_bit_identical_across_replica_counts_and_assignments(shape, batch, seeds):
+    B, DeviceStep, Session = _binding()
+    w = I.make_weights(shape, seeds[0])
+    st = I.make_step_inputs(shape, seeds[1], seeds[2], batch=batch)
+    rng = np.random.default_rng(5)
+    with Session(shape, w, max_batch=batch) as S:
+        step = DeviceStep(st, np.zeros(batch, np.int32))
+        S.forward(step)
+        torch.cuda.synchronize()
+        base_out, (base_k, base_v) = step.out_bits(), step.pools_bits()
+        S.scale(4)
+        cases = [I.even_split(batch, 2), I.even_split(batch, 4), rng.integers(0, 4, batch).astype(np.int32),
+                 np.full(batch, 3, np.int32), (np.arange(batch) % 3).astype(np.int32)]
+        for assign in cases:
+            step.reset(st)
+            step.set_assign(assign)
+            S.forward(step)
+            torch.cuda.synchronize()
+            assert B.cc_poll_device_error(S.ctx) == 0
+            k, v = step.pools_bits()
+            assert np.array_equal(step.out_bits(), base_out), f"outputs differ for assignment {assign}"
+            assert np.array_equal(k, base_k) and np.array_equal(v, base_v)
+
+
+def test_replica_copy_is_byte_exact_and_stays_inside_its_slot():
+    B, DeviceStep, Session = _binding()
+    shape = I.CFG1
+    w = I.make_weights(shape, 1001)
+    with Session(shape, w, max_batch=4) as S:
+        S.arena.fill_(0xA5)                                       # guard pattern over the whole donated range
+        torch.cuda.synchronize()
+        B.cc_ctx_set_copy_chunk(S.ctx, 1 << 20)                   # several chunks per blob (blob ~1.4 MiB)
+        S.scale(4)
+        torch.cuda.synchronize()
+        assert B.cc_query(S.layer) == (4, 0)
+        p0, n0 = B.cc_replica_blob(S.layer, 0)
+        src = _read_device(p0, n0)
+        want = oracle.replica_copy(src)                           # the oracle's definition: memcpy
+        arena = S.arena.cpu().numpy()
+        base = S.arena.data_ptr()
+        covered = np.zeros(arena.shape[0], dtype=bool)
+        for r in (1, 2, 3):
+            p, n = B.cc_replica_blob(S.layer, r)
+            assert n == n0 and p % 1024 == 0
+            off = p - base
+            assert np.array_equal(arena[off:off + n], want), f"replica {r} differs from slot 0"
+            covered[off:off + n] = True
+        assert (arena[~covered] == 0xA5).all(), "bytes outside the slots were touched"
+
+
+@pytest.mark.parametrize("nbytes", [16, 48, 4096, 1 << 20, (1 << 20) + 16, 3 * (1 << 20) + 4080])
+def test_copy_kernel_ragged_sizes(nbytes):
+    B, _, _ = _binding()
+    ctx = B.cc_ctx_create(0)
+    try:
+        g = torch.Generator(device="cpu").manual_seed(nbytes)
+        src = torch.randint(0, 256, (nbytes + 64,), dtype=torch.uint8, generator=g).cuda()
+        dst = torch.full((nbytes + 64,), 0x5A, dtype=torch.uint8, device="cuda")
+        B.cc_replica_copy(ctx, dst[32:], src[32:], nbytes, 1 << 20, torch.cuda.current_stream())
+        torch.cuda.synchronize()
+        d, s = dst.cpu().numpy(), src.cpu().numpy()
+        assert np.array_equal(d[32:32 + nbytes], oracle.replica_copy(s[32:32 + nbytes]))
+        assert (d[:32] == 0x5A).all() and (d[32 + nbytes:] == 0x5A).all()
+        with pytest.raises(B.CcError):
+            B.cc_replica_copy(ctx, dst[16:], src[32:], 32, 0, None)            # dst not 32-byte aligned
+    finally:
+        B.cc_ctx_destroy(ctx)
+
+
+def test_one_graph_survives_scale_up_and_down_without_recapture():
+    B, DeviceStep, Session = _binding()
+    shape, batch = MID, 21
+    w = I.make_weights(shape, 1007)
+    st = I.make_step_inputs(shape, 2007, 3007, batch=batch)
+    with Session(shape, w, max_batch=batch) as S:
+        step = DeviceStep(st, np.zeros(batch, np.int32))
+        S.forward(step)                                            # warm-up outside capture
+        torch.cuda.synchronize()
+        base = step.out_bits()
+        graph = torch.cuda.CUDAGraph()
+        captures = 0
+        step.reset(st)
+        with torch.cuda.graph(graph):
+            S.forward(step, torch.cuda.current_stream())
+        captures += 1
+        exec_id = id(graph)
+
+        def replay(assign):
+            step.reset(st)
+            step.set_assign(assign)
+            graph.replay()
+            torch.cuda.synchronize()
+            assert B.cc_poll_device_error(S.ctx) == 0
+            return step.out_bits()
+
+        assert np.array_equal(replay(np.zeros(batch, np.int32)), base)
+        # scale up: copy on the side stream, publish on the replay stream; same graph, no recapture
+        S.scale(2)
+        assert B.cc_query(S.layer) == (2, 0)
+        two = I.even_split(batch, 2)
+        assert np.array_equal(replay(two), base)
+        # prove the replayed graph really reads replica 1's slot through the table: corrupt that slot
+        p1, n1 = B.cc_replica_blob(S.layer, 1)
+        off = p1 - S.arena.data_ptr()
+        saved = S.arena[off:off + n1].clone()
+        S.arena[off:off + n1].zero_()
+        out = replay(two)
+        assert np.array_equal(out[two == 0], base[two == 0])
+        assert not np.array_equal(out[two == 1], base[two == 1])
+        S.arena[off:off + n1].copy_(saved)
+        assert np.array_equal(replay(two), base)
+        # scale down: retire the row first, then the slot returns to the allocator
+        S.scale(1)
+        assert B.cc_query(S.layer) == (1, 0)
+        assert np.array_equal(replay(np.zeros(batch, np.int32)), base)
+        # a row still naming the retired replica is served by replica 0 and flagged, never a fault
+        step.reset(st)
+        step.set_assign(two)
+        graph.replay()
+        torch.cuda.synchronize()
+        assert B.cc_poll_device_error(S.ctx) == B.CC_DEVERR_BAD_REPLICA
+        assert np.array_equal(step.out_bits(), base)
+        assert captures == 1 and id(graph) == exec_id
+
+
+def test_two_phase_publish_and_slot_reuse():
+    B, DeviceStep, Session = _binding()
+    shape = I.CFG1
+    w = I.make_weights(shape, 1001)
+    with Session(shape, w, max_batch=4, n_slots=2) as S:
+        B.cc_scale_layer(S.layer, 3)
+        assert B.cc_query(S.layer) == (1, 2)                        # copies enqueued, nothing visible yet
+        B.cc_commit(S.layer, torch.cuda.current_stream())
+        assert B.cc_query(S.layer) == (3, 0)
+        with pytest.raises(B.CcError) as e:
+            B.cc_scale_layer(S.layer, 4)                           # only two slots were donated
+        assert e.value.status == B.CC_ERR_NO_SLOT
+        assert B.cc_query(S.layer) == (3, 0)
+        with pytest.raises(B.CcError) as e:
+            B.cc_release_replica(S.layer, 0)
+        assert e.value.status == B.CC_ERR_STATE
+        p1, _ = B.cc_replica_blob(S.layer, 1)
+        B.cc_release_replica(S.layer, 1)
+        with pytest.raises(B.CcError) as e:
+            B.cc_release_replica(S.layer, 1)                       # already retiring
+        assert e.value.status == B.CC_ERR_STATE
+        with pytest.raises(B.CcError) as e:
+            B.cc_ctx_reclaim(S.ctx, S.arena)                       # live slots inside
+        assert e.value.status == B.CC_ERR_BUSY
+        B.cc_commit(S.layer, torch.cuda.current_stream())
+        assert B.cc_query(S.layer) == (2, 0)
+        torch.cuda.synchronize()
+        S.scale(3)                                                 # the freed (lowest) slot is reused
+        q1, _ = B.cc_replica_blob(S.layer, 1)
+        assert q1 == p1
+        # outputs with the re-created replica are still those of the unreplicated layer
+        st = I.make_step_inputs(shape, 2001, 3001)
+        step = DeviceStep(st, np.zeros(4, np.int32))
+        S.forward(step)
+        torch.cuda.synchronize()
+        base = step.out_bits()
+        step.reset(st)
+        step.set_assign(np.array([1, 1, 2, 0], np.int32))
+        S.forward(step)
+        torch.cuda.synchronize()
+        assert np.array_equal(step.out_bits(), base)
+
+
+def test_device_error_word_and_bad_rows():
+    B, DeviceStep, Session = _binding()
+    shape = I.CFG1
+    w = I.make_weights(shape, 1001)
+    st = I.make_step_inputs(shape, 2001, 3001)
+    with Session(shape, w, max_batch=4) as S:
+        step = DeviceStep(st, np.zeros(4, np.int32))
+        S.forward(step)
+        torch.cuda.synchronize()
+        base = step.out_bits()
+        # seq_len beyond what the block table can address: row skipped, flagged
+        bad = st.clone()
+        bad.seq_lens[2] = shape.max_blocks * shape.page + 5
+        step2 = DeviceStep(bad, np.zeros(4, np.int32))
+        S.forward(step2)
+        torch.cuda.synchronize()
+        assert B.cc_poll_device_error(S.ctx) & B.CC_DEVERR_BAD_SEQLEN
+        out = step2.out_bits()
+        assert np.array_equal(out[2], st.hidden[2])
+        assert np.array_equal(out[[0, 1, 3]], base[[0, 1, 3]])
+        # a block-table entry of -1 below seq_len: flagged, no fault
+        bad = st.clone()
+        bad.block_table[1, 0] = -1
+        step3 = DeviceStep(bad, np.zeros(4, np.int32))
+        S.forward(step3)
+        torch.cuda.synchronize()
+        assert B.cc_poll_device_error(S.ctx) & B.CC_DEVERR_BAD_PAGE
+        assert np.array_equal(step3.out_bits()[[0, 2, 3]], base[[0, 2, 3]])
+        assert B.cc_poll_device_error(S.ctx) == 0                  # reading clears
+
+
+def test_forward_host_matches_forward():
+    B, DeviceStep, Session = _binding()
+    shape = I.CFG1
+    w = I.make_weights(shape, 1001)
+    st = I.make_step_inputs(shape, 2001, 3001)
+    assign = I.even_split(4, 2)
+    with Session(shape, w, max_batch=4) as S:
+        S.scale(2)
+        step = DeviceStep(st, assign)
+        S.forward(step)
+        torch.cuda.synchronize()
+        want = step.out_bits()
+        step.reset(st)
+        hidden = torch.from_numpy(st.hidden.view(np.int16).copy()).pin_memory()
+        bt = torch.from_numpy(st.block_table.copy()).pin_memory()
+        sl = torch.from_numpy(st.seq_lens.copy()).pin_memory()
+        ra = torch.from_numpy(assign.copy()).pin_memory()
+        B.cc_forward_host(S.layer, hidden, step.k_pool, step.v_pool, step.n_pages, bt, sl, ra, 4,
+                          torch.cuda.current_stream())
+        assert np.array_equal(hidden.numpy().view(np.uint16), want)
+        assert B.cc_forward_launch_count(S.layer) == 12
