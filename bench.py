@@ -279,15 +279,16 @@ def run_ours(args):
     for r in (1, 2, 4):
         S.scale(r)
         step.set_assign(I.even_split(batch, r))
-        for _ in range(5):
+        n_r = min(K, 50)
+        for _ in range(min(K, 5)):
             graph.replay()
         a, b_ = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         a.record()
-        for _ in range(50):
+        for _ in range(n_r):
             graph.replay()
         b_.record()
         torch.cuda.synchronize()
-        ms = a.elapsed_time(b_) / 50
+        ms = a.elapsed_time(b_) / n_r
         ab = I.forward_algorithmic_bytes(shape, st.seq_lens, r)
         by_r[str(r)] = {"tokens_per_s": round(batch / (ms * 1e-3), 1), "ms_per_step": round(ms, 5),
                         "algorithmic_GBps": round(ab / (ms * 1e-3) / 1e9, 1),

@@ -51,8 +51,8 @@ k_attn(const int* __restrict__ seq_lens, CcKv kv, CcDims D, CcWork W) {
     float* merge = reinterpret_cast<float*>(smem_raw + (size_t)kAttnWarps * kAttnStages * C::kStageBytes);
     const uint32_t ring_u32 = smem_u32(ring);
 
-    pdl_launch_dependents();
     pdl_wait();
+    pdl_launch_dependents();
 
     const int G = D.G, Hkv = D.Hkv;
     const int n_items = W.sched->n_items * Hkv;

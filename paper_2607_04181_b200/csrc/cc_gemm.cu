@@ -58,8 +58,10 @@ k_gemm(CcGemmGeo G, const uint8_t* __restrict__ act, int planes, float* __restri
         fence_mbar_init();
     }
     if (warp == 1) tmem_alloc<kTmemCols>(&H->tmem_base);
-    pdl_launch_dependents();
-    pdl_wait();
+    // The grouping (k_group) and the replica table were written at least two kernels back in the
+    // chain; every kernel of the chain waits for its predecessor BEFORE it lets its successor
+    // start, so both are complete and visible here although this kernel's own predecessor (the
+    // producer of the activations) may still be running.
     if (threadIdx.x < CC_MAXR) {
         H->cnt[threadIdx.x] = sched->cnt[threadIdx.x];
         H->goff[threadIdx.x] = sched->goff[threadIdx.x];
@@ -80,71 +82,107 @@ k_gemm(CcGemmGeo G, const uint8_t* __restrict__ act, int planes, float* __restri
     const long long a_begin = cc_range_begin(G, blockIdx.x), a_end = cc_range_begin(G, blockIdx.x + 1);
     const uint32_t tmem_base = H->tmem_base;
 
+    const int kb_begin = (int)(a_begin % G.KB);
     if (nmax > 0 && a_begin < a_end) {
+        // Producer and MMA issuer: the whole warp walks the (warp-uniform) atom loop and one lane
+        // issues; every per-atom quantity is carried incrementally (no division, no 64-bit
+        // multiply inside the loops) -- the single issuing thread is the critical path of a
+        // weight-streaming kernel, ~40 instructions per 16 KiB atom here.
         if (warp == 0) {
             // ===================== producer =====================
-            if (lane == 0) {
-                const uint64_t pol_w = policy_evict_first();
+            // Weights do not depend on the previous kernel: the ring is filled with weight atoms
+            // first (mode 0), then the kernel waits for its predecessor, adds the activation
+            // slabs of those stages and carries on (mode 1), so the HBM stream restarts while
+            // the small kernel between two GEMMs is still running.
+            const uint64_t pol_w = policy_evict_first();
+            const size_t kb_stride = (size_t)Mpad * 128;
+            const long long per_rep = a_end - a_begin;
+            int n_act = 0;
+            for (int r = 0; r < CC_MAXR; ++r) n_act += H->cnt[r] > 0;
+            const long long total = per_rep * n_act;
+            const int n_pre = total < n_stages ? (int)total : n_stages;
+            auto run = [&](const int mode) {
                 int stage = 0;
                 uint32_t ph = 0;
+                uint8_t* sW = stage0;
+                long long idx = 0;
                 for (int r = 0; r < CC_MAXR; ++r) {
                     const int cnt = H->cnt[r];
                     if (cnt == 0) continue;
-                    const uint32_t n = (uint32_t)((cnt + 15) & ~15);
-                    const uint8_t* wsrc = H->blob[r] + G.w_off;
-                    const int goff = H->goff[r];
-                    for (long long a = a_begin; a < a_end; ++a) {
-                        const int kb = (int)(a % G.KB);
-                        mbar_wait(&H->empty[stage], ph ^ 1);
-                        uint8_t* sW = stage0 + (size_t)stage * stage_bytes;
-                        mbar_expect_tx(&H->full[stage], CC_A_TILE_BYTES + (uint32_t)planes * n * 128);
-                        bulk_g2s_hint(sW, wsrc + (size_t)a * CC_A_TILE_BYTES, CC_A_TILE_BYTES, &H->full[stage], pol_w);
-                        const uint8_t* asrc = act + ((size_t)kb * Mpad + goff) * 128;
-                        for (int pl = 0; pl < planes; ++pl)
-                            bulk_g2s(sW + CC_A_TILE_BYTES + pl * act_bytes_max, asrc + pl * plane_stride, n * 128,
-                                     &H->full[stage]);
-                        if (++stage == n_stages) { stage = 0; ph ^= 1; }
+                    const uint32_t nb = (uint32_t)((cnt + 15) & ~15) * 128u;   // bytes of one activation slab
+                    const uint32_t tx = CC_A_TILE_BYTES + (uint32_t)planes * nb;
+                    const uint8_t* wsrc = H->blob[r] + G.w_off + (size_t)a_begin * CC_A_TILE_BYTES;
+                    const uint8_t* abase = act + (size_t)H->goff[r] * 128;
+                    const uint8_t* asrc = abase + (size_t)kb_begin * kb_stride;
+                    int kb = kb_begin;
+                    for (long long a = a_begin; a < a_end; ++a, ++idx) {
+                        if (mode == 0 && idx >= n_pre) return;
+                        const bool pre = idx < n_pre;            // stage already holds its weights
+                        if (mode == 1 && !pre) mbar_wait(&H->empty[stage], ph ^ 1);
+                        if (lane == 0) {
+                            if (mode == 0 || !pre) {
+                                mbar_expect_tx(&H->full[stage], tx);
+                                bulk_g2s_hint(sW, wsrc, CC_A_TILE_BYTES, &H->full[stage], pol_w);
+                            }
+                            if (mode == 1) {
+                                bulk_g2s(sW + CC_A_TILE_BYTES, asrc, nb, &H->full[stage]);
+                                if (planes == 2)
+                                    bulk_g2s(sW + CC_A_TILE_BYTES + act_bytes_max, asrc + plane_stride, nb, &H->full[stage]);
+                            }
+                        }
+                        wsrc += CC_A_TILE_BYTES;
+                        asrc += kb_stride;
+                        if (++kb == G.KB) { kb = 0; asrc = abase; }
+                        sW += stage_bytes;
+                        if (++stage == n_stages) { stage = 0; ph ^= 1; sW = stage0; }
                     }
                 }
-            }
+            };
+            run(0);
+            pdl_wait();
+            if (lane == 0) pdl_launch_dependents();
+            run(1);
         } else if (warp == 1) {
             // ===================== MMA issuer =====================
-            if (lane == 0) {
-                int stage = 0;
-                uint32_t ph = 0;
-                uint32_t pc = 0;   // pieces started so far
-                for (int r = 0; r < CC_MAXR; ++r) {
-                    const int cnt = H->cnt[r];
-                    if (cnt == 0) continue;
-                    const uint32_t n = (uint32_t)((cnt + 15) & ~15);
-                    const uint32_t idesc = umma_idesc_bf16_m128(n);
-                    for (long long a = a_begin; a < a_end; ++a) {
-                        const int kb = (int)(a % G.KB);
-                        const bool first = (a == a_begin) || kb == 0;
-                        const bool last = (a == a_end - 1) || kb == G.KB - 1;
-                        const uint32_t buf = pc & 1;
-                        if (first) {
-                            mbar_wait(&H->tmem_empty[buf], ((pc >> 1) & 1) ^ 1);
-                            tc_fence_after();
-                        }
-                        mbar_wait(&H->full[stage], ph);
+            int stage = 0;
+            uint32_t ph = 0;
+            uint32_t pc = 0;   // pieces started so far
+            const uint32_t desc_hi = (uint32_t)(umma_desc_sw128(0) >> 32);
+            const uint32_t desc_lo0 = (uint32_t)umma_desc_sw128(smem_u32(stage0));
+            const uint32_t dstage = stage_bytes >> 4, dact = CC_A_TILE_BYTES >> 4, dlo = act_bytes_max >> 4;
+            uint32_t da = desc_lo0;
+            for (int r = 0; r < CC_MAXR; ++r) {
+                const int cnt = H->cnt[r];
+                if (cnt == 0) continue;
+                const uint32_t idesc = umma_idesc_bf16_m128((uint32_t)((cnt + 15) & ~15));
+                int kb = kb_begin;
+                bool first = true;
+                for (long long a = a_begin; a < a_end; ++a) {
+                    const bool last = (a == a_end - 1) || kb == G.KB - 1;
+                    const uint32_t buf = pc & 1;
+                    if (first) {
+                        mbar_wait(&H->tmem_empty[buf], ((pc >> 1) & 1) ^ 1);
                         tc_fence_after();
-                        const uint32_t sW = smem_u32(stage0 + (size_t)stage * stage_bytes);
-                        const uint64_t da = umma_desc_sw128(sW), db = umma_desc_sw128(sW + CC_A_TILE_BYTES);
-                        const uint64_t dlo = act_bytes_max >> 4;   // descriptor step from the hi to the lo plane
+                    }
+                    mbar_wait(&H->full[stage], ph);
+                    tc_fence_after();
+                    if (lane == 0) {
                         const uint32_t d_tmem = tmem_base + buf * 256;
+                        const uint32_t db = da + dact;
 #pragma unroll
                         for (int k = 0; k < CC_TILE_K / 16; ++k) {
-                            umma_bf16(d_tmem, da + 2 * k, db + 2 * k, idesc, (first && k == 0) ? 0u : 1u);
-                            if (planes == 2) umma_bf16(d_tmem, da + 2 * k, db + dlo + 2 * k, idesc, 1u);
+                            umma_bf16_lo(d_tmem, da + 2 * k, db + 2 * k, desc_hi, idesc, (first && k == 0) ? 0u : 1u);
+                            if (planes == 2) umma_bf16_lo(d_tmem, da + 2 * k, db + dlo + 2 * k, desc_hi, idesc, 1u);
                         }
                         umma_commit(&H->empty[stage]);
-                        if (last) {
-                            umma_commit(&H->tmem_full[buf]);
-                            ++pc;
-                        }
-                        if (++stage == n_stages) { stage = 0; ph ^= 1; }
+                        if (last) umma_commit(&H->tmem_full[buf]);
                     }
+                    __syncwarp();
+                    first = last;
+                    if (last) ++pc;
+                    if (++kb == G.KB) kb = 0;
+                    da += dstage;
+                    if (++stage == n_stages) { stage = 0; ph ^= 1; da = desc_lo0; }
                 }
             }
         } else {

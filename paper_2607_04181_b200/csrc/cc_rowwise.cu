@@ -59,8 +59,8 @@ __global__ void __launch_bounds__(256) k_group(const int* __restrict__ assign, c
     __shared__ int s_wnch[8];              // attention chunks in warp w
     __shared__ int s_goff[CC_MAXR + 1], s_cnt[CC_MAXR];
     const int b = threadIdx.x, warp = b >> 5, lane = b & 31;
-    pdl_launch_dependents();
     pdl_wait();
+    pdl_launch_dependents();
     const uint32_t mask = tab->active_mask;
     int rep = -1, nch = 0;
     if (b < batch) {
@@ -147,8 +147,8 @@ __global__ void __launch_bounds__(kNormThreads) k_rmsnorm_in(const __nv_bfloat16
                                                              const CcLayerTable* __restrict__ tab, CcWork W) {
     __shared__ float red[kNormThreads / 32];
     const int pos = blockIdx.x;
-    pdl_launch_dependents();
     pdl_wait();
+    pdl_launch_dependents();
     if (pos >= W.sched->n_pos) return;
     const int b = W.perm[pos];
     if (b < 0) return;
@@ -192,8 +192,8 @@ constexpr int kRopeRows = 4;
 __global__ void __launch_bounds__(64 * kRopeRows) k_rope_append(const int* __restrict__ seq_lens, CcKv kv, CcDims D,
                                                                 CcWork W) {
     const int t = blockIdx.x, pos = blockIdx.y * kRopeRows + threadIdx.y;
-    pdl_launch_dependents();
     pdl_wait();
+    pdl_launch_dependents();
     if (pos >= W.sched->n_pos) return;
     const int b = W.perm[pos];
     if (b < 0) return;
@@ -243,8 +243,8 @@ __global__ void __launch_bounds__(64 * kRopeRows) k_rope_append(const int* __res
 // ---------------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(64) k_attn_combine(const int* __restrict__ seq_lens, CcDims D, CcWork W) {
     const int hq = blockIdx.x, pos = blockIdx.y;
-    pdl_launch_dependents();
     pdl_wait();
+    pdl_launch_dependents();
     if (pos >= W.sched->n_pos) return;
     const int b = W.perm[pos];
     if (b < 0) return;
@@ -278,8 +278,8 @@ __global__ void __launch_bounds__(kNormThreads) k_resid_norm(const __nv_bfloat16
                                                              const CcLayerTable* __restrict__ tab, CcWork W) {
     __shared__ float red[kNormThreads / 32];
     const int pos = blockIdx.x;
-    pdl_launch_dependents();
     pdl_wait();
+    pdl_launch_dependents();
     if (pos >= W.sched->n_pos) return;
     const int b = W.perm[pos];
     if (b < 0) return;
@@ -329,8 +329,8 @@ __global__ void __launch_bounds__(kNormThreads) k_resid_norm(const __nv_bfloat16
 constexpr int kEpiRows = 8;
 __global__ void __launch_bounds__(32 * kEpiRows) k_swiglu(CcDims D, CcWork W) {
     const int t = blockIdx.x, pos = blockIdx.y * kEpiRows + threadIdx.y;
-    pdl_launch_dependents();
     pdl_wait();
+    pdl_launch_dependents();
     if (pos >= W.sched->n_pos) return;
     if (W.perm[pos] < 0) return;
     const int f = threadIdx.x * 4;
@@ -358,8 +358,8 @@ __global__ void __launch_bounds__(32 * kEpiRows) k_swiglu(CcDims D, CcWork W) {
 // ---------------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(32 * kEpiRows) k_final(__nv_bfloat16* __restrict__ hidden, CcDims D, CcWork W) {
     const int t = blockIdx.x, pos = blockIdx.y * kEpiRows + threadIdx.y;
-    pdl_launch_dependents();
     pdl_wait();
+    pdl_launch_dependents();
     if (pos >= W.sched->n_pos) return;
     const int b = W.perm[pos];
     if (b < 0) return;
