@@ -300,14 +300,14 @@ namespace {
 
 CcGemmGeo make_geo(int n_out, int k_in, int n_sms, size_t w_off) {
     CcGemmGeo g{};
-    g.T = (n_out + CC_TILE_N - 1) / CC_TILE_N;
+    g.ST = (n_out + CC_G * CC_TILE_N - 1) / (CC_G * CC_TILE_N);
     g.KB = (k_in + CC_TILE_K - 1) / CC_TILE_K;
-    const long long atoms = (long long)g.T * g.KB;
-    g.P = atoms < n_sms ? (int)atoms : n_sms;   // no empty range => every piece slot is written
+    const long long units = (long long)g.ST * g.KB;
+    g.P = units < n_sms ? (int)units : n_sms;   // no empty range => every piece slot is written
     g.w_off = w_off;
     return g;
 }
-size_t geo_bytes(const CcGemmGeo& g) { return (size_t)g.T * g.KB * CC_A_TILE_BYTES; }
+size_t geo_bytes(const CcGemmGeo& g) { return (size_t)g.ST * CC_G * g.KB * CC_A_TILE_BYTES; }
 
 struct Carver {   // bump allocator over one cudaMalloc
     size_t off = 0;
@@ -389,7 +389,7 @@ cc_status cc_create_layer(cc_ctx* ctx, const cc_layer_desc* desc, const cc_layer
     const size_t o_o = ws.take((size_t)D.o.KB * Mp * 128);
     const size_t o_y = ws.take((size_t)2 * D.gu.KB * Mp * 128);
     const size_t o_a = ws.take((size_t)2 * D.dn.KB * Mp * 128);
-    auto part_bytes = [&](const CcGemmGeo& g) { return (size_t)(g.P + g.T) * Mp * 128 * 4; };
+    auto part_bytes = [&](const CcGemmGeo& g) { return (size_t)(g.P + g.ST) * CC_G * Mp * 128 * 4; };
     const size_t o_pq = ws.take(part_bytes(D.qkv));
     const size_t o_po = ws.take(part_bytes(D.o));
     const size_t o_pg = ws.take(part_bytes(D.gu));
@@ -443,15 +443,15 @@ cc_status cc_create_layer(cc_ctx* ctx, const cc_layer_desc* desc, const cc_layer
     // one-time re-pack of the nine tensors into the blob (tcgen05 operand tile images + gains)
     typedef const __nv_bfloat16* bp;
     if (e == cudaSuccess)
-        e = cc_launch_pack(L->blob0 + D.qkv.w_off, (bp)w->wq, (bp)w->wk, (bp)w->wv, D.QD, D.KD, D.KD, 0, D.d, D.qkv.T,
+        e = cc_launch_pack(L->blob0 + D.qkv.w_off, (bp)w->wq, (bp)w->wk, (bp)w->wv, D.QD, D.KD, D.KD, 0, D.d, D.qkv.ST * CC_G,
                            D.qkv.KB, 0);
     if (e == cudaSuccess)
-        e = cc_launch_pack(L->blob0 + D.o.w_off, (bp)w->wo, nullptr, nullptr, D.d, 0, 0, 0, D.QD, D.o.T, D.o.KB, 0);
+        e = cc_launch_pack(L->blob0 + D.o.w_off, (bp)w->wo, nullptr, nullptr, D.d, 0, 0, 0, D.QD, D.o.ST * CC_G, D.o.KB, 0);
     if (e == cudaSuccess)
-        e = cc_launch_pack(L->blob0 + D.gu.w_off, (bp)w->wgate, (bp)w->wup, nullptr, D.F, D.F, 0, 1, D.d, D.gu.T,
+        e = cc_launch_pack(L->blob0 + D.gu.w_off, (bp)w->wgate, (bp)w->wup, nullptr, D.F, D.F, 0, 1, D.d, D.gu.ST * CC_G,
                            D.gu.KB, 0);
     if (e == cudaSuccess)
-        e = cc_launch_pack(L->blob0 + D.dn.w_off, (bp)w->wdown, nullptr, nullptr, D.d, 0, 0, 0, D.F, D.dn.T, D.dn.KB, 0);
+        e = cc_launch_pack(L->blob0 + D.dn.w_off, (bp)w->wdown, nullptr, nullptr, D.d, 0, 0, 0, D.F, D.dn.ST * CC_G, D.dn.KB, 0);
     if (e == cudaSuccess) e = cudaMemcpy(L->blob0 + D.off_g1, w->g1, (size_t)D.d * 2, cudaMemcpyDeviceToDevice);
     if (e == cudaSuccess) e = cudaMemcpy(L->blob0 + D.off_g2, w->g2, (size_t)D.d * 2, cudaMemcpyDeviceToDevice);
     L->rep[0].state = REP_LIVE;
@@ -728,15 +728,13 @@ cc_status cc_debug_tap(cc_layer* L, cc_tap which, float* out_host, int batch) {
     const CcDims& D = L->D;
     const void* src;
     int kind, dim;
-    size_t plane = 0;
-    const size_t Mp128 = (size_t)D.Mpad * 128;
     switch (which) {
-        case CC_TAP_X: src = L->W.x_act; kind = 2; dim = D.d; plane = D.qkv.KB * Mp128; break;
+        case CC_TAP_X: src = L->W.x_act; kind = 2; dim = D.d; break;
         case CC_TAP_Q: src = L->W.q_rot; kind = 1; dim = D.QD; break;
         case CC_TAP_O: src = L->W.o_act; kind = 0; dim = D.QD; break;
         case CC_TAP_H1: src = L->W.h1; kind = 1; dim = D.d; break;
-        case CC_TAP_Y: src = L->W.y_act; kind = 2; dim = D.d; plane = D.gu.KB * Mp128; break;
-        case CC_TAP_A: src = L->W.a_act; kind = 2; dim = D.F; plane = D.dn.KB * Mp128; break;
+        case CC_TAP_Y: src = L->W.y_act; kind = 2; dim = D.d; break;
+        case CC_TAP_A: src = L->W.a_act; kind = 2; dim = D.F; break;
         default: return fail(CC_ERR_INVALID, "unknown tap");
     }
     CC_CUDA(cudaSetDevice(L->ctx->device));
@@ -745,7 +743,7 @@ cc_status cc_debug_tap(cc_layer* L, cc_tap which, float* out_host, int batch) {
     const size_t bytes = (size_t)batch * dim * 4;
     CC_CUDA(cudaMalloc(&tmp, bytes));
     cudaError_t e = cudaMemset(tmp, 0, bytes);
-    if (e == cudaSuccess) e = cc_launch_tap(src, kind, dim, plane, D, L->W, tmp, batch, 0);
+    if (e == cudaSuccess) e = cc_launch_tap(src, kind, dim, D, L->W, tmp, batch, 0);
     if (e == cudaSuccess) e = cudaMemcpy(out_host, tmp, bytes, cudaMemcpyDeviceToHost);
     cudaFree(tmp);
     if (e != cudaSuccess) return fail(CC_ERR_CUDA, "cc_debug_tap: %s", cudaGetErrorString(e));

@@ -30,32 +30,48 @@ struct CcLayerTable {
     uint32_t pad_[3];
 };
 
-// Geometry of one weight-streaming GEMM (swap-AB: the packed weight tile is the UMMA A operand,
+// Geometry of one weight-streaming GEMM (swap-AB: packed weight tiles are the UMMA A operand,
 // M = 128 output features; the activations are the B operand, N = rows of one replica group).
-// The (tile, k-block) "atoms" of 16 KiB are numbered tile-major and cut into P contiguous
+// CC_G adjacent tiles (a "super tile" of CC_G * 128 output features) are streamed together: one
+// pipeline stage holds the CC_G weight atoms of one k-block (contiguous in the blob, ONE bulk
+// copy of CC_G * 16 KiB) plus the activation slab of that k-block (ONE bulk copy), so the slab
+// is fetched from L2 once per CC_G atoms and the single producer thread issues two copies per
+// 32 KiB of weights (measured: the copy-issue rate, not HBM, bounded the one-atom-per-stage
+// version; profiles/r01_microbench.md).
+// The (super tile, k-block) "units" are numbered super-tile-major and cut into P contiguous
 // ranges, range i owned by CTA i.  P and the cut points depend on the layer shape and the SM
 // count only -- never on the batch split -- so every output element is summed in one fixed
 // order whatever the replica count (PAPER.md:385 bit-wise consistency).
+#define CC_G 2
 struct CcGemmGeo {
-    int T;        // tiles of 128 output features
+    int ST;       // super tiles of CC_G * 128 output features
     int KB;       // k-blocks of 64 per tile
     int P;        // CTAs (ranges)
     int pad_;
     size_t w_off; // byte offset of the packed matrix inside a replica blob
 };
-// Range of CTA i: atoms [cc_range_begin(i), cc_range_begin(i+1)).
+// Range of CTA i: units [cc_range_begin(i), cc_range_begin(i+1)).
 __host__ __device__ __forceinline__ long long cc_range_begin(const CcGemmGeo& g, int i) {
-    return (long long)i * g.T * g.KB / g.P;
+    return (long long)i * g.ST * g.KB / g.P;
 }
-// CTA whose range holds atom a (inverse of cc_range_begin).
-__host__ __device__ __forceinline__ int cc_range_of_atom(const CcGemmGeo& g, long long a) {
-    return (int)(((a + 1) * g.P - 1) / ((long long)g.T * g.KB));
+// CTA whose range holds unit u (inverse of cc_range_begin).
+__host__ __device__ __forceinline__ int cc_range_of_unit(const CcGemmGeo& g, long long u) {
+    return (int)(((u + 1) * g.P - 1) / ((long long)g.ST * g.KB));
 }
-// A "piece" is the part of one tile that one CTA accumulated; piece id = CTA + tile (unique and
-// increasing along the atom axis).  Partial sums live at part[piece][pos][128] fp32.
-__host__ __device__ __forceinline__ void cc_tile_pieces(const CcGemmGeo& g, int t, int& first, int& last) {
-    first = cc_range_of_atom(g, (long long)t * g.KB) + t;
-    last = cc_range_of_atom(g, (long long)(t + 1) * g.KB - 1) + t;
+// A "piece" is the part of one 128-feature tile that one CTA accumulated.  Piece slot of
+// (CTA c, super tile st, tile j of the super tile) = (c + st) * CC_G + j: unique, and increasing
+// along the unit axis.  Partial sums live at part[slot][pos][128] fp32.  The pieces of tile t
+// are `count` slots starting at `first`, CC_G apart, to be added in that order.
+__host__ __device__ __forceinline__ void cc_tile_pieces(const CcGemmGeo& g, int t, int& first, int& count) {
+    const int st = t / CC_G, j = t - st * CC_G;
+    const int c0 = cc_range_of_unit(g, (long long)st * g.KB);
+    const int c1 = cc_range_of_unit(g, (long long)(st + 1) * g.KB - 1);
+    first = (c0 + st) * CC_G + j;
+    count = c1 - c0 + 1;
+}
+// Byte offset of packed weight atom (tile t, k-block kb) inside its matrix.
+__host__ __device__ __forceinline__ size_t cc_atom_off(int KB, int t, int kb) {
+    return (((size_t)(t / CC_G) * KB + kb) * CC_G + (t % CC_G)) * (size_t)CC_A_TILE_BYTES;
 }
 
 // Static per-layer geometry, passed to kernels by value.
@@ -90,11 +106,16 @@ __device__ __forceinline__ uint32_t pack_bf16(float lo, float hi) {
 __device__ __forceinline__ uint32_t smem_u32(const void* p) {
     return static_cast<uint32_t>(__cvta_generic_to_shared(p));
 }
-// Byte offset of element (row, k) inside a packed activation buffer [K/64][Mpad][64] whose
-// 128-byte rows are stored in the 128B-swizzle pattern (16-byte chunk c of row r at c ^ (r & 7)).
-__device__ __forceinline__ size_t act_chunk_off(int row, int k, int Mpad) {
-    int kb = k >> 6, c = (k >> 3) & 7;
-    return ((size_t)kb * Mpad + row) * 128 + (size_t)((c ^ (row & 7)) << 4);
+// Byte offset of the 16-byte chunk holding element (row, k) of plane `pl` inside a packed
+// activation buffer [K/64][Mpad/8][planes][8 rows][128 B]: 8-row groups of the hi and lo planes
+// alternate, so the slab of one k-block and one row group (rows goff .. goff+n, both multiples of
+// 8) is ONE contiguous range holding both planes; inside an 8-row group the 128-byte rows are
+// stored in the 128B-swizzle pattern (16-byte chunk c of row r at c ^ (r & 7)).  The UMMA
+// descriptor of a plane uses a stride of planes * 1024 bytes between 8-row groups.
+__device__ __forceinline__ size_t act_chunk_off(int row, int k, int Mpad, int planes, int pl) {
+    const int kb = k >> 6, c = (k >> 3) & 7;
+    return ((((size_t)kb * (Mpad >> 3) + (row >> 3)) * planes + pl) << 10) + (size_t)((row & 7) << 7) +
+           (size_t)((c ^ (row & 7)) << 4);
 }
 
 // ---- mbarrier / bulk-copy / TMA ----------------------------------------------------------
@@ -192,17 +213,17 @@ __device__ __forceinline__ void umma_bf16(uint32_t d_tmem, uint64_t a_desc, uint
         "l"(a_desc), "l"(b_desc), "r"(idesc), "r"(accumulate)
         : "memory");
 }
-// Same, with the two descriptors given as 32-bit low words sharing one high word (all the fields
-// that change from MMA to MMA -- the start address -- live in the low word).
-__device__ __forceinline__ void umma_bf16_lo(uint32_t d_tmem, uint32_t a_lo, uint32_t b_lo, uint32_t desc_hi,
+// Same, with the two descriptors given as 32-bit low words plus their (loop-invariant) high words:
+// all the fields that change from MMA to MMA -- the start address -- live in the low word.
+__device__ __forceinline__ void umma_bf16_lo(uint32_t d_tmem, uint32_t a_lo, uint32_t b_lo, uint32_t a_hi, uint32_t b_hi,
                                              uint32_t idesc, uint32_t accumulate) {
     asm volatile(
         "{\n\t.reg .pred p;\n\t.reg .b64 da, db;\n\t"
-        "setp.ne.b32 p, %5, 0;\n\t"
+        "setp.ne.b32 p, %6, 0;\n\t"
         "mov.b64 da, {%1, %3};\n\t"
-        "mov.b64 db, {%2, %3};\n\t"
-        "tcgen05.mma.cta_group::1.kind::f16 [%0], da, db, %4, p;\n\t}" ::"r"(d_tmem),
-        "r"(a_lo), "r"(b_lo), "r"(desc_hi), "r"(idesc), "r"(accumulate)
+        "mov.b64 db, {%2, %4};\n\t"
+        "tcgen05.mma.cta_group::1.kind::f16 [%0], da, db, %5, p;\n\t}" ::"r"(d_tmem),
+        "r"(a_lo), "r"(b_lo), "r"(a_hi), "r"(b_hi), "r"(idesc), "r"(accumulate)
         : "memory");
 }
 // mbarrier arrive once all previously issued tcgen05.mma of this thread have completed.
@@ -225,11 +246,11 @@ __device__ __forceinline__ void tmem_ld_wait() { asm volatile("tcgen05.wait::ld.
 // Shared-memory matrix descriptor: K-major operand, 128B swizzle, rows of 128 bytes, 8-row
 // groups 1024 bytes apart (SBO), descriptor version 1 (sm_100).  Tile base must be 1024-aligned;
 // advancing K by 16 bf16 inside the swizzle atom adds 32 bytes to the start address.
-__device__ __forceinline__ uint64_t umma_desc_sw128(uint32_t smem_addr) {
+__device__ __forceinline__ uint64_t umma_desc_sw128(uint32_t smem_addr, uint32_t sbo_bytes = 1024) {
     uint64_t d = 0;
     d |= (uint64_t)((smem_addr & 0x3FFFFu) >> 4);   // start address  [0,14)
     d |= (uint64_t)1 << 16;                          // LBO (unused for swizzled K-major) [16,30)
-    d |= (uint64_t)(1024 >> 4) << 32;                // SBO = 1024 B   [32,46)
+    d |= (uint64_t)(sbo_bytes >> 4) << 32;           // SBO: bytes between 8-row groups [32,46)
     d |= (uint64_t)1 << 46;                          // version = 1    [46,48)
     d |= (uint64_t)2 << 61;                          // SWIZZLE_128B   [61,64)
     return d;

@@ -3,19 +3,21 @@
 // SURVEY.md 8(a) rows a2 (QKV), a6 (O), a8 (gate/up), a9 (down); replica indirection row a10.
 // Decode is HBM-bound: every weight byte is read once per replica group, so the kernel is built
 // around the weight stream, not around the MMA:
-//   * swap-AB: the packed weight tile (128 output features x 64 k, a 16 KiB pre-swizzled image
+//   * swap-AB: a packed weight tile (128 output features x 64 k, a 16 KiB pre-swizzled image
 //     made once at cc_create_layer) is the tcgen05 A operand (M = 128); the activations of one
 //     replica group (n rows, n = multiple of 16, <= 256) are the B operand (N = n), held as two
 //     bf16 planes hi + lo that are both multiplied into the same accumulator (cc_rowwise.cu).
-//     The fp32 accumulator D[128][n] lives in TMEM (n columns), double-buffered.
-//   * one persistent CTA per SM, stream-K: the (tile, k-block) atoms are cut into P contiguous
-//     ranges fixed by the layer shape (cc_common.cuh); CTA i streams range i of EVERY active
-//     replica's blob, whose base it reads from the device replica table at run time
-//     (PAPER.md:391-393 re-captures a graph when the replica set changes; here nothing does).
-//   * warp 0 = producer: 1-D bulk copies (TMA engine, no tensor map) of 16 KiB weight atoms and
-//     of the matching activation slab into a ring of smem stages guarded by mbarriers;
-//     warp 1 = MMA issuer (one elected thread, 4 x tcgen05.mma K=16 per atom, tcgen05.commit
-//     frees the stage); warps 2..5 = epilogue (tcgen05.ld -> fp32 partials in global memory).
+//   * CC_G = 2 adjacent tiles form a super tile: one pipeline stage = the two weight atoms of
+//     one k-block (32 KiB, contiguous in the blob, one bulk copy) + the activation slab of that
+//     k-block (both planes, one bulk copy), feeding two fp32 accumulators D[128][n] in TMEM
+//     (double-buffered while 2 * CC_G * n <= 512 columns).
+//   * one persistent CTA per SM, stream-K: the (super tile, k-block) units are cut into P
+//     contiguous ranges fixed by the layer shape (cc_common.cuh); CTA i streams range i of
+//     EVERY active replica's blob, whose base it reads from the device replica table at run
+//     time (PAPER.md:391-393 re-captures a graph when the replica set changes; here nothing does).
+//   * warp 0 = producer: 1-D bulk copies (TMA engine, no tensor map) into a ring of smem stages
+//     guarded by mbarriers; warp 1 = MMA issuer (one elected thread, tcgen05.commit frees the
+//     stage); warps 2..5 = epilogue (tcgen05.ld -> fp32 partials in global memory).
 //   * a tile's partial sums ("pieces") are added up in fixed order by the next kernel of the
 //     chain, which also applies the fused epilogue (RoPE, residual + RMSNorm, SwiGLU, ...).
 #include "cc_kernels.h"
@@ -23,9 +25,10 @@
 namespace {
 
 constexpr int kGemmThreads = 192;
-constexpr int kMaxStages = 12;
-constexpr int kGemmSmem = 200 * 1024;     // dynamic shared memory per CTA
-constexpr int kTmemCols = 512;            // two accumulators of up to 256 columns
+constexpr int kMaxStages = 8;
+constexpr int kGemmSmem = 225 * 1024;     // dynamic shared memory per CTA
+constexpr int kTmemCols = 512;
+constexpr uint32_t kWStage = CC_G * CC_A_TILE_BYTES;   // weight bytes per stage (32 KiB)
 
 struct GemmSmemHdr {                      // lives at the start of dynamic smem
     uint64_t full[kMaxStages];
@@ -72,22 +75,25 @@ k_gemm(CcGemmGeo G, const uint8_t* __restrict__ act, int planes, float* __restri
     tc_fence_after();
 
     const int nmax = sched->nmax;
-    const uint32_t act_bytes_max = (uint32_t)((nmax * 128 + 1023) & ~1023);
-    const uint32_t stage_bytes = CC_A_TILE_BYTES + (uint32_t)planes * act_bytes_max;
-    const size_t plane_stride = (size_t)G.KB * Mpad * 128;   // bytes between the hi and lo operand planes
+    const uint32_t act_bytes_max = (uint32_t)planes * (uint32_t)nmax * 128u;   // nmax % 16 == 0 => multiple of 2 KiB
+    const uint32_t stage_bytes = kWStage + act_bytes_max;
     uint8_t* stage0 = smem_raw + 1024;                      // header occupies the first KiB
     int n_stages = (kGemmSmem - 1024) / (int)stage_bytes;
     if (n_stages > kMaxStages) n_stages = kMaxStages;
+    // TMEM: accumulator (buf, j) at column buf * 256 + j * acc_cols; one buffer only when the two
+    // accumulators of a super tile need more than 256 columns
+    const uint32_t nbuf_log2 = nmax <= 128 ? 1u : 0u;
+    const uint32_t acc_cols = nmax <= 128 ? 128u : 256u;
 
-    const long long a_begin = cc_range_begin(G, blockIdx.x), a_end = cc_range_begin(G, blockIdx.x + 1);
+    const long long u_begin = cc_range_begin(G, blockIdx.x), u_end = cc_range_begin(G, blockIdx.x + 1);
     const uint32_t tmem_base = H->tmem_base;
 
-    const int kb_begin = (int)(a_begin % G.KB);
-    if (nmax > 0 && a_begin < a_end) {
-        // Producer and MMA issuer: the whole warp walks the (warp-uniform) atom loop and one lane
-        // issues; every per-atom quantity is carried incrementally (no division, no 64-bit
+    const int kb_begin = (int)(u_begin % G.KB);
+    if (nmax > 0 && u_begin < u_end) {
+        // Producer and MMA issuer: the whole warp walks the (warp-uniform) unit loop and one lane
+        // issues; every per-unit quantity is carried incrementally (no division, no 64-bit
         // multiply inside the loops) -- the single issuing thread is the critical path of a
-        // weight-streaming kernel, ~40 instructions per 16 KiB atom here.
+        // weight-streaming kernel.
         if (warp == 0) {
             // ===================== producer =====================
             // Weights do not depend on the previous kernel: the ring is filled with weight atoms
@@ -95,8 +101,8 @@ k_gemm(CcGemmGeo G, const uint8_t* __restrict__ act, int planes, float* __restri
             // slabs of those stages and carries on (mode 1), so the HBM stream restarts while
             // the small kernel between two GEMMs is still running.
             const uint64_t pol_w = policy_evict_first();
-            const size_t kb_stride = (size_t)Mpad * 128;
-            const long long per_rep = a_end - a_begin;
+            const size_t kb_stride = (size_t)(Mpad >> 3) * planes * 1024;   // bytes between k-blocks of the operand
+            const long long per_rep = u_end - u_begin;
             int n_act = 0;
             for (int r = 0; r < CC_MAXR; ++r) n_act += H->cnt[r] > 0;
             const long long total = per_rep * n_act;
@@ -109,28 +115,24 @@ k_gemm(CcGemmGeo G, const uint8_t* __restrict__ act, int planes, float* __restri
                 for (int r = 0; r < CC_MAXR; ++r) {
                     const int cnt = H->cnt[r];
                     if (cnt == 0) continue;
-                    const uint32_t nb = (uint32_t)((cnt + 15) & ~15) * 128u;   // bytes of one activation slab
-                    const uint32_t tx = CC_A_TILE_BYTES + (uint32_t)planes * nb;
-                    const uint8_t* wsrc = H->blob[r] + G.w_off + (size_t)a_begin * CC_A_TILE_BYTES;
-                    const uint8_t* abase = act + (size_t)H->goff[r] * 128;
+                    const uint32_t nb = (uint32_t)((cnt + 15) & ~15) * 128u * (uint32_t)planes;   // bytes of one slab
+                    const uint32_t tx = kWStage + nb;
+                    const uint8_t* wsrc = H->blob[r] + G.w_off + (size_t)u_begin * kWStage;
+                    const uint8_t* abase = act + (size_t)(H->goff[r] >> 3) * planes * 1024;
                     const uint8_t* asrc = abase + (size_t)kb_begin * kb_stride;
                     int kb = kb_begin;
-                    for (long long a = a_begin; a < a_end; ++a, ++idx) {
+                    for (long long u = u_begin; u < u_end; ++u, ++idx) {
                         if (mode == 0 && idx >= n_pre) return;
                         const bool pre = idx < n_pre;            // stage already holds its weights
                         if (mode == 1 && !pre) mbar_wait(&H->empty[stage], ph ^ 1);
                         if (lane == 0) {
                             if (mode == 0 || !pre) {
                                 mbar_expect_tx(&H->full[stage], tx);
-                                bulk_g2s_hint(sW, wsrc, CC_A_TILE_BYTES, &H->full[stage], pol_w);
+                                bulk_g2s_hint(sW, wsrc, kWStage, &H->full[stage], pol_w);
                             }
-                            if (mode == 1) {
-                                bulk_g2s(sW + CC_A_TILE_BYTES, asrc, nb, &H->full[stage]);
-                                if (planes == 2)
-                                    bulk_g2s(sW + CC_A_TILE_BYTES + act_bytes_max, asrc + plane_stride, nb, &H->full[stage]);
-                            }
+                            if (mode == 1) bulk_g2s(sW + kWStage, asrc, nb, &H->full[stage]);
                         }
-                        wsrc += CC_A_TILE_BYTES;
+                        wsrc += kWStage;
                         asrc += kb_stride;
                         if (++kb == G.KB) { kb = 0; asrc = abase; }
                         sW += stage_bytes;
@@ -146,10 +148,11 @@ k_gemm(CcGemmGeo G, const uint8_t* __restrict__ act, int planes, float* __restri
             // ===================== MMA issuer =====================
             int stage = 0;
             uint32_t ph = 0;
-            uint32_t pc = 0;   // pieces started so far
-            const uint32_t desc_hi = (uint32_t)(umma_desc_sw128(0) >> 32);
+            uint32_t pc = 0;   // super-tile pieces started so far
+            const uint32_t a_hi = (uint32_t)(umma_desc_sw128(0) >> 32);
+            const uint32_t b_hi = (uint32_t)(umma_desc_sw128(0, (uint32_t)planes * 1024u) >> 32);
             const uint32_t desc_lo0 = (uint32_t)umma_desc_sw128(smem_u32(stage0));
-            const uint32_t dstage = stage_bytes >> 4, dact = CC_A_TILE_BYTES >> 4, dlo = act_bytes_max >> 4;
+            const uint32_t dstage = stage_bytes >> 4, dact = kWStage >> 4;
             uint32_t da = desc_lo0;
             for (int r = 0; r < CC_MAXR; ++r) {
                 const int cnt = H->cnt[r];
@@ -157,22 +160,26 @@ k_gemm(CcGemmGeo G, const uint8_t* __restrict__ act, int planes, float* __restri
                 const uint32_t idesc = umma_idesc_bf16_m128((uint32_t)((cnt + 15) & ~15));
                 int kb = kb_begin;
                 bool first = true;
-                for (long long a = a_begin; a < a_end; ++a) {
-                    const bool last = (a == a_end - 1) || kb == G.KB - 1;
-                    const uint32_t buf = pc & 1;
+                for (long long u = u_begin; u < u_end; ++u) {
+                    const bool last = (u == u_end - 1) || kb == G.KB - 1;
+                    const uint32_t buf = pc & nbuf_log2;
                     if (first) {
-                        mbar_wait(&H->tmem_empty[buf], ((pc >> 1) & 1) ^ 1);
+                        mbar_wait(&H->tmem_empty[buf], ((pc >> nbuf_log2) & 1) ^ 1);
                         tc_fence_after();
                     }
                     mbar_wait(&H->full[stage], ph);
                     tc_fence_after();
                     if (lane == 0) {
-                        const uint32_t d_tmem = tmem_base + buf * 256;
                         const uint32_t db = da + dact;
 #pragma unroll
-                        for (int k = 0; k < CC_TILE_K / 16; ++k) {
-                            umma_bf16_lo(d_tmem, da + 2 * k, db + 2 * k, desc_hi, idesc, (first && k == 0) ? 0u : 1u);
-                            if (planes == 2) umma_bf16_lo(d_tmem, da + 2 * k, db + dlo + 2 * k, desc_hi, idesc, 1u);
+                        for (int j = 0; j < CC_G; ++j) {
+                            const uint32_t d_tmem = tmem_base + buf * 256 + (uint32_t)j * acc_cols;
+                            const uint32_t daj = da + (uint32_t)j * (CC_A_TILE_BYTES >> 4);
+#pragma unroll
+                            for (int k = 0; k < CC_TILE_K / 16; ++k) {
+                                umma_bf16_lo(d_tmem, daj + 2 * k, db + 2 * k, a_hi, b_hi, idesc, (first && k == 0) ? 0u : 1u);
+                                if (planes == 2) umma_bf16_lo(d_tmem, daj + 2 * k, db + 64 + 2 * k, a_hi, b_hi, idesc, 1u);
+                            }
                         }
                         umma_commit(&H->empty[stage]);
                         if (last) umma_commit(&H->tmem_full[buf]);
@@ -195,28 +202,32 @@ k_gemm(CcGemmGeo G, const uint8_t* __restrict__ act, int planes, float* __restri
                 if (cnt == 0) continue;
                 const int n = (cnt + 15) & ~15;
                 const int goff = H->goff[r];
-                long long a = a_begin;
-                while (a < a_end) {
-                    const int t = (int)(a / G.KB);
-                    long long a_next = (long long)(t + 1) * G.KB;
-                    if (a_next > a_end) a_next = a_end;
-                    const uint32_t buf = pc & 1;
-                    mbar_wait(&H->tmem_full[buf], (pc >> 1) & 1);
+                long long u = u_begin;
+                while (u < u_end) {
+                    const int st = (int)(u / G.KB);
+                    long long u_next = (long long)(st + 1) * G.KB;
+                    if (u_next > u_end) u_next = u_end;
+                    const uint32_t buf = pc & nbuf_log2;
+                    mbar_wait(&H->tmem_full[buf], (pc >> nbuf_log2) & 1);
                     tc_fence_after();
-                    float* dst = part + ((size_t)(blockIdx.x + t) * Mpad + goff) * 128 + f;
-                    for (int c = 0; c < n; c += 16) {
-                        uint32_t v[16];
-                        tmem_ld_32x32b_x16(tmem_base + ((uint32_t)(q * 32) << 16) + buf * 256 + c, v);
-                        tmem_ld_wait();
 #pragma unroll
-                        for (int j = 0; j < 16; ++j)
-                            if (c + j < cnt) dst[(size_t)(c + j) * 128] = __uint_as_float(v[j]);
+                    for (int j = 0; j < CC_G; ++j) {
+                        float* dst = part + ((size_t)((blockIdx.x + st) * CC_G + j) * Mpad + goff) * 128 + f;
+                        const uint32_t tcol = tmem_base + ((uint32_t)(q * 32) << 16) + buf * 256 + (uint32_t)j * acc_cols;
+                        for (int c = 0; c < n; c += 16) {
+                            uint32_t v[16];
+                            tmem_ld_32x32b_x16(tcol + c, v);
+                            tmem_ld_wait();
+#pragma unroll
+                            for (int i = 0; i < 16; ++i)
+                                if (c + i < cnt) dst[(size_t)(c + i) * 128] = __uint_as_float(v[i]);
+                        }
                     }
                     tc_fence_before();
                     __syncwarp();
                     if (lane == 0) mbar_arrive(&H->tmem_empty[buf]);
                     ++pc;
-                    a = a_next;
+                    u = u_next;
                 }
             }
         }

@@ -54,7 +54,8 @@ __global__ void k_publish(CcLayerTable* row, CcLayerTable value) {
 }
 
 // One-time weight re-pack: [out][in] bf16 rows -> 16 KiB tile images (128 rows x 64 k, 128B swizzle),
-// tile (t, kb) at ((t * k_blocks + kb) * 16 KiB).  Rows / k beyond the matrix are zero.
+// tile (t, kb) at cc_atom_off(k_blocks, t, kb): the CC_G tiles of a super tile are adjacent per k-block.
+// Rows / k beyond the matrix are zero.
 __global__ void __launch_bounds__(256) k_pack(uint8_t* __restrict__ dst, const __nv_bfloat16* __restrict__ src0,
                                               const __nv_bfloat16* __restrict__ src1,
                                               const __nv_bfloat16* __restrict__ src2, int rows0, int rows1, int rows2,
@@ -76,7 +77,7 @@ __global__ void __launch_bounds__(256) k_pack(uint8_t* __restrict__ dst, const _
         }
         uint4 v = make_uint4(0, 0, 0, 0);
         if (row && k0 < K) v = *reinterpret_cast<const uint4*>(row + k0);   // K % 8 == 0
-        *reinterpret_cast<uint4*>(dst + tk * CC_A_TILE_BYTES + (size_t)i * 128 + ((c ^ (i & 7)) << 4)) = v;
+        *reinterpret_cast<uint4*>(dst + cc_atom_off(k_blocks, t, kb) + (size_t)i * 128 + ((c ^ (i & 7)) << 4)) = v;
     }
 }
 

@@ -7,11 +7,11 @@ struct CcWork {
     CcSched* sched;
     int* perm;           // [Mpad] original row at grouped position, or -1
     int2* items;         // attention work items (pos, chunk), at most max_batch * nch_max
-    uint8_t* x_act;      // packed bf16 GEMM operands, [plane hi|lo][K/64][Mpad][128 B swizzled]
+    uint8_t* x_act;      // packed bf16 GEMM operands, [K/64][Mpad/8][plane hi|lo][8][128 B swizzled]
     uint8_t* o_act;      // (one plane)
     uint8_t* y_act;
     uint8_t* a_act;
-    float* qkv_part;     // stream-K partial sums, [P + T][Mpad][128] fp32 (piece-major)
+    float* qkv_part;     // stream-K partial sums, [(P + ST) * CC_G][Mpad][128] fp32 (piece-major)
     float* o_part;
     float* gu_part;
     float* d_part;
@@ -62,7 +62,7 @@ cudaError_t cc_launch_pack(uint8_t* dst, const __nv_bfloat16* src0, const __nv_b
                            const __nv_bfloat16* src2, int rows0, int rows1, int rows2, int mode, int K, int n_tiles,
                            int k_blocks, cudaStream_t st);
 // which: 0 = one packed bf16 plane (K = dim), 1 = fp32 row buffer [Mpad][dim], 2 = hi + lo planes
-cudaError_t cc_launch_tap(const void* src, int which, int dim, size_t plane, const CcDims& D, const CcWork& W,
+cudaError_t cc_launch_tap(const void* src, int which, int dim, const CcDims& D, const CcWork& W,
                           float* out_dev, int batch, cudaStream_t st);
 int cc_max_hidden();
 

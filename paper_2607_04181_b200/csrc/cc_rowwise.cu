@@ -156,7 +156,6 @@ __global__ void __launch_bounds__(kNormThreads) k_rmsnorm_in(const __nv_bfloat16
     const uint4* g = reinterpret_cast<const uint4*>(tab->rep[r].blob + D.off_g1);
     const uint4* row = reinterpret_cast<const uint4*>(hidden + (size_t)b * D.d);
     const int nchunk = D.d >> 3;
-    const size_t plane = (size_t)D.qkv.KB * D.Mpad * 128;
     float ss = 0.f;
     for (int c = threadIdx.x; c < nchunk; c += kNormThreads) {
         const uint4 v = row[c];
@@ -176,9 +175,9 @@ __global__ void __launch_bounds__(kNormThreads) k_rmsnorm_in(const __nv_bfloat16
 #pragma unroll
         for (int i = 0; i < 4; ++i)
             split_hilo(bf16lo(w[i]) * inv * bf16lo(gw[i]), bf16hi(w[i]) * inv * bf16hi(gw[i]), hi[i], lo[i]);
-        uint8_t* dst = W.x_act + act_chunk_off(pos, c << 3, D.Mpad);
+        uint8_t* dst = W.x_act + act_chunk_off(pos, c << 3, D.Mpad, 2, 0);
         *reinterpret_cast<uint4*>(dst) = make_uint4(hi[0], hi[1], hi[2], hi[3]);
-        *reinterpret_cast<uint4*>(dst + plane) = make_uint4(lo[0], lo[1], lo[2], lo[3]);
+        *reinterpret_cast<uint4*>(dst + 1024) = make_uint4(lo[0], lo[1], lo[2], lo[3]);
     }
 }
 
@@ -200,11 +199,11 @@ __global__ void __launch_bounds__(64 * kRopeRows) k_rope_append(const int* __res
     const int half = D.Dh >> 1;
     const int j = threadIdx.x;
     const int f0 = (j / half) * D.Dh + (j % half);         // first column of the pair inside the tile
-    int p0, p1;
-    cc_tile_pieces(D.qkv, t, p0, p1);
+    int p0, np;
+    cc_tile_pieces(D.qkv, t, p0, np);
     float a = 0.f, bb = 0.f;
-    for (int p = p0; p <= p1; ++p) {
-        const float* src = W.qkv_part + ((size_t)p * D.Mpad + pos) * 128;
+    for (int i = 0; i < np; ++i) {
+        const float* src = W.qkv_part + ((size_t)(p0 + i * CC_G) * D.Mpad + pos) * 128;
         a += src[f0];
         bb += src[f0 + half];
     }
@@ -265,7 +264,7 @@ __global__ void __launch_bounds__(64) k_attn_combine(const int* __restrict__ seq
     }
     const float inv = 1.f / L;
     const int e = hq * D.Dh + dim;
-    uint8_t* dst = W.o_act + act_chunk_off(pos, e, D.Mpad) + (e & 7) * 2;
+    uint8_t* dst = W.o_act + act_chunk_off(pos, e, D.Mpad, 1, 0) + (e & 7) * 2;
     *reinterpret_cast<uint32_t*>(dst) = pack_bf16(a0 * inv, a1 * inv);
 }
 
@@ -285,7 +284,6 @@ __global__ void __launch_bounds__(kNormThreads) k_resid_norm(const __nv_bfloat16
     if (b < 0) return;
     const int r = replica_of_pos(W.sched, pos);
     const __nv_bfloat16* g = reinterpret_cast<const __nv_bfloat16*>(tab->rep[r].blob + D.off_g2);
-    const size_t plane = (size_t)D.gu.KB * D.Mpad * 128;
     float4 v[kMaxVecPerThread];
     float ss = 0.f;
 #pragma unroll
@@ -293,11 +291,11 @@ __global__ void __launch_bounds__(kNormThreads) k_resid_norm(const __nv_bfloat16
         const int col = (it * kNormThreads + threadIdx.x) * 4;
         if (col >= D.d) break;
         const int t = col >> 7, f = col & 127;
-        int p0, p1;
-        cc_tile_pieces(D.o, t, p0, p1);
+        int p0, np;
+        cc_tile_pieces(D.o, t, p0, np);
         float4 acc = make_float4(0.f, 0.f, 0.f, 0.f);
-        for (int p = p0; p <= p1; ++p) {
-            const float4 q = *reinterpret_cast<const float4*>(W.o_part + ((size_t)p * D.Mpad + pos) * 128 + f);
+        for (int i = 0; i < np; ++i) {
+            const float4 q = *reinterpret_cast<const float4*>(W.o_part + ((size_t)(p0 + i * CC_G) * D.Mpad + pos) * 128 + f);
             acc.x += q.x; acc.y += q.y; acc.z += q.z; acc.w += q.w;
         }
         const uint2 hb = *reinterpret_cast<const uint2*>(hidden + (size_t)b * D.d + col);
@@ -316,9 +314,9 @@ __global__ void __launch_bounds__(kNormThreads) k_resid_norm(const __nv_bfloat16
         uint32_t hi0, lo0, hi1, lo1;
         split_hilo(v[it].x * inv * bf16lo(gb.x), v[it].y * inv * bf16hi(gb.x), hi0, lo0);
         split_hilo(v[it].z * inv * bf16lo(gb.y), v[it].w * inv * bf16hi(gb.y), hi1, lo1);
-        uint8_t* dst = W.y_act + act_chunk_off(pos, col, D.Mpad) + (col & 7) * 2;
+        uint8_t* dst = W.y_act + act_chunk_off(pos, col, D.Mpad, 2, 0) + (col & 7) * 2;
         *reinterpret_cast<uint2*>(dst) = make_uint2(hi0, hi1);
-        *reinterpret_cast<uint2*>(dst + plane) = make_uint2(lo0, lo1);
+        *reinterpret_cast<uint2*>(dst + 1024) = make_uint2(lo0, lo1);
     }
 }
 
@@ -334,11 +332,11 @@ __global__ void __launch_bounds__(32 * kEpiRows) k_swiglu(CcDims D, CcWork W) {
     if (pos >= W.sched->n_pos) return;
     if (W.perm[pos] < 0) return;
     const int f = threadIdx.x * 4;
-    int p0, p1;
-    cc_tile_pieces(D.gu, t, p0, p1);
+    int p0, np;
+    cc_tile_pieces(D.gu, t, p0, np);
     float4 acc = make_float4(0.f, 0.f, 0.f, 0.f);
-    for (int p = p0; p <= p1; ++p) {
-        const float4 q = *reinterpret_cast<const float4*>(W.gu_part + ((size_t)p * D.Mpad + pos) * 128 + f);
+    for (int i = 0; i < np; ++i) {
+        const float4 q = *reinterpret_cast<const float4*>(W.gu_part + ((size_t)(p0 + i * CC_G) * D.Mpad + pos) * 128 + f);
         acc.x += q.x; acc.y += q.y; acc.z += q.z; acc.w += q.w;
     }
     const float a0 = acc.x / (1.f + __expf(-acc.x)) * acc.y;
@@ -346,10 +344,10 @@ __global__ void __launch_bounds__(32 * kEpiRows) k_swiglu(CcDims D, CcWork W) {
     uint32_t hi, lo;
     split_hilo(a0, a1, hi, lo);
     const int k = t * 64 + threadIdx.x * 2;                 // output index (K index of the down GEMM)
-    const size_t plane = (size_t)D.dn.KB * D.Mpad * 128;
-    uint8_t* dst = W.a_act + act_chunk_off(pos, k, D.Mpad) + (k & 7) * 2;
+    if (k >= D.dn.KB * CC_TILE_K) return;                   // padding tiles of the last super tile
+    uint8_t* dst = W.a_act + act_chunk_off(pos, k, D.Mpad, 2, 0) + (k & 7) * 2;
     *reinterpret_cast<uint32_t*>(dst) = hi;
-    *reinterpret_cast<uint32_t*>(dst + plane) = lo;
+    *reinterpret_cast<uint32_t*>(dst + 1024) = lo;
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -365,12 +363,12 @@ __global__ void __launch_bounds__(32 * kEpiRows) k_final(__nv_bfloat16* __restri
     if (b < 0) return;
     const int f = threadIdx.x * 4, col = t * 128 + f;
     if (col >= D.d) return;
-    int p0, p1;
-    cc_tile_pieces(D.dn, t, p0, p1);
+    int p0, np;
+    cc_tile_pieces(D.dn, t, p0, np);
     float4 acc = *reinterpret_cast<const float4*>(W.h1 + (size_t)pos * D.d + col);
     float4 sum = make_float4(0.f, 0.f, 0.f, 0.f);
-    for (int p = p0; p <= p1; ++p) {
-        const float4 q = *reinterpret_cast<const float4*>(W.d_part + ((size_t)p * D.Mpad + pos) * 128 + f);
+    for (int i = 0; i < np; ++i) {
+        const float4 q = *reinterpret_cast<const float4*>(W.d_part + ((size_t)(p0 + i * CC_G) * D.Mpad + pos) * 128 + f);
         sum.x += q.x; sum.y += q.y; sum.z += q.z; sum.w += q.w;
     }
     uint2 o;
@@ -380,8 +378,8 @@ __global__ void __launch_bounds__(32 * kEpiRows) k_final(__nv_bfloat16* __restri
 }
 
 // Test tap: widen a workspace buffer to fp32 [batch][dim] in original row order.
-// which: 0 = one bf16 plane, 1 = fp32 rows, 2 = hi + lo planes (plane stride in bytes = `plane`).
-__global__ void __launch_bounds__(256) k_tap(const void* __restrict__ src, int which, int dim, size_t plane, CcDims D,
+// which: 0 = one bf16 plane, 1 = fp32 rows, 2 = hi + lo planes.
+__global__ void __launch_bounds__(256) k_tap(const void* __restrict__ src, int which, int dim, CcDims D,
                                              CcWork W, float* __restrict__ out, int batch) {
     const int pos = blockIdx.x;
     if (pos >= W.sched->n_pos) return;
@@ -392,9 +390,9 @@ __global__ void __launch_bounds__(256) k_tap(const void* __restrict__ src, int w
         if (which == 1) {
             v = reinterpret_cast<const float*>(src)[(size_t)pos * dim + k];
         } else {
-            const uint8_t* p = reinterpret_cast<const uint8_t*>(src) + act_chunk_off(pos, k, D.Mpad) + (k & 7) * 2;
+            const uint8_t* p = reinterpret_cast<const uint8_t*>(src) + act_chunk_off(pos, k, D.Mpad, which == 2 ? 2 : 1, 0) + (k & 7) * 2;
             v = __bfloat162float(*reinterpret_cast<const __nv_bfloat16*>(p));
-            if (which == 2) v += __bfloat162float(*reinterpret_cast<const __nv_bfloat16*>(p + plane));
+            if (which == 2) v += __bfloat162float(*reinterpret_cast<const __nv_bfloat16*>(p + 1024));
         }
         out[(size_t)b * dim + k] = v;
     }
@@ -413,7 +411,7 @@ cudaError_t cc_launch_rmsnorm_in(const __nv_bfloat16* hidden, const CcDims& D, c
 }
 cudaError_t cc_launch_rope_append(const int* seq_lens, const CcKv& kv, const CcDims& D, const CcWork& W,
                                   const CcLaunch& L) {
-    const dim3 grid(D.qkv.T, (D.Mpad + kRopeRows - 1) / kRopeRows), block(64, kRopeRows);
+    const dim3 grid(D.qkv.ST * CC_G, (D.Mpad + kRopeRows - 1) / kRopeRows), block(64, kRopeRows);
     return cc_launch_kernel(k_rope_append, grid, block, 0, L, seq_lens, kv, D, W);
 }
 cudaError_t cc_launch_attn_combine(const int* seq_lens, const CcDims& D, const CcWork& W, const CcLaunch& L) {
@@ -424,16 +422,16 @@ cudaError_t cc_launch_resid_norm(const __nv_bfloat16* hidden, const CcDims& D, c
     return cc_launch_kernel(k_resid_norm, dim3(D.Mpad), dim3(kNormThreads), 0, L, hidden, D, tab, W);
 }
 cudaError_t cc_launch_swiglu(const CcDims& D, const CcWork& W, const CcLaunch& L) {
-    const dim3 grid(D.gu.T, (D.Mpad + kEpiRows - 1) / kEpiRows), block(32, kEpiRows);
+    const dim3 grid(D.gu.ST * CC_G, (D.Mpad + kEpiRows - 1) / kEpiRows), block(32, kEpiRows);
     return cc_launch_kernel(k_swiglu, grid, block, 0, L, D, W);
 }
 cudaError_t cc_launch_final(__nv_bfloat16* hidden, const CcDims& D, const CcWork& W, const CcLaunch& L) {
-    const dim3 grid(D.dn.T, (D.Mpad + kEpiRows - 1) / kEpiRows), block(32, kEpiRows);
+    const dim3 grid(D.dn.ST * CC_G, (D.Mpad + kEpiRows - 1) / kEpiRows), block(32, kEpiRows);
     return cc_launch_kernel(k_final, grid, block, 0, L, hidden, D, W);
 }
-cudaError_t cc_launch_tap(const void* src, int which, int dim, size_t plane, const CcDims& D, const CcWork& W,
+cudaError_t cc_launch_tap(const void* src, int which, int dim, const CcDims& D, const CcWork& W,
                           float* out_dev, int batch, cudaStream_t st) {
-    k_tap<<<D.Mpad, 256, 0, st>>>(src, which, dim, plane, D, W, out_dev, batch);
+    k_tap<<<D.Mpad, 256, 0, st>>>(src, which, dim, D, W, out_dev, batch);
     return cudaGetLastError();
 }
 int cc_max_hidden() { return kMaxVecPerThread * 4 * kNormThreads; }
