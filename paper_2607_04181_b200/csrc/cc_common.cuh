@@ -154,6 +154,25 @@ __device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
         if (++spins > (1u << 26)) __trap();
     }
 }
+// One lane of a fully converged warp (elect.sync).  Code under `if (elect_one())` in warp-uniform
+// control flow keeps its operands in uniform registers, so single-thread instructions (UBLKCP,
+// UTCHMMA, UTCBAR) are issued directly; under `if (lane == 0)` the compiler wraps every one of them
+// in an ELECT / R2UR.BROADCAST / BRA.U.ANY waterfall loop (~100 cycles per tcgen05.mma, measured).
+__device__ __forceinline__ bool elect_one() {
+    uint32_t pred;
+    asm volatile(
+        "{\n\t.reg .pred p;\n\t"
+        "elect.sync _|p, 0xffffffff;\n\t"
+        "selp.u32 %0, 1, 0, p;\n\t}"
+        : "=r"(pred));
+    return pred != 0;
+}
+// Tell the compiler a value is warp-uniform (broadcast from lane 0).
+__device__ __forceinline__ int uniform(int v) { return __shfl_sync(0xffffffffu, v, 0); }
+__device__ __forceinline__ uint32_t uniform(uint32_t v) { return __shfl_sync(0xffffffffu, v, 0); }
+__device__ __forceinline__ const uint8_t* uniform(const uint8_t* p) {
+    return reinterpret_cast<const uint8_t*>(__shfl_sync(0xffffffffu, reinterpret_cast<unsigned long long>(p), 0));
+}
 // Programmatic dependent launch: wait for the preceding kernel's memory / let the next one start.
 __device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
 __device__ __forceinline__ void pdl_launch_dependents() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }

@@ -46,7 +46,7 @@ k_gemm(CcGemmGeo G, const uint8_t* __restrict__ act, int planes, float* __restri
        const CcLayerTable* __restrict__ tab, const CcSched* __restrict__ sched) {
     extern __shared__ __align__(1024) uint8_t smem_raw[];
     GemmSmemHdr* H = reinterpret_cast<GemmSmemHdr*>(smem_raw);
-    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int warp = uniform((int)(threadIdx.x >> 5)), lane = threadIdx.x & 31;
 
     // ---- one-time setup (independent of the previous kernel: overlaps its tail under PDL) ----
     if (threadIdx.x == 0) {
@@ -74,7 +74,7 @@ k_gemm(CcGemmGeo G, const uint8_t* __restrict__ act, int planes, float* __restri
     __syncthreads();
     tc_fence_after();
 
-    const int nmax = sched->nmax;
+    const int nmax = uniform(sched->nmax);
     const uint32_t act_bytes_max = (uint32_t)planes * (uint32_t)nmax * 128u;   // nmax % 16 == 0 => multiple of 2 KiB
     const uint32_t stage_bytes = kWStage + act_bytes_max;
     uint8_t* stage0 = smem_raw + 1024;                      // header occupies the first KiB
@@ -86,7 +86,7 @@ k_gemm(CcGemmGeo G, const uint8_t* __restrict__ act, int planes, float* __restri
     const uint32_t acc_cols = nmax <= 128 ? 128u : 256u;
 
     const long long u_begin = cc_range_begin(G, blockIdx.x), u_end = cc_range_begin(G, blockIdx.x + 1);
-    const uint32_t tmem_base = H->tmem_base;
+    const uint32_t tmem_base = uniform(H->tmem_base);
 
     const int kb_begin = (int)(u_begin % G.KB);
     if (nmax > 0 && u_begin < u_end) {
@@ -104,7 +104,7 @@ k_gemm(CcGemmGeo G, const uint8_t* __restrict__ act, int planes, float* __restri
             const size_t kb_stride = (size_t)(Mpad >> 3) * planes * 1024;   // bytes between k-blocks of the operand
             const long long per_rep = u_end - u_begin;
             int n_act = 0;
-            for (int r = 0; r < CC_MAXR; ++r) n_act += H->cnt[r] > 0;
+            for (int r = 0; r < CC_MAXR; ++r) n_act += uniform(H->cnt[r]) > 0;
             const long long total = per_rep * n_act;
             const int n_pre = total < n_stages ? (int)total : n_stages;
             auto run = [&](const int mode) {
@@ -113,19 +113,19 @@ k_gemm(CcGemmGeo G, const uint8_t* __restrict__ act, int planes, float* __restri
                 uint8_t* sW = stage0;
                 long long idx = 0;
                 for (int r = 0; r < CC_MAXR; ++r) {
-                    const int cnt = H->cnt[r];
+                    const int cnt = uniform(H->cnt[r]);
                     if (cnt == 0) continue;
                     const uint32_t nb = (uint32_t)((cnt + 15) & ~15) * 128u * (uint32_t)planes;   // bytes of one slab
                     const uint32_t tx = kWStage + nb;
-                    const uint8_t* wsrc = H->blob[r] + G.w_off + (size_t)u_begin * kWStage;
-                    const uint8_t* abase = act + (size_t)(H->goff[r] >> 3) * planes * 1024;
+                    const uint8_t* wsrc = uniform(H->blob[r]) + G.w_off + (size_t)u_begin * kWStage;
+                    const uint8_t* abase = act + (size_t)(uniform(H->goff[r]) >> 3) * planes * 1024;
                     const uint8_t* asrc = abase + (size_t)kb_begin * kb_stride;
                     int kb = kb_begin;
                     for (long long u = u_begin; u < u_end; ++u, ++idx) {
                         if (mode == 0 && idx >= n_pre) return;
                         const bool pre = idx < n_pre;            // stage already holds its weights
                         if (mode == 1 && !pre) mbar_wait(&H->empty[stage], ph ^ 1);
-                        if (lane == 0) {
+                        if (elect_one()) {
                             if (mode == 0 || !pre) {
                                 mbar_expect_tx(&H->full[stage], tx);
                                 bulk_g2s_hint(sW, wsrc, kWStage, &H->full[stage], pol_w);
@@ -142,7 +142,7 @@ k_gemm(CcGemmGeo G, const uint8_t* __restrict__ act, int planes, float* __restri
             };
             run(0);
             pdl_wait();
-            if (lane == 0) pdl_launch_dependents();
+            if (elect_one()) pdl_launch_dependents();
             run(1);
         } else if (warp == 1) {
             // ===================== MMA issuer =====================
@@ -155,7 +155,7 @@ k_gemm(CcGemmGeo G, const uint8_t* __restrict__ act, int planes, float* __restri
             const uint32_t dstage = stage_bytes >> 4, dact = kWStage >> 4;
             uint32_t da = desc_lo0;
             for (int r = 0; r < CC_MAXR; ++r) {
-                const int cnt = H->cnt[r];
+                const int cnt = uniform(H->cnt[r]);
                 if (cnt == 0) continue;
                 const uint32_t idesc = umma_idesc_bf16_m128((uint32_t)((cnt + 15) & ~15));
                 int kb = kb_begin;
@@ -169,7 +169,7 @@ k_gemm(CcGemmGeo G, const uint8_t* __restrict__ act, int planes, float* __restri
                     }
                     mbar_wait(&H->full[stage], ph);
                     tc_fence_after();
-                    if (lane == 0) {
+                    if (elect_one()) {
                         const uint32_t db = da + dact;
 #pragma unroll
                         for (int j = 0; j < CC_G; ++j) {
