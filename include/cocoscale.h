@@ -22,6 +22,10 @@
  *     No exception or abort crosses this boundary.
  *   - One control thread per cc_ctx.  cc_forward only ENQUEUES work (no allocation, no
  *     synchronisation, no host read of device data) and is safe inside stream capture.
+ *   - Forwards of one context must not overlap on the device: enqueue them on ONE stream (or
+ *     order the streams with events).  The GEMM kernels are persistent (one CTA per SM) and their
+ *     CTAs wait for one another in the stream-K fixup; two such grids sharing the SMs could
+ *     starve each other.  Replica copies on the side stream may overlap freely.
  *   - Caller-owned buffers handed to cc_forward (hidden, KV pools, block table, seq_lens,
  *     replica_assign) must keep their addresses while a captured graph that contains the call is
  *     alive ("tensor memory addresses remain constant across iterations").
@@ -184,9 +188,9 @@ cc_status cc_forward_host(cc_layer *layer, void *hidden_host, void *k_pool_dev, 
 /* The same step, launched kernel by kernel with a CUDA event between consecutive kernels (so
  * without programmatic dependent launch), synchronised; stage_ms_host[i] (host, fp32
  * [cc_forward_launch_count]) receives the device time of kernel i in milliseconds, in launch
- * order: grouping, input norm, QKV GEMM, RoPE+append, attention, chunk merge, O GEMM,
- * residual+norm, gate/up GEMM, SwiGLU, down GEMM, residual/write-back.  For per-kernel roofline
- * accounting; not capture-safe. */
+ * order: grouping, input norm, QKV GEMM (+RoPE, KV append), attention, chunk merge, O GEMM
+ * (+residual, norm statistics), gate/up GEMM (+norm scale, SwiGLU), down GEMM (+residual, request
+ * order).  For per-kernel roofline accounting; not capture-safe. */
 cc_status cc_forward_profiled(cc_layer *layer, void *hidden_dev, const cc_kv_pages *kv, const int32_t *seq_lens_dev,
                               const int32_t *replica_assign_dev, int batch, void *stream, float *stage_ms_host);
 
@@ -205,7 +209,7 @@ typedef enum {
     CC_TAP_Q = 1,   /* [batch][Hq*Dh]       q after RoPE (fp32)                                 */
     CC_TAP_O = 2,   /* [batch][Hq*Dh]       attention output (GEMM operand: one bf16 plane)     */
     CC_TAP_H1 = 3,  /* [batch][hidden]      hidden + O-projection (fp32)                        */
-    CC_TAP_Y = 4,   /* [batch][hidden]      post-attention RMSNorm output (bf16 hi + lo)        */
+    CC_TAP_Y = 4,   /* [batch][hidden]      post-attention RMSNorm output (hi + lo operand x 1/rms) */
     CC_TAP_A = 5    /* [batch][ffn]         silu(gate)*up (bf16 hi + lo)                        */
 } cc_tap;
 /* out_host: fp32 [batch][dim] in ORIGINAL row order; padding rows are zero. Synchronous. */

@@ -376,6 +376,11 @@ cc_status cc_create_layer(cc_ctx* ctx, const cc_layer_desc* desc, const cc_layer
     D.off_g1 = blob.take((size_t)D.d * 2);
     D.off_g2 = blob.take((size_t)D.d * 2);
     L->blob_bytes = blob.take(0);
+    if (D.qkv.ST > CC_FLAG_STRIDE || D.o.ST > CC_FLAG_STRIDE || D.gu.ST > CC_FLAG_STRIDE || D.dn.ST > CC_FLAG_STRIDE ||
+        D.Mpad > CC_MAX_MPAD) {
+        delete L;
+        return fail(CC_ERR_INVALID, "shape exceeds the stream-K bookkeeping limits (%d super tiles, %d rows)", CC_FLAG_STRIDE, CC_MAX_MPAD);
+    }
 
     // workspace
     CcWork& W = L->W;
@@ -396,6 +401,8 @@ cc_status cc_create_layer(cc_ctx* ctx, const cc_layer_desc* desc, const cc_layer
     const size_t o_pd = ws.take(part_bytes(D.dn));
     const size_t o_qrot = ws.take(Mp * D.QD * 4);
     const size_t o_h1 = ws.take(Mp * D.d * 4);
+    const size_t o_ssq = ws.take((size_t)((D.d + 127) / 128) * Mp * 4);
+    const size_t o_flags = ws.take((size_t)4 * CC_FLAG_STRIDE * 4);
     const size_t o_atto = ws.take(Mp * D.Hq * W.nch_max * D.Dh * 4);
     const size_t o_attml = ws.take(Mp * D.Hq * W.nch_max * sizeof(float2));
     const size_t o_rope = ws.take((size_t)d.max_position * (D.Dh / 2) * sizeof(float2));
@@ -421,6 +428,7 @@ cc_status cc_create_layer(cc_ctx* ctx, const cc_layer_desc* desc, const cc_layer
     W.qkv_part = (float*)(wb + o_pq); W.o_part = (float*)(wb + o_po); W.gu_part = (float*)(wb + o_pg);
     W.d_part = (float*)(wb + o_pd);
     W.q_rot = (float*)(wb + o_qrot); W.h1 = (float*)(wb + o_h1);
+    W.ssq = (float*)(wb + o_ssq); W.flags = (int*)(wb + o_flags);
     W.att_o = (float*)(wb + o_atto); W.att_ml = (float2*)(wb + o_attml);
     W.rope_cs = (const float2*)(wb + o_rope);
     W.err = ctx->err_dev;
@@ -625,7 +633,7 @@ cc_status cc_replica_blob(cc_layer* L, int replica, const void** blob_dev, size_
 
 // ---- the hot path -------------------------------------------------------------------------------
 namespace {
-constexpr int kForwardLaunches = 12;
+constexpr int kForwardLaunches = 8;
 
 cudaError_t enqueue_forward(cc_layer* L, __nv_bfloat16* hidden, const CcKv& kv, const int* seq_lens, const int* assign,
                             int batch, cudaStream_t st, cudaEvent_t* ev = nullptr) {
@@ -635,23 +643,19 @@ cudaError_t enqueue_forward(cc_layer* L, __nv_bfloat16* hidden, const CcKv& kv, 
     const CcLayerTable* tab = ctx->table_dev + L->row;
     CcLaunch Ln{st, ctx->n_sms, ctx->pdl && ev == nullptr};
     cudaError_t e = cudaSuccess;
-    // a0 grouping | a1 norm | a2 QKV | a3+a4 RoPE + append | a5 attention | a5 chunk merge | a6 O |
-    // a6+a7 residual + norm | a8 gate/up | a8 SwiGLU | a9 down | a9 residual, original row order
+    // a0 grouping | a1 norm | a2 QKV (+ a3 RoPE, a4 append) | a5 attention | a5 chunk merge |
+    // a6 O (+ residual, a7 statistics) | a8 gate/up (+ a7 scale, SwiGLU) | a9 down (+ residual, request order)
     for (int stage = 0; stage < kForwardLaunches && e == cudaSuccess; ++stage) {
         if (ev && (e = cudaEventRecord(ev[stage], st)) != cudaSuccess) break;
         switch (stage) {
             case 0: e = cc_launch_group(assign, seq_lens, batch, D, tab, W, Ln); break;
             case 1: e = cc_launch_rmsnorm_in(hidden, D, tab, W, Ln); break;
-            case 2: e = cc_launch_gemm(0, D, tab, W, Ln); break;
-            case 3: e = cc_launch_rope_append(seq_lens, kv, D, W, Ln); break;
-            case 4: e = cc_launch_attention(seq_lens, kv, D, W, Ln); break;
-            case 5: e = cc_launch_attn_combine(seq_lens, D, W, Ln); break;
-            case 6: e = cc_launch_gemm(1, D, tab, W, Ln); break;
-            case 7: e = cc_launch_resid_norm(hidden, D, tab, W, Ln); break;
-            case 8: e = cc_launch_gemm(2, D, tab, W, Ln); break;
-            case 9: e = cc_launch_swiglu(D, W, Ln); break;
-            case 10: e = cc_launch_gemm(3, D, tab, W, Ln); break;
-            default: e = cc_launch_final(hidden, D, W, Ln); break;
+            case 2: e = cc_launch_gemm(0, D, tab, W, seq_lens, kv, hidden, Ln); break;
+            case 3: e = cc_launch_attention(seq_lens, kv, D, W, Ln); break;
+            case 4: e = cc_launch_attn_combine(seq_lens, D, tab, W, Ln); break;
+            case 5: e = cc_launch_gemm(1, D, tab, W, seq_lens, kv, hidden, Ln); break;
+            case 6: e = cc_launch_gemm(2, D, tab, W, seq_lens, kv, hidden, Ln); break;
+            default: e = cc_launch_gemm(3, D, tab, W, seq_lens, kv, hidden, Ln); break;
         }
     }
     if (ev && e == cudaSuccess) e = cudaEventRecord(ev[kForwardLaunches], st);
@@ -733,7 +737,7 @@ cc_status cc_debug_tap(cc_layer* L, cc_tap which, float* out_host, int batch) {
         case CC_TAP_Q: src = L->W.q_rot; kind = 1; dim = D.QD; break;
         case CC_TAP_O: src = L->W.o_act; kind = 0; dim = D.QD; break;
         case CC_TAP_H1: src = L->W.h1; kind = 1; dim = D.d; break;
-        case CC_TAP_Y: src = L->W.y_act; kind = 2; dim = D.d; break;
+        case CC_TAP_Y: src = L->W.y_act; kind = 3; dim = D.d; break;
         case CC_TAP_A: src = L->W.a_act; kind = 2; dim = D.F; break;
         default: return fail(CC_ERR_INVALID, "unknown tap");
     }

@@ -18,13 +18,17 @@
 //   * warp 0 = producer: 1-D bulk copies (TMA engine, no tensor map) into a ring of smem stages
 //     guarded by mbarriers; warp 1 = MMA issuer (one elected thread, tcgen05.commit frees the
 //     stage); warps 2..5 = epilogue (tcgen05.ld -> fp32 partials in global memory).
-//   * a tile's partial sums ("pieces") are added up in fixed order by the next kernel of the
-//     chain, which also applies the fused epilogue (RoPE, residual + RMSNorm, SwiGLU, ...).
+//   * stream-K fixup inside the kernel: when a CTA has streamed its whole range it signals a
+//     per-super-tile counter; the m CTAs that share a super tile then each add up the m fp32
+//     partials ("pieces", fixed order 0..m-1) of every m-th row and apply the fused epilogue of
+//     the projection (RoPE + KV append | residual + norm statistics + operand packing | SwiGLU |
+//     residual + write-back in request order), so no separate reduce kernel runs between GEMMs.
 #include "cc_kernels.h"
 
 namespace {
 
-constexpr int kGemmThreads = 192;
+constexpr int kGemmThreads = 512;         // warp 0 producer, 1 MMA, 2..5 TMEM epilogue, 6..15 row tables; all 16 in the fixup
+constexpr int kHdrBytes = 8192;           // barriers + per-row tables in front of the stage ring
 constexpr int kMaxStages = 8;
 constexpr int kGemmSmem = 225 * 1024;     // dynamic shared memory per CTA
 constexpr int kTmemCols = 512;
@@ -39,11 +43,194 @@ struct GemmSmemHdr {                      // lives at the start of dynamic smem
     int cnt[CC_MAXR];
     int goff[CC_MAXR];
     const uint8_t* blob[CC_MAXR];
+    int perm[CC_MAX_MPAD];                // original row at grouped position, or -1
+    int aux[CC_MAX_MPAD];                 // QKV: position s-1; gate/up: bits of 1/rms of the row
+    int page[CC_MAX_MPAD];                // QKV: page that holds position s-1, or -1
+};
+static_assert(sizeof(GemmSmemHdr) <= kHdrBytes, "header does not fit");
+
+// ---- fused epilogues of the stream-K fixup -----------------------------------------------------------
+// One warp owns one item = (tile t, grouped row p); lane l holds the four summed output features
+// t*128 + 4l .. 4l+3 of original row b.  Each epilogue is split into `pre` (issue every global load
+// that does not depend on the sum, together with the loads of the partial sums) and `fin` (math +
+// stores), so that one fixup iteration costs one L2 round trip.
+enum { EPI_QKV = 0, EPI_O = 1, EPI_GU = 2, EPI_DN = 3 };
+struct CcEpi {
+    const int* seq_lens;
+    CcKv kv;
+    __nv_bfloat16* hidden;
+};
+struct EpiPre {
+    float4 f0, f1;      // QKV: (cos, sin) x 4; down: h1
+    uint2 u0, u1;       // O: hidden bits, g2 bits
 };
 
+__device__ __forceinline__ int replica_of_pos(const int* cnt, const int* goff, int pos) {
+    int r = 0;
+#pragma unroll
+    for (int i = 1; i < CC_MAXR; ++i)
+        if (cnt[i] > 0 && pos >= goff[i]) r = i;
+    return r;
+}
+__device__ __forceinline__ void split_hilo(float v0, float v1, uint32_t& hi, uint32_t& lo) {
+    hi = pack_bf16(v0, v1);
+    lo = pack_bf16(v0 - bf16lo(hi), v1 - bf16hi(hi));
+}
+
+template <int KIND>
+__device__ __forceinline__ void epi_pre(EpiPre& P, const CcEpi& E, const CcDims& D, const CcWork& W, const GemmSmemHdr* H,
+                                        int t, int p, int b, int lane) {
+    const int col = t * 128 + 4 * lane;
+    if (KIND == EPI_QKV) {
+        if (col < D.QD + D.KD) {
+            const int half = D.Dh >> 1;
+            const float4* cs = reinterpret_cast<const float4*>(W.rope_cs + (size_t)H->aux[p] * half + ((col % D.Dh) % half));
+            P.f0 = cs[0];
+            P.f1 = cs[1];
+        }
+    } else if (KIND == EPI_O) {
+        if (col < D.d) {
+            const uint8_t* blob = H->blob[replica_of_pos(H->cnt, H->goff, p)];
+            P.u0 = *reinterpret_cast<const uint2*>(E.hidden + (size_t)b * D.d + col);
+            P.u1 = *reinterpret_cast<const uint2*>(blob + D.off_g2 + (size_t)col * 2);
+        }
+    } else if (KIND == EPI_DN) {
+        if (col < D.d) P.f0 = *reinterpret_cast<const float4*>(W.h1 + (size_t)p * D.d + col);
+    }
+}
+
+template <int KIND>
+__device__ __forceinline__ void epi_fin(const EpiPre& P, const CcEpi& E, const CcDims& D, const CcWork& W,
+                                        const GemmSmemHdr* H, int t, int p, int b, float4 a, int lane) {
+    const int col = t * 128 + 4 * lane;
+    if (KIND == EPI_QKV) {
+        // a3 + a4: RoPE at position s-1 (rotate-half pairs (i, i + Dh/2), fp64-built cos/sin table), q kept
+        // in fp32, bf16(k), bf16(v) stored into the page slot of position s-1 (PAPER.md:103 local append).
+        const int hl = D.Dh >> 3;                                // lanes per half head: 16 (Dh 128) or 8 (Dh 64)
+        float4 o;                                                // the partner half of the same head
+        o.x = __shfl_xor_sync(0xffffffffu, a.x, hl); o.y = __shfl_xor_sync(0xffffffffu, a.y, hl);
+        o.z = __shfl_xor_sync(0xffffffffu, a.z, hl); o.w = __shfl_xor_sync(0xffffffffu, a.w, hl);
+        if (col >= D.QD + 2 * D.KD) return;                      // padding columns of the last tile
+        const int pos = H->aux[p], i0 = col % D.Dh;
+        if (col < D.QD + D.KD) {                                 // q or k: rotate
+            const float sg = (lane & hl) ? 1.f : -1.f;           // first half: a cos - b sin; second: b cos + a sin
+            a.x = a.x * P.f0.x + sg * o.x * P.f0.y; a.y = a.y * P.f0.z + sg * o.y * P.f0.w;
+            a.z = a.z * P.f1.x + sg * o.z * P.f1.y; a.w = a.w * P.f1.z + sg * o.w * P.f1.w;
+            if (col < D.QD) {
+                *reinterpret_cast<float4*>(W.q_rot + (size_t)p * D.QD + col) = a;
+                return;
+            }
+        }
+        const int page = H->page[p];
+        if (page < 0 || page >= E.kv.n_pages) {
+            if (lane == 0) atomicOr(W.err, CC_DEVERR_BAD_PAGE);
+            return;
+        }
+        const bool is_k = col < D.QD + D.KD;
+        const int hk = (col - D.QD - (is_k ? 0 : D.KD)) / D.Dh;
+        __nv_bfloat16* dst = (is_k ? E.kv.k_pool : E.kv.v_pool) + (((size_t)page * D.Hkv + hk) * CC_PAGE + pos % CC_PAGE) * D.Dh + i0;
+        *reinterpret_cast<uint2*>(dst) = make_uint2(pack_bf16(a.x, a.y), pack_bf16(a.z, a.w));
+    } else if (KIND == EPI_O) {
+        // a6 + first half of a7: h1 = h + O-projection (kept in fp32); sum of squares of this tile's 128
+        // columns (the RMSNorm statistic; the 1/rms factor is applied by the gate/up epilogue, the GEMM
+        // being linear in a per-row scale); operand y' = h1 * g2 as hi + lo planes.
+        float ss = 0.f;
+        if (col < D.d) {
+            a.x += bf16lo(P.u0.x); a.y += bf16hi(P.u0.x); a.z += bf16lo(P.u0.y); a.w += bf16hi(P.u0.y);
+            *reinterpret_cast<float4*>(W.h1 + (size_t)p * D.d + col) = a;
+            ss = (a.x * a.x + a.y * a.y) + (a.z * a.z + a.w * a.w);
+            uint32_t hi0, lo0, hi1, lo1;
+            split_hilo(a.x * bf16lo(P.u1.x), a.y * bf16hi(P.u1.x), hi0, lo0);
+            split_hilo(a.z * bf16lo(P.u1.y), a.w * bf16hi(P.u1.y), hi1, lo1);
+            uint8_t* dst = W.y_act + act_chunk_off(p, col, D.Mpad, 2, 0) + (col & 7) * 2;
+            *reinterpret_cast<uint2*>(dst) = make_uint2(hi0, hi1);
+            *reinterpret_cast<uint2*>(dst + 1024) = make_uint2(lo0, lo1);
+        }
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) ss += __shfl_xor_sync(0xffffffffu, ss, o);
+        if (lane == 0) W.ssq[(size_t)t * D.Mpad + p] = ss;
+    } else if (KIND == EPI_GU) {
+        // second half of a7 + a8: scale by 1/rms of the row, a_j = silu(gate_j) * up_j with gate_j, up_j at
+        // interleaved columns 2j, 2j+1 -> hi + lo operand of the down projection.
+        const float inv = __int_as_float(H->aux[p]);
+        const float g0 = a.x * inv, u0 = a.y * inv, g1 = a.z * inv, u1 = a.w * inv;
+        const int k = t * 64 + 2 * lane;                          // output index = K index of the down GEMM
+        if (k >= D.dn.KB * CC_TILE_K) return;                     // padding tile of the last super tile
+        uint32_t hi, lo;
+        split_hilo(g0 / (1.f + __expf(-g0)) * u0, g1 / (1.f + __expf(-g1)) * u1, hi, lo);
+        uint8_t* dst = W.a_act + act_chunk_off(p, k, D.Mpad, 2, 0) + (k & 7) * 2;
+        *reinterpret_cast<uint32_t*>(dst) = hi;
+        *reinterpret_cast<uint32_t*>(dst + 1024) = lo;
+    } else {
+        // a9: out[b] = bf16(h1 + down projection), written to row b = original request order.
+        if (col >= D.d) return;
+        *reinterpret_cast<uint2*>(E.hidden + (size_t)b * D.d + col) =
+            make_uint2(pack_bf16(P.f0.x + a.x, P.f0.y + a.y), pack_bf16(P.f0.z + a.z, P.f0.w + a.w));
+    }
+}
+
+// Slice of the fixup of super tile `st` done by contributor k of m: rows k, k + m, ... of both tiles.
+// KI items (row, tile) per warp iteration, QU pieces of each loaded per round trip (KI * QU loads in
+// flight per lane); pieces are added in the order 0..m-1 whatever KI and QU are.
+template <int KIND, int KI, int QU>
+__device__ __forceinline__ void fixup_tile(const float* __restrict__ part, const CcEpi& E, const CcDims& D, const CcWork& W,
+                                           const GemmSmemHdr* H, int st, int c0, int m, int k, int n_pos, int warp,
+                                           int lane) {
+    constexpr int kWarps = kGemmThreads / 32;
+    const int Mpad = D.Mpad;
+    const int my_rows = (n_pos - k + m - 1) / m;
+    const int n_items = my_rows * CC_G;
+    const size_t piece_stride = (size_t)CC_G * Mpad * 128;     // floats between consecutive pieces of a tile
+    for (int it0 = warp * KI; it0 < n_items; it0 += kWarps * KI) {
+        const float* src[KI];
+        int pp[KI], bb[KI], tt[KI];
+        float4 acc[KI];
+        EpiPre pre[KI];
+#pragma unroll
+        for (int u = 0; u < KI; ++u) {
+            const int it = it0 + u;
+            const int row = it / CC_G, j = it - row * CC_G;
+            pp[u] = k + row * m;
+            tt[u] = st * CC_G + j;
+            bb[u] = (it < n_items) ? H->perm[pp[u]] : -1;
+            src[u] = part + ((size_t)((c0 + st) * CC_G + j) * Mpad + pp[u]) * 128 + 4 * lane;
+            acc[u] = make_float4(0.f, 0.f, 0.f, 0.f);
+            if (bb[u] >= 0) epi_pre<KIND>(pre[u], E, D, W, H, tt[u], pp[u], bb[u], lane);
+        }
+        for (int q0 = 0; q0 < m; q0 += QU) {
+            float4 v[KI][QU];
+#pragma unroll
+            for (int u = 0; u < KI; ++u)
+#pragma unroll
+                for (int qq = 0; qq < QU; ++qq)
+                    v[u][qq] = (bb[u] >= 0 && q0 + qq < m)
+                                   ? __ldcg(reinterpret_cast<const float4*>(src[u] + (size_t)(q0 + qq) * piece_stride))
+                                   : make_float4(0.f, 0.f, 0.f, 0.f);
+#pragma unroll
+            for (int u = 0; u < KI; ++u)
+#pragma unroll
+                for (int qq = 0; qq < QU; ++qq) {
+                    acc[u].x += v[u][qq].x; acc[u].y += v[u][qq].y; acc[u].z += v[u][qq].z; acc[u].w += v[u][qq].w;
+                }
+        }
+#pragma unroll
+        for (int u = 0; u < KI; ++u)
+            if (bb[u] >= 0) epi_fin<KIND>(pre[u], E, D, W, H, tt[u], pp[u], bb[u], acc[u], lane);   // warp-uniform branch
+    }
+}
+
+__device__ __forceinline__ int ld_acquire(const int* p) {
+    int v;
+    asm volatile("ld.acquire.gpu.global.s32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+    return v;
+}
+
+template <int KIND>
 __global__ void __launch_bounds__(kGemmThreads, 1)
-k_gemm(CcGemmGeo G, const uint8_t* __restrict__ act, int planes, float* __restrict__ part, int Mpad,
-       const CcLayerTable* __restrict__ tab, const CcSched* __restrict__ sched) {
+k_gemm(CcGemmGeo G, const uint8_t* __restrict__ act, int planes, float* __restrict__ part, int* __restrict__ flags,
+       CcEpi E, CcDims D, CcWork W, const CcLayerTable* __restrict__ tab, CcGemmGeo Gnext) {
+    const CcSched* __restrict__ sched = W.sched;
+    const int Mpad = D.Mpad;
     extern __shared__ __align__(1024) uint8_t smem_raw[];
     GemmSmemHdr* H = reinterpret_cast<GemmSmemHdr*>(smem_raw);
     const int warp = uniform((int)(threadIdx.x >> 5)), lane = threadIdx.x & 31;
@@ -77,8 +264,8 @@ k_gemm(CcGemmGeo G, const uint8_t* __restrict__ act, int planes, float* __restri
     const int nmax = uniform(sched->nmax);
     const uint32_t act_bytes_max = (uint32_t)planes * (uint32_t)nmax * 128u;   // nmax % 16 == 0 => multiple of 2 KiB
     const uint32_t stage_bytes = kWStage + act_bytes_max;
-    uint8_t* stage0 = smem_raw + 1024;                      // header occupies the first KiB
-    int n_stages = (kGemmSmem - 1024) / (int)stage_bytes;
+    uint8_t* stage0 = smem_raw + kHdrBytes;                 // barriers and row tables live in front of the ring
+    int n_stages = (kGemmSmem - kHdrBytes) / (int)stage_bytes;
     if (n_stages > kMaxStages) n_stages = kMaxStages;
     // TMEM: accumulator (buf, j) at column buf * 256 + j * acc_cols; one buffer only when the two
     // accumulators of a super tile need more than 256 columns
@@ -144,6 +331,12 @@ k_gemm(CcGemmGeo G, const uint8_t* __restrict__ act, int planes, float* __restri
             pdl_wait();
             if (elect_one()) pdl_launch_dependents();
             run(1);
+            // everything of this GEMM is in flight: warm L2 with the head of the next GEMM's stream
+            if (Gnext.P > 0 && elect_one()) {
+                int r0 = 0;
+                while (r0 < CC_MAXR - 1 && H->cnt[r0] == 0) ++r0;
+                cc_prefetch_gemm_head(Gnext, H->blob[r0], (int)blockIdx.x);
+            }
         } else if (warp == 1) {
             // ===================== MMA issuer =====================
             int stage = 0;
@@ -192,7 +385,7 @@ k_gemm(CcGemmGeo G, const uint8_t* __restrict__ act, int planes, float* __restri
                     if (++stage == n_stages) { stage = 0; ph ^= 1; da = desc_lo0; }
                 }
             }
-        } else {
+        } else if (warp < 6) {
             // ===================== epilogue: TMEM -> fp32 partial pieces =====================
             const int q = warp & 3;                          // TMEM lane quarter this warp may read
             const int f = q * 32 + lane;                     // output feature within the tile
@@ -230,30 +423,91 @@ k_gemm(CcGemmGeo G, const uint8_t* __restrict__ act, int planes, float* __restri
                     u = u_next;
                 }
             }
+        } else {
+            // ===================== helper warps: per-row tables of the fused epilogue =====================
+            // built while the weights stream; the rows' statistics come from the previous kernel
+            pdl_wait();
+            const int n_pos = sched->n_pos;
+            for (int p = (int)threadIdx.x - 6 * 32; p < n_pos; p += kGemmThreads - 6 * 32) {
+                const int b = W.perm[p];
+                H->perm[p] = b;
+                if (KIND == EPI_QKV) {
+                    int pos = -1, page = -1;
+                    if (b >= 0) {
+                        pos = E.seq_lens[b] - 1;
+                        page = E.kv.block_table[(size_t)b * D.max_blocks + pos / CC_PAGE];
+                    }
+                    H->aux[p] = pos;
+                    H->page[p] = page;
+                } else if (KIND == EPI_GU) {
+                    float ss = 0.f;
+                    if (b >= 0) {
+                        const int nt = (D.d + 127) >> 7;
+                        for (int t = 0; t < nt; ++t) ss += W.ssq[(size_t)t * Mpad + p];   // tile order: fixed
+                    }
+                    H->aux[p] = __float_as_int(rsqrtf(ss / (float)D.d + D.eps));
+                }
+            }
         }
     }
+    __threadfence();                      // partial sums of this CTA are visible GPU-wide before the signal
     tc_fence_before();
     __syncthreads();
     if (warp == 1) tmem_dealloc<kTmemCols>(tmem_base);
+    if (nmax == 0) return;
+
+    // ---- stream-K fixup: the CTAs c0..c1 whose ranges meet in a super tile split its rows ----------
+    // Every reduction below adds pieces 0..m-1 in that order, whatever CTA does it and whatever the
+    // replica split.  All CTAs of the grid are co-resident (one per SM, P <= SMs), and
+    // each signals before it waits, so the waits are short and cannot deadlock.
+    const int n_pos = uniform(sched->n_pos);
+    const int st_first = (int)(u_begin / G.KB), st_last = (int)((u_end - 1) / G.KB);
+    if (threadIdx.x == 0) {
+        __threadfence();
+        for (int st = st_first; st <= st_last; ++st) atomicAdd(&flags[st], 1);
+    }
+    for (int st = st_first; st <= st_last; ++st) {
+        const int c0 = cc_range_of_unit(G, (long long)st * G.KB);
+        const int c1 = cc_range_of_unit(G, (long long)(st + 1) * G.KB - 1);
+        const int m = c1 - c0 + 1, k = (int)blockIdx.x - c0;
+        if (threadIdx.x == 0) {
+            uint32_t spins = 0;
+            while (ld_acquire(&flags[st]) < m) {
+                __nanosleep(40);
+                if (++spins > (1u << 24)) __trap();
+            }
+        }
+        __syncthreads();
+        // few contributors: several items per warp; many: one item, its pieces loaded together
+        if (m <= 3) fixup_tile<KIND, 4, 3>(part, E, D, W, H, st, c0, m, k, n_pos, warp, lane);
+        else if (m <= 8) fixup_tile<KIND, 2, 4>(part, E, D, W, H, st, c0, m, k, n_pos, warp, lane);
+        else fixup_tile<KIND, 1, 8>(part, E, D, W, H, st, c0, m, k, n_pos, warp, lane);
+    }
 }
 
 }  // namespace
 
 cudaError_t cc_gemm_configure() {
-    return cudaFuncSetAttribute(k_gemm, cudaFuncAttributeMaxDynamicSharedMemorySize, kGemmSmem);
+    cudaError_t e = cudaFuncSetAttribute(k_gemm<EPI_QKV>, cudaFuncAttributeMaxDynamicSharedMemorySize, kGemmSmem);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_gemm<EPI_O>, cudaFuncAttributeMaxDynamicSharedMemorySize, kGemmSmem);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_gemm<EPI_GU>, cudaFuncAttributeMaxDynamicSharedMemorySize, kGemmSmem);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_gemm<EPI_DN>, cudaFuncAttributeMaxDynamicSharedMemorySize, kGemmSmem);
+    return e;
 }
 
-cudaError_t cc_launch_gemm(int which, const CcDims& D, const CcLayerTable* tab, const CcWork& W, const CcLaunch& L) {
-    const CcGemmGeo* G;
-    const uint8_t* act;
-    float* part;
-    int planes = 2;   // hi + lo activation planes; the O projection's input needs one
+// which: 0 = QKV, 1 = O, 2 = gate/up, 3 = down
+cudaError_t cc_launch_gemm(int which, const CcDims& D, const CcLayerTable* tab, const CcWork& W, const int* seq_lens,
+                           const CcKv& kv, __nv_bfloat16* hidden, const CcLaunch& L) {
+    const dim3 block(kGemmThreads);
+    const size_t smem = (size_t)kGemmSmem;
+    CcEpi E{seq_lens, kv, hidden};
+    int* flags = W.flags + which * CC_FLAG_STRIDE;
+    CcGemmGeo none{};   // P = 0: nothing to prefetch (attention / the next layer follows)
+    // hi + lo activation planes; the O projection's input needs one
     switch (which) {
-        case 0: G = &D.qkv; act = W.x_act; part = W.qkv_part; break;
-        case 1: G = &D.o; act = W.o_act; part = W.o_part; planes = 1; break;
-        case 2: G = &D.gu; act = W.y_act; part = W.gu_part; break;
-        default: G = &D.dn; act = W.a_act; part = W.d_part; break;
+        case 0: return cc_launch_kernel(k_gemm<EPI_QKV>, dim3(D.qkv.P), block, smem, L, D.qkv, W.x_act, 2, W.qkv_part, flags, E, D, W, tab, none);
+        case 1: return cc_launch_kernel(k_gemm<EPI_O>, dim3(D.o.P), block, smem, L, D.o, W.o_act, 1, W.o_part, flags, E, D, W, tab, D.gu);
+        case 2: return cc_launch_kernel(k_gemm<EPI_GU>, dim3(D.gu.P), block, smem, L, D.gu, W.y_act, 2, W.gu_part, flags, E, D, W, tab, D.dn);
+        default: return cc_launch_kernel(k_gemm<EPI_DN>, dim3(D.dn.P), block, smem, L, D.dn, W.a_act, 2, W.d_part, flags, E, D, W, tab, none);
     }
-    return cc_launch_kernel(k_gemm, dim3(G->P), dim3(kGemmThreads), (size_t)kGemmSmem, L, *G, act, planes, part, D.Mpad,
-                            tab, W.sched);
 }

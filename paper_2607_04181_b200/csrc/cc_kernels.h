@@ -17,6 +17,8 @@ struct CcWork {
     float* d_part;
     float* q_rot;        // [Mpad][Hq*Dh] fp32, q after RoPE
     float* h1;           // [Mpad][d]     fp32, hidden + O projection
+    float* ssq;          // [d/128][Mpad] fp32, per-tile sum of squares of h1 (post-attention RMSNorm statistic)
+    int* flags;          // [4][CC_FLAG_STRIDE] stream-K fixup counters, zeroed by k_group every step
     float* att_o;        // [Mpad*Hq][nch_max][Dh] fp32 un-normalised chunk outputs
     float2* att_ml;      // [Mpad*Hq][nch_max] (max in log2 units, sum)
     const float2* rope_cs;  // [max_position][Dh/2] (cos, sin), built in fp64 on the host
@@ -44,16 +46,12 @@ cudaError_t cc_launch_group(const int* assign, const int* seq_lens, int batch, c
 cudaError_t cc_launch_rmsnorm_in(const __nv_bfloat16* hidden, const CcDims& D, const CcLayerTable* tab,
                                  const CcWork& W, const CcLaunch& L);
 // which: 0 = QKV, 1 = O, 2 = gate/up, 3 = down
-cudaError_t cc_launch_gemm(int which, const CcDims& D, const CcLayerTable* tab, const CcWork& W, const CcLaunch& L);
-cudaError_t cc_launch_rope_append(const int* seq_lens, const CcKv& kv, const CcDims& D, const CcWork& W,
-                                  const CcLaunch& L);
+cudaError_t cc_launch_gemm(int which, const CcDims& D, const CcLayerTable* tab, const CcWork& W, const int* seq_lens,
+                           const CcKv& kv, __nv_bfloat16* hidden, const CcLaunch& L);
 cudaError_t cc_launch_attention(const int* seq_lens, const CcKv& kv, const CcDims& D, const CcWork& W,
                                 const CcLaunch& L);
-cudaError_t cc_launch_attn_combine(const int* seq_lens, const CcDims& D, const CcWork& W, const CcLaunch& L);
-cudaError_t cc_launch_resid_norm(const __nv_bfloat16* hidden, const CcDims& D, const CcLayerTable* tab,
-                                 const CcWork& W, const CcLaunch& L);
-cudaError_t cc_launch_swiglu(const CcDims& D, const CcWork& W, const CcLaunch& L);
-cudaError_t cc_launch_final(__nv_bfloat16* hidden, const CcDims& D, const CcWork& W, const CcLaunch& L);
+cudaError_t cc_launch_attn_combine(const int* seq_lens, const CcDims& D, const CcLayerTable* tab, const CcWork& W,
+                                   const CcLaunch& L);
 
 cudaError_t cc_launch_copy(void* dst, const void* src, size_t bytes, int n_sms, cudaStream_t st);
 cudaError_t cc_launch_publish(CcLayerTable* row_dev, const CcLayerTable& value, cudaStream_t st);
@@ -61,7 +59,8 @@ cudaError_t cc_launch_publish(CcLayerTable* row_dev, const CcLayerTable& value, 
 cudaError_t cc_launch_pack(uint8_t* dst, const __nv_bfloat16* src0, const __nv_bfloat16* src1,
                            const __nv_bfloat16* src2, int rows0, int rows1, int rows2, int mode, int K, int n_tiles,
                            int k_blocks, cudaStream_t st);
-// which: 0 = one packed bf16 plane (K = dim), 1 = fp32 row buffer [Mpad][dim], 2 = hi + lo planes
+// which: 0 = one packed bf16 plane (K = dim), 1 = fp32 row buffer [Mpad][dim], 2 = hi + lo planes,
+// 3 = hi + lo planes scaled by the row's 1/rms from W.ssq (the un-normalised y' operand)
 cudaError_t cc_launch_tap(const void* src, int which, int dim, const CcDims& D, const CcWork& W,
                           float* out_dev, int batch, cudaStream_t st);
 int cc_max_hidden();
