@@ -29,6 +29,9 @@ __device__ __forceinline__ void st_stream32(u32x8* p, const u32x8& r) {
 // n32 = number of 32-byte words; the (< 32 byte) remainder is copied as 16-byte words by block 0.
 __global__ void __launch_bounds__(kCopyThreads) k_copy(u32x8* __restrict__ dst, const u32x8* __restrict__ src, size_t n32,
                                                        int tail16) {
+    // Chunks are independent: let the next chunk's kernel start while this one drains (programmatic
+    // dependent launch on the side stream) ...
+    pdl_launch_dependents();
     const size_t span = (size_t)kCopyThreads * kCopyUnroll;
     const size_t stride = (size_t)gridDim.x * span;
     size_t base = (size_t)blockIdx.x * span;
@@ -44,6 +47,9 @@ __global__ void __launch_bounds__(kCopyThreads) k_copy(u32x8* __restrict__ dst, 
     }
     if (tail16 && blockIdx.x == 0 && threadIdx.x == 0)
         reinterpret_cast<uint4*>(dst + n32)[0] = reinterpret_cast<const uint4*>(src + n32)[0];
+    // ... but do not retire before the previous chunk has: the event recorded after the last chunk
+    // then covers every chunk of the replica.
+    pdl_wait();
 }
 
 // a12: the flip.  One thread rewrites the layer's table row; ordering comes from the stream.
@@ -93,9 +99,9 @@ cudaError_t cc_launch_copy(void* dst, const void* src, size_t bytes, int n_sms, 
     if (blocks == 0) blocks = 1;
     const size_t cap = (size_t)n_sms * 4;   // 4 resident blocks of 512 threads per SM
     if (blocks > cap) blocks = cap;
-    k_copy<<<(unsigned)blocks, kCopyThreads, 0, st>>>(reinterpret_cast<u32x8*>(dst), reinterpret_cast<const u32x8*>(src), n32,
-                                                      tail16);
-    return cudaGetLastError();
+    CcLaunch L{st, n_sms, true};
+    return cc_launch_kernel(k_copy, dim3((unsigned)blocks), dim3(kCopyThreads), 0, L, reinterpret_cast<u32x8*>(dst),
+                            reinterpret_cast<const u32x8*>(src), n32, tail16);
 }
 cudaError_t cc_launch_publish(CcLayerTable* row_dev, const CcLayerTable& value, cudaStream_t st) {
     k_publish<<<1, 1, 0, st>>>(row_dev, value);
