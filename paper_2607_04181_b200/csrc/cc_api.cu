@@ -385,6 +385,10 @@ cc_status cc_create_layer(cc_ctx* ctx, const cc_layer_desc* desc, const cc_layer
     // workspace
     CcWork& W = L->W;
     W.nch_max = (d.max_position + CC_ATTN_CHUNK - 1) / CC_ATTN_CHUNK;
+    if ((long long)d.max_batch * W.nch_max >= 65536) {
+        delete L;
+        return fail(CC_ERR_INVALID, "max_batch * ceil(max_position / %d) must stay below 65536 attention work items", CC_ATTN_CHUNK);
+    }
     Carver ws;
     const size_t Mp = (size_t)D.Mpad;
     const size_t o_sched = ws.take(sizeof(CcSched));
@@ -403,6 +407,8 @@ cc_status cc_create_layer(cc_ctx* ctx, const cc_layer_desc* desc, const cc_layer
     const size_t o_h1 = ws.take(Mp * D.d * 4);
     const size_t o_ssq = ws.take((size_t)((D.d + 127) / 128) * Mp * 4);
     const size_t o_flags = ws.take((size_t)4 * CC_FLAG_STRIDE * 4);
+    const size_t o_actr = ws.take(64);
+    const size_t o_acnt = ws.take(Mp * D.Hkv * 4);
     const size_t o_atto = ws.take(Mp * D.Hq * W.nch_max * D.Dh * 4);
     const size_t o_attml = ws.take(Mp * D.Hq * W.nch_max * sizeof(float2));
     const size_t o_rope = ws.take((size_t)d.max_position * (D.Dh / 2) * sizeof(float2));
@@ -429,6 +435,7 @@ cc_status cc_create_layer(cc_ctx* ctx, const cc_layer_desc* desc, const cc_layer
     W.d_part = (float*)(wb + o_pd);
     W.q_rot = (float*)(wb + o_qrot); W.h1 = (float*)(wb + o_h1);
     W.ssq = (float*)(wb + o_ssq); W.flags = (int*)(wb + o_flags);
+    W.attn_ctr = (int*)(wb + o_actr); W.attn_cnt = (int*)(wb + o_acnt);
     W.att_o = (float*)(wb + o_atto); W.att_ml = (float2*)(wb + o_attml);
     W.rope_cs = (const float2*)(wb + o_rope);
     W.err = ctx->err_dev;
@@ -633,7 +640,7 @@ cc_status cc_replica_blob(cc_layer* L, int replica, const void** blob_dev, size_
 
 // ---- the hot path -------------------------------------------------------------------------------
 namespace {
-constexpr int kForwardLaunches = 8;
+constexpr int kForwardLaunches = 7;
 
 cudaError_t enqueue_forward(cc_layer* L, __nv_bfloat16* hidden, const CcKv& kv, const int* seq_lens, const int* assign,
                             int batch, cudaStream_t st, cudaEvent_t* ev = nullptr) {
@@ -643,7 +650,7 @@ cudaError_t enqueue_forward(cc_layer* L, __nv_bfloat16* hidden, const CcKv& kv, 
     const CcLayerTable* tab = ctx->table_dev + L->row;
     CcLaunch Ln{st, ctx->n_sms, ctx->pdl && ev == nullptr};
     cudaError_t e = cudaSuccess;
-    // a0 grouping | a1 norm | a2 QKV (+ a3 RoPE, a4 append) | a5 attention | a5 chunk merge |
+    // a0 grouping | a1 norm | a2 QKV (+ a3 RoPE, a4 append) | a5 attention (+ chunk merge) |
     // a6 O (+ residual, a7 statistics) | a8 gate/up (+ a7 scale, SwiGLU) | a9 down (+ residual, request order)
     for (int stage = 0; stage < kForwardLaunches && e == cudaSuccess; ++stage) {
         if (ev && (e = cudaEventRecord(ev[stage], st)) != cudaSuccess) break;
@@ -651,10 +658,9 @@ cudaError_t enqueue_forward(cc_layer* L, __nv_bfloat16* hidden, const CcKv& kv, 
             case 0: e = cc_launch_group(assign, seq_lens, batch, D, tab, W, Ln); break;
             case 1: e = cc_launch_rmsnorm_in(hidden, D, tab, W, Ln); break;
             case 2: e = cc_launch_gemm(0, D, tab, W, seq_lens, kv, hidden, Ln); break;
-            case 3: e = cc_launch_attention(seq_lens, kv, D, W, Ln); break;
-            case 4: e = cc_launch_attn_combine(seq_lens, D, tab, W, Ln); break;
-            case 5: e = cc_launch_gemm(1, D, tab, W, seq_lens, kv, hidden, Ln); break;
-            case 6: e = cc_launch_gemm(2, D, tab, W, seq_lens, kv, hidden, Ln); break;
+            case 3: e = cc_launch_attention(seq_lens, kv, D, tab, W, Ln); break;
+            case 4: e = cc_launch_gemm(1, D, tab, W, seq_lens, kv, hidden, Ln); break;
+            case 5: e = cc_launch_gemm(2, D, tab, W, seq_lens, kv, hidden, Ln); break;
             default: e = cc_launch_gemm(3, D, tab, W, seq_lens, kv, hidden, Ln); break;
         }
     }

@@ -12,8 +12,12 @@
 //   * pages land in smem XOR-swizzled at 16-byte granularity, so the ldmatrix reads of the
 //     K (B operand of q.K^T) and V (transposed B operand of p.V) fragments are conflict-free;
 //   * softmax is online per warp (running max / sum in log2 units, fp32), the 4 warps of a CTA
-//     are merged in fixed order through smem, chunks are merged in fixed order by
-//     k_attn_combine.  The chunking depends on seq_len only => bit-identical across replicas.
+//     are merged in fixed order through smem; the chunk partials of one (row, kv head) are merged
+//     in chunk order by whichever CTA finishes that pair's last chunk (a counter per pair), so no
+//     separate combine kernel runs.  The chunking depends on seq_len only and every merge order
+//     is fixed => bit-identical across replicas, whatever CTA does the work.
+//   * CTAs draw work items from a device counter (first item static), full chunks first and the
+//     ragged last chunks at the end of the list, which evens out the tail of the kernel.
 #include "cc_kernels.h"
 
 namespace {
@@ -32,7 +36,7 @@ struct AttnCfg {
     static constexpr int kChunksPerRow = DH / 8;               // 16-byte chunks per token row
     static constexpr int kMergeStride = DH + 2;                // floats per (warp, head): o[DH], m, l
     static size_t smem_bytes(int G) {
-        return (size_t)kAttnWarps * kAttnStages * kStageBytes + (size_t)kAttnWarps * G * kMergeStride * 4;
+        return (size_t)kAttnWarps * kAttnStages * kStageBytes + (size_t)kAttnWarps * G * kMergeStride * 4 + 32;
     }
 };
 
@@ -42,7 +46,7 @@ struct ItemMeta {
 
 template <int DH>
 __global__ void __launch_bounds__(kAttnThreads, 2)
-k_attn(const int* __restrict__ seq_lens, CcKv kv, CcDims D, CcWork W) {
+k_attn(const int* __restrict__ seq_lens, CcKv kv, CcDims D, CcWork W, const CcLayerTable* __restrict__ tab) {
     using C = AttnCfg<DH>;
     extern __shared__ __align__(1024) uint8_t smem_raw[];
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
@@ -51,22 +55,33 @@ k_attn(const int* __restrict__ seq_lens, CcKv kv, CcDims D, CcWork W) {
     float* merge = reinterpret_cast<float*>(smem_raw + (size_t)kAttnWarps * kAttnStages * C::kStageBytes);
     const uint32_t ring_u32 = smem_u32(ring);
 
+    int* s_seq = reinterpret_cast<int*>(merge + (size_t)kAttnWarps * D.G * C::kMergeStride);   // [4] item ids + [1] flag
     pdl_wait();
     pdl_launch_dependents();
 
     const int G = D.G, Hkv = D.Hkv;
-    const int n_items = W.sched->n_items * Hkv;
-    const int my_items = ((int)blockIdx.x < n_items) ? (n_items - 1 - (int)blockIdx.x) / (int)gridDim.x + 1 : 0;
-    const int n_slots = my_items * kSlotsPerItem;
+    const int n_total = W.sched->n_items * Hkv;
+    // item sequence of this CTA: seq[0] = blockIdx.x, later ones from the counter; seq[n + 2] is drawn
+    // while item n runs, so the loads of the next item can be in flight before the current one ends
+    if (threadIdx.x == 0) {
+        s_seq[0] = (int)blockIdx.x;
+        s_seq[1] = (int)gridDim.x + atomicAdd(W.attn_ctr, 1);
+    }
+    __syncthreads();
 
     // ---- producer side: issue the cp.async copies of page slot k of this warp -------------------
     ItemMeta pm = {0, 0, 0, 0};
-    int p_hk = 0, p_item = -1, p_page_id = 0;      // p_page_id: lane l < 16 holds page id l of the chunk
+    int p_hk = 0, p_item = -1, p_page_id[2] = {0, 0};   // lane l holds the ids of pages l and l + 32 of the chunk
+    static_assert(kPagesPerChunk <= 64, "two page ids per lane");
     auto prefetch = [&](int k) {
         const int it = k / kSlotsPerItem, i = k % kSlotsPerItem;
         if (it != p_item) {
             p_item = it;
-            const int j = (int)blockIdx.x + it * (int)gridDim.x;
+            const int j = s_seq[it & 3];
+            if (j >= n_total) {
+                pm.s = 0;
+                return;
+            }
             const int base = j / Hkv;
             p_hk = j - base * Hkv;
             const int2 rec = W.items[base];
@@ -75,20 +90,24 @@ k_attn(const int* __restrict__ seq_lens, CcKv kv, CcDims D, CcWork W) {
             pm.b = W.perm[rec.x];
             pm.s = seq_lens[pm.b];
             const int n_row_pages = (pm.s + CC_PAGE - 1) / CC_PAGE;
-            const int pg = pm.chunk * kPagesPerChunk + (lane & 15);
-            int id = 0;
-            if (pg < n_row_pages) {
-                id = kv.block_table[(size_t)pm.b * D.max_blocks + pg];
-                if (id < 0 || id >= kv.n_pages) {
-                    atomicOr(W.err, CC_DEVERR_BAD_PAGE);
-                    id = 0;
+#pragma unroll
+            for (int h = 0; h < 2; ++h) {
+                const int pg = pm.chunk * kPagesPerChunk + lane + 32 * h;
+                int id = 0;
+                if (lane + 32 * h < kPagesPerChunk && pg < n_row_pages) {
+                    id = kv.block_table[(size_t)pm.b * D.max_blocks + pg];
+                    if (id < 0 || id >= kv.n_pages) {
+                        atomicOr(W.err, CC_DEVERR_BAD_PAGE);
+                        id = 0;
+                    }
                 }
+                p_page_id[h] = id;
             }
-            p_page_id = id;
         }
         const int pl = warp + i * kAttnWarps;                       // page within the chunk
         const int tok0 = pm.chunk * CC_ATTN_CHUNK + pl * CC_PAGE;   // first token of the page
-        const int page = __shfl_sync(0xffffffffu, p_page_id, pl);
+        const int page0 = __shfl_sync(0xffffffffu, p_page_id[0], pl & 31), page1 = __shfl_sync(0xffffffffu, p_page_id[1], pl & 31);
+        const int page = pl < 32 ? page0 : page1;
         if (tok0 < pm.s) {
             const int valid = min(CC_PAGE, pm.s - tok0);
             const size_t src_off = ((size_t)page * Hkv + p_hk) * (size_t)(CC_PAGE * DH);
@@ -112,7 +131,7 @@ k_attn(const int* __restrict__ seq_lens, CcKv kv, CcDims D, CcWork W) {
     };
 
     for (int k = 0; k < kAttnStages - 1; ++k) {
-        if (k < n_slots) prefetch(k);
+        prefetch(k);
         cp_async_commit();
     }
 
@@ -123,13 +142,16 @@ k_attn(const int* __restrict__ seq_lens, CcKv kv, CcDims D, CcWork W) {
     float o[DH / 8][4];
     float m_run = -INFINITY, l_run = 0.f;
 
-    for (int k = 0; k < n_slots; ++k) {
+    int next_id = 0;                                       // thread 0: the id drawn for seq[it + 2]
+    for (int k = 0;; ++k) {
         const int it = k / kSlotsPerItem, i = k % kSlotsPerItem;
-        if (k + kAttnStages - 1 < n_slots) prefetch(k + kAttnStages - 1);
+        if (i == 0 && s_seq[it & 3] >= n_total) break;     // CTA-uniform: the list is exhausted
+        prefetch(k + kAttnStages - 1);
         cp_async_commit();
 
         if (i == 0) {   // new item: metadata, Q fragments, reset the running softmax state
-            const int j = (int)blockIdx.x + it * (int)gridDim.x;
+            if (threadIdx.x == 0) next_id = (int)gridDim.x + atomicAdd(W.attn_ctr, 1);
+            const int j = s_seq[it & 3];
             const int base = j / Hkv;
             c_hk = j - base * Hkv;
             const int2 rec = W.items[base];
@@ -226,26 +248,77 @@ k_attn(const int* __restrict__ seq_lens, CcKv kv, CcDims D, CcWork W) {
                     mrow[DH + 1] = l_tot;
                 }
             }
+            if (threadIdx.x == 0) s_seq[(it + 2) & 3] = next_id;
             __syncthreads();
-            for (int e = threadIdx.x; e < G * DH; e += kAttnThreads) {
+            const int nch = (cm.s + CC_ATTN_CHUNK - 1) / CC_ATTN_CHUNK;     // CTA-uniform
+            for (int e = 2 * threadIdx.x; e < G * DH; e += 2 * kAttnThreads) {
                 const int hg = e / DH, dim = e - hg * DH;
                 float M = -INFINITY;
 #pragma unroll
                 for (int w = 0; w < kAttnWarps; ++w) M = fmaxf(M, merge[(size_t)(w * G + hg) * C::kMergeStride + DH]);
-                float acc = 0.f, L = 0.f;
+                float a0 = 0.f, a1 = 0.f, L = 0.f;
 #pragma unroll
                 for (int w = 0; w < kAttnWarps; ++w) {
                     const float* mr = merge + (size_t)(w * G + hg) * C::kMergeStride;
                     const float sc = exp2f(mr[DH] - M);
-                    acc += sc * mr[dim];
+                    a0 += sc * mr[dim];
+                    a1 += sc * mr[dim + 1];
                     L += sc * mr[DH + 1];
                 }
-                const size_t row = ((size_t)cm.pos * D.Hq + (size_t)(c_hk * G + hg)) * W.nch_max + cm.chunk;
-                W.att_o[row * DH + dim] = acc;
-                if (dim == 0) W.att_ml[row] = make_float2(M, L);
+                const int hq = c_hk * G + hg;
+                if (nch == 1) {   // the only chunk of this row: normalise and write the O-projection operand
+                    const float inv = 1.f / L;
+                    const int col = hq * DH + dim;
+                    uint8_t* dst = W.o_act + act_chunk_off(cm.pos, col, D.Mpad, 1, 0) + (col & 7) * 2;
+                    *reinterpret_cast<uint32_t*>(dst) = pack_bf16(a0 * inv, a1 * inv);
+                } else {
+                    const size_t row = ((size_t)cm.pos * D.Hq + hq) * W.nch_max + cm.chunk;
+                    *reinterpret_cast<float2*>(W.att_o + row * DH + dim) = make_float2(a0, a1);
+                    if (dim == 0) W.att_ml[row] = make_float2(M, L);
+                }
             }
-            __syncthreads();   // merge buffer is reused by the next item
+            if (nch > 1) {
+                // ---- the CTA that finishes the pair's last chunk merges all of them, in chunk order
+                __threadfence();
+                __syncthreads();
+                if (threadIdx.x == 0) {
+                    int* cnt = W.attn_cnt + cm.pos * Hkv + c_hk;
+                    const int last = atomicAdd(cnt, 1) == nch - 1;
+                    if (last) *cnt = 0;                             // ready for the next step
+                    s_seq[4] = last;
+                }
+                __syncthreads();
+                if (s_seq[4]) {
+                    __threadfence();
+                    for (int e = 2 * threadIdx.x; e < G * DH; e += 2 * kAttnThreads) {
+                        const int hg = e / DH, dim = e - hg * DH, hq = c_hk * G + hg;
+                        const size_t row = ((size_t)cm.pos * D.Hq + hq) * W.nch_max;
+                        float M = -INFINITY;
+                        for (int c = 0; c < nch; ++c) M = fmaxf(M, __ldcg(&W.att_ml[row + c]).x);
+                        float L = 0.f, a0 = 0.f, a1 = 0.f;
+                        for (int c = 0; c < nch; ++c) {
+                            const float2 ml = __ldcg(&W.att_ml[row + c]);
+                            const float w = exp2f(ml.x - M);
+                            const float2 ov = __ldcg(reinterpret_cast<const float2*>(W.att_o + (row + c) * DH + dim));
+                            L += w * ml.y;
+                            a0 += w * ov.x;
+                            a1 += w * ov.y;
+                        }
+                        const float inv = 1.f / L;
+                        const int col = hq * DH + dim;
+                        uint8_t* dst = W.o_act + act_chunk_off(cm.pos, col, D.Mpad, 1, 0) + (col & 7) * 2;
+                        *reinterpret_cast<uint32_t*>(dst) = pack_bf16(a0 * inv, a1 * inv);
+                    }
+                }
+            }
+            __syncthreads();   // merge buffer and flags are reused by the next item
         }
+    }
+    // out of items: warm L2 with the head of the O-projection weight stream of the first non-empty group
+    if (threadIdx.x == 0) {
+        int r0 = 0;
+        while (r0 < CC_MAXR - 1 && W.sched->cnt[r0] == 0) ++r0;
+        cc_prefetch_gemm_head(D.o, tab->rep[r0].blob, (int)blockIdx.x);
     }
     cp_async_wait<0>();
 }
@@ -258,10 +331,10 @@ cudaError_t cc_attn_configure() {
     return cudaFuncSetAttribute(k_attn<64>, cudaFuncAttributeMaxDynamicSharedMemorySize, 112 * 1024);
 }
 
-cudaError_t cc_launch_attention(const int* seq_lens, const CcKv& kv, const CcDims& D, const CcWork& W,
-                                const CcLaunch& L) {
+cudaError_t cc_launch_attention(const int* seq_lens, const CcKv& kv, const CcDims& D, const CcLayerTable* tab,
+                                const CcWork& W, const CcLaunch& L) {
     const dim3 grid(2 * L.n_sms), block(kAttnThreads);
     if (D.Dh == 128)
-        return cc_launch_kernel(k_attn<128>, grid, block, AttnCfg<128>::smem_bytes(D.G), L, seq_lens, kv, D, W);
-    return cc_launch_kernel(k_attn<64>, grid, block, AttnCfg<64>::smem_bytes(D.G), L, seq_lens, kv, D, W);
+        return cc_launch_kernel(k_attn<128>, grid, block, AttnCfg<128>::smem_bytes(D.G), L, seq_lens, kv, D, W, tab);
+    return cc_launch_kernel(k_attn<64>, grid, block, AttnCfg<64>::smem_bytes(D.G), L, seq_lens, kv, D, W, tab);
 }

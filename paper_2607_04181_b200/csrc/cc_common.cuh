@@ -13,7 +13,7 @@
 #define CC_ROW_ALIGN 16        // group offsets are multiples of this (UMMA N granularity)
 #define CC_MAX_MPAD 320        // (256 rows + 16 * CC_MAXR group padding): upper bound of CcDims::Mpad
 #define CC_FLAG_STRIDE 256     // stream-K fixup counters per projection (>= super tiles of any projection)
-#define CC_ATTN_CHUNK 256      // tokens per split-KV work item (a function of nothing but this)
+#define CC_ATTN_CHUNK 1024     // tokens per split-KV work item (a function of nothing but this)
 
 #define CC_DEVERR_BAD_REPLICA 1u
 #define CC_DEVERR_BAD_PAGE 2u

@@ -19,6 +19,8 @@ struct CcWork {
     float* h1;           // [Mpad][d]     fp32, hidden + O projection
     float* ssq;          // [d/128][Mpad] fp32, per-tile sum of squares of h1 (post-attention RMSNorm statistic)
     int* flags;          // [4][CC_FLAG_STRIDE] stream-K fixup counters, zeroed by k_group every step
+    int* attn_ctr;       // next attention work item (zeroed by k_group every step)
+    int* attn_cnt;       // [Mpad][Hkv] chunks finished per (row, kv head); the last finisher merges and resets
     float* att_o;        // [Mpad*Hq][nch_max][Dh] fp32 un-normalised chunk outputs
     float2* att_ml;      // [Mpad*Hq][nch_max] (max in log2 units, sum)
     const float2* rope_cs;  // [max_position][Dh/2] (cos, sin), built in fp64 on the host
@@ -48,10 +50,8 @@ cudaError_t cc_launch_rmsnorm_in(const __nv_bfloat16* hidden, const CcDims& D, c
 // which: 0 = QKV, 1 = O, 2 = gate/up, 3 = down
 cudaError_t cc_launch_gemm(int which, const CcDims& D, const CcLayerTable* tab, const CcWork& W, const int* seq_lens,
                            const CcKv& kv, __nv_bfloat16* hidden, const CcLaunch& L);
-cudaError_t cc_launch_attention(const int* seq_lens, const CcKv& kv, const CcDims& D, const CcWork& W,
-                                const CcLaunch& L);
-cudaError_t cc_launch_attn_combine(const int* seq_lens, const CcDims& D, const CcLayerTable* tab, const CcWork& W,
-                                   const CcLaunch& L);
+cudaError_t cc_launch_attention(const int* seq_lens, const CcKv& kv, const CcDims& D, const CcLayerTable* tab,
+                                const CcWork& W, const CcLaunch& L);
 
 cudaError_t cc_launch_copy(void* dst, const void* src, size_t bytes, int n_sms, cudaStream_t st);
 cudaError_t cc_launch_publish(CcLayerTable* row_dev, const CcLayerTable& value, cudaStream_t st);

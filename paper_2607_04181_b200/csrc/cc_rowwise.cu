@@ -2,8 +2,7 @@
 // (sm_100a):
 //   k_group        a0     micro-batch grouping + attention work list (device-built, graph-safe)
 //   k_rmsnorm_in   a1     input RMSNorm -> GEMM operand
-//   k_attn_combine a5     fixed-order merge of the split-KV partials -> GEMM operand
-// RoPE + KV append, residual + post-attention norm, SwiGLU and the final residual are the fused
+// The split-KV merge is done by the attention kernel itself (cc_attention.cu); RoPE + KV append, residual + post-attention norm, SwiGLU and the final residual are the fused
 // epilogues of the stream-K fixup inside the GEMM kernel (cc_gemm.cu).  Every reduction order in
 // this file is a function of the layer shape and seq_len only (never of the batch split), which
 // is what makes outputs bit-identical across replica counts.
@@ -51,7 +50,7 @@ __device__ __forceinline__ void split_hilo(float v0, float v1, uint32_t& hi, uin
 __global__ void __launch_bounds__(256) k_group(const int* __restrict__ assign, const int* __restrict__ seq_lens,
                                                int batch, CcDims D, const CcLayerTable* __restrict__ tab, CcWork W) {
     __shared__ int s_wcnt[8][CC_MAXR];     // rows of replica r in warp w
-    __shared__ int s_wnch[8];              // attention chunks in warp w
+    __shared__ int s_wnch[8];              // attention chunks in warp w (full | ragged << 16)
     __shared__ int s_goff[CC_MAXR + 1], s_cnt[CC_MAXR];
     const int b = threadIdx.x, warp = b >> 5, lane = b & 31;
     pdl_wait();
@@ -109,8 +108,10 @@ __global__ void __launch_bounds__(256) k_group(const int* __restrict__ assign, c
         pos = s_goff[rep] + rank;
         W.perm[pos] = b;
     }
-    // work list ordered by request index b (any fixed order is fine: items are independent)
-    int pre = nch;
+    // work list: every full 256-token chunk first (request order), then the ragged last chunks, so that
+    // the attention CTAs, which draw items from a counter, finish on the short ones
+    const int nfull = (rep >= 0) ? seq_lens[b] / CC_ATTN_CHUNK : 0, npart = nch - nfull;
+    int pre = nfull | (npart << 16);                      // two prefix sums in one scan (each < 2^16)
 #pragma unroll
     for (int o = 1; o < 32; o <<= 1) {
         const int v = __shfl_up_sync(0xffffffffu, pre, o);
@@ -118,12 +119,17 @@ __global__ void __launch_bounds__(256) k_group(const int* __restrict__ assign, c
     }
     if (lane == 31) s_wnch[warp] = pre;
     __syncthreads();
-    int base = pre - nch;
-    for (int w = 0; w < warp; ++w) base += s_wnch[w];
-    for (int c = 0; c < nch; ++c) W.items[base + c] = make_int2(pos, c);
+    int base = pre - (nfull | (npart << 16)), tot = 0;
+    for (int w = 0; w < 8; ++w) {
+        if (w < warp) base += s_wnch[w];
+        tot += s_wnch[w];
+    }
+    const int total_full = tot & 0xffff, total = total_full + (tot >> 16);
+    for (int c = 0; c < nfull; ++c) W.items[(base & 0xffff) + c] = make_int2(pos, c);
+    if (npart) W.items[total_full + (base >> 16)] = make_int2(pos, nfull);
     if (b == 0) {
-        int total = 0, nmax = 0;
-        for (int w = 0; w < 8; ++w) total += s_wnch[w];
+        int nmax = 0;
+        *W.attn_ctr = 0;                                   // dynamic item counter of the attention kernel
         for (int r = 0; r < CC_MAXR; ++r) {
             W.sched->cnt[r] = s_cnt[r];
             W.sched->goff[r] = s_goff[r];
@@ -182,45 +188,6 @@ __global__ void __launch_bounds__(kNormThreads) k_rmsnorm_in(const __nv_bfloat16
     }
 }
 
-// ---------------------------------------------------------------------------------------------
-// a5 (second half): merge the split-KV partials of one (row, head) in chunk order -> bf16 operand
-// (one plane: the O projection does not need more).
-// grid (Hq, row); block = Dh/2 threads, two dims each.
-// ---------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(64) k_attn_combine(const int* __restrict__ seq_lens, CcDims D,
-                                                     const CcLayerTable* __restrict__ tab, CcWork W) {
-    const int hq = blockIdx.x, pos = blockIdx.y;
-    pdl_wait();
-    pdl_launch_dependents();
-    if (threadIdx.x == 0) {   // warm L2 with the head of the O-projection weight stream
-        int r0 = 0;
-        while (r0 < CC_MAXR - 1 && W.sched->cnt[r0] == 0) ++r0;
-        cc_prefetch_gemm_head(D.o, tab->rep[r0].blob, (int)(blockIdx.y * gridDim.x + blockIdx.x));
-    }
-    if (pos >= W.sched->n_pos) return;
-    const int b = W.perm[pos];
-    if (b < 0) return;
-    const int nch = (seq_lens[b] + CC_ATTN_CHUNK - 1) / CC_ATTN_CHUNK;
-    const int dim = threadIdx.x * 2;
-    if (dim >= D.Dh) return;
-    const size_t row = ((size_t)pos * D.Hq + hq) * W.nch_max;
-    float M = -INFINITY;
-    for (int c = 0; c < nch; ++c) M = fmaxf(M, W.att_ml[row + c].x);
-    float L = 0.f, a0 = 0.f, a1 = 0.f;
-    for (int c = 0; c < nch; ++c) {
-        const float2 ml = W.att_ml[row + c];
-        const float w = exp2f(ml.x - M);
-        const float2 o = *reinterpret_cast<const float2*>(W.att_o + (row + c) * D.Dh + dim);
-        L += w * ml.y;
-        a0 += w * o.x;
-        a1 += w * o.y;
-    }
-    const float inv = 1.f / L;
-    const int e = hq * D.Dh + dim;
-    uint8_t* dst = W.o_act + act_chunk_off(pos, e, D.Mpad, 1, 0) + (e & 7) * 2;
-    *reinterpret_cast<uint32_t*>(dst) = pack_bf16(a0 * inv, a1 * inv);
-}
-
 constexpr int kMaxVecPerThread = 4;   // hidden <= 4 * 4 * 512 = 8192 (operand layout and epilogue limits)
 
 // Test tap: widen a workspace buffer to fp32 [batch][dim] in original row order.
@@ -262,10 +229,6 @@ cudaError_t cc_launch_group(const int* assign, const int* seq_lens, int batch, c
 cudaError_t cc_launch_rmsnorm_in(const __nv_bfloat16* hidden, const CcDims& D, const CcLayerTable* tab,
                                  const CcWork& W, const CcLaunch& L) {
     return cc_launch_kernel(k_rmsnorm_in, dim3(D.Mpad), dim3(kNormThreads), 0, L, hidden, D, tab, W);
-}
-cudaError_t cc_launch_attn_combine(const int* seq_lens, const CcDims& D, const CcLayerTable* tab, const CcWork& W,
-                                   const CcLaunch& L) {
-    return cc_launch_kernel(k_attn_combine, dim3(D.Hq, D.Mpad), dim3(64), 0, L, seq_lens, D, tab, W);
 }
 cudaError_t cc_launch_tap(const void* src, int which, int dim, const CcDims& D, const CcWork& W,
                           float* out_dev, int batch, cudaStream_t st) {
