@@ -6,11 +6,14 @@
 // head are the (zero-padded) 16 rows of an mma.sync m16n8k16 tile, so one KV read serves the
 // whole GQA group.  This is a memory kernel with M <= 8 real rows: the legacy warp-level
 // tensor path is ample here (tcgen05 needs M >= 64), the design effort goes into the stream:
-//   * each warp owns 4 of the chunk's 16 pages (w, w+4, w+8, w+12) and a private ring of
-//     cp.async stages (one stage = one K page + one V page = 2 x 16 x Dh bf16), so loads of the
-//     next pages -- and of the next work item -- are in flight while a page is being used;
-//   * pages land in smem XOR-swizzled at 16-byte granularity, so the ldmatrix reads of the
-//     K (B operand of q.K^T) and V (transposed B operand of p.V) fragments are conflict-free;
+//   * each warp owns every 4th page of the chunk (w, w+4, ...) and a private ring of stages (one
+//     stage = one K page + one V page of one kv head = 2 x 16 x Dh bf16) filled by TMA: one elected
+//     lane issues cp.async.bulk.tensor boxes of 16 tokens x 128 bytes through a tensor map of the
+//     caller's pool (built on the host per forward), completion on one mbarrier per stage; loads of
+//     the next pages -- and of the next work item -- are in flight while a page is being used.
+//     (The earlier per-lane 16-byte cp.async path topped out at 4.7 TB/s with the math removed.)
+//   * the tensor map's 128-byte swizzle lands the rows so that the ldmatrix reads of the K
+//     (B operand of q.K^T) and V (transposed B operand of p.V) fragments are conflict-free;
 //   * softmax is online per warp (running max / sum in log2 units, fp32), the 4 warps of a CTA
 //     are merged in fixed order through smem; the chunk partials of one (row, kv head) are merged
 //     in chunk order by whichever CTA finishes that pair's last chunk (a counter per pair), so no
@@ -19,6 +22,7 @@
 //   * CTAs draw work items from a device counter (first item static), full chunks first and the
 //     ragged last chunks at the end of the list, which evens out the tail of the kernel.
 #include "cc_kernels.h"
+#include <cuda.h>
 
 namespace {
 
@@ -33,10 +37,9 @@ struct AttnCfg {
     static constexpr int kRowBytes = DH * 2;
     static constexpr int kPageBytes = CC_PAGE * kRowBytes;     // one K (or V) page of one kv head
     static constexpr int kStageBytes = 2 * kPageBytes;
-    static constexpr int kChunksPerRow = DH / 8;               // 16-byte chunks per token row
     static constexpr int kMergeStride = DH + 2;                // floats per (warp, head): o[DH], m, l
     static size_t smem_bytes(int G) {
-        return (size_t)kAttnWarps * kAttnStages * kStageBytes + (size_t)kAttnWarps * G * kMergeStride * 4 + 32;
+        return (size_t)kAttnWarps * kAttnStages * kStageBytes + (size_t)kAttnWarps * G * kMergeStride * 4 + 32 + (size_t)kAttnWarps * kAttnStages * 8;
     }
 };
 
@@ -46,16 +49,24 @@ struct ItemMeta {
 
 template <int DH>
 __global__ void __launch_bounds__(kAttnThreads, 2)
-k_attn(const int* __restrict__ seq_lens, CcKv kv, CcDims D, CcWork W, const CcLayerTable* __restrict__ tab) {
+k_attn(const int* __restrict__ seq_lens, CcKv kv, CcDims D, CcWork W, const CcLayerTable* __restrict__ tab,
+       const __grid_constant__ CUtensorMap tmK, const __grid_constant__ CUtensorMap tmV) {
     using C = AttnCfg<DH>;
     extern __shared__ __align__(1024) uint8_t smem_raw[];
-    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int warp = uniform((int)(threadIdx.x >> 5)), lane = threadIdx.x & 31;
     const int g = lane >> 2, t4 = lane & 3;
     uint8_t* ring = smem_raw + (size_t)warp * kAttnStages * C::kStageBytes;
     float* merge = reinterpret_cast<float*>(smem_raw + (size_t)kAttnWarps * kAttnStages * C::kStageBytes);
     const uint32_t ring_u32 = smem_u32(ring);
 
     int* s_seq = reinterpret_cast<int*>(merge + (size_t)kAttnWarps * D.G * C::kMergeStride);   // [4] item ids + [1] flag
+    uint64_t* bars = reinterpret_cast<uint64_t*>(s_seq + 8) + warp * kAttnStages;              // "stage full", per warp
+    if (lane == 0) {
+#pragma unroll
+        for (int i = 0; i < kAttnStages; ++i) mbar_init(&bars[i], 1);
+        fence_mbar_init();
+    }
+    __syncwarp();
     pdl_wait();
     pdl_launch_dependents();
 
@@ -108,32 +119,24 @@ k_attn(const int* __restrict__ seq_lens, CcKv kv, CcDims D, CcWork W, const CcLa
         const int tok0 = pm.chunk * CC_ATTN_CHUNK + pl * CC_PAGE;   // first token of the page
         const int page0 = __shfl_sync(0xffffffffu, p_page_id[0], pl & 31), page1 = __shfl_sync(0xffffffffu, p_page_id[1], pl & 31);
         const int page = pl < 32 ? page0 : page1;
-        if (tok0 < pm.s) {
-            const int valid = min(CC_PAGE, pm.s - tok0);
-            const size_t src_off = ((size_t)page * Hkv + p_hk) * (size_t)(CC_PAGE * DH);
-            const __nv_bfloat16* ksrc = kv.k_pool + src_off;
-            const __nv_bfloat16* vsrc = kv.v_pool + src_off;
-            const uint32_t dstK = ring_u32 + (uint32_t)(k % kAttnStages) * C::kStageBytes;
-            const uint32_t dstV = dstK + C::kPageBytes;
+        // warp-uniform values + elect.sync keep the TMA issue on the uniform datapath (no per-lane waterfall)
+        const int do_load = uniform((int)(tok0 < pm.s));
+        const int row0 = uniform((page * Hkv + p_hk) * CC_PAGE);     // row of the pool seen as [pages*Hkv*16][DH]
+        const int st = k % kAttnStages;
+        if (do_load && elect_one()) {
+            const uint32_t dstK = ring_u32 + (uint32_t)st * C::kStageBytes, dstV = dstK + C::kPageBytes;
+            const uint32_t bar = smem_u32(&bars[st]);
+            mbar_expect_tx(&bars[st], C::kStageBytes);
 #pragma unroll
-            for (int q = lane; q < CC_PAGE * C::kChunksPerRow; q += 32) {
-                const int tok = q / C::kChunksPerRow, ch = q % C::kChunksPerRow;
-                const uint32_t off = (uint32_t)tok * C::kRowBytes + (uint32_t)((ch ^ (tok & 7)) << 4);
-                const uint32_t sz = tok < valid ? 16u : 0u;        // rows past seq_len are zero-filled
-                asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;" ::"r"(dstK + off),
-                             "l"(ksrc + tok * DH + ch * 8), "r"(sz)
-                             : "memory");
-                asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;" ::"r"(dstV + off),
-                             "l"(vsrc + tok * DH + ch * 8), "r"(sz)
-                             : "memory");
+            for (int h = 0; h < DH / 64; ++h) {                       // boxes of 16 tokens x 64 dims (128 bytes)
+                tma_load_2d(dstK + h * 2048, &tmK, h * 64, row0, bar);
+                tma_load_2d(dstV + h * 2048, &tmV, h * 64, row0, bar);
             }
         }
     };
 
-    for (int k = 0; k < kAttnStages - 1; ++k) {
-        prefetch(k);
-        cp_async_commit();
-    }
+    for (int k = 0; k < kAttnStages - 1; ++k) prefetch(k);
+    uint32_t phases = 0;                                   // bit st = parity of the next completion of stage st
 
     // ---- consumer state ----------------------------------------------------------------------
     ItemMeta cm = {0, 0, 0, 0};
@@ -147,7 +150,6 @@ k_attn(const int* __restrict__ seq_lens, CcKv kv, CcDims D, CcWork W, const CcLa
         const int it = k / kSlotsPerItem, i = k % kSlotsPerItem;
         if (i == 0 && s_seq[it & 3] >= n_total) break;     // CTA-uniform: the list is exhausted
         prefetch(k + kAttnStages - 1);
-        cp_async_commit();
 
         if (i == 0) {   // new item: metadata, Q fragments, reset the running softmax state
             if (threadIdx.x == 0) next_id = (int)gridDim.x + atomicAdd(W.attn_ctr, 1);
@@ -176,26 +178,34 @@ k_attn(const int* __restrict__ seq_lens, CcKv kv, CcDims D, CcWork W, const CcLa
             l_run = 0.f;
         }
 
-        cp_async_wait<kAttnStages - 1>();
-        __syncwarp();
-
         const int pl = warp + i * kAttnWarps;
         const int tok0 = cm.chunk * CC_ATTN_CHUNK + pl * CC_PAGE;
         if (tok0 < cm.s) {
             const int valid = min(CC_PAGE, cm.s - tok0);
-            const uint32_t sK = ring_u32 + (uint32_t)(k % kAttnStages) * C::kStageBytes;
+            const int st = k % kAttnStages;
+            const uint32_t sK = ring_u32 + (uint32_t)st * C::kStageBytes;
             const uint32_t sV = sK + C::kPageBytes;
+            mbar_wait(&bars[st], (phases >> st) & 1u);
+            phases ^= 1u << st;
+            if (valid < CC_PAGE) {   // ragged last page: the V rows past seq_len hold other data; p = 0 must meet 0
+                for (int q = lane; q < (CC_PAGE - valid) * (DH / 8); q += 32) {
+                    const int r = valid + q / (DH / 8), c = q % (DH / 8);
+                    asm volatile("st.shared.v4.b32 [%0], {%1, %1, %1, %1};" ::"r"(sV + (c >> 3) * 2048 + r * 128 + ((c & 7) << 4)), "r"(0) : "memory");
+                }
+                fence_proxy_async_smem();   // a later TMA refill of this stage must not pass these stores
+                __syncwarp();
+            }
             // ---- scores: S[16 x 16] = Q[16 x DH] . K^T
             float s0[4] = {0.f, 0.f, 0.f, 0.f}, s1[4] = {0.f, 0.f, 0.f, 0.f};
             {
                 const int mi = lane >> 3, rr = lane & 7;
                 const int tok = ((mi >> 1) << 3) + rr;
-                const uint32_t rowaddr = sK + (uint32_t)tok * C::kRowBytes;
+                const uint32_t rowaddr = sK + (uint32_t)tok * 128;
 #pragma unroll
                 for (int ks = 0; ks < DH / 16; ++ks) {
                     const int ch = ks * 2 + (mi & 1);
                     uint32_t r0, r1, r2, r3;
-                    ldsm_x4(rowaddr + (uint32_t)((ch ^ (tok & 7)) << 4), r0, r1, r2, r3);
+                    ldsm_x4(rowaddr + (uint32_t)((ch >> 3) * 2048 + (((ch & 7) ^ (tok & 7)) << 4)), r0, r1, r2, r3);
                     mma_bf16_16816(s0, qa0[ks], 0u, qa2[ks], 0u, r0, r1);
                     mma_bf16_16816(s1, qa0[ks], 0u, qa2[ks], 0u, r2, r3);
                 }
@@ -218,12 +228,12 @@ k_attn(const int* __restrict__ seq_lens, CcKv kv, CcDims D, CcWork W, const CcLa
             {
                 const int mi = lane >> 3, rr = lane & 7;
                 const int tok = ((mi & 1) << 3) + rr;
-                const uint32_t rowaddr = sV + (uint32_t)tok * C::kRowBytes;
+                const uint32_t rowaddr = sV + (uint32_t)tok * 128;
 #pragma unroll
                 for (int jn = 0; jn < DH / 16; ++jn) {
                     const int ch = jn * 2 + (mi >> 1);
                     uint32_t r0, r1, r2, r3;
-                    ldsm_x4_trans(rowaddr + (uint32_t)((ch ^ (tok & 7)) << 4), r0, r1, r2, r3);
+                    ldsm_x4_trans(rowaddr + (uint32_t)((ch >> 3) * 2048 + (((ch & 7) ^ (tok & 7)) << 4)), r0, r1, r2, r3);
                     o[2 * jn][0] *= alpha; o[2 * jn][1] *= alpha;
                     o[2 * jn + 1][0] *= alpha; o[2 * jn + 1][1] *= alpha;
                     mma_bf16_16816(o[2 * jn], pa0, 0u, pa2, 0u, r0, r1);
@@ -320,7 +330,6 @@ k_attn(const int* __restrict__ seq_lens, CcKv kv, CcDims D, CcWork W, const CcLa
         while (r0 < CC_MAXR - 1 && W.sched->cnt[r0] == 0) ++r0;
         cc_prefetch_gemm_head(D.o, tab->rep[r0].blob, (int)blockIdx.x);
     }
-    cp_async_wait<0>();
 }
 
 }  // namespace
@@ -331,10 +340,40 @@ cudaError_t cc_attn_configure() {
     return cudaFuncSetAttribute(k_attn<64>, cudaFuncAttributeMaxDynamicSharedMemorySize, 112 * 1024);
 }
 
+// Tensor map of a caller-owned KV pool seen as a 2-D bf16 tensor [n_pages * Hkv * 16 rows][Dh], boxes of
+// 16 rows x 64 elements (128 bytes) with the 128-byte swizzle.  cuTensorMapEncodeTiled is a driver entry
+// point; it is looked up once through the runtime, so the library needs no link against libcuda.
+static cudaError_t make_kv_tensor_map(CUtensorMap* out, const void* pool, int n_pages, int Hkv, int Dh) {
+    typedef CUresult (*EncodeFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
+                                 const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                 CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+    static EncodeFn encode = nullptr;
+    if (!encode) {
+        void* fn = nullptr;
+        cudaDriverEntryPointQueryResult qr;
+        cudaError_t e = cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qr);
+        if (e != cudaSuccess) return e;
+        if (qr != cudaDriverEntryPointSuccess || !fn) return cudaErrorNotSupported;
+        encode = (EncodeFn)fn;
+    }
+    const cuuint64_t dims[2] = {(cuuint64_t)Dh, (cuuint64_t)n_pages * Hkv * CC_PAGE};
+    const cuuint64_t strides[1] = {(cuuint64_t)Dh * 2};
+    const cuuint32_t box[2] = {64, CC_PAGE};
+    const cuuint32_t estr[2] = {1, 1};
+    const CUresult r = encode(out, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, const_cast<void*>(pool), dims, strides, box, estr,
+                              CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                              CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    return r == CUDA_SUCCESS ? cudaSuccess : cudaErrorInvalidValue;
+}
+
 cudaError_t cc_launch_attention(const int* seq_lens, const CcKv& kv, const CcDims& D, const CcLayerTable* tab,
                                 const CcWork& W, const CcLaunch& L) {
+    CUtensorMap tmK, tmV;
+    cudaError_t e = make_kv_tensor_map(&tmK, kv.k_pool, kv.n_pages, D.Hkv, D.Dh);
+    if (e == cudaSuccess) e = make_kv_tensor_map(&tmV, kv.v_pool, kv.n_pages, D.Hkv, D.Dh);
+    if (e != cudaSuccess) return e;
     const dim3 grid(2 * L.n_sms), block(kAttnThreads);
     if (D.Dh == 128)
-        return cc_launch_kernel(k_attn<128>, grid, block, AttnCfg<128>::smem_bytes(D.G), L, seq_lens, kv, D, W, tab);
-    return cc_launch_kernel(k_attn<64>, grid, block, AttnCfg<64>::smem_bytes(D.G), L, seq_lens, kv, D, W, tab);
+        return cc_launch_kernel(k_attn<128>, grid, block, AttnCfg<128>::smem_bytes(D.G), L, seq_lens, kv, D, W, tab, tmK, tmV);
+    return cc_launch_kernel(k_attn<64>, grid, block, AttnCfg<64>::smem_bytes(D.G), L, seq_lens, kv, D, W, tab, tmK, tmV);
 }

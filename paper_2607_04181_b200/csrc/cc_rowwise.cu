@@ -52,6 +52,7 @@ __global__ void __launch_bounds__(256) k_group(const int* __restrict__ assign, c
     __shared__ int s_wcnt[8][CC_MAXR];     // rows of replica r in warp w
     __shared__ int s_wnch[8];              // attention chunks in warp w (full | ragged << 16)
     __shared__ int s_goff[CC_MAXR + 1], s_cnt[CC_MAXR];
+    __shared__ int s_rem[256];             // tokens in the ragged last chunk of row b (0: none)
     const int b = threadIdx.x, warp = b >> 5, lane = b & 31;
     pdl_wait();
     pdl_launch_dependents();
@@ -108,8 +109,8 @@ __global__ void __launch_bounds__(256) k_group(const int* __restrict__ assign, c
         pos = s_goff[rep] + rank;
         W.perm[pos] = b;
     }
-    // work list: every full 256-token chunk first (request order), then the ragged last chunks, so that
-    // the attention CTAs, which draw items from a counter, finish on the short ones
+    // work list: every full chunk first (request order), then the ragged last chunks, longest first, so
+    // that the attention CTAs, which draw items from a counter, finish on the shortest ones
     const int nfull = (rep >= 0) ? seq_lens[b] / CC_ATTN_CHUNK : 0, npart = nch - nfull;
     int pre = nfull | (npart << 16);                      // two prefix sums in one scan (each < 2^16)
 #pragma unroll
@@ -118,6 +119,8 @@ __global__ void __launch_bounds__(256) k_group(const int* __restrict__ assign, c
         if (lane >= o) pre += v;
     }
     if (lane == 31) s_wnch[warp] = pre;
+    const int rem = npart ? seq_lens[b] % CC_ATTN_CHUNK : 0;
+    s_rem[b] = rem;
     __syncthreads();
     int base = pre - (nfull | (npart << 16)), tot = 0;
     for (int w = 0; w < 8; ++w) {
@@ -126,7 +129,11 @@ __global__ void __launch_bounds__(256) k_group(const int* __restrict__ assign, c
     }
     const int total_full = tot & 0xffff, total = total_full + (tot >> 16);
     for (int c = 0; c < nfull; ++c) W.items[(base & 0xffff) + c] = make_int2(pos, c);
-    if (npart) W.items[total_full + (base >> 16)] = make_int2(pos, nfull);
+    if (npart) {
+        int rank = 0;                                      // ragged chunks longer than this one (ties: lower row first)
+        for (int o = 0; o < 256; ++o) rank += (s_rem[o] > rem) || (s_rem[o] == rem && o < b);
+        W.items[total_full + rank] = make_int2(pos, nfull);
+    }
     if (b == 0) {
         int nmax = 0;
         *W.attn_ctr = 0;                                   // dynamic item counter of the attention kernel
