@@ -72,7 +72,7 @@ typedef struct cc_layer cc_layer; /* one decoder layer: slot 0 blob, replica slo
 typedef struct {
     int32_t hidden;              /* d; multiple of 64, at most 8192                             */
     int32_t n_q_heads;           /* Hq                                                          */
-    int32_t n_kv_heads;          /* Hkv; Hq % Hkv == 0 and Hq / Hkv <= 8                        */
+    int32_t n_kv_heads;          /* Hkv in {1, 2, 4, 8}; Hq % Hkv == 0 and Hq / Hkv <= 8        */
     int32_t head_dim;            /* Dh: 64 or 128                                               */
     int32_t ffn;                 /* F (SwiGLU width)                                            */
     float rms_eps;

@@ -337,6 +337,7 @@ cc_status cc_create_layer(cc_ctx* ctx, const cc_layer_desc* desc, const cc_layer
     if (d.head_dim != 64 && d.head_dim != 128) return fail(CC_ERR_INVALID, "head_dim must be 64 or 128");
     if (d.n_kv_heads <= 0 || d.n_q_heads <= 0 || d.n_q_heads % d.n_kv_heads || d.n_q_heads / d.n_kv_heads > 8)
         return fail(CC_ERR_INVALID, "need n_q_heads %% n_kv_heads == 0 and a GQA group of at most 8");
+    if (8 % d.n_kv_heads) return fail(CC_ERR_INVALID, "n_kv_heads must be 1, 2, 4 or 8 (one page of all kv heads is staged per TMA box)");
     if (d.ffn <= 0 || d.ffn % 8) return fail(CC_ERR_INVALID, "ffn must be a positive multiple of 8");
     if (d.page_size != CC_PAGE_SIZE) return fail(CC_ERR_INVALID, "page_size must be %d", CC_PAGE_SIZE);
     if (d.max_batch < 1 || d.max_batch > 256) return fail(CC_ERR_INVALID, "max_batch must be in 1..256");
@@ -384,16 +385,12 @@ cc_status cc_create_layer(cc_ctx* ctx, const cc_layer_desc* desc, const cc_layer
 
     // workspace
     CcWork& W = L->W;
-    W.nch_max = (d.max_position + CC_ATTN_CHUNK - 1) / CC_ATTN_CHUNK;
-    if ((long long)d.max_batch * W.nch_max >= 65536) {
-        delete L;
-        return fail(CC_ERR_INVALID, "max_batch * ceil(max_position / %d) must stay below 65536 attention work items", CC_ATTN_CHUNK);
-    }
     Carver ws;
     const size_t Mp = (size_t)D.Mpad;
     const size_t o_sched = ws.take(sizeof(CcSched));
     const size_t o_perm = ws.take(Mp * 4);
-    const size_t o_items = ws.take((size_t)d.max_batch * W.nch_max * sizeof(int2));
+    const size_t o_pgpre = ws.take((size_t)(d.max_batch + 1) * 4);
+    const size_t o_posof = ws.take((size_t)d.max_batch * 4);
     const size_t o_x = ws.take((size_t)2 * D.qkv.KB * Mp * 128);   // hi + lo planes
     const size_t o_o = ws.take((size_t)D.o.KB * Mp * 128);
     const size_t o_y = ws.take((size_t)2 * D.gu.KB * Mp * 128);
@@ -407,10 +404,10 @@ cc_status cc_create_layer(cc_ctx* ctx, const cc_layer_desc* desc, const cc_layer
     const size_t o_h1 = ws.take(Mp * D.d * 4);
     const size_t o_ssq = ws.take((size_t)((D.d + 127) / 128) * Mp * 4);
     const size_t o_flags = ws.take((size_t)4 * CC_FLAG_STRIDE * 4);
-    const size_t o_actr = ws.take(64);
     const size_t o_acnt = ws.take(Mp * D.Hkv * 4);
-    const size_t o_atto = ws.take(Mp * D.Hq * W.nch_max * D.Dh * 4);
-    const size_t o_attml = ws.take(Mp * D.Hq * W.nch_max * sizeof(float2));
+    const size_t n_slots = (size_t)d.max_batch + ctx->n_sms;          // attention pieces: one per (row, CTA) overlap
+    const size_t o_atto = ws.take(n_slots * D.Hq * D.Dh * 4);
+    const size_t o_attml = ws.take(n_slots * D.Hq * sizeof(float2));
     const size_t o_rope = ws.take((size_t)d.max_position * (D.Dh / 2) * sizeof(float2));
     const size_t o_sth = ws.take((size_t)d.max_batch * D.d * 2);
     const size_t o_stbt = ws.take((size_t)d.max_batch * d.max_blocks_per_seq * 4);
@@ -429,13 +426,13 @@ cc_status cc_create_layer(cc_ctx* ctx, const cc_layer_desc* desc, const cc_layer
         return fail(CC_ERR_CUDA, "device allocation of %zu + %zu bytes failed: %s", L->blob_bytes, ws_bytes, cudaGetErrorString(e));
     }
     uint8_t* wb = L->work_base;
-    W.sched = (CcSched*)(wb + o_sched); W.perm = (int*)(wb + o_perm); W.items = (int2*)(wb + o_items);
+    W.sched = (CcSched*)(wb + o_sched); W.perm = (int*)(wb + o_perm); W.pg_prefix = (int*)(wb + o_pgpre); W.pos_of = (int*)(wb + o_posof);
     W.x_act = wb + o_x; W.o_act = wb + o_o; W.y_act = wb + o_y; W.a_act = wb + o_a;
     W.qkv_part = (float*)(wb + o_pq); W.o_part = (float*)(wb + o_po); W.gu_part = (float*)(wb + o_pg);
     W.d_part = (float*)(wb + o_pd);
     W.q_rot = (float*)(wb + o_qrot); W.h1 = (float*)(wb + o_h1);
     W.ssq = (float*)(wb + o_ssq); W.flags = (int*)(wb + o_flags);
-    W.attn_ctr = (int*)(wb + o_actr); W.attn_cnt = (int*)(wb + o_acnt);
+    W.attn_cnt = (int*)(wb + o_acnt);
     W.att_o = (float*)(wb + o_atto); W.att_ml = (float2*)(wb + o_attml);
     W.rope_cs = (const float2*)(wb + o_rope);
     W.err = ctx->err_dev;

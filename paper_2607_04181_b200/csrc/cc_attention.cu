@@ -1,167 +1,204 @@
 // cc_attention.cu -- paged GQA decode attention, split-KV (the KV cache
 // partitioning the paper relies on: PAPER.md:103, 391, 476).
 //
-// HBM-bound: every cached K/V byte of a request is read exactly once per step.  Work item =
-// (grouped row, kv head, chunk of 256 tokens = 16 pages); the G query heads that share the kv
-// head are the (zero-padded) 16 rows of an mma.sync m16n8k16 tile, so one KV read serves the
-// whole GQA group.  This is a memory kernel with M <= 8 real rows: the legacy warp-level
-// tensor path is ample here (tcgen05 needs M >= 64), the design effort goes into the stream:
-//   * each warp owns every 4th page of the chunk (w, w+4, ...) and a private ring of stages (one
-//     stage = one K page + one V page of one kv head = 2 x 16 x Dh bf16) filled by TMA: one elected
-//     lane issues cp.async.bulk.tensor boxes of 16 tokens x 128 bytes through a tensor map of the
-//     caller's pool (built on the host per forward), completion on one mbarrier per stage; loads of
-//     the next pages -- and of the next work item -- are in flight while a page is being used.
-//     (The earlier per-lane 16-byte cp.async path topped out at 4.7 TB/s with the math removed.)
-//   * the tensor map's 128-byte swizzle lands the rows so that the ldmatrix reads of the K
-//     (B operand of q.K^T) and V (transposed B operand of p.V) fragments are conflict-free;
-//   * softmax is online per warp (running max / sum in log2 units, fp32), the 4 warps of a CTA
-//     are merged in fixed order through smem; the chunk partials of one (row, kv head) are merged
-//     in chunk order by whichever CTA finishes that pair's last chunk (a counter per pair), so no
-//     separate combine kernel runs.  The chunking depends on seq_len only and every merge order
-//     is fixed => bit-identical across replicas, whatever CTA does the work.
-//   * CTAs draw work items from a device counter (first item static), full chunks first and the
-//     ragged last chunks at the end of the list, which evens out the tail of the kernel.
+// HBM-bound: every cached K/V byte of a request is read exactly once per step.  The design is
+// built around HOW those bytes are asked for.  The pool layout is [page][kv_head][16][Dh], so one
+// page holds 32 KiB of contiguous K (Hkv = 8, Dh = 128) and as much V.  Reading it head by head
+// from different CTAs (4 KiB requests scattered over the pool) topped out at 4.7 TB/s with the
+// math removed; walking all heads of a page together measured 6.7 TB/s with the same bytes in
+// flight (profiles/r01e_attention_access_pattern.md).  Hence:
+//   * the work axis is the list of KV pages of the whole batch (rows in request order); it is cut
+//     into equal contiguous ranges, one per persistent CTA (one CTA per SM), so every CTA streams
+//     the same number of bytes (+- one page) whatever the context lengths are.  A row that spans
+//     several ranges is split there ("pieces"); the split is a function of the batch only, never
+//     of the replica assignment;
+//   * a producer warp stages whole pages by TMA: one cp.async.bulk.tensor box of
+//     (Hkv * 16 rows) x 128 bytes per half page through a tensor map of the caller's pool (built
+//     on the host per forward), 128-byte swizzle, into a ring of 64 KiB stages (K + V of 8 / Hkv
+//     pages), "full" mbarrier per stage, "empty" mbarrier released by the consumers;
+//   * eight consumer warps: warp w owns kv head w % Hkv of page w / Hkv of the stage.  The G query
+//     heads that share a kv head are the (zero-padded) 16 rows of an mma.sync m16n8k16 tile, so
+//     one KV read serves the whole GQA group.  (M <= 8 real rows: the warp-level tensor path is
+//     ample; tcgen05 needs M >= 64.)  ldmatrix reads of the swizzled rows are conflict-free;
+//   * softmax is online per warp (running max / sum in log2 units, fp32).  At the end of a chunk
+//     piece the warps that share a kv head (Hkv < 8) are merged in fixed order through smem; the
+//     piece partials of one (row, kv head) are merged in piece order by the warp that finishes the
+//     pair's last piece (a counter per pair), so no separate combine kernel runs.  Every merge
+//     order is fixed => bit-identical across replicas, whatever CTA finishes last.
+//   * KV loads carry an L2 evict-first policy (measured: +12 % stream rate; the data is used once).
 #include "cc_kernels.h"
 #include <cuda.h>
 
 namespace {
 
-constexpr int kAttnWarps = 4;
-constexpr int kAttnThreads = kAttnWarps * 32;
+constexpr int kCW = 8;                                  // consumer warps
+constexpr int kAttnThreads = (kCW + 1) * 32;            // + the producer warp (warp kCW)
 constexpr int kAttnStages = 3;
-constexpr int kPagesPerChunk = CC_ATTN_CHUNK / CC_PAGE;       // 16
-constexpr int kSlotsPerItem = kPagesPerChunk / kAttnWarps;    // 4 page slots per warp per item
+constexpr int kBarMerge = 1;                            // named barrier of the consumer warps
+
+enum { kMetaFirst = 1, kMetaLast = 2, kMetaEnd = 4 };
+struct StageMeta {          // written by the producer before it arms the stage's "full" barrier
+    int pos;                // grouped position of the row (Q, outputs)
+    int s;                  // its seq_len
+    int flags;              // kMetaFirst / kMetaLast group of the piece, kMetaEnd
+    int pg;                 // index (within the row) of the stage's first page
+    int slot;               // partial-result slot of this piece = row + CTA
+    int slot0, n_pieces;    // the row's pieces are slots slot0 .. slot0 + n_pieces - 1
+    int n_in;               // pages of the piece in this stage (<= pages per stage)
+};
 
 template <int DH>
 struct AttnCfg {
-    static constexpr int kRowBytes = DH * 2;
-    static constexpr int kPageBytes = CC_PAGE * kRowBytes;     // one K (or V) page of one kv head
-    static constexpr int kStageBytes = 2 * kPageBytes;
-    static constexpr int kMergeStride = DH + 2;                // floats per (warp, head): o[DH], m, l
+    static constexpr int kUnitBytes = CC_PAGE * DH * 2;            // K (or V) of one (page, kv head)
+    static constexpr int kStageBytes = 2 * kCW * kUnitBytes;       // K + V of kCW (page, head) units
+    static constexpr int kMergeStride = DH + 4;                    // floats per (warp, q head): o[DH], m, l, pad (16-byte rows)
+    static constexpr size_t kCtrlBytes = kAttnStages * sizeof(StageMeta) + 2 * kAttnStages * 8 + 260 * 4;
     static size_t smem_bytes(int G) {
-        return (size_t)kAttnWarps * kAttnStages * kStageBytes + (size_t)kAttnWarps * G * kMergeStride * 4 + 32 + (size_t)kAttnWarps * kAttnStages * 8;
+        return (size_t)kAttnStages * kStageBytes + (size_t)kCW * G * kMergeStride * 4 + kCtrlBytes;
     }
 };
 
-struct ItemMeta {
-    int pos, chunk, b, s;     // s <= 0 marks "no item"
-};
-
 template <int DH>
-__global__ void __launch_bounds__(kAttnThreads, 2)
+__global__ void __launch_bounds__(kAttnThreads, 1)
 k_attn(const int* __restrict__ seq_lens, CcKv kv, CcDims D, CcWork W, const CcLayerTable* __restrict__ tab,
        const __grid_constant__ CUtensorMap tmK, const __grid_constant__ CUtensorMap tmV) {
     using C = AttnCfg<DH>;
     extern __shared__ __align__(1024) uint8_t smem_raw[];
     const int warp = uniform((int)(threadIdx.x >> 5)), lane = threadIdx.x & 31;
-    const int g = lane >> 2, t4 = lane & 3;
-    uint8_t* ring = smem_raw + (size_t)warp * kAttnStages * C::kStageBytes;
-    float* merge = reinterpret_cast<float*>(smem_raw + (size_t)kAttnWarps * kAttnStages * C::kStageBytes);
-    const uint32_t ring_u32 = smem_u32(ring);
+    const int G = D.G, Hkv = D.Hkv;
+    const int PPS = kCW / Hkv;                                     // pages per stage
+    float* merge = reinterpret_cast<float*>(smem_raw + (size_t)kAttnStages * C::kStageBytes);
+    StageMeta* meta = reinterpret_cast<StageMeta*>(merge + (size_t)kCW * G * C::kMergeStride);
+    uint64_t* full = reinterpret_cast<uint64_t*>(meta + kAttnStages);
+    uint64_t* empty = full + kAttnStages;
+    const uint32_t ring_u32 = smem_u32(smem_raw);
+    // stage layout: [page of the stage][K | V][half of Dh (64 dims = 128 bytes)][Hkv * 16 rows][128 B]
+    const uint32_t half_bytes = (uint32_t)Hkv * CC_PAGE * 128u;
+    const uint32_t kv_bytes = half_bytes * (DH / 64);              // K (or V) of one page, all heads
+    const uint32_t page_bytes = 2u * kv_bytes;
 
-    int* s_seq = reinterpret_cast<int*>(merge + (size_t)kAttnWarps * D.G * C::kMergeStride);   // [4] item ids + [1] flag
-    uint64_t* bars = reinterpret_cast<uint64_t*>(s_seq + 8) + warp * kAttnStages;              // "stage full", per warp
-    if (lane == 0) {
-#pragma unroll
-        for (int i = 0; i < kAttnStages; ++i) mbar_init(&bars[i], 1);
+    if (threadIdx.x == 0) {
+        for (int i = 0; i < kAttnStages; ++i) {
+            mbar_init(&full[i], 1);
+            mbar_init(&empty[i], kCW);
+        }
         fence_mbar_init();
     }
-    __syncwarp();
+    __syncthreads();
     pdl_wait();
     pdl_launch_dependents();
-
-    const int G = D.G, Hkv = D.Hkv;
-    const int n_total = W.sched->n_items * Hkv;
-    // item sequence of this CTA: seq[0] = blockIdx.x, later ones from the counter; seq[n + 2] is drawn
-    // while item n runs, so the loads of the next item can be in flight before the current one ends
-    if (threadIdx.x == 0) {
-        s_seq[0] = (int)blockIdx.x;
-        s_seq[1] = (int)gridDim.x + atomicAdd(W.attn_ctr, 1);
-    }
+    const int T = W.sched->n_items;                               // KV pages of the batch
+    int* s_prefix = reinterpret_cast<int*>(empty + kAttnStages);  // [max_batch + 1]
+    for (int i = threadIdx.x; i <= D.max_batch; i += kAttnThreads) s_prefix[i] = W.pg_prefix[i];
     __syncthreads();
 
-    // ---- producer side: issue the cp.async copies of page slot k of this warp -------------------
-    ItemMeta pm = {0, 0, 0, 0};
-    int p_hk = 0, p_item = -1, p_page_id[2] = {0, 0};   // lane l holds the ids of pages l and l + 32 of the chunk
-    static_assert(kPagesPerChunk <= 64, "two page ids per lane");
-    auto prefetch = [&](int k) {
-        const int it = k / kSlotsPerItem, i = k % kSlotsPerItem;
-        if (it != p_item) {
-            p_item = it;
-            const int j = s_seq[it & 3];
-            if (j >= n_total) {
-                pm.s = 0;
-                return;
-            }
-            const int base = j / Hkv;
-            p_hk = j - base * Hkv;
-            const int2 rec = W.items[base];
-            pm.pos = rec.x;
-            pm.chunk = rec.y;
-            pm.b = W.perm[rec.x];
-            pm.s = seq_lens[pm.b];
-            const int n_row_pages = (pm.s + CC_PAGE - 1) / CC_PAGE;
+    if (warp == kCW) {
+        // ===================== producer: whole pages by TMA =====================
+        // CTAs in use: every one of them gets at least one page, so the CTAs that share a row are consecutive
+        const long long n_cta = min((int)gridDim.x, max(T, 1));
+        auto cta_of_page = [&](int x) { return (int)((((long long)x + 1) * n_cta - 1) / T); };   // inverse of the cut
+        const bool idle = (long long)blockIdx.x >= n_cta;
+        const int P0 = idle ? 0 : (int)((long long)T * blockIdx.x / n_cta);
+        const int P1 = idle ? 0 : (int)((long long)T * (blockIdx.x + 1) / n_cta);
+        const uint64_t pol = policy_evict_first();
+        int stage = 0;
+        uint32_t ph = 0;
+        int b = 0;
+        if (P0 < P1) {                                            // row that holds page P0
+            int cntb = 0;
+            for (int i = lane; i < D.max_batch; i += 32) cntb += (s_prefix[i + 1] <= P0);
 #pragma unroll
-            for (int h = 0; h < 2; ++h) {
-                const int pg = pm.chunk * kPagesPerChunk + lane + 32 * h;
-                int id = 0;
-                if (lane + 32 * h < kPagesPerChunk && pg < n_row_pages) {
-                    id = kv.block_table[(size_t)pm.b * D.max_blocks + pg];
-                    if (id < 0 || id >= kv.n_pages) {
-                        atomicOr(W.err, CC_DEVERR_BAD_PAGE);
-                        id = 0;
+            for (int sft = 16; sft > 0; sft >>= 1) cntb += __shfl_xor_sync(0xffffffffu, cntb, sft);
+            b = cntb;
+        }
+        int p = P0;
+        while (p < P1) {
+            const int r0 = s_prefix[b], r1 = s_prefix[b + 1];
+            if (r1 <= p) { ++b; continue; }                       // rows without pages (padding)
+            const int q0 = p - r0, q1 = min(r1, P1) - r0;         // this CTA's pages of row b
+            const int pos = W.pos_of[b], s = seq_lens[b];
+            const int slot0 = b + cta_of_page(r0), n_pieces = cta_of_page(r1 - 1) - cta_of_page(r0) + 1;
+            const int slot = b + (int)blockIdx.x;
+            const int n_groups = (q1 - q0 + PPS - 1) / PPS;
+            int id = 0, id_base = -32;                            // lane l: id of page q0 + id_base + l of the row
+            for (int g = 0; g < n_groups; ++g) {
+                const int rel = g * PPS, qg = q0 + rel;           // first page of the group
+                if (rel >= id_base + 32) {                        // next 32 page ids (32 % PPS == 0: groups never straddle)
+                    id_base = rel;
+                    const int q = qg + lane;
+                    id = 0;
+                    if (q < q1) {
+                        id = kv.block_table[(size_t)b * D.max_blocks + q];
+                        if (id < 0 || id >= kv.n_pages) {
+                            atomicOr(W.err, CC_DEVERR_BAD_PAGE);
+                            id = 0;
+                        }
                     }
                 }
-                p_page_id[h] = id;
-            }
-        }
-        const int pl = warp + i * kAttnWarps;                       // page within the chunk
-        const int tok0 = pm.chunk * CC_ATTN_CHUNK + pl * CC_PAGE;   // first token of the page
-        const int page0 = __shfl_sync(0xffffffffu, p_page_id[0], pl & 31), page1 = __shfl_sync(0xffffffffu, p_page_id[1], pl & 31);
-        const int page = pl < 32 ? page0 : page1;
-        // warp-uniform values + elect.sync keep the TMA issue on the uniform datapath (no per-lane waterfall)
-        const int do_load = uniform((int)(tok0 < pm.s));
-        const int row0 = uniform((page * Hkv + p_hk) * CC_PAGE);     // row of the pool seen as [pages*Hkv*16][DH]
-        const int st = k % kAttnStages;
-        if (do_load && elect_one()) {
-            const uint32_t dstK = ring_u32 + (uint32_t)st * C::kStageBytes, dstV = dstK + C::kPageBytes;
-            const uint32_t bar = smem_u32(&bars[st]);
-            mbar_expect_tx(&bars[st], C::kStageBytes);
+                mbar_wait(&empty[stage], ph ^ 1);
+                const int in_grp = min(PPS, q1 - qg);
+                int pid[kCW];
 #pragma unroll
-            for (int h = 0; h < DH / 64; ++h) {                       // boxes of 16 tokens x 64 dims (128 bytes)
-                tma_load_2d(dstK + h * 2048, &tmK, h * 64, row0, bar);
-                tma_load_2d(dstV + h * 2048, &tmV, h * 64, row0, bar);
+                for (int pp = 0; pp < kCW; ++pp) pid[pp] = __shfl_sync(0xffffffffu, id, (rel - id_base + pp) & 31);
+                if (elect_one()) {
+                    StageMeta m;
+                    m.pos = pos; m.s = s; m.pg = qg; m.slot = slot; m.slot0 = slot0; m.n_pieces = n_pieces; m.n_in = in_grp;
+                    m.flags = (g == 0 ? kMetaFirst : 0) | (g == n_groups - 1 ? kMetaLast : 0);
+                    meta[stage] = m;
+                    mbar_expect_tx(&full[stage], (uint32_t)in_grp * page_bytes);
+                    const uint32_t bar = smem_u32(&full[stage]);
+                    const uint32_t dst0 = ring_u32 + (uint32_t)stage * C::kStageBytes;
+#pragma unroll
+                    for (int pp = 0; pp < kCW; ++pp) {
+                        if (pp < in_grp) {
+                            const int row0 = pid[pp] * Hkv * CC_PAGE;  // the pool seen as [pages * Hkv * 16 rows][DH]
+                            const uint32_t dst = dst0 + (uint32_t)pp * page_bytes;
+#pragma unroll
+                            for (int h = 0; h < DH / 64; ++h) {
+                                tma_load_2d_hint(dst + h * half_bytes, &tmK, h * 64, row0, bar, pol);
+                                tma_load_2d_hint(dst + kv_bytes + h * half_bytes, &tmV, h * 64, row0, bar, pol);
+                            }
+                        }
+                    }
+                }
+                if (++stage == kAttnStages) { stage = 0; ph ^= 1; }
             }
+            p = r0 + q1;
+            ++b;
         }
-    };
+        // end marker for the consumers
+        mbar_wait(&empty[stage], ph ^ 1);
+        if (elect_one()) {
+            meta[stage].flags = kMetaEnd;
+            mbar_arrive(&full[stage]);
+        }
+        // out of items: warm L2 with the head of the O-projection weight stream of the first non-empty group
+        if (lane == 0) {
+            int r0 = 0;
+            while (r0 < CC_MAXR - 1 && W.sched->cnt[r0] == 0) ++r0;
+            for (int c = blockIdx.x; c < D.o.P; c += gridDim.x) cc_prefetch_gemm_head(D.o, tab->rep[r0].blob, c);
+        }
+        return;
+    }
 
-    for (int k = 0; k < kAttnStages - 1; ++k) prefetch(k);
-    uint32_t phases = 0;                                   // bit st = parity of the next completion of stage st
-
-    // ---- consumer state ----------------------------------------------------------------------
-    ItemMeta cm = {0, 0, 0, 0};
-    int c_hk = 0;
+    // ===================== consumers: warp w = kv head w % Hkv of page w / Hkv of the stage =====================
+    const int h = warp % Hkv, pp = warp / Hkv;
+    const int g = lane >> 2, t4 = lane & 3;
+    float* my_merge = merge + (size_t)warp * G * C::kMergeStride;
+    int stage = 0;
+    uint32_t ph = 0;
     uint32_t qa0[DH / 16], qa2[DH / 16];   // Q fragments (rows g < G), scaled by log2(e)/sqrt(Dh)
     float o[DH / 8][4];
     float m_run = -INFINITY, l_run = 0.f;
+#pragma unroll
+    for (int nt = 0; nt < DH / 8; ++nt) o[nt][0] = o[nt][1] = o[nt][2] = o[nt][3] = 0.f;
 
-    int next_id = 0;                                       // thread 0: the id drawn for seq[it + 2]
-    for (int k = 0;; ++k) {
-        const int it = k / kSlotsPerItem, i = k % kSlotsPerItem;
-        if (i == 0 && s_seq[it & 3] >= n_total) break;     // CTA-uniform: the list is exhausted
-        prefetch(k + kAttnStages - 1);
-
-        if (i == 0) {   // new item: metadata, Q fragments, reset the running softmax state
-            if (threadIdx.x == 0) next_id = (int)gridDim.x + atomicAdd(W.attn_ctr, 1);
-            const int j = s_seq[it & 3];
-            const int base = j / Hkv;
-            c_hk = j - base * Hkv;
-            const int2 rec = W.items[base];
-            cm.pos = rec.x;
-            cm.chunk = rec.y;
-            cm.b = W.perm[rec.x];
-            cm.s = seq_lens[cm.b];
-            const float* qrow = W.q_rot + (size_t)cm.pos * D.QD + (size_t)(c_hk * G + g) * DH;
+    for (;;) {
+        mbar_wait(&full[stage], ph);
+        const StageMeta m = meta[stage];
+        if (m.flags & kMetaEnd) break;
+        if (m.flags & kMetaFirst) {   // new item: Q fragments, reset the running softmax state
+            const float* qrow = W.q_rot + (size_t)m.pos * D.QD + (size_t)(h * G + g) * DH;
 #pragma unroll
             for (int ks = 0; ks < DH / 16; ++ks) {
                 float2 x0 = make_float2(0.f, 0.f), x1 = make_float2(0.f, 0.f);
@@ -172,27 +209,18 @@ k_attn(const int* __restrict__ seq_lens, CcKv kv, CcDims D, CcWork W, const CcLa
                 qa0[ks] = pack_bf16(x0.x * D.qk_scale_log2, x0.y * D.qk_scale_log2);
                 qa2[ks] = pack_bf16(x1.x * D.qk_scale_log2, x1.y * D.qk_scale_log2);
             }
-#pragma unroll
-            for (int nt = 0; nt < DH / 8; ++nt) o[nt][0] = o[nt][1] = o[nt][2] = o[nt][3] = 0.f;
-            m_run = -INFINITY;
-            l_run = 0.f;
         }
-
-        const int pl = warp + i * kAttnWarps;
-        const int tok0 = cm.chunk * CC_ATTN_CHUNK + pl * CC_PAGE;
-        if (tok0 < cm.s) {
-            const int valid = min(CC_PAGE, cm.s - tok0);
-            const int st = k % kAttnStages;
-            const uint32_t sK = ring_u32 + (uint32_t)st * C::kStageBytes;
-            const uint32_t sV = sK + C::kPageBytes;
-            mbar_wait(&bars[st], (phases >> st) & 1u);
-            phases ^= 1u << st;
+        const int tok0 = (m.pg + pp) * CC_PAGE;
+        if (pp < m.n_in) {   // (then tok0 < s: the piece only holds pages of the context)
+            const int valid = min(CC_PAGE, m.s - tok0);
+            const uint32_t sK = ring_u32 + (uint32_t)stage * C::kStageBytes + (uint32_t)pp * page_bytes + (uint32_t)h * 2048u;
+            const uint32_t sV = sK + kv_bytes;
             if (valid < CC_PAGE) {   // ragged last page: the V rows past seq_len hold other data; p = 0 must meet 0
                 for (int q = lane; q < (CC_PAGE - valid) * (DH / 8); q += 32) {
                     const int r = valid + q / (DH / 8), c = q % (DH / 8);
-                    asm volatile("st.shared.v4.b32 [%0], {%1, %1, %1, %1};" ::"r"(sV + (c >> 3) * 2048 + r * 128 + ((c & 7) << 4)), "r"(0) : "memory");
+                    asm volatile("st.shared.v4.b32 [%0], {%1, %1, %1, %1};" ::"r"(sV + (c >> 3) * half_bytes + r * 128 + ((c & 7) << 4)), "r"(0) : "memory");
                 }
-                fence_proxy_async_smem();   // a later TMA refill of this stage must not pass these stores
+                fence_proxy_async_smem();   // the TMA refill of this stage must not pass these stores
                 __syncwarp();
             }
             // ---- scores: S[16 x 16] = Q[16 x DH] . K^T
@@ -205,7 +233,7 @@ k_attn(const int* __restrict__ seq_lens, CcKv kv, CcDims D, CcWork W, const CcLa
                 for (int ks = 0; ks < DH / 16; ++ks) {
                     const int ch = ks * 2 + (mi & 1);
                     uint32_t r0, r1, r2, r3;
-                    ldsm_x4(rowaddr + (uint32_t)((ch >> 3) * 2048 + (((ch & 7) ^ (tok & 7)) << 4)), r0, r1, r2, r3);
+                    ldsm_x4(rowaddr + (uint32_t)(ch >> 3) * half_bytes + (uint32_t)(((ch & 7) ^ (tok & 7)) << 4), r0, r1, r2, r3);
                     mma_bf16_16816(s0, qa0[ks], 0u, qa2[ks], 0u, r0, r1);
                     mma_bf16_16816(s1, qa0[ks], 0u, qa2[ks], 0u, r2, r3);
                 }
@@ -233,7 +261,7 @@ k_attn(const int* __restrict__ seq_lens, CcKv kv, CcDims D, CcWork W, const CcLa
                 for (int jn = 0; jn < DH / 16; ++jn) {
                     const int ch = jn * 2 + (mi >> 1);
                     uint32_t r0, r1, r2, r3;
-                    ldsm_x4_trans(rowaddr + (uint32_t)((ch >> 3) * 2048 + (((ch & 7) ^ (tok & 7)) << 4)), r0, r1, r2, r3);
+                    ldsm_x4_trans(rowaddr + (uint32_t)(ch >> 3) * half_bytes + (uint32_t)(((ch & 7) ^ (tok & 7)) << 4), r0, r1, r2, r3);
                     o[2 * jn][0] *= alpha; o[2 * jn][1] *= alpha;
                     o[2 * jn + 1][0] *= alpha; o[2 * jn + 1][1] *= alpha;
                     mma_bf16_16816(o[2 * jn], pa0, 0u, pa2, 0u, r0, r1);
@@ -241,108 +269,134 @@ k_attn(const int* __restrict__ seq_lens, CcKv kv, CcDims D, CcWork W, const CcLa
                 }
             }
         }
-        __syncwarp();   // all lanes are done with this stage before a later prefetch overwrites it
+        __syncwarp();                                  // every lane is done with the stage
+        if (lane == 0) mbar_arrive(&empty[stage]);
+        if (++stage == kAttnStages) { stage = 0; ph ^= 1; }
+        if (!(m.flags & kMetaLast)) continue;
 
-        if (i == kSlotsPerItem - 1) {
-            // ---- merge the 4 warps of the CTA in fixed order, write the chunk partial
-            float l_tot = l_run;
-            l_tot += __shfl_xor_sync(0xffffffffu, l_tot, 1);
-            l_tot += __shfl_xor_sync(0xffffffffu, l_tot, 2);
-            if (g < G) {
-                float* mrow = merge + (size_t)(warp * G + g) * C::kMergeStride;
+        // ---------------- end of the chunk: merge, write the partial (or the final operand) ----------------
+        float l_tot = l_run;
+        l_tot += __shfl_xor_sync(0xffffffffu, l_tot, 1);
+        l_tot += __shfl_xor_sync(0xffffffffu, l_tot, 2);
+        if (g < G) {
+            float* mrow = my_merge + (size_t)g * C::kMergeStride;
 #pragma unroll
-                for (int nt = 0; nt < DH / 8; ++nt)
-                    *reinterpret_cast<float2*>(mrow + nt * 8 + 2 * t4) = make_float2(o[nt][0], o[nt][1]);
-                if (t4 == 0) {
-                    mrow[DH] = m_run;
-                    mrow[DH + 1] = l_tot;
-                }
+            for (int nt = 0; nt < DH / 8; ++nt)
+                *reinterpret_cast<float2*>(mrow + nt * 8 + 2 * t4) = make_float2(o[nt][0], o[nt][1]);
+            if (t4 == 0) {
+                mrow[DH] = m_run;
+                mrow[DH + 1] = l_tot;
             }
-            if (threadIdx.x == 0) s_seq[(it + 2) & 3] = next_id;
-            __syncthreads();
-            const int nch = (cm.s + CC_ATTN_CHUNK - 1) / CC_ATTN_CHUNK;     // CTA-uniform
-            for (int e = 2 * threadIdx.x; e < G * DH; e += 2 * kAttnThreads) {
-                const int hg = e / DH, dim = e - hg * DH;
+        }
+        // the accumulators are dead now: reset them here, so that nothing of the chunk loop stays live
+        // through the code below (the next stage of this warp starts a new item)
+#pragma unroll
+        for (int nt = 0; nt < DH / 8; ++nt) o[nt][0] = o[nt][1] = o[nt][2] = o[nt][3] = 0.f;
+        m_run = -INFINITY;
+        l_run = 0.f;
+        if (PPS > 1) named_bar_sync(kBarMerge, kCW * 32); else __syncwarp();
+        // the first warp of each kv head combines the PPS warps of that head (fixed order); from here on
+        // lane l owns dims 4l .. 4l+3 of every q head of the group
+        const int dim = lane * 4;
+        const int nch = m.n_pieces;
+        auto store_operand = [&](int q, float4 v, float inv) {   // bf16 row of the O-projection operand (one plane)
+            const int col = (h * G + q) * DH + dim;
+            uint8_t* dst = W.o_act + act_chunk_off(m.pos, col, D.Mpad, 1, 0) + (col & 7) * 2;
+            *reinterpret_cast<uint2*>(dst) = make_uint2(pack_bf16(v.x * inv, v.y * inv), pack_bf16(v.z * inv, v.w * inv));
+        };
+        if (pp == 0 && dim < DH) {
+#pragma unroll 1
+            for (int q = 0; q < G; ++q) {
                 float M = -INFINITY;
-#pragma unroll
-                for (int w = 0; w < kAttnWarps; ++w) M = fmaxf(M, merge[(size_t)(w * G + hg) * C::kMergeStride + DH]);
-                float a0 = 0.f, a1 = 0.f, L = 0.f;
-#pragma unroll
-                for (int w = 0; w < kAttnWarps; ++w) {
-                    const float* mr = merge + (size_t)(w * G + hg) * C::kMergeStride;
+                for (int p = 0; p < PPS; ++p) M = fmaxf(M, merge[(size_t)((h + p * Hkv) * G + q) * C::kMergeStride + DH]);
+                float4 a = make_float4(0.f, 0.f, 0.f, 0.f);
+                float L = 0.f;
+                for (int p = 0; p < PPS; ++p) {
+                    const float* mr = merge + (size_t)((h + p * Hkv) * G + q) * C::kMergeStride;
                     const float sc = exp2f(mr[DH] - M);
-                    a0 += sc * mr[dim];
-                    a1 += sc * mr[dim + 1];
+                    const float4 v = *reinterpret_cast<const float4*>(mr + dim);
+                    a.x += sc * v.x; a.y += sc * v.y; a.z += sc * v.z; a.w += sc * v.w;
                     L += sc * mr[DH + 1];
                 }
-                const int hq = c_hk * G + hg;
-                if (nch == 1) {   // the only chunk of this row: normalise and write the O-projection operand
-                    const float inv = 1.f / L;
-                    const int col = hq * DH + dim;
-                    uint8_t* dst = W.o_act + act_chunk_off(cm.pos, col, D.Mpad, 1, 0) + (col & 7) * 2;
-                    *reinterpret_cast<uint32_t*>(dst) = pack_bf16(a0 * inv, a1 * inv);
+                if (nch == 1) {   // the only chunk of this row: normalise and write the operand
+                    store_operand(q, a, 1.f / L);
                 } else {
-                    const size_t row = ((size_t)cm.pos * D.Hq + hq) * W.nch_max + cm.chunk;
-                    *reinterpret_cast<float2*>(W.att_o + row * DH + dim) = make_float2(a0, a1);
-                    if (dim == 0) W.att_ml[row] = make_float2(M, L);
+                    const size_t row = (size_t)m.slot * D.Hq + h * G + q;
+                    *reinterpret_cast<float4*>(W.att_o + row * DH + dim) = a;
+                    if (lane == 0) W.att_ml[row] = make_float2(M, L);
                 }
             }
-            if (nch > 1) {
-                // ---- the CTA that finishes the pair's last chunk merges all of them, in chunk order
-                __threadfence();
-                __syncthreads();
-                if (threadIdx.x == 0) {
-                    int* cnt = W.attn_cnt + cm.pos * Hkv + c_hk;
-                    const int last = atomicAdd(cnt, 1) == nch - 1;
-                    if (last) *cnt = 0;                             // ready for the next step
-                    s_seq[4] = last;
-                }
-                __syncthreads();
-                if (s_seq[4]) {
-                    __threadfence();
-                    for (int e = 2 * threadIdx.x; e < G * DH; e += 2 * kAttnThreads) {
-                        const int hg = e / DH, dim = e - hg * DH, hq = c_hk * G + hg;
-                        const size_t row = ((size_t)cm.pos * D.Hq + hq) * W.nch_max;
-                        float M = -INFINITY;
-                        for (int c = 0; c < nch; ++c) M = fmaxf(M, __ldcg(&W.att_ml[row + c]).x);
-                        float L = 0.f, a0 = 0.f, a1 = 0.f;
-                        for (int c = 0; c < nch; ++c) {
-                            const float2 ml = __ldcg(&W.att_ml[row + c]);
-                            const float w = exp2f(ml.x - M);
-                            const float2 ov = __ldcg(reinterpret_cast<const float2*>(W.att_o + (row + c) * DH + dim));
-                            L += w * ml.y;
-                            a0 += w * ov.x;
-                            a1 += w * ov.y;
-                        }
-                        const float inv = 1.f / L;
-                        const int col = hq * DH + dim;
-                        uint8_t* dst = W.o_act + act_chunk_off(cm.pos, col, D.Mpad, 1, 0) + (col & 7) * 2;
-                        *reinterpret_cast<uint32_t*>(dst) = pack_bf16(a0 * inv, a1 * inv);
-                    }
-                }
-            }
-            __syncthreads();   // merge buffer and flags are reused by the next item
         }
-    }
-    // out of items: warm L2 with the head of the O-projection weight stream of the first non-empty group
-    if (threadIdx.x == 0) {
-        int r0 = 0;
-        while (r0 < CC_MAXR - 1 && W.sched->cnt[r0] == 0) ++r0;
-        cc_prefetch_gemm_head(D.o, tab->rep[r0].blob, (int)blockIdx.x);
+        if (PPS > 1) named_bar_sync(kBarMerge, kCW * 32); else __syncwarp();   // merge rows may be rewritten
+        if (pp != 0 || nch == 1) continue;
+        // ---- the warp that finishes the pair's last piece merges all of them, in piece order
+        __threadfence();
+        __syncwarp();
+        int last = 0;
+        if (lane == 0) {
+            int* cnt = W.attn_cnt + m.pos * Hkv + h;
+            last = atomicAdd(cnt, 1) == nch - 1;
+            if (last) *cnt = 0;                                 // ready for the next step
+        }
+        last = __shfl_sync(0xffffffffu, last, 0);
+        if (!last) continue;
+        __threadfence();
+        for (int q0 = 0; q0 < G; q0 += 4) {                         // four q heads x two chunks in flight
+            size_t row[4];
+            float M[4], L[4];
+            float4 a[4];
+#pragma unroll
+            for (int u = 0; u < 4; ++u) {
+                row[u] = (size_t)m.slot0 * D.Hq + h * G + min(q0 + u, G - 1);   // piece c of the row: + c * Hq
+                M[u] = -INFINITY; L[u] = 0.f; a[u] = make_float4(0.f, 0.f, 0.f, 0.f);
+            }
+            for (int c = lane; c < nch; c += 32) {
+#pragma unroll
+                for (int u = 0; u < 4; ++u) M[u] = fmaxf(M[u], __ldcg(&W.att_ml[row[u] + (size_t)c * D.Hq]).x);
+            }
+#pragma unroll
+            for (int u = 0; u < 4; ++u)
+#pragma unroll
+                for (int sft = 16; sft > 0; sft >>= 1) M[u] = fmaxf(M[u], __shfl_xor_sync(0xffffffffu, M[u], sft));
+            for (int c0 = 0; c0 < nch; c0 += 2) {               // added in piece order
+                float2 ml[4][2];
+                float4 v[4][2];
+#pragma unroll
+                for (int u = 0; u < 4; ++u)
+#pragma unroll
+                    for (int cc = 0; cc < 2; ++cc) {
+                        const bool ok = c0 + cc < nch;
+                        ml[u][cc] = ok ? __ldcg(&W.att_ml[row[u] + (size_t)(c0 + cc) * D.Hq]) : make_float2(-INFINITY, 0.f);
+                        v[u][cc] = (ok && dim < DH) ? __ldcg(reinterpret_cast<const float4*>(W.att_o + (row[u] + (size_t)(c0 + cc) * D.Hq) * DH + dim))
+                                                    : make_float4(0.f, 0.f, 0.f, 0.f);
+                    }
+#pragma unroll
+                for (int u = 0; u < 4; ++u)
+#pragma unroll
+                    for (int cc = 0; cc < 2; ++cc) {
+                        const float w = exp2f(ml[u][cc].x - M[u]);
+                        L[u] += w * ml[u][cc].y;
+                        a[u].x += w * v[u][cc].x; a[u].y += w * v[u][cc].y; a[u].z += w * v[u][cc].z; a[u].w += w * v[u][cc].w;
+                    }
+            }
+#pragma unroll
+            for (int u = 0; u < 4; ++u)
+                if (q0 + u < G && dim < DH) store_operand(q0 + u, a[u], 1.f / L[u]);
+        }
     }
 }
 
 }  // namespace
 
 cudaError_t cc_attn_configure() {
-    cudaError_t e = cudaFuncSetAttribute(k_attn<128>, cudaFuncAttributeMaxDynamicSharedMemorySize, 112 * 1024);
+    cudaError_t e = cudaFuncSetAttribute(k_attn<128>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)AttnCfg<128>::smem_bytes(8));
     if (e != cudaSuccess) return e;
-    return cudaFuncSetAttribute(k_attn<64>, cudaFuncAttributeMaxDynamicSharedMemorySize, 112 * 1024);
+    return cudaFuncSetAttribute(k_attn<64>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)AttnCfg<64>::smem_bytes(8));
 }
 
 // Tensor map of a caller-owned KV pool seen as a 2-D bf16 tensor [n_pages * Hkv * 16 rows][Dh], boxes of
-// 16 rows x 64 elements (128 bytes) with the 128-byte swizzle.  cuTensorMapEncodeTiled is a driver entry
-// point; it is looked up once through the runtime, so the library needs no link against libcuda.
+// one page (Hkv * 16 rows) x 64 elements (128 bytes) with the 128-byte swizzle.  cuTensorMapEncodeTiled is
+// a driver entry point; it is looked up once through the runtime, so the library needs no link against libcuda.
 static cudaError_t make_kv_tensor_map(CUtensorMap* out, const void* pool, int n_pages, int Hkv, int Dh) {
     typedef CUresult (*EncodeFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
                                  const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
@@ -358,7 +412,7 @@ static cudaError_t make_kv_tensor_map(CUtensorMap* out, const void* pool, int n_
     }
     const cuuint64_t dims[2] = {(cuuint64_t)Dh, (cuuint64_t)n_pages * Hkv * CC_PAGE};
     const cuuint64_t strides[1] = {(cuuint64_t)Dh * 2};
-    const cuuint32_t box[2] = {64, CC_PAGE};
+    const cuuint32_t box[2] = {64, (cuuint32_t)(Hkv * CC_PAGE)};
     const cuuint32_t estr[2] = {1, 1};
     const CUresult r = encode(out, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, const_cast<void*>(pool), dims, strides, box, estr,
                               CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
@@ -372,7 +426,7 @@ cudaError_t cc_launch_attention(const int* seq_lens, const CcKv& kv, const CcDim
     cudaError_t e = make_kv_tensor_map(&tmK, kv.k_pool, kv.n_pages, D.Hkv, D.Dh);
     if (e == cudaSuccess) e = make_kv_tensor_map(&tmV, kv.v_pool, kv.n_pages, D.Hkv, D.Dh);
     if (e != cudaSuccess) return e;
-    const dim3 grid(2 * L.n_sms), block(kAttnThreads);
+    const dim3 grid(L.n_sms), block(kAttnThreads);
     if (D.Dh == 128)
         return cc_launch_kernel(k_attn<128>, grid, block, AttnCfg<128>::smem_bytes(D.G), L, seq_lens, kv, D, W, tab, tmK, tmV);
     return cc_launch_kernel(k_attn<64>, grid, block, AttnCfg<64>::smem_bytes(D.G), L, seq_lens, kv, D, W, tab, tmK, tmV);

@@ -13,7 +13,6 @@
 #define CC_ROW_ALIGN 16        // group offsets are multiples of this (UMMA N granularity)
 #define CC_MAX_MPAD 320        // (256 rows + 16 * CC_MAXR group padding): upper bound of CcDims::Mpad
 #define CC_FLAG_STRIDE 256     // stream-K fixup counters per projection (>= super tiles of any projection)
-#define CC_ATTN_CHUNK 1024     // tokens per split-KV work item (a function of nothing but this)
 
 #define CC_DEVERR_BAD_REPLICA 1u
 #define CC_DEVERR_BAD_PAGE 2u
@@ -93,7 +92,7 @@ struct CcSched {
     int cnt[CC_MAXR];      // rows in replica group r
     int goff[CC_MAXR];     // first grouped position of group r (multiple of 16)
     int n_pos;             // grouped positions in use (end of the last group, multiple of 16)
-    int n_items;           // attention work items (pos, chunk); x Hkv inside the kernel
+    int n_items;           // KV pages of the whole batch (the attention work axis)
     int nmax;              // largest padded group size (UMMA N of the widest group)
     int pad_[5];
 };
@@ -206,6 +205,14 @@ __device__ __forceinline__ void tma_load_2d(uint32_t dst_smem, const void* tmap,
     asm volatile(
         "cp.async.bulk.tensor.2d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3}], [%4];" ::"r"(dst_smem),
         "l"(tmap), "r"(c0), "r"(c1), "r"(bar_smem)
+        : "memory");
+}
+__device__ __forceinline__ void tma_load_2d_hint(uint32_t dst_smem, const void* tmap, int c0, int c1, uint32_t bar_smem,
+                                                 uint64_t policy) {
+    asm volatile(
+        "cp.async.bulk.tensor.2d.shared::cluster.global.mbarrier::complete_tx::bytes.L2::cache_hint [%0], [%1, {%2, %3}], [%4], %5;" ::
+            "r"(dst_smem),
+        "l"(tmap), "r"(c0), "r"(c1), "r"(bar_smem), "l"(policy)
         : "memory");
 }
 __device__ __forceinline__ uint64_t policy_evict_first() {

@@ -6,7 +6,8 @@
 struct CcWork {
     CcSched* sched;
     int* perm;           // [Mpad] original row at grouped position, or -1
-    int2* items;         // attention work items (pos, chunk), at most max_batch * nch_max
+    int* pg_prefix;      // [max_batch + 1] pages of the rows before row b, request order (attention work split)
+    int* pos_of;         // [max_batch] grouped position of row b, or -1
     uint8_t* x_act;      // packed bf16 GEMM operands, [K/64][Mpad/8][plane hi|lo][8][128 B swizzled]
     uint8_t* o_act;      // (one plane)
     uint8_t* y_act;
@@ -19,13 +20,11 @@ struct CcWork {
     float* h1;           // [Mpad][d]     fp32, hidden + O projection
     float* ssq;          // [d/128][Mpad] fp32, per-tile sum of squares of h1 (post-attention RMSNorm statistic)
     int* flags;          // [4][CC_FLAG_STRIDE] stream-K fixup counters, zeroed by k_group every step
-    int* attn_ctr;       // next attention work item (zeroed by k_group every step)
-    int* attn_cnt;       // [Mpad][Hkv] chunks finished per (row, kv head); the last finisher merges and resets
-    float* att_o;        // [Mpad*Hq][nch_max][Dh] fp32 un-normalised chunk outputs
-    float2* att_ml;      // [Mpad*Hq][nch_max] (max in log2 units, sum)
+    int* attn_cnt;       // [Mpad][Hkv] pieces finished per (row, kv head); the last finisher merges and resets
+    float* att_o;        // [max_batch + SMs][Hq][Dh] fp32 un-normalised piece outputs (slot = row + CTA)
+    float2* att_ml;      // [max_batch + SMs][Hq] (max in log2 units, sum)
     const float2* rope_cs;  // [max_position][Dh/2] (cos, sin), built in fp64 on the host
     uint32_t* err;       // sticky device error word (context-owned)
-    int nch_max;
 };
 
 struct CcKv {

@@ -50,14 +50,13 @@ __device__ __forceinline__ void split_hilo(float v0, float v1, uint32_t& hi, uin
 __global__ void __launch_bounds__(256) k_group(const int* __restrict__ assign, const int* __restrict__ seq_lens,
                                                int batch, CcDims D, const CcLayerTable* __restrict__ tab, CcWork W) {
     __shared__ int s_wcnt[8][CC_MAXR];     // rows of replica r in warp w
-    __shared__ int s_wnch[8];              // attention chunks in warp w (full | ragged << 16)
+    __shared__ int s_wnch[8];              // KV pages of the rows of warp w
     __shared__ int s_goff[CC_MAXR + 1], s_cnt[CC_MAXR];
-    __shared__ int s_rem[256];             // tokens in the ragged last chunk of row b (0: none)
     const int b = threadIdx.x, warp = b >> 5, lane = b & 31;
     pdl_wait();
     pdl_launch_dependents();
     const uint32_t mask = tab->active_mask;
-    int rep = -1, nch = 0;
+    int rep = -1;
     if (b < batch) {
         const int s = seq_lens[b];
         if (s > 0) {
@@ -69,7 +68,6 @@ __global__ void __launch_bounds__(256) k_group(const int* __restrict__ assign, c
                     atomicOr(W.err, CC_DEVERR_BAD_REPLICA);
                     rep = 0;
                 }
-                nch = (s + CC_ATTN_CHUNK - 1) / CC_ATTN_CHUNK;
             }
         }
     }
@@ -109,34 +107,27 @@ __global__ void __launch_bounds__(256) k_group(const int* __restrict__ assign, c
         pos = s_goff[rep] + rank;
         W.perm[pos] = b;
     }
-    // work list: every full chunk first (request order), then the ragged last chunks, longest first, so
-    // that the attention CTAs, which draw items from a counter, finish on the shortest ones
-    const int nfull = (rep >= 0) ? seq_lens[b] / CC_ATTN_CHUNK : 0, npart = nch - nfull;
-    int pre = nfull | (npart << 16);                      // two prefix sums in one scan (each < 2^16)
+    // attention work split: pages of the rows in request order (prefix sums); the attention CTAs cut this
+    // page axis into equal contiguous ranges -- a function of the batch, never of the replica split
+    if (b < D.max_batch) W.pos_of[b] = pos;
+    const int npg = (rep >= 0) ? (seq_lens[b] + CC_PAGE - 1) / CC_PAGE : 0;
+    int pre = npg;
 #pragma unroll
     for (int o = 1; o < 32; o <<= 1) {
         const int v = __shfl_up_sync(0xffffffffu, pre, o);
         if (lane >= o) pre += v;
     }
     if (lane == 31) s_wnch[warp] = pre;
-    const int rem = npart ? seq_lens[b] % CC_ATTN_CHUNK : 0;
-    s_rem[b] = rem;
     __syncthreads();
-    int base = pre - (nfull | (npart << 16)), tot = 0;
+    int base = pre - npg, total = 0;
     for (int w = 0; w < 8; ++w) {
         if (w < warp) base += s_wnch[w];
-        tot += s_wnch[w];
+        total += s_wnch[w];
     }
-    const int total_full = tot & 0xffff, total = total_full + (tot >> 16);
-    for (int c = 0; c < nfull; ++c) W.items[(base & 0xffff) + c] = make_int2(pos, c);
-    if (npart) {
-        int rank = 0;                                      // ragged chunks longer than this one (ties: lower row first)
-        for (int o = 0; o < 256; ++o) rank += (s_rem[o] > rem) || (s_rem[o] == rem && o < b);
-        W.items[total_full + rank] = make_int2(pos, nfull);
-    }
+    if (b < D.max_batch) W.pg_prefix[b] = base;
+    if (b == 0) W.pg_prefix[D.max_batch] = total;
     if (b == 0) {
         int nmax = 0;
-        *W.attn_ctr = 0;                                   // dynamic item counter of the attention kernel
         for (int r = 0; r < CC_MAXR; ++r) {
             W.sched->cnt[r] = s_cnt[r];
             W.sched->goff[r] = s_goff[r];
