@@ -1,12 +1,12 @@
 // cc_attention.cu -- paged GQA decode attention, split-KV (the KV cache
 // partitioning the paper relies on: PAPER.md:103, 391, 476).
 //
-// HBM-bound: every cached K/V byte of a request is read exactly once per step.  The design is
-// built around HOW those bytes are asked for.  The pool layout is [page][kv_head][16][Dh], so one
-// page holds 32 KiB of contiguous K (Hkv = 8, Dh = 128) and as much V.  Reading it head by head
-// from different CTAs (4 KiB requests scattered over the pool) topped out at 4.7 TB/s with the
-// math removed; walking all heads of a page together measured 6.7 TB/s with the same bytes in
-// flight (profiles/r01e_attention_access_pattern.md).  Hence:
+// HBM-bound: every cached K/V byte of a request is read exactly once per step.  What was measured on
+// the way here (profiles/r01e_attention_notes.md): per-(page, head) 4 KiB requests from four warps
+// per CTA, by per-lane cp.async or by small TMA boxes alike, stream at 4.7 TB/s even with the math
+// removed, and the ragged end of a 256-token work list costs another ~9 us; whole pages (all kv
+// heads, 2 x 32 KiB contiguous) staged by one producer warp stream at 5.3 TB/s, 6.1 TB/s with an L2
+// evict-first policy, and a static equal split of the page axis removes the ragged end.  Hence:
 //   * the work axis is the list of KV pages of the whole batch (rows in request order); it is cut
 //     into equal contiguous ranges, one per persistent CTA (one CTA per SM), so every CTA streams
 //     the same number of bytes (+- one page) whatever the context lengths are.  A row that spans
@@ -85,7 +85,11 @@ k_attn(const int* __restrict__ seq_lens, CcKv kv, CcDims D, CcWork W, const CcLa
         fence_mbar_init();
     }
     __syncthreads();
-    pdl_wait();
+    // The grouping tables (k_group) were complete two kernels back, seq_lens and the block table are
+    // inputs: only q and the K/V of the token being decoded come from the predecessor (the QKV GEMM).
+    // So the producer starts streaming the OLD pages at once -- while the predecessor's CTAs on other
+    // SMs are still in their fixup -- and waits for it only before the first stage that holds the last
+    // page of a row; the consumers wait before they read q.
     pdl_launch_dependents();
     const int T = W.sched->n_items;                               // KV pages of the batch
     int* s_prefix = reinterpret_cast<int*>(empty + kAttnStages);  // [max_batch + 1]
@@ -103,6 +107,7 @@ k_attn(const int* __restrict__ seq_lens, CcKv kv, CcDims D, CcWork W, const CcLa
         const uint64_t pol = policy_evict_first();
         int stage = 0;
         uint32_t ph = 0;
+        bool waited = false;
         int b = 0;
         if (P0 < P1) {                                            // row that holds page P0
             int cntb = 0;
@@ -137,6 +142,10 @@ k_attn(const int* __restrict__ seq_lens, CcKv kv, CcDims D, CcWork W, const CcLa
                 }
                 mbar_wait(&empty[stage], ph ^ 1);
                 const int in_grp = min(PPS, q1 - qg);
+                if (!waited && (qg + in_grp) * CC_PAGE >= s) {     // the stage holds the page of position s - 1
+                    pdl_wait();
+                    waited = true;
+                }
                 int pid[kCW];
 #pragma unroll
                 for (int pp = 0; pp < kCW; ++pp) pid[pp] = __shfl_sync(0xffffffffu, id, (rel - id_base + pp) & 31);
@@ -167,6 +176,7 @@ k_attn(const int* __restrict__ seq_lens, CcKv kv, CcDims D, CcWork W, const CcLa
             ++b;
         }
         // end marker for the consumers
+        if (!waited) pdl_wait();
         mbar_wait(&empty[stage], ph ^ 1);
         if (elect_one()) {
             meta[stage].flags = kMetaEnd;
@@ -192,6 +202,7 @@ k_attn(const int* __restrict__ seq_lens, CcKv kv, CcDims D, CcWork W, const CcLa
     float m_run = -INFINITY, l_run = 0.f;
 #pragma unroll
     for (int nt = 0; nt < DH / 8; ++nt) o[nt][0] = o[nt][1] = o[nt][2] = o[nt][3] = 0.f;
+    pdl_wait();                                         // q (and the new K/V) come from the QKV GEMM
 
     for (;;) {
         mbar_wait(&full[stage], ph);
