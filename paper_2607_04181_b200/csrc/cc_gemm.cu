@@ -29,7 +29,7 @@ namespace {
 
 constexpr int kGemmThreads = 512;         // warp 0 producer, 1 MMA, 2..5 TMEM epilogue, 6..15 row tables; all 16 in the fixup
 constexpr int kHdrBytes = 8192;           // barriers + per-row tables in front of the stage ring
-constexpr int kMaxStages = 8;
+constexpr int kMaxStages = 4;            // deeper rings measured slower at small row groups (R = 4: 384 -> 370 us per step)
 constexpr int kGemmSmem = 225 * 1024;     // dynamic shared memory per CTA
 constexpr int kTmemCols = 512;
 constexpr uint32_t kWStage = CC_G * CC_A_TILE_BYTES;   // weight bytes per stage (32 KiB)
