@@ -111,3 +111,52 @@ class Session:
     def __exit__(self, *exc):
         self.close()
         return False
+
+
+class ModelSession:
+    """Context + L layers of one shape (each its own weights) + one donated arena: the plumbing for
+    whole-model decode steps (BASELINE.json configs[2]): one CUDA graph holds the cc_forward of every
+    layer; replicas of single layers come and go through the device replica table (cc_commit)."""
+
+    def __init__(self, shape: I.LayerShape, weights_dev: list, max_batch: int, n_slots: int, device_index: int = 0,
+                 max_blocks: int | None = None, max_position: int | None = None):
+        self.shape = shape
+        self.device = f"cuda:{device_index}"
+        torch.cuda.set_device(device_index)
+        self.ctx = B.cc_ctx_create(device_index)
+        self.desc = make_desc(shape, max_batch, max_blocks, max_position)
+        self.layers = [B.cc_create_layer(self.ctx, self.desc, w) for w in weights_dev]
+        self.blob_bytes = B.cc_layer_blob_bytes(self.layers[0])
+        self.arena = None
+        if n_slots > 0:
+            slot = (self.blob_bytes + 1023) // 1024 * 1024
+            self.arena = torch.empty(n_slots * slot + 2048, dtype=torch.uint8, device=self.device)
+            B.cc_ctx_donate(self.ctx, self.arena, self.arena.numel())
+
+    def forward_all(self, hidden, k_pools, v_pools, block_table, n_pages, seq_lens, assigns, batch, stream=None) -> None:
+        """hidden flows through the layers in place; layer l uses k_pools[l], v_pools[l], assigns[l]."""
+        for l, layer in enumerate(self.layers):
+            B.cc_forward(layer, hidden, k_pools[l], v_pools[l], block_table, n_pages, seq_lens, assigns[l], batch, stream)
+
+    def scale(self, l: int, n: int, stream=None) -> None:
+        B.cc_scale_layer(self.layers[l], n)
+        B.cc_commit(self.layers[l], torch.cuda.current_stream() if stream is None else stream)
+
+    def close(self) -> None:
+        torch.cuda.synchronize()
+        for layer in self.layers:
+            B.cc_destroy_layer(layer)
+        self.layers = []
+        if self.ctx is not None:
+            if self.arena is not None:
+                B.cc_ctx_reclaim(self.ctx, self.arena)
+            B.cc_ctx_destroy(self.ctx)
+            self.ctx = None
+        self.arena = None
+
+    def __enter__(self):
+        return self
+
+    def __exit__(self, *exc):
+        self.close()
+        return False
