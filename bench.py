@@ -47,6 +47,9 @@ def parse_args():
     ap.add_argument("--replicas", type=int, default=2, choices=[1, 2, 3, 4])
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--workload", default="cfg2", choices=["cfg2", "cfg3"],
+                    help="cfg2 (default): the headline layer benchmark; cfg3: BASELINE.json configs[2], the 32-layer "
+                         "decode graph with layers 10-12 flipped to 2 replicas and back (latency series, not the headline)")
     return ap.parse_args()
 
 
@@ -382,10 +385,132 @@ def run_ours(args):
     return 0
 
 
+# ---------------------------------------------------------------------------------------------
+# cfg3 (BASELINE.json configs[2]): whole-model decode graph with mid-run layer flips
+# ---------------------------------------------------------------------------------------------
+def run_cfg3(args):
+    import torch
+
+    from paper_2607_04181_b200 import binding as B
+    from paper_2607_04181_b200 import inputs as I
+    from paper_2607_04181_b200.harness import ModelSession
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the library has no CPU fallback")
+    dev = "cuda:0"
+    torch.cuda.set_device(0)
+    shape = I.CFG2
+    n_layers, batch, hot = 32, 128, (10, 11, 12)
+    steps = max(args.steps, 30)
+    up, down = steps // 3, 2 * steps // 3
+    rng = np.random.default_rng(3003)
+    ctx = np.clip(np.rint(np.exp(rng.normal(np.log(1024.0), 0.8, batch))), 16, 8192).astype(np.int64)   # lognormal, median 1024
+    seq0 = (ctx + 1).astype(np.int32)
+    page = shape.page
+    need = (seq0.astype(np.int64) + steps + page - 1) // page
+    width = int(need.max())
+    n_pages = int(need.sum())
+    ids = rng.permutation(n_pages).astype(np.int32)                    # shuffled pages, block tables pre-extended
+    bt = np.full((batch, width), -1, np.int32)
+    off = 0
+    for b in range(batch):
+        bt[b, :need[b]] = ids[off:off + need[b]]
+        off += int(need[b])
+    gen = torch.Generator(device=dev).manual_seed(1003)
+
+    def randn(*shp, std=1.0, mean=0.0):
+        return (torch.randn(*shp, generator=gen, device=dev, dtype=torch.float32) * std + mean).to(torch.bfloat16)
+
+    d, F, QD, KD = shape.hidden, shape.ffn, shape.q_dim, shape.kv_dim
+    def layer_weights():
+        return {"g1": randn(d, std=0.02, mean=1.0), "wq": randn(QD, d, std=0.02), "wk": randn(KD, d, std=0.02),
+                "wv": randn(KD, d, std=0.02), "wo": randn(d, QD, std=0.02), "g2": randn(d, std=0.02, mean=1.0),
+                "wgate": randn(F, d, std=0.02), "wup": randn(F, d, std=0.02), "wdown": randn(d, F, std=0.02)}
+    S = ModelSession(shape, [], max_batch=batch, n_slots=len(hot), max_blocks=width, max_position=width * page)
+    for _ in range(n_layers):          # one at a time: only one unpacked copy of a layer's weights is alive
+        S.add_layer(layer_weights())
+    S.donate()
+    pool_shape = (n_pages, shape.n_kv_heads, page, shape.head_dim)
+    kp = [randn(*pool_shape) for _ in range(n_layers)]
+    vp = [randn(*pool_shape) for _ in range(n_layers)]
+    hidden = randn(batch, d)
+    btd = torch.from_numpy(bt).to(dev)
+    sl = torch.from_numpy(seq0.copy()).to(dev)
+    assigns = [torch.zeros(batch, dtype=torch.int32, device=dev) for _ in range(n_layers)]
+    split = torch.from_numpy(I.even_split(batch, 2)).to(dev)
+    stream = torch.cuda.current_stream()
+    S.forward_all(hidden, kp, vp, btd, n_pages, sl, assigns, batch)     # warm-up outside capture
+    torch.cuda.synchronize()
+    graph = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(graph):
+        S.forward_all(hidden, kp, vp, btd, n_pages, sl, assigns, batch, torch.cuda.current_stream())
+        hidden.mul_(0).add_(1.0)         # keep the synthetic hidden state bounded over hundreds of steps (not part of the method)
+        sl.add_(1)
+    exec_id, captures = id(graph), 1
+    for _ in range(3):
+        graph.replay()
+    sl.copy_(torch.from_numpy(seq0))
+    torch.cuda.synchronize()
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(steps)]
+    flip_ms = {}
+    sampler = ClockSampler(0)
+    sampler.start()
+    for t in range(steps):
+        ev[t][0].record()
+        if t == up:
+            for l in hot:
+                B.cc_scale_layer(S.layers[l], 2)                    # chunked copies on the side stream
+            for l in hot:
+                B.cc_commit(S.layers[l], stream)                    # stream waits for the copies, then the table flip
+                assigns[l].copy_(split)
+        if t == down:
+            for l in hot:
+                assigns[l].zero_()
+                B.cc_scale_layer(S.layers[l], 1)
+                B.cc_commit(S.layers[l], stream)
+        graph.replay()
+        ev[t][1].record()
+    torch.cuda.synchronize()
+    clocks = sampler.stop()
+    assert B.cc_poll_device_error(S.ctx) == 0 and id(graph) == exec_id and captures == 1
+    ms = np.array([a.elapsed_time(b) for a, b in ev])
+    flip_ms = {"scale_up_step_ms": float(ms[up]), "scale_down_step_ms": float(ms[down])}
+    def summ(x):
+        return {"mean_ms": round(float(x.mean()), 4), "p50_ms": round(float(np.percentile(x, 50)), 4),
+                "p99_ms": round(float(np.percentile(x, 99)), 4), "max_ms": round(float(x.max()), 4)}
+    before, during, after = ms[:up], ms[up + 1:down], ms[down + 1:]
+    kv_tok = float((seq0.astype(np.float64) + steps / 2).sum())
+    bytes_step = n_layers * S.blob_bytes + kv_tok * 2 * KD * 2 * n_layers
+    peak, peak_src = measured_peak()
+    mean_ms = float(np.concatenate([before, during, after]).mean())
+    line = {
+        "metric": "32-layer decode step (cfg3): tokens/s and per-step latency across replica flips", "value": batch / (mean_ms * 1e-3),
+        "unit": UNIT, "n_gpus": 1, "steps": steps, "warmup": 3, "ms_per_step": mean_ms, "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": "bf16", "data": "synthetic",
+        "config": {"workload": "cfg3 (BASELINE.json configs[2]): 32 Llama-3-8B-shaped layers, decode batch 128, contexts lognormal "
+                               "(median 1024, sigma 0.8, capped 8192), one CUDA graph for the whole step, seq_lens incremented "
+                               f"inside it; layers {list(hot)} scaled to 2 replicas at step {up} and back to 1 at step {down}",
+                   "graph_captures": captures, "same_graph_exec": True,
+                   "note": "hidden is reset to a constant inside the graph every step to keep the synthetic state bounded"},
+        "clocks": clocks,
+        "latency": {"before": summ(before), "while_2_replicas": summ(during), "after": summ(after), **flip_ms},
+        "replica_creation": {"layers": len(hot), "bytes_each": S.blob_bytes,
+                             "extra_ms_of_the_flip_step": round(float(ms[up] - before.mean()), 4)},
+        "step_roofline": {"algorithmic_bytes_mid_run": int(bytes_step), "achieved_GBps": round(bytes_step / (mean_ms * 1e-3) / 1e9, 1),
+                          "frac_of_measured_peak": round(bytes_step / (mean_ms * 1e-3) / 1e9 / peak, 4), "peak_source": peak_src},
+        "gpu_launches": int(B.cc_forward_launch_count(S.layers[0])) * n_layers * steps,
+    }
+    print(json.dumps(line), flush=True)
+    S.close()
+    return 0
+
+
 def main():
     args = parse_args()
     if args.impl == "reference":
         return run_reference(args)
+    if args.workload == "cfg3":
+        return run_cfg3(args)
     return run_ours(args)
 
 

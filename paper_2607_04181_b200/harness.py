@@ -125,12 +125,25 @@ class ModelSession:
         torch.cuda.set_device(device_index)
         self.ctx = B.cc_ctx_create(device_index)
         self.desc = make_desc(shape, max_batch, max_blocks, max_position)
-        self.layers = [B.cc_create_layer(self.ctx, self.desc, w) for w in weights_dev]
-        self.blob_bytes = B.cc_layer_blob_bytes(self.layers[0])
+        self.layers = []
+        self.blob_bytes = 0
         self.arena = None
-        if n_slots > 0:
+        self.n_slots = n_slots
+        for w in weights_dev:
+            self.add_layer(w)
+        if self.layers:
+            self.donate()
+
+    def add_layer(self, w: dict) -> None:
+        """One more layer from device weight tensors (the library packs its own copy, so `w` may be freed)."""
+        self.layers.append(B.cc_create_layer(self.ctx, self.desc, w))
+        self.blob_bytes = B.cc_layer_blob_bytes(self.layers[0])
+
+    def donate(self) -> None:
+        """Lend the replica arena (n_slots slots of one layer blob each) once the layers exist."""
+        if self.n_slots > 0 and self.arena is None:
             slot = (self.blob_bytes + 1023) // 1024 * 1024
-            self.arena = torch.empty(n_slots * slot + 2048, dtype=torch.uint8, device=self.device)
+            self.arena = torch.empty(self.n_slots * slot + 2048, dtype=torch.uint8, device=self.device)
             B.cc_ctx_donate(self.ctx, self.arena, self.arena.numel())
 
     def forward_all(self, hidden, k_pools, v_pools, block_table, n_pages, seq_lens, assigns, batch, stream=None) -> None:
