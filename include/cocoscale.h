@@ -207,7 +207,7 @@ cc_status cc_replica_copy(cc_ctx *ctx, void *dst_dev, const void *src_dev, size_
 typedef enum {
     CC_TAP_X = 0,   /* [batch][hidden]      input RMSNorm output (GEMM operand: bf16 hi + lo)   */
     CC_TAP_Q = 1,   /* [batch][Hq*Dh]       q after RoPE (fp32)                                 */
-    CC_TAP_O = 2,   /* [batch][Hq*Dh]       attention output (GEMM operand: one bf16 plane)     */
+    CC_TAP_O = 2,   /* [batch][Hq*Dh]       attention output (GEMM operand: bf16 hi + lo)       */
     CC_TAP_H1 = 3,  /* [batch][hidden]      hidden + O-projection (fp32)                        */
     CC_TAP_Y = 4,   /* [batch][hidden]      post-attention RMSNorm output (hi + lo operand x 1/rms) */
     CC_TAP_A = 5    /* [batch][ffn]         silu(gate)*up (bf16 hi + lo)                        */

@@ -392,7 +392,7 @@ cc_status cc_create_layer(cc_ctx* ctx, const cc_layer_desc* desc, const cc_layer
     const size_t o_pgpre = ws.take((size_t)(d.max_batch + 1) * 4);
     const size_t o_posof = ws.take((size_t)d.max_batch * 4);
     const size_t o_x = ws.take((size_t)2 * D.qkv.KB * Mp * 128);   // hi + lo planes
-    const size_t o_o = ws.take((size_t)D.o.KB * Mp * 128);
+    const size_t o_o = ws.take((size_t)2 * D.o.KB * Mp * 128);
     const size_t o_y = ws.take((size_t)2 * D.gu.KB * Mp * 128);
     const size_t o_a = ws.take((size_t)2 * D.dn.KB * Mp * 128);
     auto part_bytes = [&](const CcGemmGeo& g) { return (size_t)(g.P + g.ST) * CC_G * Mp * 128 * 4; };
@@ -738,7 +738,7 @@ cc_status cc_debug_tap(cc_layer* L, cc_tap which, float* out_host, int batch) {
     switch (which) {
         case CC_TAP_X: src = L->W.x_act; kind = 2; dim = D.d; break;
         case CC_TAP_Q: src = L->W.q_rot; kind = 1; dim = D.QD; break;
-        case CC_TAP_O: src = L->W.o_act; kind = 0; dim = D.QD; break;
+        case CC_TAP_O: src = L->W.o_act; kind = 2; dim = D.QD; break;
         case CC_TAP_H1: src = L->W.h1; kind = 1; dim = D.d; break;
         case CC_TAP_Y: src = L->W.y_act; kind = 3; dim = D.d; break;
         case CC_TAP_A: src = L->W.a_act; kind = 2; dim = D.F; break;

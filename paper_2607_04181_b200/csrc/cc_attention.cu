@@ -310,10 +310,14 @@ k_attn(const int* __restrict__ seq_lens, CcKv kv, CcDims D, CcWork W, const CcLa
         // lane l owns dims 4l .. 4l+3 of every q head of the group
         const int dim = lane * 4;
         const int nch = m.n_pieces;
-        auto store_operand = [&](int q, float4 v, float inv) {   // bf16 row of the O-projection operand (one plane)
+        auto store_operand = [&](int q, float4 v, float inv) {   // row of the O-projection operand, hi + lo bf16 planes
             const int col = (h * G + q) * DH + dim;
-            uint8_t* dst = W.o_act + act_chunk_off(m.pos, col, D.Mpad, 1, 0) + (col & 7) * 2;
-            *reinterpret_cast<uint2*>(dst) = make_uint2(pack_bf16(v.x * inv, v.y * inv), pack_bf16(v.z * inv, v.w * inv));
+            const float x0 = v.x * inv, x1 = v.y * inv, x2 = v.z * inv, x3 = v.w * inv;
+            const uint32_t h0 = pack_bf16(x0, x1), h1 = pack_bf16(x2, x3);
+            const uint32_t l0 = pack_bf16(x0 - bf16lo(h0), x1 - bf16hi(h0)), l1 = pack_bf16(x2 - bf16lo(h1), x3 - bf16hi(h1));
+            uint8_t* dst = W.o_act + act_chunk_off(m.pos, col, D.Mpad, 2, 0) + (col & 7) * 2;
+            *reinterpret_cast<uint2*>(dst) = make_uint2(h0, h1);
+            *reinterpret_cast<uint2*>(dst + 1024) = make_uint2(l0, l1);
         };
         if (pp == 0 && dim < DH) {
 #pragma unroll 1

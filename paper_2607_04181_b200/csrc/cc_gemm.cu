@@ -503,10 +503,10 @@ cudaError_t cc_launch_gemm(int which, const CcDims& D, const CcLayerTable* tab, 
     CcEpi E{seq_lens, kv, hidden};
     int* flags = W.flags + which * CC_FLAG_STRIDE;
     CcGemmGeo none{};   // P = 0: nothing to prefetch (attention / the next layer follows)
-    // hi + lo activation planes; the O projection's input needs one
+    // every projection takes its activations as hi + lo bf16 planes
     switch (which) {
         case 0: return cc_launch_kernel(k_gemm<EPI_QKV>, dim3(D.qkv.P), block, smem, L, D.qkv, W.x_act, 2, W.qkv_part, flags, E, D, W, tab, none);
-        case 1: return cc_launch_kernel(k_gemm<EPI_O>, dim3(D.o.P), block, smem, L, D.o, W.o_act, 1, W.o_part, flags, E, D, W, tab, D.gu);
+        case 1: return cc_launch_kernel(k_gemm<EPI_O>, dim3(D.o.P), block, smem, L, D.o, W.o_act, 2, W.o_part, flags, E, D, W, tab, D.gu);
         case 2: return cc_launch_kernel(k_gemm<EPI_GU>, dim3(D.gu.P), block, smem, L, D.gu, W.y_act, 2, W.gu_part, flags, E, D, W, tab, D.dn);
         default: return cc_launch_kernel(k_gemm<EPI_DN>, dim3(D.dn.P), block, smem, L, D.dn, W.a_act, 2, W.d_part, flags, E, D, W, tab, none);
     }

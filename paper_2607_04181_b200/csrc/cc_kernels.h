@@ -9,7 +9,7 @@ struct CcWork {
     int* pg_prefix;      // [max_batch + 1] pages of the rows before row b, request order (attention work split)
     int* pos_of;         // [max_batch] grouped position of row b, or -1
     uint8_t* x_act;      // packed bf16 GEMM operands, [K/64][Mpad/8][plane hi|lo][8][128 B swizzled]
-    uint8_t* o_act;      // (one plane)
+    uint8_t* o_act;
     uint8_t* y_act;
     uint8_t* a_act;
     float* qkv_part;     // stream-K partial sums, [(P + ST) * CC_G][Mpad][128] fp32 (piece-major)

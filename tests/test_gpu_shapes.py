@@ -1,0 +1,45 @@
+"""GPU parity on the other layer shapes the configs name and on the kernel's corner shapes, each against
+the oracle with stage taps (tests/test_gpu_parity.py): the 14B-class layer of configs[3], model B of
+configs[4], every supported kv-head count (1, 2, 4, 8: the attention kernel stages 8 / Hkv pages per
+TMA stage), GQA groups of 5, 6 and 8, head_dim 64 and 128, and the maximum batch of 256 rows over four
+uneven replica groups including contexts of zero cached tokens."""
+import numpy as np
+import pytest
+
+from paper_2607_04181_b200 import inputs as I
+from tests.test_gpu_parity import check_against_oracle, check_grouping, run_case
+
+pytestmark = pytest.mark.gpu
+
+CASES = {
+    # name: (shape, batch, replicas)
+    "cfg4_layer": (I.LayerShape("cfg4s", 5120, 40, 8, 128, 17408, 1e-5, 500000.0, 8, 256, 700), 8, 2),   # configs[3]: contexts from 256 up
+    "model_b": (I.LayerShape("modelBs", 1536, 12, 2, 128, 8960, 1e-6, 10000.0, 10, 30, 400), 10, 3),
+    "hkv4_dh64": (I.LayerShape("hkv4", 512, 8, 4, 64, 1024, 1e-5, 10000.0, 9, 10, 150), 9, 2),
+    "hkv1_g8": (I.LayerShape("hkv1", 256, 8, 1, 128, 512, 1e-5, 10000.0, 5, 20, 200), 5, 1),
+    "hkv8_g1": (I.LayerShape("hkv8", 1024, 8, 8, 128, 2048, 1e-5, 500000.0, 7, 100, 600), 7, 4),
+}
+
+
+@pytest.mark.parametrize("name", list(CASES))
+def test_shape_parity(name):
+    shape, batch, R = CASES[name]
+    rng = np.random.default_rng(7)
+    assign = rng.integers(0, R, batch).astype(np.int32)
+    st, ref, out, kp, vp, gtaps, grouping, assign = run_case(shape, batch, R, assign=assign, seeds=(1201, 2201, 3201))
+    rel = check_against_oracle(shape, st, ref, out, kp, vp, gtaps, assign, R)
+    check_grouping(grouping, assign, st.seq_lens, R)
+    print(name, "normalised rms error per stage:", {k: round(v, 5) for k, v in rel.items()})
+    assert max(rel.values()) < 1e-2
+
+
+def test_max_batch_256_rows_uneven_groups_and_empty_contexts():
+    shape = I.LayerShape("wide", 256, 4, 2, 64, 688, 1e-6, 10000.0, 256, 0, 40)
+    rng = np.random.default_rng(11)
+    assign = rng.choice(4, size=256, p=[0.55, 0.05, 0.3, 0.1]).astype(np.int32)
+    ctx = rng.integers(0, 41, 256).astype(np.int32)
+    ctx[:5] = 0                                                    # seq_len 1: attention over the new token only
+    st, ref, out, kp, vp, gtaps, grouping, assign = run_case(shape, 256, 4, assign=assign, contexts=ctx,
+                                                             seeds=(1202, 2202, 3202))
+    check_against_oracle(shape, st, ref, out, kp, vp, gtaps, assign, 4)
+    check_grouping(grouping, assign, st.seq_lens, 4)
