@@ -188,7 +188,7 @@ cc_status cc_forward_host(cc_layer *layer, void *hidden_host, void *k_pool_dev, 
 /* The same step, launched kernel by kernel with a CUDA event between consecutive kernels (so
  * without programmatic dependent launch), synchronised; stage_ms_host[i] (host, fp32
  * [cc_forward_launch_count]) receives the device time of kernel i in milliseconds, in launch
- * order: grouping, input norm, QKV GEMM (+RoPE, KV append), attention (+chunk merge), O GEMM
+ * order: grouping + input norm, QKV GEMM (+RoPE, KV append), attention (+chunk merge), O GEMM
  * (+residual, norm statistics), gate/up GEMM (+norm scale, SwiGLU), down GEMM (+residual, request
  * order).  For per-kernel roofline accounting; not capture-safe. */
 cc_status cc_forward_profiled(cc_layer *layer, void *hidden_dev, const cc_kv_pages *kv, const int32_t *seq_lens_dev,

@@ -208,7 +208,7 @@ def cc_forward_host(layer, hidden_host, k_pool, v_pool, n_pages: int, block_tabl
                                 C.c_int(batch), _stream(stream)))
 
 
-STAGE_NAMES = ("group", "rmsnorm_in", "gemm_qkv", "attention", "gemm_o", "gemm_gate_up", "gemm_down")
+STAGE_NAMES = ("prologue", "gemm_qkv", "attention", "gemm_o", "gemm_gate_up", "gemm_down")
 
 
 def cc_forward_profiled(layer, hidden, k_pool, v_pool, block_table, n_pages: int, seq_lens, replica_assign,

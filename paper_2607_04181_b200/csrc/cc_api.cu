@@ -637,7 +637,7 @@ cc_status cc_replica_blob(cc_layer* L, int replica, const void** blob_dev, size_
 
 // ---- the hot path -------------------------------------------------------------------------------
 namespace {
-constexpr int kForwardLaunches = 7;
+constexpr int kForwardLaunches = 6;
 
 cudaError_t enqueue_forward(cc_layer* L, __nv_bfloat16* hidden, const CcKv& kv, const int* seq_lens, const int* assign,
                             int batch, cudaStream_t st, cudaEvent_t* ev = nullptr) {
@@ -647,18 +647,17 @@ cudaError_t enqueue_forward(cc_layer* L, __nv_bfloat16* hidden, const CcKv& kv, 
     const CcLayerTable* tab = ctx->table_dev + L->row;
     CcLaunch Ln{st, ctx->n_sms, ctx->pdl && ev == nullptr};
     cudaError_t e = cudaSuccess;
-    // a0 grouping | a1 norm | a2 QKV (+ a3 RoPE, a4 append) | a5 attention (+ chunk merge) |
+    // a0 grouping + a1 norm | a2 QKV (+ a3 RoPE, a4 append) | a5 attention (+ chunk merge) |
     // a6 O (+ residual, a7 statistics) | a8 gate/up (+ a7 scale, SwiGLU) | a9 down (+ residual, request order)
     for (int stage = 0; stage < kForwardLaunches && e == cudaSuccess; ++stage) {
         if (ev && (e = cudaEventRecord(ev[stage], st)) != cudaSuccess) break;
         switch (stage) {
-            case 0: e = cc_launch_group(assign, seq_lens, batch, D, tab, W, Ln); break;
-            case 1: e = cc_launch_rmsnorm_in(hidden, D, tab, W, Ln); break;
-            case 2: e = cc_launch_gemm(0, D, tab, W, seq_lens, kv, hidden, Ln); break;
-            case 3: e = cc_launch_attention(seq_lens, kv, D, tab, W, Ln); break;
-            case 4: e = cc_launch_gemm(1, D, tab, W, seq_lens, kv, hidden, Ln); break;
-            case 5: e = cc_launch_gemm(2, D, tab, W, seq_lens, kv, hidden, Ln); break;
-            default: e = cc_launch_gemm(3, D, tab, W, seq_lens, kv, hidden, Ln); break;
+            case 0: e = cc_launch_prologue(assign, seq_lens, batch, hidden, D, tab, W, Ln); break;
+            case 1: e = cc_launch_gemm(0, D, tab, W, seq_lens, assign, batch, kv, hidden, Ln); break;
+            case 2: e = cc_launch_attention(seq_lens, kv, D, tab, W, Ln); break;
+            case 3: e = cc_launch_gemm(1, D, tab, W, seq_lens, assign, batch, kv, hidden, Ln); break;
+            case 4: e = cc_launch_gemm(2, D, tab, W, seq_lens, assign, batch, kv, hidden, Ln); break;
+            default: e = cc_launch_gemm(3, D, tab, W, seq_lens, assign, batch, kv, hidden, Ln); break;
         }
     }
     if (ev && e == cudaSuccess) e = cudaEventRecord(ev[kForwardLaunches], st);

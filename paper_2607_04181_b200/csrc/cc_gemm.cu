@@ -56,6 +56,8 @@ static_assert(sizeof(GemmSmemHdr) <= kHdrBytes, "header does not fit");
 // stores), so that one fixup iteration costs one L2 round trip.
 enum { EPI_QKV = 0, EPI_O = 1, EPI_GU = 2, EPI_DN = 3 };
 struct CcEpi {
+    const int* assign;          // replica_assign and batch: the QKV GEMM counts the groups itself
+    int batch;
     const int* seq_lens;
     CcKv kv;
     __nv_bfloat16* hidden;
@@ -248,11 +250,34 @@ k_gemm(CcGemmGeo G, const uint8_t* __restrict__ act, int planes, float* __restri
         fence_mbar_init();
     }
     if (warp == 1) tmem_alloc<kTmemCols>(&H->tmem_base);
-    // The grouping (k_group) and the replica table were written at least two kernels back in the
-    // chain; every kernel of the chain waits for its predecessor BEFORE it lets its successor
-    // start, so both are complete and visible here although this kernel's own predecessor (the
-    // producer of the activations) may still be running.
-    if (threadIdx.x < CC_MAXR) {
+    // The replica table was written long ago; the grouping tables (k_prologue) were complete two kernels
+    // back for every projection but the first: the QKV GEMM starts while k_prologue may still be running
+    // (programmatic dependent launch), so it counts the groups from the inputs itself -- the same rule,
+    // cc_row_replica -- to know which replica's weights to stream first and how wide the row groups are.
+    if (KIND == EPI_QKV) {
+        int* wcnt = H->aux;                                   // [8 warps][CC_MAXR], free until the helper warps run
+        if (threadIdx.x < 256) {
+            uint32_t err = 0;
+            const int rep = cc_row_replica(E.assign, E.seq_lens, threadIdx.x, E.batch, D, tab->active_mask, err);
+#pragma unroll
+            for (int r = 0; r < CC_MAXR; ++r) {
+                const uint32_t bal = __ballot_sync(0xffffffffu, rep == r);
+                if (lane == 0) wcnt[warp * CC_MAXR + r] = __popc(bal);
+            }
+        }
+        __syncthreads();
+        if (threadIdx.x == 0) {
+            int off = 0;
+            for (int r = 0; r < CC_MAXR; ++r) {
+                int c = 0;
+                for (int w = 0; w < 8; ++w) c += wcnt[w * CC_MAXR + r];
+                H->cnt[r] = c;
+                H->goff[r] = off;
+                off += (c + CC_ROW_ALIGN - 1) / CC_ROW_ALIGN * CC_ROW_ALIGN;
+            }
+        }
+        if (threadIdx.x < CC_MAXR) H->blob[threadIdx.x] = tab->rep[threadIdx.x].blob;
+    } else if (threadIdx.x < CC_MAXR) {
         H->cnt[threadIdx.x] = sched->cnt[threadIdx.x];
         H->goff[threadIdx.x] = sched->goff[threadIdx.x];
         H->blob[threadIdx.x] = tab->rep[threadIdx.x].blob;
@@ -261,7 +286,10 @@ k_gemm(CcGemmGeo G, const uint8_t* __restrict__ act, int planes, float* __restri
     __syncthreads();
     tc_fence_after();
 
-    const int nmax = uniform(sched->nmax);
+    int nmax = 0;
+#pragma unroll
+    for (int r = 0; r < CC_MAXR; ++r) nmax = max(nmax, (H->cnt[r] + CC_ROW_ALIGN - 1) / CC_ROW_ALIGN * CC_ROW_ALIGN);
+    nmax = uniform(nmax);
     const uint32_t act_bytes_max = (uint32_t)planes * (uint32_t)nmax * 128u;   // nmax % 16 == 0 => multiple of 2 KiB
     const uint32_t stage_bytes = kWStage + act_bytes_max;
     uint8_t* stage0 = smem_raw + kHdrBytes;                 // barriers and row tables live in front of the ring
@@ -497,10 +525,10 @@ cudaError_t cc_gemm_configure() {
 
 // which: 0 = QKV, 1 = O, 2 = gate/up, 3 = down
 cudaError_t cc_launch_gemm(int which, const CcDims& D, const CcLayerTable* tab, const CcWork& W, const int* seq_lens,
-                           const CcKv& kv, __nv_bfloat16* hidden, const CcLaunch& L) {
+                           const int* assign, int batch, const CcKv& kv, __nv_bfloat16* hidden, const CcLaunch& L) {
     const dim3 block(kGemmThreads);
     const size_t smem = (size_t)kGemmSmem;
-    CcEpi E{seq_lens, kv, hidden};
+    CcEpi E{assign, batch, seq_lens, kv, hidden};
     int* flags = W.flags + which * CC_FLAG_STRIDE;
     CcGemmGeo none{};   // P = 0: nothing to prefetch (attention / the next layer follows)
     // every projection takes its activations as hi + lo bf16 planes

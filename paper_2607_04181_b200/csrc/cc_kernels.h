@@ -19,7 +19,7 @@ struct CcWork {
     float* q_rot;        // [Mpad][Hq*Dh] fp32, q after RoPE
     float* h1;           // [Mpad][d]     fp32, hidden + O projection
     float* ssq;          // [d/128][Mpad] fp32, per-tile sum of squares of h1 (post-attention RMSNorm statistic)
-    int* flags;          // [4][CC_FLAG_STRIDE] stream-K fixup counters, zeroed by k_group every step
+    int* flags;          // [4][CC_FLAG_STRIDE] stream-K fixup counters, zeroed by k_prologue every step
     int* attn_cnt;       // [Mpad][Hkv] pieces finished per (row, kv head); the last finisher merges and resets
     float* att_o;        // [max_batch + SMs][Hq][Dh] fp32 un-normalised piece outputs (slot = row + CTA)
     float2* att_ml;      // [max_batch + SMs][Hq] (max in log2 units, sum)
@@ -42,13 +42,11 @@ struct CcLaunch {
 };
 
 
-cudaError_t cc_launch_group(const int* assign, const int* seq_lens, int batch, const CcDims& D,
-                            const CcLayerTable* tab, const CcWork& W, const CcLaunch& L);
-cudaError_t cc_launch_rmsnorm_in(const __nv_bfloat16* hidden, const CcDims& D, const CcLayerTable* tab,
-                                 const CcWork& W, const CcLaunch& L);
+cudaError_t cc_launch_prologue(const int* assign, const int* seq_lens, int batch, const __nv_bfloat16* hidden,
+                               const CcDims& D, const CcLayerTable* tab, const CcWork& W, const CcLaunch& L);
 // which: 0 = QKV, 1 = O, 2 = gate/up, 3 = down
 cudaError_t cc_launch_gemm(int which, const CcDims& D, const CcLayerTable* tab, const CcWork& W, const int* seq_lens,
-                           const CcKv& kv, __nv_bfloat16* hidden, const CcLaunch& L);
+                           const int* assign, int batch, const CcKv& kv, __nv_bfloat16* hidden, const CcLaunch& L);
 cudaError_t cc_launch_attention(const int* seq_lens, const CcKv& kv, const CcDims& D, const CcLayerTable* tab,
                                 const CcWork& W, const CcLaunch& L);
 

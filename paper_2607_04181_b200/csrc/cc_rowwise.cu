@@ -1,7 +1,6 @@
 // cc_rowwise.cu -- the small memory-bound kernels around the GEMMs of the replicated decoder layer
 // (sm_100a):
-//   k_group        a0     micro-batch grouping + attention work list (device-built, graph-safe)
-//   k_rmsnorm_in   a1     input RMSNorm -> GEMM operand
+//   k_prologue     a0+a1  micro-batch grouping, page prefix of the attention split, input RMSNorm -> operand
 // The split-KV merge is done by the attention kernel itself (cc_attention.cu); RoPE + KV append, residual + post-attention norm, SwiGLU and the final residual are the fused
 // epilogues of the stream-K fixup inside the GEMM kernel (cc_gemm.cu).  Every reduction order in
 // this file is a function of the layer shape and seq_len only (never of the batch split), which
@@ -44,44 +43,45 @@ __device__ __forceinline__ void split_hilo(float v0, float v1, uint32_t& hi, uin
 }
 
 // ---------------------------------------------------------------------------------------------
-// a0: grouping.  One block; thread b owns row b.  Stable partition by replica,
-// groups start at multiples of 16 rows; builds the split-KV work list (pos, chunk).
+// a0 + a1 in one kernel, one block per grouped position.
+// a0: grouping.  Every block repeats it (256 rows: a few ballots), thread b owns row b.  Stable partition
+// by replica, groups start at multiples of 16 rows; page prefix of the attention work
+// split.  Block 0 publishes the tables; each block keeps the one row that lands on its position.
+// a1: x = h * rsqrt(mean(h^2) + eps) * g1  ->  hi/lo operand planes of that row (kept in registers
+// between the two passes).
 // ---------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(256) k_group(const int* __restrict__ assign, const int* __restrict__ seq_lens,
-                                               int batch, CcDims D, const CcLayerTable* __restrict__ tab, CcWork W) {
+constexpr int kNormThreads = 512;
+constexpr int kNormVec = 2;            // uint4 (8 bf16) per thread: hidden <= 8 * 2 * 512 = 8192
+__global__ void __launch_bounds__(kNormThreads) k_prologue(const int* __restrict__ assign, const int* __restrict__ seq_lens,
+                                                           int batch, const __nv_bfloat16* __restrict__ hidden, CcDims D,
+                                                           const CcLayerTable* __restrict__ tab, CcWork W) {
     __shared__ int s_wcnt[8][CC_MAXR];     // rows of replica r in warp w
     __shared__ int s_wnch[8];              // KV pages of the rows of warp w
     __shared__ int s_goff[CC_MAXR + 1], s_cnt[CC_MAXR];
+    __shared__ int s_myb;
+    __shared__ float red[kNormThreads / 32];
     const int b = threadIdx.x, warp = b >> 5, lane = b & 31;
+    const bool pub = blockIdx.x == 0;      // this block writes the tables
     pdl_wait();
     pdl_launch_dependents();
-    const uint32_t mask = tab->active_mask;
-    int rep = -1;
-    if (b < batch) {
-        const int s = seq_lens[b];
-        if (s > 0) {
-            if (s > D.max_position || (s + CC_PAGE - 1) / CC_PAGE > D.max_blocks) {
-                atomicOr(W.err, CC_DEVERR_BAD_SEQLEN);
-            } else {
-                rep = assign[b];
-                if (rep < 0 || rep >= CC_MAXR || !((mask >> rep) & 1u)) {
-                    atomicOr(W.err, CC_DEVERR_BAD_REPLICA);
-                    rep = 0;
-                }
-            }
+    if (b == 0) s_myb = -1;
+    int rep = -1, pos = -1;
+    if (b < 256) {
+        uint32_t err = 0;
+        rep = cc_row_replica(assign, seq_lens, b, batch, D, tab->active_mask, err);
+        if (pub && err) atomicOr(W.err, err);
+        uint32_t bal[CC_MAXR];
+#pragma unroll
+        for (int r = 0; r < CC_MAXR; ++r) bal[r] = __ballot_sync(0xffffffffu, rep == r);
+        if (lane == 0) {
+#pragma unroll
+            for (int r = 0; r < CC_MAXR; ++r) s_wcnt[warp][r] = __popc(bal[r]);
         }
-    }
-    for (int i = b; i < D.Mpad; i += blockDim.x) W.perm[i] = -1;
-    for (int i = b; i < 4 * CC_FLAG_STRIDE; i += blockDim.x) W.flags[i] = 0;   // stream-K fixup counters of this step
-    // rank of this row among the rows of its replica: ballots inside the warp + warp prefix
-    uint32_t bal[CC_MAXR];
-#pragma unroll
-    for (int r = 0; r < CC_MAXR; ++r) bal[r] = __ballot_sync(0xffffffffu, rep == r);
-    // attention chunks ahead of this row inside the warp (rows keep request order in the work list
-    // only within a replica group, so the list is ordered by grouped position below)
-    if (lane == 0) {
-#pragma unroll
-        for (int r = 0; r < CC_MAXR; ++r) s_wcnt[warp][r] = __popc(bal[r]);
+        __syncwarp();
+        if (pub) {
+            for (int i = b; i < D.Mpad; i += 256) W.perm[i] = -1;
+            for (int i = b; i < 4 * CC_FLAG_STRIDE; i += 256) W.flags[i] = 0;   // stream-K fixup counters of this step
+        }
     }
     __syncthreads();
     if (b == 0) {
@@ -96,75 +96,83 @@ __global__ void __launch_bounds__(256) k_group(const int* __restrict__ assign, c
         s_goff[CC_MAXR] = off;
     }
     __syncthreads();
-    int pos = -1;
-    if (rep >= 0) {
+    if (b < 256) {
+        // rank of this row among the rows of its replica: ballot of its warp + the warps before it
+        // (the ballots are taken again -- cheaper than keeping four of them alive across the barriers)
         uint32_t mine = 0;
 #pragma unroll
-        for (int r = 0; r < CC_MAXR; ++r)
-            if (rep == r) mine = bal[r];
-        int rank = __popc(mine & ((1u << lane) - 1u));
-        for (int w = 0; w < warp; ++w) rank += s_wcnt[w][rep];
-        pos = s_goff[rep] + rank;
-        W.perm[pos] = b;
-    }
-    // attention work split: pages of the rows in request order (prefix sums); the attention CTAs cut this
-    // page axis into equal contiguous ranges -- a function of the batch, never of the replica split
-    if (b < D.max_batch) W.pos_of[b] = pos;
-    const int npg = (rep >= 0) ? (seq_lens[b] + CC_PAGE - 1) / CC_PAGE : 0;
-    int pre = npg;
-#pragma unroll
-    for (int o = 1; o < 32; o <<= 1) {
-        const int v = __shfl_up_sync(0xffffffffu, pre, o);
-        if (lane >= o) pre += v;
-    }
-    if (lane == 31) s_wnch[warp] = pre;
-    __syncthreads();
-    int base = pre - npg, total = 0;
-    for (int w = 0; w < 8; ++w) {
-        if (w < warp) base += s_wnch[w];
-        total += s_wnch[w];
-    }
-    if (b < D.max_batch) W.pg_prefix[b] = base;
-    if (b == 0) W.pg_prefix[D.max_batch] = total;
-    if (b == 0) {
-        int nmax = 0;
         for (int r = 0; r < CC_MAXR; ++r) {
-            W.sched->cnt[r] = s_cnt[r];
-            W.sched->goff[r] = s_goff[r];
-            nmax = max(nmax, (s_cnt[r] + CC_ROW_ALIGN - 1) / CC_ROW_ALIGN * CC_ROW_ALIGN);
+            const uint32_t br = __ballot_sync(0xffffffffu, rep == r);
+            if (rep == r) mine = br;
         }
-        W.sched->n_pos = s_goff[CC_MAXR];
-        W.sched->n_items = total;
-        W.sched->nmax = nmax;
+        if (rep >= 0) {
+            int rank = __popc(mine & ((1u << lane) - 1u));
+            for (int w = 0; w < warp; ++w) rank += s_wcnt[w][rep];
+            pos = s_goff[rep] + rank;
+            if (pub) W.perm[pos] = b;
+            if (pos == (int)blockIdx.x) s_myb = b;
+        }
+        // attention work split: pages of the rows in request order (prefix sums); the attention CTAs cut this
+        // page axis into equal contiguous ranges -- a function of the batch, never of the replica split
+        if (pub) {
+            if (b < D.max_batch) W.pos_of[b] = pos;
+            const int npg = (rep >= 0) ? (seq_lens[b] + CC_PAGE - 1) / CC_PAGE : 0;
+            int pre = npg;
+#pragma unroll
+            for (int o = 1; o < 32; o <<= 1) {
+                const int v = __shfl_up_sync(0xffffffffu, pre, o);
+                if (lane >= o) pre += v;
+            }
+            if (lane == 31) s_wnch[warp] = pre;
+            named_bar_sync(1, 256);
+            int base = pre - npg, total = 0;
+            for (int w = 0; w < 8; ++w) {
+                if (w < warp) base += s_wnch[w];
+                total += s_wnch[w];
+            }
+            if (b < D.max_batch) W.pg_prefix[b] = base;
+            if (b == 0) {
+                W.pg_prefix[D.max_batch] = total;
+                int nmax = 0;
+                for (int r = 0; r < CC_MAXR; ++r) {
+                    W.sched->cnt[r] = s_cnt[r];
+                    W.sched->goff[r] = s_goff[r];
+                    nmax = max(nmax, (s_cnt[r] + CC_ROW_ALIGN - 1) / CC_ROW_ALIGN * CC_ROW_ALIGN);
+                }
+                W.sched->n_pos = s_goff[CC_MAXR];
+                W.sched->n_items = total;
+                W.sched->nmax = nmax;
+            }
+        }
     }
-}
-
-// ---------------------------------------------------------------------------------------------
-// a1: x = h * rsqrt(mean(h^2) + eps) * g1  ->  hi/lo operand planes.  One block per position.
-// ---------------------------------------------------------------------------------------------
-constexpr int kNormThreads = 512;
-__global__ void __launch_bounds__(kNormThreads) k_rmsnorm_in(const __nv_bfloat16* __restrict__ hidden, CcDims D,
-                                                             const CcLayerTable* __restrict__ tab, CcWork W) {
-    __shared__ float red[kNormThreads / 32];
-    const int pos = blockIdx.x;
-    pdl_wait();
-    pdl_launch_dependents();
+    __syncthreads();
     if (threadIdx.x == 0) {   // warm L2 with the head of the QKV weight stream of the first non-empty group
         int r0 = 0;
-        while (r0 < CC_MAXR - 1 && W.sched->cnt[r0] == 0) ++r0;
+        while (r0 < CC_MAXR - 1 && s_cnt[r0] == 0) ++r0;
         for (int c = blockIdx.x; c < D.qkv.P; c += gridDim.x) cc_prefetch_gemm_head(D.qkv, tab->rep[r0].blob, c);
     }
-    if (pos >= W.sched->n_pos) return;
-    const int b = W.perm[pos];
-    if (b < 0) return;
-    const int r = replica_of_pos(W.sched, pos);
+    const int my_b = s_myb;
+    if (my_b < 0) return;                  // block-uniform: padding position
+    const int mypos = blockIdx.x;
+    int r = 0;
+#pragma unroll
+    for (int i = 1; i < CC_MAXR; ++i)
+        if (s_cnt[i] > 0 && mypos >= s_goff[i]) r = i;
     const uint4* g = reinterpret_cast<const uint4*>(tab->rep[r].blob + D.off_g1);
-    const uint4* row = reinterpret_cast<const uint4*>(hidden + (size_t)b * D.d);
+    const uint4* row = reinterpret_cast<const uint4*>(hidden + (size_t)my_b * D.d);
     const int nchunk = D.d >> 3;
+    uint4 v[kNormVec], gv[kNormVec];
     float ss = 0.f;
-    for (int c = threadIdx.x; c < nchunk; c += kNormThreads) {
-        const uint4 v = row[c];
-        const uint32_t w[4] = {v.x, v.y, v.z, v.w};
+#pragma unroll
+    for (int j = 0; j < kNormVec; ++j) {
+        const int c = threadIdx.x + j * kNormThreads;
+        v[j] = make_uint4(0, 0, 0, 0);
+        gv[j] = make_uint4(0, 0, 0, 0);
+        if (c < nchunk) {
+            v[j] = row[c];
+            gv[j] = g[c];
+        }
+        const uint32_t w[4] = {v[j].x, v[j].y, v[j].z, v[j].w};
 #pragma unroll
         for (int i = 0; i < 4; ++i) {
             const float a = bf16lo(w[i]), bb = bf16hi(w[i]);
@@ -173,20 +181,20 @@ __global__ void __launch_bounds__(kNormThreads) k_rmsnorm_in(const __nv_bfloat16
     }
     ss = block_sum(ss, red);
     const float inv = rsqrtf(ss / (float)D.d + D.eps);
-    for (int c = threadIdx.x; c < nchunk; c += kNormThreads) {
-        const uint4 v = row[c], gv = g[c];
-        const uint32_t w[4] = {v.x, v.y, v.z, v.w}, gw[4] = {gv.x, gv.y, gv.z, gv.w};
+#pragma unroll
+    for (int j = 0; j < kNormVec; ++j) {
+        const int c = threadIdx.x + j * kNormThreads;
+        if (c >= nchunk) break;
+        const uint32_t w[4] = {v[j].x, v[j].y, v[j].z, v[j].w}, gw[4] = {gv[j].x, gv[j].y, gv[j].z, gv[j].w};
         uint32_t hi[4], lo[4];
 #pragma unroll
         for (int i = 0; i < 4; ++i)
             split_hilo(bf16lo(w[i]) * inv * bf16lo(gw[i]), bf16hi(w[i]) * inv * bf16hi(gw[i]), hi[i], lo[i]);
-        uint8_t* dst = W.x_act + act_chunk_off(pos, c << 3, D.Mpad, 2, 0);
+        uint8_t* dst = W.x_act + act_chunk_off(mypos, c << 3, D.Mpad, 2, 0);
         *reinterpret_cast<uint4*>(dst) = make_uint4(hi[0], hi[1], hi[2], hi[3]);
         *reinterpret_cast<uint4*>(dst + 1024) = make_uint4(lo[0], lo[1], lo[2], lo[3]);
     }
 }
-
-constexpr int kMaxVecPerThread = 4;   // hidden <= 4 * 4 * 512 = 8192 (operand layout and epilogue limits)
 
 // Test tap: widen a workspace buffer to fp32 [batch][dim] in original row order.
 // which: 0 = one bf16 plane, 1 = fp32 rows, 2 = hi + lo planes, 3 = hi + lo planes times the row's
@@ -220,17 +228,13 @@ __global__ void __launch_bounds__(256) k_tap(const void* __restrict__ src, int w
 }  // namespace
 
 // ---- launchers ---------------------------------------------------------------------------------
-cudaError_t cc_launch_group(const int* assign, const int* seq_lens, int batch, const CcDims& D,
-                            const CcLayerTable* tab, const CcWork& W, const CcLaunch& L) {
-    return cc_launch_kernel(k_group, dim3(1), dim3(256), 0, L, assign, seq_lens, batch, D, tab, W);
-}
-cudaError_t cc_launch_rmsnorm_in(const __nv_bfloat16* hidden, const CcDims& D, const CcLayerTable* tab,
-                                 const CcWork& W, const CcLaunch& L) {
-    return cc_launch_kernel(k_rmsnorm_in, dim3(D.Mpad), dim3(kNormThreads), 0, L, hidden, D, tab, W);
+cudaError_t cc_launch_prologue(const int* assign, const int* seq_lens, int batch, const __nv_bfloat16* hidden,
+                               const CcDims& D, const CcLayerTable* tab, const CcWork& W, const CcLaunch& L) {
+    return cc_launch_kernel(k_prologue, dim3(D.Mpad), dim3(kNormThreads), 0, L, assign, seq_lens, batch, hidden, D, tab, W);
 }
 cudaError_t cc_launch_tap(const void* src, int which, int dim, const CcDims& D, const CcWork& W,
                           float* out_dev, int batch, cudaStream_t st) {
     k_tap<<<D.Mpad, 256, 0, st>>>(src, which, dim, D, W, out_dev, batch);
     return cudaGetLastError();
 }
-int cc_max_hidden() { return kMaxVecPerThread * 4 * kNormThreads; }
+int cc_max_hidden() { return kNormVec * 8 * kNormThreads; }
