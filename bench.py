@@ -345,6 +345,29 @@ def run_ours(args):
                     "frac_of_copy_peak": round(2 * blob / (cms * 1e-3) / 1e9 / peak, 4),
                     "graph_recaptures": 0}
 
+    # ---- KV partition per replica (NEXT-1): plan on the host, migrate pages on the device -------------
+    kv_migration = None
+    try:
+        new_bt, src, dst = B.cc_kv_plan_migration(st.block_table, st.seq_lens, I.even_split(batch, 2), st.n_pages, 2)
+        page_bytes = shape.n_kv_heads * shape.page * shape.head_dim * 2
+        d_src, d_dst = torch.from_numpy(src).to(f"cuda:{local}"), torch.from_numpy(dst).to(f"cuda:{local}")
+        mig_ms = []
+        for _ in range(6):
+            a, b_ = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a.record()
+            B.cc_kv_migrate(S.ctx, step.k_pool, step.v_pool, page_bytes, d_src, d_dst, len(src), stream)
+            b_.record()
+            torch.cuda.synchronize()
+            mig_ms.append(a.elapsed_time(b_))
+        mms = float(np.median(mig_ms[2:]))
+        moved = 2 * len(src) * page_bytes                          # K and V
+        kv_migration = {"pages_moved": int(len(src)), "bytes_moved": int(moved), "ms": round(mms, 4),
+                        "GBps_read_plus_write": round(2 * moved / (mms * 1e-3) / 1e9, 1),
+                        "frac_of_copy_peak": round(2 * moved / (mms * 1e-3) / 1e9 / peak, 4),
+                        "what": "batch split 32 + 32 over two page partitions; every page outside its replica's partition moved"}
+    except B.CcError as e:
+        kv_migration = {"error": str(e)}
+
     # ---- the oracle on this box's host cores, bounded sample (rank 0, N = 1) --------------------------
     cpu = None
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
@@ -376,6 +399,7 @@ def run_ours(args):
             "stages": stages,
             "by_replicas": by_r,
             "replica_copy": replica_copy,
+            "kv_migration": kv_migration,
             "cpu_baseline": cpu,
         }
         print(json.dumps(line), flush=True)

@@ -203,6 +203,28 @@ cc_status cc_forward_launch_count(const cc_layer *layer, int *n);
 cc_status cc_replica_copy(cc_ctx *ctx, void *dst_dev, const void *src_dev, size_t bytes, size_t chunk_bytes,
                           void *stream);
 
+/* ---- KV partition per replica (a replica holds its requests' KV; PAPER.md:103, 119:
+ * the cache is redistributed, chunk by chunk, when the parallelism degree changes) --------------- */
+/* Host-only planner.  The page pool [0, n_pages) is cut into n_replicas equal partitions, partition r =
+ * pages [r * (n_pages / n_replicas), (r + 1) * (n_pages / n_replicas)).  For the rows in increasing
+ * order and their pages in increasing order (only pages below ceil(seq_len / 16), rows with
+ * seq_len <= 0 are skipped), every page that lies outside the partition of the row's replica moves to
+ * the LOWEST page of that partition that no live row referenced before the call and no earlier move
+ * took.  Outputs: the re-mapped block table (same shape; untouched entries copied), the move list
+ * src -> dst in that order, its length.  CC_ERR_NO_SLOT (outputs unspecified) when a partition has too
+ * few free pages; CC_ERR_INVALID on a bad table (entry out of range or referenced twice). */
+cc_status cc_kv_plan_migration(const int32_t *block_table_host, const int32_t *seq_lens_host,
+                               const int32_t *replica_assign_host, int batch, int max_blocks_per_seq, int n_pages,
+                               int n_replicas, int32_t *new_block_table_host, int32_t *src_pages_host,
+                               int32_t *dst_pages_host, int *n_moves);
+
+/* Copies page src[i] -> dst[i] (all kv heads, page_bytes = n_kv_heads * 16 * head_dim * 2) in both pools,
+ * for i < n_moves; src/dst lists are DEVICE int32.  Sources and destinations must be disjoint sets (the
+ * planner guarantees it).  Enqueue-only on `stream`: put it between decode steps, or on a side stream
+ * ordered before the step that uses the new block table. */
+cc_status cc_kv_migrate(cc_ctx *ctx, void *k_pool_dev, void *v_pool_dev, size_t page_bytes,
+                        const int32_t *src_pages_dev, const int32_t *dst_pages_dev, int n_moves, void *stream);
+
 /* ---- stage taps (tests only; reads the workspace left by the last cc_forward) ---------------- */
 typedef enum {
     CC_TAP_X = 0,   /* [batch][hidden]      input RMSNorm output (GEMM operand: bf16 hi + lo)   */

@@ -70,3 +70,50 @@ class SlotAllocSim:
 def split_counts(bs: int, v: int):
     """the heaviest device processes ceil(bs/v) tokens, the others floor(bs/v)."""
     return -(-bs // v), bs // v
+
+
+# ---------------------------------------------------------------------------------------------
+# KV partition per replica (SURVEY.md 8(f) NEXT-1; PAPER.md:91, 103, 119).  Independent statement of
+# the planner's rule, written with sets and searches instead of the library's cursor walk.
+# ---------------------------------------------------------------------------------------------
+def plan_kv_migration(block_table, seq_lens, assign, n_pages: int, n_replicas: int, page: int = 16):
+    """Rule: partition r = pages [r*psz, (r+1)*psz), psz = n_pages // n_replicas.  Rows in increasing order,
+    their pages in increasing order: a page outside the partition of its row's replica moves to the lowest
+    page of that partition that was referenced by no live row before the call and was not taken by an
+    earlier move.  Returns (new_block_table, moves) with moves = [(src, dst), ...], or None when a
+    partition runs out of free pages."""
+    import numpy as np
+    bt = np.array(block_table, dtype=np.int64)
+    psz = n_pages // n_replicas
+    referenced = set()
+    for b in range(bt.shape[0]):
+        if seq_lens[b] > 0:
+            for j in range(-(-int(seq_lens[b]) // page)):
+                referenced.add(int(bt[b, j]))
+    taken = set()
+    moves = []
+    new_bt = bt.copy()
+    for b in range(bt.shape[0]):
+        if seq_lens[b] <= 0:
+            continue
+        r = int(assign[b])
+        part = range(r * psz, (r + 1) * psz)
+        for j in range(-(-int(seq_lens[b]) // page)):
+            pg = int(bt[b, j])
+            if pg in part:
+                continue
+            free = [q for q in part if q not in referenced and q not in taken]
+            if not free:
+                return None
+            q = min(free)
+            taken.add(q)
+            moves.append((pg, q))
+            new_bt[b, j] = q
+    return new_bt.astype(np.int32), moves
+
+
+def apply_kv_migration(k_pool, v_pool, moves):
+    """Byte copy of whole pages (all kv heads) in both pools, in move order."""
+    for s, d in moves:
+        k_pool[d] = k_pool[s]
+        v_pool[d] = v_pool[s]

@@ -29,7 +29,7 @@ EXPORTS = (
     "cc_ctx_create", "cc_ctx_destroy", "cc_ctx_donate", "cc_ctx_reclaim", "cc_ctx_set_copy_chunk",
     "cc_ctx_set_pdl", "cc_poll_device_error", "cc_create_layer", "cc_destroy_layer", "cc_layer_blob_bytes",
     "cc_scale_layer", "cc_commit", "cc_release_replica", "cc_query", "cc_replica_blob", "cc_forward",
-    "cc_forward_host", "cc_forward_profiled", "cc_forward_launch_count", "cc_replica_copy", "cc_debug_tap", "cc_debug_grouping",
+    "cc_forward_host", "cc_forward_profiled", "cc_forward_launch_count", "cc_replica_copy", "cc_kv_plan_migration", "cc_kv_migrate", "cc_debug_tap", "cc_debug_grouping",
     "cc_slotalloc_create", "cc_slotalloc_destroy", "cc_slotalloc_donate", "cc_slotalloc_reclaim",
     "cc_slotalloc_alloc", "cc_slotalloc_free", "cc_slotalloc_free_bytes", "cc_last_error", "cc_version",
 )
@@ -229,6 +229,27 @@ def cc_forward_launch_count(layer) -> int:
 def cc_replica_copy(ctx, dst, src, nbytes: int, chunk_bytes: int = 0, stream=None) -> None:
     _check(_lib.cc_replica_copy(ctx, _ptr(dst), _ptr(src), C.c_size_t(nbytes), C.c_size_t(chunk_bytes),
                                 _stream(stream)))
+
+
+# ---- KV partition per replica ----------------------------------------------------------------------
+def cc_kv_plan_migration(block_table: np.ndarray, seq_lens: np.ndarray, assign: np.ndarray, n_pages: int, n_replicas: int):
+    """-> (new_block_table, src_pages, dst_pages); host arrays, argument marshalling only."""
+    bt = np.ascontiguousarray(block_table, dtype=np.int32)
+    sl = np.ascontiguousarray(seq_lens, dtype=np.int32)
+    ra = np.ascontiguousarray(assign, dtype=np.int32)
+    batch, width = bt.shape
+    new_bt = np.empty_like(bt)
+    src = np.empty(batch * width, dtype=np.int32)
+    dst = np.empty(batch * width, dtype=np.int32)
+    n = C.c_int(0)
+    _check(_lib.cc_kv_plan_migration(_ptr(bt), _ptr(sl), _ptr(ra), C.c_int(batch), C.c_int(width), C.c_int(n_pages),
+                                     C.c_int(n_replicas), _ptr(new_bt), _ptr(src), _ptr(dst), C.byref(n)))
+    return new_bt, src[:n.value].copy(), dst[:n.value].copy()
+
+
+def cc_kv_migrate(ctx, k_pool, v_pool, page_bytes: int, src_pages, dst_pages, n_moves: int, stream=None) -> None:
+    _check(_lib.cc_kv_migrate(ctx, _ptr(k_pool), _ptr(v_pool), C.c_size_t(page_bytes), _ptr(src_pages), _ptr(dst_pages),
+                              C.c_int(n_moves), _stream(stream)))
 
 
 # ---- stage taps (tests) ------------------------------------------------------------------------

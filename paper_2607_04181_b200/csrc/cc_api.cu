@@ -727,6 +727,60 @@ cc_status cc_forward_launch_count(const cc_layer* L, int* n) {
     return CC_OK;
 }
 
+// ---- KV partition per replica: planner (host) + page migration (device) ---------------------------------
+cc_status cc_kv_plan_migration(const int32_t* bt, const int32_t* seq_lens, const int32_t* assign, int batch, int max_blocks,
+                               int n_pages, int n_replicas, int32_t* new_bt, int32_t* src, int32_t* dst, int* n_moves) {
+    if (!bt || !seq_lens || !assign || !new_bt || !src || !dst || !n_moves) return fail(CC_ERR_INVALID, "null argument");
+    if (batch < 1 || max_blocks < 1 || n_pages < 1 || n_replicas < 1 || n_replicas > CC_MAX_REPLICAS || n_pages < n_replicas)
+        return fail(CC_ERR_INVALID, "bad sizes");
+    const int psz = n_pages / n_replicas;
+    std::vector<char> used((size_t)n_pages, 0);
+    for (int b = 0; b < batch; ++b) {
+        const int need = seq_lens[b] > 0 ? (seq_lens[b] + CC_PAGE_SIZE - 1) / CC_PAGE_SIZE : 0;
+        if (need > max_blocks) return fail(CC_ERR_INVALID, "row %d needs %d pages, table has %d", b, need, max_blocks);
+        if (need && (assign[b] < 0 || assign[b] >= n_replicas)) return fail(CC_ERR_INVALID, "row %d: replica %d out of range", b, assign[b]);
+        for (int j = 0; j < need; ++j) {
+            const int pg = bt[(size_t)b * max_blocks + j];
+            if (pg < 0 || pg >= n_pages) return fail(CC_ERR_INVALID, "row %d page %d: id %d out of range", b, j, pg);
+            if (used[pg]) return fail(CC_ERR_INVALID, "page %d is referenced twice", pg);
+            used[pg] = 1;
+        }
+    }
+    std::memcpy(new_bt, bt, (size_t)batch * max_blocks * sizeof(int32_t));
+    int cursor[CC_MAX_REPLICAS];                               // lowest candidate of each partition
+    for (int r = 0; r < n_replicas; ++r) cursor[r] = r * psz;
+    int n = 0;
+    for (int b = 0; b < batch; ++b) {
+        const int need = seq_lens[b] > 0 ? (seq_lens[b] + CC_PAGE_SIZE - 1) / CC_PAGE_SIZE : 0;
+        if (!need) continue;
+        const int r = assign[b], lo = r * psz, hi = lo + psz;
+        for (int j = 0; j < need; ++j) {
+            const int pg = bt[(size_t)b * max_blocks + j];
+            if (pg >= lo && pg < hi) continue;
+            while (cursor[r] < hi && used[cursor[r]]) ++cursor[r];
+            if (cursor[r] >= hi) return fail(CC_ERR_NO_SLOT, "partition %d has no free page left for row %d", r, b);
+            used[cursor[r]] = 1;                               // sources stay "used": never a destination of this plan
+            src[n] = pg;
+            dst[n] = cursor[r];
+            new_bt[(size_t)b * max_blocks + j] = cursor[r];
+            ++n;
+        }
+    }
+    *n_moves = n;
+    return CC_OK;
+}
+
+cc_status cc_kv_migrate(cc_ctx* ctx, void* k_pool_dev, void* v_pool_dev, size_t page_bytes, const int32_t* src_dev,
+                        const int32_t* dst_dev, int n_moves, void* stream) {
+    if (!ctx || !k_pool_dev || !v_pool_dev) return fail(CC_ERR_INVALID, "null argument");
+    if (n_moves < 0 || (n_moves > 0 && (!src_dev || !dst_dev))) return fail(CC_ERR_INVALID, "bad move list");
+    if (page_bytes == 0 || page_bytes % 32 || (((uintptr_t)k_pool_dev | (uintptr_t)v_pool_dev) & 31))
+        return fail(CC_ERR_INVALID, "page_bytes must be a multiple of 32 and the pools 32-byte aligned");
+    CC_CUDA(cudaSetDevice(ctx->device));
+    CC_CUDA(cc_launch_page_copy(k_pool_dev, v_pool_dev, page_bytes, src_dev, dst_dev, n_moves, (cudaStream_t)stream));
+    return CC_OK;
+}
+
 // ---- stage taps (tests only) ----------------------------------------------------------------------
 cc_status cc_debug_tap(cc_layer* L, cc_tap which, float* out_host, int batch) {
     if (!L || !out_host) return fail(CC_ERR_INVALID, "null argument");

@@ -52,6 +52,24 @@ __global__ void __launch_bounds__(kCopyThreads) k_copy(u32x8* __restrict__ dst, 
     pdl_wait();
 }
 
+// KV page migration (NEXT-1): block (move i, pool) copies one page of all kv heads, 256-bit accesses.
+__global__ void __launch_bounds__(256) k_page_copy(uint8_t* __restrict__ k_pool, uint8_t* __restrict__ v_pool, size_t page_bytes,
+                                                   const int* __restrict__ src, const int* __restrict__ dst) {
+    uint8_t* pool = blockIdx.y ? v_pool : k_pool;
+    const u32x8* s = reinterpret_cast<const u32x8*>(pool + (size_t)src[blockIdx.x] * page_bytes);
+    u32x8* d = reinterpret_cast<u32x8*>(pool + (size_t)dst[blockIdx.x] * page_bytes);
+    const size_t n32 = page_bytes / 32;
+    for (size_t i = threadIdx.x; i < n32; i += 4 * 256) {
+        u32x8 v[4];
+#pragma unroll
+        for (int j = 0; j < 4; ++j)
+            if (i + j * 256 < n32) v[j] = ld_stream32(s + i + j * 256);
+#pragma unroll
+        for (int j = 0; j < 4; ++j)
+            if (i + j * 256 < n32) st_stream32(d + i + j * 256, v[j]);
+    }
+}
+
 // a12: the flip.  One thread rewrites the layer's table row; ordering comes from the stream.
 __global__ void k_publish(CcLayerTable* row, CcLayerTable value) {
     for (int r = 0; r < CC_MAXR; ++r) row->rep[r].blob = value.rep[r].blob;
@@ -111,5 +129,11 @@ cudaError_t cc_launch_pack(uint8_t* dst, const __nv_bfloat16* src0, const __nv_b
                            const __nv_bfloat16* src2, int rows0, int rows1, int rows2, int mode, int K, int n_tiles,
                            int k_blocks, cudaStream_t st) {
     k_pack<<<1184, 256, 0, st>>>(dst, src0, src1, src2, rows0, rows1, rows2, mode, K, n_tiles, k_blocks);
+    return cudaGetLastError();
+}
+cudaError_t cc_launch_page_copy(void* k_pool, void* v_pool, size_t page_bytes, const int* src, const int* dst, int n_moves,
+                                cudaStream_t st) {
+    if (n_moves <= 0) return cudaSuccess;
+    k_page_copy<<<dim3((unsigned)n_moves, 2), 256, 0, st>>>((uint8_t*)k_pool, (uint8_t*)v_pool, page_bytes, src, dst);
     return cudaGetLastError();
 }

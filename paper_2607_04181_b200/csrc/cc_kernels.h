@@ -51,6 +51,8 @@ cudaError_t cc_launch_attention(const int* seq_lens, const CcKv& kv, const CcDim
                                 const CcWork& W, const CcLaunch& L);
 
 cudaError_t cc_launch_copy(void* dst, const void* src, size_t bytes, int n_sms, cudaStream_t st);
+cudaError_t cc_launch_page_copy(void* k_pool, void* v_pool, size_t page_bytes, const int* src, const int* dst, int n_moves,
+                                cudaStream_t st);
 cudaError_t cc_launch_publish(CcLayerTable* row_dev, const CcLayerTable& value, cudaStream_t st);
 // mode 0: rows of src0, then src1, then src2 (concatenated); mode 1: rows alternate src0[j], src1[j].
 cudaError_t cc_launch_pack(uint8_t* dst, const __nv_bfloat16* src0, const __nv_bfloat16* src1,
