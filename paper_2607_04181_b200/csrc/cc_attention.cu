@@ -182,12 +182,6 @@ k_attn(const int* __restrict__ seq_lens, CcKv kv, CcDims D, CcWork W, const CcLa
             meta[stage].flags = kMetaEnd;
             mbar_arrive(&full[stage]);
         }
-        // out of items: warm L2 with the head of the O-projection weight stream of the first non-empty group
-        if (lane == 0) {
-            int r0 = 0;
-            while (r0 < CC_MAXR - 1 && W.sched->cnt[r0] == 0) ++r0;
-            for (int c = blockIdx.x; c < D.o.P; c += gridDim.x) cc_prefetch_gemm_head(D.o, tab->rep[r0].blob, c);
-        }
         return;
     }
 

@@ -245,21 +245,6 @@ __device__ __forceinline__ uint64_t policy_evict_last() {
     asm volatile("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;" : "=l"(p));
     return p;
 }
-// L2 prefetch of the head of GEMM CTA `cta`'s weight range (first CC_PF_BYTES of it) in `blob`: issued
-// by the kernel that runs just before that GEMM, while HBM is otherwise idle (the tail of the previous
-// GEMM, the small row-wise kernels), so the GEMM's first pipeline stages are L2 hits.  One thread.
-#define CC_PF_BYTES (256u * 1024u)
-__device__ __forceinline__ void bulk_prefetch_l2(const void* src, uint32_t bytes) {
-    asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(src), "r"(bytes) : "memory");
-}
-__device__ __forceinline__ void cc_prefetch_gemm_head(const CcGemmGeo& g, const uint8_t* blob, int cta) {
-    if (blob == nullptr || cta >= g.P) return;
-    const long long ub = cc_range_begin(g, cta), ue = cc_range_begin(g, cta + 1);
-    long long bytes = (ue - ub) * (long long)(CC_G * CC_A_TILE_BYTES);
-    if (bytes > (long long)CC_PF_BYTES) bytes = CC_PF_BYTES;
-    const uint8_t* src = blob + g.w_off + (size_t)ub * (CC_G * CC_A_TILE_BYTES);
-    for (long long off = 0; off < bytes; off += CC_G * CC_A_TILE_BYTES) bulk_prefetch_l2(src + off, CC_G * CC_A_TILE_BYTES);
-}
 // ---- tcgen05 / TMEM --------------------------------------------------------------------------
 template <int kCols>
 __device__ __forceinline__ void tmem_alloc(uint32_t* dst_smem) {   // one full warp

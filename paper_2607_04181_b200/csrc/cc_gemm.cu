@@ -230,7 +230,7 @@ __device__ __forceinline__ int ld_acquire(const int* p) {
 template <int KIND>
 __global__ void __launch_bounds__(kGemmThreads, 1)
 k_gemm(CcGemmGeo G, const uint8_t* __restrict__ act, int planes, float* __restrict__ part, int* __restrict__ flags,
-       CcEpi E, CcDims D, CcWork W, const CcLayerTable* __restrict__ tab, CcGemmGeo Gnext) {
+       CcEpi E, CcDims D, CcWork W, const CcLayerTable* __restrict__ tab) {
     const CcSched* __restrict__ sched = W.sched;
     const int Mpad = D.Mpad;
     extern __shared__ __align__(1024) uint8_t smem_raw[];
@@ -359,12 +359,6 @@ k_gemm(CcGemmGeo G, const uint8_t* __restrict__ act, int planes, float* __restri
             pdl_wait();
             if (elect_one()) pdl_launch_dependents();
             run(1);
-            // everything of this GEMM is in flight: warm L2 with the head of the next GEMM's stream
-            if (Gnext.P > 0 && elect_one()) {
-                int r0 = 0;
-                while (r0 < CC_MAXR - 1 && H->cnt[r0] == 0) ++r0;
-                cc_prefetch_gemm_head(Gnext, H->blob[r0], (int)blockIdx.x);
-            }
         } else if (warp == 1) {
             // ===================== MMA issuer =====================
             int stage = 0;
@@ -530,12 +524,11 @@ cudaError_t cc_launch_gemm(int which, const CcDims& D, const CcLayerTable* tab, 
     const size_t smem = (size_t)kGemmSmem;
     CcEpi E{assign, batch, seq_lens, kv, hidden};
     int* flags = W.flags + which * CC_FLAG_STRIDE;
-    CcGemmGeo none{};   // P = 0: nothing to prefetch (attention / the next layer follows)
     // every projection takes its activations as hi + lo bf16 planes
     switch (which) {
-        case 0: return cc_launch_kernel(k_gemm<EPI_QKV>, dim3(D.qkv.P), block, smem, L, D.qkv, W.x_act, 2, W.qkv_part, flags, E, D, W, tab, none);
-        case 1: return cc_launch_kernel(k_gemm<EPI_O>, dim3(D.o.P), block, smem, L, D.o, W.o_act, 2, W.o_part, flags, E, D, W, tab, D.gu);
-        case 2: return cc_launch_kernel(k_gemm<EPI_GU>, dim3(D.gu.P), block, smem, L, D.gu, W.y_act, 2, W.gu_part, flags, E, D, W, tab, D.dn);
-        default: return cc_launch_kernel(k_gemm<EPI_DN>, dim3(D.dn.P), block, smem, L, D.dn, W.a_act, 2, W.d_part, flags, E, D, W, tab, none);
+        case 0: return cc_launch_kernel(k_gemm<EPI_QKV>, dim3(D.qkv.P), block, smem, L, D.qkv, W.x_act, 2, W.qkv_part, flags, E, D, W, tab);
+        case 1: return cc_launch_kernel(k_gemm<EPI_O>, dim3(D.o.P), block, smem, L, D.o, W.o_act, 2, W.o_part, flags, E, D, W, tab);
+        case 2: return cc_launch_kernel(k_gemm<EPI_GU>, dim3(D.gu.P), block, smem, L, D.gu, W.y_act, 2, W.gu_part, flags, E, D, W, tab);
+        default: return cc_launch_kernel(k_gemm<EPI_DN>, dim3(D.dn.P), block, smem, L, D.dn, W.a_act, 2, W.d_part, flags, E, D, W, tab);
     }
 }

@@ -146,11 +146,6 @@ __global__ void __launch_bounds__(kNormThreads) k_prologue(const int* __restrict
         }
     }
     __syncthreads();
-    if (threadIdx.x == 0) {   // warm L2 with the head of the QKV weight stream of the first non-empty group
-        int r0 = 0;
-        while (r0 < CC_MAXR - 1 && s_cnt[r0] == 0) ++r0;
-        for (int c = blockIdx.x; c < D.qkv.P; c += gridDim.x) cc_prefetch_gemm_head(D.qkv, tab->rep[r0].blob, c);
-    }
     const int my_b = s_myb;
     if (my_b < 0) return;                  // block-uniform: padding position
     const int mypos = blockIdx.x;
