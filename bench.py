@@ -185,6 +185,7 @@ def run_ours(args):
 
     from paper_2607_04181_b200 import binding as B
     from paper_2607_04181_b200 import inputs as I
+    from paper_2607_04181_b200 import multirank as M
     from paper_2607_04181_b200.harness import DeviceStep, Session
 
     world = int(os.environ.get("WORLD_SIZE", "1"))
@@ -239,12 +240,7 @@ def run_ours(args):
             graph.replay()
         torch.cuda.synchronize()
     clocks = sampler.stop()
-    if world > 1:
-        t = torch.tensor([ms_total], device=f"cuda:{local}")
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms_total = float(t.item())
-    ms_step = ms_total / K
-    value = world * batch * K / (ms_total / 1e3)
+    value, ms_step = M.job_throughput(batch, K, ms_total, f"cuda:{local}")     # all ranks' tokens / slowest rank's time
     assert B.cc_poll_device_error(S.ctx) == 0
 
     # ---- per-kernel roofline: the same step launched kernel by kernel with events between ---------
@@ -313,10 +309,7 @@ def run_ours(args):
         B.cc_forward_host(S.layer, h_hidden, step.k_pool, step.v_pool, step.n_pages, h_bt, h_sl, h_ra, batch, stream)
     torch.cuda.synchronize()
     e2e_s = time.perf_counter() - t0
-    if world > 1:
-        t = torch.tensor([e2e_s], device=f"cuda:{local}")
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        e2e_s = float(t.item())
+    e2e_s = M.max_over_ranks(e2e_s, f"cuda:{local}")
     h2d = h_hidden.numel() * 2 + h_bt.numel() * 4 + h_sl.numel() * 4 + h_ra.numel() * 4
     e2e = {"value": world * batch * K / e2e_s, "unit": UNIT, "h2d_bytes_per_step": int(h2d),
            "d2h_bytes_per_step": int(h_hidden.numel() * 2), "ms_per_step": e2e_s / K * 1e3,
