@@ -315,7 +315,8 @@ k_gemm(CcGemmGeo G, const uint8_t* __restrict__ act, int planes, float* __restri
             // first (mode 0), then the kernel waits for its predecessor, adds the activation
             // slabs of those stages and carries on (mode 1), so the HBM stream restarts while
             // the small kernel between two GEMMs is still running.
-            const uint64_t pol_w = policy_evict_first();
+            const uint64_t pol_w = policy_evict_first();   // weights: used once
+            const uint64_t pol_a = policy_evict_last();    // activation slabs: re-read by every CTA, keep them in L2
             const size_t kb_stride = (size_t)(Mpad >> 3) * planes * 1024;   // bytes between k-blocks of the operand
             const long long per_rep = u_end - u_begin;
             int n_act = 0;
@@ -345,7 +346,7 @@ k_gemm(CcGemmGeo G, const uint8_t* __restrict__ act, int planes, float* __restri
                                 mbar_expect_tx(&H->full[stage], tx);
                                 bulk_g2s_hint(sW, wsrc, kWStage, &H->full[stage], pol_w);
                             }
-                            if (mode == 1) bulk_g2s(sW + kWStage, asrc, nb, &H->full[stage]);
+                            if (mode == 1) bulk_g2s_hint(sW + kWStage, asrc, nb, &H->full[stage], pol_a);
                         }
                         wsrc += kWStage;
                         asrc += kb_stride;
