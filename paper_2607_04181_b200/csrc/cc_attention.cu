@@ -85,7 +85,7 @@ k_attn(const int* __restrict__ seq_lens, CcKv kv, CcDims D, CcWork W, const CcLa
         fence_mbar_init();
     }
     __syncthreads();
-    // The grouping tables (k_group) were complete two kernels back, seq_lens and the block table are
+    // The grouping tables (k_prologue) were complete two kernels back, seq_lens and the block table are
     // inputs: only q and the K/V of the token being decoded come from the predecessor (the QKV GEMM).
     // So the producer starts streaming the OLD pages at once -- while the predecessor's CTAs on other
     // SMs are still in their fixup -- and waits for it only before the first stage that holds the last

@@ -38,7 +38,7 @@ struct CcLayerTable {
 // copy of CC_G * 16 KiB) plus the activation slab of that k-block (ONE bulk copy), so the slab
 // is fetched from L2 once per CC_G atoms and the single producer thread issues two copies per
 // 32 KiB of weights (measured: the copy-issue rate, not HBM, bounded the one-atom-per-stage
-// version; profiles/r01_microbench.md).
+// version).
 // The (super tile, k-block) "units" are numbered super-tile-major and cut into P contiguous
 // ranges, range i owned by CTA i.  P and the cut points depend on the layer shape and the SM
 // count only -- never on the batch split -- so every output element is summed in one fixed
@@ -87,7 +87,7 @@ struct CcDims {
     size_t off_g1, off_g2;      // gains inside the blob (bf16 [d])
 };
 
-// Per-forward schedule, rebuilt on the device by k_group every step (row a0).
+// Per-forward schedule, rebuilt on the device by k_prologue every step (row a0).
 struct CcSched {
     int cnt[CC_MAXR];      // rows in replica group r
     int goff[CC_MAXR];     // first grouped position of group r (multiple of 16)

@@ -6,7 +6,7 @@
 //   * swap-AB: a packed weight tile (128 output features x 64 k, a 16 KiB pre-swizzled image
 //     made once at cc_create_layer) is the tcgen05 A operand (M = 128); the activations of one
 //     replica group (n rows, n = multiple of 16, <= 256) are the B operand (N = n), held as two
-//     bf16 planes hi + lo that are both multiplied into the same accumulator (cc_rowwise.cu).
+//     bf16 planes hi + lo that are both multiplied into the same accumulator.
 //   * CC_G = 2 adjacent tiles form a super tile: one pipeline stage = the two weight atoms of
 //     one k-block (32 KiB, contiguous in the blob, one bulk copy) + the activation slab of that
 //     k-block (both planes, one bulk copy), feeding two fp32 accumulators D[128][n] in TMEM
