@@ -250,3 +250,29 @@ def test_forward_host_matches_forward():
                           torch.cuda.current_stream())
         assert np.array_equal(hidden.numpy().view(np.uint16), want)
         assert B.cc_forward_launch_count(S.layer) == len(B.STAGE_NAMES)
+
+
+def test_run_to_run_determinism_and_pdl_off_is_bitwise_the_same():
+    """The fixups and merges are finished by whichever CTA arrives last: the result must not depend on that.
+    Twenty replays from the same inputs, with and without programmatic dependent launch, give one bit pattern
+    (PAPER.md:385 asks for bit-wise consistency; a timing-dependent sum order would break it silently)."""
+    B, DeviceStep, Session = _binding()
+    shape, batch = MID, 21
+    w = I.make_weights(shape, 1007)
+    st = I.make_step_inputs(shape, 2007, 3007, batch=batch)
+    assign = (np.arange(batch) * 5 % 3).astype(np.int32)
+    outs = []
+    with Session(shape, w, max_batch=batch) as S:
+        S.scale(3)
+        step = DeviceStep(st, assign)
+        for pdl in (1, 0):
+            B.cc_ctx_set_pdl(S.ctx, pdl)
+            for _ in range(10):
+                step.reset(st)
+                S.forward(step)
+                torch.cuda.synchronize()
+                kp, vp = step.pools_bits()
+                outs.append((step.out_bits(), kp, vp))
+        assert B.cc_poll_device_error(S.ctx) == 0
+    for o, kp, vp in outs[1:]:
+        assert np.array_equal(o, outs[0][0]) and np.array_equal(kp, outs[0][1]) and np.array_equal(vp, outs[0][2])
