@@ -225,6 +225,33 @@ cc_status cc_kv_plan_migration(const int32_t *block_table_host, const int32_t *s
 cc_status cc_kv_migrate(cc_ctx *ctx, void *k_pool_dev, void *v_pool_dev, size_t page_bytes,
                         const int32_t *src_pages_dev, const int32_t *dst_pages_dev, int n_moves, void *stream);
 
+/* ---- the paper's cost / speed-up model and scaling decision (host only; Eq. 1-10,
+ * PAPER.md:290-353 Algorithm 2).  The hot path takes replica counts and replica_assign from its caller;
+ * this is the piece that would choose them.  Readings: DESIGN.md 7c. -------------------------------- */
+typedef struct {
+    int32_t L;                    /* layers of the model                                             */
+    int32_t P_max;                /* largest parallelism degree considered, <= CC_MAX_REPLICAS        */
+    double slo;                   /* latency objective                                               */
+    double delta;                 /* tolerance band |latency - SLO| / SLO <= delta: no action          */
+    double beta[CC_MAX_REPLICAS + 1]; /* beta(P) = T(P) / (L * t_comp), index P (beta[1] = 0)          */
+    double cost_per_device;       /* Cost(N, P) = cost_per_device * (P - 1) + cost_per_layer_copy * N * (P - 1) */
+    double cost_per_layer_copy;
+} cc_ctl_params;
+typedef enum { CC_CTL_NONE = 0, CC_CTL_UPDATED = 1, CC_CTL_INSTANCE_SCALE = 2 } cc_ctl_action;
+
+double cc_ctl_mem_bytes(int N, int P, int bs, int l, int d_hidden, double kappa);             /* Eq. 1 */
+double cc_ctl_flops(int N, int P, int bs, int l, int d_hidden);                               /* Eq. 2 */
+double cc_ctl_comm_seconds(int P, int bs, int l, int d_hidden, double kappa, double bandwidth_bytes_per_s); /* Eq. 5 */
+double cc_ctl_speedup(int L, int N, int P, double beta);                                      /* Eq. 7 */
+double cc_ctl_speedup_vec(const int32_t *v, int L, int bs, double t_comp_s, int d_hidden, double kappa,
+                          double bandwidth_bytes_per_s);                                      /* Eq. 8-10 */
+int cc_ctl_distance(int N0, int P0, int N1, int P1);                  /* Dist of Algorithm 2, nested segments */
+int cc_ctl_candidate_count(int L, int P_max);                         /* L * P_max            */
+/* One pass of Algorithm 2's body for one instance: on CC_CTL_UPDATED the new (N, P) is written and
+ * *cold_capacity reduced by the resource difference (increased when it is negative). */
+cc_status cc_ctl_decide(const cc_ctl_params *p, int N_cur, int P_cur, double latency, double *cold_capacity,
+                        int *N_new, int *P_new, cc_ctl_action *action);
+
 /* ---- stage taps (tests only; reads the workspace left by the last cc_forward) ---------------- */
 typedef enum {
     CC_TAP_X = 0,   /* [batch][hidden]      input RMSNorm output (GEMM operand: bf16 hi + lo)   */

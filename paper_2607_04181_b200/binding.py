@@ -32,6 +32,8 @@ EXPORTS = (
     "cc_forward_host", "cc_forward_profiled", "cc_forward_launch_count", "cc_replica_copy", "cc_kv_plan_migration", "cc_kv_migrate", "cc_debug_tap", "cc_debug_grouping",
     "cc_slotalloc_create", "cc_slotalloc_destroy", "cc_slotalloc_donate", "cc_slotalloc_reclaim",
     "cc_slotalloc_alloc", "cc_slotalloc_free", "cc_slotalloc_free_bytes", "cc_last_error", "cc_version",
+    "cc_ctl_mem_bytes", "cc_ctl_flops", "cc_ctl_comm_seconds", "cc_ctl_speedup", "cc_ctl_speedup_vec", "cc_ctl_distance",
+    "cc_ctl_candidate_count", "cc_ctl_decide",
 )
 
 
@@ -250,6 +252,41 @@ def cc_kv_plan_migration(block_table: np.ndarray, seq_lens: np.ndarray, assign: 
 def cc_kv_migrate(ctx, k_pool, v_pool, page_bytes: int, src_pages, dst_pages, n_moves: int, stream=None) -> None:
     _check(_lib.cc_kv_migrate(ctx, _ptr(k_pool), _ptr(v_pool), C.c_size_t(page_bytes), _ptr(src_pages), _ptr(dst_pages),
                               C.c_int(n_moves), _stream(stream)))
+
+
+# ---- cost / speed-up model and scaling decision (host only) --------------------------------------------
+class cc_ctl_params(C.Structure):
+    _fields_ = [("L", C.c_int32), ("P_max", C.c_int32), ("slo", C.c_double), ("delta", C.c_double),
+                ("beta", C.c_double * (CC_MAX_REPLICAS + 1)), ("cost_per_device", C.c_double),
+                ("cost_per_layer_copy", C.c_double)]
+
+
+CC_CTL_NONE, CC_CTL_UPDATED, CC_CTL_INSTANCE_SCALE = range(3)
+for _n, _res, _args in (
+        ("cc_ctl_mem_bytes", C.c_double, [C.c_int, C.c_int, C.c_int, C.c_int, C.c_int, C.c_double]),
+        ("cc_ctl_flops", C.c_double, [C.c_int, C.c_int, C.c_int, C.c_int, C.c_int]),
+        ("cc_ctl_comm_seconds", C.c_double, [C.c_int, C.c_int, C.c_int, C.c_int, C.c_double, C.c_double]),
+        ("cc_ctl_speedup", C.c_double, [C.c_int, C.c_int, C.c_int, C.c_double]),
+        ("cc_ctl_speedup_vec", C.c_double, [C.c_void_p, C.c_int, C.c_int, C.c_double, C.c_int, C.c_double, C.c_double]),
+        ("cc_ctl_distance", C.c_int, [C.c_int, C.c_int, C.c_int, C.c_int]),
+        ("cc_ctl_candidate_count", C.c_int, [C.c_int, C.c_int])):
+    getattr(_lib, _n).restype = _res
+    getattr(_lib, _n).argtypes = _args
+cc_ctl_mem_bytes, cc_ctl_flops, cc_ctl_comm_seconds = _lib.cc_ctl_mem_bytes, _lib.cc_ctl_flops, _lib.cc_ctl_comm_seconds
+cc_ctl_speedup, cc_ctl_distance, cc_ctl_candidate_count = _lib.cc_ctl_speedup, _lib.cc_ctl_distance, _lib.cc_ctl_candidate_count
+
+
+def cc_ctl_speedup_vec(v, bs: int, t_comp_s: float, d_hidden: int, kappa: float, bandwidth: float) -> float:
+    a = np.ascontiguousarray(v, dtype=np.int32)
+    return _lib.cc_ctl_speedup_vec(_ptr(a), len(a), bs, t_comp_s, d_hidden, kappa, bandwidth)
+
+
+def cc_ctl_decide(params: "cc_ctl_params", N_cur: int, P_cur: int, latency: float, cold_capacity: float):
+    """-> (action, N_new, P_new, cold_capacity_after)"""
+    cold, n, p_, act = C.c_double(cold_capacity), C.c_int(0), C.c_int(0), C.c_int(0)
+    _check(_lib.cc_ctl_decide(C.byref(params), C.c_int(N_cur), C.c_int(P_cur), C.c_double(latency), C.byref(cold),
+                              C.byref(n), C.byref(p_), C.byref(act)))
+    return act.value, n.value, p_.value, cold.value
 
 
 # ---- stage taps (tests) ------------------------------------------------------------------------

@@ -1,0 +1,84 @@
+"""NEXT-4: the paper's cost / speed-up model and Algorithm 2.  The library (cc_control.cu)
+against the values the paper prints (tests/golden/paper_values.txt), against closed forms, and against the
+independent restatement in oracle/controller.py on random states."""
+import math
+
+import numpy as np
+import pytest
+
+from oracle import controller as O
+from paper_2607_04181_b200 import binding as B
+
+
+def _params(L=64, P_max=4, slo=30.0, delta=0.1, beta=(0, 0, 0.01, 0.015, 0.0175), c_dev=1.0, c_copy=0.0):
+    p = B.cc_ctl_params()
+    p.L, p.P_max, p.slo, p.delta, p.cost_per_device, p.cost_per_layer_copy = L, P_max, slo, delta, c_dev, c_copy
+    for i, b in enumerate(beta):
+        p.beta[i] = b
+    return p
+
+
+def test_values_the_paper_prints():
+    assert B.cc_ctl_speedup(60, 20, 2, 0.0) == pytest.approx(1.2, abs=1e-12)        # PAPER.md:127 with Eq. 7
+    assert B.cc_ctl_candidate_count(64, 4) == 256
+    d, bs, l = 4096, 8, 1
+    assert B.cc_ctl_mem_bytes(1, 1, 0, l, d, 2.0) == 2.0 * 12 * d * d               # Eq. 1: 12 d^2 parameters x kappa
+    assert B.cc_ctl_flops(1, 1, bs, l, d) == 24.0 * bs * l * d * d                  # Eq. 2
+    # bs = 1 and v > 1 cannot speed up (ceil(1/P) = 1), whatever the bandwidth
+    assert B.cc_ctl_speedup_vec([1] * 10 + [4] * 20 + [1] * 10, 1, 1e-3, d, 2.0, 1e30) == pytest.approx(1.0, abs=1e-9)
+
+
+def test_closed_forms_and_limits():
+    assert B.cc_ctl_speedup(32, 0, 4, 0.0) == 1.0 and B.cc_ctl_speedup(32, 7, 1, 0.0) == 1.0
+    assert B.cc_ctl_speedup(32, 32, 4, 0.0) == pytest.approx(4.0)                   # Amdahl's limit, alpha = 1
+    for P in (2, 3, 4):                                                             # monotone in N at fixed P (beta fixed)
+        s = [B.cc_ctl_speedup(40, N, P, 0.02) for N in range(41)]
+        assert all(b > a for a, b in zip(s, s[1:]))
+    # Eq. 8-10 reduce to Eq. 6 when bs divides evenly (one segment => two boundaries, each 2 * bs (P-1)/P * d * kappa / B)
+    L, N, P, bs, t, d, k, Bw = 48, 12, 4, 64, 2e-4, 4096, 2.0, 4e11
+    T = 2 * (2 * bs * (P - 1) / P * d * k / Bw)
+    want = L * t / ((L - N) * t + N * t / P + T)
+    assert B.cc_ctl_speedup_vec([1] * 5 + [P] * N + [1] * (L - N - 5), bs, t, d, k, Bw) == pytest.approx(want, rel=1e-12)
+    assert B.cc_ctl_comm_seconds(1, bs, 1, d, k, Bw) == 0.0
+    assert B.cc_ctl_distance(10, 2, 20, 2) == 10 and B.cc_ctl_distance(20, 2, 10, 2) == 10
+    assert B.cc_ctl_distance(10, 2, 10, 4) == 20 and B.cc_ctl_distance(0, 1, 5, 3) == 10
+
+
+def test_library_matches_the_plain_restatement_on_random_states():
+    rng = np.random.default_rng(3)
+    for _ in range(300):
+        L, P_max = int(rng.integers(2, 70)), int(rng.integers(1, 5))
+        beta = [0.0, 0.0] + sorted(rng.uniform(0, 0.05, 3).tolist())
+        slo, delta = float(rng.uniform(5, 40)), float(rng.uniform(0.0, 0.3))
+        c_dev, c_copy = float(rng.integers(0, 2)), float(rng.integers(0, 2)) * 0.25
+        N, P = int(rng.integers(0, L + 1)), int(rng.integers(1, P_max + 1))
+        lat, cold = slo * float(rng.uniform(0.4, 2.0)), float(rng.integers(0, 6))
+        p = _params(L, P_max, slo, delta, beta, c_dev, c_copy)
+        act, n1, p1, cold1 = B.cc_ctl_decide(p, N, P, lat, cold)
+        want = O.decide(L, P_max, slo, delta, beta, c_dev, c_copy, N, P, lat, cold)
+        assert (("none", "updated", "instance_scale")[act], n1, p1) == want[:3] and cold1 == pytest.approx(want[3])
+        for (n0, p0, n2, p2) in rng.integers(0, 5, (4, 4)).tolist():
+            n0, n2, p0, p2 = min(n0 * L // 4, L), min(n2 * L // 4, L), max(p0, 1), max(p2, 1)
+            assert B.cc_ctl_distance(n0, p0, n2, p2) == O.distance(L, n0, p0, n2, p2)
+
+
+def test_the_papers_worked_example_does_not_follow_from_its_own_rule():
+    """N=10, P=2 at 1.3 x SLO 'identifies N=20, P=2 as the nearest candidate satisfying S >= alpha_req'.
+    With Eq. 7 and Alg. 2 line 5, alpha_req = S(10, 2) * 1.3 > S(20, 2) for every model the paper evaluates (36, 40, 64
+    layers; it holds only below ~27 layers), so (20, 2) is not even a candidate there.  Recorded here so that nobody 'fixes' the controller to match the example."""
+    for L in (36, 40, 60, 64, 80):
+        assert B.cc_ctl_speedup(L, 10, 2, 0.0) * 1.3 > B.cc_ctl_speedup(L, 20, 2, 0.0)
+    p = _params(L=60, beta=(0, 0, 0, 0, 0), c_dev=1.0, c_copy=0.0, delta=0.05)
+    act, n1, p1, _ = B.cc_ctl_decide(p, 10, 2, 1.3 * p.slo, 0.0)
+    # what the rule does give with no cold device: the nearest configuration with S >= 1.418 at P = 2 (no new device)
+    assert act == B.CC_CTL_UPDATED and p1 == 2 and B.cc_ctl_speedup(60, n1, 2, 0.0) >= B.cc_ctl_speedup(60, 10, 2, 0.0) * 1.3
+    assert B.cc_ctl_speedup(60, n1 - 1, 2, 0.0) < B.cc_ctl_speedup(60, 10, 2, 0.0) * 1.3
+
+
+def test_decisions_scale_down_none_and_instance_scale():
+    p = _params(L=64, beta=(0, 0, 0, 0, 0), delta=0.1)
+    assert B.cc_ctl_decide(p, 16, 2, p.slo * 1.05, 0.0)[0] == B.CC_CTL_NONE          # inside the tolerance band
+    act, n1, p1, cold = B.cc_ctl_decide(p, 32, 4, p.slo * 0.5, 0.0)                  # over-provisioned: scale down, devices returned
+    assert act == B.CC_CTL_UPDATED and cold >= 0.0 and B.cc_ctl_speedup(64, n1, p1, 0.0) >= B.cc_ctl_speedup(64, 32, 4, 0.0) * 0.5
+    act, n1, p1, cold = B.cc_ctl_decide(p, 64, 4, p.slo * 1.5, 10.0)                 # already at the model's limit
+    assert act == B.CC_CTL_INSTANCE_SCALE and (n1, p1) == (64, 4) and cold == 10.0
