@@ -50,6 +50,9 @@ def parse_args():
     ap.add_argument("--replicas", type=int, default=2, choices=[1, 2, 3, 4])
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--batch", type=int, default=0,
+                    help="decode batch of the cfg2 layer benchmark (default: the config's 64); larger batches are for the "
+                         "tensor-pipe evidence of the GEMMs (DESIGN.md section 9), not the headline")
     ap.add_argument("--workload", default="cfg2", choices=["cfg2", "cfg3"],
                     help="cfg2 (default): the headline layer benchmark; cfg3: BASELINE.json configs[2], the 32-layer "
                          "decode graph with layers 10-12 flipped to 2 replicas and back (latency series, not the headline)")
@@ -206,6 +209,8 @@ def run_ours(args):
         torch.cuda.synchronize()
 
     shape, R, K, W = I.CFG2, args.replicas, args.steps, max(args.warmup, 3)
+    if args.batch:
+        shape = shape.with_batch(args.batch)
     batch = shape.batch
     w = I.make_weights(shape, 1002)
     st = I.make_step_inputs(shape, 2002 + 10 * rank, 3002 + 10 * rank)     # every rank its own batch
@@ -258,9 +263,15 @@ def run_ours(args):
                                           step.n_pages, step.seq_lens, step.assign, batch, stream)
     stage_ms /= n_prof
     sb = stage_bytes(shape, st.seq_lens, R)
+    # tensor work of the GEMMs: two bf16 planes (hi + lo) of the activations, 2 flops per multiply-add
+    rows = int((st.seq_lens > 0).sum())
+    gemm_flops = {"gemm_qkv": (shape.q_dim + 2 * shape.kv_dim) * shape.hidden, "gemm_o": shape.hidden * shape.q_dim,
+                  "gemm_gate_up": 2 * shape.ffn * shape.hidden, "gemm_down": shape.hidden * shape.ffn}
     stages = {}
     for i, name in enumerate(B.STAGE_NAMES):
         e = {"ms": round(float(stage_ms[i]), 5)}
+        if name in gemm_flops:
+            e["tensor_TFLOPs_two_planes"] = round(2 * 2.0 * rows * gemm_flops[name] / (stage_ms[i] * 1e-3) / 1e12, 1)
         if name in sb:
             e["bytes"] = sb[name]
             e["GBps"] = round(sb[name] / (stage_ms[i] * 1e-3) / 1e9, 1)
@@ -382,7 +393,7 @@ def run_ours(args):
             "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "bf16", "data": "synthetic",
             "config": {"workload": "cfg2 (BASELINE.json configs[1]): Llama-3-8B-shaped decoder layer, hidden 4096, "
-                                   "32 q / 8 kv heads x 128, FFN 14336, decode batch 64, contexts U{512..2048}, "
+                                   f"32 q / 8 kv heads x 128, FFN 14336, decode batch {batch}, contexts U{{512..2048}}, "
                                    "16-token pages, shuffled block tables",
                        "replicas": R, "batch_split": np.bincount(assign, minlength=R).tolist(),
                        "launch": "one CUDA graph of cc_forward, replayed; PDL between its kernels",
