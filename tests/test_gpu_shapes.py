@@ -17,6 +17,8 @@ CASES = {
     "model_b": (I.LayerShape("modelBs", 1536, 12, 2, 128, 8960, 1e-6, 10000.0, 10, 30, 400), 10, 3),
     "hkv4_dh64": (I.LayerShape("hkv4", 512, 8, 4, 64, 1024, 1e-5, 10000.0, 9, 10, 150), 9, 2),
     "hkv1_g8": (I.LayerShape("hkv1", 256, 8, 1, 128, 512, 1e-5, 10000.0, 5, 20, 200), 5, 1),
+    # nothing a multiple of 128: hidden 5 x 64, q width 5 x 64, FFN 200 (not a multiple of 64), odd GQA group
+    "odd_sizes": (I.LayerShape("odd", 320, 5, 1, 64, 200, 1e-5, 10000.0, 6, 10, 90), 6, 2),
     "hkv8_g1": (I.LayerShape("hkv8", 1024, 8, 8, 128, 2048, 1e-5, 500000.0, 7, 100, 600), 7, 4),
 }
 
