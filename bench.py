@@ -53,9 +53,11 @@ def parse_args():
     ap.add_argument("--batch", type=int, default=0,
                     help="decode batch of the cfg2 layer benchmark (default: the config's 64); larger batches are for the "
                          "tensor-pipe evidence of the GEMMs (DESIGN.md section 9), not the headline")
-    ap.add_argument("--workload", default="cfg2", choices=["cfg2", "cfg3"],
+    ap.add_argument("--workload", default="cfg2", choices=["cfg2", "cfg3", "cfg5"],
                     help="cfg2 (default): the headline layer benchmark; cfg3: BASELINE.json configs[2], the 32-layer "
-                         "decode graph with layers 10-12 flipped to 2 replicas and back (latency series, not the headline)")
+                         "decode graph with layers 10-12 flipped to 2 replicas and back (latency series, not the headline); "
+                         "cfg5: configs[4], the co-located serving loop (decode only)")
+    ap.add_argument("--horizon", type=float, default=120.0, help="cfg5: seconds of synthetic arrivals")
     return ap.parse_args()
 
 
@@ -591,10 +593,58 @@ def run_cfg3(args):
     return 0
 
 
+# ---------------------------------------------------------------------------------------------
+# cfg5 (BASELINE.json configs[4]): skewed co-located serving, decode only (no prefill kernel yet: NEXT-2)
+# ---------------------------------------------------------------------------------------------
+def run_cfg5(args):
+    import torch
+
+    from paper_2607_04181_b200 import inputs as I
+    from paper_2607_04181_b200 import serving as S
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the library has no CPU fallback")
+    torch.cuda.set_device(0)
+    rng = np.random.default_rng(3005)
+    load = rng.lognormal(0.0, 1.0, 32)                               # synthetic per-layer load: the top 25 % are "hot"
+    hot = tuple(sorted(np.argsort(-load)[:8].tolist()))
+    arrivals = S.make_arrivals(seed=3005, horizon_s=args.horizon, base_rps=7.0, burst_x=5.0, burst_len_s=10.0, burst_every_s=60.0,
+                               frac_a=0.75, prompt_mean=512, out_mean=256, sigma=1.0, max_prompt=4096, max_out=1024)
+    shape_a = I.CFG2
+    shape_b = I.MODEL_B_LAYER
+    A = S.ModelRunner("A", shape_a, 32, 128, 12000, 5120, seed=1005, n_slots=0, hot_layers=hot)
+    Bm = S.ModelRunner("B", shape_b, 28, 64, 6000, 5120, seed=1006, n_slots=0)
+    sampler = ClockSampler(0)
+    sampler.start()
+    t0 = time.perf_counter()
+    out, _ = S.simulate(A, Bm, arrivals, burst_hi=48, burst_lo=16)
+    wall = time.perf_counter() - t0
+    clocks = sampler.stop()
+    A.close()
+    Bm.close()
+    line = {
+        "metric": "co-located serving (cfg5): model A tokens/s and per-token latency", "value": out["A"]["tokens_per_s_while_stepping"],
+        "unit": UNIT, "n_gpus": 1, "steps": out["steps"], "warmup": 0,
+        "ms_per_step": 1e3 * out["clock_s"] / max(1, out["steps"]), "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "bf16", "data": "synthetic",
+        "config": {"workload": "cfg5 (BASELINE.json configs[4]): model A = 32 Llama-3-8B-shaped layers (75 % of the requests), model B = 28 "
+                               "layers of hidden 1536 / 12 q / 2 kv heads x 128 / FFN 8960; Poisson arrivals 7 req/s with 5x bursts of 10 s every "
+                               f"60 s over {args.horizon:.0f} s, prompts lognormal (mean 512), outputs lognormal (mean 256); decode only: prompts count as "
+                               "cached KV (no prefill kernel yet); A's 8 hot layers get a second replica in memory lent from B's KV reserve "
+                               "while A's backlog is >= 48 requests",
+                   "hot_layers": list(hot), "requests": len(arrivals)},
+        "clocks": clocks, "serving": out, "wall_s": round(wall, 1),
+    }
+    print(json.dumps(line), flush=True)
+    return 0
+
+
 def main():
     args = parse_args()
     if args.impl == "reference":
         return run_reference(args)
+    if args.workload == "cfg5":
+        return run_cfg5(args)
     if args.workload == "cfg3":
         return run_cfg3(args)
     return run_ours(args)
