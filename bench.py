@@ -35,7 +35,8 @@ if ROOT not in sys.path:
 METRIC = "replicated decode-layer tokens/s"
 UNIT = "tokens/s"
 REF_ROWS_PER_STEP = 4       # --impl reference: rows of the batch the oracle computes per step
-CPU_BASELINE_ROWS = 32      # cpu_baseline leg of the default arm (about 10 s of CPU work)
+CPU_BASELINE_ROWS = 64      # cpu_baseline leg of the default arm: the whole batch ...
+CPU_BASELINE_STEPS = 4      # ... four times (about 10 s of CPU work on 16 cores)
 # dram__bytes_read.sum + dram__bytes_write.sum of the gate/up GEMM (k_gemm<2>) per launch at R = 2, from the
 # ncu --set full capture summarised in profiles/r01k_full_R2.md (470 888 448 + 7 401 984 bytes)
 NCU_TRAFFIC_GATE_UP_R2 = 478290432
@@ -431,10 +432,10 @@ def run_ours(args):
     # ---- the oracle on this box's host cores, bounded sample (rank 0, N = 1) --------------------------
     cpu = None
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
-        tps, s_per_step, cores = time_oracle(shape, w, st, CPU_BASELINE_ROWS, 1, 0)
+        tps, s_per_step, cores = time_oracle(shape, w, st, min(CPU_BASELINE_ROWS, batch), CPU_BASELINE_STEPS, 0)
         cpu = {"value": tps, "unit": UNIT, "cores": cores, "kind": "oracle",
-               "sample": f"first {CPU_BASELINE_ROWS} of the 64 rows of the same cfg2 batch, one full layer step, "
-                         f"{s_per_step:.1f} s of oracle/cc_oracle.c (OpenMP)"}
+               "sample": f"all {min(CPU_BASELINE_ROWS, batch)} rows of the same cfg2 batch, {CPU_BASELINE_STEPS} full layer steps of "
+                         f"{s_per_step:.1f} s each, oracle/cc_oracle.c (OpenMP)"}
     S.close()
 
     if rank == 0:
