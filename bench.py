@@ -426,6 +426,34 @@ def run_ours(args):
                         "GBps_read_plus_write": round(2 * moved / (mms * 1e-3) / 1e9, 1),
                         "frac_of_copy_peak": round(2 * moved / (mms * 1e-3) / 1e9 / peak, 4),
                         "what": "batch split 32 + 32 over two page partitions; every page outside its replica's partition moved"}
+        # the same move list, chunked on a side stream under a train of decode steps: what do the
+        # steps pay, what does the copy pay?  (pre-copy protocol: harness.KvLiveMigration, tests/test_kv_migration.py)
+        side, ev, n_mt, chunk = torch.cuda.Stream(), torch.cuda.Event(), 4, 4096
+
+        def mtrain(with_mig: bool):
+            a, b_ = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a.record()
+            if with_mig:
+                side.wait_stream(stream)
+                for c0 in range(0, len(src), chunk):
+                    n = min(chunk, len(src) - c0)
+                    B.cc_kv_migrate(S.ctx, step.k_pool, step.v_pool, page_bytes, d_src[c0:c0 + n], d_dst[c0:c0 + n], n, side)
+                ev.record(side)
+            for _ in range(n_mt):
+                graph.replay()
+            if with_mig:
+                stream.wait_event(ev)
+            b_.record()
+            torch.cuda.synchronize()
+            return a.elapsed_time(b_)
+        for _ in range(2):
+            mtrain(False), mtrain(True)
+        tp = float(np.median([mtrain(False) for _ in range(5)]))
+        tm = float(np.median([mtrain(True) for _ in range(5)]))
+        kv_migration["overlapped"] = {"steps_in_train": n_mt, "chunk_pages": chunk, "ms_train_plain": round(tp, 4),
+                                      "ms_train_with_migration": round(tm, 4), "step_inflation": round(tm / tp - 1.0, 4),
+                                      "ms_if_serialised": round(tp + mms, 4),
+                                      "ms_bandwidth_bound": round(tp + 2 * moved / (peak * 1e9) * 1e3, 4)}
     except B.CcError as e:
         kv_migration = {"error": str(e)}
 

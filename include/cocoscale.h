@@ -218,6 +218,23 @@ cc_status cc_kv_plan_migration(const int32_t *block_table_host, const int32_t *s
                                int n_replicas, int32_t *new_block_table_host, int32_t *src_pages_host,
                                int32_t *dst_pages_host, int *n_moves);
 
+/* Pre-copy migration, second half (the transfer is chunked and fitted between decode steps, so
+ * decoding goes on -- with the OLD table -- while the bulk of a plan is copied on a side stream).  Once that copy
+ * has finished, this plans what the steps wrote meanwhile.  seq_lens_planned is the seq_lens array the first
+ * plan was made with (of the last step enqueued before it, or of the next one: a step writes position
+ * seq_len - 1, so either way only positions >= seq_lens_planned - 1 can have changed).  For every row, pages
+ * with index < (seq_lens_planned - 1) / 16 keep the place `planned_block_table` gave them; the tail page of
+ * then and every page added since are taken from `block_table_now` and planned by cc_kv_plan_migration's
+ * rule over that hybrid table.  seq_lens_now[b] >= seq_lens_planned[b], or 0 for a row
+ * that finished (a slot re-used by a new request passes seq_lens_planned[b] = 0).  The caller must not have
+ * handed out a destination of the first plan as a new page meanwhile (CC_ERR_INVALID: referenced twice).
+ * Outputs as cc_kv_plan_migration: `final_block_table` is the table to swap in after the returned moves ran. */
+cc_status cc_kv_plan_catchup(const int32_t *block_table_now_host, const int32_t *seq_lens_planned_host,
+                             const int32_t *seq_lens_now_host, const int32_t *planned_block_table_host,
+                             const int32_t *replica_assign_host, int batch, int max_blocks_per_seq, int n_pages,
+                             int n_replicas, int32_t *final_block_table_host, int32_t *src_pages_host,
+                             int32_t *dst_pages_host, int *n_moves);
+
 /* Copies page src[i] -> dst[i] (all kv heads, page_bytes = n_kv_heads * 16 * head_dim * 2) in both pools,
  * for i < n_moves; src/dst lists are DEVICE int32.  Sources and destinations must be disjoint sets (the
  * planner guarantees it).  Enqueue-only on `stream`: put it between decode steps, or on a side stream

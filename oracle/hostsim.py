@@ -112,6 +112,28 @@ def plan_kv_migration(block_table, seq_lens, assign, n_pages: int, n_replicas: i
     return new_bt.astype(np.int32), moves
 
 
+def plan_kv_catchup(block_table_now, seq_planned, seq_now, planned_block_table, assign, n_pages: int, n_replicas: int,
+                    page: int = 16):
+    """Second half of a pre-copy migration (decoding continues while the cache is moved chunk by
+    chunk).  Token t of a row lives in page t // page of its row, and a decode step of length s only writes
+    token s - 1: after a plan made with seq_planned, only tokens >= seq_planned - 1 can have been
+    written.  Pages holding such a token -- wherever the row holds them NOW -- are (re)planned by
+    plan_kv_migration's rule, the others stay where the first plan put them.  Returns (final_block_table, moves) or None when a partition is full."""
+    import numpy as np
+    now = np.array(block_table_now, dtype=np.int64)
+    planned = np.array(planned_block_table, dtype=np.int64)
+    mixed = now.copy()
+    for b in range(now.shape[0]):
+        if seq_now[b] <= 0:
+            continue
+        assert seq_now[b] >= seq_planned[b]
+        for j in range(-(-int(seq_now[b]) // page)):
+            written_since = (j + 1) * page > int(seq_planned[b]) - 1            # holds a token position >= seq_planned - 1
+            if not written_since:
+                mixed[b, j] = planned[b, j]
+    return plan_kv_migration(mixed, seq_now, assign, n_pages, n_replicas, page)
+
+
 def apply_kv_migration(k_pool, v_pool, moves):
     """Byte copy of whole pages (all kv heads) in both pools, in move order."""
     for s, d in moves:

@@ -29,7 +29,7 @@ EXPORTS = (
     "cc_ctx_create", "cc_ctx_destroy", "cc_ctx_donate", "cc_ctx_reclaim", "cc_ctx_set_copy_chunk",
     "cc_ctx_set_pdl", "cc_poll_device_error", "cc_create_layer", "cc_destroy_layer", "cc_layer_blob_bytes",
     "cc_scale_layer", "cc_commit", "cc_release_replica", "cc_query", "cc_replica_blob", "cc_forward",
-    "cc_forward_host", "cc_forward_profiled", "cc_forward_launch_count", "cc_replica_copy", "cc_kv_plan_migration", "cc_kv_migrate", "cc_debug_tap", "cc_debug_grouping",
+    "cc_forward_host", "cc_forward_profiled", "cc_forward_launch_count", "cc_replica_copy", "cc_kv_plan_migration", "cc_kv_plan_catchup", "cc_kv_migrate", "cc_debug_tap", "cc_debug_grouping",
     "cc_slotalloc_create", "cc_slotalloc_destroy", "cc_slotalloc_donate", "cc_slotalloc_reclaim",
     "cc_slotalloc_alloc", "cc_slotalloc_free", "cc_slotalloc_free_bytes", "cc_last_error", "cc_version",
     "cc_ctl_mem_bytes", "cc_ctl_flops", "cc_ctl_comm_seconds", "cc_ctl_speedup", "cc_ctl_speedup_vec", "cc_ctl_distance",
@@ -247,6 +247,25 @@ def cc_kv_plan_migration(block_table: np.ndarray, seq_lens: np.ndarray, assign: 
     _check(_lib.cc_kv_plan_migration(_ptr(bt), _ptr(sl), _ptr(ra), C.c_int(batch), C.c_int(width), C.c_int(n_pages),
                                      C.c_int(n_replicas), _ptr(new_bt), _ptr(src), _ptr(dst), C.byref(n)))
     return new_bt, src[:n.value].copy(), dst[:n.value].copy()
+
+
+def cc_kv_plan_catchup(block_table_now: np.ndarray, seq_lens_planned: np.ndarray, seq_lens_now: np.ndarray,
+                       planned_block_table: np.ndarray, assign: np.ndarray, n_pages: int, n_replicas: int):
+    """-> (final_block_table, src_pages, dst_pages); host arrays, argument marshalling only."""
+    bt = np.ascontiguousarray(block_table_now, dtype=np.int32)
+    s0 = np.ascontiguousarray(seq_lens_planned, dtype=np.int32)
+    s1 = np.ascontiguousarray(seq_lens_now, dtype=np.int32)
+    pb = np.ascontiguousarray(planned_block_table, dtype=np.int32)
+    ra = np.ascontiguousarray(assign, dtype=np.int32)
+    batch, width = bt.shape
+    assert pb.shape == bt.shape
+    final_bt = np.empty_like(bt)
+    src = np.empty(batch * width, dtype=np.int32)
+    dst = np.empty(batch * width, dtype=np.int32)
+    n = C.c_int(0)
+    _check(_lib.cc_kv_plan_catchup(_ptr(bt), _ptr(s0), _ptr(s1), _ptr(pb), _ptr(ra), C.c_int(batch), C.c_int(width),
+                                   C.c_int(n_pages), C.c_int(n_replicas), _ptr(final_bt), _ptr(src), _ptr(dst), C.byref(n)))
+    return final_bt, src[:n.value].copy(), dst[:n.value].copy()
 
 
 def cc_kv_migrate(ctx, k_pool, v_pool, page_bytes: int, src_pages, dst_pages, n_moves: int, stream=None) -> None:

@@ -770,6 +770,26 @@ cc_status cc_kv_plan_migration(const int32_t* bt, const int32_t* seq_lens, const
     return CC_OK;
 }
 
+// Catch-up plan of a pre-copy migration: pages that cannot have been written since the first plan keep their
+// planned place; the rest (the tail page of then, pages added since) is planned again from the table the decode
+// steps kept using.
+cc_status cc_kv_plan_catchup(const int32_t* bt_now, const int32_t* seq_planned, const int32_t* seq_now, const int32_t* planned_bt,
+                             const int32_t* assign, int batch, int max_blocks, int n_pages, int n_replicas, int32_t* final_bt,
+                             int32_t* src, int32_t* dst, int* n_moves) {
+    if (!bt_now || !seq_planned || !seq_now || !planned_bt || !final_bt) return fail(CC_ERR_INVALID, "null argument");
+    if (batch < 1 || max_blocks < 1) return fail(CC_ERR_INVALID, "bad sizes");
+    std::vector<int32_t> hybrid(bt_now, bt_now + (size_t)batch * max_blocks);
+    for (int b = 0; b < batch; ++b) {
+        if (seq_now[b] <= 0) continue;                         // the row finished meanwhile: nothing to keep
+        if (seq_now[b] < seq_planned[b]) return fail(CC_ERR_INVALID, "row %d shrank from %d to %d tokens during the migration", b, seq_planned[b], seq_now[b]);
+        // a step with seq_len s writes position s - 1: whether the step of seq_planned had run or not when the plan
+        // was made, only positions >= seq_planned - 1 can have been written since -- pages below that are clean
+        const int clean = seq_planned[b] > 0 ? (seq_planned[b] - 1) / CC_PAGE_SIZE : 0;
+        for (int j = 0; j < clean && j < max_blocks; ++j) hybrid[(size_t)b * max_blocks + j] = planned_bt[(size_t)b * max_blocks + j];
+    }
+    return cc_kv_plan_migration(hybrid.data(), seq_now, assign, batch, max_blocks, n_pages, n_replicas, final_bt, src, dst, n_moves);
+}
+
 cc_status cc_kv_migrate(cc_ctx* ctx, void* k_pool_dev, void* v_pool_dev, size_t page_bytes, const int32_t* src_dev,
                         const int32_t* dst_dev, int n_moves, void* stream) {
     if (!ctx || !k_pool_dev || !v_pool_dev) return fail(CC_ERR_INVALID, "null argument");

@@ -173,3 +173,60 @@ class ModelSession:
     def __exit__(self, *exc):
         self.close()
         return False
+
+
+class KvLiveMigration:
+    """KV redistribution overlapped with decoding, as a pre-copy:
+
+      start()   plans on the table as it is (cc_kv_plan_migration) and enqueues the page copies chunk by chunk
+                on a side stream; decode steps keep running on the main stream with the OLD table;
+      finish()  makes the main stream wait for that copy, plans what the steps wrote meanwhile
+                (cc_kv_plan_catchup: the tail page of then, pages added since), copies those few pages on the
+                main stream and overwrites the device block table in place -- the next replay of a captured
+                graph reads the new table from the same address.
+
+    One copy block moves one page, so the hardware already interleaves the copy with the decode kernels page by
+    page; cutting the list into many launches only adds launch gaps (measured: DESIGN.md 7b), hence the large
+    default chunk.  Plumbing only: both plans are the library's, both copies are its kernel.  While a migration runs the page
+    allocator of the caller must not hand out `reserved` (the destinations of the first plan)."""
+
+    def __init__(self, ctx, step: DeviceStep, page_bytes: int, n_replicas: int, chunk_pages: int = 4096):
+        self.ctx, self.step, self.page_bytes, self.R, self.chunk = ctx, step, page_bytes, n_replicas, max(1, chunk_pages)
+        self.done = torch.cuda.Event()
+        self.planned_bt = self.seq_planned = self.assign = None
+        self.reserved: set[int] = set()
+        self.bulk_moves = self.catchup_moves = 0
+        self._keep = []
+
+    def _enqueue(self, src: np.ndarray, dst: np.ndarray, stream) -> None:
+        if len(src) == 0:
+            return
+        s = torch.from_numpy(src).to(self.step.device)
+        d = torch.from_numpy(dst).to(self.step.device)
+        self._keep += [s, d]                       # the lists must outlive the kernels that read them
+        for c0 in range(0, len(src), self.chunk):
+            n = min(self.chunk, len(src) - c0)
+            B.cc_kv_migrate(self.ctx, self.step.k_pool, self.step.v_pool, self.page_bytes, s[c0:c0 + n], d[c0:c0 + n], n, stream)
+
+    def start(self, block_table_host: np.ndarray, seq_lens_host: np.ndarray, assign: np.ndarray, side_stream) -> int:
+        self.seq_planned = np.array(seq_lens_host, dtype=np.int32)
+        self.assign = np.array(assign, dtype=np.int32)
+        self.planned_bt, src, dst = B.cc_kv_plan_migration(block_table_host, self.seq_planned, self.assign, self.step.n_pages, self.R)
+        self.reserved = set(dst.tolist())
+        self.bulk_moves = len(src)
+        side_stream.wait_stream(torch.cuda.current_stream())   # pages written by steps already enqueued are final
+        self._enqueue(src, dst, side_stream)
+        self.done.record(side_stream)
+        return self.bulk_moves
+
+    def finish(self, block_table_now_host: np.ndarray, seq_lens_now_host: np.ndarray, stream=None) -> np.ndarray:
+        stream = torch.cuda.current_stream() if stream is None else stream
+        stream.wait_event(self.done)
+        final_bt, src, dst = B.cc_kv_plan_catchup(block_table_now_host, self.seq_planned, seq_lens_now_host, self.planned_bt,
+                                                  self.assign, self.step.n_pages, self.R)
+        self.catchup_moves = len(src)
+        with torch.cuda.stream(stream):
+            self._enqueue(src, dst, stream)
+            self.step.block_table.copy_(torch.from_numpy(final_bt))
+        self.reserved = set()
+        return final_bt

@@ -99,3 +99,164 @@ def test_migrated_cache_gives_bit_identical_outputs():
         for b in range(batch):
             for j in range((int(st.seq_lens[b]) + 15) // 16):
                 assert assign[b] * psz <= new_bt[b, j] < (assign[b] + 1) * psz
+
+
+def _pages_of(bt, seq):
+    return {int(bt[b, j]) for b in range(bt.shape[0]) if seq[b] > 0 for j in range((int(seq[b]) + 15) // 16)}
+
+
+def _grow(rng, bt, seq, n_pages, reserved, steps, finish_prob=0.0):
+    """Rows decode `steps` more tokens with the old table: a new page (any free one that is not reserved, drawn at
+    random so that it usually lies outside the row's partition) whenever a token starts a page."""
+    bt, seq = bt.copy(), seq.copy()
+    free = sorted(set(range(n_pages)) - _pages_of(bt, seq) - set(reserved))
+    rng.shuffle(free)
+    for _ in range(steps):
+        for b in range(len(seq)):
+            if seq[b] <= 0 or seq[b] >= bt.shape[1] * 16:
+                continue
+            seq[b] += 1
+            if (seq[b] - 1) % 16 == 0:                                     # the token being decoded opens a page
+                bt[b, (seq[b] - 1) // 16] = free.pop()
+    for b in range(len(seq)):
+        if seq[b] > 0 and rng.random() < finish_prob:
+            seq[b] = 0
+    return bt, seq
+
+
+def test_catchup_plan_matches_the_host_simulation_exactly():
+    """Pre-copy migration: decode steps go on with the old table while the bulk is copied; the
+    catch-up plan covers what they wrote.  Library == independent simulation, plus what must hold whatever the
+    rule: untouched pages keep their first-plan place, everything ends in its partition, nothing is shared."""
+    from paper_2607_04181_b200 import binding as B
+    rng = np.random.default_rng(11)
+    done = 0
+    for trial in range(80):
+        R = int(rng.integers(1, 5))
+        batch, width = int(rng.integers(1, 12)), int(rng.integers(2, 8))
+        n_pages = int(batch * width * rng.uniform(2.5, 4.0)) + 4 * R
+        bt, seq, assign = _scenario(rng, batch, n_pages, width, R)
+        first = hostsim.plan_kv_migration(bt, seq, assign, n_pages, R)
+        if first is None:
+            continue
+        planned_bt, moves = first
+        bt_now, seq_now = _grow(rng, bt, seq, n_pages, [d for _, d in moves], int(rng.integers(0, 40)), finish_prob=0.1)
+        want = hostsim.plan_kv_catchup(bt_now, seq, seq_now, planned_bt, assign, n_pages, R)
+        try:
+            final_bt, src, dst = B.cc_kv_plan_catchup(bt_now, seq, seq_now, planned_bt, assign, n_pages, R)
+        except B.CcError as e:
+            assert e.status == B.CC_ERR_NO_SLOT and want is None
+            continue
+        assert want is not None
+        assert np.array_equal(final_bt, want[0]) and list(zip(src.tolist(), dst.tolist())) == want[1]
+        psz = n_pages // R
+        seen = set()
+        for b in range(batch):
+            if seq_now[b] <= 0:
+                continue
+            for j in range((int(seq_now[b]) + 15) // 16):
+                pg = int(final_bt[b, j])
+                assert assign[b] * psz <= pg < (assign[b] + 1) * psz and pg not in seen
+                seen.add(pg)
+                if (j + 1) * 16 <= seq[b] - 1:                              # only tokens < seq_planned - 1: never rewritten
+                    assert pg == planned_bt[b, j]
+        # no page is both read and written by the catch-up copy, and it moves only what the steps touched
+        assert not (set(dst.tolist()) & set(src.tolist())) and len(set(dst.tolist())) == len(dst)
+        assert len(src) <= sum(1 + (int(seq_now[b]) + 15) // 16 - (int(seq[b]) + 15) // 16 if seq[b] > 0 else (int(seq_now[b]) + 15) // 16
+                               for b in range(batch) if seq_now[b] > 0)
+        done += 1
+    assert done > 40
+
+
+def test_catchup_rejects_a_row_that_shrank():
+    from paper_2607_04181_b200 import binding as B
+    bt = np.array([[0, 1, 2]], np.int32)
+    with pytest.raises(B.CcError) as e:
+        B.cc_kv_plan_catchup(bt, np.array([40], np.int32), np.array([33], np.int32), bt, np.zeros(1, np.int32), 8, 1)
+    assert e.value.status == B.CC_ERR_INVALID
+
+
+@pytest.mark.gpu
+def test_migration_overlapped_with_decode_steps_changes_nothing():
+    """the cache is redistributed while decoding goes on.  Six decode steps (rows grow, some open
+    a page) run while the bulk copy is in flight on a side stream; catch-up + table swap; two more steps.  Every
+    step's output and, at the end, every row's cache (gathered through its table) equal the run without migration
+    bit for bit; all pages end inside their replica's partition; the graph is never re-captured."""
+    import torch
+    from paper_2607_04181_b200 import binding as B
+    from paper_2607_04181_b200.harness import DeviceStep, KvLiveMigration, Session
+
+    shape = I.LayerShape("mid", 512, 8, 2, 128, 1408, 1e-5, 500000.0, 23, 200, 690)
+    batch, R, during, after = 23, 2, 6, 2
+    w = I.make_weights(shape, 1302)
+    n_pages = 4 * batch * shape.max_blocks
+    ctx = I.draw_contexts(shape, 3302, batch)
+    ctx[:4] = [207, 208, 223, 224]                  # rows that open a page at the first step, just did, or will later
+    st = I.make_step_inputs(shape, 2302, 3302, batch=batch, n_pages=n_pages, contexts=ctx)
+    assign = I.even_split(batch, R)
+    page_bytes = shape.n_kv_heads * shape.page * shape.head_dim * 2
+    rng = np.random.default_rng(7)
+
+    def run(migrate: bool):
+        with Session(shape, w, max_batch=batch) as S:
+            S.scale(R)
+            step = DeviceStep(st, assign)
+            h0 = step.hidden.clone()
+            bt, seq = st.block_table.copy(), st.seq_lens.copy()
+            graph = torch.cuda.CUDAGraph()
+            main = torch.cuda.Stream()
+            side = torch.cuda.Stream()
+            outs = []
+            with torch.cuda.stream(main):
+                S.forward(step, main)                                       # warm-up (appends position seq - 1)
+                main.synchronize()
+                with torch.cuda.graph(graph, stream=main):
+                    S.forward(step, main)
+                mig = KvLiveMigration(S.ctx, step, page_bytes, R, chunk_pages=64)
+                free = None
+                for i in range(during + after):
+                    if migrate and i == 0:
+                        assert mig.start(bt, seq, assign, side) > 100
+                    if migrate and i == during:
+                        final_bt = mig.finish(bt, seq, main)
+                        assert mig.catchup_moves > 0
+                        bt = final_bt.copy()
+                        free = None                                         # old places are free again, new ones taken
+                    if free is None:
+                        free = sorted(set(range(n_pages)) - _pages_of(bt, seq) - mig.reserved)
+                        rng.shuffle(free)
+                    # the step decodes one more token per row
+                    seq = seq + 1
+                    for b in range(batch):
+                        if (seq[b] - 1) % 16 == 0:
+                            bt[b, (seq[b] - 1) // 16] = free.pop()
+                    step.block_table.copy_(torch.from_numpy(bt))
+                    step.seq_lens.copy_(torch.from_numpy(seq))
+                    step.hidden.copy_(h0)
+                    graph.replay()
+                    outs.append(step.hidden.clone())
+                main.synchronize()
+            side.synchronize()
+            assert B.cc_poll_device_error(S.ctx) == 0
+            kp, vp = step.pools_bits()
+            rows = [(kp[bt[b, :(seq[b] + 15) // 16]].copy(), vp[bt[b, :(seq[b] + 15) // 16]].copy()) for b in range(batch)]
+            return [o.cpu().view(torch.int16).numpy() for o in outs], rows, bt, seq
+
+    rng = np.random.default_rng(7)
+    base_out, base_rows, _, _ = run(False)
+    rng = np.random.default_rng(7)
+    mig_out, mig_rows, bt, seq = run(True)
+    for i, (a, b_) in enumerate(zip(base_out, mig_out)):
+        assert np.array_equal(a, b_), f"step {i} differs"
+    for b in range(batch):
+        n_tok = int(seq[b])
+        for (x, y) in zip(base_rows[b], mig_rows[b]):
+            # [pages][kv heads][16][head_dim] -> compare the tokens that exist
+            xs = x.transpose(1, 0, 2, 3).reshape(shape.n_kv_heads, -1, shape.head_dim)[:, :n_tok]
+            ys = y.transpose(1, 0, 2, 3).reshape(shape.n_kv_heads, -1, shape.head_dim)[:, :n_tok]
+            assert np.array_equal(xs, ys)
+    psz = n_pages // R
+    for b in range(batch):
+        # pages present at the swap are in the partition (the two later steps may have opened one anywhere)
+        for j in range((int(seq[b]) - after + 15) // 16):
+            assert assign[b] * psz <= bt[b, j] < (assign[b] + 1) * psz
