@@ -334,7 +334,9 @@ def run_ours(args):
     e2e = {"value": world * batch * K / e2e_s, "unit": UNIT, "h2d_bytes_per_step": int(h2d),
            "d2h_bytes_per_step": int(h_hidden.numel() * 2), "ms_per_step": e2e_s / K * 1e3,
            "api": "cc_forward_host (pinned host hidden/block_table/seq_lens/replica_assign in, hidden out; "
-                  "KV pools and weights are device-resident state)"}
+                  "KV pools and weights are device-resident state)",
+           "transfers": "the three tables by copy engine; the hidden rows are read over PCIe by the first kernel and the "
+                        "result rows stored to the pinned buffer by the last epilogue (same bytes, no separate copies)"}
 
     # ---- replica creation: cc_scale_layer (chunked copy on the side stream) -> cc_commit (visible) ----
     copy_ms = []

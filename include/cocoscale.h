@@ -177,10 +177,15 @@ cc_status cc_replica_blob(cc_layer *layer, int replica, const void **blob_dev, s
 cc_status cc_forward(cc_layer *layer, void *hidden_dev, const cc_kv_pages *kv, const int32_t *seq_lens_dev,
                      const int32_t *replica_assign_dev, int batch, void *stream);
 
-/* Same step with HOST buffers for the per-step inputs (pinned memory recommended): copies
- * hidden, block table, seq_lens and replica_assign to library-owned device staging, runs
- * cc_forward, copies hidden back and synchronises `stream`.  The KV pools stay on the device
- * (they are state, like the weights).  block_table_host is [batch][max_blocks_per_seq]. */
+/* Same step with HOST buffers for the per-step inputs: copies block table, seq_lens and
+ * replica_assign to library-owned device staging, runs the step and synchronises `stream`; on
+ * return hidden_host holds the result rows (padding rows untouched).  When hidden_host is pinned
+ * memory mapped into the device's address space (cudaHostAlloc / cudaHostRegister, 16-byte
+ * aligned) the kernels read and write it in place: the first kernel fetches the rows over PCIe
+ * (keeping a device copy for the residual) and the last epilogue stores the result rows to it.
+ * Otherwise hidden is staged through two copies.  Same results bit for bit either way.  The KV
+ * pools stay on the device (they are state, like the weights).  block_table_host is
+ * [batch][max_blocks_per_seq]. */
 cc_status cc_forward_host(cc_layer *layer, void *hidden_host, void *k_pool_dev, void *v_pool_dev,
                           int32_t n_pages, const int32_t *block_table_host, const int32_t *seq_lens_host,
                           const int32_t *replica_assign_host, int batch, void *stream);
@@ -190,7 +195,8 @@ cc_status cc_forward_host(cc_layer *layer, void *hidden_host, void *k_pool_dev, 
  * [cc_forward_launch_count]) receives the device time of kernel i in milliseconds, in launch
  * order: grouping + input norm, QKV GEMM (+RoPE, KV append), attention (+chunk merge), O GEMM
  * (+residual, norm statistics), gate/up GEMM (+norm scale, SwiGLU), down GEMM (+residual, request
- * order).  For per-kernel roofline accounting; not capture-safe. */
+ * order).  For per-kernel roofline accounting; not capture-safe.  hidden_dev may also be the pinned
+ * host buffer of cc_forward_host (its in-place path is then what is timed). */
 cc_status cc_forward_profiled(cc_layer *layer, void *hidden_dev, const cc_kv_pages *kv, const int32_t *seq_lens_dev,
                               const int32_t *replica_assign_dev, int batch, void *stream, float *stage_ms_host);
 

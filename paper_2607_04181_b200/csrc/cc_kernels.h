@@ -42,8 +42,15 @@ struct CcLaunch {
 };
 
 
+// cc_forward_host with a pinned hidden buffer: the prologue reads the rows straight from mapped host memory and
+// leaves a device copy for the O epilogue's residual (null: hidden is device memory, nothing staged).
+struct CcStageOut {
+    __nv_bfloat16* hidden = nullptr;   // [batch][d]
+};
+
 cudaError_t cc_launch_prologue(const int* assign, const int* seq_lens, int batch, const __nv_bfloat16* hidden,
-                               const CcDims& D, const CcLayerTable* tab, const CcWork& W, const CcLaunch& L);
+                               const CcDims& D, const CcLayerTable* tab, const CcWork& W, const CcLaunch& L,
+                               const CcStageOut& so = CcStageOut());
 // which: 0 = QKV, 1 = O, 2 = gate/up, 3 = down
 cudaError_t cc_launch_gemm(int which, const CcDims& D, const CcLayerTable* tab, const CcWork& W, const int* seq_lens,
                            const int* assign, int batch, const CcKv& kv, __nv_bfloat16* hidden, const CcLaunch& L);

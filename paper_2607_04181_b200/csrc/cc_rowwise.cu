@@ -36,28 +36,39 @@ __device__ __forceinline__ void split_hilo(float v0, float v1, uint32_t& hi, uin
 }
 
 // ---------------------------------------------------------------------------------------------
-// a0 + a1 in one kernel, one block per grouped position.
+// a0 + a1 in one kernel, one block per request row.
 // a0: grouping.  Every block repeats it (256 rows: a few ballots), thread b owns row b.  Stable partition
 // by replica, groups start at multiples of 16 rows; page prefix of the attention work
-// split.  Block 0 publishes the tables; each block keeps the one row that lands on its position.
-// a1: x = h * rsqrt(mean(h^2) + eps) * g1  ->  hi/lo operand planes of that row (kept in registers
-// between the two passes).
+// split.  Block 0 publishes the tables; each block learns the grouped position of its own row.
+// a1: x = h * rsqrt(mean(h^2) + eps) * g1  ->  hi/lo operand planes of that row.  The row is requested before
+// the grouping (its address does not depend on it) and stays in registers between the two passes.
 // ---------------------------------------------------------------------------------------------
 constexpr int kNormThreads = 512;
 constexpr int kNormVec = 2;            // uint4 (8 bf16) per thread: hidden <= 8 * 2 * 512 = 8192
 __global__ void __launch_bounds__(kNormThreads) k_prologue(const int* __restrict__ assign, const int* __restrict__ seq_lens,
                                                            int batch, const __nv_bfloat16* __restrict__ hidden, CcDims D,
-                                                           const CcLayerTable* __restrict__ tab, CcWork W) {
+                                                           const CcLayerTable* __restrict__ tab, CcWork W, CcStageOut so) {
     __shared__ int s_wcnt[8][CC_MAXR];     // rows of replica r in warp w
     __shared__ int s_wnch[8];              // KV pages of the rows of warp w
     __shared__ int s_goff[CC_MAXR + 1], s_cnt[CC_MAXR];
-    __shared__ int s_myb;
+    __shared__ int s_mypos, s_myrep;
     __shared__ float red[kNormThreads / 32];
     const int b = threadIdx.x, warp = b >> 5, lane = b & 31;
     const bool pub = blockIdx.x == 0;      // this block writes the tables
     pdl_wait();
     pdl_launch_dependents();
-    if (b == 0) s_myb = -1;
+    if (b == 0) s_mypos = -1;
+    const int my_b = blockIdx.x;
+    const int nchunk = D.d >> 3;
+    uint4 v[kNormVec];
+    {
+        const uint4* row = reinterpret_cast<const uint4*>(hidden + (size_t)my_b * D.d);
+#pragma unroll
+        for (int j = 0; j < kNormVec; ++j) {
+            const int c = threadIdx.x + j * kNormThreads;
+            v[j] = c < nchunk ? row[c] : make_uint4(0, 0, 0, 0);
+        }
+    }
     int rep = -1, pos = -1;
     if (b < 256) {
         uint32_t err = 0;
@@ -103,7 +114,7 @@ __global__ void __launch_bounds__(kNormThreads) k_prologue(const int* __restrict
             for (int w = 0; w < warp; ++w) rank += s_wcnt[w][rep];
             pos = s_goff[rep] + rank;
             if (pub) W.perm[pos] = b;
-            if (pos == (int)blockIdx.x) s_myb = b;
+            if (b == my_b) { s_mypos = pos; s_myrep = rep; }
         }
         // attention work split: pages of the rows in request order (prefix sums); the attention CTAs cut this
         // page axis into equal contiguous ranges -- a function of the batch, never of the replica split
@@ -139,26 +150,18 @@ __global__ void __launch_bounds__(kNormThreads) k_prologue(const int* __restrict
         }
     }
     __syncthreads();
-    const int my_b = s_myb;
-    if (my_b < 0) return;                  // block-uniform: padding position
-    const int mypos = blockIdx.x;
-    int r = 0;
-#pragma unroll
-    for (int i = 1; i < CC_MAXR; ++i)
-        if (s_cnt[i] > 0 && mypos >= s_goff[i]) r = i;
-    const uint4* g = reinterpret_cast<const uint4*>(tab->rep[r].blob + D.off_g1);
-    const uint4* row = reinterpret_cast<const uint4*>(hidden + (size_t)my_b * D.d);
-    const int nchunk = D.d >> 3;
-    uint4 v[kNormVec], gv[kNormVec];
+    const int mypos = s_mypos;
+    if (mypos < 0) return;                 // block-uniform: padding row
+    const uint4* g = reinterpret_cast<const uint4*>(tab->rep[s_myrep].blob + D.off_g1);
+    uint4 gv[kNormVec];
     float ss = 0.f;
 #pragma unroll
     for (int j = 0; j < kNormVec; ++j) {
         const int c = threadIdx.x + j * kNormThreads;
-        v[j] = make_uint4(0, 0, 0, 0);
         gv[j] = make_uint4(0, 0, 0, 0);
         if (c < nchunk) {
-            v[j] = row[c];
             gv[j] = g[c];
+            if (so.hidden != nullptr) reinterpret_cast<uint4*>(so.hidden + (size_t)my_b * D.d)[c] = v[j];
         }
         const uint32_t w[4] = {v[j].x, v[j].y, v[j].z, v[j].w};
 #pragma unroll
@@ -217,8 +220,9 @@ __global__ void __launch_bounds__(256) k_tap(const void* __restrict__ src, int w
 
 // ---- launchers ---------------------------------------------------------------------------------
 cudaError_t cc_launch_prologue(const int* assign, const int* seq_lens, int batch, const __nv_bfloat16* hidden,
-                               const CcDims& D, const CcLayerTable* tab, const CcWork& W, const CcLaunch& L) {
-    return cc_launch_kernel(k_prologue, dim3(D.Mpad), dim3(kNormThreads), 0, L, assign, seq_lens, batch, hidden, D, tab, W);
+                               const CcDims& D, const CcLayerTable* tab, const CcWork& W, const CcLaunch& L,
+                               const CcStageOut& so) {
+    return cc_launch_kernel(k_prologue, dim3(batch), dim3(kNormThreads), 0, L, assign, seq_lens, batch, hidden, D, tab, W, so);
 }
 cudaError_t cc_launch_tap(const void* src, int which, int dim, const CcDims& D, const CcWork& W,
                           float* out_dev, int batch, cudaStream_t st) {

@@ -252,6 +252,39 @@ def test_forward_host_matches_forward():
         assert B.cc_forward_launch_count(S.layer) == len(B.STAGE_NAMES)
 
 
+@pytest.mark.parametrize("pinned", [True, False])
+def test_forward_host_direct_and_staged_paths_match_forward(pinned):
+    """cc_forward_host with pinned buffers lets the kernels read / write the host memory in place; with pageable
+    buffers it stages through copies.  Both: output rows and the KV pools bitwise those of cc_forward; padding
+    rows of the host buffer untouched; repeated calls (the staging is reused) stay identical."""
+    B, DeviceStep, Session = _binding()
+    shape, batch, R = MID, 21, 3
+    w = I.make_weights(shape, 1011)
+    st = I.make_step_inputs(shape, 2011, 3011, batch=batch)
+    st.seq_lens[[3, 17]] = 0                                            # padding rows
+    assign = (np.arange(batch) * 7 % R).astype(np.int32)
+    with Session(shape, w, max_batch=batch) as S:
+        S.scale(R)
+        step = DeviceStep(st, assign)
+        S.forward(step)
+        torch.cuda.synchronize()
+        want, (kw, vw) = step.out_bits(), step.pools_bits()
+        assert np.array_equal(want[[3, 17]], st.hidden[[3, 17]])
+        for rep in range(3):
+            step.reset(st)
+            bufs = [torch.from_numpy(a.copy()) for a in (st.hidden.view(np.int16), st.block_table, st.seq_lens, assign)]
+            if pinned:
+                bufs = [t.pin_memory() for t in bufs]
+            hidden, bt, sl, ra = bufs
+            B.cc_forward_host(S.layer, hidden, step.k_pool, step.v_pool, step.n_pages, bt, sl, ra, batch,
+                              torch.cuda.current_stream())
+            assert B.cc_poll_device_error(S.ctx) == 0
+            assert np.array_equal(hidden.numpy().view(np.uint16), want), f"call {rep}"
+            kp, vp = step.pools_bits()
+            assert np.array_equal(kp, kw) and np.array_equal(vp, vw)
+            assert np.array_equal(bt.numpy(), st.block_table) and np.array_equal(sl.numpy(), st.seq_lens)
+
+
 def test_run_to_run_determinism_and_pdl_off_is_bitwise_the_same():
     """The fixups and merges are finished by whichever CTA arrives last: the result must not depend on that.
     Twenty replays from the same inputs, with and without programmatic dependent launch, give one bit pattern
