@@ -38,8 +38,8 @@ REF_ROWS_PER_STEP = 4       # --impl reference: rows of the batch the oracle com
 CPU_BASELINE_ROWS = 64      # cpu_baseline leg of the default arm: the whole batch ...
 CPU_BASELINE_STEPS = 4      # ... four times (about 10 s of CPU work on 16 cores)
 # dram__bytes_read.sum + dram__bytes_write.sum of the gate/up GEMM (k_gemm<2>) per launch at R = 2, from the
-# ncu --set full capture summarised in profiles/r01k_full_R2.md (470 888 448 + 7 401 984 bytes)
-NCU_TRAFFIC_GATE_UP_R2 = 478290432
+# ncu --set full capture summarised in profiles/r01q_full_R2.md (470 888 448 + 7 641 088 bytes)
+NCU_TRAFFIC_GATE_UP_R2 = 478529536
 FALLBACK_HBM_GBS = 6650.0   # /opt/skills/guides/B200_PROFILING.md, used only if MEASURED_PEAKS.json is absent
 
 
@@ -286,7 +286,7 @@ def run_ours(args):
     roofline = {"bound": "hbm", "kernel": dom, "achieved": round(achieved, 1), "peak": peak, "unit": "GB/s",
                 "frac": round(achieved / peak, 4),
                 "traffic": NCU_TRAFFIC_GATE_UP_R2 if (R == 2 and dom == "gemm_gate_up") else None,
-                "traffic_source": "ncu --set full, profiles/r01k_full_R2.md" if (R == 2 and dom == "gemm_gate_up") else None,
+                "traffic_source": "ncu --set full, profiles/r01q_full_R2.md" if (R == 2 and dom == "gemm_gate_up") else None,
                 "peak_source": peak_src,
                 "kernel_ms": round(dom_ms, 5), "algorithmic_bytes": sb[dom],
                 "how": f"mean of {n_prof} launches, CUDA events around the kernel on its stream (cc_forward_profiled)"}
