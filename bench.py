@@ -335,7 +335,7 @@ def run_ours(args):
            "d2h_bytes_per_step": int(h_hidden.numel() * 2), "ms_per_step": e2e_s / K * 1e3,
            "api": "cc_forward_host (pinned host hidden/block_table/seq_lens/replica_assign in, hidden out; "
                   "KV pools and weights are device-resident state)",
-           "transfers": "the three tables by copy engine; the hidden rows are read over PCIe by the first kernel and the "
+           "transfers": "the three tables in one copy-engine transfer; the hidden rows are read over PCIe by the first kernel and the "
                         "result rows stored to the pinned buffer by the last epilogue (same bytes, no separate copies)"}
 
     # ---- replica creation: cc_scale_layer (chunked copy on the side stream) -> cc_commit (visible) ----

@@ -178,7 +178,8 @@ cc_status cc_forward(cc_layer *layer, void *hidden_dev, const cc_kv_pages *kv, c
                      const int32_t *replica_assign_dev, int batch, void *stream);
 
 /* Same step with HOST buffers for the per-step inputs: copies block table, seq_lens and
- * replica_assign to library-owned device staging, runs the step and synchronises `stream`; on
+ * replica_assign to library-owned device staging (through a pinned mirror, one transfer; the
+ * three buffers may be pageable), runs the step and synchronises `stream`; on
  * return hidden_host holds the result rows (padding rows untouched).  When hidden_host is pinned
  * memory mapped into the device's address space (cudaHostAlloc / cudaHostRegister, 16-byte
  * aligned) the kernels read and write it in place: the first kernel fetches the rows over PCIe

@@ -163,6 +163,7 @@ struct cc_layer {
     int* st_bt = nullptr;
     int* st_sl = nullptr;
     int* st_ra = nullptr;
+    void* st_tbl_host = nullptr;         // pinned mirror of [st_sl | st_ra | st_bt]
     int last_batch = 0;
 };
 
@@ -322,6 +323,17 @@ struct Carver {   // bump allocator over one cudaMalloc
 void destroy_layer_memory(cc_layer* L) {
     cudaFree(L->blob0);
     cudaFree(L->work_base);
+    if (L->st_tbl_host) cudaFreeHost(L->st_tbl_host);
+}
+
+// cc_forward_host: the three per-step tables through the layer's pinned mirror, one host-to-device copy.
+cudaError_t stage_tables(cc_layer* L, const int32_t* bt, const int32_t* sl, const int32_t* ra, int batch, cudaStream_t st) {
+    const size_t mb = (size_t)L->desc.max_batch, bb = (size_t)batch * L->desc.max_blocks_per_seq * 4;
+    uint8_t* h = (uint8_t*)L->st_tbl_host;
+    std::memcpy(h, sl, (size_t)batch * 4);
+    std::memcpy(h + mb * 4, ra, (size_t)batch * 4);
+    std::memcpy(h + mb * 8, bt, bb);
+    return cudaMemcpyAsync(L->st_sl, h, mb * 8 + bb, cudaMemcpyHostToDevice, st);
 }
 
 }  // namespace
@@ -410,13 +422,14 @@ cc_status cc_create_layer(cc_ctx* ctx, const cc_layer_desc* desc, const cc_layer
     const size_t o_attml = ws.take(n_slots * D.Hq * sizeof(float2));
     const size_t o_rope = ws.take((size_t)d.max_position * (D.Dh / 2) * sizeof(float2));
     const size_t o_sth = ws.take((size_t)d.max_batch * D.d * 2);
-    const size_t o_stbt = ws.take((size_t)d.max_batch * d.max_blocks_per_seq * 4);
-    const size_t o_stsl = ws.take((size_t)d.max_batch * 4);
-    const size_t o_stra = ws.take((size_t)d.max_batch * 4);
+    // cc_forward_host's tables as one region [seq_lens | replica_assign | block table]: one copy from a pinned mirror
+    const size_t tbl_bytes = (size_t)d.max_batch * 8 + (size_t)d.max_batch * d.max_blocks_per_seq * 4;
+    const size_t o_tbl = ws.take(tbl_bytes);
     const size_t ws_bytes = ws.take(0);
 
     cudaError_t e = cudaMalloc(&L->blob0, L->blob_bytes);
     if (e == cudaSuccess) e = cudaMalloc(&L->work_base, ws_bytes);
+    if (e == cudaSuccess) e = cudaHostAlloc(&L->st_tbl_host, tbl_bytes, cudaHostAllocDefault);
     if (e == cudaSuccess) e = cudaMemset(L->work_base, 0, ws_bytes);
     if (e == cudaSuccess) e = cudaMemset(L->blob0, 0, L->blob_bytes);
     if (e != cudaSuccess) {
@@ -436,8 +449,8 @@ cc_status cc_create_layer(cc_ctx* ctx, const cc_layer_desc* desc, const cc_layer
     W.att_o = (float*)(wb + o_atto); W.att_ml = (float2*)(wb + o_attml);
     W.rope_cs = (const float2*)(wb + o_rope);
     W.err = ctx->err_dev;
-    L->st_hidden = (__nv_bfloat16*)(wb + o_sth); L->st_bt = (int*)(wb + o_stbt);
-    L->st_sl = (int*)(wb + o_stsl); L->st_ra = (int*)(wb + o_stra);
+    L->st_hidden = (__nv_bfloat16*)(wb + o_sth);
+    L->st_sl = (int*)(wb + o_tbl); L->st_ra = L->st_sl + d.max_batch; L->st_bt = L->st_ra + d.max_batch;
 
     // RoPE table in fp64 on the host: angle = p * base^(-2i/Dh)  (rotate-half pairing, reading 4)
     {
@@ -706,15 +719,13 @@ cc_status cc_forward_host(cc_layer* L, void* hidden_host, void* k_pool_dev, void
     if (batch < 1 || batch > L->desc.max_batch) return fail(CC_ERR_INVALID, "batch %d outside 1..max_batch=%d", batch, L->desc.max_batch);
     cudaStream_t st = (cudaStream_t)stream;
     CC_CUDA(cudaSetDevice(L->ctx->device));
-    const size_t hb = (size_t)batch * L->D.d * 2, bb = (size_t)batch * L->desc.max_blocks_per_seq * 4;
+    const size_t hb = (size_t)batch * L->D.d * 2;
     // Pinned hidden buffer: the kernels read and write it in place (measured: 280 us per cfg2 step against 300 us
     // with the two 512 KB copies; reading the three small tables in place as well costs more than their copies).
     if (void* alias = mapped_host(hidden_host)) {
         if (!k_pool_dev || !v_pool_dev || n_pages < 1) return fail(CC_ERR_INVALID, "bad KV pool arguments");
         if (((uintptr_t)k_pool_dev | (uintptr_t)v_pool_dev) & 15) return fail(CC_ERR_INVALID, "KV pools must be 16-byte aligned");
-        CC_CUDA(cudaMemcpyAsync(L->st_bt, block_table_host, bb, cudaMemcpyHostToDevice, st));
-        CC_CUDA(cudaMemcpyAsync(L->st_sl, seq_lens_host, (size_t)batch * 4, cudaMemcpyHostToDevice, st));
-        CC_CUDA(cudaMemcpyAsync(L->st_ra, replica_assign_host, (size_t)batch * 4, cudaMemcpyHostToDevice, st));
+        CC_CUDA(stage_tables(L, block_table_host, seq_lens_host, replica_assign_host, batch, st));
         CcKv k{(__nv_bfloat16*)k_pool_dev, (__nv_bfloat16*)v_pool_dev, L->st_bt, n_pages};
         cudaError_t e = enqueue_forward(L, L->st_hidden, k, L->st_sl, L->st_ra, batch, st, nullptr, (__nv_bfloat16*)alias);
         if (e != cudaSuccess) return fail(CC_ERR_CUDA, "cc_forward_host launch: %s", cudaGetErrorString(e));
@@ -723,9 +734,7 @@ cc_status cc_forward_host(cc_layer* L, void* hidden_host, void* k_pool_dev, void
         return CC_OK;
     }
     CC_CUDA(cudaMemcpyAsync(L->st_hidden, hidden_host, hb, cudaMemcpyHostToDevice, st));
-    CC_CUDA(cudaMemcpyAsync(L->st_bt, block_table_host, bb, cudaMemcpyHostToDevice, st));
-    CC_CUDA(cudaMemcpyAsync(L->st_sl, seq_lens_host, (size_t)batch * 4, cudaMemcpyHostToDevice, st));
-    CC_CUDA(cudaMemcpyAsync(L->st_ra, replica_assign_host, (size_t)batch * 4, cudaMemcpyHostToDevice, st));
+    CC_CUDA(stage_tables(L, block_table_host, seq_lens_host, replica_assign_host, batch, st));
     cc_kv_pages kv{k_pool_dev, v_pool_dev, L->st_bt, n_pages};
     cc_status s = cc_forward(L, L->st_hidden, &kv, L->st_sl, L->st_ra, batch, stream);
     if (s != CC_OK) return s;
