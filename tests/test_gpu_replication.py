@@ -283,6 +283,14 @@ def test_forward_host_direct_and_staged_paths_match_forward(pinned):
             kp, vp = step.pools_bits()
             assert np.array_equal(kp, kw) and np.array_equal(vp, vw)
             assert np.array_equal(bt.numpy(), st.block_table) and np.array_equal(sl.numpy(), st.seq_lens)
+        if pinned:
+            # the kernel-by-kernel timing call takes the same pinned buffer (tables on the device)
+            step.reset(st)
+            hidden = torch.from_numpy(st.hidden.view(np.int16).copy()).pin_memory()
+            ms = B.cc_forward_profiled(S.layer, hidden, step.k_pool, step.v_pool, step.block_table, step.n_pages,
+                                       step.seq_lens, step.assign, batch, torch.cuda.current_stream())
+            assert len(ms) == len(B.STAGE_NAMES) and (ms > 0).all()
+            assert np.array_equal(hidden.numpy().view(np.uint16), want)
 
 
 def test_run_to_run_determinism_and_pdl_off_is_bitwise_the_same():
