@@ -45,3 +45,34 @@ def test_max_batch_256_rows_uneven_groups_and_empty_contexts():
                                                              seeds=(1202, 2202, 3202))
     check_against_oracle(shape, st, ref, out, kp, vp, gtaps, assign, 4)
     check_grouping(grouping, assign, st.seq_lens, 4)
+
+
+@pytest.mark.parametrize("seed", range(10))
+def test_random_shapes_batches_and_assignments(seed):
+    """Seeded random layers inside what cc_create_layer accepts (hidden a multiple of 64, FFN of 8, 1/2/4/8 kv
+    heads, GQA groups 1..8, head_dim 64/128), random batch, contexts, replica counts and assignments (some replicas
+    left empty, some rows padding): every stage tap, the output and the appended KV against the oracle."""
+    rng = np.random.default_rng(9000 + seed)
+    dh = int(rng.choice([64, 128]))
+    hkv = int(rng.choice([1, 2, 4, 8]))
+    g = int(rng.integers(1, 9))
+    hidden = 64 * int(rng.integers(2, 17))
+    ffn = 8 * int(rng.integers(8, 260))
+    batch = int(rng.integers(1, 49))
+    R = int(rng.integers(1, 5))
+    lo = int(rng.integers(0, 30))
+    hi = lo + int(rng.integers(1, 400))
+    shape = I.LayerShape(f"rnd{seed}", hidden, hkv * g, hkv, dh, ffn, 1e-5, float(rng.choice([10000.0, 500000.0])), batch, lo, hi)
+    assign = rng.integers(0, R, batch).astype(np.int32)
+    if R > 1 and seed % 2:
+        assign[assign == R - 1] = 0                                   # an active replica that serves no row
+    seq = None
+    if batch > 3 and seed % 3 == 0:
+        ctx = I.draw_contexts(shape, 3300 + seed, batch)
+        seq = (ctx + 1).astype(np.int32)
+        seq[rng.integers(0, batch, 2)] = 0                            # padding rows
+    st, ref, out, kp, vp, gtaps, grouping, assign = run_case(shape, batch, R, assign=assign, seeds=(1300 + seed, 2300 + seed, 3300 + seed),
+                                                             seq_override=seq)
+    rel = check_against_oracle(shape, st, ref, out, kp, vp, gtaps, assign, R)
+    check_grouping(grouping, assign, st.seq_lens, R)
+    print(shape, "R", R, {k: round(v, 5) for k, v in rel.items()})
