@@ -76,3 +76,8 @@ def test_random_shapes_batches_and_assignments(seed):
     rel = check_against_oracle(shape, st, ref, out, kp, vp, gtaps, assign, R)
     check_grouping(grouping, assign, st.seq_lens, R)
     print(shape, "R", R, {k: round(v, 5) for k, v in rel.items()})
+    if R > 1:
+        # the same batch through one replica gives the same bits (outputs and appended KV)
+        _, _, out1, kp1, vp1, _, _, _ = run_case(shape, batch, 1, assign=np.zeros(batch, np.int32),
+                                                 seeds=(1300 + seed, 2300 + seed, 3300 + seed), seq_override=seq, taps=False)
+        assert np.array_equal(out1, out) and np.array_equal(kp1, kp) and np.array_equal(vp1, vp)
