@@ -433,10 +433,11 @@ cc_status cc_create_layer(cc_ctx* ctx, const cc_layer_desc* desc, const cc_layer
     if (e == cudaSuccess) e = cudaMemset(L->work_base, 0, ws_bytes);
     if (e == cudaSuccess) e = cudaMemset(L->blob0, 0, L->blob_bytes);
     if (e != cudaSuccess) {
+        const size_t blob_bytes = L->blob_bytes;
         destroy_layer_memory(L);
         delete L;
         cudaGetLastError();
-        return fail(CC_ERR_CUDA, "device allocation of %zu + %zu bytes failed: %s", L->blob_bytes, ws_bytes, cudaGetErrorString(e));
+        return fail(CC_ERR_CUDA, "device allocation of %zu + %zu bytes failed: %s", blob_bytes, ws_bytes, cudaGetErrorString(e));
     }
     uint8_t* wb = L->work_base;
     W.sched = (CcSched*)(wb + o_sched); W.perm = (int*)(wb + o_perm); W.pg_prefix = (int*)(wb + o_pgpre); W.pos_of = (int*)(wb + o_posof);
