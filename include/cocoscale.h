@@ -276,6 +276,31 @@ int cc_ctl_candidate_count(int L, int P_max);                         /* L * P_m
 cc_status cc_ctl_decide(const cc_ctl_params *p, int N_cur, int P_cur, double latency, double *cold_capacity,
                         int *N_new, int *P_new, cc_ctl_action *action);
 
+/* Algorithm 1, initial global placement: instances in descending Priority = load - capacity
+ * (Eq. 11) each take, among the (N, P) with 1 <= N <= L, 2 <= P <= P_max whose per-device memory C_mem(N, P)
+ * (Eq. 1) fits on at least P - 1 devices of the pool (Load < tau_idle, not yet taken), the one of largest S(N, P)
+ * (Eq. 7 with p->beta; ties: fewer devices, then fewer layers) and the P - 1 fitting devices of largest free
+ * memory (ties: lower index).  Only P_max and beta of `p` are used.  `out` has room for n_inst entries;
+ * instances that fit nowhere get none.  On one GPU there is nothing to place: this is the paper's bootstrap
+ * step stated for completeness of the controller. */
+typedef struct {
+    int32_t L, bs, l, d_hidden;   /* layers, batch size, sequence length, hidden size (Eq. 1)            */
+    double kappa;                 /* bytes per element                                                   */
+    double load, capacity;        /* current load and sustainable load of the instance (Eq. 11)          */
+} cc_ctl_instance;
+typedef struct {
+    double load;                  /* compute utilisation of the device, same unit as tau_idle            */
+    double free_mem_bytes;
+} cc_ctl_device;
+typedef struct {
+    int32_t instance, N, P;
+    int32_t devices[CC_MAX_REPLICAS - 1];   /* P - 1 device indices, then -1                              */
+    double speedup;
+} cc_ctl_placement;
+cc_status cc_ctl_place(const cc_ctl_params *p, const cc_ctl_instance *instances, int n_instances,
+                       const cc_ctl_device *devices, int n_devices, double tau_idle, cc_ctl_placement *out,
+                       int *n_out);
+
 /* ---- stage taps (tests only; reads the workspace left by the last cc_forward) ---------------- */
 typedef enum {
     CC_TAP_X = 0,   /* [batch][hidden]      input RMSNorm output (GEMM operand: bf16 hi + lo)   */

@@ -55,3 +55,31 @@ def decide(L, P_max, slo, delta, beta, c_dev, c_copy, N_cur, P_cur, latency, col
         if d_res <= 0 or cold >= d_res:
             return "updated", N, P, cold - d_res
     return ("instance_scale" if latency > slo else "none"), N_cur, P_cur, cold
+
+
+def place(P_max, beta, instances, devices, tau_idle):
+    """Algorithm 1 written as list operations.  instances: dicts with L, bs, l, d, kappa, load,
+    capacity; devices: dicts with load, free_mem.  -> [(instance index, N, P, [device indices], S)].
+    Readings: equal priorities keep their input order; speed-ups equal to 1e-12 relative are ties, won
+    by fewer devices, then fewer layers; the devices are those of largest free memory that fit, lower index first."""
+    pool = [i for i, d in enumerate(devices) if d["load"] < tau_idle]                          # line 3
+    order = sorted(range(len(instances)), key=lambda k: -(instances[k]["load"] - instances[k]["capacity"]))   # lines 4-7 (stable)
+    plan = []
+    for k in order:
+        I = instances[k]
+        feasible = []
+        for N in range(1, I["L"] + 1):
+            for P in range(2, P_max + 1):
+                need = mem_bytes(N, P, I["bs"], I["l"], I["d"], I["kappa"])                  # Eq. 1
+                fits = [i for i in pool if devices[i]["free_mem"] >= need]
+                if len(fits) >= P - 1:
+                    fits.sort(key=lambda i: (-devices[i]["free_mem"], i))
+                    feasible.append((speedup(I["L"], N, P, beta[P]), N, P, fits[:P - 1]))
+        if not feasible:
+            continue
+        top = max(f[0] for f in feasible)
+        ties = [f for f in feasible if abs(f[0] - top) <= 1e-12 * top]
+        s, N, P, devs = min(ties, key=lambda f: (f[2], f[1]))
+        plan.append((k, N, P, devs, s))
+        pool = [i for i in pool if i not in devs]                                            # line 21
+    return plan

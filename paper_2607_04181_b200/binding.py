@@ -33,7 +33,7 @@ EXPORTS = (
     "cc_slotalloc_create", "cc_slotalloc_destroy", "cc_slotalloc_donate", "cc_slotalloc_reclaim",
     "cc_slotalloc_alloc", "cc_slotalloc_free", "cc_slotalloc_free_bytes", "cc_last_error", "cc_version",
     "cc_ctl_mem_bytes", "cc_ctl_flops", "cc_ctl_comm_seconds", "cc_ctl_speedup", "cc_ctl_speedup_vec", "cc_ctl_distance",
-    "cc_ctl_candidate_count", "cc_ctl_decide",
+    "cc_ctl_candidate_count", "cc_ctl_decide", "cc_ctl_place",
 )
 
 
@@ -306,6 +306,31 @@ def cc_ctl_decide(params: "cc_ctl_params", N_cur: int, P_cur: int, latency: floa
     _check(_lib.cc_ctl_decide(C.byref(params), C.c_int(N_cur), C.c_int(P_cur), C.c_double(latency), C.byref(cold),
                               C.byref(n), C.byref(p_), C.byref(act)))
     return act.value, n.value, p_.value, cold.value
+
+
+class cc_ctl_instance(C.Structure):
+    _fields_ = [("L", C.c_int32), ("bs", C.c_int32), ("l", C.c_int32), ("d_hidden", C.c_int32), ("kappa", C.c_double),
+                ("load", C.c_double), ("capacity", C.c_double)]
+
+
+class cc_ctl_device(C.Structure):
+    _fields_ = [("load", C.c_double), ("free_mem_bytes", C.c_double)]
+
+
+class cc_ctl_placement(C.Structure):
+    _fields_ = [("instance", C.c_int32), ("N", C.c_int32), ("P", C.c_int32), ("devices", C.c_int32 * (CC_MAX_REPLICAS - 1)),
+                ("speedup", C.c_double)]
+
+
+def cc_ctl_place(params: "cc_ctl_params", instances: list, devices: list, tau_idle: float) -> list:
+    """Algorithm 1.  instances: cc_ctl_instance, devices: cc_ctl_device -> [(instance, N, P, [devices], speedup)]"""
+    ia = (cc_ctl_instance * max(len(instances), 1))(*instances)
+    da = (cc_ctl_device * max(len(devices), 1))(*devices)
+    out = (cc_ctl_placement * max(len(instances), 1))()
+    n = C.c_int(0)
+    _check(_lib.cc_ctl_place(C.byref(params), ia, C.c_int(len(instances)), da, C.c_int(len(devices)), C.c_double(tau_idle),
+                             out, C.byref(n)))
+    return [(o.instance, o.N, o.P, [d for d in o.devices if d >= 0], o.speedup) for o in out[:n.value]]
 
 
 # ---- stage taps (tests) ------------------------------------------------------------------------

@@ -1,6 +1,6 @@
 // cc_control.cu -- host-only: the paper's cost / speed-up model and one decision of its unified layer-wise
 // scaling loop.  PAPER.md:151-217 (section 4.2, Eq. 1-10), PAPER.md:290-353 (section
-// 4.4, Algorithm 2).  No GPU work: the hot path takes `replica_assign` and the replica counts from its caller;
+// 4.4, Algorithm 2), PAPER.md:219-288 (section 4.3, Algorithm 1).  No GPU work: the hot path takes `replica_assign` and the replica counts from its caller;
 // this is the piece that would choose them.  Readings of what the paper leaves open: DESIGN.md section 7c.
 #include "../../include/cocoscale.h"
 
@@ -90,6 +90,60 @@ cc_status cc_ctl_decide(const cc_ctl_params* p, int N_cur, int P_cur, double lat
         }
     }
     if (latency > p->slo) *action = CC_CTL_INSTANCE_SCALE;                                    // lines 17-19
+    return CC_OK;
+}
+
+// Algorithm 1: initial global placement, a priority-greedy pass over the instances.
+// Line 3: the pool is the devices with Load < tau_idle.  Lines 4-7: instances by descending Priority = load -
+// capacity (Eq. 11; ties: lower index first).  Lines 10-17: every (N, P), 1 <= N <= L, 2 <= P <= P_max, whose
+// per-device memory C_mem(N, P) (Eq. 1) fits on at least P - 1 pool devices is feasible.  Line 19: the feasible
+// candidate of largest S(N, P) wins (ties: fewer devices, then fewer layers); its devices are the P - 1 of largest
+// free memory among those that fit (ties: lower index) and leave the pool (line 21).
+cc_status cc_ctl_place(const cc_ctl_params* p, const cc_ctl_instance* inst, int n_inst, const cc_ctl_device* dev, int n_dev,
+                       double tau_idle, cc_ctl_placement* out, int* n_out) {
+    if (!p || !inst || !dev || !out || !n_out || n_inst < 0 || n_dev < 0 || p->P_max < 1 || p->P_max > CC_MAX_REPLICAS)
+        return CC_ERR_INVALID;
+    for (int k = 0; k < n_inst; ++k)
+        if (inst[k].L < 1 || inst[k].bs < 1 || inst[k].l < 0 || inst[k].d_hidden < 1 || !(inst[k].kappa > 0.0)) return CC_ERR_INVALID;
+    std::vector<char> in_pool((size_t)n_dev);
+    for (int d = 0; d < n_dev; ++d) in_pool[d] = dev[d].load < tau_idle;                      // line 3
+    std::vector<int> order((size_t)n_inst);
+    for (int k = 0; k < n_inst; ++k) order[k] = k;
+    std::stable_sort(order.begin(), order.end(), [&](int a, int b) {                          // lines 4-7
+        return inst[a].load - inst[a].capacity > inst[b].load - inst[b].capacity;
+    });
+    int n = 0;
+    for (int k : order) {                                                                     // line 9
+        const cc_ctl_instance& I = inst[k];
+        double best_s = 0.0;
+        int best_N = 0, best_P = 0;
+        for (int N = 1; N <= I.L; ++N)
+            for (int P = 2; P <= p->P_max; ++P) {                                             // line 10
+                const double need = cc_ctl_mem_bytes(N, P, I.bs, I.l, I.d_hidden, I.kappa);  // line 11
+                int fit = 0;
+                for (int d = 0; d < n_dev; ++d) fit += in_pool[d] && dev[d].free_mem_bytes >= need;   // line 12
+                if (fit < P - 1) continue;                                                    // line 13
+                const double s = cc_ctl_speedup(I.L, N, P, p->beta[P]);
+                // speed-ups that agree to 1e-12 are a tie (N (1 - 1/P) takes the same value for many pairs when beta = 0)
+                const bool tie = best_P != 0 && std::fabs(s - best_s) <= 1e-12 * best_s;
+                if (best_P == 0 || (!tie && s > best_s) || (tie && (P < best_P || (P == best_P && N < best_N)))) {
+                    best_s = s; best_N = N; best_P = P;                                       // line 19
+                }
+            }
+        if (best_P == 0) continue;                                                            // line 18
+        const double need = cc_ctl_mem_bytes(best_N, best_P, I.bs, I.l, I.d_hidden, I.kappa);
+        cc_ctl_placement& pl = out[n++];
+        pl.instance = k; pl.N = best_N; pl.P = best_P; pl.speedup = best_s;
+        for (int j = 0; j < CC_MAX_REPLICAS - 1; ++j) pl.devices[j] = -1;
+        for (int j = 0; j < best_P - 1; ++j) {                                                // line 14, largest idle memory first
+            int pick = -1;
+            for (int d = 0; d < n_dev; ++d)
+                if (in_pool[d] && dev[d].free_mem_bytes >= need && (pick < 0 || dev[d].free_mem_bytes > dev[pick].free_mem_bytes)) pick = d;
+            pl.devices[j] = pick;
+            in_pool[pick] = 0;                                                                // line 21
+        }
+    }
+    *n_out = n;
     return CC_OK;
 }
 

@@ -82,3 +82,98 @@ def test_decisions_scale_down_none_and_instance_scale():
     assert act == B.CC_CTL_UPDATED and cold >= 0.0 and B.cc_ctl_speedup(64, n1, p1, 0.0) >= B.cc_ctl_speedup(64, 32, 4, 0.0) * 0.5
     act, n1, p1, cold = B.cc_ctl_decide(p, 64, 4, p.slo * 1.5, 10.0)                 # already at the model's limit
     assert act == B.CC_CTL_INSTANCE_SCALE and (n1, p1) == (64, 4) and cold == 10.0
+
+
+# ---- Algorithm 1: initial global placement ------------------------------------------------
+def _inst(L, bs, l, d, kappa, load, cap):
+    return B.cc_ctl_instance(L, bs, l, d, kappa, load, cap), dict(L=L, bs=bs, l=l, d=d, kappa=kappa, load=load, capacity=cap)
+
+
+def _random_cluster(rng):
+    n_inst, n_dev = int(rng.integers(1, 6)), int(rng.integers(0, 9))
+    insts = [_inst(int(rng.integers(2, 20)), int(rng.integers(1, 65)), int(rng.integers(1, 4097)), 64 * int(rng.integers(1, 80)),
+                   float(rng.choice([1.0, 2.0])), float(rng.uniform(0, 50)), float(rng.uniform(0, 50))) for _ in range(n_inst)]
+    per_layer = max(i[1]["kappa"] * 12 * i[1]["d"] ** 2 for i in insts)
+    devs = [(float(rng.uniform(0, 1)), float(rng.uniform(0, 12) * per_layer)) for _ in range(n_dev)]
+    return insts, devs
+
+
+def test_placement_matches_the_plain_restatement_on_random_clusters():
+    rng = np.random.default_rng(23)
+    placed = 0
+    for trial in range(200):
+        insts, devs = _random_cluster(rng)
+        P_max = int(rng.integers(2, 5))
+        beta = [0.0, 0.0] + (sorted(rng.uniform(0, 0.05, 3).tolist()) if trial % 3 else [0.0, 0.0, 0.0])   # beta = 0: many exact ties
+        p = _params(P_max=P_max, beta=beta)
+        tau = float(rng.uniform(0.3, 0.9))
+        got = B.cc_ctl_place(p, [i[0] for i in insts], [B.cc_ctl_device(a, m) for a, m in devs], tau)
+        want = O.place(P_max, beta, [i[1] for i in insts], [dict(load=a, free_mem=m) for a, m in devs], tau)
+        assert [(g[0], g[1], g[2], g[3]) for g in got] == [(w[0], w[1], w[2], w[3]) for w in want], trial
+        for g, w in zip(got, want):
+            assert g[4] == pytest.approx(w[4], rel=1e-12)
+        # invariants that hold whatever the tie rules: a device serves one instance, was idle enough and large enough;
+        # instances appear in descending priority; P - 1 devices each
+        used = [d for g in got for d in g[3]]
+        assert len(used) == len(set(used))
+        prio = [insts[g[0]][1]["load"] - insts[g[0]][1]["capacity"] for g in got]
+        assert all(a >= b for a, b in zip(prio, prio[1:]))
+        for k, N, P, ds, s in got:
+            I = insts[k][1]
+            need = O.mem_bytes(N, P, I["bs"], I["l"], I["d"], I["kappa"])
+            assert len(ds) == P - 1 and 1 <= N <= I["L"] and 2 <= P <= P_max
+            assert all(devs[d][0] < tau and devs[d][1] >= need for d in ds)
+        placed += len(got)
+    assert placed > 100
+
+
+def test_placement_is_the_best_feasible_choice_for_the_first_instance():
+    """Brute force over every (N, P) and every device subset for the highest-priority instance: no feasible choice
+    has a larger speed-up than the one Algorithm 1 returns (the subset search collapses)."""
+    import itertools
+    rng = np.random.default_rng(29)
+    checked = 0
+    for trial in range(60):
+        insts, devs = _random_cluster(rng)
+        if len(devs) > 6:
+            devs = devs[:6]
+        beta = [0.0, 0.0] + sorted(rng.uniform(0, 0.05, 3).tolist())
+        p = _params(P_max=4, beta=beta)
+        tau = 0.7                                                                   # PAPER.md:225: tau_idle = 70 %
+        got = B.cc_ctl_place(p, [i[0] for i in insts], [B.cc_ctl_device(a, m) for a, m in devs], tau)
+        first = max(range(len(insts)), key=lambda k: (insts[k][1]["load"] - insts[k][1]["capacity"], -k))
+        I = insts[first][1]
+        pool = [i for i, (a, m) in enumerate(devs) if a < tau]
+        best = 0.0
+        for N in range(1, I["L"] + 1):
+            for P in range(2, 5):
+                need = O.mem_bytes(N, P, I["bs"], I["l"], I["d"], I["kappa"])
+                for sub in itertools.combinations(pool, P - 1):
+                    if all(devs[i][1] >= need for i in sub):
+                        best = max(best, O.speedup(I["L"], N, P, beta[P]))
+                        break
+        mine = [g for g in got if g[0] == first]
+        if best == 0.0:
+            assert not mine
+        else:
+            assert mine and got[0][0] == first and mine[0][4] == pytest.approx(best, rel=1e-12)
+            checked += 1
+    assert checked > 15
+
+
+def test_placement_hand_cases():
+    p = _params(P_max=4, beta=(0, 0, 0, 0, 0))
+    d, bs, l = 1024, 8, 128
+    per_layer = 2.0 * (12 * d * d + bs / 2 * l * d)                                 # Eq. 1 at N = 1, P = 2
+    hot, hot_d = _inst(8, bs, l, d, 2.0, 10.0, 2.0)
+    cold, cold_d = _inst(8, bs, l, d, 2.0, 3.0, 2.0)
+    # one idle device with room for exactly three layers at P = 2; a busy one (Load >= tau) with plenty of room
+    devs = [B.cc_ctl_device(0.2, 3.0 * per_layer), B.cc_ctl_device(0.95, 100 * per_layer)]
+    got = B.cc_ctl_place(p, [cold, hot], devs, 0.7)
+    assert got == [(1, 3, 2, [0], pytest.approx(1.0 / (1 - 3 / 8 + 3 / 16)))]     # the hot instance takes it; nothing left for the other
+    # nobody idle: nothing placed
+    assert B.cc_ctl_place(p, [hot], [B.cc_ctl_device(0.9, 100 * per_layer)], 0.7) == []
+    # three roomy idle devices, beta = 0: all layers at P = 4 (Amdahl's limit 4x), devices by free memory
+    devs = [B.cc_ctl_device(0.1, 50 * per_layer), B.cc_ctl_device(0.1, 70 * per_layer), B.cc_ctl_device(0.1, 60 * per_layer)]
+    got = B.cc_ctl_place(p, [hot], devs, 0.7)
+    assert got == [(0, 8, 4, [1, 2, 0], pytest.approx(4.0))]
