@@ -301,6 +301,18 @@ cc_status cc_ctl_place(const cc_ctl_params *p, const cc_ctl_instance *instances,
                        const cc_ctl_device *devices, int n_devices, double tau_idle, cc_ctl_placement *out,
                        int *n_out);
 
+/* ---- timeline of a tracing build (measurement aid) ---------------------------------------------
+ * A library built with -DCC_TRACE (python -m paper_2607_04181_b200.build --trace) records, for every kernel of
+ * cc_forward and every trace point in it, the earliest and latest %globaltimer value (ns) over the CTAs that
+ * passed the point.  out_host (may be NULL): uint64 [16][8][2] = [kernel][point][min, max]; kernel 0 = prologue
+ * (points: entry, dependency wait done, end), 1 = attention (entry, dependency wait done, consumers saw the end),
+ * 2..5 = QKV / O / gate-up / down GEMM (entry, dependency wait done, producer issued all, mainloop drained and
+ * partials stored, first fixup wait done, end); 8..11 = min / max duration of a CTA's first ([0]) and second ([1])
+ * stream-K fixup pass of those GEMMs, 12..15 = [0..1][max] number of such passes, [2..3][max] their summed
+ * duration.  reset != 0 re-arms the buffer after the read.  Synchronises the device.  CC_ERR_STATE in a product
+ * build (the points compile to nothing there).  Driver: python -m paper_2607_04181_b200.timeline. */
+cc_status cc_debug_trace(cc_ctx *ctx, uint64_t *out_host, int reset);
+
 /* ---- stage taps (tests only; reads the workspace left by the last cc_forward) ---------------- */
 typedef enum {
     CC_TAP_X = 0,   /* [batch][hidden]      input RMSNorm output (GEMM operand: bf16 hi + lo)   */

@@ -29,7 +29,7 @@ EXPORTS = (
     "cc_ctx_create", "cc_ctx_destroy", "cc_ctx_donate", "cc_ctx_reclaim", "cc_ctx_set_copy_chunk",
     "cc_ctx_set_pdl", "cc_poll_device_error", "cc_create_layer", "cc_destroy_layer", "cc_layer_blob_bytes",
     "cc_scale_layer", "cc_commit", "cc_release_replica", "cc_query", "cc_replica_blob", "cc_forward",
-    "cc_forward_host", "cc_forward_profiled", "cc_forward_launch_count", "cc_replica_copy", "cc_kv_plan_migration", "cc_kv_plan_catchup", "cc_kv_migrate", "cc_debug_tap", "cc_debug_grouping",
+    "cc_forward_host", "cc_forward_profiled", "cc_forward_launch_count", "cc_replica_copy", "cc_kv_plan_migration", "cc_kv_plan_catchup", "cc_kv_migrate", "cc_debug_tap", "cc_debug_grouping", "cc_debug_trace",
     "cc_slotalloc_create", "cc_slotalloc_destroy", "cc_slotalloc_donate", "cc_slotalloc_reclaim",
     "cc_slotalloc_alloc", "cc_slotalloc_free", "cc_slotalloc_free_bytes", "cc_last_error", "cc_version",
     "cc_ctl_mem_bytes", "cc_ctl_flops", "cc_ctl_comm_seconds", "cc_ctl_speedup", "cc_ctl_speedup_vec", "cc_ctl_distance",
@@ -58,11 +58,14 @@ class cc_kv_pages(C.Structure):
     _fields_ = [("k_pool", C.c_void_p), ("v_pool", C.c_void_p), ("block_table", C.c_void_p), ("n_pages", C.c_int32)]
 
 
+_TRACE = os.environ.get("COCOSCALE_TRACE", "0") not in ("", "0")   # load the tracing build (timeline.py sets it)
+
+
 def _load() -> C.CDLL:
-    path = _build.LIB
-    if _build.needs_build():
+    path = _build.LIB_TRACE if _TRACE else _build.LIB
+    if _build.needs_build(_TRACE):
         try:
-            _build.build()
+            _build.build(trace=_TRACE)
         except Exception as e:  # no nvcc and no prebuilt library: fail loudly, never fall back
             if not os.path.exists(path):
                 raise ImportError(f"libcocoscale.so is missing and could not be built: {e}") from e
@@ -80,7 +83,7 @@ _lib.cc_slotalloc_destroy.restype = None
 
 
 def library_path() -> str:
-    return _build.LIB
+    return _build.LIB_TRACE if _TRACE else _build.LIB
 
 
 def _ptr(x) -> C.c_void_p:
@@ -331,6 +334,14 @@ def cc_ctl_place(params: "cc_ctl_params", instances: list, devices: list, tau_id
     _check(_lib.cc_ctl_place(C.byref(params), ia, C.c_int(len(instances)), da, C.c_int(len(devices)), C.c_double(tau_idle),
                              out, C.byref(n)))
     return [(o.instance, o.N, o.P, [d for d in o.devices if d >= 0], o.speedup) for o in out[:n.value]]
+
+
+# ---- timeline of a tracing build -----------------------------------------------------------------
+def cc_debug_trace(ctx, reset: bool = True):
+    """-> uint64 [16][8][2] (kernel, point, min / max of %globaltimer); CcError(CC_ERR_STATE) in a product build."""
+    out = np.zeros((16, 8, 2), dtype=np.uint64)
+    _check(_lib.cc_debug_trace(ctx, _ptr(out), C.c_int(1 if reset else 0)))
+    return out
 
 
 # ---- stage taps (tests) ------------------------------------------------------------------------

@@ -1,6 +1,8 @@
 """Builds libcocoscale.so (the C-ABI CUDA library) in-tree with nvcc for sm_100a.
 
-    python -m paper_2607_04181_b200.build [--force]
+    python -m paper_2607_04181_b200.build [--force] [-v] [--trace]
+
+--trace builds libcocoscale_trace.so, the same sources with -DCC_TRACE (globaltimer trace points, timeline.py).
 
 nvcc cross-compiles without a GPU.  The library lands next to this file so that it travels with
 the repository snapshot to the GPU box; it is git-ignored.
@@ -27,22 +29,27 @@ def _nvcc() -> str:
     return "nvcc"
 
 
-def needs_build() -> bool:
-    if not os.path.exists(LIB):
+LIB_TRACE = os.path.join(HERE, "libcocoscale_trace.so")   # the same sources with -DCC_TRACE (timeline.py)
+
+
+def needs_build(trace: bool = False) -> bool:
+    lib = LIB_TRACE if trace else LIB
+    if not os.path.exists(lib):
         return True
-    t = os.path.getmtime(LIB)
+    t = os.path.getmtime(lib)
     deps = [os.path.join(CSRC, f) for f in SOURCES + HEADERS] + [os.path.abspath(__file__)]
     return any(os.path.getmtime(d) > t for d in deps)
 
 
-def build(force: bool = False, verbose: bool = False) -> str:
-    if not force and not needs_build():
-        return LIB
+def build(force: bool = False, verbose: bool = False, trace: bool = False) -> str:
+    lib = LIB_TRACE if trace else LIB
+    if not force and not needs_build(trace):
+        return lib
     objs = []
     procs = []
     for src in SOURCES:
-        obj = os.path.join(CSRC, src.replace(".cu", ".o"))
-        cmd = [_nvcc(), *NVCC_FLAGS, "-c", os.path.join(CSRC, src), "-o", obj]
+        obj = os.path.join(CSRC, src.replace(".cu", ".trace.o" if trace else ".o"))
+        cmd = [_nvcc(), *NVCC_FLAGS, *(["-DCC_TRACE"] if trace else []), "-c", os.path.join(CSRC, src), "-o", obj]
         if verbose:
             cmd.insert(1, "-Xptxas=-v")
         procs.append((src, subprocess.Popen(cmd, stdout=subprocess.PIPE, stderr=subprocess.STDOUT, text=True)))
@@ -53,16 +60,16 @@ def build(force: bool = False, verbose: bool = False) -> str:
             print(out)
         if p.returncode:
             raise RuntimeError(f"nvcc failed on {src}:\n{out}")
-    tmp = LIB + ".tmp"
+    tmp = lib + ".tmp"
     link = [_nvcc(), "-shared", "-o", tmp, *objs, "-cudart", "static", "-Xlinker", "--no-undefined", "-lpthread", "-ldl", "-lrt"]
     r = subprocess.run(link, stdout=subprocess.PIPE, stderr=subprocess.STDOUT, text=True)
     if r.returncode:
         raise RuntimeError("link failed:\n" + r.stdout)
-    os.replace(tmp, LIB)
+    os.replace(tmp, lib)
     for o in objs:
         os.remove(o)
-    return LIB
+    return lib
 
 
 if __name__ == "__main__":
-    print(build(force="--force" in sys.argv, verbose="-v" in sys.argv))
+    print(build(force="--force" in sys.argv, verbose="-v" in sys.argv, trace="--trace" in sys.argv))

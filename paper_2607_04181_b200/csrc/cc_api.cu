@@ -140,6 +140,7 @@ struct cc_ctx {
     cc_slotalloc* slots = nullptr;
     CcLayerTable* table_dev = nullptr;   // [CC_MAX_LAYERS], fixed address for the life of the context
     uint32_t* err_dev = nullptr;
+    unsigned long long* trace_dev = nullptr;   // CC_TRACE builds only
     size_t chunk = (size_t)32 << 20;
     bool row_used[CC_MAX_LAYERS] = {};
     int n_layers = 0;
@@ -224,6 +225,9 @@ cc_status cc_ctx_create(int device, cc_ctx** out) {
     CC_CUDA(cudaMemset(ctx->table_dev, 0, sizeof(CcLayerTable) * CC_MAX_LAYERS));
     CC_CUDA(cudaMalloc(&ctx->err_dev, 256));
     CC_CUDA(cudaMemset(ctx->err_dev, 0, 256));
+#ifdef CC_TRACE
+    CC_CUDA(cudaMalloc(&ctx->trace_dev, sizeof(unsigned long long) * CC_TRACE_KERNELS * CC_TRACE_POINTS * 2));
+#endif
     CC_CUDA(cc_gemm_configure());
     CC_CUDA(cc_attn_configure());
     ctx->slots = cc_slotalloc_create();
@@ -242,6 +246,7 @@ cc_status cc_ctx_destroy(cc_ctx* ctx) {
     cudaStreamDestroy(ctx->side);
     cudaFree(ctx->table_dev);
     cudaFree(ctx->err_dev);
+    cudaFree(ctx->trace_dev);
     cc_slotalloc_destroy(ctx->slots);
     delete ctx;
     return CC_OK;
@@ -450,6 +455,7 @@ cc_status cc_create_layer(cc_ctx* ctx, const cc_layer_desc* desc, const cc_layer
     W.att_o = (float*)(wb + o_atto); W.att_ml = (float2*)(wb + o_attml);
     W.rope_cs = (const float2*)(wb + o_rope);
     W.err = ctx->err_dev;
+    W.trace = ctx->trace_dev;
     L->st_hidden = (__nv_bfloat16*)(wb + o_sth);
     L->st_sl = (int*)(wb + o_tbl); L->st_ra = L->st_sl + d.max_batch; L->st_bt = L->st_ra + d.max_batch;
 
@@ -842,6 +848,26 @@ cc_status cc_kv_migrate(cc_ctx* ctx, void* k_pool_dev, void* v_pool_dev, size_t 
     CC_CUDA(cudaSetDevice(ctx->device));
     CC_CUDA(cc_launch_page_copy(k_pool_dev, v_pool_dev, page_bytes, src_dev, dst_dev, n_moves, (cudaStream_t)stream));
     return CC_OK;
+}
+
+// ---- %globaltimer trace of a tracing build --------------------------------------------------------
+cc_status cc_debug_trace(cc_ctx* ctx, uint64_t* out_host, int reset) {
+    if (!ctx) return fail(CC_ERR_INVALID, "null argument");
+#ifdef CC_TRACE
+    constexpr size_t n = (size_t)CC_TRACE_KERNELS * CC_TRACE_POINTS * 2;
+    CC_CUDA(cudaSetDevice(ctx->device));
+    CC_CUDA(cudaDeviceSynchronize());
+    if (out_host) CC_CUDA(cudaMemcpy(out_host, ctx->trace_dev, n * 8, cudaMemcpyDeviceToHost));
+    if (reset) {
+        std::vector<unsigned long long> h(n);
+        for (size_t i = 0; i < n; ++i) h[i] = (i & 1) ? 0ull : ~0ull;         // [min, max] pairs
+        CC_CUDA(cudaMemcpy(ctx->trace_dev, h.data(), n * 8, cudaMemcpyHostToDevice));
+    }
+    return CC_OK;
+#else
+    (void)out_host; (void)reset;
+    return fail(CC_ERR_STATE, "this library was built without CC_TRACE (python -m paper_2607_04181_b200.build --trace)");
+#endif
 }
 
 // ---- stage taps (tests only) ----------------------------------------------------------------------

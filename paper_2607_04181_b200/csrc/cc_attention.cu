@@ -90,6 +90,7 @@ k_attn(const int* __restrict__ seq_lens, CcKv kv, CcDims D, CcWork W, const CcLa
     // So the producer starts streaming the OLD pages at once -- while the predecessor's CTAs on other
     // SMs are still in their fixup -- and waits for it only before the first stage that holds the last
     // page of a row; the consumers wait before they read q.
+    if (threadIdx.x == 0) CC_TP(W, 1, 0);
     pdl_launch_dependents();
     const int T = W.sched->n_items;                               // KV pages of the batch
     int* s_prefix = reinterpret_cast<int*>(empty + kAttnStages);  // [max_batch + 1]
@@ -197,11 +198,15 @@ k_attn(const int* __restrict__ seq_lens, CcKv kv, CcDims D, CcWork W, const CcLa
 #pragma unroll
     for (int nt = 0; nt < DH / 8; ++nt) o[nt][0] = o[nt][1] = o[nt][2] = o[nt][3] = 0.f;
     pdl_wait();                                         // q (and the new K/V) come from the QKV GEMM
+    if (threadIdx.x == 32) CC_TP(W, 1, 1);
 
     for (;;) {
         mbar_wait(&full[stage], ph);
         const StageMeta m = meta[stage];
-        if (m.flags & kMetaEnd) break;
+        if (m.flags & kMetaEnd) {
+            if (threadIdx.x == 32) CC_TP(W, 1, 2);
+            break;
+        }
         if (m.flags & kMetaFirst) {   // new item: Q fragments, reset the running softmax state
             const float* qrow = W.q_rot + (size_t)m.pos * D.QD + (size_t)(h * G + g) * DH;
 #pragma unroll

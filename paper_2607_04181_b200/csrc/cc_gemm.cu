@@ -237,6 +237,7 @@ k_gemm(CcGemmGeo G, const uint8_t* __restrict__ act, int planes, float* __restri
     GemmSmemHdr* H = reinterpret_cast<GemmSmemHdr*>(smem_raw);
     const int warp = uniform((int)(threadIdx.x >> 5)), lane = threadIdx.x & 31;
 
+    if (threadIdx.x == 0) CC_TP(W, 2 + KIND, 0);
     // ---- one-time setup (independent of the previous kernel: overlaps its tail under PDL) ----
     if (threadIdx.x == 0) {
         for (int i = 0; i < kMaxStages; ++i) {
@@ -358,8 +359,12 @@ k_gemm(CcGemmGeo G, const uint8_t* __restrict__ act, int planes, float* __restri
             };
             run(0);
             pdl_wait();
+            if (lane == 0) CC_TP(W, 2 + KIND, 1);
+            __syncwarp();
             if (elect_one()) pdl_launch_dependents();
             run(1);
+            if (lane == 0) CC_TP(W, 2 + KIND, 2);
+            __syncwarp();
         } else if (warp == 1) {
             // ===================== MMA issuer =====================
             int stage = 0;
@@ -477,6 +482,7 @@ k_gemm(CcGemmGeo G, const uint8_t* __restrict__ act, int planes, float* __restri
     tc_fence_before();
     __syncthreads();
     if (warp == 1) tmem_dealloc<kTmemCols>(tmem_base);
+    if (threadIdx.x == 0) CC_TP(W, 2 + KIND, 3);
     if (nmax == 0) return;
 
     // ---- stream-K fixup: the CTAs c0..c1 whose ranges meet in a super tile split its rows ----------
@@ -501,11 +507,29 @@ k_gemm(CcGemmGeo G, const uint8_t* __restrict__ act, int planes, float* __restri
             }
         }
         __syncthreads();
+        if (threadIdx.x == 0 && st == st_first) CC_TP(W, 2 + KIND, 4);
+#ifdef CC_TRACE
+        const unsigned long long t_pass = cc_gtime();
+#endif
         // few contributors: several items per warp; many: one item, its pieces loaded together
         if (m <= 3) fixup_tile<KIND, 4, 3>(part, E, D, W, H, st, c0, m, k, n_pos, warp, lane);
         else if (m <= 8) fixup_tile<KIND, 2, 4>(part, E, D, W, H, st, c0, m, k, n_pos, warp, lane);
         else fixup_tile<KIND, 1, 8>(part, E, D, W, H, st, c0, m, k, n_pos, warp, lane);
+#ifdef CC_TRACE
+        __syncthreads();
+        if (threadIdx.x == 0 && W.trace != nullptr) {           // duration of this CTA's fixup pass
+            const unsigned long long dt = cc_gtime() - t_pass;
+            const int slot = st == st_first ? 0 : 1;
+            cc_trace_minmax(W.trace, 8 + KIND, slot, dt);
+            atomicAdd(W.trace + ((size_t)(12 + KIND) * CC_TRACE_POINTS + slot) * 2 + 1, 1ull);
+            atomicAdd(W.trace + ((size_t)(12 + KIND) * CC_TRACE_POINTS + 2 + slot) * 2 + 1, dt);
+        }
+#endif
     }
+#ifdef CC_TRACE
+    __syncthreads();
+    if (threadIdx.x == 0) CC_TP(W, 2 + KIND, 5);
+#endif
 }
 
 }  // namespace

@@ -25,7 +25,31 @@ struct CcWork {
     float2* att_ml;      // [max_batch + SMs][Hq] (max in log2 units, sum)
     const float2* rope_cs;  // [max_position][Dh/2] (cos, sin), built in fp64 on the host
     uint32_t* err;       // sticky device error word (context-owned)
+    unsigned long long* trace;   // CC_TRACE builds: [CC_TRACE_KERNELS][CC_TRACE_POINTS][min, max] of %globaltimer; else null
 };
+
+// ---- tracing build (python -m paper_2607_04181_b200.build --trace; read with cc_debug_trace / timeline.py) ----
+// A CC_TRACE build records, per kernel and trace point, the earliest and the latest %globaltimer value over the
+// CTAs that pass it (one thread per CTA); the product build compiles the points away.
+#define CC_TRACE_KERNELS 16
+#define CC_TRACE_POINTS 8
+#if defined(CC_TRACE) && defined(__CUDACC__)
+__device__ __forceinline__ unsigned long long cc_gtime() {
+    unsigned long long t;
+    asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t)::"memory");
+    return t;
+}
+__device__ __forceinline__ void cc_trace_minmax(unsigned long long* tr, int k, int pt, unsigned long long v) {
+    if (tr == nullptr) return;
+    atomicMin(tr + ((size_t)k * CC_TRACE_POINTS + pt) * 2, v);
+    atomicMax(tr + ((size_t)k * CC_TRACE_POINTS + pt) * 2 + 1, v);
+}
+#define CC_TP(W, k, pt) cc_trace_minmax((W).trace, (k), (pt), cc_gtime())
+#else
+#define CC_TP(W, k, pt) ((void)0)
+#endif
+// kernel ids of the trace: 0 prologue, 1 attention, 2..5 the four GEMMs (2 + KIND); 8 + KIND: duration of the
+// first ([0]) and second ([1]) stream-K fixup pass of a CTA, 12 + KIND: [0][max] passes counted / [2][max] their sum
 
 struct CcKv {
     __nv_bfloat16* k_pool;

@@ -55,7 +55,9 @@ __global__ void __launch_bounds__(kNormThreads) k_prologue(const int* __restrict
     __shared__ float red[kNormThreads / 32];
     const int b = threadIdx.x, warp = b >> 5, lane = b & 31;
     const bool pub = blockIdx.x == 0;      // this block writes the tables
+    if (b == 0) CC_TP(W, 0, 0);
     pdl_wait();
+    if (b == 0) CC_TP(W, 0, 1);
     pdl_launch_dependents();
     if (b == 0) s_mypos = -1;
     const int my_b = blockIdx.x;
@@ -185,6 +187,7 @@ __global__ void __launch_bounds__(kNormThreads) k_prologue(const int* __restrict
         *reinterpret_cast<uint4*>(dst) = make_uint4(hi[0], hi[1], hi[2], hi[3]);
         *reinterpret_cast<uint4*>(dst + 1024) = make_uint4(lo[0], lo[1], lo[2], lo[3]);
     }
+    if (b == 0) CC_TP(W, 0, 2);
 }
 
 // Test tap: widen a workspace buffer to fp32 [batch][dim] in original row order.
