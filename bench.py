@@ -54,6 +54,7 @@ def parse_args():
     ap.add_argument("--batch", type=int, default=0,
                     help="decode batch of the cfg2 layer benchmark (default: the config's 64); larger batches are for the "
                          "tensor-pipe evidence of the GEMMs (DESIGN.md section 9), not the headline")
+    ap.add_argument("--copy-sweep", action="store_true", help="also sweep the chunk size of the replica copy (replica_copy.chunk_sweep)")
     ap.add_argument("--workload", default="cfg2", choices=["cfg2", "cfg3", "cfg5"],
                     help="cfg2 (default): the headline layer benchmark; cfg3: BASELINE.json configs[2], the 32-layer "
                          "decode graph with layers 10-12 flipped to 2 replicas and back (latency series, not the headline); "
@@ -354,11 +355,32 @@ def run_ours(args):
         torch.cuda.synchronize()
     cms = float(np.median(copy_ms[2:]))
     blob = S.blob_bytes
+    copy_sweep = None
+    if args.copy_sweep:                           # chunk size of the side-stream copy (cc_ctx_set_copy_chunk); default 32 MiB
+        copy_sweep = {}
+        for mib in (4, 8, 16, 32, 64, 128, 512):
+            B.cc_ctx_set_copy_chunk(S.ctx, mib << 20)
+            ts = []
+            for _ in range(8):
+                a, b_ = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                a.record()
+                B.cc_scale_layer(S.layer, 2)
+                B.cc_commit(S.layer, stream)
+                b_.record()
+                torch.cuda.synchronize()
+                ts.append(a.elapsed_time(b_))
+                S.scale(1)
+                torch.cuda.synchronize()
+            t = float(np.median(ts[2:]))
+            copy_sweep[f"{mib}MiB"] = {"ms_call_to_visible": round(t, 4), "GBps_read_plus_write": round(2 * blob / (t * 1e-3) / 1e9, 1)}
+        B.cc_ctx_set_copy_chunk(S.ctx, 32 << 20)
     replica_copy = {"blob_bytes": blob, "ms_call_to_visible": round(cms, 4),
                     "GBps_read_plus_write": round(2 * blob / (cms * 1e-3) / 1e9, 1),
                     "GBps_payload": round(blob / (cms * 1e-3) / 1e9, 1),
                     "frac_of_copy_peak": round(2 * blob / (cms * 1e-3) / 1e9 / peak, 4),
                     "graph_recaptures": 0}
+    if copy_sweep is not None:
+        replica_copy["chunk_sweep"] = copy_sweep
 
     # ---- replica creation WHILE decoding (the one-GPU analogue of PAPER.md:385's "< 3 % fluctuation"): the copy
     # runs on the side stream under a train of graph replays; what does it cost the steps, and the copy? --------
