@@ -171,6 +171,10 @@ cc_status cc_replica_blob(cc_layer *layer, int replica, const void **blob_dev, s
  *                   seq_lens[b] <= 0 marks a padding row: left untouched, no KV write.
  *   replica_assign_dev  int32 [batch], DEVICE: which replica's weights serve row b
  *                   (PAPER.md:93 sub-batches; any assignment, any group sizes including 0).
+ * Several rows may belong to ONE request (a prompt chunk): they carry copies of its block-table row and
+ * consecutive seq_lens t+1, t+2, ...; every row's K/V is appended before any row attends, so the row
+ * of token t attends exactly positions <= t (causal prefill through the decode kernels; such rows must
+ * name the same replica if the caller keeps KV partitions).  tests/test_prefill_chunk.py.
  * Rows are grouped by replica on the device; each group streams ITS replica's weight slot, read
  * through the device replica table, so a graph captured around this call keeps working across
  * cc_commit.  Results are bit-identical for any assignment and replica count. */

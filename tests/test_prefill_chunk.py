@@ -1,0 +1,96 @@
+"""Chunked prefill through the decode path (the part that needs no new kernel): the tokens of
+a prompt chunk are rows of one step that share their request's block-table row, token t at seq_len = t + 1.  Every
+row's K/V is appended before any row attends (PAPER.md:103 appends, then the attention of the step), so row t sees
+exactly the positions <= t: causal attention over the paged cache.  Pins: on the oracle one step over the chunk equals
+the same tokens decoded one by one BITWISE; on the GPU the chunk step matches the oracle within the tolerance, and its
+KV cache equals the one-by-one GPU run bitwise.  (Cost: each row streams its own prefix, so this is the functional
+path for short chunks, not the large-M kernels NEXT-2 asks for -- DESIGN.md section 10.)"""
+import numpy as np
+import pytest
+
+import oracle
+from paper_2607_04181_b200 import inputs as I
+
+SHAPE = I.LayerShape("chunk", 512, 8, 2, 128, 1408, 1e-5, 500000.0, 8, 40, 300)
+N_CHUNK, CACHED = 37, 90                      # the chunk covers positions 90..126: crosses pages 5|6 and 6|7
+
+
+def _scenario():
+    """6 ordinary decode rows + one request whose 37-token chunk starts after 90 cached tokens."""
+    base = I.make_step_inputs(SHAPE, 2401, 3401, batch=7, n_pages=7 * SHAPE.max_blocks,
+                              contexts=np.array([41, 300, 77, 128, 255, 64, CACHED + N_CHUNK - 1], np.int32))
+    rng = np.random.default_rng(2402)
+    B = 6 + N_CHUNK
+    hidden = np.empty((B, SHAPE.hidden), np.uint16)
+    hidden[:6] = base.hidden[:6]
+    hidden[6:] = I._normal_bf16(rng, (N_CHUNK, SHAPE.hidden), 0.0, 1.0)
+    bt = np.vstack([base.block_table[:6]] + [base.block_table[6:7]] * N_CHUNK).astype(np.int32)
+    seq = np.concatenate([base.seq_lens[:6], CACHED + 1 + np.arange(N_CHUNK)]).astype(np.int32)
+    assign = np.concatenate([[0, 1, 0, 1, 0, 1], np.ones(N_CHUNK)]).astype(np.int32)    # a request lives on ONE replica
+    return I.StepInputs(hidden, base.k_pool, base.v_pool, bt, seq, base.n_pages), assign
+
+
+def _one_by_one(st, assign):
+    """The same tokens as single steps: the decode rows and token 0 of the chunk first, then one chunk token per step."""
+    steps = [np.arange(7)] + [np.array([6 + t]) for t in range(1, N_CHUNK)]
+    return [(rows, I.StepInputs(st.hidden[rows], None, None, st.block_table[rows], st.seq_lens[rows], st.n_pages), assign[rows])
+            for rows in steps]
+
+
+def test_oracle_chunk_step_equals_one_token_at_a_time_bitwise():
+    w = I.make_weights(SHAPE, 1401)
+    st, assign = _scenario()
+    chunk = oracle.layer_forward(SHAPE, w, st.hidden, st.k_pool, st.v_pool, st.block_table, st.seq_lens, assign, 2)
+    kp, vp = st.k_pool, st.v_pool
+    out = np.empty_like(st.hidden)
+    for rows, s, a in _one_by_one(st, assign):
+        r = oracle.layer_forward(SHAPE, w, s.hidden, kp, vp, s.block_table, s.seq_lens, a, 2)
+        out[rows], kp, vp = r["out"], r["k_pool"], r["v_pool"]
+    assert np.array_equal(out, chunk["out"])
+    assert np.array_equal(kp, chunk["k_pool"]) and np.array_equal(vp, chunk["v_pool"])
+    # and causality has teeth: a chunk row's output changes when an EARLIER chunk token's input changes, not a later one's
+    h2 = st.hidden.copy()
+    h2[6 + 20] ^= 0x0040
+    again = oracle.layer_forward(SHAPE, w, h2, st.k_pool, st.v_pool, st.block_table, st.seq_lens, assign, 2)["out"]
+    assert np.array_equal(again[:6 + 20], chunk["out"][:6 + 20])              # rows before token 20: untouched
+    assert all(not np.array_equal(again[6 + t], chunk["out"][6 + t]) for t in range(20, N_CHUNK))
+
+
+@pytest.mark.gpu
+def test_gpu_chunk_step_matches_oracle_and_the_one_by_one_cache_bitwise():
+    import torch
+    from paper_2607_04181_b200 import binding as B
+    from paper_2607_04181_b200.harness import DeviceStep, Session
+    from tests.test_gpu_parity import within
+
+    w = I.make_weights(SHAPE, 1401)
+    st, assign = _scenario()
+    ref = oracle.layer_forward(SHAPE, w, st.hidden, st.k_pool, st.v_pool, st.block_table, st.seq_lens, assign, 2, taps=True)
+    batch = st.hidden.shape[0]
+    with Session(SHAPE, w, max_batch=batch) as S:
+        S.scale(2)
+        step = DeviceStep(st, assign)
+        S.forward(step)
+        torch.cuda.synchronize()
+        assert B.cc_poll_device_error(S.ctx) == 0
+        out, (kp, vp) = step.out_bits(), step.pools_bits()
+        within(I.bf16_bits_to_f32(out), I.bf16_bits_to_f32(ref["out"]), "chunk step output")
+        within(S.tap(B.CC_TAP_O, batch), ref["taps"]["o"], "chunk step attention output")
+        # the same tokens one by one on the GPU: the cache must come out bit for bit the same (per-row GEMM results do not
+        # depend on the batch), the outputs within the tolerance of the same oracle values
+        step.reset(st)
+        seq_out = np.empty_like(out)
+        for rows, s, a in _one_by_one(st, assign):
+            n = len(rows)
+            step.hidden[:n].copy_(torch.from_numpy(s.hidden.view(np.int16)).cuda().view(torch.bfloat16))
+            step.block_table[:n].copy_(torch.from_numpy(s.block_table))
+            step.seq_lens.zero_()
+            step.seq_lens[:n].copy_(torch.from_numpy(s.seq_lens))
+            step.assign[:n].copy_(torch.from_numpy(a))
+            S.forward(step)
+            torch.cuda.synchronize()
+            seq_out[rows] = step.out_bits()[:n]
+        kp1, vp1 = step.pools_bits()
+        assert np.array_equal(kp1, kp) and np.array_equal(vp1, vp)
+        within(I.bf16_bits_to_f32(seq_out), I.bf16_bits_to_f32(ref["out"]), "one-by-one output")
+        assert B.cc_poll_device_error(S.ctx) == 0
