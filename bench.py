@@ -54,6 +54,8 @@ def parse_args():
     ap.add_argument("--batch", type=int, default=0,
                     help="decode batch of the cfg2 layer benchmark (default: the config's 64); larger batches are for the "
                          "tensor-pipe evidence of the GEMMs (DESIGN.md section 9), not the headline")
+    ap.add_argument("--prefill-rows", type=int, default=64,
+                    help="cfg5: prompt tokens carried by every step of model A as extra rows (half as many for B); 0 = decode only")
     ap.add_argument("--copy-sweep", action="store_true", help="also sweep the chunk size of the replica copy (replica_copy.chunk_sweep)")
     ap.add_argument("--workload", default="cfg2", choices=["cfg2", "cfg3", "cfg5"],
                     help="cfg2 (default): the headline layer benchmark; cfg3: BASELINE.json configs[2], the 32-layer "
@@ -665,8 +667,8 @@ def run_cfg5(args):
                                frac_a=0.75, prompt_mean=512, out_mean=256, sigma=1.0, max_prompt=4096, max_out=1024)
     shape_a = I.CFG2
     shape_b = I.MODEL_B_LAYER
-    A = S.ModelRunner("A", shape_a, 32, 128, 12000, 5120, seed=1005, n_slots=0, hot_layers=hot)
-    Bm = S.ModelRunner("B", shape_b, 28, 64, 6000, 5120, seed=1006, n_slots=0)
+    A = S.ModelRunner("A", shape_a, 32, 128, 12000, 5120, seed=1005, n_slots=0, hot_layers=hot, prefill_rows=args.prefill_rows)
+    Bm = S.ModelRunner("B", shape_b, 28, 64, 6000, 5120, seed=1006, n_slots=0, prefill_rows=args.prefill_rows // 2)
     sampler = ClockSampler(0)
     sampler.start()
     t0 = time.perf_counter()
@@ -682,8 +684,11 @@ def run_cfg5(args):
         "vs_baseline": None, "dtype": "bf16", "data": "synthetic",
         "config": {"workload": "cfg5 (BASELINE.json configs[4]): model A = 32 Llama-3-8B-shaped layers (75 % of the requests), model B = 28 "
                                "layers of hidden 1536 / 12 q / 2 kv heads x 128 / FFN 8960; Poisson arrivals 7 req/s with 5x bursts of 10 s every "
-                               f"60 s over {args.horizon:.0f} s, prompts lognormal (mean 512), outputs lognormal (mean 256); decode only: prompts count as "
-                               "cached KV (no prefill kernel yet); A's 8 hot layers get a second replica in memory lent from B's KV reserve "
+                               f"60 s over {args.horizon:.0f} s, prompts lognormal (mean 512), outputs lognormal (mean 256); "
+                               + (f"mixed steps: up to {args.prefill_rows} (A) / {args.prefill_rows // 2} (B) prompt tokens per step run as rows of "
+                                  "the decode path (causal chunked prefill through the decode kernels; the large-M prefill kernels are not built); "
+                                  if args.prefill_rows else "decode only: prompts count as cached KV; ") +
+                               "A's 8 hot layers get a second replica in memory lent from B's KV reserve "
                                "while A's backlog is >= 48 requests",
                    "hot_layers": list(hot), "requests": len(arrivals)},
         "clocks": clocks, "serving": out, "wall_s": round(wall, 1),

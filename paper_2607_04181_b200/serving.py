@@ -2,8 +2,12 @@
 continuous batching of decode steps, a paged-KV allocator per model, and layer-wise scaling of the hot model's
 hot layers into memory reclaimed from the cold model's KV budget.
 
-What it is not: there is no prefill (NEXT-2) -- a request's prompt counts as already cached KV (pages are
-allocated, their contents are whatever the pool holds), so only decode steps run.  Time is the sum of the measured
+Prefill: with prefill_rows = 0 a request's prompt counts as already cached KV (pages are allocated, their contents
+are whatever the pool holds) and only decode steps run.  With prefill_rows = P every step is a MIXED step: beside the
+decode rows it carries up to P tokens of the oldest admitted prompt as rows that share the request's block-table row
+at consecutive seq_lens -- causal chunked prefill through the decode kernels (tests/test_prefill_chunk.py; the
+efficient prefill kernels are NEXT-2) -- and a request starts decoding when its prompt is done, so the first token's
+latency includes its prefill.  Time is the sum of the measured
 device times of the steps (CUDA events); arrivals are a seeded synthetic process on that clock.  Parity: unpinned
 by the paper; the tests check conservation (every request finishes with its token count, no page is lost or
 shared) and that the steps go through the same cc_forward graphs as everything else.
@@ -27,8 +31,9 @@ class Request:
     rid: int
     model: str
     arrival: float          # seconds on the simulated clock
-    prompt: int             # tokens treated as cached
+    prompt: int             # prompt tokens (treated as cached when the runner has no prefill rows)
     out_len: int            # tokens to generate
+    prefilled: int = 0      # prompt tokens whose KV has been computed
     pages: list = field(default_factory=list)
     slot: int = -1
     generated: int = 0
@@ -89,7 +94,9 @@ class ModelRunner:
     every layer's K/V pool), request slots = rows of the decode batch."""
 
     def __init__(self, name: str, shape: I.LayerShape, n_layers: int, max_batch: int, n_pages: int, max_tokens: int,
-                 seed: int, n_slots: int, hot_layers=(), device: str = "cuda:0"):
+                 seed: int, n_slots: int, hot_layers=(), device: str = "cuda:0", prefill_rows: int = 0):
+        self.n_decode, self.P = max_batch, prefill_rows            # rows [0, n_decode): request slots; then the prompt chunk
+        max_batch = max_batch + prefill_rows                       # rows of the captured step
         self.name, self.shape, self.L, self.max_batch, self.dev = name, shape, n_layers, max_batch, device
         self.width = (max_tokens + shape.page - 1) // shape.page
         gen = torch.Generator(device=device).manual_seed(seed)
@@ -118,7 +125,10 @@ class ModelRunner:
         self.assigns = [torch.zeros(max_batch, dtype=torch.int32, device=device) for _ in range(n_layers)]
         self.hot = tuple(hot_layers)
         self.replicas = 1
-        self.slots = [None] * max_batch
+        self.slots = [None] * self.n_decode
+        self.prefilling = []            # admitted requests whose prompt is not done yet, oldest first
+        self.prompt_tokens = 0
+        self._decoded = []              # slots that decoded a token in the last step
         self.graph = None
         self.captures = 0
         self.scale_events = []          # (clock, n_replicas, ms, GB/s read+write)
@@ -152,12 +162,31 @@ class ModelRunner:
         self.slots[r.slot] = r
         self.bt_host[r.slot].fill_(-1)
         self.bt_host[r.slot, :need] = torch.tensor(pages, dtype=torch.int32)
+        if self.P > 0:
+            r.prefilled = 0
+            self.prefilling.append(r)
+        else:
+            r.prefilled = r.prompt
         return True
 
     def step(self) -> float:
-        """One decode step for every active request; returns the device time in seconds."""
+        """One step: a decode token for every request whose prompt is done and, with prefill rows, the next chunk of the
+        oldest unfinished prompt; returns the device time in seconds."""
+        self._decoded = []
         for b, r in enumerate(self.slots):
-            self.sl_host[b] = 0 if r is None else r.prompt + r.generated + 1
+            live = r is not None and r.prefilled >= r.prompt
+            self.sl_host[b] = r.prompt + r.generated + 1 if live else 0
+            if live:
+                self._decoded.append(b)
+        chunk = 0
+        if self.P > 0:
+            self.sl_host[self.n_decode:] = 0
+            if self.prefilling:
+                r = self.prefilling[0]
+                chunk = min(self.P, r.prompt - r.prefilled)
+                rows = slice(self.n_decode, self.n_decode + chunk)
+                self.bt_host[rows] = self.bt_host[r.slot]                          # the chunk's rows share the request's pages
+                self.sl_host[rows] = torch.arange(r.prefilled + 1, r.prefilled + chunk + 1, dtype=torch.int32)
         self.bt.copy_(self.bt_host, non_blocking=True)
         self.sl.copy_(self.sl_host, non_blocking=True)
         e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
@@ -165,12 +194,17 @@ class ModelRunner:
         self.graph.replay()
         e1.record()
         e1.synchronize()
+        if chunk:
+            r = self.prefilling[0]
+            r.prefilled += chunk
+            self.prompt_tokens += chunk
+            if r.prefilled >= r.prompt:
+                self.prefilling.pop(0)                                             # decodes from the next step on
         return e0.elapsed_time(e1) * 1e-3
 
     def finish_tokens(self, now: float, lat_out: list, done_out: list) -> None:
-        for b, r in enumerate(self.slots):
-            if r is None:
-                continue
+        for b in self._decoded:
+            r = self.slots[b]
             r.generated += 1
             lat_out.append(now - r.last_token_at)
             r.last_token_at = now
@@ -277,6 +311,7 @@ def simulate(A: ModelRunner, Bm: ModelRunner, arrivals, burst_hi: int, burst_lo:
                      "token_latency_ms_p50": None if not lat[name] else 1e3 * pct(lat[name], 50),
                      "token_latency_ms_p99": None if not lat[name] else 1e3 * pct(lat[name], 99),
                      "mean_batch": float(np.mean([s[1] for s in step_s[name]])) if step_s[name] else 0.0,
+                     "prompt_tokens_prefilled": m.prompt_tokens, "prefill_rows": m.P,
                      "pages_in_use_at_end": m.pool.used()}
     by_rep = {}
     for dt, nb, rep in step_s["A"]:
