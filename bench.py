@@ -57,7 +57,7 @@ def parse_args():
     ap.add_argument("--prefill-rows", type=int, default=64,
                     help="cfg5: prompt tokens carried by every step of model A as extra rows (half as many for B); 0 = decode only")
     ap.add_argument("--copy-sweep", action="store_true", help="also sweep the chunk size of the replica copy (replica_copy.chunk_sweep)")
-    ap.add_argument("--workload", default="cfg2", choices=["cfg2", "cfg3", "cfg5"],
+    ap.add_argument("--workload", default="cfg2", choices=["cfg2", "cfg3", "cfg4", "cfg5"],
                     help="cfg2 (default): the headline layer benchmark; cfg3: BASELINE.json configs[2], the 32-layer "
                          "decode graph with layers 10-12 flipped to 2 replicas and back (latency series, not the headline); "
                          "cfg5: configs[4], the co-located serving loop (decode only)")
@@ -651,6 +651,122 @@ def run_cfg3(args):
 # ---------------------------------------------------------------------------------------------
 # cfg5 (BASELINE.json configs[4]): skewed co-located serving, decode only (no prefill kernel yet: NEXT-2)
 # ---------------------------------------------------------------------------------------------
+def run_cfg4(args):
+    """BASELINE.json configs[3], ONE layer of the 14B-class shape: a mixed step of two 2048-token prompt chunks and 256
+    decode rows.  There is no large-M kernel (NEXT-2): the step runs as 17 cc_forward calls of 256 rows each -- eight per
+    prompt (rows = consecutive tokens sharing the request's block-table row: causal prefill through the decode path,
+    tests/test_prefill_chunk.py), one for the decode rows -- captured in one graph.  Reported so that the config has a
+    measured line; what it shows is the GEMM at n = 256 (tensor-bound) and an attention that re-reads every prefix."""
+    import torch
+
+    from paper_2607_04181_b200 import binding as B
+    from paper_2607_04181_b200 import inputs as I
+    from paper_2607_04181_b200.harness import ModelSession
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the library has no CPU fallback")
+    dev = "cuda:0"
+    torch.cuda.set_device(0)
+    shape = I.CFG4_LAYER
+    page, rows, prompt, n_prompts = shape.page, 256, 2048, 2
+    rng = np.random.default_rng(3004)
+    dec_ctx = rng.integers(256, 4097, rows)                                   # decode contexts U{256..4096}
+    width = (4096 + 1 + page - 1) // page
+    need = np.concatenate([[prompt // page] * n_prompts, (dec_ctx + 1 + page - 1) // page]).astype(np.int64)
+    n_pages = int(need.sum())
+    ids = rng.permutation(n_pages).astype(np.int32)
+    req_bt = np.full((n_prompts + rows, width), -1, np.int32)
+    off = 0
+    for i, n in enumerate(need):
+        req_bt[i, :n] = ids[off:off + n]
+        off += int(n)
+    gen = torch.Generator(device=dev).manual_seed(1004)
+
+    def randn(*shp, std=1.0, mean=0.0):
+        return (torch.randn(*shp, generator=gen, device=dev, dtype=torch.float32) * std + mean).to(torch.bfloat16)
+    d, F, QD, KD = shape.hidden, shape.ffn, shape.q_dim, shape.kv_dim
+    S = ModelSession(shape, [], max_batch=rows, n_slots=1, max_blocks=width, max_position=width * page)
+    S.add_layer({"g1": randn(d, std=0.02, mean=1.0), "wq": randn(QD, d, std=0.02), "wk": randn(KD, d, std=0.02),
+                 "wv": randn(KD, d, std=0.02), "wo": randn(d, QD, std=0.02), "g2": randn(d, std=0.02, mean=1.0),
+                 "wgate": randn(F, d, std=0.02), "wup": randn(F, d, std=0.02), "wdown": randn(d, F, std=0.02)})
+    S.donate()
+    S.scale(0, 2)                                                             # configs[3]: the hot layers run at R = 2
+    pool_shape = (n_pages, shape.n_kv_heads, page, shape.head_dim)
+    kp, vp = randn(*pool_shape), randn(*pool_shape)
+    subs = []                                                                 # (hidden, block table, seq_lens, assign) per call
+    for r in range(n_prompts):
+        for c in range(prompt // rows):
+            seq = np.arange(c * rows + 1, (c + 1) * rows + 1, dtype=np.int32)
+            subs.append((randn(rows, d), torch.from_numpy(np.repeat(req_bt[r:r + 1], rows, 0)).to(dev), torch.from_numpy(seq).to(dev),
+                         torch.full((rows,), r % 2, dtype=torch.int32, device=dev)))       # a request lives on one replica
+    subs.append((randn(rows, d), torch.from_numpy(req_bt[n_prompts:]).to(dev), torch.from_numpy((dec_ctx + 1).astype(np.int32)).to(dev),
+                 torch.from_numpy(I.even_split(rows, 2)).to(dev)))
+    stream = torch.cuda.current_stream()
+
+    def mixed_step(st):
+        for h, bt, sl, ra in subs:
+            B.cc_forward(S.layers[0], h, kp, vp, bt, n_pages, sl, ra, rows, st)
+    mixed_step(stream)
+    torch.cuda.synchronize()
+    assert B.cc_poll_device_error(S.ctx) == 0
+    graph = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(graph):
+        mixed_step(torch.cuda.current_stream())
+    K, W = max(args.steps // 10, 10), max(args.warmup // 4, 3)
+    for _ in range(W):
+        graph.replay()
+    sampler = ClockSampler(0)
+    sampler.start()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for _ in range(K):
+        graph.replay()
+    e1.record()
+    torch.cuda.synchronize()
+    ms = e0.elapsed_time(e1) / K
+    t_end = time.perf_counter() + 1.0
+    while time.perf_counter() < t_end:
+        graph.replay()
+        torch.cuda.synchronize()
+    clocks = sampler.stop()
+    # per-kernel times of the 17 calls (kernel by kernel, no PDL)
+    stage = np.zeros(len(B.STAGE_NAMES))
+    for rep in range(3):
+        acc = np.zeros(len(B.STAGE_NAMES))
+        for h, bt, sl, ra in subs:
+            acc += B.cc_forward_profiled(S.layers[0], h, kp, vp, bt, n_pages, sl, ra, rows, stream)
+        stage = acc if rep == 0 else np.minimum(stage, acc)
+    tokens = len(subs) * rows
+    n_w = d * (QD + 2 * KD) + QD * d + 3 * d * F
+    gemm_ms = float(sum(stage[i] for i, n in enumerate(B.STAGE_NAMES) if n.startswith("gemm")))
+    attn_ms = float(stage[B.STAGE_NAMES.index("attention")])
+    kv_tok = sum(int(sl.sum().item()) for _, _, sl, _ in subs)
+    peaks = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json"))) if os.path.exists(os.path.join(ROOT, "MEASURED_PEAKS.json")) else {}
+    S.close()
+    line = {
+        "metric": "mixed prefill + decode step of one 14B-class layer (cfg4): tokens/s", "value": tokens / (ms * 1e-3), "unit": UNIT,
+        "n_gpus": 1, "steps": K, "warmup": W, "ms_per_step": ms, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "bf16", "data": "synthetic",
+        "config": {"workload": "cfg4 (BASELINE.json configs[3]), ONE layer: hidden 5120, 40 q / 8 kv heads x 128, FFN 17408, R = 2; mixed step = "
+                               "2 x 2048 prompt tokens + 256 decode rows (contexts U{256..4096}) = 4352 rows, run as 17 cc_forward calls of 256 rows "
+                               "in one CUDA graph (no large-M kernel: every call streams the layer's weights; a prompt token re-reads its prefix)",
+                   "calls_per_step": len(subs), "rows_per_call": rows},
+        "clocks": clocks, "gpu_launches": K * len(subs) * len(B.STAGE_NAMES),
+        "gemm": {"ms_per_step_kernel_by_kernel": round(gemm_ms, 4), "flops_per_step_one_plane": 2.0 * tokens * n_w,
+                 "TFLOPs_one_plane": round(2.0 * tokens * n_w / (gemm_ms * 1e-3) / 1e12, 1),
+                 "TFLOPs_issued_two_planes": round(4.0 * tokens * n_w / (gemm_ms * 1e-3) / 1e12, 1),
+                 "measured_bf16_peak_TFLOPs_burst": peaks.get("bf16_tflops"), "measured_bf16_peak_TFLOPs_sustained": peaks.get("bf16_tflops_sustained"),
+                 "weight_bytes_streamed": len(subs) * n_w * 2},
+        "attention": {"ms_per_step_kernel_by_kernel": round(attn_ms, 4), "kv_bytes_streamed": kv_tok * 2 * KD * 2,
+                      "GBps_per_row_algorithmic": round(kv_tok * 2 * KD * 2 / (attn_ms * 1e-3) / 1e9, 1),
+                      "note": "bytes counted per row; the 256 rows of a prompt call read the same pages, so most of them are L2 hits "
+                              "(the figure can exceed the HBM peak)"},
+        "stages_ms": {n: round(float(x), 4) for n, x in zip(B.STAGE_NAMES, stage)},
+    }
+    print(json.dumps(line), flush=True)
+    return 0
+
+
 def run_cfg5(args):
     import torch
 
@@ -705,6 +821,8 @@ def main():
         return run_cfg5(args)
     if args.workload == "cfg3":
         return run_cfg3(args)
+    if args.workload == "cfg4":
+        return run_cfg4(args)
     return run_ours(args)
 
 
