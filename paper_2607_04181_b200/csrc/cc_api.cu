@@ -408,6 +408,7 @@ cc_status cc_create_layer(cc_ctx* ctx, const cc_layer_desc* desc, const cc_layer
     const size_t o_perm = ws.take(Mp * 4);
     const size_t o_pgpre = ws.take((size_t)(d.max_batch + 1) * 4);
     const size_t o_posof = ws.take((size_t)d.max_batch * 4);
+    const size_t o_fwr = ws.take((size_t)d.max_batch * 4);
     const size_t o_x = ws.take((size_t)2 * D.qkv.KB * Mp * 128);   // hi + lo planes
     const size_t o_o = ws.take((size_t)2 * D.o.KB * Mp * 128);
     const size_t o_y = ws.take((size_t)2 * D.gu.KB * Mp * 128);
@@ -446,6 +447,7 @@ cc_status cc_create_layer(cc_ctx* ctx, const cc_layer_desc* desc, const cc_layer
     }
     uint8_t* wb = L->work_base;
     W.sched = (CcSched*)(wb + o_sched); W.perm = (int*)(wb + o_perm); W.pg_prefix = (int*)(wb + o_pgpre); W.pos_of = (int*)(wb + o_posof);
+    W.first_wr = (int*)(wb + o_fwr);
     W.x_act = wb + o_x; W.o_act = wb + o_o; W.y_act = wb + o_y; W.a_act = wb + o_a;
     W.qkv_part = (float*)(wb + o_pq); W.o_part = (float*)(wb + o_po); W.gu_part = (float*)(wb + o_pg);
     W.d_part = (float*)(wb + o_pd);
@@ -688,7 +690,7 @@ cudaError_t enqueue_forward(cc_layer* L, __nv_bfloat16* hidden, const CcKv& kv, 
     for (int stage = 0; stage < kForwardLaunches && e == cudaSuccess; ++stage) {
         if (ev && (e = cudaEventRecord(ev[stage], st)) != cudaSuccess) break;
         switch (stage) {
-            case 0: e = cc_launch_prologue(assign, seq_lens, batch, h_in, D, tab, W, Ln, so); break;
+            case 0: e = cc_launch_prologue(assign, seq_lens, kv.block_table, batch, h_in, D, tab, W, Ln, so); break;
             case 1: e = cc_launch_gemm(0, D, tab, W, seq_lens, assign, batch, kv, hidden, Ln); break;
             case 2: e = cc_launch_attention(seq_lens, kv, D, tab, W, Ln); break;
             case 3: e = cc_launch_gemm(1, D, tab, W, seq_lens, assign, batch, kv, hidden, Ln); break;

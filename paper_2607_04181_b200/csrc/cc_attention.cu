@@ -88,8 +88,9 @@ k_attn(const int* __restrict__ seq_lens, CcKv kv, CcDims D, CcWork W, const CcLa
     // The grouping tables (k_prologue) were complete two kernels back, seq_lens and the block table are
     // inputs: only q and the K/V of the token being decoded come from the predecessor (the QKV GEMM).
     // So the producer starts streaming the OLD pages at once -- while the predecessor's CTAs on other
-    // SMs are still in their fixup -- and waits for it only before the first stage that holds the last
-    // page of a row; the consumers wait before they read q.
+    // SMs are still in their fixup -- and waits for it only before the first stage that holds a page
+    // this step appends to (the last page of a lone row; for the rows of a prompt chunk the lowest page
+    // any of them writes: W.first_wr from the prologue); the consumers wait before they read q.
     if (threadIdx.x == 0) CC_TP(W, 1, 0);
     pdl_launch_dependents();
     const int T = W.sched->n_items;                               // KV pages of the batch
@@ -122,7 +123,7 @@ k_attn(const int* __restrict__ seq_lens, CcKv kv, CcDims D, CcWork W, const CcLa
             const int r0 = s_prefix[b], r1 = s_prefix[b + 1];
             if (r1 <= p) { ++b; continue; }                       // rows without pages (padding)
             const int q0 = p - r0, q1 = min(r1, P1) - r0;         // this CTA's pages of row b
-            const int pos = W.pos_of[b], s = seq_lens[b];
+            const int pos = W.pos_of[b], s = seq_lens[b], first_wr = W.first_wr[b];
             const int slot0 = b + cta_of_page(r0), n_pieces = cta_of_page(r1 - 1) - cta_of_page(r0) + 1;
             const int slot = b + (int)blockIdx.x;
             const int n_groups = (q1 - q0 + PPS - 1) / PPS;
@@ -143,7 +144,7 @@ k_attn(const int* __restrict__ seq_lens, CcKv kv, CcDims D, CcWork W, const CcLa
                 }
                 mbar_wait(&empty[stage], ph ^ 1);
                 const int in_grp = min(PPS, q1 - qg);
-                if (!waited && (qg + in_grp) * CC_PAGE >= s) {     // the stage holds the page of position s - 1
+                if (!waited && qg + in_grp > first_wr) {          // the stage holds a page this step appends to
                     pdl_wait();
                     waited = true;
                 }

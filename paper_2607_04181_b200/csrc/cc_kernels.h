@@ -8,6 +8,7 @@ struct CcWork {
     int* perm;           // [Mpad] original row at grouped position, or -1
     int* pg_prefix;      // [max_batch + 1] pages of the rows before row b, request order (attention work split)
     int* pos_of;         // [max_batch] grouped position of row b, or -1
+    int* first_wr;       // [max_batch] lowest page index of row b's request that some row of this step appends to
     uint8_t* x_act;      // packed bf16 GEMM operands, [K/64][Mpad/8][plane hi|lo][8][128 B swizzled]
     uint8_t* o_act;
     uint8_t* y_act;
@@ -72,9 +73,9 @@ struct CcStageOut {
     __nv_bfloat16* hidden = nullptr;   // [batch][d]
 };
 
-cudaError_t cc_launch_prologue(const int* assign, const int* seq_lens, int batch, const __nv_bfloat16* hidden,
-                               const CcDims& D, const CcLayerTable* tab, const CcWork& W, const CcLaunch& L,
-                               const CcStageOut& so = CcStageOut());
+cudaError_t cc_launch_prologue(const int* assign, const int* seq_lens, const int* block_table, int batch,
+                               const __nv_bfloat16* hidden, const CcDims& D, const CcLayerTable* tab, const CcWork& W,
+                               const CcLaunch& L, const CcStageOut& so = CcStageOut());
 // which: 0 = QKV, 1 = O, 2 = gate/up, 3 = down
 cudaError_t cc_launch_gemm(int which, const CcDims& D, const CcLayerTable* tab, const CcWork& W, const int* seq_lens,
                            const int* assign, int batch, const CcKv& kv, __nv_bfloat16* hidden, const CcLaunch& L);

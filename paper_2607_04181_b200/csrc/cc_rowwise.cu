@@ -46,15 +46,18 @@ __device__ __forceinline__ void split_hilo(float v0, float v1, uint32_t& hi, uin
 constexpr int kNormThreads = 512;
 constexpr int kNormVec = 2;            // uint4 (8 bf16) per thread: hidden <= 8 * 2 * 512 = 8192
 __global__ void __launch_bounds__(kNormThreads) k_prologue(const int* __restrict__ assign, const int* __restrict__ seq_lens,
-                                                           int batch, const __nv_bfloat16* __restrict__ hidden, CcDims D,
+                                                           const int* __restrict__ block_table, int batch,
+                                                           const __nv_bfloat16* __restrict__ hidden, CcDims D,
                                                            const CcLayerTable* __restrict__ tab, CcWork W, CcStageOut so) {
     __shared__ int s_wcnt[8][CC_MAXR];     // rows of replica r in warp w
     __shared__ int s_wnch[8];              // KV pages of the rows of warp w
     __shared__ int s_goff[CC_MAXR + 1], s_cnt[CC_MAXR];
     __shared__ int s_mypos, s_myrep;
+    __shared__ int s_key[256], s_wpg[256];   // first page id of row b (names its request), page index row b appends to
     __shared__ float red[kNormThreads / 32];
     const int b = threadIdx.x, warp = b >> 5, lane = b & 31;
     const bool pub = blockIdx.x == 0;      // this block writes the tables
+    const bool scan = blockIdx.x == gridDim.x - 1;   // this one finds the rows that share a request (prompt chunks)
     if (b == 0) CC_TP(W, 0, 0);
     pdl_wait();
     if (b == 0) CC_TP(W, 0, 1);
@@ -76,6 +79,11 @@ __global__ void __launch_bounds__(kNormThreads) k_prologue(const int* __restrict
         uint32_t err = 0;
         rep = cc_row_replica(assign, seq_lens, b, batch, D, tab->active_mask, err);
         if (pub && err) atomicOr(W.err, err);
+        if (scan) {
+            // rows of one request carry copies of its block-table row, so its first page id names the request
+            s_key[b] = rep >= 0 ? block_table[(size_t)b * D.max_blocks] : -1 - b;
+            s_wpg[b] = rep >= 0 ? (seq_lens[b] - 1) / CC_PAGE : 0x7fffffff;
+        }
         uint32_t bal[CC_MAXR];
 #pragma unroll
         for (int r = 0; r < CC_MAXR; ++r) bal[r] = __ballot_sync(0xffffffffu, rep == r);
@@ -102,6 +110,16 @@ __global__ void __launch_bounds__(kNormThreads) k_prologue(const int* __restrict
         s_goff[CC_MAXR] = off;
     }
     __syncthreads();
+    if (scan && b < batch && rep >= 0) {
+        // The attention kernel streams a row's pages before this step's appends are finished, up to the first page
+        // some row of the step writes.  For a lone decode row that is its last page; for the rows of a prompt chunk
+        // (one request, consecutive positions) it is the lowest page any of them appends to.
+        const int key = s_key[b];
+        int m = s_wpg[b];
+        for (int j = 0; j < batch; ++j)
+            if (s_key[j] == key) m = min(m, s_wpg[j]);
+        W.first_wr[b] = m;
+    }
     if (b < 256) {
         // rank of this row among the rows of its replica: ballot of its warp + the warps before it
         // (the ballots are taken again -- cheaper than keeping four of them alive across the barriers)
@@ -222,10 +240,11 @@ __global__ void __launch_bounds__(256) k_tap(const void* __restrict__ src, int w
 }  // namespace
 
 // ---- launchers ---------------------------------------------------------------------------------
-cudaError_t cc_launch_prologue(const int* assign, const int* seq_lens, int batch, const __nv_bfloat16* hidden,
-                               const CcDims& D, const CcLayerTable* tab, const CcWork& W, const CcLaunch& L,
-                               const CcStageOut& so) {
-    return cc_launch_kernel(k_prologue, dim3(batch), dim3(kNormThreads), 0, L, assign, seq_lens, batch, hidden, D, tab, W, so);
+cudaError_t cc_launch_prologue(const int* assign, const int* seq_lens, const int* block_table, int batch,
+                               const __nv_bfloat16* hidden, const CcDims& D, const CcLayerTable* tab, const CcWork& W,
+                               const CcLaunch& L, const CcStageOut& so) {
+    return cc_launch_kernel(k_prologue, dim3(batch), dim3(kNormThreads), 0, L, assign, seq_lens, block_table, batch, hidden, D, tab,
+                            W, so);
 }
 cudaError_t cc_launch_tap(const void* src, int which, int dim, const CcDims& D, const CcWork& W,
                           float* out_dev, int batch, cudaStream_t st) {

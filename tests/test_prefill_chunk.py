@@ -27,7 +27,14 @@ def _scenario():
     bt = np.vstack([base.block_table[:6]] + [base.block_table[6:7]] * N_CHUNK).astype(np.int32)
     seq = np.concatenate([base.seq_lens[:6], CACHED + 1 + np.arange(N_CHUNK)]).astype(np.int32)
     assign = np.concatenate([[0, 1, 0, 1, 0, 1], np.ones(N_CHUNK)]).astype(np.int32)    # a request lives on ONE replica
-    return I.StepInputs(hidden, base.k_pool, base.v_pool, bt, seq, base.n_pages), assign
+    # every cache slot the chunk is going to fill holds NaN beforehand: a row that read a position before the row of
+    # that position had appended it (the attention kernel streams pages ahead of the QKV kernel's end) shows up as NaN
+    k_pool, v_pool = base.k_pool.copy(), base.v_pool.copy()
+    for t in range(CACHED, CACHED + N_CHUNK):
+        pg = int(base.block_table[6, t // SHAPE.page])
+        k_pool[pg, :, t % SHAPE.page, :] = 0x7FC0
+        v_pool[pg, :, t % SHAPE.page, :] = 0x7FC0
+    return I.StepInputs(hidden, k_pool, v_pool, bt, seq, base.n_pages), assign
 
 
 def _one_by_one(st, assign):
