@@ -11,12 +11,14 @@ import pytest
 import oracle
 from paper_2607_04181_b200 import inputs as I
 
-SHAPE = I.LayerShape("chunk", 512, 8, 2, 128, 1408, 1e-5, 500000.0, 8, 40, 300)
-N_CHUNK, CACHED = 37, 90                      # the chunk covers positions 90..126: crosses pages 5|6 and 6|7
+SHAPE = I.LayerShape("chunk", 512, 8, 2, 128, 1408, 1e-5, 500000.0, 8, 40, 1800)
+# (tokens already cached, chunk length): positions 90..126 cross pages 5|6 and 6|7; the long one writes 13 pages behind
+# 94 pages of prefix, which the attention kernel streams while the QKV kernel is still appending
+CASES = [(90, 37), (1500, 200)]
 
 
-def _scenario():
-    """6 ordinary decode rows + one request whose 37-token chunk starts after 90 cached tokens."""
+def _scenario(CACHED, N_CHUNK):
+    """6 ordinary decode rows + one request whose N_CHUNK-token chunk starts after CACHED cached tokens."""
     base = I.make_step_inputs(SHAPE, 2401, 3401, batch=7, n_pages=7 * SHAPE.max_blocks,
                               contexts=np.array([41, 300, 77, 128, 255, 64, CACHED + N_CHUNK - 1], np.int32))
     rng = np.random.default_rng(2402)
@@ -39,14 +41,16 @@ def _scenario():
 
 def _one_by_one(st, assign):
     """The same tokens as single steps: the decode rows and token 0 of the chunk first, then one chunk token per step."""
-    steps = [np.arange(7)] + [np.array([6 + t]) for t in range(1, N_CHUNK)]
+    steps = [np.arange(7)] + [np.array([6 + t]) for t in range(1, st.hidden.shape[0] - 6)]
     return [(rows, I.StepInputs(st.hidden[rows], None, None, st.block_table[rows], st.seq_lens[rows], st.n_pages), assign[rows])
             for rows in steps]
 
 
-def test_oracle_chunk_step_equals_one_token_at_a_time_bitwise():
+@pytest.mark.parametrize("cached,n_chunk", CASES)
+def test_oracle_chunk_step_equals_one_token_at_a_time_bitwise(cached, n_chunk):
     w = I.make_weights(SHAPE, 1401)
-    st, assign = _scenario()
+    st, assign = _scenario(cached, n_chunk)
+    N_CHUNK = n_chunk
     chunk = oracle.layer_forward(SHAPE, w, st.hidden, st.k_pool, st.v_pool, st.block_table, st.seq_lens, assign, 2)
     kp, vp = st.k_pool, st.v_pool
     out = np.empty_like(st.hidden)
@@ -64,14 +68,15 @@ def test_oracle_chunk_step_equals_one_token_at_a_time_bitwise():
 
 
 @pytest.mark.gpu
-def test_gpu_chunk_step_matches_oracle_and_the_one_by_one_cache_bitwise():
+@pytest.mark.parametrize("cached,n_chunk", CASES)
+def test_gpu_chunk_step_matches_oracle_and_the_one_by_one_cache_bitwise(cached, n_chunk):
     import torch
     from paper_2607_04181_b200 import binding as B
     from paper_2607_04181_b200.harness import DeviceStep, Session
     from tests.test_gpu_parity import within
 
     w = I.make_weights(SHAPE, 1401)
-    st, assign = _scenario()
+    st, assign = _scenario(cached, n_chunk)
     ref = oracle.layer_forward(SHAPE, w, st.hidden, st.k_pool, st.v_pool, st.block_table, st.seq_lens, assign, 2, taps=True)
     batch = st.hidden.shape[0]
     with Session(SHAPE, w, max_batch=batch) as S:
