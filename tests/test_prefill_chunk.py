@@ -106,3 +106,65 @@ def test_gpu_chunk_step_matches_oracle_and_the_one_by_one_cache_bitwise(cached, 
         assert np.array_equal(kp1, kp) and np.array_equal(vp1, vp)
         within(I.bf16_bits_to_f32(seq_out), I.bf16_bits_to_f32(ref["out"]), "one-by-one output")
         assert B.cc_poll_device_error(S.ctx) == 0
+
+
+def _random_mixed_step(seed):
+    """1-3 requests with a prompt chunk each (random cached length and chunk length), 0-9 decode rows, a random small
+    layer shape and replica count; the rows of a request name one replica but need not be adjacent or in position
+    order; every slot a chunk will write holds NaN beforehand."""
+    rng = np.random.default_rng(seed)
+    dh, hkv, g = int(rng.choice([64, 128])), int(rng.choice([1, 2, 4, 8])), int(rng.integers(1, 5))
+    shape = I.LayerShape(f"mix{seed}", 64 * int(rng.integers(2, 9)), hkv * g, hkv, dh, 8 * int(rng.integers(8, 120)), 1e-5, 10000.0, 8, 0, 900)
+    R, n_req, n_dec = int(rng.integers(1, 5)), int(rng.integers(1, 4)), int(rng.integers(0, 10))
+    cached, chunk, dec_ctx = rng.integers(0, 700, n_req), rng.integers(1, 70, n_req), rng.integers(0, 800, n_dec)
+    base = I.make_step_inputs(shape, 5000 + seed, 6000 + seed, batch=n_req + n_dec, n_pages=(n_req + n_dec) * shape.max_blocks,
+                              contexts=np.concatenate([cached + chunk - 1, dec_ctx]).astype(np.int32))
+    k_pool, v_pool = base.k_pool.copy(), base.v_pool.copy()
+    bt, seq, ra = [], [], []
+    for r in range(n_req):
+        rep = int(rng.integers(0, R))
+        for t in range(int(cached[r]), int(cached[r] + chunk[r])):
+            bt.append(base.block_table[r]); seq.append(t + 1); ra.append(rep)
+            pg = int(base.block_table[r, t // shape.page])
+            k_pool[pg, :, t % shape.page, :] = 0x7FC0
+            v_pool[pg, :, t % shape.page, :] = 0x7FC0
+    for j in range(n_dec):
+        bt.append(base.block_table[n_req + j]); seq.append(int(dec_ctx[j]) + 1); ra.append(int(rng.integers(0, R)))
+    order = rng.permutation(len(seq)) if seed % 2 else np.arange(len(seq))
+    hidden = I._normal_bf16(rng, (len(seq), shape.hidden), 0.0, 1.0)
+    st = I.StepInputs(hidden, k_pool, v_pool, np.stack(bt)[order].astype(np.int32), np.array(seq, np.int32)[order], base.n_pages)
+    return shape, R, st, np.array(ra, np.int32)[order]
+
+
+@pytest.mark.gpu
+@pytest.mark.parametrize("seed", range(8))
+def test_gpu_random_mixed_prefill_and_decode_steps(seed):
+    import torch
+    from paper_2607_04181_b200 import binding as B
+    from paper_2607_04181_b200.harness import DeviceStep, Session
+    from tests.test_gpu_parity import within
+
+    shape, R, st, ra = _random_mixed_step(seed)
+    w = I.make_weights(shape, 7000 + seed)
+    ref = oracle.layer_forward(shape, w, st.hidden, st.k_pool, st.v_pool, st.block_table, st.seq_lens, ra, R, taps=True)
+    batch = st.hidden.shape[0]
+    with Session(shape, w, max_batch=batch) as S:
+        if R > 1:
+            S.scale(R)
+        step = DeviceStep(st, ra)
+        first = None
+        for rep in range(3):
+            step.reset(st)
+            S.forward(step)
+            torch.cuda.synchronize()
+            assert B.cc_poll_device_error(S.ctx) == 0
+            out, (kp, vp) = step.out_bits(), step.pools_bits()
+            within(I.bf16_bits_to_f32(out), I.bf16_bits_to_f32(ref["out"]), "mixed step output")
+            within(S.tap(B.CC_TAP_O, batch), ref["taps"]["o"], "mixed step attention output")
+            written = ~np.isnan(I.bf16_bits_to_f32(ref["k_pool"]))            # NaN left = slots nobody wrote (none attended)
+            within(I.bf16_bits_to_f32(kp)[written], I.bf16_bits_to_f32(ref["k_pool"])[written], "K cache")
+            within(I.bf16_bits_to_f32(vp)[written], I.bf16_bits_to_f32(ref["v_pool"])[written], "V cache")
+            if first is None:
+                first = (out, kp, vp)
+            else:                                                             # and the same bits every time
+                assert np.array_equal(out, first[0]) and np.array_equal(kp, first[1]) and np.array_equal(vp, first[2])
