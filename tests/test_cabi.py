@@ -40,6 +40,31 @@ def test_struct_layouts_match_the_header():
     assert B.cc_layer_desc.rms_eps.offset == 20 and B.cc_layer_desc.page_size.offset == 28
 
 
+def test_struct_layouts_match_what_the_c_compiler_sees(tmp_path):
+    """sizeof and every field offset of the structs that cross the boundary, as gcc lays them out from
+    include/cocoscale.h, against the ctypes mirrors in binding.py."""
+    import os
+    import subprocess
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    structs = {"cc_layer_desc": B.cc_layer_desc, "cc_layer_weights": B.cc_layer_weights, "cc_kv_pages": B.cc_kv_pages,
+               "cc_ctl_params": B.cc_ctl_params, "cc_ctl_instance": B.cc_ctl_instance, "cc_ctl_device": B.cc_ctl_device,
+               "cc_ctl_placement": B.cc_ctl_placement}
+    lines = ['#include <stdio.h>', '#include <stddef.h>', '#include "include/cocoscale.h"', 'int main(void) {']
+    for name, st in structs.items():
+        lines.append(f'  printf("{name} %zu\\n", sizeof({name}));')
+        for field, _ in st._fields_:
+            lines.append(f'  printf("{name}.{field} %zu\\n", offsetof({name}, {field}));')
+    lines += ['  return 0;', '}']
+    src, exe = tmp_path / "layout.c", tmp_path / "layout"
+    src.write_text("\n".join(lines))
+    subprocess.run(["gcc", "-std=c99", "-I", root, str(src), "-o", str(exe)], check=True)
+    seen = dict(l.split() for l in subprocess.run([str(exe)], check=True, stdout=subprocess.PIPE, text=True).stdout.splitlines())
+    for name, st in structs.items():
+        assert int(seen[name]) == ctypes.sizeof(st), name
+        for field, _ in st._fields_:
+            assert int(seen[f"{name}.{field}"]) == getattr(st, field).offset, f"{name}.{field}"
+
+
 def test_no_cpu_fallback_without_a_device():
     import torch
     if torch.cuda.is_available():
