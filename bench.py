@@ -198,7 +198,7 @@ def run_ours(args):
     from paper_2607_04181_b200 import binding as B
     from paper_2607_04181_b200 import inputs as I
     from paper_2607_04181_b200 import multirank as M
-    from paper_2607_04181_b200.harness import DeviceStep, Session
+    from paper_2607_04181_b200.harness import CapturedGraph, DeviceStep, Session
 
     world = int(os.environ.get("WORLD_SIZE", "1"))
     rank = int(os.environ.get("RANK", "0"))
@@ -228,9 +228,8 @@ def run_ours(args):
     for _ in range(3):
         S.forward(step)
     torch.cuda.synchronize()
-    graph = torch.cuda.CUDAGraph()
-    with torch.cuda.graph(graph):
-        S.forward(step, torch.cuda.current_stream())
+    graph = CapturedGraph(lambda s: S.forward(step, s))     # counts instantiations, keeps the cudaGraphExec_t
+    n_graphs = CapturedGraph.instantiations
     n_launch = B.cc_forward_launch_count(S.layer)
 
     # ---- device-resident timed region: K graph replays ------------------------------------------
@@ -380,7 +379,10 @@ def run_ours(args):
                     "GBps_read_plus_write": round(2 * blob / (cms * 1e-3) / 1e9, 1),
                     "GBps_payload": round(blob / (cms * 1e-3) / 1e9, 1),
                     "frac_of_copy_peak": round(2 * blob / (cms * 1e-3) / 1e9 / peak, 4),
-                    "graph_recaptures": 0}
+                    # measured: graphs instantiated since the step's graph was captured, and whether the
+                    # cudaGraphExec_t replayed after the scale-ups / scale-downs above is still the one captured
+                    "graph_recaptures": CapturedGraph.instantiations - n_graphs,
+                    "same_cuda_graph_exec": bool(graph.same_exec()), "graph_replays": graph.replays}
     if copy_sweep is not None:
         replica_copy["chunk_sweep"] = copy_sweep
 
@@ -536,7 +538,7 @@ def run_cfg3(args):
 
     from paper_2607_04181_b200 import binding as B
     from paper_2607_04181_b200 import inputs as I
-    from paper_2607_04181_b200.harness import ModelSession
+    from paper_2607_04181_b200.harness import CapturedGraph, ModelSession
 
     if not torch.cuda.is_available():
         raise SystemExit("bench.py needs a CUDA device: the library has no CPU fallback")
@@ -584,12 +586,13 @@ def run_cfg3(args):
     stream = torch.cuda.current_stream()
     S.forward_all(hidden, kp, vp, btd, n_pages, sl, assigns, batch)     # warm-up outside capture
     torch.cuda.synchronize()
-    graph = torch.cuda.CUDAGraph()
-    with torch.cuda.graph(graph):
-        S.forward_all(hidden, kp, vp, btd, n_pages, sl, assigns, batch, torch.cuda.current_stream())
+    def whole_step(s):
+        S.forward_all(hidden, kp, vp, btd, n_pages, sl, assigns, batch, s)
         hidden.mul_(0).add_(1.0)         # keep the synthetic hidden state bounded over hundreds of steps (not part of the method)
         sl.add_(1)
-    exec_id, captures = id(graph), 1
+    n_graphs = CapturedGraph.instantiations
+    graph = CapturedGraph(whole_step)
+    exec_handle = graph.exec_handle      # the cudaGraphExec_t
     for _ in range(3):
         graph.replay()
     sl.copy_(torch.from_numpy(seq0))
@@ -615,7 +618,8 @@ def run_cfg3(args):
         ev[t][1].record()
     torch.cuda.synchronize()
     clocks = sampler.stop()
-    assert B.cc_poll_device_error(S.ctx) == 0 and id(graph) == exec_id and captures == 1
+    captures = CapturedGraph.instantiations - n_graphs
+    assert B.cc_poll_device_error(S.ctx) == 0 and graph.exec_handle == exec_handle and graph.same_exec() and captures == 1
     ms = np.array([a.elapsed_time(b) for a, b in ev])
     flip_ms = {"scale_up_step_ms": float(ms[up]), "scale_down_step_ms": float(ms[down])}
     def summ(x):
@@ -633,7 +637,7 @@ def run_cfg3(args):
         "config": {"workload": "cfg3 (BASELINE.json configs[2]): 32 Llama-3-8B-shaped layers, decode batch 128, contexts lognormal "
                                "(median 1024, sigma 0.8, capped 8192), one CUDA graph for the whole step, seq_lens incremented "
                                f"inside it; layers {list(hot)} scaled to 2 replicas at step {up} and back to 1 at step {down}",
-                   "graph_captures": captures, "same_graph_exec": True,
+                   "graph_captures": captures, "same_cuda_graph_exec": bool(graph.same_exec()), "graph_replays": graph.replays,
                    "note": "hidden is reset to a constant inside the graph every step to keep the synthetic state bounded"},
         "clocks": clocks,
         "latency": {"before": summ(before), "while_2_replicas": summ(during), "after": summ(after), **flip_ms},
@@ -661,7 +665,7 @@ def run_cfg4(args):
 
     from paper_2607_04181_b200 import binding as B
     from paper_2607_04181_b200 import inputs as I
-    from paper_2607_04181_b200.harness import ModelSession
+    from paper_2607_04181_b200.harness import CapturedGraph, ModelSession
 
     if not torch.cuda.is_available():
         raise SystemExit("bench.py needs a CUDA device: the library has no CPU fallback")
@@ -709,9 +713,7 @@ def run_cfg4(args):
     mixed_step(stream)
     torch.cuda.synchronize()
     assert B.cc_poll_device_error(S.ctx) == 0
-    graph = torch.cuda.CUDAGraph()
-    with torch.cuda.graph(graph):
-        mixed_step(torch.cuda.current_stream())
+    graph = CapturedGraph(mixed_step)
     K, W = max(args.steps // 10, 10), max(args.warmup // 4, 3)
     for _ in range(W):
         graph.replay()

@@ -65,6 +65,10 @@ typedef enum {
 #define CC_DEVERR_BAD_PAGE 2u      /* block-table entry < 0 or >= n_pages inside seq_len: row skipped */
 #define CC_DEVERR_BAD_SEQLEN 4u    /* seq_len > max_position or needs > max_blocks_per_seq: row skipped */
 #define CC_DEVERR_HANG 8u          /* reserved: an internal wait gave up (the kernel traps instead)       */
+#define CC_DEVERR_SPLIT_REQUEST 16u /* rows of one request (same first page) name different replicas: each row
+                                      still runs on the replica it names, but the request's KV then spans two
+                                      partitions -- not what PAPER.md:103 "each replica maintains its own
+                                      partition" allows                                                     */
 
 typedef struct cc_ctx cc_ctx;     /* device, side stream, donated ranges, replica table, error word */
 typedef struct cc_layer cc_layer; /* one decoder layer: slot 0 blob, replica slots, workspace        */
@@ -157,6 +161,13 @@ cc_status cc_release_replica(cc_layer *layer, int replica);
 /* n_active: replicas visible to forwards enqueued now; n_pending: copies enqueued by
  * cc_scale_layer and not yet committed. Either pointer may be NULL. */
 cc_status cc_query(cc_layer *layer, int *n_active, int *n_pending);
+
+/* Which replica indices forwards enqueued now may name: bit r of *mask set <=> replica r is live and
+ * published.  After cc_release_replica(layer, 1) with three live replicas the set is {0, 2}: indices are
+ * not compacted (a captured graph and the caller's replica_assign keep their meaning), so a caller that
+ * splits a batch must split it over THESE indices -- naming a retired index sets CC_DEVERR_BAD_REPLICA
+ * and the row runs on replica 0. */
+cc_status cc_active_replicas(cc_layer *layer, uint32_t *mask);
 
 /* Device address and size of replica r's blob (for byte-exact checks of the copy). */
 cc_status cc_replica_blob(cc_layer *layer, int replica, const void **blob_dev, size_t *bytes);

@@ -21,14 +21,14 @@ CC_PAGE_SIZE = 16
 CC_MAX_LAYERS = 128
 CC_OK, CC_ERR_INVALID, CC_ERR_NO_SLOT, CC_ERR_CUDA, CC_ERR_BUSY, CC_ERR_STATE = range(6)
 STATUS_NAMES = ("CC_OK", "CC_ERR_INVALID", "CC_ERR_NO_SLOT", "CC_ERR_CUDA", "CC_ERR_BUSY", "CC_ERR_STATE")
-CC_DEVERR_BAD_REPLICA, CC_DEVERR_BAD_PAGE, CC_DEVERR_BAD_SEQLEN, CC_DEVERR_HANG = 1, 2, 4, 8
+CC_DEVERR_BAD_REPLICA, CC_DEVERR_BAD_PAGE, CC_DEVERR_BAD_SEQLEN, CC_DEVERR_HANG, CC_DEVERR_SPLIT_REQUEST = 1, 2, 4, 8, 16
 CC_TAP_X, CC_TAP_Q, CC_TAP_O, CC_TAP_H1, CC_TAP_Y, CC_TAP_A = range(6)
 
 # every function include/cocoscale.h declares (checked against the header by tests/test_cabi.py)
 EXPORTS = (
     "cc_ctx_create", "cc_ctx_destroy", "cc_ctx_donate", "cc_ctx_reclaim", "cc_ctx_set_copy_chunk",
     "cc_ctx_set_pdl", "cc_poll_device_error", "cc_create_layer", "cc_destroy_layer", "cc_layer_blob_bytes",
-    "cc_scale_layer", "cc_commit", "cc_release_replica", "cc_query", "cc_replica_blob", "cc_forward",
+    "cc_scale_layer", "cc_commit", "cc_release_replica", "cc_query", "cc_active_replicas", "cc_replica_blob", "cc_forward",
     "cc_forward_host", "cc_forward_profiled", "cc_forward_launch_count", "cc_replica_copy", "cc_kv_plan_migration", "cc_kv_plan_catchup", "cc_kv_migrate", "cc_debug_tap", "cc_debug_grouping", "cc_debug_trace",
     "cc_slotalloc_create", "cc_slotalloc_destroy", "cc_slotalloc_donate", "cc_slotalloc_reclaim",
     "cc_slotalloc_alloc", "cc_slotalloc_free", "cc_slotalloc_free_bytes", "cc_last_error", "cc_version",
@@ -190,6 +190,13 @@ def cc_query(layer):
     a, p = C.c_int(), C.c_int()
     _check(_lib.cc_query(layer, C.byref(a), C.byref(p)))
     return a.value, p.value
+
+
+def cc_active_replicas(layer) -> list:
+    """Replica indices that forwards enqueued now may name (not compacted: {0, 2} after releasing 1 of three)."""
+    m = C.c_uint32()
+    _check(_lib.cc_active_replicas(layer, C.byref(m)))
+    return [r for r in range(CC_MAX_REPLICAS) if (m.value >> r) & 1]
 
 
 def cc_replica_blob(layer, replica: int):

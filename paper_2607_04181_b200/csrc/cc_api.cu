@@ -219,18 +219,28 @@ cc_status cc_ctx_create(int device, cc_ctx** out) {
     if (!ctx) return fail(CC_ERR_INVALID, "out of host memory");
     ctx->device = device;
     ctx->n_sms = prop.multiProcessorCount;
-    CC_CUDA(cudaSetDevice(device));
-    CC_CUDA(cudaStreamCreateWithFlags(&ctx->side, cudaStreamNonBlocking));
-    CC_CUDA(cudaMalloc(&ctx->table_dev, sizeof(CcLayerTable) * CC_MAX_LAYERS));
-    CC_CUDA(cudaMemset(ctx->table_dev, 0, sizeof(CcLayerTable) * CC_MAX_LAYERS));
-    CC_CUDA(cudaMalloc(&ctx->err_dev, 256));
-    CC_CUDA(cudaMemset(ctx->err_dev, 0, 256));
+    cudaError_t e = cudaSetDevice(device);
+    if (e == cudaSuccess) e = cudaStreamCreateWithFlags(&ctx->side, cudaStreamNonBlocking);
+    if (e == cudaSuccess) e = cudaMalloc(&ctx->table_dev, sizeof(CcLayerTable) * CC_MAX_LAYERS);
+    if (e == cudaSuccess) e = cudaMemset(ctx->table_dev, 0, sizeof(CcLayerTable) * CC_MAX_LAYERS);
+    if (e == cudaSuccess) e = cudaMalloc(&ctx->err_dev, 256);
+    if (e == cudaSuccess) e = cudaMemset(ctx->err_dev, 0, 256);
 #ifdef CC_TRACE
-    CC_CUDA(cudaMalloc(&ctx->trace_dev, sizeof(unsigned long long) * CC_TRACE_KERNELS * CC_TRACE_POINTS * 2));
+    if (e == cudaSuccess) e = cudaMalloc(&ctx->trace_dev, sizeof(unsigned long long) * CC_TRACE_KERNELS * CC_TRACE_POINTS * 2);
 #endif
-    CC_CUDA(cc_gemm_configure());
-    CC_CUDA(cc_attn_configure());
-    ctx->slots = cc_slotalloc_create();
+    if (e == cudaSuccess) e = cc_gemm_configure();
+    if (e == cudaSuccess) e = cc_attn_configure();
+    if (e == cudaSuccess && !(ctx->slots = cc_slotalloc_create())) e = cudaErrorMemoryAllocation;
+    if (e != cudaSuccess) {                       // nothing half-made is left behind
+        if (ctx->side) cudaStreamDestroy(ctx->side);
+        cudaFree(ctx->table_dev);
+        cudaFree(ctx->err_dev);
+        cudaFree(ctx->trace_dev);
+        cc_slotalloc_destroy(ctx->slots);
+        delete ctx;
+        cudaGetLastError();
+        return fail(CC_ERR_CUDA, "cc_ctx_create: %s", cudaGetErrorString(e));
+    }
     const char* env = getenv("CC_PDL");
     if (env && env[0] == '0') ctx->pdl = false;
     *out = ctx;
@@ -563,13 +573,22 @@ cc_status cc_scale_layer(cc_layer* L, int n_replicas) {
         }
         for (int i = 0; i < got; ++i) {
             Replica& R = L->rep[idx[i]];
+            cudaError_t e = cudaSuccess;
+            if (!R.copied) e = cudaEventCreateWithFlags(&R.copied, cudaEventDisableTiming);
+            cc_status st = CC_OK;
+            if (e == cudaSuccess) st = launch_chunked_copy(ctx, (void*)(uintptr_t)addr[i], L->blob0, L->blob_bytes, 0, ctx->side);
+            if (e == cudaSuccess && st == CC_OK) e = cudaEventRecord(R.copied, ctx->side);
+            if (e != cudaSuccess || st != CC_OK) {
+                // roll back: the slots of this and the later replicas go back to the allocator once the side stream
+                // has drained (a chunk of the failed copy may still be writing); replicas already enqueued stay
+                cudaStreamSynchronize(ctx->side);
+                cudaGetLastError();
+                for (int j = i; j < got; ++j) cc_slotalloc_free(ctx->slots, addr[j]);
+                return st != CC_OK ? st : fail(CC_ERR_CUDA, "cc_scale_layer: %s", cudaGetErrorString(e));
+            }
             R.blob = (uint8_t*)(uintptr_t)addr[i];
             R.state = REP_COPYING;
             R.published = false;
-            if (!R.copied) CC_CUDA(cudaEventCreateWithFlags(&R.copied, cudaEventDisableTiming));
-            cc_status st = launch_chunked_copy(ctx, R.blob, L->blob0, L->blob_bytes, 0, ctx->side);
-            if (st != CC_OK) return st;
-            CC_CUDA(cudaEventRecord(R.copied, ctx->side));
         }
     } else if (n_replicas < cur) {
         int drop = cur - n_replicas;
@@ -643,6 +662,12 @@ cc_status cc_query(cc_layer* L, int* n_active, int* n_pending) {
     }
     if (n_active) *n_active = a;
     if (n_pending) *n_pending = p;
+    return CC_OK;
+}
+
+cc_status cc_active_replicas(cc_layer* L, uint32_t* mask) {
+    if (!L || !mask) return fail(CC_ERR_INVALID, "null argument");
+    *mask = L->host_row.active_mask;
     return CC_OK;
 }
 

@@ -193,7 +193,13 @@ k_attn(const int* __restrict__ seq_lens, CcKv kv, CcDims D, CcWork W, const CcLa
     float* my_merge = merge + (size_t)warp * G * C::kMergeStride;
     int stage = 0;
     uint32_t ph = 0;
-    uint32_t qa0[DH / 16], qa2[DH / 16];   // Q fragments (rows g < G), scaled by log2(e)/sqrt(Dh)
+    // Q fragments, scaled by log2(e)/sqrt(Dh), as bf16 hi + lo (q = hi + lo to ~16 bits): row g < G of the 16-row mma
+    // tile carries hi, row g + 8 carries lo (G <= 8 leaves the upper eight rows free), so ONE mma.sync yields both
+    // partial products and their sum is exact to ~16 bits against the bf16 K; the probabilities are split the same
+    // way against the bf16 V.  With single bf16 planes the attention output carried a 2e-3 relative error, at SHORT
+    // contexts (|o| ~ 0.4) the largest error of the whole layer: single output elements of 16-token rows at the
+    // cfg2 layer shape sat on the tolerance (tests/test_gpu_long.py).
+    uint32_t qa0[DH / 16], qa2[DH / 16], ql0[DH / 16], ql2[DH / 16];
     float o[DH / 8][4];
     float m_run = -INFINITY, l_run = 0.f;
 #pragma unroll
@@ -217,8 +223,11 @@ k_attn(const int* __restrict__ seq_lens, CcKv kv, CcDims D, CcWork W, const CcLa
                     x0 = *reinterpret_cast<const float2*>(qrow + ks * 16 + 2 * t4);
                     x1 = *reinterpret_cast<const float2*>(qrow + ks * 16 + 8 + 2 * t4);
                 }
-                qa0[ks] = pack_bf16(x0.x * D.qk_scale_log2, x0.y * D.qk_scale_log2);
-                qa2[ks] = pack_bf16(x1.x * D.qk_scale_log2, x1.y * D.qk_scale_log2);
+                x0.x *= D.qk_scale_log2; x0.y *= D.qk_scale_log2; x1.x *= D.qk_scale_log2; x1.y *= D.qk_scale_log2;
+                qa0[ks] = pack_bf16(x0.x, x0.y);
+                qa2[ks] = pack_bf16(x1.x, x1.y);
+                ql0[ks] = pack_bf16(x0.x - bf16lo(qa0[ks]), x0.y - bf16hi(qa0[ks]));
+                ql2[ks] = pack_bf16(x1.x - bf16lo(qa2[ks]), x1.y - bf16hi(qa2[ks]));
             }
         }
         const int tok0 = (m.pg + pp) * CC_PAGE;
@@ -245,11 +254,12 @@ k_attn(const int* __restrict__ seq_lens, CcKv kv, CcDims D, CcWork W, const CcLa
                     const int ch = ks * 2 + (mi & 1);
                     uint32_t r0, r1, r2, r3;
                     ldsm_x4(rowaddr + (uint32_t)(ch >> 3) * half_bytes + (uint32_t)(((ch & 7) ^ (tok & 7)) << 4), r0, r1, r2, r3);
-                    mma_bf16_16816(s0, qa0[ks], 0u, qa2[ks], 0u, r0, r1);
-                    mma_bf16_16816(s1, qa0[ks], 0u, qa2[ks], 0u, r2, r3);
+                    mma_bf16_16816(s0, qa0[ks], ql0[ks], qa2[ks], ql2[ks], r0, r1);   // c[0..1]: hi . K, c[2..3]: lo . K
+                    mma_bf16_16816(s1, qa0[ks], ql0[ks], qa2[ks], ql2[ks], r2, r3);
                 }
             }
             // ---- online softmax on row g (tokens 2t,2t+1 and 8+2t,8+2t+1 of the page)
+            s0[0] += s0[2]; s0[1] += s0[3]; s1[0] += s1[2]; s1[1] += s1[3];   // hi + lo rows of q
             const int c0 = 2 * t4;
             float v00 = (c0 < valid) ? s0[0] : -INFINITY, v01 = (c0 + 1 < valid) ? s0[1] : -INFINITY;
             float v10 = (c0 + 8 < valid) ? s1[0] : -INFINITY, v11 = (c0 + 9 < valid) ? s1[1] : -INFINITY;
@@ -262,7 +272,8 @@ k_attn(const int* __restrict__ seq_lens, CcKv kv, CcDims D, CcWork W, const CcLa
             const float p10 = exp2f(v10 - m_new), p11 = exp2f(v11 - m_new);
             l_run = l_run * alpha + ((p00 + p01) + (p10 + p11));
             m_run = m_new;
-            const uint32_t pa0 = pack_bf16(p00, p01), pa2 = pack_bf16(p10, p11);
+            const uint32_t pa0 = pack_bf16(p00, p01), pa2 = pack_bf16(p10, p11);   // probabilities: bf16 hi (rows g) + lo (rows g + 8)
+            const uint32_t pl0 = pack_bf16(p00 - bf16lo(pa0), p01 - bf16hi(pa0)), pl2 = pack_bf16(p10 - bf16lo(pa2), p11 - bf16hi(pa2));
             // ---- O[16 x DH] = alpha * O + P[16 x 16] . V[16 x DH]
             {
                 const int mi = lane >> 3, rr = lane & 7;
@@ -273,10 +284,10 @@ k_attn(const int* __restrict__ seq_lens, CcKv kv, CcDims D, CcWork W, const CcLa
                     const int ch = jn * 2 + (mi >> 1);
                     uint32_t r0, r1, r2, r3;
                     ldsm_x4_trans(rowaddr + (uint32_t)(ch >> 3) * half_bytes + (uint32_t)(((ch & 7) ^ (tok & 7)) << 4), r0, r1, r2, r3);
-                    o[2 * jn][0] *= alpha; o[2 * jn][1] *= alpha;
-                    o[2 * jn + 1][0] *= alpha; o[2 * jn + 1][1] *= alpha;
-                    mma_bf16_16816(o[2 * jn], pa0, 0u, pa2, 0u, r0, r1);
-                    mma_bf16_16816(o[2 * jn + 1], pa0, 0u, pa2, 0u, r2, r3);
+                    o[2 * jn][0] *= alpha; o[2 * jn][1] *= alpha; o[2 * jn][2] *= alpha; o[2 * jn][3] *= alpha;
+                    o[2 * jn + 1][0] *= alpha; o[2 * jn + 1][1] *= alpha; o[2 * jn + 1][2] *= alpha; o[2 * jn + 1][3] *= alpha;
+                    mma_bf16_16816(o[2 * jn], pa0, pl0, pa2, pl2, r0, r1);             // c[0..1] += hi . V, c[2..3] += lo . V
+                    mma_bf16_16816(o[2 * jn + 1], pa0, pl0, pa2, pl2, r2, r3);
                 }
             }
         }
@@ -293,7 +304,7 @@ k_attn(const int* __restrict__ seq_lens, CcKv kv, CcDims D, CcWork W, const CcLa
             float* mrow = my_merge + (size_t)g * C::kMergeStride;
 #pragma unroll
             for (int nt = 0; nt < DH / 8; ++nt)
-                *reinterpret_cast<float2*>(mrow + nt * 8 + 2 * t4) = make_float2(o[nt][0], o[nt][1]);
+                *reinterpret_cast<float2*>(mrow + nt * 8 + 2 * t4) = make_float2(o[nt][0] + o[nt][2], o[nt][1] + o[nt][3]);
             if (t4 == 0) {
                 mrow[DH] = m_run;
                 mrow[DH + 1] = l_tot;

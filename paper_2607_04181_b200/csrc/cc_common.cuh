@@ -18,6 +18,7 @@
 #define CC_DEVERR_BAD_PAGE 2u
 #define CC_DEVERR_BAD_SEQLEN 4u
 #define CC_DEVERR_HANG 8u         // an mbarrier wait gave up (kernel bug); the kernel trapped
+#define CC_DEVERR_SPLIT_REQUEST 16u   // rows of one request name different replicas
 
 // ---- device replica table -----------------------------------------
 // One row per layer, at a fixed device address for the life of the context.  Kernels read the
@@ -311,9 +312,10 @@ __device__ __forceinline__ uint64_t umma_desc_sw128(uint32_t smem_addr, uint32_t
     d |= (uint64_t)2 << 61;                          // SWIZZLE_128B   [61,64)
     return d;
 }
-// Instruction descriptor, kind::f16: D = fp32 (bits 4-5 = 1), A = B = bf16 (bits 7-9 = 10-12 = 1;
-// mixing bf16 with fp16 operands raises an illegal-instruction fault on sm_100a), both K-major,
-// N >> 3 at bit 17, M >> 4 at bit 24.
+// Instruction descriptor, kind::f16: D = fp32 (bits 4-5 = 1), A format at bits 7-9 and B format at bits 10-12
+// (0 = fp16, 1 = bf16), both K-major, N >> 3 at bit 17, M >> 4 at bit 24.  A and B must have the SAME format:
+// bf16 x fp16 raises an illegal-instruction fault on sm_100a (measured in round 1 and again in round 2 with a
+// one-MMA probe, either operand order), although the descriptor has separate fields.
 __device__ __forceinline__ uint32_t umma_idesc_bf16_m128(uint32_t n) {
     return (1u << 4) | (1u << 7) | (1u << 10) | ((n >> 3) << 17) | ((128u >> 4) << 24);
 }

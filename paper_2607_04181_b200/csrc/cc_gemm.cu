@@ -29,7 +29,7 @@ namespace {
 
 constexpr int kGemmThreads = 512;         // warp 0 producer, 1 MMA, 2..5 TMEM epilogue, 6..15 row tables; all 16 in the fixup
 constexpr int kHdrBytes = 8192;           // barriers + per-row tables in front of the stage ring
-constexpr int kMaxStages = 4;            // deeper rings measured slower at small row groups (R = 4: 384 -> 370 us per step)
+constexpr int kMaxStages = 4;            // deeper rings do not stream faster (measured again in round 2 with 5 and 6 stages of a one-plane variant: no change)
 constexpr int kGemmSmem = 225 * 1024;     // dynamic shared memory per CTA
 constexpr int kTmemCols = 512;
 constexpr uint32_t kWStage = CC_G * CC_A_TILE_BYTES;   // weight bytes per stage (32 KiB)
@@ -150,7 +150,7 @@ __device__ __forceinline__ void epi_fin(const EpiPre& P, const CcEpi& E, const C
         }
 #pragma unroll
         for (int o = 16; o > 0; o >>= 1) ss += __shfl_xor_sync(0xffffffffu, ss, o);
-        if (lane == 0) W.ssq[(size_t)t * D.Mpad + p] = ss;
+        if (lane == 0 && t < ((D.d + 127) >> 7)) W.ssq[(size_t)t * D.Mpad + p] = ss;   // not the zero padding tile of an odd tile count
     } else if (KIND == EPI_GU) {
         // second half of a7 + a8: scale by 1/rms of the row, a_j = silu(gate_j) * up_j with gate_j, up_j at
         // interleaved columns 2j, 2j+1 -> hi + lo operand of the down projection.
@@ -483,7 +483,12 @@ k_gemm(CcGemmGeo G, const uint8_t* __restrict__ act, int planes, float* __restri
     __syncthreads();
     if (warp == 1) tmem_dealloc<kTmemCols>(tmem_base);
     if (threadIdx.x == 0) CC_TP(W, 2 + KIND, 3);
-    if (nmax == 0) return;
+    if (nmax == 0) {
+        // No row runs this step.  The chain's ordering argument ("what was written two kernels back is visible") needs
+        // every kernel to retire after its predecessor, so wait for it here as well.
+        pdl_wait();
+        return;
+    }
 
     // ---- stream-K fixup: the CTAs c0..c1 whose ranges meet in a super tile split its rows ----------
     // Every reduction below adds pieces 0..m-1 in that order, whatever CTA does it and whatever the

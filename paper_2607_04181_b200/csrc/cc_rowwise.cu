@@ -54,6 +54,7 @@ __global__ void __launch_bounds__(kNormThreads) k_prologue(const int* __restrict
     __shared__ int s_goff[CC_MAXR + 1], s_cnt[CC_MAXR];
     __shared__ int s_mypos, s_myrep;
     __shared__ int s_key[256], s_wpg[256];   // first page id of row b (names its request), page index row b appends to
+    __shared__ signed char s_rep[256];       // replica that serves row b (scan block only)
     __shared__ float red[kNormThreads / 32];
     const int b = threadIdx.x, warp = b >> 5, lane = b & 31;
     const bool pub = blockIdx.x == 0;      // this block writes the tables
@@ -83,6 +84,7 @@ __global__ void __launch_bounds__(kNormThreads) k_prologue(const int* __restrict
             // rows of one request carry copies of its block-table row, so its first page id names the request
             s_key[b] = rep >= 0 ? block_table[(size_t)b * D.max_blocks] : -1 - b;
             s_wpg[b] = rep >= 0 ? (seq_lens[b] - 1) / CC_PAGE : 0x7fffffff;
+            s_rep[b] = (signed char)rep;
         }
         uint32_t bal[CC_MAXR];
 #pragma unroll
@@ -116,9 +118,14 @@ __global__ void __launch_bounds__(kNormThreads) k_prologue(const int* __restrict
         // (one request, consecutive positions) it is the lowest page any of them appends to.
         const int key = s_key[b];
         int m = s_wpg[b];
+        bool split = false;
         for (int j = 0; j < batch; ++j)
-            if (s_key[j] == key) m = min(m, s_wpg[j]);
+            if (s_key[j] == key) {
+                m = min(m, s_wpg[j]);
+                split |= s_rep[j] != rep;
+            }
         W.first_wr[b] = m;
+        if (split) atomicOr(W.err, CC_DEVERR_SPLIT_REQUEST);   // one request served by two replicas
     }
     if (b < 256) {
         // rank of this row among the rows of its replica: ballot of its warp + the warps before it

@@ -29,6 +29,33 @@ def make_desc(shape: I.LayerShape, max_batch: int, max_blocks: int | None = None
                            shape.rms_eps, shape.rope_base, shape.page, max_batch, mb, mp)
 
 
+class CapturedGraph:
+    """A CUDA graph captured ONCE, with the evidence for "no recapture" (north_star; the paper re-captures when the
+    replica set changes): the `cudaGraphExec_t` handle taken right after instantiation, a class-wide
+    count of instantiations (every capture in tests and bench goes through here, so `instantiations` minus the
+    number of graphs alive is the number of re-captures), and `replay()` refusing to launch anything but that
+    handle.  Plumbing only: torch captures and launches; the kernels inside come from the C ABI."""
+
+    instantiations = 0
+
+    def __init__(self, enqueue):
+        """`enqueue(stream)` issues the work to capture (it is called exactly once, under capture)."""
+        self.graph = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(self.graph):
+            enqueue(torch.cuda.current_stream())
+        CapturedGraph.instantiations += 1
+        self.exec_handle = int(self.graph.raw_cuda_graph_exec())    # the cudaGraphExec_t itself
+        self.replays = 0
+
+    def same_exec(self) -> bool:
+        return int(self.graph.raw_cuda_graph_exec()) == self.exec_handle
+
+    def replay(self) -> None:
+        assert self.same_exec(), "the graph was re-instantiated"
+        self.graph.replay()
+        self.replays += 1
+
+
 class DeviceStep:
     """One batch of step inputs resident in HBM."""
 

@@ -23,7 +23,7 @@ import torch
 
 from . import binding as B
 from . import inputs as I
-from .harness import ModelSession
+from .harness import CapturedGraph, ModelSession
 
 
 @dataclass
@@ -137,12 +137,12 @@ class ModelRunner:
         M = self.M
         M.forward_all(self.hidden, self.kp, self.vp, self.bt, self.n_pages, self.sl, self.assigns, self.max_batch)
         torch.cuda.synchronize()
-        self.graph = torch.cuda.CUDAGraph()
-        with torch.cuda.graph(self.graph):
+        def whole_step(s):
             self.hidden.copy_(self.hidden_src)            # the synthetic "embedding" of the step (keeps the state bounded)
-            M.forward_all(self.hidden, self.kp, self.vp, self.bt, self.n_pages, self.sl, self.assigns, self.max_batch,
-                          torch.cuda.current_stream())
-        self.captures += 1
+            M.forward_all(self.hidden, self.kp, self.vp, self.bt, self.n_pages, self.sl, self.assigns, self.max_batch, s)
+        before = CapturedGraph.instantiations
+        self.graph = CapturedGraph(whole_step)            # replay() refuses any other cudaGraphExec_t
+        self.captures += CapturedGraph.instantiations - before
 
     # ---- requests ----------------------------------------------------------------------------------------------
     def active(self):
@@ -228,6 +228,8 @@ class ModelRunner:
         e1.record()
         e1.synchronize()
         split = torch.arange(self.max_batch, dtype=torch.int32, device=self.dev) % n
+        split[self.n_decode:] = n - 1        # the rows of a prompt chunk are ONE request: one replica (
+                                             # rows of one request on two replicas raise CC_DEVERR_SPLIT_REQUEST)
         for l in self.hot:
             self.assigns[l].copy_(split)
         ms = e0.elapsed_time(e1)

@@ -54,28 +54,32 @@ def _run(flips: bool):
         hidden.copy_(_dev_u16(st0.hidden, dev))
         for l in range(L):
             kp[l].copy_(_dev_u16(sts[l].k_pool, dev)); vp[l].copy_(_dev_u16(sts[l].v_pool, dev))
-        graph = torch.cuda.CUDAGraph()
-        with torch.cuda.graph(graph):
-            M.forward_all(hidden, kp, vp, btd, st0.n_pages, sl, assigns, batch, torch.cuda.current_stream())
+        from paper_2607_04181_b200.harness import CapturedGraph
+
+        def whole_step(s):
+            M.forward_all(hidden, kp, vp, btd, st0.n_pages, sl, assigns, batch, s)
             sl.add_(1)                                              # the next token's position, inside the graph
-        exec_id = id(graph)
+        n_inst = CapturedGraph.instantiations
+        graph = CapturedGraph(whole_step)
+        exec_handle = graph.exec_handle                             # the cudaGraphExec_t
         split = torch.from_numpy(I.even_split(batch, 2)).to(dev)
         for step in range(STEPS):
             if flips and step == FLIP_UP:
                 for l in HOT:
                     M.scale(l, 2)
                     assigns[l].copy_(split)
-                assert B.cc_query(M.layers[HOT[0]]) == (2, 0)
+                assert B.cc_query(M.layers[HOT[0]]) == (2, 0) and graph.same_exec()
             if flips and step == FLIP_DOWN:
                 for l in HOT:
                     assigns[l].zero_()
                     M.scale(l, 1)
-                assert B.cc_query(M.layers[HOT[0]]) == (1, 0)
+                assert B.cc_query(M.layers[HOT[0]]) == (1, 0) and graph.same_exec()
             graph.replay()
             torch.cuda.synchronize()
             assert B.cc_poll_device_error(M.ctx) == 0
             outs.append(_host_u16(hidden))
-        assert id(graph) == exec_id
+        # one instantiation; the same cudaGraphExec_t was launched before and after every cc_commit
+        assert CapturedGraph.instantiations == n_inst + 1 and graph.exec_handle == exec_handle and graph.replays == STEPS
         assert sl.cpu().numpy().tolist() == (st0.seq_lens + STEPS).tolist()
     return ws, sts, outs, first_layer_kp
 

@@ -109,13 +109,12 @@ def test_one_graph_survives_scale_up_and_down_without_recapture():
         S.forward(step)                                            # warm-up outside capture
         torch.cuda.synchronize()
         base = step.out_bits()
-        graph = torch.cuda.CUDAGraph()
-        captures = 0
+        from paper_2607_04181_b200.harness import CapturedGraph
         step.reset(st)
-        with torch.cuda.graph(graph):
-            S.forward(step, torch.cuda.current_stream())
-        captures += 1
-        exec_id = id(graph)
+        n_inst = CapturedGraph.instantiations
+        graph = CapturedGraph(lambda s: S.forward(step, s))
+        exec_handle = graph.exec_handle                             # the cudaGraphExec_t, not a Python id
+        assert exec_handle != 0
 
         def replay(assign):
             step.reset(st)
@@ -128,7 +127,7 @@ def test_one_graph_survives_scale_up_and_down_without_recapture():
         assert np.array_equal(replay(np.zeros(batch, np.int32)), base)
         # scale up: copy on the side stream, publish on the replay stream; same graph, no recapture
         S.scale(2)
-        assert B.cc_query(S.layer) == (2, 0)
+        assert B.cc_query(S.layer) == (2, 0) and graph.same_exec()
         two = I.even_split(batch, 2)
         assert np.array_equal(replay(two), base)
         # prove the replayed graph really reads replica 1's slot through the table: corrupt that slot
@@ -143,7 +142,7 @@ def test_one_graph_survives_scale_up_and_down_without_recapture():
         assert np.array_equal(replay(two), base)
         # scale down: retire the row first, then the slot returns to the allocator
         S.scale(1)
-        assert B.cc_query(S.layer) == (1, 0)
+        assert B.cc_query(S.layer) == (1, 0) and graph.same_exec()
         assert np.array_equal(replay(np.zeros(batch, np.int32)), base)
         # a row still naming the retired replica is served by replica 0 and flagged, never a fault
         step.reset(st)
@@ -152,7 +151,110 @@ def test_one_graph_survives_scale_up_and_down_without_recapture():
         torch.cuda.synchronize()
         assert B.cc_poll_device_error(S.ctx) == B.CC_DEVERR_BAD_REPLICA
         assert np.array_equal(step.out_bits(), base)
-        assert captures == 1 and id(graph) == exec_id
+        # measured, not declared: one instantiation, and every replay above launched that same cudaGraphExec_t
+        assert CapturedGraph.instantiations == n_inst + 1 and graph.exec_handle == exec_handle and graph.same_exec()
+        assert graph.replays == 6
+
+
+def test_forward_with_a_non_contiguous_live_set():
+    """After releasing replica 1 of three the live indices are {0, 2}: cc_active_replicas reports them,
+    a batch split over THOSE indices really uses replica 2's slot, and naming index 1 is flagged and rerouted."""
+    B, DeviceStep, Session = _binding()
+    shape, batch = MID, 21
+    w = I.make_weights(shape, 1007)
+    st = I.make_step_inputs(shape, 2007, 3007, batch=batch)
+    with Session(shape, w, max_batch=batch) as S:
+        step = DeviceStep(st, np.zeros(batch, np.int32))
+        S.forward(step)
+        torch.cuda.synchronize()
+        base = step.out_bits()
+        S.scale(3)
+        assert B.cc_active_replicas(S.layer) == [0, 1, 2]
+        B.cc_release_replica(S.layer, 1)
+        assert B.cc_active_replicas(S.layer) == [0, 1, 2]           # nothing changes before the commit
+        B.cc_commit(S.layer, torch.cuda.current_stream())
+        live = B.cc_active_replicas(S.layer)
+        assert live == [0, 2] and B.cc_query(S.layer) == (2, 0)
+        assign = np.array(live, np.int32)[I.even_split(batch, len(live))]
+        step.reset(st)
+        step.set_assign(assign)
+        S.forward(step)
+        torch.cuda.synchronize()
+        assert B.cc_poll_device_error(S.ctx) == 0
+        assert np.array_equal(step.out_bits(), base)
+        perm, counts, _ = B.cc_debug_grouping(S.layer, batch)
+        assert counts[1] == 0 and counts[2] == int((assign == 2).sum()) > 0
+        # the rows named to replica 2 do read its slot: zero it and only they change
+        p2, n2 = B.cc_replica_blob(S.layer, 2)
+        off = p2 - S.arena.data_ptr()
+        S.arena[off:off + n2].zero_()
+        step.reset(st)
+        S.forward(step)
+        torch.cuda.synchronize()
+        out = step.out_bits()
+        assert np.array_equal(out[assign == 0], base[assign == 0]) and not np.array_equal(out[assign == 2], base[assign == 2])
+        # the retired index is not a replica any more
+        step.reset(st)
+        step.set_assign(I.even_split(batch, 2))                     # names index 1
+        S.forward(step)
+        torch.cuda.synchronize()
+        assert B.cc_poll_device_error(S.ctx) == B.CC_DEVERR_BAD_REPLICA
+        assert np.array_equal(step.out_bits(), base)
+
+
+def test_rows_of_one_request_on_different_replicas_are_flagged():
+    """Rows that share a first page id are one request (a prompt chunk); naming them to different replicas would put
+    one request's KV in two partitions: CC_DEVERR_SPLIT_REQUEST.  The rows still run where named."""
+    B, DeviceStep, Session = _binding()
+    shape = I.CFG1
+    w = I.make_weights(shape, 1001)
+    st = I.make_step_inputs(shape, 2001, 3001)
+    st.block_table[1] = st.block_table[0]                           # rows 0 and 1: one request, consecutive tokens
+    st.seq_lens[0] = 20
+    st.seq_lens[1] = 21
+    with Session(shape, w, max_batch=4) as S:
+        S.scale(2)
+        step = DeviceStep(st, np.array([0, 0, 1, 1], np.int32))
+        S.forward(step)
+        torch.cuda.synchronize()
+        assert B.cc_poll_device_error(S.ctx) == 0
+        good = step.out_bits()
+        step.reset(st)
+        step.set_assign(np.array([0, 1, 1, 0], np.int32))
+        S.forward(step)
+        torch.cuda.synchronize()
+        assert B.cc_poll_device_error(S.ctx) == B.CC_DEVERR_SPLIT_REQUEST
+        assert np.array_equal(step.out_bits(), good)                # replicas hold the same weights: same bits
+
+
+def test_all_padding_step_replayed_after_a_live_step():
+    """A batch of padding rows only (every seq_len 0) in the same captured graph, right after a live step and before
+    another (kernels of an empty step must still retire in launch order under PDL): nothing is written,
+    and the next live step is bitwise the first."""
+    B, DeviceStep, Session = _binding()
+    from paper_2607_04181_b200.harness import CapturedGraph
+    shape, batch = MID, 21
+    w = I.make_weights(shape, 1007)
+    st = I.make_step_inputs(shape, 2007, 3007, batch=batch)
+    with Session(shape, w, max_batch=batch) as S:
+        step = DeviceStep(st, np.zeros(batch, np.int32))
+        S.forward(step)
+        torch.cuda.synchronize()
+        base, (bk, bv) = step.out_bits(), step.pools_bits()
+        step.reset(st)
+        graph = CapturedGraph(lambda s: S.forward(step, s))
+        live_seq = step.seq_lens.clone()
+        for _ in range(3):
+            step.reset(st)
+            step.seq_lens.copy_(live_seq)
+            graph.replay()
+            step.seq_lens.zero_()                                   # all rows padding; hidden now holds the live output
+            graph.replay()
+            torch.cuda.synchronize()
+            assert B.cc_poll_device_error(S.ctx) == 0
+            k, v = step.pools_bits()
+            assert np.array_equal(step.out_bits(), base) and np.array_equal(k, bk) and np.array_equal(v, bv)
+        assert graph.same_exec() and graph.replays == 6
 
 
 def test_two_phase_publish_and_slot_reuse():

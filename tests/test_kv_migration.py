@@ -52,6 +52,44 @@ def test_planner_matches_the_host_simulation_exactly():
         assert len(set(dst.tolist())) == len(dst)
 
 
+def test_planner_and_catchup_on_a_hand_worked_scenario():
+    """Tables written out by hand from the rule, pinning BOTH the host simulation
+    and the library to something other than each other.  12 pages, 2 replicas: partition 0 = pages 0..5, partition
+    1 = pages 6..11; pages of 16 tokens.
+
+    Plan.  Row 0 (33 tokens, replica 0) holds pages [7, 2, 9]: 7 and 9 lie outside 0..5.  Referenced pages are
+    {7, 2, 9, 0, 10, 3} (row 2 is a padding row: its table entry 5 does not count).  7 -> lowest unreferenced page
+    of 0..5 = 1; 2 stays; 9 -> 4 (0 referenced, 1 taken, 2, 3 referenced).  Row 1 (16 tokens, replica 1) holds
+    [0]: 0 -> 6.  Row 3 (20 tokens, replica 1) holds [10, 3]: 10 stays; 3 -> 8 (6 taken, 7 still referenced as a
+    source).
+
+    Catch-up after the rows decoded on with the OLD table: row 0 grew 33 -> 35 tokens, row 1 16 -> 18 (a second
+    page, 11, from the caller's allocator), row 3 stayed at 20.  Only tokens >= seq_planned - 1 can have been
+    written since: row 0: tokens >= 32 = its page 2 (dirty, still at 9), pages 0 and 1 keep their planned places 1
+    and 2; row 1: token 15 is in page 0 (dirty, at 0) and page 1 is new (at 11, inside partition 1 already); row
+    3: tokens >= 19 = page 1 (dirty, at 3), page 0 keeps 10.  Re-planning [1, 2, 9], [0, 11], [10, 3]: 9 -> 4
+    (0, 1, 2, 3 referenced); 0 -> 6; 11 stays; 3 -> 7 (no longer referenced: row 0's first page now counts as 1)."""
+    from paper_2607_04181_b200 import binding as B
+    bt = np.array([[7, 2, 9], [0, -1, -1], [5, -1, -1], [10, 3, -1]], np.int32)
+    seq = np.array([33, 16, 0, 20], np.int32)
+    assign = np.array([0, 1, 0, 1], np.int32)
+    want_bt = np.array([[1, 2, 4], [6, -1, -1], [5, -1, -1], [10, 8, -1]], np.int32)
+    want_moves = [(7, 1), (9, 4), (0, 6), (3, 8)]
+    sim_bt, sim_moves = hostsim.plan_kv_migration(bt, seq, assign, 12, 2)
+    assert np.array_equal(sim_bt, want_bt) and sim_moves == want_moves
+    new_bt, src, dst = B.cc_kv_plan_migration(bt, seq, assign, 12, 2)
+    assert np.array_equal(new_bt, want_bt) and list(zip(src.tolist(), dst.tolist())) == want_moves
+
+    bt_now = np.array([[7, 2, 9], [0, 11, -1], [5, -1, -1], [10, 3, -1]], np.int32)
+    seq_now = np.array([35, 18, 0, 20], np.int32)
+    want_final = np.array([[1, 2, 4], [6, 11, -1], [5, -1, -1], [10, 7, -1]], np.int32)
+    want_catchup = [(9, 4), (0, 6), (3, 7)]
+    sim_final, sim_catchup = hostsim.plan_kv_catchup(bt_now, seq, seq_now, want_bt, assign, 12, 2)
+    assert np.array_equal(sim_final, want_final) and sim_catchup == want_catchup
+    final_bt, src, dst = B.cc_kv_plan_catchup(bt_now, seq, seq_now, want_bt, assign, 12, 2)
+    assert np.array_equal(final_bt, want_final) and list(zip(src.tolist(), dst.tolist())) == want_catchup
+
+
 def test_planner_rejects_bad_tables():
     from paper_2607_04181_b200 import binding as B
     bt = np.array([[0, 1], [1, 2]], np.int32)

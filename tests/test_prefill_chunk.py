@@ -86,8 +86,8 @@ def test_gpu_chunk_step_matches_oracle_and_the_one_by_one_cache_bitwise(cached, 
         torch.cuda.synchronize()
         assert B.cc_poll_device_error(S.ctx) == 0
         out, (kp, vp) = step.out_bits(), step.pools_bits()
-        within(I.bf16_bits_to_f32(out), I.bf16_bits_to_f32(ref["out"]), "chunk step output")
-        within(S.tap(B.CC_TAP_O, batch), ref["taps"]["o"], "chunk step attention output")
+        assert within(I.bf16_bits_to_f32(out), I.bf16_bits_to_f32(ref["out"]), "chunk step output") < 1e-2
+        assert within(S.tap(B.CC_TAP_O, batch), ref["taps"]["o"], "chunk step attention output") < 1e-2
         # the same tokens one by one on the GPU: the cache must come out bit for bit the same (per-row GEMM results do not
         # depend on the batch), the outputs within the tolerance of the same oracle values
         step.reset(st)
@@ -104,7 +104,7 @@ def test_gpu_chunk_step_matches_oracle_and_the_one_by_one_cache_bitwise(cached, 
             seq_out[rows] = step.out_bits()[:n]
         kp1, vp1 = step.pools_bits()
         assert np.array_equal(kp1, kp) and np.array_equal(vp1, vp)
-        within(I.bf16_bits_to_f32(seq_out), I.bf16_bits_to_f32(ref["out"]), "one-by-one output")
+        assert within(I.bf16_bits_to_f32(seq_out), I.bf16_bits_to_f32(ref["out"]), "one-by-one output") < 1e-2
         assert B.cc_poll_device_error(S.ctx) == 0
 
 
@@ -159,11 +159,11 @@ def test_gpu_random_mixed_prefill_and_decode_steps(seed):
             torch.cuda.synchronize()
             assert B.cc_poll_device_error(S.ctx) == 0
             out, (kp, vp) = step.out_bits(), step.pools_bits()
-            within(I.bf16_bits_to_f32(out), I.bf16_bits_to_f32(ref["out"]), "mixed step output")
-            within(S.tap(B.CC_TAP_O, batch), ref["taps"]["o"], "mixed step attention output")
+            assert within(I.bf16_bits_to_f32(out), I.bf16_bits_to_f32(ref["out"]), "mixed step output") < 1e-2
+            assert within(S.tap(B.CC_TAP_O, batch), ref["taps"]["o"], "mixed step attention output") < 1e-2
             written = ~np.isnan(I.bf16_bits_to_f32(ref["k_pool"]))            # NaN left = slots nobody wrote (none attended)
-            within(I.bf16_bits_to_f32(kp)[written], I.bf16_bits_to_f32(ref["k_pool"])[written], "K cache")
-            within(I.bf16_bits_to_f32(vp)[written], I.bf16_bits_to_f32(ref["v_pool"])[written], "V cache")
+            assert within(I.bf16_bits_to_f32(kp)[written], I.bf16_bits_to_f32(ref["k_pool"])[written], "K cache") < 1e-2
+            assert within(I.bf16_bits_to_f32(vp)[written], I.bf16_bits_to_f32(ref["v_pool"])[written], "V cache") < 1e-2
             if first is None:
                 first = (out, kp, vp)
             else:                                                             # and the same bits every time
