@@ -34,12 +34,13 @@ if ROOT not in sys.path:
 
 METRIC = "replicated decode-layer tokens/s"
 UNIT = "tokens/s"
-REF_ROWS_PER_STEP = 4       # --impl reference: rows of the batch the oracle computes per step
-CPU_BASELINE_ROWS = 64      # cpu_baseline leg of the default arm: the whole batch ...
-CPU_BASELINE_STEPS = 4      # ... four times (about 10 s of CPU work on 16 cores)
-# dram__bytes_read.sum + dram__bytes_write.sum of the gate/up GEMM (k_gemm<2>) per launch at R = 2, from the
-# ncu --set full capture summarised in profiles/r01q_full_R2.md (470 888 448 + 7 641 088 bytes)
-NCU_TRAFFIC_GATE_UP_R2 = 478529536
+CPU_BASELINE_ROWS = 64      # cpu_baseline leg and --impl reference alike: the whole batch per step ...
+CPU_BASELINE_STEPS = 4      # ... cpu_baseline: four steps (about 10 s of CPU work on 16 cores)
+REF_BUDGET_STEPS = 60       # --impl reference: up to this many (steps + warmup) run on the whole batch (~2 s each);
+                            # longer runs shrink the rows per step so the arm still ends within a few minutes
+# dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel come from this file, which
+# `python -m paper_2607_04181_b200.ncu_summary` writes from an `ncu --set full` export (with the commit it was taken at)
+NCU_TRAFFIC_FILE = os.path.join(ROOT, "profiles", "ncu_traffic.json")
 FALLBACK_HBM_GBS = 6650.0   # /opt/skills/guides/B200_PROFILING.md, used only if MEASURED_PEAKS.json is absent
 
 
@@ -63,6 +64,17 @@ def parse_args():
                          "cfg5: configs[4], the co-located serving loop (decode only)")
     ap.add_argument("--horizon", type=float, default=120.0, help="cfg5: seconds of synthetic arrivals")
     return ap.parse_args()
+
+
+def ncu_traffic(kernel: str, replicas: int):
+    """(bytes per launch, source) of `kernel` at `replicas` from profiles/ncu_traffic.json, or (None, None)."""
+    try:
+        with open(NCU_TRAFFIC_FILE) as f:
+            t = json.load(f)
+        e = t["kernels"][kernel][f"R{replicas}"]
+        return int(e["dram_bytes_read"]) + int(e["dram_bytes_write"]), f"ncu --set full, {e['summary']} (commit {t['commit']})"
+    except Exception:
+        return None, None
 
 
 def measured_peak():
@@ -163,6 +175,38 @@ def time_oracle(shape, w, st, rows: int, steps: int, warmup: int):
     return rows * steps / dt, dt / steps, oracle.num_threads()
 
 
+def cpu_baseline_extras(shape, w, st, cores: int) -> dict:
+    """BASELINE.md section 4's other CPU figures, each on a bounded sample: the oracle on ONE thread, the oracle on
+    cfg1 (the tiny layer), and a host memcpy beside the replica copy (oracle.replica_copy is memcpy)."""
+    import oracle
+    from paper_2607_04181_b200 import inputs as I
+    out = {}
+    oracle.set_num_threads(1)
+    try:
+        tps1, s1, _ = time_oracle(shape, w, st, 2, 1, 0)
+        out["one_thread"] = {"value": tps1, "unit": UNIT, "cores": 1, "sample": f"2 rows of the cfg2 batch, one layer step of {s1:.1f} s"}
+    finally:
+        oracle.set_num_threads(cores)
+    w1 = I.make_weights(I.CFG1, 1001)
+    st1 = I.make_step_inputs(I.CFG1, 2001, 3001)
+    a1 = I.even_split(I.CFG1.batch, 2)
+    n1 = 20
+    t0 = time.perf_counter()
+    for _ in range(n1):
+        oracle.layer_forward(I.CFG1, w1, st1.hidden, st1.k_pool, st1.v_pool, st1.block_table, st1.seq_lens, a1, 2)
+    out["cfg1"] = {"value": I.CFG1.batch * n1 / (time.perf_counter() - t0), "unit": UNIT, "cores": cores,
+                   "sample": f"{n1} steps of configs[0] (tiny layer, batch 4, 2 replicas)"}
+    buf = np.ones(256 << 20, np.uint8)
+    oracle.replica_copy(buf)
+    t0 = time.perf_counter()
+    for _ in range(3):
+        oracle.replica_copy(buf)
+    dt = (time.perf_counter() - t0) / 3
+    out["host_memcpy"] = {"GBps_payload": buf.nbytes / dt / 1e9, "GBps_read_plus_write": 2 * buf.nbytes / dt / 1e9,
+                          "sample": "oracle.replica_copy (memcpy, one thread) of 256 MiB, mean of 3"}
+    return out
+
+
 def run_reference(args):
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
@@ -171,8 +215,12 @@ def run_reference(args):
     shape = I.CFG2
     w = I.make_weights(shape, 1002)
     st = I.make_step_inputs(shape, 2002, 3002)
-    tps, s_per_step, cores = time_oracle(shape, w, st, REF_ROWS_PER_STEP, args.steps, args.warmup)
-    sample = (f"{REF_ROWS_PER_STEP} of the 64 rows of the cfg2 decode batch per step (full contexts, full layer), "
+    # the same sample as the default arm's cpu_baseline (all 64 rows of the batch per step) at the driver's K and W;
+    # a much longer run computes fewer rows per step so that it still ends within a few minutes, and says so
+    n_runs = max(1, args.steps + args.warmup)
+    rows = CPU_BASELINE_ROWS if n_runs <= REF_BUDGET_STEPS else max(1, CPU_BASELINE_ROWS * REF_BUDGET_STEPS // n_runs)
+    tps, s_per_step, cores = time_oracle(shape, w, st, rows, args.steps, args.warmup)
+    sample = (f"{'all ' if rows == shape.batch else ''}{rows} of the {shape.batch} rows of the cfg2 decode batch per step (full contexts, full layer), "
               f"oracle/cc_oracle.c as it stands, OpenMP over {cores} threads")
     line = {
         "impl": "reference", "metric": METRIC, "value": tps, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
@@ -285,10 +333,10 @@ def run_ours(args):
     dom = max(sb, key=sb.get)
     dom_ms = float(stage_ms[B.STAGE_NAMES.index(dom)])
     achieved = sb[dom] / (dom_ms * 1e-3) / 1e9
+    traffic, traffic_src = ncu_traffic(dom, R) if batch == I.CFG2.batch else (None, None)
     roofline = {"bound": "hbm", "kernel": dom, "achieved": round(achieved, 1), "peak": peak, "unit": "GB/s",
                 "frac": round(achieved / peak, 4),
-                "traffic": NCU_TRAFFIC_GATE_UP_R2 if (R == 2 and dom == "gemm_gate_up") else None,
-                "traffic_source": "ncu --set full, profiles/r01q_full_R2.md" if (R == 2 and dom == "gemm_gate_up") else None,
+                "traffic": traffic, "traffic_source": traffic_src,
                 "peak_source": peak_src,
                 "kernel_ms": round(dom_ms, 5), "algorithmic_bytes": sb[dom],
                 "how": f"mean of {n_prof} launches, CUDA events around the kernel on its stream (cc_forward_profiled)"}
@@ -492,6 +540,7 @@ def run_ours(args):
         cpu = {"value": tps, "unit": UNIT, "cores": cores, "kind": "oracle",
                "sample": f"all {min(CPU_BASELINE_ROWS, batch)} rows of the same cfg2 batch, {CPU_BASELINE_STEPS} full layer steps of "
                          f"{s_per_step:.1f} s each, oracle/cc_oracle.c (OpenMP)"}
+        cpu.update(cpu_baseline_extras(shape, w, st, cores))
     S.close()
 
     if rank == 0:

@@ -301,7 +301,8 @@ def simulate(A: ModelRunner, Bm: ModelRunner, arrivals, burst_hi: int, burst_lo:
     def pct(x, p):
         return float(np.percentile(x, p)) if len(x) else None
 
-    out = {"clock_s": now, "steps": steps, "requests": {k: len(v) for k, v in done.items()},
+    out = {"clock": "simulated: the sum of the measured device times of the steps (no host time, no queueing outside a step)",
+           "clock_s": now, "steps": steps, "requests": {k: len(v) for k, v in done.items()},
            "unfinished": {k: len(queue[k]) + len(m.active()) for k, m in (("A", A), ("B", Bm))},
            "graph_captures": {"A": A.captures, "B": Bm.captures}}
     for name, m in (("A", A), ("B", Bm)):
