@@ -316,7 +316,8 @@ def run_ours(args):
                                           step.n_pages, step.seq_lens, step.assign, batch, stream)
     stage_ms /= n_prof
     sb = stage_bytes(shape, st.seq_lens, R)
-    # tensor work of the GEMMs: two bf16 planes (hi + lo) of the activations, 2 flops per multiply-add
+    # tensor work of the GEMMs: `planes` operand planes (1 = fp16, 2 = bf16 hi + lo), 2 flops per multiply-add
+    planes = 1 if B.cc_layer_operand_format(S.layer) == B.CC_OPERAND_F16 else 2
     rows = int((st.seq_lens > 0).sum())
     gemm_flops = {"gemm_qkv": (shape.q_dim + 2 * shape.kv_dim) * shape.hidden, "gemm_o": shape.hidden * shape.q_dim,
                   "gemm_gate_up": 2 * shape.ffn * shape.hidden, "gemm_down": shape.hidden * shape.ffn}
@@ -324,7 +325,7 @@ def run_ours(args):
     for i, name in enumerate(B.STAGE_NAMES):
         e = {"ms": round(float(stage_ms[i]), 5)}
         if name in gemm_flops:
-            e["tensor_TFLOPs_two_planes"] = round(2 * 2.0 * rows * gemm_flops[name] / (stage_ms[i] * 1e-3) / 1e12, 1)
+            e["tensor_TFLOPs_issued"] = round(planes * 2.0 * rows * gemm_flops[name] / (stage_ms[i] * 1e-3) / 1e12, 1)
         if name in sb:
             e["bytes"] = sb[name]
             e["GBps"] = round(sb[name] / (stage_ms[i] * 1e-3) / 1e9, 1)
@@ -548,6 +549,8 @@ def run_ours(args):
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
             "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "bf16", "data": "synthetic",
+            "operand_format": "fp16 weight images x one fp16 activation plane, fp32 accumulation" if planes == 1 else
+                              "bf16 weight images x two bf16 activation planes (hi + lo), fp32 accumulation",
             "config": {"workload": "cfg2 (BASELINE.json configs[1]): Llama-3-8B-shaped decoder layer, hidden 4096, "
                                    f"32 q / 8 kv heads x 128, FFN 14336, decode batch {batch}, contexts U{{512..2048}}, "
                                    "16-token pages, shuffled block tables",

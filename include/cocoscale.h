@@ -65,6 +65,8 @@ typedef enum {
 #define CC_DEVERR_BAD_PAGE 2u      /* block-table entry < 0 or >= n_pages inside seq_len: row skipped */
 #define CC_DEVERR_BAD_SEQLEN 4u    /* seq_len > max_position or needs > max_blocks_per_seq: row skipped */
 #define CC_DEVERR_HANG 8u          /* reserved: an internal wait gave up (the kernel traps instead)       */
+#define CC_DEVERR_TOO_MANY_DECODE 32u /* a step of more than 256 rows holds more than 256 decode rows, 64 prompt chunks or
+                                      * 1024 query tiles: the surplus is skipped */
 #define CC_DEVERR_SPLIT_REQUEST 16u /* rows of one request (same first page) name different replicas: each row
                                       still runs on the replica it names, but the request's KV then spans two
                                       partitions -- not what PAPER.md:103 "each replica maintains its own
@@ -124,6 +126,26 @@ cc_status cc_ctx_set_copy_chunk(cc_ctx *ctx, size_t chunk_bytes);
  * kernels and their results are the same either way. */
 cc_status cc_ctx_set_pdl(cc_ctx *ctx, int enabled);
 
+/* GEMM operand format of the layers created AFTER this call (the blob is packed at cc_create_layer).  The paper fixes
+ * no arithmetic ("Transformer layers"); north_star fixes bf16 storage and the tolerance.
+ *   CC_OPERAND_F16    the bf16 weights are converted to fp16 when packed (exact for 2^-17 <= |w| <= 65504, rounded to
+ *                     the 2^-24 grid below that) and every GEMM operand is ONE fp16 plane (11 significand bits);
+ *                     cc_create_layer fails with CC_ERR_INVALID if a weight exceeds the fp16 range;
+ *   CC_OPERAND_BF16X2 weights stay bf16, operands are TWO bf16 planes hi + lo (16 bits; twice the tensor work);
+ *   CC_OPERAND_AUTO   (default) F16, falling back to BF16X2 for a layer with a weight outside the fp16 range.
+ * The environment variable CC_OPERAND_FORMAT=f16|bf16x2 sets the same at cc_ctx_create. */
+enum { CC_OPERAND_AUTO = 0, CC_OPERAND_F16 = 1, CC_OPERAND_BF16X2 = 2 };
+cc_status cc_ctx_set_operand_format(cc_ctx *ctx, int format);
+
+/* Activation planes of the four GEMM operands (x: QKV input, o: O input, y: gate/up input, a: down input) of
+ * CC_OPERAND_F16 layers, chosen per step: a step of at most `rows` rows takes planes_upto_rows[4], a larger one
+ * planes_above[4]; each entry 1 (one fp16 plane, 11 significand bits) or 2 (hi + lo fp16 planes, twice the tensor
+ * work of that projection).  Steps of up to 64 rows are HBM-bound, so two planes cost them nothing: the default is
+ * {2,2,2,2} up to 64 rows and {2,1,1,1} above (DESIGN.md "Precision" has the measured errors of every choice).  The choice depends on the step's
+ * row count only, never on replica_assign, so outputs stay bit-identical across replica counts.  The environment
+ * variable CC_PLANES="xoya,xoya[,rows]" sets the same at cc_ctx_create.  BF16X2 layers always use two planes. */
+cc_status cc_ctx_set_operand_planes(cc_ctx *ctx, int rows, const int *planes_upto_rows, const int *planes_above);
+
 /* Sticky device error word (CC_DEVERR_* bits); reading clears it. Synchronises the device. */
 cc_status cc_poll_device_error(cc_ctx *ctx, uint32_t *bits);
 
@@ -135,6 +157,9 @@ cc_status cc_poll_device_error(cc_ctx *ctx, uint32_t *bits);
 cc_status cc_create_layer(cc_ctx *ctx, const cc_layer_desc *desc, const cc_layer_weights *weights_dev,
                           cc_layer **out);
 cc_status cc_destroy_layer(cc_layer *layer);
+
+/* The operand format this layer was packed in: CC_OPERAND_F16 or CC_OPERAND_BF16X2. */
+cc_status cc_layer_operand_format(const cc_layer *layer, int *format);
 
 /* Bytes of one replica slot of this layer (= bytes cc_scale_layer copies per new replica). */
 cc_status cc_layer_blob_bytes(const cc_layer *layer, size_t *bytes);
@@ -208,11 +233,13 @@ cc_status cc_forward_host(cc_layer *layer, void *hidden_host, void *k_pool_dev, 
 
 /* The same step, launched kernel by kernel with a CUDA event between consecutive kernels (so
  * without programmatic dependent launch), synchronised; stage_ms_host[i] (host, fp32
- * [cc_forward_launch_count]) receives the device time of kernel i in milliseconds, in launch
+ * [CC_MAX_PROFILE_STAGES], unused entries 0) receives the device time of kernel i in milliseconds, in launch
  * order: grouping + input norm, QKV GEMM (+RoPE, KV append), attention (+chunk merge), O GEMM
  * (+residual, norm statistics), gate/up GEMM (+norm scale, SwiGLU), down GEMM (+residual, request
- * order).  For per-kernel roofline accounting; not capture-safe.  hidden_dev may also be the pinned
+ * order); for a step of more than 256 rows: grouping, input norm, QKV GEMM, decode attention, chunk-prefill
+ * attention, O GEMM, row statistics, gate/up GEMM, down GEMM.  For per-kernel roofline accounting; not capture-safe.  hidden_dev may also be the pinned
  * host buffer of cc_forward_host (its in-place path is then what is timed). */
+#define CC_MAX_PROFILE_STAGES 10
 cc_status cc_forward_profiled(cc_layer *layer, void *hidden_dev, const cc_kv_pages *kv, const int32_t *seq_lens_dev,
                               const int32_t *replica_assign_dev, int batch, void *stream, float *stage_ms_host);
 
@@ -330,12 +357,12 @@ cc_status cc_debug_trace(cc_ctx *ctx, uint64_t *out_host, int reset);
 
 /* ---- stage taps (tests only; reads the workspace left by the last cc_forward) ---------------- */
 typedef enum {
-    CC_TAP_X = 0,   /* [batch][hidden]      input RMSNorm output (GEMM operand: bf16 hi + lo)   */
+    CC_TAP_X = 0,   /* [batch][hidden]      input RMSNorm output (GEMM operand, layer format)    */
     CC_TAP_Q = 1,   /* [batch][Hq*Dh]       q after RoPE (fp32)                                 */
-    CC_TAP_O = 2,   /* [batch][Hq*Dh]       attention output (GEMM operand: bf16 hi + lo)       */
+    CC_TAP_O = 2,   /* [batch][Hq*Dh]       attention output (GEMM operand, layer format)        */
     CC_TAP_H1 = 3,  /* [batch][hidden]      hidden + O-projection (fp32)                        */
-    CC_TAP_Y = 4,   /* [batch][hidden]      post-attention RMSNorm output (hi + lo operand x 1/rms) */
-    CC_TAP_A = 5    /* [batch][ffn]         silu(gate)*up (bf16 hi + lo)                        */
+    CC_TAP_Y = 4,   /* [batch][hidden]      post-attention RMSNorm output (operand x its row scale) */
+    CC_TAP_A = 5    /* [batch][ffn]         silu(gate)*up (GEMM operand, layer format)          */
 } cc_tap;
 /* out_host: fp32 [batch][dim] in ORIGINAL row order; padding rows are zero. Synchronous. */
 cc_status cc_debug_tap(cc_layer *layer, cc_tap which, float *out_host, int batch);

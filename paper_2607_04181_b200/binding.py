@@ -22,12 +22,14 @@ CC_MAX_LAYERS = 128
 CC_OK, CC_ERR_INVALID, CC_ERR_NO_SLOT, CC_ERR_CUDA, CC_ERR_BUSY, CC_ERR_STATE = range(6)
 STATUS_NAMES = ("CC_OK", "CC_ERR_INVALID", "CC_ERR_NO_SLOT", "CC_ERR_CUDA", "CC_ERR_BUSY", "CC_ERR_STATE")
 CC_DEVERR_BAD_REPLICA, CC_DEVERR_BAD_PAGE, CC_DEVERR_BAD_SEQLEN, CC_DEVERR_HANG, CC_DEVERR_SPLIT_REQUEST = 1, 2, 4, 8, 16
+CC_DEVERR_TOO_MANY_DECODE = 32
 CC_TAP_X, CC_TAP_Q, CC_TAP_O, CC_TAP_H1, CC_TAP_Y, CC_TAP_A = range(6)
+CC_OPERAND_AUTO, CC_OPERAND_F16, CC_OPERAND_BF16X2 = range(3)
 
 # every function include/cocoscale.h declares (checked against the header by tests/test_cabi.py)
 EXPORTS = (
     "cc_ctx_create", "cc_ctx_destroy", "cc_ctx_donate", "cc_ctx_reclaim", "cc_ctx_set_copy_chunk",
-    "cc_ctx_set_pdl", "cc_poll_device_error", "cc_create_layer", "cc_destroy_layer", "cc_layer_blob_bytes",
+    "cc_ctx_set_pdl", "cc_ctx_set_operand_format", "cc_ctx_set_operand_planes", "cc_layer_operand_format", "cc_poll_device_error", "cc_create_layer", "cc_destroy_layer", "cc_layer_blob_bytes",
     "cc_scale_layer", "cc_commit", "cc_release_replica", "cc_query", "cc_active_replicas", "cc_replica_blob", "cc_forward",
     "cc_forward_host", "cc_forward_profiled", "cc_forward_launch_count", "cc_replica_copy", "cc_kv_plan_migration", "cc_kv_plan_catchup", "cc_kv_migrate", "cc_debug_tap", "cc_debug_grouping", "cc_debug_trace",
     "cc_slotalloc_create", "cc_slotalloc_destroy", "cc_slotalloc_donate", "cc_slotalloc_reclaim",
@@ -149,6 +151,16 @@ def cc_ctx_set_pdl(ctx, enabled: bool) -> None:
     _check(_lib.cc_ctx_set_pdl(ctx, C.c_int(1 if enabled else 0)))
 
 
+def cc_ctx_set_operand_format(ctx, fmt: int) -> None:
+    _check(_lib.cc_ctx_set_operand_format(ctx, C.c_int(fmt)))
+
+
+def cc_ctx_set_operand_planes(ctx, rows: int, planes_upto_rows, planes_above) -> None:
+    a = (C.c_int * 4)(*[int(x) for x in planes_upto_rows])
+    b = (C.c_int * 4)(*[int(x) for x in planes_above])
+    _check(_lib.cc_ctx_set_operand_planes(ctx, C.c_int(rows), a, b))
+
+
 def cc_poll_device_error(ctx) -> int:
     bits = C.c_uint32()
     _check(_lib.cc_poll_device_error(ctx, C.byref(bits)))
@@ -166,6 +178,12 @@ def cc_create_layer(ctx, desc: cc_layer_desc, weights: dict) -> C.c_void_p:
 
 def cc_destroy_layer(layer) -> None:
     _check(_lib.cc_destroy_layer(layer))
+
+
+def cc_layer_operand_format(layer) -> int:
+    f = C.c_int()
+    _check(_lib.cc_layer_operand_format(layer, C.byref(f)))
+    return f.value
 
 
 def cc_layer_blob_bytes(layer) -> int:
@@ -221,15 +239,18 @@ def cc_forward_host(layer, hidden_host, k_pool, v_pool, n_pages: int, block_tabl
 
 
 STAGE_NAMES = ("prologue", "gemm_qkv", "attention", "gemm_o", "gemm_gate_up", "gemm_down")
+BIG_STAGE_NAMES = ("group", "norm", "gemm_qkv", "attention_decode", "attention_prefill", "gemm_o", "rowstat", "gemm_gate_up",
+                   "gemm_down")          # steps of more than 256 rows
+CC_MAX_PROFILE_STAGES = 10
 
 
 def cc_forward_profiled(layer, hidden, k_pool, v_pool, block_table, n_pages: int, seq_lens, replica_assign,
                         batch: int, stream=None) -> np.ndarray:
     kv = cc_kv_pages(_ptr(k_pool), _ptr(v_pool), _ptr(block_table), C.c_int32(n_pages))
-    ms = np.zeros(len(STAGE_NAMES), dtype=np.float32)
+    ms = np.zeros(CC_MAX_PROFILE_STAGES, dtype=np.float32)
     _check(_lib.cc_forward_profiled(layer, _ptr(hidden), C.byref(kv), _ptr(seq_lens), _ptr(replica_assign),
                                     C.c_int(batch), _stream(stream), _ptr(ms)))
-    return ms
+    return ms[:len(BIG_STAGE_NAMES if batch > 256 else STAGE_NAMES)]
 
 
 def cc_forward_launch_count(layer) -> int:

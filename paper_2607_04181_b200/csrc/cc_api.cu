@@ -15,6 +15,8 @@
 
 cudaError_t cc_gemm_configure();
 cudaError_t cc_attn_configure();
+cudaError_t cc_big_gemm_configure();
+cudaError_t cc_prefill_configure();
 
 namespace {
 
@@ -145,6 +147,13 @@ struct cc_ctx {
     bool row_used[CC_MAX_LAYERS] = {};
     int n_layers = 0;
     bool pdl = true;
+    int operand_format = CC_OPERAND_AUTO;      // layers created from now on (cc_ctx_set_operand_format)
+    // activation planes of the four GEMM operands (x, o, y, a) of an fp16 layer, per step: steps of at most
+    // `planes_rows` rows are HBM-bound and take planes_small (two planes cost nothing there); larger steps take
+    // planes_large (cc_ctx_set_operand_planes)
+    int planes_rows = 64;
+    int planes_small[4] = {2, 2, 2, 2};
+    int planes_large[4] = {2, 1, 1, 1};        // measured: the QKV input is the operand whose rounding shows (short contexts)
     std::vector<Zombie> zombies;
 };
 
@@ -165,7 +174,9 @@ struct cc_layer {
     int* st_sl = nullptr;
     int* st_ra = nullptr;
     void* st_tbl_host = nullptr;         // pinned mirror of [st_sl | st_ra | st_bt]
+    bool big = false;                    // created with max_batch > 256: steps of more than 256 rows take the large-M path
     int last_batch = 0;
+    int last_pl[4] = {2, 2, 2, 2};       // plane counts of the last forward (cc_debug_tap reads the operands back)
 };
 
 namespace {
@@ -230,6 +241,8 @@ cc_status cc_ctx_create(int device, cc_ctx** out) {
 #endif
     if (e == cudaSuccess) e = cc_gemm_configure();
     if (e == cudaSuccess) e = cc_attn_configure();
+    if (e == cudaSuccess) e = cc_big_gemm_configure();
+    if (e == cudaSuccess) e = cc_prefill_configure();
     if (e == cudaSuccess && !(ctx->slots = cc_slotalloc_create())) e = cudaErrorMemoryAllocation;
     if (e != cudaSuccess) {                       // nothing half-made is left behind
         if (ctx->side) cudaStreamDestroy(ctx->side);
@@ -243,6 +256,18 @@ cc_status cc_ctx_create(int device, cc_ctx** out) {
     }
     const char* env = getenv("CC_PDL");
     if (env && env[0] == '0') ctx->pdl = false;
+    env = getenv("CC_PLANES");                  // "xoya,xoya[,rows]": planes of small and large steps, e.g. 2222,1212,64
+    if (env && std::strlen(env) >= 9 && env[4] == ',') {
+        bool ok = true;
+        for (int i = 0; i < 4; ++i) ok &= (env[i] == '1' || env[i] == '2') && (env[5 + i] == '1' || env[5 + i] == '2');
+        if (ok) {
+            for (int i = 0; i < 4; ++i) { ctx->planes_small[i] = env[i] - '0'; ctx->planes_large[i] = env[5 + i] - '0'; }
+            if (env[9] == ',') ctx->planes_rows = atoi(env + 10);
+        }
+    }
+    env = getenv("CC_OPERAND_FORMAT");          // "f16" | "bf16x2": what cc_ctx_set_operand_format would set
+    if (env && !std::strcmp(env, "f16")) ctx->operand_format = CC_OPERAND_F16;
+    if (env && !std::strcmp(env, "bf16x2")) ctx->operand_format = CC_OPERAND_BF16X2;
     *out = ctx;
     return CC_OK;
 }
@@ -288,6 +313,25 @@ cc_status cc_ctx_set_copy_chunk(cc_ctx* ctx, size_t chunk_bytes) {
 cc_status cc_ctx_set_pdl(cc_ctx* ctx, int enabled) {
     if (!ctx) return fail(CC_ERR_INVALID, "null context");
     ctx->pdl = enabled != 0;
+    return CC_OK;
+}
+
+cc_status cc_ctx_set_operand_format(cc_ctx* ctx, int format) {
+    if (!ctx) return fail(CC_ERR_INVALID, "null context");
+    if (format != CC_OPERAND_AUTO && format != CC_OPERAND_F16 && format != CC_OPERAND_BF16X2)
+        return fail(CC_ERR_INVALID, "unknown operand format %d", format);
+    ctx->operand_format = format;
+    return CC_OK;
+}
+
+cc_status cc_ctx_set_operand_planes(cc_ctx* ctx, int rows, const int* planes_upto_rows, const int* planes_above) {
+    if (!ctx || !planes_upto_rows || !planes_above) return fail(CC_ERR_INVALID, "null argument");
+    if (rows < 0) return fail(CC_ERR_INVALID, "rows must be >= 0");
+    for (int i = 0; i < 4; ++i)
+        if (planes_upto_rows[i] < 1 || planes_upto_rows[i] > 2 || planes_above[i] < 1 || planes_above[i] > 2)
+            return fail(CC_ERR_INVALID, "plane counts must be 1 or 2");
+    ctx->planes_rows = rows;
+    for (int i = 0; i < 4; ++i) { ctx->planes_small[i] = planes_upto_rows[i]; ctx->planes_large[i] = planes_above[i]; }
     return CC_OK;
 }
 
@@ -367,7 +411,9 @@ cc_status cc_create_layer(cc_ctx* ctx, const cc_layer_desc* desc, const cc_layer
     if (8 % d.n_kv_heads) return fail(CC_ERR_INVALID, "n_kv_heads must be 1, 2, 4 or 8 (one page of all kv heads is staged per TMA box)");
     if (d.ffn <= 0 || d.ffn % 8) return fail(CC_ERR_INVALID, "ffn must be a positive multiple of 8");
     if (d.page_size != CC_PAGE_SIZE) return fail(CC_ERR_INVALID, "page_size must be %d", CC_PAGE_SIZE);
-    if (d.max_batch < 1 || d.max_batch > 256) return fail(CC_ERR_INVALID, "max_batch must be in 1..256");
+    if (d.max_batch < 1 || d.max_batch > CC_BIG_MAX_ROWS) return fail(CC_ERR_INVALID, "max_batch must be in 1..%d", CC_BIG_MAX_ROWS);
+    if (d.max_batch > 256 && d.head_dim != 128)
+        return fail(CC_ERR_INVALID, "steps of more than 256 rows (mixed prefill + decode) need head_dim 128");
     if (d.max_blocks_per_seq < 1 || d.max_position < 1) return fail(CC_ERR_INVALID, "max_blocks_per_seq / max_position must be >= 1");
     if (!(d.rms_eps > 0.f) || !(d.rope_base > 1.f)) return fail(CC_ERR_INVALID, "bad rms_eps / rope_base");
     const void* ptrs[9] = {w->g1, w->wq, w->wk, w->wv, w->wo, w->g2, w->wgate, w->wup, w->wdown};
@@ -389,6 +435,10 @@ cc_status cc_create_layer(cc_ctx* ctx, const cc_layer_desc* desc, const cc_layer
     D.QD = D.Hq * D.Dh; D.KD = D.Hkv * D.Dh;
     D.max_batch = d.max_batch; D.max_blocks = d.max_blocks_per_seq; D.max_position = d.max_position;
     D.Mpad = (d.max_batch + 15) / 16 * 16 + 16 * CC_MAXR;
+    D.Mpart = D.Mpad < CC_MAX_MPAD ? D.Mpad : CC_MAX_MPAD;
+    const bool big = d.max_batch > 256;                       // the layer also takes steps of more than 256 rows
+    D.fmt = ctx->operand_format == CC_OPERAND_BF16X2 ? CC_FMT_BF16X2 : CC_FMT_F16;   // AUTO: fp16 unless a weight overflows it (below)
+    for (int i = 0; i < 4; ++i) D.pl[i] = 2;                                           // per step: step_dims()
     D.eps = d.rms_eps;
     D.qk_scale_log2 = (float)(1.4426950408889634 / std::sqrt((double)D.Dh));
     // blob layout: [QKV tiles][O tiles][gate/up tiles][down tiles][g1][g2]
@@ -405,7 +455,7 @@ cc_status cc_create_layer(cc_ctx* ctx, const cc_layer_desc* desc, const cc_layer
     D.off_g2 = blob.take((size_t)D.d * 2);
     L->blob_bytes = blob.take(0);
     if (D.qkv.ST > CC_FLAG_STRIDE || D.o.ST > CC_FLAG_STRIDE || D.gu.ST > CC_FLAG_STRIDE || D.dn.ST > CC_FLAG_STRIDE ||
-        D.Mpad > CC_MAX_MPAD) {
+        D.Mpart > CC_MAX_MPAD) {
         delete L;
         return fail(CC_ERR_INVALID, "shape exceeds the stream-K bookkeeping limits (%d super tiles, %d rows)", CC_FLAG_STRIDE, CC_MAX_MPAD);
     }
@@ -416,14 +466,23 @@ cc_status cc_create_layer(cc_ctx* ctx, const cc_layer_desc* desc, const cc_layer
     const size_t Mp = (size_t)D.Mpad;
     const size_t o_sched = ws.take(sizeof(CcSched));
     const size_t o_perm = ws.take(Mp * 4);
-    const size_t o_pgpre = ws.take((size_t)(d.max_batch + 1) * 4);
+    const size_t o_pgpre = ws.take((size_t)((d.max_batch > CC_BIG_MAX_DEC ? d.max_batch : CC_BIG_MAX_DEC) + 1) * 4);
     const size_t o_posof = ws.take((size_t)d.max_batch * 4);
     const size_t o_fwr = ws.take((size_t)d.max_batch * 4);
-    const size_t o_x = ws.take((size_t)2 * D.qkv.KB * Mp * 128);   // hi + lo planes
-    const size_t o_o = ws.take((size_t)2 * D.o.KB * Mp * 128);
-    const size_t o_y = ws.take((size_t)2 * D.gu.KB * Mp * 128);
-    const size_t o_a = ws.take((size_t)2 * D.dn.KB * Mp * 128);
-    auto part_bytes = [&](const CcGemmGeo& g) { return (size_t)(g.P + g.ST) * CC_G * Mp * 128 * 4; };
+    // operands: sized for two planes (the plane count is a per-step choice); a large step's last row block reads up
+    // to 256 rows past the last group, so the buffers carry that much slack behind them
+    const size_t slack = big ? (size_t)2 * 256 * 128 : 0;
+    const size_t o_x = ws.take((size_t)2 * D.qkv.KB * Mp * 128 + slack);
+    const size_t o_o = ws.take((size_t)2 * D.o.KB * Mp * 128 + slack);
+    const size_t o_y = ws.take((size_t)2 * D.gu.KB * Mp * 128 + slack);
+    const size_t o_a = ws.take((size_t)2 * D.dn.KB * Mp * 128 + slack);
+    const size_t o_invin = ws.take(Mp * 4);
+    const size_t o_bs = ws.take(sizeof(CcBigSched));
+    const size_t o_rpos = ws.take(big ? Mp * 4 : 0), o_rpage = ws.take(big ? Mp * 4 : 0), o_gus = ws.take(big ? Mp * 4 : 0);
+    const size_t o_dec = ws.take((size_t)(CC_BIG_MAX_DEC + 1) * 4);
+    const size_t o_cr0 = ws.take((size_t)CC_BIG_MAX_CHUNKS * 4), o_clen = ws.take((size_t)CC_BIG_MAX_CHUNKS * 4);
+    const size_t o_ic = ws.take((size_t)CC_BIG_MAX_ITEMS * 4), o_it = ws.take((size_t)CC_BIG_MAX_ITEMS * 4);
+    auto part_bytes = [&](const CcGemmGeo& g) { return (size_t)(g.P + g.ST) * CC_G * D.Mpart * 128 * 4; };
     const size_t o_pq = ws.take(part_bytes(D.qkv));
     const size_t o_po = ws.take(part_bytes(D.o));
     const size_t o_pg = ws.take(part_bytes(D.gu));
@@ -463,6 +522,12 @@ cc_status cc_create_layer(cc_ctx* ctx, const cc_layer_desc* desc, const cc_layer
     W.d_part = (float*)(wb + o_pd);
     W.q_rot = (float*)(wb + o_qrot); W.h1 = (float*)(wb + o_h1);
     W.ssq = (float*)(wb + o_ssq); W.flags = (int*)(wb + o_flags);
+    W.inv_in = (float*)(wb + o_invin);
+    W.bs = (CcBigSched*)(wb + o_bs);
+    W.row_pos = (int*)(wb + o_rpos); W.row_page = (int*)(wb + o_rpage); W.gu_scale = (float*)(wb + o_gus);
+    W.dec_rows = (int*)(wb + o_dec); W.chunk_row0 = (int*)(wb + o_cr0); W.chunk_len = (int*)(wb + o_clen);
+    W.item_chunk = (int*)(wb + o_ic); W.item_tile = (int*)(wb + o_it);
+    L->big = big;
     W.attn_cnt = (int*)(wb + o_acnt);
     W.att_o = (float*)(wb + o_atto); W.att_ml = (float2*)(wb + o_attml);
     W.rope_cs = (const float2*)(wb + o_rope);
@@ -484,18 +549,32 @@ cc_status cc_create_layer(cc_ctx* ctx, const cc_layer_desc* desc, const cc_layer
         }
         e = cudaMemcpy(wb + o_rope, tab.data(), tab.size() * sizeof(float2), cudaMemcpyHostToDevice);
     }
-    // one-time re-pack of the nine tensors into the blob (tcgen05 operand tile images + gains)
+    // one-time re-pack of the nine tensors into the blob (tcgen05 operand tile images + gains).  fp16 images unless a
+    // weight does not fit fp16 (then, in AUTO, the layer falls back to bf16 images and two activation planes).
     typedef const __nv_bfloat16* bp;
-    if (e == cudaSuccess)
-        e = cc_launch_pack(L->blob0 + D.qkv.w_off, (bp)w->wq, (bp)w->wk, (bp)w->wv, D.QD, D.KD, D.KD, 0, D.d, D.qkv.ST * CC_G,
-                           D.qkv.KB, 0);
-    if (e == cudaSuccess)
-        e = cc_launch_pack(L->blob0 + D.o.w_off, (bp)w->wo, nullptr, nullptr, D.d, 0, 0, 0, D.QD, D.o.ST * CC_G, D.o.KB, 0);
-    if (e == cudaSuccess)
-        e = cc_launch_pack(L->blob0 + D.gu.w_off, (bp)w->wgate, (bp)w->wup, nullptr, D.F, D.F, 0, 1, D.d, D.gu.ST * CC_G,
-                           D.gu.KB, 0);
-    if (e == cudaSuccess)
-        e = cc_launch_pack(L->blob0 + D.dn.w_off, (bp)w->wdown, nullptr, nullptr, D.d, 0, 0, 0, D.F, D.dn.ST * CC_G, D.dn.KB, 0);
+    uint32_t* ovf = ctx->err_dev + 16;
+    for (int attempt = 0; attempt < 2 && e == cudaSuccess; ++attempt) {
+        e = cudaMemset(ovf, 0, 4);
+        if (e == cudaSuccess)
+            e = cc_launch_pack(L->blob0 + D.qkv.w_off, (bp)w->wq, (bp)w->wk, (bp)w->wv, D.QD, D.KD, D.KD, 0, D.d, D.qkv.ST * CC_G,
+                               D.qkv.KB, D.fmt, ovf, 0);
+        if (e == cudaSuccess)
+            e = cc_launch_pack(L->blob0 + D.o.w_off, (bp)w->wo, nullptr, nullptr, D.d, 0, 0, 0, D.QD, D.o.ST * CC_G, D.o.KB, D.fmt, ovf, 0);
+        if (e == cudaSuccess)
+            e = cc_launch_pack(L->blob0 + D.gu.w_off, (bp)w->wgate, (bp)w->wup, nullptr, D.F, D.F, 0, 1, D.d, D.gu.ST * CC_G,
+                               D.gu.KB, D.fmt, ovf, 0);
+        if (e == cudaSuccess)
+            e = cc_launch_pack(L->blob0 + D.dn.w_off, (bp)w->wdown, nullptr, nullptr, D.d, 0, 0, 0, D.F, D.dn.ST * CC_G, D.dn.KB, D.fmt, ovf, 0);
+        uint32_t overflow = 0;
+        if (e == cudaSuccess) e = cudaMemcpy(&overflow, ovf, 4, cudaMemcpyDeviceToHost);
+        if (e != cudaSuccess || !overflow || D.fmt != CC_FMT_F16) break;
+        if (ctx->operand_format == CC_OPERAND_F16) {
+            destroy_layer_memory(L);
+            delete L;
+            return fail(CC_ERR_INVALID, "a weight does not fit fp16 (|w| > 65504 or not finite) and the context demands CC_OPERAND_F16");
+        }
+        D.fmt = CC_FMT_BF16X2;
+    }
     if (e == cudaSuccess) e = cudaMemcpy(L->blob0 + D.off_g1, w->g1, (size_t)D.d * 2, cudaMemcpyDeviceToDevice);
     if (e == cudaSuccess) e = cudaMemcpy(L->blob0 + D.off_g2, w->g2, (size_t)D.d * 2, cudaMemcpyDeviceToDevice);
     L->rep[0].state = REP_LIVE;
@@ -535,6 +614,12 @@ cc_status cc_destroy_layer(cc_layer* L) {
     ctx->row_used[L->row] = false;
     ctx->n_layers--;
     delete L;
+    return CC_OK;
+}
+
+cc_status cc_layer_operand_format(const cc_layer* L, int* format) {
+    if (!L || !format) return fail(CC_ERR_INVALID, "null argument");
+    *format = L->D.fmt == CC_FMT_F16 ? CC_OPERAND_F16 : CC_OPERAND_BF16X2;
     return CC_OK;
 }
 
@@ -693,10 +778,52 @@ void* mapped_host(const void* p) {
     return a.type == cudaMemoryTypeHost && !((uintptr_t)a.devicePointer & 15) ? a.devicePointer : nullptr;
 }
 
+// Geometry of one step: the layer's, with the activation plane counts of a step of `batch` rows.
+CcDims step_dims(cc_layer* L, int batch) {
+    CcDims D = L->D;
+    const cc_ctx* ctx = L->ctx;
+    for (int i = 0; i < 4; ++i)
+        D.pl[i] = D.fmt == CC_FMT_BF16X2 ? 2 : (batch <= ctx->planes_rows ? ctx->planes_small[i] : ctx->planes_large[i]);
+    for (int i = 0; i < 4; ++i) L->last_pl[i] = D.pl[i];
+    // the row tables of the small-step kernels and of the decode attention hold at most 256 rows: a small step of a
+    // large layer sees 256, a large step's attention walks its (at most CC_BIG_MAX_DEC) decode rows
+    if (D.max_batch > 256) D.max_batch = 256;
+    return D;
+}
+
+
+// A step of more than 256 rows (prompt chunks + decode rows): plain stream order, no PDL.
+cudaError_t enqueue_big(cc_layer* L, __nv_bfloat16* hidden, const CcKv& kv, const int* seq_lens, const int* assign, int batch,
+                        cudaStream_t st, cudaEvent_t* ev) {
+    cc_ctx* ctx = L->ctx;
+    CcDims D = step_dims(L, batch);
+    const CcWork& W = L->W;
+    const CcLayerTable* tab = ctx->table_dev + L->row;
+    CcLaunch Ln{st, ctx->n_sms, false};
+    cudaError_t e = cudaSuccess;
+    for (int stage = 0; stage < 9 && e == cudaSuccess; ++stage) {
+        if (ev && (e = cudaEventRecord(ev[stage], st)) != cudaSuccess) break;
+        switch (stage) {
+            case 0: e = cc_launch_big_group(assign, seq_lens, kv.block_table, batch, D, tab, W, st); break;
+            case 1: e = cc_launch_big_norm(hidden, batch, D, tab, W, st); break;
+            case 2: e = cc_launch_big_gemm(0, D, tab, W, seq_lens, assign, batch, kv, hidden, Ln); break;
+            case 3: e = cc_launch_attention(seq_lens, kv, D, tab, W, Ln, W.dec_rows); break;
+            case 4: e = cc_launch_prefill_attention(seq_lens, kv, D, W, Ln); break;
+            case 5: e = cc_launch_big_gemm(1, D, tab, W, seq_lens, assign, batch, kv, hidden, Ln); break;
+            case 6: e = cc_launch_big_rowstat(D, W, st); break;
+            case 7: e = cc_launch_big_gemm(2, D, tab, W, seq_lens, assign, batch, kv, hidden, Ln); break;
+            default: e = cc_launch_big_gemm(3, D, tab, W, seq_lens, assign, batch, kv, hidden, Ln); break;
+        }
+    }
+    if (ev && e == cudaSuccess) e = cudaEventRecord(ev[9], st);
+    return e;
+}
+
 cudaError_t enqueue_forward(cc_layer* L, __nv_bfloat16* hidden, const CcKv& kv, const int* seq_lens, const int* assign,
                             int batch, cudaStream_t st, cudaEvent_t* ev = nullptr, __nv_bfloat16* hidden_host_alias = nullptr) {
+    if (batch > 256) return enqueue_big(L, hidden, kv, seq_lens, assign, batch, st, ev);
     cc_ctx* ctx = L->ctx;
-    const CcDims& D = L->D;
+    const CcDims D = step_dims(L, batch);
     const CcWork& W = L->W;
     const CcLayerTable* tab = ctx->table_dev + L->row;
     CcLaunch Ln{st, ctx->n_sms, ctx->pdl && ev == nullptr};
@@ -756,7 +883,7 @@ cc_status cc_forward_host(cc_layer* L, void* hidden_host, void* k_pool_dev, void
     const size_t hb = (size_t)batch * L->D.d * 2;
     // Pinned hidden buffer: the kernels read and write it in place (measured: 280 us per cfg2 step against 300 us
     // with the two 512 KB copies; reading the three small tables in place as well costs more than their copies).
-    if (void* alias = mapped_host(hidden_host)) {
+    if (void* alias = batch <= 256 ? mapped_host(hidden_host) : nullptr) {
         if (!k_pool_dev || !v_pool_dev || n_pages < 1) return fail(CC_ERR_INVALID, "bad KV pool arguments");
         if (((uintptr_t)k_pool_dev | (uintptr_t)v_pool_dev) & 15) return fail(CC_ERR_INVALID, "KV pools must be 16-byte aligned");
         CC_CUDA(stage_tables(L, block_table_host, seq_lens_host, replica_assign_host, batch, st));
@@ -783,15 +910,17 @@ cc_status cc_forward_profiled(cc_layer* L, void* hidden_dev, const cc_kv_pages* 
         return fail(CC_ERR_INVALID, "null argument");
     if (batch < 1 || batch > L->desc.max_batch) return fail(CC_ERR_INVALID, "batch %d outside 1..max_batch=%d", batch, L->desc.max_batch);
     CC_CUDA(cudaSetDevice(L->ctx->device));
-    cudaEvent_t ev[kForwardLaunches + 1];
+    cudaEvent_t ev[CC_MAX_PROFILE_STAGES + 1];
     for (auto& x : ev) CC_CUDA(cudaEventCreate(&x));
+    const int n_stages = batch > 256 ? 9 : kForwardLaunches;
+    for (int i = 0; i < CC_MAX_PROFILE_STAGES; ++i) stage_ms_host[i] = 0.f;
     CcKv k{(__nv_bfloat16*)kv->k_pool, (__nv_bfloat16*)kv->v_pool, kv->block_table, kv->n_pages};
     // a pinned host `hidden`: the stages of cc_forward_host's in-place path (the rows are staged for the residual)
-    void* alias = mapped_host(hidden_dev);
+    void* alias = batch <= 256 ? mapped_host(hidden_dev) : nullptr;
     cudaError_t e = enqueue_forward(L, alias ? L->st_hidden : (__nv_bfloat16*)hidden_dev, k, seq_lens_dev, replica_assign_dev,
                                     batch, (cudaStream_t)stream, ev, (__nv_bfloat16*)alias);
     if (e == cudaSuccess) e = cudaStreamSynchronize((cudaStream_t)stream);
-    for (int i = 0; i < kForwardLaunches && e == cudaSuccess; ++i) e = cudaEventElapsedTime(&stage_ms_host[i], ev[i], ev[i + 1]);
+    for (int i = 0; i < n_stages && e == cudaSuccess; ++i) e = cudaEventElapsedTime(&stage_ms_host[i], ev[i], ev[i + 1]);
     for (auto& x : ev) cudaEventDestroy(x);
     if (e != cudaSuccess) return fail(CC_ERR_CUDA, "cc_forward_profiled: %s", cudaGetErrorString(e));
     return CC_OK;
@@ -903,14 +1032,14 @@ cc_status cc_debug_tap(cc_layer* L, cc_tap which, float* out_host, int batch) {
     if (batch < 1 || batch > L->desc.max_batch) return fail(CC_ERR_INVALID, "bad batch");
     const CcDims& D = L->D;
     const void* src;
-    int kind, dim;
+    int kind, dim, planes = 1;
     switch (which) {
-        case CC_TAP_X: src = L->W.x_act; kind = 2; dim = D.d; break;
+        case CC_TAP_X: src = L->W.x_act; kind = 2; dim = D.d; planes = L->last_pl[0]; break;
         case CC_TAP_Q: src = L->W.q_rot; kind = 1; dim = D.QD; break;
-        case CC_TAP_O: src = L->W.o_act; kind = 2; dim = D.QD; break;
+        case CC_TAP_O: src = L->W.o_act; kind = 2; dim = D.QD; planes = L->last_pl[1]; break;
         case CC_TAP_H1: src = L->W.h1; kind = 1; dim = D.d; break;
-        case CC_TAP_Y: src = L->W.y_act; kind = 3; dim = D.d; break;
-        case CC_TAP_A: src = L->W.a_act; kind = 2; dim = D.F; break;
+        case CC_TAP_Y: src = L->W.y_act; kind = 3; dim = D.d; planes = L->last_pl[2]; break;
+        case CC_TAP_A: src = L->W.a_act; kind = 2; dim = D.F; planes = L->last_pl[3]; break;
         default: return fail(CC_ERR_INVALID, "unknown tap");
     }
     CC_CUDA(cudaSetDevice(L->ctx->device));
@@ -919,7 +1048,7 @@ cc_status cc_debug_tap(cc_layer* L, cc_tap which, float* out_host, int batch) {
     const size_t bytes = (size_t)batch * dim * 4;
     CC_CUDA(cudaMalloc(&tmp, bytes));
     cudaError_t e = cudaMemset(tmp, 0, bytes);
-    if (e == cudaSuccess) e = cc_launch_tap(src, kind, dim, D, L->W, tmp, batch, 0);
+    if (e == cudaSuccess) e = cc_launch_tap(src, kind, planes, dim, D, L->W, tmp, batch, 0);
     if (e == cudaSuccess) e = cudaMemcpy(out_host, tmp, bytes, cudaMemcpyDeviceToHost);
     cudaFree(tmp);
     if (e != cudaSuccess) return fail(CC_ERR_CUDA, "cc_debug_tap: %s", cudaGetErrorString(e));

@@ -61,7 +61,7 @@ struct AttnCfg {
 template <int DH>
 __global__ void __launch_bounds__(kAttnThreads, 1)
 k_attn(const int* __restrict__ seq_lens, CcKv kv, CcDims D, CcWork W, const CcLayerTable* __restrict__ tab,
-       const __grid_constant__ CUtensorMap tmK, const __grid_constant__ CUtensorMap tmV) {
+       const int* __restrict__ rowmap, const __grid_constant__ CUtensorMap tmK, const __grid_constant__ CUtensorMap tmV) {
     using C = AttnCfg<DH>;
     extern __shared__ __align__(1024) uint8_t smem_raw[];
     const int warp = uniform((int)(threadIdx.x >> 5)), lane = threadIdx.x & 31;
@@ -123,7 +123,9 @@ k_attn(const int* __restrict__ seq_lens, CcKv kv, CcDims D, CcWork W, const CcLa
             const int r0 = s_prefix[b], r1 = s_prefix[b + 1];
             if (r1 <= p) { ++b; continue; }                       // rows without pages (padding)
             const int q0 = p - r0, q1 = min(r1, P1) - r0;         // this CTA's pages of row b
-            const int pos = W.pos_of[b], s = seq_lens[b], first_wr = W.first_wr[b];
+            // large steps: the work axis runs over the decode rows only, b indexes that list (k_big_group)
+            const int rb = rowmap ? rowmap[b] : b;
+            const int pos = W.pos_of[rb], s = seq_lens[rb], first_wr = W.first_wr[rb];
             const int slot0 = b + cta_of_page(r0), n_pieces = cta_of_page(r1 - 1) - cta_of_page(r0) + 1;
             const int slot = b + (int)blockIdx.x;
             const int n_groups = (q1 - q0 + PPS - 1) / PPS;
@@ -135,7 +137,7 @@ k_attn(const int* __restrict__ seq_lens, CcKv kv, CcDims D, CcWork W, const CcLa
                     const int q = qg + lane;
                     id = 0;
                     if (q < q1) {
-                        id = kv.block_table[(size_t)b * D.max_blocks + q];
+                        id = kv.block_table[(size_t)rb * D.max_blocks + q];
                         if (id < 0 || id >= kv.n_pages) {
                             atomicOr(W.err, CC_DEVERR_BAD_PAGE);
                             id = 0;
@@ -321,14 +323,9 @@ k_attn(const int* __restrict__ seq_lens, CcKv kv, CcDims D, CcWork W, const CcLa
         // lane l owns dims 4l .. 4l+3 of every q head of the group
         const int dim = lane * 4;
         const int nch = m.n_pieces;
-        auto store_operand = [&](int q, float4 v, float inv) {   // row of the O-projection operand, hi + lo bf16 planes
-            const int col = (h * G + q) * DH + dim;
-            const float x0 = v.x * inv, x1 = v.y * inv, x2 = v.z * inv, x3 = v.w * inv;
-            const uint32_t h0 = pack_bf16(x0, x1), h1 = pack_bf16(x2, x3);
-            const uint32_t l0 = pack_bf16(x0 - bf16lo(h0), x1 - bf16hi(h0)), l1 = pack_bf16(x2 - bf16lo(h1), x3 - bf16hi(h1));
-            uint8_t* dst = W.o_act + act_chunk_off(m.pos, col, D.Mpad, 2, 0) + (col & 7) * 2;
-            *reinterpret_cast<uint2*>(dst) = make_uint2(h0, h1);
-            *reinterpret_cast<uint2*>(dst + 1024) = make_uint2(l0, l1);
+        auto store_operand = [&](int q, float4 v, float inv) {   // row of the O-projection operand, in the layer's operand format
+            const float x[4] = {v.x * inv, v.y * inv, v.z * inv, v.w * inv};
+            act_store<4>(W.o_act, D, D.pl[CC_OP_O], m.pos, (h * G + q) * DH + dim, x);
         };
         if (pp == 0 && dim < DH) {
 #pragma unroll 1
@@ -421,9 +418,9 @@ cudaError_t cc_attn_configure() {
 }
 
 // Tensor map of a caller-owned KV pool seen as a 2-D bf16 tensor [n_pages * Hkv * 16 rows][Dh], boxes of
-// one page (Hkv * 16 rows) x 64 elements (128 bytes) with the 128-byte swizzle.  cuTensorMapEncodeTiled is
+// box_rows rows (one page of all kv heads: Hkv * 16; one page of one head: 16) x 64 elements (128 bytes) with the 128-byte swizzle.  cuTensorMapEncodeTiled is
 // a driver entry point; it is looked up once through the runtime, so the library needs no link against libcuda.
-static cudaError_t make_kv_tensor_map(CUtensorMap* out, const void* pool, int n_pages, int Hkv, int Dh) {
+cudaError_t cc_make_kv_tensor_map(CUtensorMap* out, const void* pool, int n_pages, int Hkv, int Dh, int box_rows) {
     typedef CUresult (*EncodeFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
                                  const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
                                  CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
@@ -438,7 +435,7 @@ static cudaError_t make_kv_tensor_map(CUtensorMap* out, const void* pool, int n_
     }
     const cuuint64_t dims[2] = {(cuuint64_t)Dh, (cuuint64_t)n_pages * Hkv * CC_PAGE};
     const cuuint64_t strides[1] = {(cuuint64_t)Dh * 2};
-    const cuuint32_t box[2] = {64, (cuuint32_t)(Hkv * CC_PAGE)};
+    const cuuint32_t box[2] = {64, (cuuint32_t)box_rows};
     const cuuint32_t estr[2] = {1, 1};
     const CUresult r = encode(out, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, const_cast<void*>(pool), dims, strides, box, estr,
                               CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
@@ -447,13 +444,13 @@ static cudaError_t make_kv_tensor_map(CUtensorMap* out, const void* pool, int n_
 }
 
 cudaError_t cc_launch_attention(const int* seq_lens, const CcKv& kv, const CcDims& D, const CcLayerTable* tab,
-                                const CcWork& W, const CcLaunch& L) {
+                                const CcWork& W, const CcLaunch& L, const int* rowmap) {
     CUtensorMap tmK, tmV;
-    cudaError_t e = make_kv_tensor_map(&tmK, kv.k_pool, kv.n_pages, D.Hkv, D.Dh);
-    if (e == cudaSuccess) e = make_kv_tensor_map(&tmV, kv.v_pool, kv.n_pages, D.Hkv, D.Dh);
+    cudaError_t e = cc_make_kv_tensor_map(&tmK, kv.k_pool, kv.n_pages, D.Hkv, D.Dh, D.Hkv * CC_PAGE);
+    if (e == cudaSuccess) e = cc_make_kv_tensor_map(&tmV, kv.v_pool, kv.n_pages, D.Hkv, D.Dh, D.Hkv * CC_PAGE);
     if (e != cudaSuccess) return e;
     const dim3 grid(L.n_sms), block(kAttnThreads);
     if (D.Dh == 128)
-        return cc_launch_kernel(k_attn<128>, grid, block, AttnCfg<128>::smem_bytes(D.G), L, seq_lens, kv, D, W, tab, tmK, tmV);
-    return cc_launch_kernel(k_attn<64>, grid, block, AttnCfg<64>::smem_bytes(D.G), L, seq_lens, kv, D, W, tab, tmK, tmV);
+        return cc_launch_kernel(k_attn<128>, grid, block, AttnCfg<128>::smem_bytes(D.G), L, seq_lens, kv, D, W, tab, rowmap, tmK, tmV);
+    return cc_launch_kernel(k_attn<64>, grid, block, AttnCfg<64>::smem_bytes(D.G), L, seq_lens, kv, D, W, tab, rowmap, tmK, tmV);
 }

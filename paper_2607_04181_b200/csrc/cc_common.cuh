@@ -3,6 +3,7 @@
 #pragma once
 #include <cuda_runtime.h>
 #include <cuda_bf16.h>
+#include <cuda_fp16.h>
 #include <stdint.h>
 
 #define CC_MAXR 4              // CC_MAX_REPLICAS
@@ -14,11 +15,20 @@
 #define CC_MAX_MPAD 320        // (256 rows + 16 * CC_MAXR group padding): upper bound of CcDims::Mpad
 #define CC_FLAG_STRIDE 256     // stream-K fixup counters per projection (>= super tiles of any projection)
 
+// GEMM operand formats (chosen per layer at cc_create_layer).  F16: the bf16 weights are converted to fp16 when they
+// are packed (exact for 2^-17 <= |w| <= 65504) and the activations are ONE fp16 plane (11 significand bits).
+// BF16X2: weights stay bf16, activations are two bf16 planes hi + lo (16 bits) -- twice the tensor work and slab
+// traffic; the fallback for weights outside the fp16 range.  tcgen05 kind::f16 needs A and B in the SAME format.
+#define CC_FMT_BF16X2 0
+#define CC_FMT_F16 1
+
 #define CC_DEVERR_BAD_REPLICA 1u
 #define CC_DEVERR_BAD_PAGE 2u
 #define CC_DEVERR_BAD_SEQLEN 4u
 #define CC_DEVERR_HANG 8u         // an mbarrier wait gave up (kernel bug); the kernel trapped
 #define CC_DEVERR_SPLIT_REQUEST 16u   // rows of one request name different replicas
+#define CC_DEVERR_TOO_MANY_DECODE 32u  // a large step holds more decode rows, prompt chunks or prefill tiles than its tables
+#define CC_BIG_MAX_ROWS 8192          // rows of a large step (cc_layer_desc.max_batch of a large layer)
 
 // ---- device replica table -----------------------------------------
 // One row per layer, at a fixed device address for the life of the context.  Kernels read the
@@ -81,6 +91,10 @@ struct CcDims {
     int d, Hq, Hkv, Dh, G, F;
     int QD, KD;                 // Hq*Dh, Hkv*Dh
     int Mpad;                   // rows of every grouped workspace buffer (multiple of 16)
+    int Mpart;                  // rows of the stream-K partial buffers (small steps only: min(Mpad, CC_MAX_MPAD))
+    int fmt;                    // GEMM operand format of this layer: CC_FMT_F16 or CC_FMT_BF16X2
+    int pl[4];                  // activation planes of the four GEMM operands (x, o, y, a): 1 = one plane, 2 = hi + lo; set per
+                                // step by the host (cc_api.cu plane policy); BF16X2 layers always use 2
     int max_batch, max_blocks, max_position;
     float eps;
     float qk_scale_log2;        // log2(e) / sqrt(Dh)
@@ -118,12 +132,33 @@ __device__ __forceinline__ int cc_row_replica(const int* __restrict__ assign, co
     return rep;
 }
 
+// Replica group that holds grouped position `pos` (groups are laid out in replica order).
+__device__ __forceinline__ int replica_of_pos(const int* cnt, const int* goff, int pos) {
+    int r = 0;
+#pragma unroll
+    for (int i = 1; i < CC_MAXR; ++i)
+        if (cnt[i] > 0 && pos >= goff[i]) r = i;
+    return r;
+}
+
 // ---- small helpers -----------------------------------------------------------------------
 __device__ __forceinline__ float bf16lo(uint32_t w) { return __uint_as_float(w << 16); }
 __device__ __forceinline__ float bf16hi(uint32_t w) { return __uint_as_float(w & 0xffff0000u); }
 __device__ __forceinline__ uint32_t pack_bf16(float lo, float hi) {
     __nv_bfloat162 v = __floats2bfloat162_rn(lo, hi);   // .x = lo (low 16 bits)
     return *reinterpret_cast<uint32_t*>(&v);
+}
+// two floats -> fp16x2 bits (round to nearest even, clamped to the finite fp16 range so that a drifting benchmark
+// input saturates instead of turning into inf - inf = NaN)
+__device__ __forceinline__ uint32_t pack_f16(float lo, float hi) {
+    lo = fminf(fmaxf(lo, -65504.f), 65504.f);
+    hi = fminf(fmaxf(hi, -65504.f), 65504.f);
+    __half2 v = __floats2half2_rn(lo, hi);   // .x = lo (low 16 bits)
+    return *reinterpret_cast<uint32_t*>(&v);
+}
+__device__ __forceinline__ void split_hilo(float v0, float v1, uint32_t& hi, uint32_t& lo) {
+    hi = pack_bf16(v0, v1);
+    lo = pack_bf16(v0 - bf16lo(hi), v1 - bf16hi(hi));
 }
 __device__ __forceinline__ uint32_t smem_u32(const void* p) {
     return static_cast<uint32_t>(__cvta_generic_to_shared(p));
@@ -138,6 +173,39 @@ __device__ __forceinline__ size_t act_chunk_off(int row, int k, int Mpad, int pl
     const int kb = k >> 6, c = (k >> 3) & 7;
     return ((((size_t)kb * (Mpad >> 3) + (row >> 3)) * planes + pl) << 10) + (size_t)((row & 7) << 7) +
            (size_t)((c ^ (row & 7)) << 4);
+}
+
+// Stores N = 2, 4 or 8 consecutive operand values (k a multiple of N) of grouped row `row` in the layer's element
+// format, as `planes` planes: one plane = the rounded value, two = hi + lo (lo = the rounded remainder).
+enum { CC_OP_X = 0, CC_OP_O = 1, CC_OP_Y = 2, CC_OP_A = 3 };
+template <int N>
+__device__ __forceinline__ void act_store(uint8_t* act, const CcDims& D, int planes, int row, int k, const float (&v)[N]) {
+    uint8_t* dst = act + act_chunk_off(row, k, D.Mpad, planes, 0) + (k & 7) * 2;
+    uint32_t a[N / 2], b[N / 2] = {};
+    if (D.fmt == CC_FMT_F16) {
+#pragma unroll
+        for (int i = 0; i < N / 2; ++i) {
+            a[i] = pack_f16(v[2 * i], v[2 * i + 1]);
+            if (planes == 2) {
+                const float2 h = __half22float2(*reinterpret_cast<const __half2*>(&a[i]));
+                b[i] = pack_f16(v[2 * i] - h.x, v[2 * i + 1] - h.y);
+            }
+        }
+    } else {
+#pragma unroll
+        for (int i = 0; i < N / 2; ++i) split_hilo(v[2 * i], v[2 * i + 1], a[i], b[i]);
+    }
+    if constexpr (N == 2) {
+        *reinterpret_cast<uint32_t*>(dst) = a[0];
+        if (planes == 2) *reinterpret_cast<uint32_t*>(dst + 1024) = b[0];
+    } else if constexpr (N == 4) {
+        *reinterpret_cast<uint2*>(dst) = make_uint2(a[0], a[1]);
+        if (planes == 2) *reinterpret_cast<uint2*>(dst + 1024) = make_uint2(b[0], b[1]);
+    } else {
+        static_assert(N == 8, "act_store: N must be 2, 4 or 8");
+        *reinterpret_cast<uint4*>(dst) = make_uint4(a[0], a[1], a[2], a[3]);
+        if (planes == 2) *reinterpret_cast<uint4*>(dst + 1024) = make_uint4(b[0], b[1], b[2], b[3]);
+    }
 }
 
 // ---- mbarrier / bulk-copy / TMA ----------------------------------------------------------
@@ -316,8 +384,76 @@ __device__ __forceinline__ uint64_t umma_desc_sw128(uint32_t smem_addr, uint32_t
 // (0 = fp16, 1 = bf16), both K-major, N >> 3 at bit 17, M >> 4 at bit 24.  A and B must have the SAME format:
 // bf16 x fp16 raises an illegal-instruction fault on sm_100a (measured in round 1 and again in round 2 with a
 // one-MMA probe, either operand order), although the descriptor has separate fields.
-__device__ __forceinline__ uint32_t umma_idesc_bf16_m128(uint32_t n) {
-    return (1u << 4) | (1u << 7) | (1u << 10) | ((n >> 3) << 17) | ((128u >> 4) << 24);
+__device__ __forceinline__ uint32_t umma_idesc_m128(uint32_t n, int fmt) {
+    const uint32_t ab = fmt == CC_FMT_F16 ? 0u : 1u;
+    return (1u << 4) | (ab << 7) | (ab << 10) | ((n >> 3) << 17) | ((128u >> 4) << 24);
+}
+
+// ---- thread-block clusters / CTA pairs (cta_group::2) -------------------------------------------------
+__device__ __forceinline__ uint32_t cluster_ctarank() {
+    uint32_t r;
+    asm volatile("mov.u32 %0, %%cluster_ctarank;" : "=r"(r));
+    return r;
+}
+__device__ __forceinline__ void cluster_sync_all() {
+    asm volatile("barrier.cluster.arrive.release.aligned;" ::: "memory");
+    asm volatile("barrier.cluster.wait.acquire.aligned;" ::: "memory");
+}
+// shared::cluster address of `local_smem_addr` in CTA `cta` of the cluster
+__device__ __forceinline__ uint32_t mapa_u32(uint32_t local_smem_addr, uint32_t cta) {
+    uint32_t r;
+    asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(r) : "r"(local_smem_addr), "r"(cta));
+    return r;
+}
+__device__ __forceinline__ void mbar_arrive_cluster(uint32_t cluster_addr) {
+    asm volatile("mbarrier.arrive.release.cluster.shared::cluster.b64 _, [%0];" ::"r"(cluster_addr) : "memory");
+}
+template <int kCols>
+__device__ __forceinline__ void tmem_alloc_pair(uint32_t* dst_smem) {   // one full warp in EACH CTA of the pair
+    asm volatile("tcgen05.alloc.cta_group::2.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(dst_smem)), "n"(kCols)
+                 : "memory");
+    asm volatile("tcgen05.relinquish_alloc_permit.cta_group::2.sync.aligned;" ::: "memory");
+}
+template <int kCols>
+__device__ __forceinline__ void tmem_dealloc_pair(uint32_t taddr) {
+    asm volatile("tcgen05.dealloc.cta_group::2.sync.aligned.b32 %0, %1;" ::"r"(taddr), "n"(kCols) : "memory");
+}
+// D[tmem of both CTAs] (+)= A * B over the CTA pair: M = 256 (128 rows of A from each CTA), N = n (n / 2 rows of B
+// from each CTA); issued by ONE thread of the leader CTA (rank 0); descriptors are smem offsets valid in both CTAs.
+__device__ __forceinline__ void umma_pair_lo(uint32_t d_tmem, uint32_t a_lo, uint32_t b_lo, uint32_t a_hi, uint32_t b_hi,
+                                             uint32_t idesc, uint32_t accumulate) {
+    asm volatile(
+        "{\n\t.reg .pred p;\n\t.reg .b64 da, db;\n\t"
+        "setp.ne.b32 p, %6, 0;\n\t"
+        "mov.b64 da, {%1, %3};\n\t"
+        "mov.b64 db, {%2, %4};\n\t"
+        "tcgen05.mma.cta_group::2.kind::f16 [%0], da, db, %5, p;\n\t}" ::"r"(d_tmem),
+        "r"(a_lo), "r"(b_lo), "r"(a_hi), "r"(b_hi), "r"(idesc), "r"(accumulate)
+        : "memory");
+}
+// mbarrier arrive in BOTH CTAs of the pair (same smem offset) once all previously issued MMAs have completed
+__device__ __forceinline__ void umma_commit_pair(uint64_t* bar) {
+    asm volatile("tcgen05.commit.cta_group::2.mbarrier::arrive::one.shared::cluster.multicast::cluster.b64 [%0], %1;" ::"r"(
+                     smem_u32(bar)),
+                 "h"((uint16_t)3)
+                 : "memory");
+}
+__device__ __forceinline__ uint32_t umma_idesc_pair_m256(uint32_t n, int fmt) {
+    const uint32_t ab = fmt == CC_FMT_F16 ? 0u : 1u;
+    return (1u << 4) | (ab << 7) | (ab << 10) | ((n >> 3) << 17) | ((256u >> 4) << 24);
+}
+// TMEM -> registers: this warp's 32 lanes x 32 consecutive fp32 columns.
+__device__ __forceinline__ void tmem_ld_32x32b_x32(uint32_t taddr, uint32_t (&r)[32]) {
+    asm volatile(
+        "tcgen05.ld.sync.aligned.32x32b.x32.b32 "
+        "{%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15, "
+        "%16, %17, %18, %19, %20, %21, %22, %23, %24, %25, %26, %27, %28, %29, %30, %31}, [%32];"
+        : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7]), "=r"(r[8]),
+          "=r"(r[9]), "=r"(r[10]), "=r"(r[11]), "=r"(r[12]), "=r"(r[13]), "=r"(r[14]), "=r"(r[15]), "=r"(r[16]),
+          "=r"(r[17]), "=r"(r[18]), "=r"(r[19]), "=r"(r[20]), "=r"(r[21]), "=r"(r[22]), "=r"(r[23]), "=r"(r[24]),
+          "=r"(r[25]), "=r"(r[26]), "=r"(r[27]), "=r"(r[28]), "=r"(r[29]), "=r"(r[30]), "=r"(r[31])
+        : "r"(taddr)
+        : "memory");
 }
 
 // ---- legacy tensor path used by decode attention (HBM-bound, tiny M): mma.sync + ldmatrix ----

@@ -5,8 +5,9 @@
 // around the weight stream, not around the MMA:
 //   * swap-AB: a packed weight tile (128 output features x 64 k, a 16 KiB pre-swizzled image
 //     made once at cc_create_layer) is the tcgen05 A operand (M = 128); the activations of one
-//     replica group (n rows, n = multiple of 16, <= 256) are the B operand (N = n), held as two
-//     bf16 planes hi + lo that are both multiplied into the same accumulator.
+//     replica group (n rows, n = multiple of 16, <= 256) are the B operand (N = n): one fp16 plane
+//     against fp16 weight images, or two bf16 planes hi + lo that are both multiplied into the
+//     same accumulator against bf16 images (CcDims::fmt).
 //   * CC_G = 2 adjacent tiles form a super tile: one pipeline stage = the two weight atoms of
 //     one k-block (32 KiB, contiguous in the blob, one bulk copy) + the activation slab of that
 //     k-block (both planes, one bulk copy), feeding two fp32 accumulators D[128][n] in TMEM
@@ -23,7 +24,7 @@
 //     partials ("pieces", fixed order 0..m-1) of every m-th row and apply the fused epilogue of
 //     the projection (RoPE + KV append | residual + norm statistics + operand packing | SwiGLU |
 //     residual + write-back in request order), so no separate reduce kernel runs between GEMMs.
-#include "cc_kernels.h"
+#include "cc_epilogue.cuh"
 
 namespace {
 
@@ -44,132 +45,18 @@ struct GemmSmemHdr {                      // lives at the start of dynamic smem
     int goff[CC_MAXR];
     const uint8_t* blob[CC_MAXR];
     int perm[CC_MAX_MPAD];                // original row at grouped position, or -1
-    int aux[CC_MAX_MPAD];                 // QKV: position s-1; gate/up: bits of 1/rms of the row
+    int aux[CC_MAX_MPAD];                 // QKV: position s-1; O: bits of 1/rms of the input row; gate/up: bits of rms_in/rms of h1
     int page[CC_MAX_MPAD];                // QKV: page that holds position s-1, or -1
 };
 static_assert(sizeof(GemmSmemHdr) <= kHdrBytes, "header does not fit");
 
-// ---- fused epilogues of the stream-K fixup -----------------------------------------------------------
-// One warp owns one item = (tile t, grouped row p); lane l holds the four summed output features
-// t*128 + 4l .. 4l+3 of original row b.  Each epilogue is split into `pre` (issue every global load
-// that does not depend on the sum, together with the loads of the partial sums) and `fin` (math +
-// stores), so that one fixup iteration costs one L2 round trip.
-enum { EPI_QKV = 0, EPI_O = 1, EPI_GU = 2, EPI_DN = 3 };
-struct CcEpi {
-    const int* assign;          // replica_assign and batch: the QKV GEMM counts the groups itself
-    int batch;
-    const int* seq_lens;
-    CcKv kv;
-    __nv_bfloat16* hidden;
+// per-row tables of the fused epilogues, held in shared memory (built by the helper warps)
+struct SmemTab {
+    const GemmSmemHdr* H;
+    __device__ __forceinline__ int aux(int p) const { return H->aux[p]; }
+    __device__ __forceinline__ int page(int p) const { return H->page[p]; }
+    __device__ __forceinline__ const uint8_t* blob(int p) const { return H->blob[replica_of_pos(H->cnt, H->goff, p)]; }
 };
-struct EpiPre {
-    float4 f0, f1;      // QKV: (cos, sin) x 4; down: h1
-    uint2 u0, u1;       // O: hidden bits, g2 bits
-};
-
-__device__ __forceinline__ int replica_of_pos(const int* cnt, const int* goff, int pos) {
-    int r = 0;
-#pragma unroll
-    for (int i = 1; i < CC_MAXR; ++i)
-        if (cnt[i] > 0 && pos >= goff[i]) r = i;
-    return r;
-}
-__device__ __forceinline__ void split_hilo(float v0, float v1, uint32_t& hi, uint32_t& lo) {
-    hi = pack_bf16(v0, v1);
-    lo = pack_bf16(v0 - bf16lo(hi), v1 - bf16hi(hi));
-}
-
-template <int KIND>
-__device__ __forceinline__ void epi_pre(EpiPre& P, const CcEpi& E, const CcDims& D, const CcWork& W, const GemmSmemHdr* H,
-                                        int t, int p, int b, int lane) {
-    const int col = t * 128 + 4 * lane;
-    if (KIND == EPI_QKV) {
-        if (col < D.QD + D.KD) {
-            const int half = D.Dh >> 1;
-            const float4* cs = reinterpret_cast<const float4*>(W.rope_cs + (size_t)H->aux[p] * half + ((col % D.Dh) % half));
-            P.f0 = cs[0];
-            P.f1 = cs[1];
-        }
-    } else if (KIND == EPI_O) {
-        if (col < D.d) {
-            const uint8_t* blob = H->blob[replica_of_pos(H->cnt, H->goff, p)];
-            P.u0 = *reinterpret_cast<const uint2*>(E.hidden + (size_t)b * D.d + col);
-            P.u1 = *reinterpret_cast<const uint2*>(blob + D.off_g2 + (size_t)col * 2);
-        }
-    } else if (KIND == EPI_DN) {
-        if (col < D.d) P.f0 = *reinterpret_cast<const float4*>(W.h1 + (size_t)p * D.d + col);
-    }
-}
-
-template <int KIND>
-__device__ __forceinline__ void epi_fin(const EpiPre& P, const CcEpi& E, const CcDims& D, const CcWork& W,
-                                        const GemmSmemHdr* H, int t, int p, int b, float4 a, int lane) {
-    const int col = t * 128 + 4 * lane;
-    if (KIND == EPI_QKV) {
-        // a3 + a4: RoPE at position s-1 (rotate-half pairs (i, i + Dh/2), fp64-built cos/sin table), q kept
-        // in fp32, bf16(k), bf16(v) stored into the page slot of position s-1 (PAPER.md:103 local append).
-        const int hl = D.Dh >> 3;                                // lanes per half head: 16 (Dh 128) or 8 (Dh 64)
-        float4 o;                                                // the partner half of the same head
-        o.x = __shfl_xor_sync(0xffffffffu, a.x, hl); o.y = __shfl_xor_sync(0xffffffffu, a.y, hl);
-        o.z = __shfl_xor_sync(0xffffffffu, a.z, hl); o.w = __shfl_xor_sync(0xffffffffu, a.w, hl);
-        if (col >= D.QD + 2 * D.KD) return;                      // padding columns of the last tile
-        const int pos = H->aux[p], i0 = col % D.Dh;
-        if (col < D.QD + D.KD) {                                 // q or k: rotate
-            const float sg = (lane & hl) ? 1.f : -1.f;           // first half: a cos - b sin; second: b cos + a sin
-            a.x = a.x * P.f0.x + sg * o.x * P.f0.y; a.y = a.y * P.f0.z + sg * o.y * P.f0.w;
-            a.z = a.z * P.f1.x + sg * o.z * P.f1.y; a.w = a.w * P.f1.z + sg * o.w * P.f1.w;
-            if (col < D.QD) {
-                *reinterpret_cast<float4*>(W.q_rot + (size_t)p * D.QD + col) = a;
-                return;
-            }
-        }
-        const int page = H->page[p];
-        if (page < 0 || page >= E.kv.n_pages) {
-            if (lane == 0) atomicOr(W.err, CC_DEVERR_BAD_PAGE);
-            return;
-        }
-        const bool is_k = col < D.QD + D.KD;
-        const int hk = (col - D.QD - (is_k ? 0 : D.KD)) / D.Dh;
-        __nv_bfloat16* dst = (is_k ? E.kv.k_pool : E.kv.v_pool) + (((size_t)page * D.Hkv + hk) * CC_PAGE + pos % CC_PAGE) * D.Dh + i0;
-        *reinterpret_cast<uint2*>(dst) = make_uint2(pack_bf16(a.x, a.y), pack_bf16(a.z, a.w));
-    } else if (KIND == EPI_O) {
-        // a6 + first half of a7: h1 = h + O-projection (kept in fp32); sum of squares of this tile's 128
-        // columns (the RMSNorm statistic; the 1/rms factor is applied by the gate/up epilogue, the GEMM
-        // being linear in a per-row scale); operand y' = h1 * g2 as hi + lo planes.
-        float ss = 0.f;
-        if (col < D.d) {
-            a.x += bf16lo(P.u0.x); a.y += bf16hi(P.u0.x); a.z += bf16lo(P.u0.y); a.w += bf16hi(P.u0.y);
-            *reinterpret_cast<float4*>(W.h1 + (size_t)p * D.d + col) = a;
-            ss = (a.x * a.x + a.y * a.y) + (a.z * a.z + a.w * a.w);
-            uint32_t hi0, lo0, hi1, lo1;
-            split_hilo(a.x * bf16lo(P.u1.x), a.y * bf16hi(P.u1.x), hi0, lo0);
-            split_hilo(a.z * bf16lo(P.u1.y), a.w * bf16hi(P.u1.y), hi1, lo1);
-            uint8_t* dst = W.y_act + act_chunk_off(p, col, D.Mpad, 2, 0) + (col & 7) * 2;
-            *reinterpret_cast<uint2*>(dst) = make_uint2(hi0, hi1);
-            *reinterpret_cast<uint2*>(dst + 1024) = make_uint2(lo0, lo1);
-        }
-#pragma unroll
-        for (int o = 16; o > 0; o >>= 1) ss += __shfl_xor_sync(0xffffffffu, ss, o);
-        if (lane == 0 && t < ((D.d + 127) >> 7)) W.ssq[(size_t)t * D.Mpad + p] = ss;   // not the zero padding tile of an odd tile count
-    } else if (KIND == EPI_GU) {
-        // second half of a7 + a8: scale by 1/rms of the row, a_j = silu(gate_j) * up_j with gate_j, up_j at
-        // interleaved columns 2j, 2j+1 -> hi + lo operand of the down projection.
-        const float inv = __int_as_float(H->aux[p]);
-        const float g0 = a.x * inv, u0 = a.y * inv, g1 = a.z * inv, u1 = a.w * inv;
-        const int k = t * 64 + 2 * lane;                          // output index = K index of the down GEMM
-        if (k >= D.dn.KB * CC_TILE_K) return;                     // padding tile of the last super tile
-        uint32_t hi, lo;
-        split_hilo(g0 / (1.f + __expf(-g0)) * u0, g1 / (1.f + __expf(-g1)) * u1, hi, lo);
-        uint8_t* dst = W.a_act + act_chunk_off(p, k, D.Mpad, 2, 0) + (k & 7) * 2;
-        *reinterpret_cast<uint32_t*>(dst) = hi;
-        *reinterpret_cast<uint32_t*>(dst + 1024) = lo;
-    } else {
-        // a9: out[b] = bf16(h1 + down projection), written to row b = original request order.
-        if (col >= D.d) return;
-        *reinterpret_cast<uint2*>(E.hidden + (size_t)b * D.d + col) =
-            make_uint2(pack_bf16(P.f0.x + a.x, P.f0.y + a.y), pack_bf16(P.f0.z + a.z, P.f0.w + a.w));
-    }
-}
 
 // Slice of the fixup of super tile `st` done by contributor k of m: rows k, k + m, ... of both tiles.
 // KI items (row, tile) per warp iteration, QU pieces of each loaded per round trip (KI * QU loads in
@@ -179,7 +66,7 @@ __device__ __forceinline__ void fixup_tile(const float* __restrict__ part, const
                                            const GemmSmemHdr* H, int st, int c0, int m, int k, int n_pos, int warp,
                                            int lane) {
     constexpr int kWarps = kGemmThreads / 32;
-    const int Mpad = D.Mpad;
+    const int Mpad = D.Mpart;
     const int my_rows = (n_pos - k + m - 1) / m;
     const int n_items = my_rows * CC_G;
     const size_t piece_stride = (size_t)CC_G * Mpad * 128;     // floats between consecutive pieces of a tile
@@ -197,7 +84,7 @@ __device__ __forceinline__ void fixup_tile(const float* __restrict__ part, const
             bb[u] = (it < n_items) ? H->perm[pp[u]] : -1;
             src[u] = part + ((size_t)((c0 + st) * CC_G + j) * Mpad + pp[u]) * 128 + 4 * lane;
             acc[u] = make_float4(0.f, 0.f, 0.f, 0.f);
-            if (bb[u] >= 0) epi_pre<KIND>(pre[u], E, D, W, H, tt[u], pp[u], bb[u], lane);
+            if (bb[u] >= 0) epi_pre<KIND>(pre[u], E, D, W, SmemTab{H}, tt[u], pp[u], bb[u], lane);
         }
         for (int q0 = 0; q0 < m; q0 += QU) {
             float4 v[KI][QU];
@@ -217,7 +104,7 @@ __device__ __forceinline__ void fixup_tile(const float* __restrict__ part, const
         }
 #pragma unroll
         for (int u = 0; u < KI; ++u)
-            if (bb[u] >= 0) epi_fin<KIND>(pre[u], E, D, W, H, tt[u], pp[u], bb[u], acc[u], lane);   // warp-uniform branch
+            if (bb[u] >= 0) epi_fin<KIND>(pre[u], E, D, W, SmemTab{H}, tt[u], pp[u], bb[u], acc[u], lane);   // warp-uniform branch
     }
 }
 
@@ -229,8 +116,9 @@ __device__ __forceinline__ int ld_acquire(const int* p) {
 
 template <int KIND>
 __global__ void __launch_bounds__(kGemmThreads, 1)
-k_gemm(CcGemmGeo G, const uint8_t* __restrict__ act, int planes, float* __restrict__ part, int* __restrict__ flags,
+k_gemm(CcGemmGeo G, const uint8_t* __restrict__ act, float* __restrict__ part, int* __restrict__ flags,
        CcEpi E, CcDims D, CcWork W, const CcLayerTable* __restrict__ tab) {
+    const int planes = D.pl[KIND];             // operand of projection KIND: x, o, y, a
     const CcSched* __restrict__ sched = W.sched;
     const int Mpad = D.Mpad;
     extern __shared__ __align__(1024) uint8_t smem_raw[];
@@ -378,7 +266,7 @@ k_gemm(CcGemmGeo G, const uint8_t* __restrict__ act, int planes, float* __restri
             for (int r = 0; r < CC_MAXR; ++r) {
                 const int cnt = uniform(H->cnt[r]);
                 if (cnt == 0) continue;
-                const uint32_t idesc = umma_idesc_bf16_m128((uint32_t)((cnt + 15) & ~15));
+                const uint32_t idesc = umma_idesc_m128((uint32_t)((cnt + 15) & ~15), D.fmt);
                 int kb = kb_begin;
                 bool first = true;
                 for (long long u = u_begin; u < u_end; ++u) {
@@ -433,7 +321,7 @@ k_gemm(CcGemmGeo G, const uint8_t* __restrict__ act, int planes, float* __restri
                     tc_fence_after();
 #pragma unroll
                     for (int j = 0; j < CC_G; ++j) {
-                        float* dst = part + ((size_t)((blockIdx.x + st) * CC_G + j) * Mpad + goff) * 128 + f;
+                        float* dst = part + ((size_t)((blockIdx.x + st) * CC_G + j) * D.Mpart + goff) * 128 + f;
                         const uint32_t tcol = tmem_base + ((uint32_t)(q * 32) << 16) + buf * 256 + (uint32_t)j * acc_cols;
                         for (int c = 0; c < n; c += 16) {
                             uint32_t v[16];
@@ -473,7 +361,9 @@ k_gemm(CcGemmGeo G, const uint8_t* __restrict__ act, int planes, float* __restri
                         const int nt = (D.d + 127) >> 7;
                         for (int t = 0; t < nt; ++t) ss += W.ssq[(size_t)t * Mpad + p];   // tile order: fixed
                     }
-                    H->aux[p] = __float_as_int(rsqrtf(ss / (float)D.d + D.eps));
+                    H->aux[p] = __float_as_int(b >= 0 ? rsqrtf(ss / (float)D.d + D.eps) / W.inv_in[p] : 0.f);
+                } else if (KIND == EPI_O) {
+                    H->aux[p] = __float_as_int(b >= 0 ? W.inv_in[p] : 0.f);
                 }
             }
         }
@@ -554,11 +444,10 @@ cudaError_t cc_launch_gemm(int which, const CcDims& D, const CcLayerTable* tab, 
     const size_t smem = (size_t)kGemmSmem;
     CcEpi E{assign, batch, seq_lens, kv, hidden};
     int* flags = W.flags + which * CC_FLAG_STRIDE;
-    // every projection takes its activations as hi + lo bf16 planes
     switch (which) {
-        case 0: return cc_launch_kernel(k_gemm<EPI_QKV>, dim3(D.qkv.P), block, smem, L, D.qkv, W.x_act, 2, W.qkv_part, flags, E, D, W, tab);
-        case 1: return cc_launch_kernel(k_gemm<EPI_O>, dim3(D.o.P), block, smem, L, D.o, W.o_act, 2, W.o_part, flags, E, D, W, tab);
-        case 2: return cc_launch_kernel(k_gemm<EPI_GU>, dim3(D.gu.P), block, smem, L, D.gu, W.y_act, 2, W.gu_part, flags, E, D, W, tab);
-        default: return cc_launch_kernel(k_gemm<EPI_DN>, dim3(D.dn.P), block, smem, L, D.dn, W.a_act, 2, W.d_part, flags, E, D, W, tab);
+        case 0: return cc_launch_kernel(k_gemm<EPI_QKV>, dim3(D.qkv.P), block, smem, L, D.qkv, W.x_act, W.qkv_part, flags, E, D, W, tab);
+        case 1: return cc_launch_kernel(k_gemm<EPI_O>, dim3(D.o.P), block, smem, L, D.o, W.o_act, W.o_part, flags, E, D, W, tab);
+        case 2: return cc_launch_kernel(k_gemm<EPI_GU>, dim3(D.gu.P), block, smem, L, D.gu, W.y_act, W.gu_part, flags, E, D, W, tab);
+        default: return cc_launch_kernel(k_gemm<EPI_DN>, dim3(D.dn.P), block, smem, L, D.dn, W.a_act, W.d_part, flags, E, D, W, tab);
     }
 }

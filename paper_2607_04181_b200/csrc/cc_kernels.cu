@@ -77,13 +77,14 @@ __global__ void k_publish(CcLayerTable* row, CcLayerTable value) {
     row->active_mask = value.active_mask;
 }
 
-// One-time weight re-pack: [out][in] bf16 rows -> 16 KiB tile images (128 rows x 64 k, 128B swizzle),
+// One-time weight re-pack: [out][in] bf16 rows -> 16 KiB tile images (fp16 or bf16 elements: CcDims::fmt) (128 rows x 64 k, 128B swizzle),
 // tile (t, kb) at cc_atom_off(k_blocks, t, kb): the CC_G tiles of a super tile are adjacent per k-block.
 // Rows / k beyond the matrix are zero.
 __global__ void __launch_bounds__(256) k_pack(uint8_t* __restrict__ dst, const __nv_bfloat16* __restrict__ src0,
                                               const __nv_bfloat16* __restrict__ src1,
                                               const __nv_bfloat16* __restrict__ src2, int rows0, int rows1, int rows2,
-                                              int mode, int K, int n_tiles, int k_blocks) {
+                                              int mode, int K, int n_tiles, int k_blocks, int fmt,
+                                              uint32_t* __restrict__ overflow) {
     const size_t total = (size_t)n_tiles * k_blocks * (CC_A_TILE_BYTES / 16);
     for (size_t idx = (size_t)blockIdx.x * blockDim.x + threadIdx.x; idx < total; idx += (size_t)gridDim.x * blockDim.x) {
         const int c = idx & 7, i = (idx >> 3) & 127;
@@ -101,6 +102,19 @@ __global__ void __launch_bounds__(256) k_pack(uint8_t* __restrict__ dst, const _
         }
         uint4 v = make_uint4(0, 0, 0, 0);
         if (row && k0 < K) v = *reinterpret_cast<const uint4*>(row + k0);   // K % 8 == 0
+        if (fmt == CC_FMT_F16) {
+            // bf16 -> fp16: exact for 2^-17 <= |w| <= 65504 (fp16 subnormals included), rounded to the 2^-24 grid below that
+            uint32_t w[4] = {v.x, v.y, v.z, v.w};
+            bool bad = false;
+#pragma unroll
+            for (int j = 0; j < 4; ++j) {
+                const float a = bf16lo(w[j]), b = bf16hi(w[j]);
+                bad |= !(fabsf(a) <= 65504.f) || !(fabsf(b) <= 65504.f);
+                w[j] = pack_f16(a, b);
+            }
+            if (bad) atomicOr(overflow, 1u);
+            v = make_uint4(w[0], w[1], w[2], w[3]);
+        }
         *reinterpret_cast<uint4*>(dst + cc_atom_off(k_blocks, t, kb) + (size_t)i * 128 + ((c ^ (i & 7)) << 4)) = v;
     }
 }
@@ -127,8 +141,8 @@ cudaError_t cc_launch_publish(CcLayerTable* row_dev, const CcLayerTable& value, 
 }
 cudaError_t cc_launch_pack(uint8_t* dst, const __nv_bfloat16* src0, const __nv_bfloat16* src1,
                            const __nv_bfloat16* src2, int rows0, int rows1, int rows2, int mode, int K, int n_tiles,
-                           int k_blocks, cudaStream_t st) {
-    k_pack<<<1184, 256, 0, st>>>(dst, src0, src1, src2, rows0, rows1, rows2, mode, K, n_tiles, k_blocks);
+                           int k_blocks, int fmt, uint32_t* overflow_dev, cudaStream_t st) {
+    k_pack<<<1184, 256, 0, st>>>(dst, src0, src1, src2, rows0, rows1, rows2, mode, K, n_tiles, k_blocks, fmt, overflow_dev);
     return cudaGetLastError();
 }
 cudaError_t cc_launch_page_copy(void* k_pool, void* v_pool, size_t page_bytes, const int* src, const int* dst, int n_moves,

@@ -2,6 +2,7 @@
 #pragma once
 #include "cc_common.cuh"
 
+struct CcBigSched;
 // Device workspace of one layer (allocated once at cc_create_layer; PAPER.md:393 persistent pool).
 struct CcWork {
     CcSched* sched;
@@ -9,7 +10,7 @@ struct CcWork {
     int* pg_prefix;      // [max_batch + 1] pages of the rows before row b, request order (attention work split)
     int* pos_of;         // [max_batch] grouped position of row b, or -1
     int* first_wr;       // [max_batch] lowest page index of row b's request that some row of this step appends to
-    uint8_t* x_act;      // packed bf16 GEMM operands, [K/64][Mpad/8][plane hi|lo][8][128 B swizzled]
+    uint8_t* x_act;      // packed GEMM operands, [K/64][Mpad/8][planes][8][128 B swizzled]: one fp16 plane or bf16 hi|lo
     uint8_t* o_act;
     uint8_t* y_act;
     uint8_t* a_act;
@@ -20,13 +21,34 @@ struct CcWork {
     float* q_rot;        // [Mpad][Hq*Dh] fp32, q after RoPE
     float* h1;           // [Mpad][d]     fp32, hidden + O projection
     float* ssq;          // [d/128][Mpad] fp32, per-tile sum of squares of h1 (post-attention RMSNorm statistic)
+    float* inv_in;       // [Mpad] 1/rms of the input row (k_prologue): the O epilogue stores y' = h1 * g2 * inv_in so that the
+                         // operand stays O(1) whatever the scale of `hidden` (fp16 range); the gate/up epilogue divides it out
     int* flags;          // [4][CC_FLAG_STRIDE] stream-K fixup counters, zeroed by k_prologue every step
     int* attn_cnt;       // [Mpad][Hkv] pieces finished per (row, kv head); the last finisher merges and resets
     float* att_o;        // [max_batch + SMs][Hq][Dh] fp32 un-normalised piece outputs (slot = row + CTA)
     float2* att_ml;      // [max_batch + SMs][Hq] (max in log2 units, sum)
+    // ---- large-M path (layers created with max_batch > 256; steps of more than 256 rows: DESIGN.md "Mixed steps") ----
+    CcBigSched* bs;      // counts of the step: decode rows, prompt chunks, prefill work items, the work counter
+    int* row_pos;        // [Mpad] position s-1 of grouped row p, or -1
+    int* row_page;       // [Mpad] page that holds that position, or -1
+    float* gu_scale;     // [Mpad] rms of the input row over rms of h1 (the gate/up epilogue's row scale)
+    int* dec_rows;       // [CC_BIG_MAX_DEC] original row of decode row i (a row outside every prompt chunk)
+    int* chunk_row0;     // [CC_BIG_MAX_CHUNKS] first original row of prompt chunk c (its rows are consecutive)
+    int* chunk_len;      // [CC_BIG_MAX_CHUNKS] rows (tokens) of chunk c
+    int* item_chunk;     // [CC_BIG_MAX_ITEMS] prefill work item -> chunk
+    int* item_tile;      // [CC_BIG_MAX_ITEMS] prefill work item -> query tile of that chunk
     const float2* rope_cs;  // [max_position][Dh/2] (cos, sin), built in fp64 on the host
     uint32_t* err;       // sticky device error word (context-owned)
     unsigned long long* trace;   // CC_TRACE builds: [CC_TRACE_KERNELS][CC_TRACE_POINTS][min, max] of %globaltimer; else null
+};
+
+#define CC_BIG_MAX_DEC 256       // decode rows of a large step (they go through k_attn's page-range split)
+#define CC_BIG_MAX_CHUNKS 64     // prompt chunks of a large step
+#define CC_BIG_MAX_ITEMS 1024    // (chunk, query tile) items of a large step
+struct CcBigSched {
+    int n_dec, n_chunks, n_items, work;
+    int n_dec_pages;             // KV pages of the decode rows (the attention work axis of the large step)
+    int pad_[3];
 };
 
 // ---- tracing build (python -m paper_2607_04181_b200.build --trace; read with cc_debug_trace / timeline.py) ----
@@ -79,20 +101,31 @@ cudaError_t cc_launch_prologue(const int* assign, const int* seq_lens, const int
 // which: 0 = QKV, 1 = O, 2 = gate/up, 3 = down
 cudaError_t cc_launch_gemm(int which, const CcDims& D, const CcLayerTable* tab, const CcWork& W, const int* seq_lens,
                            const int* assign, int batch, const CcKv& kv, __nv_bfloat16* hidden, const CcLaunch& L);
+// rowmap (large steps): original row of entry i of the attention work axis (the decode rows); null = row i itself
 cudaError_t cc_launch_attention(const int* seq_lens, const CcKv& kv, const CcDims& D, const CcLayerTable* tab,
-                                const CcWork& W, const CcLaunch& L);
+                                const CcWork& W, const CcLaunch& L, const int* rowmap = nullptr);
+// ---- large steps (cc_big.cu, cc_big_gemm.cu, cc_prefill.cu) ----
+cudaError_t cc_launch_big_group(const int* assign, const int* seq_lens, const int* block_table, int batch, const CcDims& D,
+                                const CcLayerTable* tab, const CcWork& W, cudaStream_t st);
+cudaError_t cc_launch_big_norm(const __nv_bfloat16* hidden, int batch, const CcDims& D, const CcLayerTable* tab, const CcWork& W,
+                               cudaStream_t st);
+cudaError_t cc_launch_big_rowstat(const CcDims& D, const CcWork& W, cudaStream_t st);
+cudaError_t cc_launch_big_gemm(int which, const CcDims& D, const CcLayerTable* tab, const CcWork& W, const int* seq_lens,
+                               const int* assign, int batch, const CcKv& kv, __nv_bfloat16* hidden, const CcLaunch& L);
+cudaError_t cc_launch_prefill_attention(const int* seq_lens, const CcKv& kv, const CcDims& D, const CcWork& W, const CcLaunch& L);
 
 cudaError_t cc_launch_copy(void* dst, const void* src, size_t bytes, int n_sms, cudaStream_t st);
 cudaError_t cc_launch_page_copy(void* k_pool, void* v_pool, size_t page_bytes, const int* src, const int* dst, int n_moves,
                                 cudaStream_t st);
 cudaError_t cc_launch_publish(CcLayerTable* row_dev, const CcLayerTable& value, cudaStream_t st);
 // mode 0: rows of src0, then src1, then src2 (concatenated); mode 1: rows alternate src0[j], src1[j].
+// fmt = CC_FMT_F16 converts the bf16 weights to fp16; *overflow_dev is set when a weight does not fit (|w| > 65504 or not finite).
 cudaError_t cc_launch_pack(uint8_t* dst, const __nv_bfloat16* src0, const __nv_bfloat16* src1,
                            const __nv_bfloat16* src2, int rows0, int rows1, int rows2, int mode, int K, int n_tiles,
-                           int k_blocks, cudaStream_t st);
-// which: 0 = one packed bf16 plane (K = dim), 1 = fp32 row buffer [Mpad][dim], 2 = hi + lo planes,
-// 3 = hi + lo planes scaled by the row's 1/rms from W.ssq (the un-normalised y' operand)
-cudaError_t cc_launch_tap(const void* src, int which, int dim, const CcDims& D, const CcWork& W,
+                           int k_blocks, int fmt, uint32_t* overflow_dev, cudaStream_t st);
+// which: 1 = fp32 row buffer [Mpad][dim], 2 = packed operand in the layer's format,
+// 3 = packed operand times the row's 1/rms from W.ssq over W.inv_in (the y' operand is stored before its statistic is known)
+cudaError_t cc_launch_tap(const void* src, int which, int planes, int dim, const CcDims& D, const CcWork& W,
                           float* out_dev, int batch, cudaStream_t st);
 int cc_max_hidden();
 

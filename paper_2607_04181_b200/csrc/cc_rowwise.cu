@@ -7,10 +7,10 @@
 // this file is a function of the layer shape and seq_len only (never of the batch split), which
 // is what makes outputs bit-identical across replica counts.
 //
-// GEMM operands are written as TWO bf16 planes, hi = bf16(v) and lo = bf16(v - hi): the tensor
-// core multiplies the bf16 weights by both and accumulates in fp32, so the activations carry
-// ~16 mantissa bits.  One bf16 plane alone costs ~6e-3 rms on the layer output at d = 4096,
-// too close to the 1e-2 absolute tolerance.
+// GEMM operands are written in the layer's operand format (act_store, cc_common.cuh): ONE fp16 plane
+// (11 significand bits) against fp16 weights, or TWO bf16 planes hi = bf16(v), lo = bf16(v - hi) against
+// bf16 weights.  One bf16 plane alone costs ~6e-3 rms on the layer output at d = 4096, too close to the
+// 1e-2 absolute tolerance.
 #include "cc_kernels.h"
 
 namespace {
@@ -27,12 +27,6 @@ __device__ __forceinline__ float block_sum(float v, float* red) {
     const int nw = blockDim.x >> 5;
     for (int i = 0; i < nw; ++i) t += red[i];
     return t;
-}
-
-// hi/lo split of two values -> packed bf16x2 words of the two planes.
-__device__ __forceinline__ void split_hilo(float v0, float v1, uint32_t& hi, uint32_t& lo) {
-    hi = pack_bf16(v0, v1);
-    lo = pack_bf16(v0 - bf16lo(hi), v1 - bf16hi(hi));
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -204,21 +198,22 @@ __global__ void __launch_bounds__(kNormThreads) k_prologue(const int* __restrict
         const int c = threadIdx.x + j * kNormThreads;
         if (c >= nchunk) break;
         const uint32_t w[4] = {v[j].x, v[j].y, v[j].z, v[j].w}, gw[4] = {gv[j].x, gv[j].y, gv[j].z, gv[j].w};
-        uint32_t hi[4], lo[4];
+        float x[8];
 #pragma unroll
-        for (int i = 0; i < 4; ++i)
-            split_hilo(bf16lo(w[i]) * inv * bf16lo(gw[i]), bf16hi(w[i]) * inv * bf16hi(gw[i]), hi[i], lo[i]);
-        uint8_t* dst = W.x_act + act_chunk_off(mypos, c << 3, D.Mpad, 2, 0);
-        *reinterpret_cast<uint4*>(dst) = make_uint4(hi[0], hi[1], hi[2], hi[3]);
-        *reinterpret_cast<uint4*>(dst + 1024) = make_uint4(lo[0], lo[1], lo[2], lo[3]);
+        for (int i = 0; i < 4; ++i) {
+            x[2 * i] = bf16lo(w[i]) * inv * bf16lo(gw[i]);
+            x[2 * i + 1] = bf16hi(w[i]) * inv * bf16hi(gw[i]);
+        }
+        act_store<8>(W.x_act, D, D.pl[CC_OP_X], mypos, c << 3, x);
     }
+    if (threadIdx.x == 0) W.inv_in[mypos] = inv;
     if (b == 0) CC_TP(W, 0, 2);
 }
 
 // Test tap: widen a workspace buffer to fp32 [batch][dim] in original row order.
-// which: 0 = one bf16 plane, 1 = fp32 rows, 2 = hi + lo planes, 3 = hi + lo planes times the row's
-// 1/rms (the y' operand is stored un-normalised; its statistic lives in W.ssq).
-__global__ void __launch_bounds__(256) k_tap(const void* __restrict__ src, int which, int dim, CcDims D,
+// which: 1 = fp32 rows, 2 = packed operand (the layer's format), 3 = packed operand times the row's
+// 1/rms over the input row's 1/rms (the y' operand is stored before its statistic, W.ssq, is known).
+__global__ void __launch_bounds__(256) k_tap(const void* __restrict__ src, int which, int planes, int dim, CcDims D,
                                              CcWork W, float* __restrict__ out, int batch) {
     const int pos = blockIdx.x;
     if (pos >= W.sched->n_pos) return;
@@ -228,16 +223,21 @@ __global__ void __launch_bounds__(256) k_tap(const void* __restrict__ src, int w
     if (which == 3) {
         float ss = 0.f;
         for (int t = 0; t < (D.d + 127) / 128; ++t) ss += W.ssq[(size_t)t * D.Mpad + pos];
-        scale = rsqrtf(ss / (float)D.d + D.eps);
+        scale = rsqrtf(ss / (float)D.d + D.eps) / W.inv_in[pos];
     }
     for (int k = threadIdx.x; k < dim; k += blockDim.x) {
         float v;
         if (which == 1) {
             v = reinterpret_cast<const float*>(src)[(size_t)pos * dim + k];
         } else {
-            const uint8_t* p = reinterpret_cast<const uint8_t*>(src) + act_chunk_off(pos, k, D.Mpad, which >= 2 ? 2 : 1, 0) + (k & 7) * 2;
-            v = __bfloat162float(*reinterpret_cast<const __nv_bfloat16*>(p));
-            if (which >= 2) v += __bfloat162float(*reinterpret_cast<const __nv_bfloat16*>(p + 1024));
+            const uint8_t* p = reinterpret_cast<const uint8_t*>(src) + act_chunk_off(pos, k, D.Mpad, planes, 0) + (k & 7) * 2;
+            if (D.fmt == CC_FMT_F16) {
+                v = __half2float(*reinterpret_cast<const __half*>(p));
+                if (planes == 2) v += __half2float(*reinterpret_cast<const __half*>(p + 1024));
+            } else {
+                v = __bfloat162float(*reinterpret_cast<const __nv_bfloat16*>(p));
+                v += __bfloat162float(*reinterpret_cast<const __nv_bfloat16*>(p + 1024));
+            }
             v *= scale;
         }
         out[(size_t)b * dim + k] = v;
@@ -253,9 +253,9 @@ cudaError_t cc_launch_prologue(const int* assign, const int* seq_lens, const int
     return cc_launch_kernel(k_prologue, dim3(batch), dim3(kNormThreads), 0, L, assign, seq_lens, block_table, batch, hidden, D, tab,
                             W, so);
 }
-cudaError_t cc_launch_tap(const void* src, int which, int dim, const CcDims& D, const CcWork& W,
+cudaError_t cc_launch_tap(const void* src, int which, int planes, int dim, const CcDims& D, const CcWork& W,
                           float* out_dev, int batch, cudaStream_t st) {
-    k_tap<<<D.Mpad, 256, 0, st>>>(src, which, dim, D, W, out_dev, batch);
+    k_tap<<<D.Mpad, 256, 0, st>>>(src, which, planes, dim, D, W, out_dev, batch);
     return cudaGetLastError();
 }
 int cc_max_hidden() { return kNormVec * 8 * kNormThreads; }

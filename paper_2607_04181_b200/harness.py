@@ -90,11 +90,14 @@ class Session:
     """Context + one layer + a donated arena for replica slots."""
 
     def __init__(self, shape: I.LayerShape, weights: dict, max_batch: int, n_slots: int = I.MAX_REPLICAS - 1,
-                 device_index: int = 0, max_blocks: int | None = None, max_position: int | None = None):
+                 device_index: int = 0, max_blocks: int | None = None, max_position: int | None = None,
+                 operand_format: int | None = None):
         self.shape = shape
         self.device = f"cuda:{device_index}"
         torch.cuda.set_device(device_index)
         self.ctx = B.cc_ctx_create(device_index)
+        if operand_format is not None:
+            B.cc_ctx_set_operand_format(self.ctx, operand_format)
         self.desc = make_desc(shape, max_batch, max_blocks, max_position)
         wdev = {k: _dev_u16(v, self.device) for k, v in weights.items()}
         self.layer = B.cc_create_layer(self.ctx, self.desc, wdev)

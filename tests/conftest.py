@@ -24,3 +24,11 @@ def pytest_collection_modifyitems(config, items):
     for item in items:
         if "gpu" in item.keywords:
             item.add_marker(skip)
+
+
+@pytest.fixture(params=["f16", "bf16x2"])
+def operand_format(request, monkeypatch):
+    """Runs a test once per GEMM operand format (include/cocoscale.h cc_ctx_set_operand_format): cc_ctx_create reads
+    CC_OPERAND_FORMAT, so every context the test makes packs its layers in that format."""
+    monkeypatch.setenv("CC_OPERAND_FORMAT", request.param)
+    return request.param

@@ -11,7 +11,7 @@ import oracle
 from paper_2607_04181_b200 import inputs as I
 from tests.test_gpu_parity import check_against_oracle, check_grouping
 
-pytestmark = pytest.mark.gpu
+pytestmark = [pytest.mark.gpu, pytest.mark.usefixtures("operand_format")]   # both GEMM operand formats
 
 
 @pytest.fixture(scope="module")

@@ -11,7 +11,7 @@ import pytest
 from paper_2607_04181_b200 import inputs as I
 from tests.test_gpu_parity import check_against_oracle, check_grouping, run_case
 
-pytestmark = pytest.mark.gpu
+pytestmark = [pytest.mark.gpu, pytest.mark.usefixtures("operand_format")]   # both GEMM operand formats
 
 LONG = 8192                                                        # cached tokens of the long row (seq_len 8193)
 

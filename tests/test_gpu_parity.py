@@ -9,7 +9,7 @@ import torch
 import oracle
 from paper_2607_04181_b200 import inputs as I
 
-pytestmark = pytest.mark.gpu
+pytestmark = [pytest.mark.gpu, pytest.mark.usefixtures("operand_format")]   # both GEMM operand formats
 
 ATOL, RTOL = 1e-2, 2e-2
 
