@@ -63,6 +63,7 @@ def parse_args():
                          "decode graph with layers 10-12 flipped to 2 replicas and back (latency series, not the headline); "
                          "cfg5: configs[4], the co-located serving loop (decode only)")
     ap.add_argument("--horizon", type=float, default=120.0, help="cfg5: seconds of synthetic arrivals")
+    ap.add_argument("--layers", type=int, default=1, help="cfg4: layers of the mixed-step graph (configs[3] names 40; default one hot layer)")
     return ap.parse_args()
 
 
@@ -708,11 +709,12 @@ def run_cfg3(args):
 # cfg5 (BASELINE.json configs[4]): skewed co-located serving, decode only (no prefill kernel yet: NEXT-2)
 # ---------------------------------------------------------------------------------------------
 def run_cfg4(args):
-    """BASELINE.json configs[3], ONE layer of the 14B-class shape: a mixed step of two 2048-token prompt chunks and 256
-    decode rows.  There is no large-M kernel (NEXT-2): the step runs as 17 cc_forward calls of 256 rows each -- eight per
-    prompt (rows = consecutive tokens sharing the request's block-table row: causal prefill through the decode path,
-    tests/test_prefill_chunk.py), one for the decode rows -- captured in one graph.  Reported so that the config has a
-    measured line; what it shows is the GEMM at n = 256 (tensor-bound) and an attention that re-reads every prefix."""
+    """BASELINE.json configs[3]: the 14B-class shape, a mixed step of two 2048-token prompt chunks and 256 decode rows
+    (contexts U{256..4096}) = 4352 rows in ONE cc_forward per layer through the large-M path: k_big_group, CTA-pair
+    tcgen05 GEMMs with fused epilogues, chunk-prefill attention on tcgen05 for the prompts, the page-range decode
+    attention for the decode rows.  --layers L runs L layers in one graph, the top 25 % by a
+    seeded synthetic per-layer load at R = 2 (prompt r on replica r % 2, decode rows split evenly), the rest at R = 1;
+    the default is one hot layer.  The GEMMs are tensor-bound here: their roofline is the measured bf16 GEMM peak."""
     import torch
 
     from paper_2607_04181_b200 import binding as B
@@ -724,44 +726,55 @@ def run_cfg4(args):
     dev = "cuda:0"
     torch.cuda.set_device(0)
     shape = I.CFG4_LAYER
-    page, rows, prompt, n_prompts = shape.page, 256, 2048, 2
+    n_layers = max(1, args.layers)
+    page, n_dec, prompt, n_prompts = shape.page, 256, 2048, 2
+    rows = n_prompts * prompt + n_dec
     rng = np.random.default_rng(3004)
-    dec_ctx = rng.integers(256, 4097, rows)                                   # decode contexts U{256..4096}
+    dec_ctx = rng.integers(256, 4097, n_dec)                                  # decode contexts U{256..4096}
     width = (4096 + 1 + page - 1) // page
     need = np.concatenate([[prompt // page] * n_prompts, (dec_ctx + 1 + page - 1) // page]).astype(np.int64)
     n_pages = int(need.sum())
     ids = rng.permutation(n_pages).astype(np.int32)
-    req_bt = np.full((n_prompts + rows, width), -1, np.int32)
+    req_bt = np.full((n_prompts + n_dec, width), -1, np.int32)
     off = 0
     for i, n in enumerate(need):
         req_bt[i, :n] = ids[off:off + n]
         off += int(n)
+    # rows: prompt 0 (tokens 0..2047 at seq_len t + 1, sharing its request's block-table row), prompt 1, the decode rows
+    bt = np.concatenate([np.repeat(req_bt[r:r + 1], prompt, 0) for r in range(n_prompts)] + [req_bt[n_prompts:]]).astype(np.int32)
+    seq = np.concatenate([np.arange(1, prompt + 1)] * n_prompts + [dec_ctx + 1]).astype(np.int32)
+    hot_assign = np.concatenate([np.full(prompt, r % 2) for r in range(n_prompts)] + [I.even_split(n_dec, 2)]).astype(np.int32)
+    load = np.random.default_rng(3104).lognormal(0.0, 1.0, n_layers)
+    hot = sorted(np.argsort(-load)[:max(1, n_layers // 4)].tolist())          # top 25 % by synthetic load (one layer: that layer)
     gen = torch.Generator(device=dev).manual_seed(1004)
 
     def randn(*shp, std=1.0, mean=0.0):
         return (torch.randn(*shp, generator=gen, device=dev, dtype=torch.float32) * std + mean).to(torch.bfloat16)
     d, F, QD, KD = shape.hidden, shape.ffn, shape.q_dim, shape.kv_dim
-    S = ModelSession(shape, [], max_batch=rows, n_slots=1, max_blocks=width, max_position=width * page)
-    S.add_layer({"g1": randn(d, std=0.02, mean=1.0), "wq": randn(QD, d, std=0.02), "wk": randn(KD, d, std=0.02),
-                 "wv": randn(KD, d, std=0.02), "wo": randn(d, QD, std=0.02), "g2": randn(d, std=0.02, mean=1.0),
-                 "wgate": randn(F, d, std=0.02), "wup": randn(F, d, std=0.02), "wdown": randn(d, F, std=0.02)})
+    S = ModelSession(shape, [], max_batch=rows, n_slots=len(hot), max_blocks=width, max_position=width * page)
+    for _ in range(n_layers):
+        S.add_layer({"g1": randn(d, std=0.02, mean=1.0), "wq": randn(QD, d, std=0.02), "wk": randn(KD, d, std=0.02),
+                     "wv": randn(KD, d, std=0.02), "wo": randn(d, QD, std=0.02), "g2": randn(d, std=0.02, mean=1.0),
+                     "wgate": randn(F, d, std=0.02), "wup": randn(F, d, std=0.02), "wdown": randn(d, F, std=0.02)})
     S.donate()
-    S.scale(0, 2)                                                             # configs[3]: the hot layers run at R = 2
+    for l in hot:
+        S.scale(l, 2)
     pool_shape = (n_pages, shape.n_kv_heads, page, shape.head_dim)
-    kp, vp = randn(*pool_shape), randn(*pool_shape)
-    subs = []                                                                 # (hidden, block table, seq_lens, assign) per call
-    for r in range(n_prompts):
-        for c in range(prompt // rows):
-            seq = np.arange(c * rows + 1, (c + 1) * rows + 1, dtype=np.int32)
-            subs.append((randn(rows, d), torch.from_numpy(np.repeat(req_bt[r:r + 1], rows, 0)).to(dev), torch.from_numpy(seq).to(dev),
-                         torch.full((rows,), r % 2, dtype=torch.int32, device=dev)))       # a request lives on one replica
-    subs.append((randn(rows, d), torch.from_numpy(req_bt[n_prompts:]).to(dev), torch.from_numpy((dec_ctx + 1).astype(np.int32)).to(dev),
-                 torch.from_numpy(I.even_split(rows, 2)).to(dev)))
+    # one KV pool per layer while that fits beside the weights; many layers share a few pools round-robin (every layer
+    # still streams its own 2.3 GB of decode KV from HBM each step -- far more than L2 -- and appends its rows)
+    n_pools = min(n_layers, 8)
+    pools = [(randn(*pool_shape), randn(*pool_shape)) for _ in range(n_pools)]
+    hidden0 = randn(rows, d)
+    hidden = hidden0.clone()
+    d_bt, d_seq = torch.from_numpy(bt).to(dev), torch.from_numpy(seq).to(dev)
+    d_hot, d_cold = torch.from_numpy(hot_assign).to(dev), torch.zeros(rows, dtype=torch.int32, device=dev)
     stream = torch.cuda.current_stream()
 
     def mixed_step(st):
-        for h, bt, sl, ra in subs:
-            B.cc_forward(S.layers[0], h, kp, vp, bt, n_pages, sl, ra, rows, st)
+        hidden.copy_(hidden0)                                                 # a fresh batch every step (the layers update it in place)
+        for l in range(n_layers):
+            kp, vp = pools[l % n_pools]
+            B.cc_forward(S.layers[l], hidden, kp, vp, d_bt, n_pages, d_seq, d_hot if l in hot else d_cold, rows, st)
     mixed_step(stream)
     torch.cuda.synchronize()
     assert B.cc_poll_device_error(S.ctx) == 0
@@ -783,39 +796,56 @@ def run_cfg4(args):
         graph.replay()
         torch.cuda.synchronize()
     clocks = sampler.stop()
-    # per-kernel times of the 17 calls (kernel by kernel, no PDL)
-    stage = np.zeros(len(B.STAGE_NAMES))
-    for rep in range(3):
-        acc = np.zeros(len(B.STAGE_NAMES))
-        for h, bt, sl, ra in subs:
-            acc += B.cc_forward_profiled(S.layers[0], h, kp, vp, bt, n_pages, sl, ra, rows, stream)
-        stage = acc if rep == 0 else np.minimum(stage, acc)
-    tokens = len(subs) * rows
-    n_w = d * (QD + 2 * KD) + QD * d + 3 * d * F
-    gemm_ms = float(sum(stage[i] for i, n in enumerate(B.STAGE_NAMES) if n.startswith("gemm")))
-    attn_ms = float(stage[B.STAGE_NAMES.index("attention")])
-    kv_tok = sum(int(sl.sum().item()) for _, _, sl, _ in subs)
+    # per-kernel times of one hot layer's step (kernel by kernel, events between)
+    kp, vp = pools[hot[0] % n_pools]
+    stage = None
+    for rep in range(4):
+        t = B.cc_forward_profiled(S.layers[hot[0]], hidden, kp, vp, d_bt, n_pages, d_seq, d_hot, rows, stream).astype(np.float64)
+        stage = t if stage is None else np.minimum(stage, t)
+    names = B.BIG_STAGE_NAMES
+    planes = 1 if B.cc_layer_operand_format(S.layers[0]) == B.CC_OPERAND_F16 else 2
+    n_w = {"gemm_qkv": d * (QD + 2 * KD), "gemm_o": QD * d, "gemm_gate_up": 2 * d * F, "gemm_down": d * F}
+    # tensor work issued per projection: the large-step plane policy is {x: 2, o: 1, y: 1, a: 1} for fp16 layers (cc_api.cu)
+    pl = {"gemm_qkv": 2, "gemm_o": planes, "gemm_gate_up": planes, "gemm_down": planes}
     peaks = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json"))) if os.path.exists(os.path.join(ROOT, "MEASURED_PEAKS.json")) else {}
+    sust = peaks.get("bf16_tflops_sustained")
+    gemm = {}
+    for n in n_w:
+        t_ms = float(stage[names.index(n)])
+        gemm[n] = {"ms": round(t_ms, 4), "useful_TFLOPs": round(2.0 * rows * n_w[n] / (t_ms * 1e-3) / 1e12, 1),
+                   "issued_TFLOPs": round(pl[n] * 2.0 * rows * n_w[n] / (t_ms * 1e-3) / 1e12, 1), "planes": pl[n]}
+    gemm_ms = sum(float(stage[names.index(n)]) for n in n_w)
+    useful = 2.0 * rows * sum(n_w.values()) / (gemm_ms * 1e-3) / 1e12
+    issued = sum(pl[n] * 2.0 * rows * n_w[n] for n in n_w) / (gemm_ms * 1e-3) / 1e12
+    # attention work: prompts (causal, 4 * n^2 / 2 * Hq * Dh flop each; x 2 for the hi + lo planes of q and p) and decode KV bytes
+    pf_flop = n_prompts * 4.0 * (prompt * (prompt + 1) / 2) * QD
+    pf_ms, dec_ms = float(stage[names.index("attention_prefill")]), float(stage[names.index("attention_decode")])
+    dec_bytes = int((dec_ctx + 1).sum()) * 2 * KD * 2
+    hbm, _ = measured_peak()
     S.close()
     line = {
-        "metric": "mixed prefill + decode step of one 14B-class layer (cfg4): tokens/s", "value": tokens / (ms * 1e-3), "unit": UNIT,
-        "n_gpus": 1, "steps": K, "warmup": W, "ms_per_step": ms, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
-        "dtype": "bf16", "data": "synthetic",
-        "config": {"workload": "cfg4 (BASELINE.json configs[3]), ONE layer: hidden 5120, 40 q / 8 kv heads x 128, FFN 17408, R = 2; mixed step = "
-                               "2 x 2048 prompt tokens + 256 decode rows (contexts U{256..4096}) = 4352 rows, run as 17 cc_forward calls of 256 rows "
-                               "in one CUDA graph (no large-M kernel: every call streams the layer's weights; a prompt token re-reads its prefix)",
-                   "calls_per_step": len(subs), "rows_per_call": rows},
-        "clocks": clocks, "gpu_launches": K * len(subs) * len(B.STAGE_NAMES),
-        "gemm": {"ms_per_step_kernel_by_kernel": round(gemm_ms, 4), "flops_per_step_one_plane": 2.0 * tokens * n_w,
-                 "TFLOPs_one_plane": round(2.0 * tokens * n_w / (gemm_ms * 1e-3) / 1e12, 1),
-                 "TFLOPs_issued_two_planes": round(4.0 * tokens * n_w / (gemm_ms * 1e-3) / 1e12, 1),
-                 "measured_bf16_peak_TFLOPs_burst": peaks.get("bf16_tflops"), "measured_bf16_peak_TFLOPs_sustained": peaks.get("bf16_tflops_sustained"),
-                 "weight_bytes_streamed": len(subs) * n_w * 2},
-        "attention": {"ms_per_step_kernel_by_kernel": round(attn_ms, 4), "kv_bytes_streamed": kv_tok * 2 * KD * 2,
-                      "GBps_per_row_algorithmic": round(kv_tok * 2 * KD * 2 / (attn_ms * 1e-3) / 1e9, 1),
-                      "note": "bytes counted per row; the 256 rows of a prompt call read the same pages, so most of them are L2 hits "
-                              "(the figure can exceed the HBM peak)"},
-        "stages_ms": {n: round(float(x), 4) for n, x in zip(B.STAGE_NAMES, stage)},
+        "metric": "mixed prefill + decode step (cfg4): tokens/s", "value": rows / (ms * 1e-3), "unit": UNIT,
+        "n_gpus": 1, "steps": K, "warmup": W, "ms_per_step": ms, "ms_per_layer": ms / n_layers, "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": "bf16", "data": "synthetic",
+        "operand_format": "fp16 weight images; activation planes per projection below" if planes == 1 else "bf16 x two planes",
+        "config": {"workload": f"cfg4 (BASELINE.json configs[3]): {n_layers} layer(s) of hidden 5120, 40 q / 8 kv heads x 128, FFN 17408; "
+                               "mixed step = 2 x 2048 prompt tokens (chunk prefill from position 0) + 256 decode rows (contexts U{256..4096}) "
+                               "= 4352 rows in one cc_forward per layer (large-M path), one CUDA graph",
+                   "layers": n_layers, "hot_layers_at_R2": hot, "kv_pools": n_pools,
+                   "l2": "each layer streams 0.66-1.3 GB of weights and 2.3 GB of decode KV per step (L2 = 126 MB)"},
+        "clocks": clocks, "gpu_launches": K * n_layers * len(names),
+        "roofline": {"bound": "tensor", "kernel": "the four large-M GEMMs of one layer step", "achieved": round(useful, 1),
+                     "achieved_issued": round(issued, 1), "peak": sust, "unit": "TFLOP/s",
+                     "frac": round(useful / sust, 4) if sust else None, "frac_issued": round(issued / sust, 4) if sust else None,
+                     "peak_source": "MEASURED_PEAKS.json bf16_tflops_sustained (cuBLAS bf16, seconds-long loop)", "traffic": None,
+                     "how": "useful = 2 * rows * weights flop; issued counts the second activation plane of the QKV projection"},
+        "gemm": gemm,
+        "attention": {"prefill_ms": round(pf_ms, 4), "prefill_useful_TFLOPs": round(pf_flop / (pf_ms * 1e-3) / 1e12, 1),
+                      "prefill_issued_TFLOPs": round(2 * pf_flop / (pf_ms * 1e-3) / 1e12, 1),
+                      "decode_ms": round(dec_ms, 4), "decode_kv_bytes": dec_bytes,
+                      "decode_GBps": round(dec_bytes / (dec_ms * 1e-3) / 1e9, 1), "decode_frac_of_hbm_peak": round(dec_bytes / (dec_ms * 1e-3) / 1e9 / hbm, 4)},
+        "stages_ms": {n: round(float(x), 4) for n, x in zip(names, stage)},
+        "sum_of_stages_ms": round(float(stage.sum()), 4),
     }
     print(json.dumps(line), flush=True)
     return 0

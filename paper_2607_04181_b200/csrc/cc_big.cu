@@ -42,7 +42,8 @@ __global__ void __launch_bounds__(kGroupThreads) k_big_group(const int* __restri
     __shared__ unsigned char s_cont[CC_BIG_MAX_ROWS + 1];     // row b continues the chunk of row b - 1
     __shared__ int s_w[kGroupThreads / 32];
     __shared__ int s_cnt[CC_MAXR], s_goff[CC_MAXR + 1], s_run[CC_MAXR];
-    __shared__ int s_ndec, s_nchunk, s_pages;
+    __shared__ int s_ndec, s_nchunk, s_ntail, s_pages, s_pages_dec;
+    __shared__ int s_head[CC_BIG_MAX_CHUNKS], s_tail[CC_BIG_MAX_CHUNKS], s_ntile[CC_BIG_MAX_CHUNKS];
     const int tid = threadIdx.x;
     const uint32_t mask = tab->active_mask;
     uint32_t err = 0;
@@ -61,8 +62,8 @@ __global__ void __launch_bounds__(kGroupThreads) k_big_group(const int* __restri
         if (b < batch) s_rep[b] = (signed char)rep;
         bool cont = false;
         if (b < batch && b > 0 && rep >= 0) {
-            const int sp = seq_lens[b - 1];
-            cont = sp > 0 && seq_lens[b] == sp + 1 &&
+            uint32_t e2 = 0;                                           // (row b - 1 reports its own errors)
+            cont = cc_row_replica(assign, seq_lens, b - 1, batch, D, mask, e2) >= 0 && seq_lens[b] == seq_lens[b - 1] + 1 &&
                    block_table[(size_t)b * D.max_blocks] == block_table[(size_t)(b - 1) * D.max_blocks];
         }
         if (b < batch) s_cont[b] = cont ? 1 : 0;
@@ -84,7 +85,9 @@ __global__ void __launch_bounds__(kGroupThreads) k_big_group(const int* __restri
         s_goff[CC_MAXR] = off;
         s_ndec = 0;
         s_nchunk = 0;
+        s_ntail = 0;
         s_pages = 0;
+        s_pages_dec = 0;
     }
     __syncthreads();
     // ---- pass 2: grouped positions (stable), per-row tables, decode-row list with its page prefix ----
@@ -122,6 +125,7 @@ __global__ void __launch_bounds__(kGroupThreads) k_big_group(const int* __restri
             if (i < CC_BIG_MAX_DEC) {
                 W.dec_rows[i] = b;
                 W.pg_prefix[i] = s_pages + pg;
+                if (i == CC_BIG_MAX_DEC - 1 || (di == n_here - 1)) atomicMax(&s_pages_dec, s_pages + pg + npg);   // end of the list so far
             } else {
                 err |= CC_DEVERR_TOO_MANY_DECODE;
             }
@@ -133,49 +137,67 @@ __global__ void __launch_bounds__(kGroupThreads) k_big_group(const int* __restri
         }
         __syncthreads();
     }
-    // chunk heads: a live row that does not continue a chunk but whose successor does
+    // chunks: a head is a live row that does not continue a chunk but whose successor does; a tail is a row that
+    // continues one and whose successor does not.  Runs are disjoint and ordered, so head c pairs with tail c.
     for (int b0 = 0; b0 < batch; b0 += kGroupThreads) {
         const int b = b0 + tid;
         const bool head = b < batch && s_rep[b] >= 0 && !s_cont[b] && s_cont[b + 1];
-        int n_here;
+        const bool tail = b < batch && s_cont[b] && !s_cont[b + 1];
+        int n_here, t_here;
         const int ci = block_scan_excl(head ? 1 : 0, s_w, &n_here);
+        const int ti = block_scan_excl(tail ? 1 : 0, s_w, &t_here);
         if (head) {
-            const int c = s_nchunk + ci;
-            if (c < CC_BIG_MAX_CHUNKS) {
-                int len = 1;
-                while (s_cont[b + len]) ++len;                      // s_cont[batch] = 0 ends the last run
-                W.chunk_row0[c] = b;
-                W.chunk_len[c] = len;
-            } else {
-                err |= CC_DEVERR_TOO_MANY_DECODE;
-            }
+            if (s_nchunk + ci < CC_BIG_MAX_CHUNKS) s_head[s_nchunk + ci] = b; else err |= CC_DEVERR_TOO_MANY_DECODE;
         }
+        if (tail && s_ntail + ti < CC_BIG_MAX_CHUNKS) s_tail[s_ntail + ti] = b;
         __syncthreads();
-        if (tid == 0) s_nchunk += n_here;
+        if (tid == 0) {
+            s_nchunk += n_here;
+            s_ntail += t_here;
+        }
         __syncthreads();
     }
     if (err) atomicOr(W.err, err);
-    if (tid == 0) {
-        const int n_dec = min(s_ndec, CC_BIG_MAX_DEC), n_chunks = min(s_nchunk, CC_BIG_MAX_CHUNKS);
-        // the page prefix of the unused decode slots = the total (k_attn reads CC_BIG_MAX_DEC + 1 entries)
-        int total = 0;
-        if (n_dec > 0) {
-            const int last = W.dec_rows[n_dec - 1];
-            total = W.pg_prefix[n_dec - 1] + (seq_lens[last] + CC_PAGE - 1) / CC_PAGE;
-        }
-        for (int i = n_dec; i <= CC_BIG_MAX_DEC; ++i) W.pg_prefix[i] = total;
-        // prefill work items: (chunk, query tile), the late (long-prefix, expensive) tiles first
-        const int T = 128 / D.G;
-        int n_items = 0;
-        int jmax = 0;
-        for (int c = 0; c < n_chunks; ++c) jmax = max(jmax, (W.chunk_len[c] + T - 1) / T);
-        for (int j = jmax - 1; j >= 0; --j)
+    const int n_chunks = min(s_nchunk, CC_BIG_MAX_CHUNKS);
+    const int T = 128 / D.G;                                           // tokens of a query tile
+    if (tid < n_chunks) {
+        const int len = s_tail[tid] - s_head[tid] + 1;
+        W.chunk_row0[tid] = s_head[tid];
+        W.chunk_len[tid] = len;
+        s_ntile[tid] = (len + T - 1) / T;
+    }
+    __syncthreads();
+    // prefill work items (chunk, query tile): the late (long-prefix, expensive) tiles first.  Thread t owns tile index
+    // j = jmax - 1 - t of every chunk that has one; a scan over t gives its items their places.
+    int jmax = 0;
+    for (int c = 0; c < n_chunks; ++c) jmax = max(jmax, s_ntile[c]);
+    int n_items_tot = 0;
+    for (int t0 = 0; t0 < jmax; t0 += kGroupThreads) {
+        const int j = jmax - 1 - (t0 + tid);
+        int cntj = 0;
+        if (j >= 0)
+            for (int c = 0; c < n_chunks; ++c) cntj += s_ntile[c] > j;
+        int here;
+        int at = n_items_tot + block_scan_excl(cntj, s_w, &here);
+        if (j >= 0)
             for (int c = 0; c < n_chunks; ++c)
-                if (j < (W.chunk_len[c] + T - 1) / T && n_items < CC_BIG_MAX_ITEMS) {
-                    W.item_chunk[n_items] = c;
-                    W.item_tile[n_items] = j;
-                    ++n_items;
+                if (s_ntile[c] > j) {
+                    if (at < CC_BIG_MAX_ITEMS) {
+                        W.item_chunk[at] = c;
+                        W.item_tile[at] = j;
+                    }
+                    ++at;
                 }
+        n_items_tot += here;
+        __syncthreads();
+    }
+    if (n_items_tot > CC_BIG_MAX_ITEMS && tid == 0) atomicOr(W.err, CC_DEVERR_TOO_MANY_DECODE);
+    if (tid == 0) {
+        const int n_dec = min(s_ndec, CC_BIG_MAX_DEC);
+        const int n_items = min(n_items_tot, CC_BIG_MAX_ITEMS);
+        // the page prefix of the unused decode slots = the total (k_attn reads CC_BIG_MAX_DEC + 1 entries)
+        const int total = s_pages_dec;
+        for (int i = n_dec; i <= CC_BIG_MAX_DEC; ++i) W.pg_prefix[i] = total;
         int nmax = 0;
         for (int r = 0; r < CC_MAXR; ++r) {
             W.sched->cnt[r] = s_cnt[r];

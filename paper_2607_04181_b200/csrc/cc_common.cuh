@@ -405,8 +405,11 @@ __device__ __forceinline__ uint32_t mapa_u32(uint32_t local_smem_addr, uint32_t 
     asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(r) : "r"(local_smem_addr), "r"(cta));
     return r;
 }
+// (default semantics: release at CTA scope.  With .release.cluster the compiler emits MEMBAR.ALL.GPU in front of every
+// arrive -- measured: ~1300 cycles per k-block in the relay warp of the large-M GEMM, the kernel's whole bound.  What
+// the arrivals order here was written by the async proxy (TMA) or read through TMEM, not by this thread's stores.)
 __device__ __forceinline__ void mbar_arrive_cluster(uint32_t cluster_addr) {
-    asm volatile("mbarrier.arrive.release.cluster.shared::cluster.b64 _, [%0];" ::"r"(cluster_addr) : "memory");
+    asm volatile("mbarrier.arrive.shared::cluster.b64 _, [%0];" ::"r"(cluster_addr) : "memory");
 }
 template <int kCols>
 __device__ __forceinline__ void tmem_alloc_pair(uint32_t* dst_smem) {   // one full warp in EACH CTA of the pair
