@@ -373,20 +373,32 @@ def run_ours(args):
     h_bt = torch.from_numpy(st.block_table.copy()).pin_memory()
     h_sl = torch.from_numpy(st.seq_lens.copy()).pin_memory()
     h_ra = torch.from_numpy(assign.copy()).pin_memory()
+    def host_step(fn):
+        fn(S.layer, h_hidden, step.k_pool, step.v_pool, step.n_pages, h_bt, h_sl, h_ra, batch, stream)
     for _ in range(W):
-        B.cc_forward_host(S.layer, h_hidden, step.k_pool, step.v_pool, step.n_pages, h_bt, h_sl, h_ra, batch, stream)
+        host_step(B.cc_forward_host)
     barrier()
     t0 = time.perf_counter()
     for _ in range(K):
-        B.cc_forward_host(S.layer, h_hidden, step.k_pool, step.v_pool, step.n_pages, h_bt, h_sl, h_ra, batch, stream)
+        host_step(B.cc_forward_host)                 # returns after the step's result is in the host buffer
     torch.cuda.synchronize()
-    e2e_s = time.perf_counter() - t0
-    e2e_s = M.max_over_ranks(e2e_s, f"cuda:{local}")
+    e2e_sync_s = M.max_over_ranks(time.perf_counter() - t0, f"cuda:{local}")
+    # the same K steps enqueue-only (cc_forward_host_async): the host marshals step i + 1 while step i runs; one
+    # synchronisation at the end, inside the timed region -- every step still moves its inputs and its result over PCIe
+    for _ in range(W):
+        host_step(B.cc_forward_host_async)
+    barrier()
+    t0 = time.perf_counter()
+    for _ in range(K):
+        host_step(B.cc_forward_host_async)
+    torch.cuda.synchronize()
+    e2e_s = M.max_over_ranks(time.perf_counter() - t0, f"cuda:{local}")
     h2d = h_hidden.numel() * 2 + h_bt.numel() * 4 + h_sl.numel() * 4 + h_ra.numel() * 4
     e2e = {"value": world * batch * K / e2e_s, "unit": UNIT, "h2d_bytes_per_step": int(h2d),
            "d2h_bytes_per_step": int(h_hidden.numel() * 2), "ms_per_step": e2e_s / K * 1e3,
-           "api": "cc_forward_host (pinned host hidden/block_table/seq_lens/replica_assign in, hidden out; "
-                  "KV pools and weights are device-resident state)",
+           "ms_per_step_synchronised_every_step": e2e_sync_s / K * 1e3,
+           "api": "cc_forward_host_async x K + one stream synchronisation (pinned host hidden/block_table/seq_lens/replica_assign in, "
+                  "hidden out; KV pools and weights are device-resident state); cc_forward_host synchronises every step",
            "transfers": "the three tables in one copy-engine transfer; the hidden rows are read over PCIe by the first kernel and the "
                         "result rows stored to the pinned buffer by the last epilogue (same bytes, no separate copies)"}
 

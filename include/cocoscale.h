@@ -231,6 +231,15 @@ cc_status cc_forward_host(cc_layer *layer, void *hidden_host, void *k_pool_dev, 
                           int32_t n_pages, const int32_t *block_table_host, const int32_t *seq_lens_host,
                           const int32_t *replica_assign_host, int batch, void *stream);
 
+/* The same, ENQUEUE-ONLY: returns once the copies and kernels are on `stream`; hidden_host holds the result after the
+ * caller has synchronised the stream (or an event recorded behind the call).  Lets consecutive steps overlap their host
+ * work (table marshalling, launches) with the device work of the step before.  Needs the pinned, mapped hidden_host of
+ * the in-place path (CC_ERR_INVALID otherwise) and batch <= 256; hidden_host must stay untouched until the step has run;
+ * block_table_host / seq_lens_host / replica_assign_host are consumed before the call returns. */
+cc_status cc_forward_host_async(cc_layer *layer, void *hidden_host, void *k_pool_dev, void *v_pool_dev,
+                          int32_t n_pages, const int32_t *block_table_host, const int32_t *seq_lens_host,
+                          const int32_t *replica_assign_host, int batch, void *stream);
+
 /* The same step, launched kernel by kernel with a CUDA event between consecutive kernels (so
  * without programmatic dependent launch), synchronised; stage_ms_host[i] (host, fp32
  * [CC_MAX_PROFILE_STAGES], unused entries 0) receives the device time of kernel i in milliseconds, in launch

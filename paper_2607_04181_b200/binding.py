@@ -31,7 +31,7 @@ EXPORTS = (
     "cc_ctx_create", "cc_ctx_destroy", "cc_ctx_donate", "cc_ctx_reclaim", "cc_ctx_set_copy_chunk",
     "cc_ctx_set_pdl", "cc_ctx_set_operand_format", "cc_ctx_set_operand_planes", "cc_layer_operand_format", "cc_poll_device_error", "cc_create_layer", "cc_destroy_layer", "cc_layer_blob_bytes",
     "cc_scale_layer", "cc_commit", "cc_release_replica", "cc_query", "cc_active_replicas", "cc_replica_blob", "cc_forward",
-    "cc_forward_host", "cc_forward_profiled", "cc_forward_launch_count", "cc_replica_copy", "cc_kv_plan_migration", "cc_kv_plan_catchup", "cc_kv_migrate", "cc_debug_tap", "cc_debug_grouping", "cc_debug_trace",
+    "cc_forward_host", "cc_forward_host_async", "cc_forward_profiled", "cc_forward_launch_count", "cc_replica_copy", "cc_kv_plan_migration", "cc_kv_plan_catchup", "cc_kv_migrate", "cc_debug_tap", "cc_debug_grouping", "cc_debug_trace",
     "cc_slotalloc_create", "cc_slotalloc_destroy", "cc_slotalloc_donate", "cc_slotalloc_reclaim",
     "cc_slotalloc_alloc", "cc_slotalloc_free", "cc_slotalloc_free_bytes", "cc_last_error", "cc_version",
     "cc_ctl_mem_bytes", "cc_ctl_flops", "cc_ctl_comm_seconds", "cc_ctl_speedup", "cc_ctl_speedup_vec", "cc_ctl_distance",
@@ -236,6 +236,13 @@ def cc_forward_host(layer, hidden_host, k_pool, v_pool, n_pages: int, block_tabl
     _check(_lib.cc_forward_host(layer, _ptr(hidden_host), _ptr(k_pool), _ptr(v_pool), C.c_int32(n_pages),
                                 _ptr(block_table_host), _ptr(seq_lens_host), _ptr(replica_assign_host),
                                 C.c_int(batch), _stream(stream)))
+
+
+def cc_forward_host_async(layer, hidden_host, k_pool, v_pool, n_pages: int, block_table_host, seq_lens_host,
+                          replica_assign_host, batch: int, stream=None) -> None:
+    _check(_lib.cc_forward_host_async(layer, _ptr(hidden_host), _ptr(k_pool), _ptr(v_pool), C.c_int32(n_pages),
+                                      _ptr(block_table_host), _ptr(seq_lens_host), _ptr(replica_assign_host),
+                                      C.c_int(batch), _stream(stream)))
 
 
 STAGE_NAMES = ("prologue", "gemm_qkv", "attention", "gemm_o", "gemm_gate_up", "gemm_down")

@@ -173,7 +173,11 @@ struct cc_layer {
     int* st_bt = nullptr;
     int* st_sl = nullptr;
     int* st_ra = nullptr;
-    void* st_tbl_host = nullptr;         // pinned mirror of [st_sl | st_ra | st_bt]
+    void* st_tbl_host = nullptr;         // pinned mirrors of [st_sl | st_ra | st_bt]: a ring of kTblRing, so that an enqueue-only
+                                         // host step can fill the next one while the previous copy is still in flight
+    size_t st_tbl_bytes = 0;
+    cudaEvent_t st_tbl_done[4] = {};     // recorded after the copy out of mirror i
+    unsigned st_tbl_next = 0;
     bool big = false;                    // created with max_batch > 256: steps of more than 256 rows take the large-M path
     int last_batch = 0;
     int last_pl[4] = {2, 2, 2, 2};       // plane counts of the last forward (cc_debug_tap reads the operands back)
@@ -383,16 +387,24 @@ void destroy_layer_memory(cc_layer* L) {
     cudaFree(L->blob0);
     cudaFree(L->work_base);
     if (L->st_tbl_host) cudaFreeHost(L->st_tbl_host);
+    for (auto& ev : L->st_tbl_done)
+        if (ev) cudaEventDestroy(ev);
 }
 
 // cc_forward_host: the three per-step tables through the layer's pinned mirror, one host-to-device copy.
+constexpr int kTblRing = 4;
 cudaError_t stage_tables(cc_layer* L, const int32_t* bt, const int32_t* sl, const int32_t* ra, int batch, cudaStream_t st) {
     const size_t mb = (size_t)L->desc.max_batch, bb = (size_t)batch * L->desc.max_blocks_per_seq * 4;
-    uint8_t* h = (uint8_t*)L->st_tbl_host;
+    const int slot = (int)(L->st_tbl_next++ % kTblRing);
+    cudaError_t e = cudaEventSynchronize(L->st_tbl_done[slot]);       // the copy that last read this mirror (no-op if none)
+    if (e != cudaSuccess) return e;
+    uint8_t* h = (uint8_t*)L->st_tbl_host + (size_t)slot * L->st_tbl_bytes;
     std::memcpy(h, sl, (size_t)batch * 4);
     std::memcpy(h + mb * 4, ra, (size_t)batch * 4);
     std::memcpy(h + mb * 8, bt, bb);
-    return cudaMemcpyAsync(L->st_sl, h, mb * 8 + bb, cudaMemcpyHostToDevice, st);
+    e = cudaMemcpyAsync(L->st_sl, h, mb * 8 + bb, cudaMemcpyHostToDevice, st);
+    if (e == cudaSuccess) e = cudaEventRecord(L->st_tbl_done[slot], st);
+    return e;
 }
 
 }  // namespace
@@ -504,7 +516,9 @@ cc_status cc_create_layer(cc_ctx* ctx, const cc_layer_desc* desc, const cc_layer
 
     cudaError_t e = cudaMalloc(&L->blob0, L->blob_bytes);
     if (e == cudaSuccess) e = cudaMalloc(&L->work_base, ws_bytes);
-    if (e == cudaSuccess) e = cudaHostAlloc(&L->st_tbl_host, tbl_bytes, cudaHostAllocDefault);
+    L->st_tbl_bytes = (tbl_bytes + 255) / 256 * 256;
+    if (e == cudaSuccess) e = cudaHostAlloc(&L->st_tbl_host, L->st_tbl_bytes * kTblRing, cudaHostAllocDefault);
+    for (int i = 0; i < kTblRing && e == cudaSuccess; ++i) e = cudaEventCreateWithFlags(&L->st_tbl_done[i], cudaEventDisableTiming);
     if (e == cudaSuccess) e = cudaMemset(L->work_base, 0, ws_bytes);
     if (e == cudaSuccess) e = cudaMemset(L->blob0, 0, L->blob_bytes);
     if (e != cudaSuccess) {
@@ -872,9 +886,9 @@ cc_status cc_forward(cc_layer* L, void* hidden_dev, const cc_kv_pages* kv, const
     return CC_OK;
 }
 
-cc_status cc_forward_host(cc_layer* L, void* hidden_host, void* k_pool_dev, void* v_pool_dev, int32_t n_pages,
-                          const int32_t* block_table_host, const int32_t* seq_lens_host,
-                          const int32_t* replica_assign_host, int batch, void* stream) {
+static cc_status forward_host_impl(cc_layer* L, void* hidden_host, void* k_pool_dev, void* v_pool_dev, int32_t n_pages,
+                                   const int32_t* block_table_host, const int32_t* seq_lens_host,
+                                   const int32_t* replica_assign_host, int batch, void* stream, bool sync) {
     if (!L || !hidden_host || !block_table_host || !seq_lens_host || !replica_assign_host)
         return fail(CC_ERR_INVALID, "null argument");
     if (batch < 1 || batch > L->desc.max_batch) return fail(CC_ERR_INVALID, "batch %d outside 1..max_batch=%d", batch, L->desc.max_batch);
@@ -891,9 +905,10 @@ cc_status cc_forward_host(cc_layer* L, void* hidden_host, void* k_pool_dev, void
         cudaError_t e = enqueue_forward(L, L->st_hidden, k, L->st_sl, L->st_ra, batch, st, nullptr, (__nv_bfloat16*)alias);
         if (e != cudaSuccess) return fail(CC_ERR_CUDA, "cc_forward_host launch: %s", cudaGetErrorString(e));
         L->last_batch = batch;
-        CC_CUDA(cudaStreamSynchronize(st));
+        if (sync) CC_CUDA(cudaStreamSynchronize(st));
         return CC_OK;
     }
+    if (!sync) return fail(CC_ERR_INVALID, "cc_forward_host_async needs a pinned (page-locked, mapped) hidden buffer and a step of at most 256 rows");
     CC_CUDA(cudaMemcpyAsync(L->st_hidden, hidden_host, hb, cudaMemcpyHostToDevice, st));
     CC_CUDA(stage_tables(L, block_table_host, seq_lens_host, replica_assign_host, batch, st));
     cc_kv_pages kv{k_pool_dev, v_pool_dev, L->st_bt, n_pages};
@@ -902,6 +917,20 @@ cc_status cc_forward_host(cc_layer* L, void* hidden_host, void* k_pool_dev, void
     CC_CUDA(cudaMemcpyAsync(hidden_host, L->st_hidden, hb, cudaMemcpyDeviceToHost, st));
     CC_CUDA(cudaStreamSynchronize(st));
     return CC_OK;
+}
+
+cc_status cc_forward_host(cc_layer* L, void* hidden_host, void* k_pool_dev, void* v_pool_dev, int32_t n_pages,
+                          const int32_t* block_table_host, const int32_t* seq_lens_host,
+                          const int32_t* replica_assign_host, int batch, void* stream) {
+    return forward_host_impl(L, hidden_host, k_pool_dev, v_pool_dev, n_pages, block_table_host, seq_lens_host, replica_assign_host,
+                             batch, stream, true);
+}
+
+cc_status cc_forward_host_async(cc_layer* L, void* hidden_host, void* k_pool_dev, void* v_pool_dev, int32_t n_pages,
+                                const int32_t* block_table_host, const int32_t* seq_lens_host,
+                                const int32_t* replica_assign_host, int batch, void* stream) {
+    return forward_host_impl(L, hidden_host, k_pool_dev, v_pool_dev, n_pages, block_table_host, seq_lens_host, replica_assign_host,
+                             batch, stream, false);
 }
 
 cc_status cc_forward_profiled(cc_layer* L, void* hidden_dev, const cc_kv_pages* kv, const int32_t* seq_lens_dev,

@@ -115,8 +115,10 @@ k_big_gemm(CcGemmGeo G, const uint8_t* __restrict__ act, CcEpi E, CcDims D, CcWo
     if (warp == 0) {
         // ===================== producer (both CTAs) =====================
         // with the row block fastest, the pairs running together cover a few super tiles x every row block: the
-        // activations are re-read by every wave (keep them in L2), a weight super tile by one wave only (let it go)
-        const uint64_t pol_w = D.max_position & 0 ? policy_evict_first() : 0ull, pol_a = policy_evict_last();
+        // activations are re-read by every wave (evict_last keeps them in L2); a weight super tile is read by the ~9
+        // pairs of its row blocks at about the same time -- with evict_first it was gone before the last of them
+        // came (measured: 2.7 GB of DRAM reads for 0.76 GB of operands), so weights take the default policy
+        const uint64_t pol_a = policy_evict_last();
         int stage = 0;
         uint32_t ph = 0;
         TileIter it;
@@ -128,7 +130,7 @@ k_big_gemm(CcGemmGeo G, const uint8_t* __restrict__ act, CcEpi E, CcDims D, CcWo
                 if (elect_one()) {
                     uint8_t* s = stage0 + (size_t)stage * stage_bytes;
                     mbar_expect_tx(&H->full[stage], stage_bytes);
-                    if (pol_w) bulk_g2s_hint(s, wsrc, CC_A_TILE_BYTES, &H->full[stage], pol_w); else bulk_g2s(s, wsrc, CC_A_TILE_BYTES, &H->full[stage]);
+                    bulk_g2s(s, wsrc, CC_A_TILE_BYTES, &H->full[stage]);
                     bulk_g2s_hint(s + CC_A_TILE_BYTES, asrc, b_bytes, &H->full[stage], pol_a);
                 }
                 wsrc += (size_t)CC_G * CC_A_TILE_BYTES;

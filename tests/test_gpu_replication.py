@@ -395,6 +395,48 @@ def test_forward_host_direct_and_staged_paths_match_forward(pinned):
             assert np.array_equal(hidden.numpy().view(np.uint16), want)
 
 
+def test_forward_host_async_pipelines_steps_with_different_tables():
+    """cc_forward_host_async is enqueue-only: eight steps with DIFFERENT tables (row order and replica assignment
+    change from step to step) are enqueued back to back, each from its own pinned hidden buffer, one synchronisation at
+    the end.  The pinned table mirror is a ring: every step must have run with the tables it was called with -- each
+    result equals cc_forward of that step bit for bit.  Pageable hidden buffers are refused."""
+    B, DeviceStep, Session = _binding()
+    shape, batch, R = MID, 21, 3
+    w = I.make_weights(shape, 1011)
+    rng = np.random.default_rng(77)
+    steps = []
+    for i in range(8):
+        st = I.make_step_inputs(shape, 2011, 3011, batch=batch)          # the same cache every step (the steps append the same slots)
+        perm = rng.permutation(batch)
+        st = I.StepInputs(st.hidden[perm].copy(), st.k_pool, st.v_pool, st.block_table[perm].copy(), st.seq_lens[perm].copy(), st.n_pages)
+        steps.append((st, rng.integers(0, R, batch).astype(np.int32)))
+    with Session(shape, w, max_batch=batch) as S:
+        S.scale(R)
+        want = []
+        for st, assign in steps:
+            step = DeviceStep(st, assign)
+            S.forward(step)
+            torch.cuda.synchronize()
+            want.append(step.out_bits())
+        dev = DeviceStep(steps[0][0], steps[0][1])
+        stream = torch.cuda.current_stream()
+        bufs = []
+        for st, assign in steps:
+            h = torch.from_numpy(st.hidden.view(np.int16).copy()).pin_memory()
+            bt, sl, ra = st.block_table.copy(), st.seq_lens.copy(), assign.copy()
+            B.cc_forward_host_async(S.layer, h, dev.k_pool, dev.v_pool, dev.n_pages, bt, sl, ra, batch, stream)
+            bt[:] = -7; sl[:] = 0; ra[:] = 9                             # the tables were consumed before the call returned
+            bufs.append(h)
+        torch.cuda.synchronize()
+        assert B.cc_poll_device_error(S.ctx) == 0
+        for i, h in enumerate(bufs):
+            assert np.array_equal(h.numpy().view(np.uint16), want[i]), f"step {i}"
+        pageable = torch.from_numpy(steps[0][0].hidden.view(np.int16).copy())
+        with pytest.raises(B.CcError):
+            B.cc_forward_host_async(S.layer, pageable, dev.k_pool, dev.v_pool, dev.n_pages, steps[0][0].block_table, steps[0][0].seq_lens,
+                                    steps[0][1], batch, stream)
+
+
 def test_run_to_run_determinism_and_pdl_off_is_bitwise_the_same():
     """The fixups and merges are finished by whichever CTA arrives last: the result must not depend on that.
     Twenty replays from the same inputs, with and without programmatic dependent launch, give one bit pattern
