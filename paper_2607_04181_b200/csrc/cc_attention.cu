@@ -353,10 +353,10 @@ k_attn(const int* __restrict__ seq_lens, CcKv kv, CcDims D, CcWork W, const CcLa
         if (PPS > 1) named_bar_sync(kBarMerge, kCW * 32); else __syncwarp();   // merge rows may be rewritten
         if (pp != 0 || nch == 1) continue;
         // ---- the warp that finishes the pair's last piece merges all of them, in piece order
-        __threadfence();
         __syncwarp();
         int last = 0;
         if (lane == 0) {
+            __threadfence();                                    // cumulative over the warp's partial stores (ordered by the __syncwarp)
             int* cnt = W.attn_cnt + m.pos * Hkv + h;
             last = atomicAdd(cnt, 1) == nch - 1;
             if (last) *cnt = 0;                                 // ready for the next step

@@ -368,7 +368,9 @@ k_gemm(CcGemmGeo G, const uint8_t* __restrict__ act, float* __restrict__ part, i
             }
         }
     }
-    __threadfence();                      // partial sums of this CTA are visible GPU-wide before the signal
+    // (the partial sums of this CTA become visible GPU-wide through thread 0's fence below: the block barrier
+    // orders every warp's stores before it, and the fence is cumulative -- a fence in every thread cost each
+    // warp a MEMBAR.ALL.GPU on the kernel's tail)
     tc_fence_before();
     __syncthreads();
     if (warp == 1) tmem_dealloc<kTmemCols>(tmem_base);
