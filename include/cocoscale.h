@@ -187,6 +187,17 @@ cc_status cc_release_replica(cc_layer *layer, int replica);
  * cc_scale_layer and not yet committed. Either pointer may be NULL. */
 cc_status cc_query(cc_layer *layer, int *n_active, int *n_pending);
 
+/* A replica's own KV partition ("a replica holds a copy of the weights AND the KV of its requests",
+ * PAPER.md:103 "each replica maintains its own partition"): from now on the rows that replica_assign gives to
+ * `replica` append and read their K/V in THESE pools ([n_pages][n_kv_heads][16][head_dim] bf16, device memory the
+ * caller owns, 16-byte aligned), and the page ids in their block-table rows are relative to them; replicas without a
+ * partition keep using the pools passed to cc_forward.  k_pool_dev = v_pool_dev = NULL removes the partition.  The
+ * base pointers go into the layer's row of the device replica table (enqueued on `stream`; the QKV epilogue reads them
+ * there); the attention kernels take one TMA descriptor per replica as launch parameters, so a CAPTURED graph keeps
+ * the pools it was captured with: set partitions before capturing.  All rows of one request must name one replica. */
+cc_status cc_layer_set_kv_partition(cc_layer *layer, int replica, void *k_pool_dev, void *v_pool_dev, int32_t n_pages,
+                                    void *stream);
+
 /* Which replica indices forwards enqueued now may name: bit r of *mask set <=> replica r is live and
  * published.  After cc_release_replica(layer, 1) with three live replicas the set is {0, 2}: indices are
  * not compacted (a captured graph and the caller's replica_assign keep their meaning), so a caller that

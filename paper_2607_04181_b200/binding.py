@@ -30,7 +30,7 @@ CC_OPERAND_AUTO, CC_OPERAND_F16, CC_OPERAND_BF16X2 = range(3)
 EXPORTS = (
     "cc_ctx_create", "cc_ctx_destroy", "cc_ctx_donate", "cc_ctx_reclaim", "cc_ctx_set_copy_chunk",
     "cc_ctx_set_pdl", "cc_ctx_set_operand_format", "cc_ctx_set_operand_planes", "cc_layer_operand_format", "cc_poll_device_error", "cc_create_layer", "cc_destroy_layer", "cc_layer_blob_bytes",
-    "cc_scale_layer", "cc_commit", "cc_release_replica", "cc_query", "cc_active_replicas", "cc_replica_blob", "cc_forward",
+    "cc_scale_layer", "cc_commit", "cc_release_replica", "cc_query", "cc_layer_set_kv_partition", "cc_active_replicas", "cc_replica_blob", "cc_forward",
     "cc_forward_host", "cc_forward_host_async", "cc_forward_profiled", "cc_forward_launch_count", "cc_replica_copy", "cc_kv_plan_migration", "cc_kv_plan_catchup", "cc_kv_migrate", "cc_debug_tap", "cc_debug_grouping", "cc_debug_trace",
     "cc_slotalloc_create", "cc_slotalloc_destroy", "cc_slotalloc_donate", "cc_slotalloc_reclaim",
     "cc_slotalloc_alloc", "cc_slotalloc_free", "cc_slotalloc_free_bytes", "cc_last_error", "cc_version",
@@ -194,6 +194,10 @@ def cc_layer_blob_bytes(layer) -> int:
 
 def cc_scale_layer(layer, n_replicas: int) -> None:
     _check(_lib.cc_scale_layer(layer, C.c_int(n_replicas)))
+
+
+def cc_layer_set_kv_partition(layer, replica: int, k_pool, v_pool, n_pages: int, stream=None) -> None:
+    _check(_lib.cc_layer_set_kv_partition(layer, C.c_int(replica), _ptr(k_pool), _ptr(v_pool), C.c_int32(n_pages), _stream(stream)))
 
 
 def cc_commit(layer, stream=None) -> None:

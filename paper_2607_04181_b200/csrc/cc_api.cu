@@ -178,6 +178,7 @@ struct cc_layer {
     size_t st_tbl_bytes = 0;
     cudaEvent_t st_tbl_done[4] = {};     // recorded after the copy out of mirror i
     unsigned st_tbl_next = 0;
+    struct { void* k; void* v; int n; } kvp[CC_MAX_REPLICAS] = {};   // a replica's own KV partition (cc_layer_set_kv_partition)
     bool big = false;                    // created with max_batch > 256: steps of more than 256 rows take the large-M path
     int last_batch = 0;
     int last_pl[4] = {2, 2, 2, 2};       // plane counts of the last forward (cc_debug_tap reads the operands back)
@@ -740,6 +741,9 @@ cc_status cc_commit(cc_layer* L, void* stream) {
             row.rep[r].blob = L->rep[r].blob;
             row.active_mask |= 1u << r;
         }
+        row.rep[r].k_pool = L->kvp[r].k;
+        row.rep[r].v_pool = L->kvp[r].v;
+        row.rep[r].n_pages = L->kvp[r].n;
     }
     L->host_row = row;
     CC_CUDA(cc_launch_publish(ctx->table_dev + L->row, row, st));
@@ -749,6 +753,24 @@ cc_status cc_commit(cc_layer* L, void* stream) {
         CC_CUDA(cudaEventRecord(z.after_flip, st));           // everything enqueued before the flip has run
         ctx->zombies.push_back(z);
     }
+    return CC_OK;
+}
+
+cc_status cc_layer_set_kv_partition(cc_layer* L, int replica, void* k_pool_dev, void* v_pool_dev, int32_t n_pages, void* stream) {
+    if (!L) return fail(CC_ERR_INVALID, "null layer");
+    if (replica < 0 || replica >= CC_MAX_REPLICAS) return fail(CC_ERR_INVALID, "replica index out of range");
+    if ((k_pool_dev == nullptr) != (v_pool_dev == nullptr)) return fail(CC_ERR_INVALID, "give both pools or neither");
+    if (k_pool_dev && (n_pages < 1 || (((uintptr_t)k_pool_dev | (uintptr_t)v_pool_dev) & 15)))
+        return fail(CC_ERR_INVALID, "a partition needs n_pages >= 1 and 16-byte aligned pools");
+    cc_ctx* ctx = L->ctx;
+    CC_CUDA(cudaSetDevice(ctx->device));
+    L->kvp[replica].k = k_pool_dev;
+    L->kvp[replica].v = v_pool_dev;
+    L->kvp[replica].n = k_pool_dev ? n_pages : 0;
+    L->host_row.rep[replica].k_pool = L->kvp[replica].k;
+    L->host_row.rep[replica].v_pool = L->kvp[replica].v;
+    L->host_row.rep[replica].n_pages = L->kvp[replica].n;
+    CC_CUDA(cc_launch_publish(ctx->table_dev + L->row, L->host_row, (cudaStream_t)stream));
     return CC_OK;
 }
 
@@ -790,6 +812,22 @@ void* mapped_host(const void* p) {
     cudaPointerAttributes a;
     if (cudaPointerGetAttributes(&a, p) != cudaSuccess) { cudaGetLastError(); return nullptr; }
     return a.type == cudaMemoryTypeHost && !((uintptr_t)a.devicePointer & 15) ? a.devicePointer : nullptr;
+}
+
+// The KV pools of one forward: the call's pools, and per replica its own partition where it has one.
+CcKv make_kv(const cc_layer* L, void* k_pool, void* v_pool, const int* block_table, int n_pages) {
+    CcKv k{};
+    k.k_pool = (__nv_bfloat16*)k_pool;
+    k.v_pool = (__nv_bfloat16*)v_pool;
+    k.block_table = block_table;
+    k.n_pages = n_pages;
+    for (int r = 0; r < CC_MAX_REPLICAS; ++r) {
+        const bool own = L->kvp[r].k != nullptr;
+        k.k_pool_r[r] = own ? L->kvp[r].k : k_pool;
+        k.v_pool_r[r] = own ? L->kvp[r].v : v_pool;
+        k.n_pages_r[r] = own ? L->kvp[r].n : n_pages;
+    }
+    return k;
 }
 
 // Geometry of one step: the layer's, with the activation plane counts of a step of `batch` rows.
@@ -878,7 +916,7 @@ cc_status cc_forward(cc_layer* L, void* hidden_dev, const cc_kv_pages* kv, const
     if (!kv->k_pool || !kv->v_pool || !kv->block_table || kv->n_pages < 1) return fail(CC_ERR_INVALID, "bad cc_kv_pages");
     if (((uintptr_t)hidden_dev | (uintptr_t)kv->k_pool | (uintptr_t)kv->v_pool) & 15)
         return fail(CC_ERR_INVALID, "hidden and KV pools must be 16-byte aligned");
-    CcKv k{(__nv_bfloat16*)kv->k_pool, (__nv_bfloat16*)kv->v_pool, kv->block_table, kv->n_pages};
+    const CcKv k = make_kv(L, kv->k_pool, kv->v_pool, kv->block_table, kv->n_pages);
     cudaError_t e = enqueue_forward(L, (__nv_bfloat16*)hidden_dev, k, seq_lens_dev, replica_assign_dev, batch,
                                     (cudaStream_t)stream);
     if (e != cudaSuccess) return fail(CC_ERR_CUDA, "cc_forward launch: %s", cudaGetErrorString(e));
@@ -901,7 +939,7 @@ static cc_status forward_host_impl(cc_layer* L, void* hidden_host, void* k_pool_
         if (!k_pool_dev || !v_pool_dev || n_pages < 1) return fail(CC_ERR_INVALID, "bad KV pool arguments");
         if (((uintptr_t)k_pool_dev | (uintptr_t)v_pool_dev) & 15) return fail(CC_ERR_INVALID, "KV pools must be 16-byte aligned");
         CC_CUDA(stage_tables(L, block_table_host, seq_lens_host, replica_assign_host, batch, st));
-        CcKv k{(__nv_bfloat16*)k_pool_dev, (__nv_bfloat16*)v_pool_dev, L->st_bt, n_pages};
+        const CcKv k = make_kv(L, k_pool_dev, v_pool_dev, L->st_bt, n_pages);
         cudaError_t e = enqueue_forward(L, L->st_hidden, k, L->st_sl, L->st_ra, batch, st, nullptr, (__nv_bfloat16*)alias);
         if (e != cudaSuccess) return fail(CC_ERR_CUDA, "cc_forward_host launch: %s", cudaGetErrorString(e));
         L->last_batch = batch;
@@ -943,7 +981,7 @@ cc_status cc_forward_profiled(cc_layer* L, void* hidden_dev, const cc_kv_pages* 
     for (auto& x : ev) CC_CUDA(cudaEventCreate(&x));
     const int n_stages = batch > 256 ? 9 : kForwardLaunches;
     for (int i = 0; i < CC_MAX_PROFILE_STAGES; ++i) stage_ms_host[i] = 0.f;
-    CcKv k{(__nv_bfloat16*)kv->k_pool, (__nv_bfloat16*)kv->v_pool, kv->block_table, kv->n_pages};
+    const CcKv k = make_kv(L, kv->k_pool, kv->v_pool, kv->block_table, kv->n_pages);
     // a pinned host `hidden`: the stages of cc_forward_host's in-place path (the rows are staged for the residual)
     void* alias = batch <= 256 ? mapped_host(hidden_dev) : nullptr;
     cudaError_t e = enqueue_forward(L, alias ? L->st_hidden : (__nv_bfloat16*)hidden_dev, k, seq_lens_dev, replica_assign_dev,

@@ -26,8 +26,7 @@
 //     pair's last piece (a counter per pair), so no separate combine kernel runs.  Every merge
 //     order is fixed => bit-identical across replicas, whatever CTA finishes last.
 //   * KV loads carry an L2 evict-first policy (measured: +12 % stream rate; the data is used once).
-#include "cc_kernels.h"
-#include <cuda.h>
+#include "cc_kvmaps.h"
 
 namespace {
 
@@ -61,7 +60,7 @@ struct AttnCfg {
 template <int DH>
 __global__ void __launch_bounds__(kAttnThreads, 1)
 k_attn(const int* __restrict__ seq_lens, CcKv kv, CcDims D, CcWork W, const CcLayerTable* __restrict__ tab,
-       const int* __restrict__ rowmap, const __grid_constant__ CUtensorMap tmK, const __grid_constant__ CUtensorMap tmV) {
+       const int* __restrict__ rowmap, const __grid_constant__ CcKvMaps maps) {
     using C = AttnCfg<DH>;
     extern __shared__ __align__(1024) uint8_t smem_raw[];
     const int warp = uniform((int)(threadIdx.x >> 5)), lane = threadIdx.x & 31;
@@ -126,6 +125,10 @@ k_attn(const int* __restrict__ seq_lens, CcKv kv, CcDims D, CcWork W, const CcLa
             // large steps: the work axis runs over the decode rows only, b indexes that list (k_big_group)
             const int rb = rowmap ? rowmap[b] : b;
             const int pos = W.pos_of[rb], s = seq_lens[rb], first_wr = W.first_wr[rb];
+            const int rep = replica_of_pos(W.sched->cnt, W.sched->goff, pos);   // whose KV partition the row's pages are in
+            const CUtensorMap* tmK = &maps.k[rep];
+            const CUtensorMap* tmV = &maps.v[rep];
+            const int n_pool_pages = kv.n_pages_r[rep];
             const int slot0 = b + cta_of_page(r0), n_pieces = cta_of_page(r1 - 1) - cta_of_page(r0) + 1;
             const int slot = b + (int)blockIdx.x;
             const int n_groups = (q1 - q0 + PPS - 1) / PPS;
@@ -138,7 +141,7 @@ k_attn(const int* __restrict__ seq_lens, CcKv kv, CcDims D, CcWork W, const CcLa
                     id = 0;
                     if (q < q1) {
                         id = kv.block_table[(size_t)rb * D.max_blocks + q];
-                        if (id < 0 || id >= kv.n_pages) {
+                        if (id < 0 || id >= n_pool_pages) {
                             atomicOr(W.err, CC_DEVERR_BAD_PAGE);
                             id = 0;
                         }
@@ -168,8 +171,8 @@ k_attn(const int* __restrict__ seq_lens, CcKv kv, CcDims D, CcWork W, const CcLa
                             const uint32_t dst = dst0 + (uint32_t)pp * page_bytes;
 #pragma unroll
                             for (int h = 0; h < DH / 64; ++h) {
-                                tma_load_2d_hint(dst + h * half_bytes, &tmK, h * 64, row0, bar, pol);
-                                tma_load_2d_hint(dst + kv_bytes + h * half_bytes, &tmV, h * 64, row0, bar, pol);
+                                tma_load_2d_hint(dst + h * half_bytes, tmK, h * 64, row0, bar, pol);
+                                tma_load_2d_hint(dst + kv_bytes + h * half_bytes, tmV, h * 64, row0, bar, pol);
                             }
                         }
                     }
@@ -445,12 +448,29 @@ cudaError_t cc_make_kv_tensor_map(CUtensorMap* out, const void* pool, int n_page
 
 cudaError_t cc_launch_attention(const int* seq_lens, const CcKv& kv, const CcDims& D, const CcLayerTable* tab,
                                 const CcWork& W, const CcLaunch& L, const int* rowmap) {
-    CUtensorMap tmK, tmV;
-    cudaError_t e = cc_make_kv_tensor_map(&tmK, kv.k_pool, kv.n_pages, D.Hkv, D.Dh, D.Hkv * CC_PAGE);
-    if (e == cudaSuccess) e = cc_make_kv_tensor_map(&tmV, kv.v_pool, kv.n_pages, D.Hkv, D.Dh, D.Hkv * CC_PAGE);
+    CcKvMaps maps;
+    cudaError_t e = cc_make_kv_maps(&maps, kv, D.Hkv, D.Dh, D.Hkv * CC_PAGE);
     if (e != cudaSuccess) return e;
     const dim3 grid(L.n_sms), block(kAttnThreads);
     if (D.Dh == 128)
-        return cc_launch_kernel(k_attn<128>, grid, block, AttnCfg<128>::smem_bytes(D.G), L, seq_lens, kv, D, W, tab, rowmap, tmK, tmV);
-    return cc_launch_kernel(k_attn<64>, grid, block, AttnCfg<64>::smem_bytes(D.G), L, seq_lens, kv, D, W, tab, rowmap, tmK, tmV);
+        return cc_launch_kernel(k_attn<128>, grid, block, AttnCfg<128>::smem_bytes(D.G), L, seq_lens, kv, D, W, tab, rowmap, maps);
+    return cc_launch_kernel(k_attn<64>, grid, block, AttnCfg<64>::smem_bytes(D.G), L, seq_lens, kv, D, W, tab, rowmap, maps);
+}
+
+// One descriptor pair per replica; replicas that share a pool share the encoding.
+cudaError_t cc_make_kv_maps(CcKvMaps* out, const CcKv& kv, int Hkv, int Dh, int box_rows) {
+    for (int r = 0; r < CC_MAXR; ++r) {
+        int same = -1;
+        for (int q = 0; q < r; ++q)
+            if (kv.k_pool_r[q] == kv.k_pool_r[r] && kv.v_pool_r[q] == kv.v_pool_r[r] && kv.n_pages_r[q] == kv.n_pages_r[r]) same = q;
+        if (same >= 0) {
+            out->k[r] = out->k[same];
+            out->v[r] = out->v[same];
+            continue;
+        }
+        cudaError_t e = cc_make_kv_tensor_map(&out->k[r], kv.k_pool_r[r], kv.n_pages_r[r], Hkv, Dh, box_rows);
+        if (e == cudaSuccess) e = cc_make_kv_tensor_map(&out->v[r], kv.v_pool_r[r], kv.n_pages_r[r], Hkv, Dh, box_rows);
+        if (e != cudaSuccess) return e;
+    }
+    return cudaSuccess;
 }

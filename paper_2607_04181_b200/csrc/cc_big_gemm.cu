@@ -36,6 +36,9 @@ struct BigHdr {
     uint32_t tmem_base;
     int cnt[CC_MAXR], goff[CC_MAXR];
     const uint8_t* blob[CC_MAXR];
+    __nv_bfloat16* kpool[CC_MAXR];            // the KV pools replica r's rows append to (its partition, else the call's pools)
+    __nv_bfloat16* vpool[CC_MAXR];
+    int kvpages[CC_MAXR];
 };
 static_assert(sizeof(BigHdr) <= kBigHdrBytes, "header does not fit");
 
@@ -47,6 +50,9 @@ struct GlobalTab {
     __device__ __forceinline__ int aux(int p) const { return aux_[p]; }
     __device__ __forceinline__ int page(int p) const { return page_[p]; }
     __device__ __forceinline__ const uint8_t* blob(int p) const { return H->blob[replica_of_pos(H->cnt, H->goff, p)]; }
+    __device__ __forceinline__ __nv_bfloat16* k_pool(int p) const { return H->kpool[replica_of_pos(H->cnt, H->goff, p)]; }
+    __device__ __forceinline__ __nv_bfloat16* v_pool(int p) const { return H->vpool[replica_of_pos(H->cnt, H->goff, p)]; }
+    __device__ __forceinline__ int kv_pages(int p) const { return H->kvpages[replica_of_pos(H->cnt, H->goff, p)]; }
 };
 
 struct TileIter {                             // walks this pair's tiles: (replica group r, super tile st, row block rb)
@@ -102,7 +108,11 @@ k_big_gemm(CcGemmGeo G, const uint8_t* __restrict__ act, CcEpi E, CcDims D, CcWo
     if (threadIdx.x < CC_MAXR) {
         H->cnt[threadIdx.x] = W.sched->cnt[threadIdx.x];
         H->goff[threadIdx.x] = W.sched->goff[threadIdx.x];
-        H->blob[threadIdx.x] = tab->rep[threadIdx.x].blob;
+        const CcReplicaRow rr = tab->rep[threadIdx.x];
+        H->blob[threadIdx.x] = rr.blob;
+        H->kpool[threadIdx.x] = rr.k_pool ? (__nv_bfloat16*)rr.k_pool : E.kv.k_pool;
+        H->vpool[threadIdx.x] = rr.k_pool ? (__nv_bfloat16*)rr.v_pool : E.kv.v_pool;
+        H->kvpages[threadIdx.x] = rr.k_pool ? rr.n_pages : E.kv.n_pages;
     }
     if (warp == 1) tmem_alloc_pair<512>(&H->tmem_base);
     tc_fence_before();

@@ -35,6 +35,10 @@
 // weight-blob base of replica r from here at run time, so a captured graph survives flips.
 struct CcReplicaRow {
     const uint8_t* blob;   // packed weight blob of replica r (slot base), or nullptr
+    void* k_pool;          // replica r's own KV partition, or nullptr = the pools passed to cc_forward;
+    void* v_pool;          //   page ids in the block-table rows of r's requests are relative to it
+    int n_pages;
+    int pad_;
 };
 struct CcLayerTable {
     CcReplicaRow rep[CC_MAXR];

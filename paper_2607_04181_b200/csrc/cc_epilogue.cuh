@@ -2,7 +2,8 @@
 // decode GEMM (cc_gemm.cu: stream-K fixup) and the large-M GEMM (cc_big_gemm.cu: straight from TMEM).
 // One warp owns one item = (tile t of 128 output features, grouped row p); lane l holds the four summed output
 // features t*128 + 4l .. 4l+3 of original row b.  Each epilogue is split into `pre` (every global load that does
-// not depend on the sum) and `fin` (math + stores).  TAB supplies the per-row tables: aux(p), page(p), blob(p).
+// not depend on the sum) and `fin` (math + stores).  TAB supplies the per-row tables: aux(p), page(p), and
+// what the row's replica owns: blob(p), k_pool(p), v_pool(p), kv_pages(p).
 #pragma once
 #include "cc_kernels.h"
 
@@ -64,13 +65,13 @@ __device__ __forceinline__ void epi_fin(const EpiPre& P, const CcEpi& E, const C
             }
         }
         const int page = H.page(p);
-        if (page < 0 || page >= E.kv.n_pages) {
+        if (page < 0 || page >= H.kv_pages(p)) {
             if (lane == 0) atomicOr(W.err, CC_DEVERR_BAD_PAGE);
             return;
         }
         const bool is_k = col < D.QD + D.KD;
         const int hk = (col - D.QD - (is_k ? 0 : D.KD)) / D.Dh;
-        __nv_bfloat16* dst = (is_k ? E.kv.k_pool : E.kv.v_pool) + (((size_t)page * D.Hkv + hk) * CC_PAGE + pos % CC_PAGE) * D.Dh + i0;
+        __nv_bfloat16* dst = (is_k ? H.k_pool(p) : H.v_pool(p)) + (((size_t)page * D.Hkv + hk) * CC_PAGE + pos % CC_PAGE) * D.Dh + i0;
         *reinterpret_cast<uint2*>(dst) = make_uint2(pack_bf16(a.x, a.y), pack_bf16(a.z, a.w));
     } else if (KIND == EPI_O) {
         // a6 + first half of a7: h1 = h + O-projection (kept in fp32); sum of squares of this tile's 128

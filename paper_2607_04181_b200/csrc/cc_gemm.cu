@@ -44,6 +44,9 @@ struct GemmSmemHdr {                      // lives at the start of dynamic smem
     int cnt[CC_MAXR];
     int goff[CC_MAXR];
     const uint8_t* blob[CC_MAXR];
+    __nv_bfloat16* kpool[CC_MAXR];        // the KV pools replica r's rows append to (its partition, else the call's pools)
+    __nv_bfloat16* vpool[CC_MAXR];
+    int kvpages[CC_MAXR];
     int perm[CC_MAX_MPAD];                // original row at grouped position, or -1
     int aux[CC_MAX_MPAD];                 // QKV: position s-1; O: bits of 1/rms of the input row; gate/up: bits of rms_in/rms of h1
     int page[CC_MAX_MPAD];                // QKV: page that holds position s-1, or -1
@@ -56,6 +59,9 @@ struct SmemTab {
     __device__ __forceinline__ int aux(int p) const { return H->aux[p]; }
     __device__ __forceinline__ int page(int p) const { return H->page[p]; }
     __device__ __forceinline__ const uint8_t* blob(int p) const { return H->blob[replica_of_pos(H->cnt, H->goff, p)]; }
+    __device__ __forceinline__ __nv_bfloat16* k_pool(int p) const { return H->kpool[replica_of_pos(H->cnt, H->goff, p)]; }
+    __device__ __forceinline__ __nv_bfloat16* v_pool(int p) const { return H->vpool[replica_of_pos(H->cnt, H->goff, p)]; }
+    __device__ __forceinline__ int kv_pages(int p) const { return H->kvpages[replica_of_pos(H->cnt, H->goff, p)]; }
 };
 
 // Slice of the fixup of super tile `st` done by contributor k of m: rows k, k + m, ... of both tiles.
@@ -165,7 +171,13 @@ k_gemm(CcGemmGeo G, const uint8_t* __restrict__ act, float* __restrict__ part, i
                 off += (c + CC_ROW_ALIGN - 1) / CC_ROW_ALIGN * CC_ROW_ALIGN;
             }
         }
-        if (threadIdx.x < CC_MAXR) H->blob[threadIdx.x] = tab->rep[threadIdx.x].blob;
+        if (threadIdx.x < CC_MAXR) {
+            const CcReplicaRow rr = tab->rep[threadIdx.x];
+            H->blob[threadIdx.x] = rr.blob;
+            H->kpool[threadIdx.x] = rr.k_pool ? (__nv_bfloat16*)rr.k_pool : E.kv.k_pool;
+            H->vpool[threadIdx.x] = rr.k_pool ? (__nv_bfloat16*)rr.v_pool : E.kv.v_pool;
+            H->kvpages[threadIdx.x] = rr.k_pool ? rr.n_pages : E.kv.n_pages;
+        }
     } else if (threadIdx.x < CC_MAXR) {
         H->cnt[threadIdx.x] = sched->cnt[threadIdx.x];
         H->goff[threadIdx.x] = sched->goff[threadIdx.x];

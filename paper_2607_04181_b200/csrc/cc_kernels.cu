@@ -72,7 +72,7 @@ __global__ void __launch_bounds__(256) k_page_copy(uint8_t* __restrict__ k_pool,
 
 // a12: the flip.  One thread rewrites the layer's table row; ordering comes from the stream.
 __global__ void k_publish(CcLayerTable* row, CcLayerTable value) {
-    for (int r = 0; r < CC_MAXR; ++r) row->rep[r].blob = value.rep[r].blob;
+    for (int r = 0; r < CC_MAXR; ++r) row->rep[r] = value.rep[r];
     __threadfence();
     row->active_mask = value.active_mask;
 }

@@ -75,11 +75,17 @@ __device__ __forceinline__ void cc_trace_minmax(unsigned long long* tr, int k, i
 // first ([0]) and second ([1]) stream-K fixup pass of a CTA, 12 + KIND: [0][max] passes counted / [2][max] their sum
 
 struct CcKv {
-    __nv_bfloat16* k_pool;
+    __nv_bfloat16* k_pool;        // the pools passed to cc_forward: every replica without a partition of its own
     __nv_bfloat16* v_pool;
     const int* block_table;
     int n_pages;
+    // resolved on the host per forward: the pools replica r's rows live in (its partition, else the pools above); the
+    // attention launchers build one TMA descriptor pair per replica from them, the kernels bound page ids by n_pages_r
+    const void* k_pool_r[CC_MAXR];
+    const void* v_pool_r[CC_MAXR];
+    int n_pages_r[CC_MAXR];
 };
+
 
 // Launch options shared by the forward chain.
 struct CcLaunch {

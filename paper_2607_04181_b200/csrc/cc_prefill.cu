@@ -18,10 +18,7 @@
 //     bf16 by definition, and a single bf16 plane of q or p costs 2e-3 on the attention output;
 //   * items are dealt round-robin in decreasing cost; every row is finished by one item in one fixed order, so the
 //     result does not depend on the replica split or on timing.
-#include "cc_kernels.h"
-#include <cuda.h>
-
-cudaError_t cc_make_kv_tensor_map(CUtensorMap* out, const void* pool, int n_pages, int Hkv, int Dh, int box_rows);
+#include "cc_kvmaps.h"
 
 namespace {
 
@@ -93,8 +90,7 @@ __device__ __forceinline__ bool item_at(const CcWork& W, const CcDims& D, const 
 }
 
 __global__ void __launch_bounds__(kPfThreads, 1)
-k_prefill_attn(const int* __restrict__ seq_lens, CcKv kv, CcDims D, CcWork W, const __grid_constant__ CUtensorMap tmK,
-               const __grid_constant__ CUtensorMap tmV) {
+k_prefill_attn(const int* __restrict__ seq_lens, CcKv kv, CcDims D, CcWork W, const __grid_constant__ CcKvMaps maps) {
     extern __shared__ __align__(1024) uint8_t smem_raw[];
     PfHdr* H = reinterpret_cast<PfHdr*>(smem_raw);
     uint8_t* sQ = smem_raw + kPfHdr;
@@ -129,6 +125,9 @@ k_prefill_attn(const int* __restrict__ seq_lens, CcKv kv, CcDims D, CcWork W, co
         Item it;
         for (int id = blockIdx.x; item_at(W, D, seq_lens, id, it); id += gridDim.x) {
             const int n_pages = (it.s_last + CC_PAGE - 1) / CC_PAGE;
+            const int rep = replica_of_pos(W.sched->cnt, W.sched->goff, W.pos_of[it.row0]);   // whose KV partition the chunk lives in
+            const CUtensorMap* tmK = &maps.k[rep];
+            const CUtensorMap* tmV = &maps.v[rep];
             for (int j = 0; j < it.n_tiles; ++j, ++g) {
                 const int stage = (int)(g % kKvStages);
                 mbar_wait(&H->kv_empty[stage], ((g / kKvStages) & 1) ^ 1);
@@ -136,7 +135,7 @@ k_prefill_attn(const int* __restrict__ seq_lens, CcKv kv, CcDims D, CcWork W, co
                 int pid = 0;
                 if (lane < in_tile) {
                     pid = kv.block_table[(size_t)it.bt_row * D.max_blocks + pg0 + lane];
-                    if (pid < 0 || pid >= kv.n_pages) {
+                    if (pid < 0 || pid >= kv.n_pages_r[rep]) {
                         atomicOr(W.err, CC_DEVERR_BAD_PAGE);
                         pid = 0;
                     }
@@ -155,8 +154,8 @@ k_prefill_attn(const int* __restrict__ seq_lens, CcKv kv, CcDims D, CcWork W, co
                             const uint32_t d = dst0 + (uint32_t)i * 2048u;
 #pragma unroll
                             for (int hf = 0; hf < 2; ++hf) {
-                                tma_load_2d(d + hf * 8192u, &tmK, hf * 64, row0, bar);
-                                tma_load_2d(d + 16384u + hf * 8192u, &tmV, hf * 64, row0, bar);
+                                tma_load_2d(d + hf * 8192u, tmK, hf * 64, row0, bar);
+                                tma_load_2d(d + 16384u + hf * 8192u, tmV, hf * 64, row0, bar);
                             }
                         }
                     }
@@ -363,10 +362,9 @@ cudaError_t cc_prefill_configure() {
 
 cudaError_t cc_launch_prefill_attention(const int* seq_lens, const CcKv& kv, const CcDims& D, const CcWork& W, const CcLaunch& L) {
     if (D.Dh != 128) return cudaErrorInvalidValue;
-    CUtensorMap tmK, tmV;
-    cudaError_t e = cc_make_kv_tensor_map(&tmK, kv.k_pool, kv.n_pages, D.Hkv, D.Dh, CC_PAGE);
-    if (e == cudaSuccess) e = cc_make_kv_tensor_map(&tmV, kv.v_pool, kv.n_pages, D.Hkv, D.Dh, CC_PAGE);
+    CcKvMaps maps;
+    cudaError_t e = cc_make_kv_maps(&maps, kv, D.Hkv, D.Dh, CC_PAGE);
     if (e != cudaSuccess) return e;
     CcLaunch plain{L.st, L.n_sms, false};
-    return cc_launch_kernel(k_prefill_attn, dim3(L.n_sms), dim3(kPfThreads), (size_t)kPfSmem, plain, seq_lens, kv, D, W, tmK, tmV);
+    return cc_launch_kernel(k_prefill_attn, dim3(L.n_sms), dim3(kPfThreads), (size_t)kPfSmem, plain, seq_lens, kv, D, W, maps);
 }

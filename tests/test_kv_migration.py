@@ -298,3 +298,73 @@ def test_migration_overlapped_with_decode_steps_changes_nothing():
         # pages present at the swap are in the partition (the two later steps may have opened one anywhere)
         for j in range((int(seq[b]) - after + 15) // 16):
             assert assign[b] * psz <= bt[b, j] < (assign[b] + 1) * psz
+
+
+@pytest.mark.gpu
+@pytest.mark.parametrize("big", [False, True])
+def test_replica_with_its_own_kv_partition_as_a_separate_allocation(big):
+    """cc_layer_set_kv_partition (SURVEY.md 8(c) reading 17): replica 1's requests keep their pages in a
+    SEPARATE allocation, page ids relative to it.  The pages of replica 1's rows are moved there (compacted ids, their
+    old places in the shared pool poisoned with NaN); outputs must be bitwise those of the one-pool run, the appended
+    K/V must land in the partition, and the shared pool must stay untouched where replica 1's rows used to live.  Small
+    step (decode kernels) and large step (a prompt chunk through the prefill kernel + decode rows)."""
+    import torch
+    from paper_2607_04181_b200 import binding as B
+    from paper_2607_04181_b200.harness import DeviceStep, Session, _dev_u16, _host_u16
+
+    shape = I.LayerShape("kvpart", 512, 8, 2, 128, 1408, 1e-5, 500000.0, 8, 0, 600)
+    page = shape.page
+    if big:
+        from tests.test_gpu_mixed import mixed_step
+        rng = np.random.default_rng(8)
+        st, assign = mixed_step(shape, 8, [(30, 180), (0, 90)], rng.integers(0, 400, 50), 2)    # chunk 0 -> replica 0, chunk 1 -> replica 1
+    else:
+        st = I.make_step_inputs(shape, 2601, 3601, batch=24)
+        assign = (np.arange(24) % 2).astype(np.int32)
+        assign[5] = 0
+    batch = st.hidden.shape[0]
+    w = I.make_weights(shape, 1601)
+    kw = dict(max_batch=batch, max_blocks=st.block_table.shape[1], max_position=st.block_table.shape[1] * page)
+    with Session(shape, w, **kw) as S:
+        S.scale(2)
+        step = DeviceStep(st, assign)
+        S.forward(step)
+        torch.cuda.synchronize()
+        want, (kw1, vw1) = step.out_bits(), step.pools_bits()
+    # move replica 1's pages into their own pools
+    rows1 = np.nonzero((assign == 1) & (st.seq_lens > 0))[0]
+    remap, bt2 = {}, st.block_table.copy()
+    for b in rows1:                                                       # whole rows: the rows of a prompt chunk carry identical copies
+        for j in range(st.block_table.shape[1]):
+            pg = int(st.block_table[b, j])
+            if pg >= 0:
+                remap.setdefault(pg, len(remap))
+                bt2[b, j] = remap[pg]
+    n1 = len(remap)
+    old = np.array(list(remap.keys())), np.array(list(remap.values()))
+    k1 = np.zeros((n1,) + st.k_pool.shape[1:], np.uint16); v1 = np.zeros_like(k1)
+    k1[old[1]], v1[old[1]] = st.k_pool[old[0]], st.v_pool[old[0]]
+    k0, v0 = st.k_pool.copy(), st.v_pool.copy()
+    k0[old[0]] = 0x7FC0; v0[old[0]] = 0x7FC0                              # nobody may read replica 1's old pages
+    st2 = I.StepInputs(st.hidden, k0, v0, bt2, st.seq_lens, st.n_pages)
+    with Session(shape, w, **kw) as S:
+        S.scale(2)
+        d_k1, d_v1 = _dev_u16(k1, S.device), _dev_u16(v1, S.device)
+        B.cc_layer_set_kv_partition(S.layer, 1, d_k1, d_v1, n1, torch.cuda.current_stream())
+        step = DeviceStep(st2, assign)
+        S.forward(step)
+        torch.cuda.synchronize()
+        assert B.cc_poll_device_error(S.ctx) == 0
+        got, (kg0, vg0) = step.out_bits(), step.pools_bits()
+        kg1, vg1 = _host_u16(d_k1), _host_u16(d_v1)
+        # a page id beyond the partition is refused for replica 1's rows although the shared pool has that page
+        bad = bt2.copy(); bad[rows1[0], 0] = n1 + 3
+        step.block_table.copy_(torch.from_numpy(bad).to(S.device))
+        S.forward(step)
+        torch.cuda.synchronize()
+        assert B.cc_poll_device_error(S.ctx) & B.CC_DEVERR_BAD_PAGE
+    assert np.array_equal(got, want)
+    assert np.array_equal(kg1[old[1]], kw1[old[0]]) and np.array_equal(vg1[old[1]], vw1[old[0]])     # partition == what the one-pool run left on those pages
+    keep = np.ones(st.k_pool.shape[0], bool); keep[old[0]] = False
+    assert np.array_equal(kg0[keep], kw1[keep]) and np.array_equal(vg0[keep], vw1[keep])
+    assert np.array_equal(kg0[~keep], k0[~keep]) and np.array_equal(vg0[~keep], v0[~keep])             # still the poison
