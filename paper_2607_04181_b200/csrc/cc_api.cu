@@ -147,6 +147,7 @@ struct cc_ctx {
     bool row_used[CC_MAX_LAYERS] = {};
     int n_layers = 0;
     bool pdl = true;
+    bool cluster_gemm = true;                  // small steps run QKV / O / down as cluster split-K (CC_CLUSTER_GEMM=0: stream-K everywhere)
     int operand_format = CC_OPERAND_AUTO;      // layers created from now on (cc_ctx_set_operand_format)
     // activation planes of the four GEMM operands (x, o, y, a) of an fp16 layer, per step: steps of at most
     // `planes_rows` rows are HBM-bound and take planes_small (two planes cost nothing there); larger steps take
@@ -261,6 +262,8 @@ cc_status cc_ctx_create(int device, cc_ctx** out) {
     }
     const char* env = getenv("CC_PDL");
     if (env && env[0] == '0') ctx->pdl = false;
+    env = getenv("CC_CLUSTER_GEMM");
+    if (env && env[0] == '0') ctx->cluster_gemm = false;
     env = getenv("CC_PLANES");                  // "xoya,xoya[,rows]": planes of small and large steps, e.g. 2222,1212,64
     if (env && std::strlen(env) >= 9 && env[4] == ',') {
         bool ok = true;
@@ -467,6 +470,11 @@ cc_status cc_create_layer(cc_ctx* ctx, const cc_layer_desc* desc, const cc_layer
     D.off_g1 = blob.take((size_t)D.d * 2);
     D.off_g2 = blob.take((size_t)D.d * 2);
     L->blob_bytes = blob.take(0);
+    if (ctx->cluster_gemm) {
+        D.qkv.S = cc_gemm_cl_cluster_size(0, D.qkv, ctx->n_sms);
+        D.o.S = cc_gemm_cl_cluster_size(1, D.o, ctx->n_sms);
+        D.dn.S = cc_gemm_cl_cluster_size(3, D.dn, ctx->n_sms);
+    }
     if (D.qkv.ST > CC_FLAG_STRIDE || D.o.ST > CC_FLAG_STRIDE || D.gu.ST > CC_FLAG_STRIDE || D.dn.ST > CC_FLAG_STRIDE ||
         D.Mpart > CC_MAX_MPAD) {
         delete L;
@@ -891,15 +899,21 @@ cudaError_t enqueue_forward(cc_layer* L, __nv_bfloat16* hidden, const CcKv& kv, 
         so.hidden = hidden;
         h_in = h_out = hidden_host_alias;
     }
+    // the three short projections of a SMALL step run as cluster split-K (k_gemm_cl): decided by the row count alone --
+    // the worst-case grouped size of `batch` rows over CC_MAX_REPLICAS groups -- so it cannot differ between replica counts
+    const bool cl = (batch + 15) / 16 * 16 + 16 * (CC_MAX_REPLICAS - 1) <= cc_gemm_cl_max_rows();
     for (int stage = 0; stage < kForwardLaunches && e == cudaSuccess; ++stage) {
         if (ev && (e = cudaEventRecord(ev[stage], st)) != cudaSuccess) break;
         switch (stage) {
             case 0: e = cc_launch_prologue(assign, seq_lens, kv.block_table, batch, h_in, D, tab, W, Ln, so); break;
-            case 1: e = cc_launch_gemm(0, D, tab, W, seq_lens, assign, batch, kv, hidden, Ln); break;
+            case 1: e = (cl && D.qkv.S) ? cc_launch_gemm_cl(0, D, tab, W, seq_lens, assign, batch, kv, hidden, Ln)
+                                       : cc_launch_gemm(0, D, tab, W, seq_lens, assign, batch, kv, hidden, Ln); break;
             case 2: e = cc_launch_attention(seq_lens, kv, D, tab, W, Ln); break;
-            case 3: e = cc_launch_gemm(1, D, tab, W, seq_lens, assign, batch, kv, hidden, Ln); break;
+            case 3: e = (cl && D.o.S) ? cc_launch_gemm_cl(1, D, tab, W, seq_lens, assign, batch, kv, hidden, Ln)
+                                     : cc_launch_gemm(1, D, tab, W, seq_lens, assign, batch, kv, hidden, Ln); break;
             case 4: e = cc_launch_gemm(2, D, tab, W, seq_lens, assign, batch, kv, hidden, Ln); break;
-            default: e = cc_launch_gemm(3, D, tab, W, seq_lens, assign, batch, kv, h_out, Ln); break;
+            default: e = (cl && D.dn.S) ? cc_launch_gemm_cl(3, D, tab, W, seq_lens, assign, batch, kv, h_out, Ln)
+                                        : cc_launch_gemm(3, D, tab, W, seq_lens, assign, batch, kv, h_out, Ln); break;
         }
     }
     if (ev && e == cudaSuccess) e = cudaEventRecord(ev[kForwardLaunches], st);

@@ -63,7 +63,7 @@ struct CcGemmGeo {
     int ST;       // super tiles of CC_G * 128 output features
     int KB;       // k-blocks of 64 per tile
     int P;        // CTAs (ranges)
-    int pad_;
+    int S;        // cluster size of the small-step cluster split-K kernel (k_gemm_cl), 0 = stream-K only
     size_t w_off; // byte offset of the packed matrix inside a replica blob
 };
 // Range of CTA i: units [cc_range_begin(i), cc_range_begin(i+1)).

@@ -441,6 +441,281 @@ k_gemm(CcGemmGeo G, const uint8_t* __restrict__ act, float* __restrict__ part, i
 #endif
 }
 
+
+// ---------------------------------------------------------------------------------------------------------------
+// k_gemm_cl -- the same projection for SMALL steps (at most kClRows grouped rows) of the three short GEMMs (QKV, O,
+// down) as a CLUSTER split-K: one cluster of S CTAs per super tile (256 output features), CTA `rank` streams k-blocks
+// [rank KB / S, (rank + 1) KB / S) of every active replica's blob into ONE pair of TMEM accumulators (group r at
+// columns goff[r] ..), and the S partial sums are reduced through distributed shared memory instead of global
+// memory: after the main loops every CTA scatters the columns (batch rows) CTA j owns into CTA j's ring memory
+// (st.shared::cluster, slot = sender rank), a cluster barrier, and every CTA adds the S slots of its own columns in
+// rank order and runs the fused epilogue on them.  No partial sums in global memory, no arrival flags, no fixup
+// pass: the kernel's tail is one DSMEM exchange (~2 us) instead of the stream-K chain (~8 us: partial store, fence,
+// counter, wait for the slowest of the m CTAs of a super tile, one or two fixup passes).  The k split and the sum
+// order are functions of the layer shape only => bit-identical across replica counts; the host picks
+// this kernel from the step's ROW COUNT only, so the choice cannot differ between replica counts either.
+constexpr int kClRows = 128;                  // grouped rows (n_pos) the two accumulators and the exchange buffers are sized for
+constexpr int kClMaxS = 8;
+
+template <int KIND>
+__global__ void __launch_bounds__(kGemmThreads, 1)
+k_gemm_cl(CcGemmGeo G, const uint8_t* __restrict__ act, CcEpi E, CcDims D, CcWork W, const CcLayerTable* __restrict__ tab, int S) {
+    const int planes = D.pl[KIND];
+    const CcSched* __restrict__ sched = W.sched;
+    const int Mpad = D.Mpad;
+    extern __shared__ __align__(1024) uint8_t smem_raw[];
+    GemmSmemHdr* H = reinterpret_cast<GemmSmemHdr*>(smem_raw);
+    const int warp = uniform((int)(threadIdx.x >> 5)), lane = threadIdx.x & 31;
+    const int rank = (int)cluster_ctarank();
+    const int st = (int)blockIdx.x / S;                              // the cluster's super tile
+
+    if (threadIdx.x == 0) CC_TP(W, 2 + KIND, 0);
+    if (threadIdx.x == 0) {
+        for (int i = 0; i < kMaxStages; ++i) {
+            mbar_init(&H->full[i], 1);
+            mbar_init(&H->empty[i], 1);
+        }
+        mbar_init(&H->tmem_full[0], 1);
+        fence_mbar_init();
+    }
+    if (warp == 1) tmem_alloc<kTmemCols>(&H->tmem_base);
+    if (KIND == EPI_QKV) {                                           // starts before k_prologue has finished: counts the groups itself
+        int* wcnt = H->aux;
+        if (threadIdx.x < 256) {
+            uint32_t err = 0;
+            const int rep = cc_row_replica(E.assign, E.seq_lens, threadIdx.x, E.batch, D, tab->active_mask, err);
+#pragma unroll
+            for (int r = 0; r < CC_MAXR; ++r) {
+                const uint32_t bal = __ballot_sync(0xffffffffu, rep == r);
+                if (lane == 0) wcnt[warp * CC_MAXR + r] = __popc(bal);
+            }
+        }
+        __syncthreads();
+        if (threadIdx.x == 0) {
+            int off = 0;
+            for (int r = 0; r < CC_MAXR; ++r) {
+                int c = 0;
+                for (int w = 0; w < 8; ++w) c += wcnt[w * CC_MAXR + r];
+                H->cnt[r] = c;
+                H->goff[r] = off;
+                off += (c + CC_ROW_ALIGN - 1) / CC_ROW_ALIGN * CC_ROW_ALIGN;
+            }
+        }
+    } else if (threadIdx.x < CC_MAXR) {
+        H->cnt[threadIdx.x] = sched->cnt[threadIdx.x];
+        H->goff[threadIdx.x] = sched->goff[threadIdx.x];
+    }
+    if (threadIdx.x < CC_MAXR) {
+        const CcReplicaRow rr = tab->rep[threadIdx.x];
+        H->blob[threadIdx.x] = rr.blob;
+        H->kpool[threadIdx.x] = rr.k_pool ? (__nv_bfloat16*)rr.k_pool : E.kv.k_pool;
+        H->vpool[threadIdx.x] = rr.k_pool ? (__nv_bfloat16*)rr.v_pool : E.kv.v_pool;
+        H->kvpages[threadIdx.x] = rr.k_pool ? rr.n_pages : E.kv.n_pages;
+    }
+    tc_fence_before();
+    __syncthreads();
+    tc_fence_after();
+
+    int nmax = 0, n_pos = 0;
+#pragma unroll
+    for (int r = 0; r < CC_MAXR; ++r) {
+        const int n = (H->cnt[r] + CC_ROW_ALIGN - 1) / CC_ROW_ALIGN * CC_ROW_ALIGN;
+        nmax = max(nmax, n);
+        n_pos = max(n_pos, n ? H->goff[r] + n : 0);
+    }
+    nmax = uniform(nmax);
+    n_pos = uniform(n_pos);
+    const uint32_t stage_bytes = kWStage + (uint32_t)planes * (uint32_t)nmax * 128u;
+    uint8_t* stage0 = smem_raw + kHdrBytes;
+    int n_stages = (kGemmSmem - kHdrBytes) / (int)stage_bytes;
+    if (n_stages > kMaxStages) n_stages = kMaxStages;
+    const int kb0 = (int)((long long)rank * G.KB / S), kb1 = (int)((long long)(rank + 1) * G.KB / S);
+    const uint32_t tmem_base = uniform(H->tmem_base);
+    // columns (grouped rows) CTA j owns in the reduction: [j * cper, (j + 1) * cper)
+    const int cper = ((n_pos + S - 1) / S + 7) & ~7;
+
+    if (nmax > 0) {
+        if (warp == 0) {
+            // ===================== producer (as in k_gemm: weights first, then the dependency, then the slabs) =====
+            const uint64_t pol_w = policy_evict_first(), pol_a = policy_evict_last();
+            const size_t kb_stride = (size_t)(Mpad >> 3) * planes * 1024;
+            int n_act = 0;
+            for (int r = 0; r < CC_MAXR; ++r) n_act += uniform(H->cnt[r]) > 0;
+            const int total = (kb1 - kb0) * n_act;
+            const int n_pre = total < n_stages ? total : n_stages;
+            auto run = [&](const int mode) {
+                int stage = 0, idx = 0;
+                uint32_t ph = 0;
+                uint8_t* sW = stage0;
+                for (int r = 0; r < CC_MAXR; ++r) {
+                    const int cnt = uniform(H->cnt[r]);
+                    if (cnt == 0) continue;
+                    const uint32_t nb = (uint32_t)((cnt + 15) & ~15) * 128u * (uint32_t)planes;
+                    const uint32_t tx = kWStage + nb;
+                    const uint8_t* wsrc = uniform(H->blob[r]) + G.w_off + ((size_t)st * G.KB + kb0) * kWStage;
+                    const uint8_t* asrc = act + (size_t)(uniform(H->goff[r]) >> 3) * planes * 1024 + (size_t)kb0 * kb_stride;
+                    for (int kb = kb0; kb < kb1; ++kb, ++idx) {
+                        if (mode == 0 && idx >= n_pre) return;
+                        const bool pre = idx < n_pre;
+                        if (mode == 1 && !pre) mbar_wait(&H->empty[stage], ph ^ 1);
+                        if (elect_one()) {
+                            if (mode == 0 || !pre) {
+                                mbar_expect_tx(&H->full[stage], tx);
+                                bulk_g2s_hint(sW, wsrc, kWStage, &H->full[stage], pol_w);
+                            }
+                            if (mode == 1) bulk_g2s_hint(sW + kWStage, asrc, nb, &H->full[stage], pol_a);
+                        }
+                        wsrc += kWStage;
+                        asrc += kb_stride;
+                        sW += stage_bytes;
+                        if (++stage == n_stages) { stage = 0; ph ^= 1; sW = stage0; }
+                    }
+                }
+            };
+            run(0);
+            pdl_wait();
+            if (lane == 0) CC_TP(W, 2 + KIND, 1);
+            __syncwarp();
+            if (elect_one()) pdl_launch_dependents();
+            run(1);
+            if (lane == 0) CC_TP(W, 2 + KIND, 2);
+            __syncwarp();
+        } else if (warp == 1) {
+            // ===================== MMA issuer: group r accumulates into columns goff[r] .. of the two tiles =====
+            int stage = 0;
+            uint32_t ph = 0;
+            const uint32_t a_hi = (uint32_t)(umma_desc_sw128(0) >> 32);
+            const uint32_t b_hi = (uint32_t)(umma_desc_sw128(0, (uint32_t)planes * 1024u) >> 32);
+            const uint32_t desc_lo0 = (uint32_t)umma_desc_sw128(smem_u32(stage0));
+            const uint32_t dstage = stage_bytes >> 4, dact = kWStage >> 4;
+            uint32_t da = desc_lo0;
+            for (int r = 0; r < CC_MAXR; ++r) {
+                const int cnt = uniform(H->cnt[r]);
+                if (cnt == 0) continue;
+                const uint32_t idesc = umma_idesc_m128((uint32_t)((cnt + 15) & ~15), D.fmt);
+                const uint32_t col0 = (uint32_t)uniform(H->goff[r]);
+                for (int kb = kb0; kb < kb1; ++kb) {
+                    mbar_wait(&H->full[stage], ph);
+                    tc_fence_after();
+                    if (elect_one()) {
+                        const uint32_t db = da + dact;
+#pragma unroll
+                        for (int j = 0; j < CC_G; ++j) {
+                            const uint32_t d_tmem = tmem_base + (uint32_t)j * 256 + col0;
+                            const uint32_t daj = da + (uint32_t)j * (CC_A_TILE_BYTES >> 4);
+#pragma unroll
+                            for (int k = 0; k < CC_TILE_K / 16; ++k) {
+                                umma_bf16_lo(d_tmem, daj + 2 * k, db + 2 * k, a_hi, b_hi, idesc, (kb == kb0 && k == 0) ? 0u : 1u);
+                                if (planes == 2) umma_bf16_lo(d_tmem, daj + 2 * k, db + 64 + 2 * k, a_hi, b_hi, idesc, 1u);
+                            }
+                        }
+                        umma_commit(&H->empty[stage]);
+                    }
+                    __syncwarp();
+                    da += dstage;
+                    if (++stage == n_stages) { stage = 0; ph ^= 1; da = desc_lo0; }
+                }
+            }
+            if (elect_one()) umma_commit(&H->tmem_full[0]);
+            __syncwarp();
+        } else if (warp >= 6) {
+            // ===================== helper warps: per-row tables of the fused epilogue =====================
+            pdl_wait();
+            for (int p = (int)threadIdx.x - 6 * 32; p < n_pos; p += kGemmThreads - 6 * 32) {
+                const int b = W.perm[p];
+                H->perm[p] = b;
+                if (KIND == EPI_QKV) {
+                    int pos = -1, page = -1;
+                    if (b >= 0) {
+                        pos = E.seq_lens[b] - 1;
+                        page = E.kv.block_table[(size_t)b * D.max_blocks + pos / CC_PAGE];
+                    }
+                    H->aux[p] = pos;
+                    H->page[p] = page;
+                } else if (KIND == EPI_O) {
+                    H->aux[p] = __float_as_int(b >= 0 ? W.inv_in[p] : 0.f);
+                }
+            }
+        }
+        // the scatter warps wait for this CTA's accumulators here, so that "my main loop is over" reaches the barrier
+        if (warp >= 2 && warp < 6) {
+            mbar_wait(&H->tmem_full[0], 0);
+            tc_fence_after();
+        }
+    }
+    __syncthreads();
+    if (threadIdx.x == 0) CC_TP(W, 2 + KIND, 3);
+    if (nmax == 0) {                                                 // nothing runs this step (the same in every CTA of the cluster)
+        pdl_wait();
+        if (warp == 1) tmem_dealloc<kTmemCols>(tmem_base);
+        return;
+    }
+    cluster_sync_all();                                              // every ring of the cluster is dead: it becomes the exchange buffer
+    // exchange buffer in CTA j: [sender rank][tile 0 | 1][column of j's range][128 features] fp32
+    const uint32_t slot_bytes = (uint32_t)CC_G * (uint32_t)cper * 512u;
+    if (warp >= 2 && warp < 6) {
+        const int q = warp & 3, f = q * 32 + lane;                   // TMEM lane quarter; output feature within the tile
+        const uint32_t my_buf = smem_u32(stage0) + (uint32_t)rank * slot_bytes;
+        for (int c0 = 0; c0 < n_pos; c0 += 8) {                      // 8 columns: one owner
+            const int owner = c0 / cper, cl = c0 - owner * cper;
+            const uint32_t dst = mapa_u32(my_buf, (uint32_t)owner) + (uint32_t)cl * 512u + (uint32_t)f * 4u;
+#pragma unroll
+            for (int j = 0; j < CC_G; ++j) {
+                uint32_t v[8];
+                asm volatile("tcgen05.ld.sync.aligned.32x32b.x8.b32 {%0, %1, %2, %3, %4, %5, %6, %7}, [%8];"
+                             : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]), "=r"(v[7])
+                             : "r"(tmem_base + ((uint32_t)(q * 32) << 16) + (uint32_t)j * 256 + (uint32_t)c0)
+                             : "memory");
+                tmem_ld_wait();
+#pragma unroll
+                for (int i = 0; i < 8; ++i)
+                    asm volatile("st.shared::cluster.b32 [%0], %1;" ::"r"(dst + (uint32_t)j * (uint32_t)cper * 512u + (uint32_t)i * 512u), "r"(v[i])
+                                 : "memory");
+            }
+        }
+    }
+    tc_fence_before();
+    cluster_sync_all();                                              // all slots of my columns have landed (release / acquire at cluster scope)
+    if (warp == 1) tmem_dealloc<kTmemCols>(tmem_base);
+    if (threadIdx.x == 0) CC_TP(W, 2 + KIND, 4);
+    // ---- my columns: add the S slots in rank order, fused epilogue; one warp per (column, tile) item ----
+    {
+        constexpr int kWarps = kGemmThreads / 32;
+        const int c_lo = rank * cper, c_hi = min(n_pos, c_lo + cper);
+        const int n_items = max(0, c_hi - c_lo) * CC_G;
+        const float* buf = reinterpret_cast<const float*>(stage0);
+        const size_t slot_f = slot_bytes / 4;
+        for (int it0 = warp * 2; it0 < n_items; it0 += kWarps * 2) {
+            EpiPre pre[2];
+            int pp[2], bb[2], tt[2];
+            float4 acc[2];
+#pragma unroll
+            for (int u = 0; u < 2; ++u) {
+                const int it = it0 + u, cl = it / CC_G, j = it - cl * CC_G;
+                pp[u] = c_lo + cl;
+                tt[u] = st * CC_G + j;
+                bb[u] = it < n_items ? H->perm[pp[u]] : -1;
+                acc[u] = make_float4(0.f, 0.f, 0.f, 0.f);
+                if (bb[u] >= 0) {
+                    epi_pre<KIND>(pre[u], E, D, W, SmemTab{H}, tt[u], pp[u], bb[u], lane);
+                    const float* src = buf + ((size_t)j * cper + cl) * 128 + 4 * lane;
+                    for (int sdr = 0; sdr < S; ++sdr) {               // rank order: fixed
+                        const float4 v = *reinterpret_cast<const float4*>(src + (size_t)sdr * slot_f);
+                        acc[u].x += v.x; acc[u].y += v.y; acc[u].z += v.z; acc[u].w += v.w;
+                    }
+                }
+            }
+#pragma unroll
+            for (int u = 0; u < 2; ++u)
+                if (bb[u] >= 0) epi_fin<KIND>(pre[u], E, D, W, SmemTab{H}, tt[u], pp[u], bb[u], acc[u], lane);
+        }
+    }
+#ifdef CC_TRACE
+    __syncthreads();
+    if (threadIdx.x == 0) CC_TP(W, 2 + KIND, 5);
+#endif
+}
+
 }  // namespace
 
 cudaError_t cc_gemm_configure() {
@@ -448,7 +723,62 @@ cudaError_t cc_gemm_configure() {
     if (e == cudaSuccess) e = cudaFuncSetAttribute(k_gemm<EPI_O>, cudaFuncAttributeMaxDynamicSharedMemorySize, kGemmSmem);
     if (e == cudaSuccess) e = cudaFuncSetAttribute(k_gemm<EPI_GU>, cudaFuncAttributeMaxDynamicSharedMemorySize, kGemmSmem);
     if (e == cudaSuccess) e = cudaFuncSetAttribute(k_gemm<EPI_DN>, cudaFuncAttributeMaxDynamicSharedMemorySize, kGemmSmem);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_gemm_cl<EPI_QKV>, cudaFuncAttributeMaxDynamicSharedMemorySize, kGemmSmem);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_gemm_cl<EPI_O>, cudaFuncAttributeMaxDynamicSharedMemorySize, kGemmSmem);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_gemm_cl<EPI_DN>, cudaFuncAttributeMaxDynamicSharedMemorySize, kGemmSmem);
     return e;
+}
+
+// ---- cluster split-K variant (k_gemm_cl): small steps of the QKV, O and down projections --------------------------
+typedef void (*ClKernel)(CcGemmGeo, const uint8_t*, CcEpi, CcDims, CcWork, const CcLayerTable*, int);
+static ClKernel cl_kernel(int which) {
+    return which == 0 ? (ClKernel)k_gemm_cl<EPI_QKV> : which == 1 ? (ClKernel)k_gemm_cl<EPI_O> : (ClKernel)k_gemm_cl<EPI_DN>;
+}
+static void cl_config(cudaLaunchConfig_t& cfg, cudaLaunchAttribute* attr, int ST, int S, cudaStream_t st, bool pdl) {
+    cfg = cudaLaunchConfig_t{};
+    cfg.gridDim = dim3((unsigned)(ST * S));
+    cfg.blockDim = dim3(kGemmThreads);
+    cfg.dynamicSmemBytes = kGemmSmem;
+    cfg.stream = st;
+    attr[0].id = cudaLaunchAttributeClusterDimension;
+    attr[0].val.clusterDim.x = (unsigned)S;
+    attr[0].val.clusterDim.y = 1;
+    attr[0].val.clusterDim.z = 1;
+    attr[1].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[1].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = pdl ? 2 : 1;
+}
+// Largest cluster size S <= 8 for which all ST clusters of S CTAs are co-resident (one wave) and every CTA gets at
+// least one k-block; 0 = the projection stays on the stream-K kernel.  A function of the layer shape and the device.
+int cc_gemm_cl_cluster_size(int which, const CcGemmGeo& g, int n_sms) {
+    if (which == 2) return 0;                                   // gate/up: 112+ super tiles, stream-K balances them
+    int best = 0;
+    for (int S = 1; S <= kClMaxS; ++S) {
+        if (S > g.KB || g.ST * S > n_sms) continue;
+        cudaLaunchConfig_t cfg;
+        cudaLaunchAttribute attr[2];
+        cl_config(cfg, attr, g.ST, S, nullptr, false);
+        int n = 0;
+        if (cudaOccupancyMaxActiveClusters(&n, (void*)cl_kernel(which), &cfg) != cudaSuccess) {
+            cudaGetLastError();
+            continue;
+        }
+        if (n >= g.ST) best = S;
+    }
+    return best;
+}
+int cc_gemm_cl_max_rows() { return kClRows; }
+
+cudaError_t cc_launch_gemm_cl(int which, const CcDims& D, const CcLayerTable* tab, const CcWork& W, const int* seq_lens,
+                              const int* assign, int batch, const CcKv& kv, __nv_bfloat16* hidden, const CcLaunch& L) {
+    CcEpi E{assign, batch, seq_lens, kv, hidden};
+    const CcGemmGeo& g = which == 0 ? D.qkv : which == 1 ? D.o : D.dn;
+    const uint8_t* act = which == 0 ? W.x_act : which == 1 ? W.o_act : W.a_act;
+    cudaLaunchConfig_t cfg;
+    cudaLaunchAttribute attr[2];
+    cl_config(cfg, attr, g.ST, g.S, L.st, L.pdl);
+    return cudaLaunchKernelEx(&cfg, cl_kernel(which), g, act, E, D, W, tab, g.S);
 }
 
 // which: 0 = QKV, 1 = O, 2 = gate/up, 3 = down

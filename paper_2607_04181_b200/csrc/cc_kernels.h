@@ -108,6 +108,11 @@ cudaError_t cc_launch_prologue(const int* assign, const int* seq_lens, const int
 cudaError_t cc_launch_gemm(int which, const CcDims& D, const CcLayerTable* tab, const CcWork& W, const int* seq_lens,
                            const int* assign, int batch, const CcKv& kv, __nv_bfloat16* hidden, const CcLaunch& L);
 // rowmap (large steps): original row of entry i of the attention work axis (the decode rows); null = row i itself
+// small steps (at most cc_gemm_cl_max_rows() grouped rows) of QKV / O / down as a cluster split-K (cc_gemm.cu: k_gemm_cl)
+cudaError_t cc_launch_gemm_cl(int which, const CcDims& D, const CcLayerTable* tab, const CcWork& W, const int* seq_lens,
+                              const int* assign, int batch, const CcKv& kv, __nv_bfloat16* hidden, const CcLaunch& L);
+int cc_gemm_cl_cluster_size(int which, const CcGemmGeo& g, int n_sms);
+int cc_gemm_cl_max_rows();
 cudaError_t cc_launch_attention(const int* seq_lens, const CcKv& kv, const CcDims& D, const CcLayerTable* tab,
                                 const CcWork& W, const CcLaunch& L, const int* rowmap = nullptr);
 // ---- large steps (cc_big.cu, cc_big_gemm.cu, cc_prefill.cu) ----
