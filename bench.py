@@ -280,6 +280,7 @@ def run_ours(args):
     graph = CapturedGraph(lambda s: S.forward(step, s))     # counts instantiations, keeps the cudaGraphExec_t
     n_graphs = CapturedGraph.instantiations
     n_launch = B.cc_forward_launch_count(S.layer)
+    gemm_grids = B.cc_layer_gemm_grids(S.layer)          # CTAs and cluster sizes of QKV / O / gate-up / down
 
     # ---- device-resident timed region: K graph replays ------------------------------------------
     for _ in range(W):
@@ -569,6 +570,7 @@ def run_ours(args):
                                    "16-token pages, shuffled block tables",
                        "replicas": R, "batch_split": np.bincount(assign, minlength=R).tolist(),
                        "launch": "one CUDA graph of cc_forward, replayed; PDL between its kernels",
+                       "gemm_grids": dict(zip(("ctas", "cluster_size"), gemm_grids)),
                        "l2": "inputs larger than L2: each step streams R x 436 MB weights + 335 MB KV (L2 = 126 MB)",
                        "parallelism": "replicas only (one independent batch per GPU)" if world > 1 else "single GPU"},
             "clocks": clocks,

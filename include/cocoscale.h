@@ -263,6 +263,11 @@ cc_status cc_forward_host_async(cc_layer *layer, void *hidden_host, void *k_pool
 cc_status cc_forward_profiled(cc_layer *layer, void *hidden_dev, const cc_kv_pages *kv, const int32_t *seq_lens_dev,
                               const int32_t *replica_assign_dev, int batch, void *stream, float *stage_ms_host);
 
+/* Grid of the four projection kernels (QKV, O, gate/up, down) of a SMALL step (<= 80 rows) of this layer: ctas[4] CTAs
+ * each, in clusters of cluster[4] CTAs (0 = the stream-K kernel, one CTA per SM; > 0 = the cluster split-K kernel, one
+ * cluster per 256 output features).  A function of the layer shape and the device, fixed at cc_create_layer. */
+cc_status cc_layer_gemm_grids(const cc_layer *layer, int *ctas, int *cluster);
+
 /* Kernel launches one cc_forward enqueues (for launch accounting). */
 cc_status cc_forward_launch_count(const cc_layer *layer, int *n);
 

@@ -31,7 +31,7 @@ EXPORTS = (
     "cc_ctx_create", "cc_ctx_destroy", "cc_ctx_donate", "cc_ctx_reclaim", "cc_ctx_set_copy_chunk",
     "cc_ctx_set_pdl", "cc_ctx_set_operand_format", "cc_ctx_set_operand_planes", "cc_layer_operand_format", "cc_poll_device_error", "cc_create_layer", "cc_destroy_layer", "cc_layer_blob_bytes",
     "cc_scale_layer", "cc_commit", "cc_release_replica", "cc_query", "cc_layer_set_kv_partition", "cc_active_replicas", "cc_replica_blob", "cc_forward",
-    "cc_forward_host", "cc_forward_host_async", "cc_forward_profiled", "cc_forward_launch_count", "cc_replica_copy", "cc_kv_plan_migration", "cc_kv_plan_catchup", "cc_kv_migrate", "cc_debug_tap", "cc_debug_grouping", "cc_debug_trace",
+    "cc_forward_host", "cc_forward_host_async", "cc_forward_profiled", "cc_forward_launch_count", "cc_layer_gemm_grids", "cc_replica_copy", "cc_kv_plan_migration", "cc_kv_plan_catchup", "cc_kv_migrate", "cc_debug_tap", "cc_debug_grouping", "cc_debug_trace",
     "cc_slotalloc_create", "cc_slotalloc_destroy", "cc_slotalloc_donate", "cc_slotalloc_reclaim",
     "cc_slotalloc_alloc", "cc_slotalloc_free", "cc_slotalloc_free_bytes", "cc_last_error", "cc_version",
     "cc_ctl_mem_bytes", "cc_ctl_flops", "cc_ctl_comm_seconds", "cc_ctl_speedup", "cc_ctl_speedup_vec", "cc_ctl_distance",
@@ -262,6 +262,12 @@ def cc_forward_profiled(layer, hidden, k_pool, v_pool, block_table, n_pages: int
     _check(_lib.cc_forward_profiled(layer, _ptr(hidden), C.byref(kv), _ptr(seq_lens), _ptr(replica_assign),
                                     C.c_int(batch), _stream(stream), _ptr(ms)))
     return ms[:len(BIG_STAGE_NAMES if batch > 256 else STAGE_NAMES)]
+
+
+def cc_layer_gemm_grids(layer):
+    ctas, cluster = (C.c_int * 4)(), (C.c_int * 4)()
+    _check(_lib.cc_layer_gemm_grids(layer, ctas, cluster))
+    return list(ctas), list(cluster)
 
 
 def cc_forward_launch_count(layer) -> int:

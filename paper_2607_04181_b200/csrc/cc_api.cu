@@ -1007,6 +1007,16 @@ cc_status cc_forward_profiled(cc_layer* L, void* hidden_dev, const cc_kv_pages* 
     return CC_OK;
 }
 
+cc_status cc_layer_gemm_grids(const cc_layer* L, int* ctas, int* cluster) {
+    if (!L || !ctas || !cluster) return fail(CC_ERR_INVALID, "null argument");
+    const CcGemmGeo* g[4] = {&L->D.qkv, &L->D.o, &L->D.gu, &L->D.dn};
+    for (int i = 0; i < 4; ++i) {
+        cluster[i] = g[i]->S;
+        ctas[i] = g[i]->S ? g[i]->ST * g[i]->S : g[i]->P;
+    }
+    return CC_OK;
+}
+
 cc_status cc_forward_launch_count(const cc_layer* L, int* n) {
     if (!L || !n) return fail(CC_ERR_INVALID, "null argument");
     *n = kForwardLaunches;

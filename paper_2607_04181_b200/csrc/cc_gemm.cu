@@ -653,24 +653,35 @@ k_gemm_cl(CcGemmGeo G, const uint8_t* __restrict__ act, CcEpi E, CcDims D, CcWor
     cluster_sync_all();                                              // every ring of the cluster is dead: it becomes the exchange buffer
     // exchange buffer in CTA j: [sender rank][tile 0 | 1][column of j's range][128 features] fp32
     const uint32_t slot_bytes = (uint32_t)CC_G * (uint32_t)cper * 512u;
-    if (warp >= 2 && warp < 6) {
-        const int q = warp & 3, f = q * 32 + lane;                   // TMEM lane quarter; output feature within the tile
+    if (warp >= 2 && warp < 14) {                                    // three warps per TMEM lane quarter share the chunks
+        const int q = warp & 3, f = q * 32 + lane, grp = (warp - 2) >> 2;   // lane quarter; output feature within the tile
         const uint32_t my_buf = smem_u32(stage0) + (uint32_t)rank * slot_bytes;
-        for (int c0 = 0; c0 < n_pos; c0 += 8) {                      // 8 columns: one owner
-            const int owner = c0 / cper, cl = c0 - owner * cper;
-            const uint32_t dst = mapa_u32(my_buf, (uint32_t)owner) + (uint32_t)cl * 512u + (uint32_t)f * 4u;
+        int chunk = 0;
+        tc_fence_after();
+        // owners in rotation starting behind this CTA, so that the S senders write to S different CTAs at any time
+        for (int oo = 1; oo <= S; ++oo) {
+            const int owner = (rank + oo) % S;
+            const uint32_t dst_owner = mapa_u32(my_buf, (uint32_t)owner) + (uint32_t)f * 4u;
+            for (int cl = 0; cl < cper; cl += 8) {                   // 8 columns of that owner
+                const int c0 = owner * cper + cl;
+                if (c0 >= n_pos) break;
+                if (chunk++ % 3 != grp) continue;
+                uint32_t v[CC_G][8];
 #pragma unroll
-            for (int j = 0; j < CC_G; ++j) {
-                uint32_t v[8];
-                asm volatile("tcgen05.ld.sync.aligned.32x32b.x8.b32 {%0, %1, %2, %3, %4, %5, %6, %7}, [%8];"
-                             : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]), "=r"(v[7])
-                             : "r"(tmem_base + ((uint32_t)(q * 32) << 16) + (uint32_t)j * 256 + (uint32_t)c0)
-                             : "memory");
+                for (int j = 0; j < CC_G; ++j)
+                    asm volatile("tcgen05.ld.sync.aligned.32x32b.x8.b32 {%0, %1, %2, %3, %4, %5, %6, %7}, [%8];"
+                                 : "=r"(v[j][0]), "=r"(v[j][1]), "=r"(v[j][2]), "=r"(v[j][3]), "=r"(v[j][4]), "=r"(v[j][5]), "=r"(v[j][6]),
+                                   "=r"(v[j][7])
+                                 : "r"(tmem_base + ((uint32_t)(q * 32) << 16) + (uint32_t)j * 256 + (uint32_t)c0)
+                                 : "memory");
                 tmem_ld_wait();
 #pragma unroll
-                for (int i = 0; i < 8; ++i)
-                    asm volatile("st.shared::cluster.b32 [%0], %1;" ::"r"(dst + (uint32_t)j * (uint32_t)cper * 512u + (uint32_t)i * 512u), "r"(v[i])
-                                 : "memory");
+                for (int j = 0; j < CC_G; ++j)
+#pragma unroll
+                    for (int i = 0; i < 8; ++i)
+                        asm volatile("st.shared::cluster.b32 [%0], %1;" ::"r"(dst_owner + ((uint32_t)j * (uint32_t)cper + (uint32_t)(cl + i)) * 512u),
+                                     "r"(v[j][i])
+                                     : "memory");
             }
         }
     }
