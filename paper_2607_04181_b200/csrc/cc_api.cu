@@ -473,6 +473,7 @@ cc_status cc_create_layer(cc_ctx* ctx, const cc_layer_desc* desc, const cc_layer
     if (ctx->cluster_gemm) {
         D.qkv.S = cc_gemm_cl_cluster_size(0, D.qkv, ctx->n_sms);
         D.o.S = cc_gemm_cl_cluster_size(1, D.o, ctx->n_sms);
+        D.gu.S = cc_gemm_cl_cluster_size(2, D.gu, ctx->n_sms);
         D.dn.S = cc_gemm_cl_cluster_size(3, D.dn, ctx->n_sms);
     }
     if (D.qkv.ST > CC_FLAG_STRIDE || D.o.ST > CC_FLAG_STRIDE || D.gu.ST > CC_FLAG_STRIDE || D.dn.ST > CC_FLAG_STRIDE ||
@@ -911,7 +912,8 @@ cudaError_t enqueue_forward(cc_layer* L, __nv_bfloat16* hidden, const CcKv& kv, 
             case 2: e = cc_launch_attention(seq_lens, kv, D, tab, W, Ln); break;
             case 3: e = (cl && D.o.S) ? cc_launch_gemm_cl(1, D, tab, W, seq_lens, assign, batch, kv, hidden, Ln)
                                      : cc_launch_gemm(1, D, tab, W, seq_lens, assign, batch, kv, hidden, Ln); break;
-            case 4: e = cc_launch_gemm(2, D, tab, W, seq_lens, assign, batch, kv, hidden, Ln); break;
+            case 4: e = (cl && D.gu.S) ? cc_launch_gemm_cl(2, D, tab, W, seq_lens, assign, batch, kv, hidden, Ln)
+                                      : cc_launch_gemm(2, D, tab, W, seq_lens, assign, batch, kv, hidden, Ln); break;
             default: e = (cl && D.dn.S) ? cc_launch_gemm_cl(3, D, tab, W, seq_lens, assign, batch, kv, h_out, Ln)
                                         : cc_launch_gemm(3, D, tab, W, seq_lens, assign, batch, kv, h_out, Ln); break;
         }

@@ -30,7 +30,7 @@ namespace {
 
 constexpr int kGemmThreads = 512;         // warp 0 producer, 1 MMA, 2..5 TMEM epilogue, 6..15 row tables; all 16 in the fixup
 constexpr int kHdrBytes = 8192;           // barriers + per-row tables in front of the stage ring
-constexpr int kMaxStages = 4;            // deeper rings do not stream faster (measured again in round 2 with 5 and 6 stages of a one-plane variant: no change)
+constexpr int kMaxStages = 4;            // deeper rings do not stream faster (measured again in round 2: 5 stages no change, 6 stages slower at R = 4)
 constexpr int kGemmSmem = 225 * 1024;     // dynamic shared memory per CTA
 constexpr int kTmemCols = 512;
 constexpr uint32_t kWStage = CC_G * CC_A_TILE_BYTES;   // weight bytes per stage (32 KiB)
@@ -443,8 +443,7 @@ k_gemm(CcGemmGeo G, const uint8_t* __restrict__ act, float* __restrict__ part, i
 
 
 // ---------------------------------------------------------------------------------------------------------------
-// k_gemm_cl -- the same projection for SMALL steps (at most kClRows grouped rows) of the three short GEMMs (QKV, O,
-// down) as a CLUSTER split-K: one cluster of S CTAs per super tile (256 output features), CTA `rank` streams k-blocks
+// k_gemm_cl -- the same projections for SMALL steps (at most kClRows grouped rows) as a CLUSTER split-K: one cluster of S CTAs per super tile (256 output features), CTA `rank` streams k-blocks
 // [rank KB / S, (rank + 1) KB / S) of every active replica's blob into ONE pair of TMEM accumulators (group r at
 // columns goff[r] ..), and the S partial sums are reduced through distributed shared memory instead of global
 // memory: after the main loops every CTA scatters the columns (batch rows) CTA j owns into CTA j's ring memory
@@ -454,7 +453,7 @@ k_gemm(CcGemmGeo G, const uint8_t* __restrict__ act, float* __restrict__ part, i
 // counter, wait for the slowest of the m CTAs of a super tile, one or two fixup passes).  The k split and the sum
 // order are functions of the layer shape only => bit-identical across replica counts; the host picks
 // this kernel from the step's ROW COUNT only, so the choice cannot differ between replica counts either.
-constexpr int kClRows = 128;                  // grouped rows (n_pos) the two accumulators and the exchange buffers are sized for
+constexpr int kClRows = 192;                  // grouped rows (n_pos) the two accumulators and the exchange buffers are sized for
 constexpr int kClMaxS = 8;
 
 template <int KIND>
@@ -634,6 +633,13 @@ k_gemm_cl(CcGemmGeo G, const uint8_t* __restrict__ act, CcEpi E, CcDims D, CcWor
                     H->page[p] = page;
                 } else if (KIND == EPI_O) {
                     H->aux[p] = __float_as_int(b >= 0 ? W.inv_in[p] : 0.f);
+                } else if (KIND == EPI_GU) {
+                    float ss = 0.f;
+                    if (b >= 0) {
+                        const int nt = (D.d + 127) >> 7;
+                        for (int t = 0; t < nt; ++t) ss += W.ssq[(size_t)t * Mpad + p];   // tile order: fixed
+                    }
+                    H->aux[p] = __float_as_int(b >= 0 ? rsqrtf(ss / (float)D.d + D.eps) / W.inv_in[p] : 0.f);
                 }
             }
         }
@@ -737,13 +743,15 @@ cudaError_t cc_gemm_configure() {
     if (e == cudaSuccess) e = cudaFuncSetAttribute(k_gemm_cl<EPI_QKV>, cudaFuncAttributeMaxDynamicSharedMemorySize, kGemmSmem);
     if (e == cudaSuccess) e = cudaFuncSetAttribute(k_gemm_cl<EPI_O>, cudaFuncAttributeMaxDynamicSharedMemorySize, kGemmSmem);
     if (e == cudaSuccess) e = cudaFuncSetAttribute(k_gemm_cl<EPI_DN>, cudaFuncAttributeMaxDynamicSharedMemorySize, kGemmSmem);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_gemm_cl<EPI_GU>, cudaFuncAttributeMaxDynamicSharedMemorySize, kGemmSmem);
     return e;
 }
 
 // ---- cluster split-K variant (k_gemm_cl): small steps of the QKV, O and down projections --------------------------
 typedef void (*ClKernel)(CcGemmGeo, const uint8_t*, CcEpi, CcDims, CcWork, const CcLayerTable*, int);
 static ClKernel cl_kernel(int which) {
-    return which == 0 ? (ClKernel)k_gemm_cl<EPI_QKV> : which == 1 ? (ClKernel)k_gemm_cl<EPI_O> : (ClKernel)k_gemm_cl<EPI_DN>;
+    return which == 0 ? (ClKernel)k_gemm_cl<EPI_QKV> : which == 1 ? (ClKernel)k_gemm_cl<EPI_O>
+           : which == 2 ? (ClKernel)k_gemm_cl<EPI_GU> : (ClKernel)k_gemm_cl<EPI_DN>;
 }
 static void cl_config(cudaLaunchConfig_t& cfg, cudaLaunchAttribute* attr, int ST, int S, cudaStream_t st, bool pdl) {
     cfg = cudaLaunchConfig_t{};
@@ -761,9 +769,11 @@ static void cl_config(cudaLaunchConfig_t& cfg, cudaLaunchAttribute* attr, int ST
     cfg.numAttrs = pdl ? 2 : 1;
 }
 // Largest cluster size S <= 8 for which all ST clusters of S CTAs are co-resident (one wave) and every CTA gets at
-// least one k-block; 0 = the projection stays on the stream-K kernel.  A function of the layer shape and the device.
+// least one k-block; 0 = the projection stays on the stream-K kernel -- also when the clusters would use fewer than 60 %
+// of the CTAs stream-K would (too few SMs pulling on HBM).  A function of the layer shape and the device.  At cfg2 on a
+// B200: QKV 24 x 5 = 120 CTAs, O and down 16 x 6 = 96, gate/up 112 x 1 = 112 (no split at all: one CTA streams the whole
+// K of its super tile and runs the epilogue straight from its accumulators).
 int cc_gemm_cl_cluster_size(int which, const CcGemmGeo& g, int n_sms) {
-    if (which == 2) return 0;                                   // gate/up: 112+ super tiles, stream-K balances them
     int best = 0;
     for (int S = 1; S <= kClMaxS; ++S) {
         if (S > g.KB || g.ST * S > n_sms) continue;
@@ -777,6 +787,7 @@ int cc_gemm_cl_cluster_size(int which, const CcGemmGeo& g, int n_sms) {
         }
         if (n >= g.ST) best = S;
     }
+    if (best && (long long)g.ST * best * 10 < (long long)g.P * 6) best = 0;
     return best;
 }
 int cc_gemm_cl_max_rows() { return kClRows; }
@@ -784,8 +795,8 @@ int cc_gemm_cl_max_rows() { return kClRows; }
 cudaError_t cc_launch_gemm_cl(int which, const CcDims& D, const CcLayerTable* tab, const CcWork& W, const int* seq_lens,
                               const int* assign, int batch, const CcKv& kv, __nv_bfloat16* hidden, const CcLaunch& L) {
     CcEpi E{assign, batch, seq_lens, kv, hidden};
-    const CcGemmGeo& g = which == 0 ? D.qkv : which == 1 ? D.o : D.dn;
-    const uint8_t* act = which == 0 ? W.x_act : which == 1 ? W.o_act : W.a_act;
+    const CcGemmGeo& g = which == 0 ? D.qkv : which == 1 ? D.o : which == 2 ? D.gu : D.dn;
+    const uint8_t* act = which == 0 ? W.x_act : which == 1 ? W.o_act : which == 2 ? W.y_act : W.a_act;
     cudaLaunchConfig_t cfg;
     cudaLaunchAttribute attr[2];
     cl_config(cfg, attr, g.ST, g.S, L.st, L.pdl);

@@ -181,3 +181,42 @@ def test_small_steps_of_a_large_layer_take_the_decode_path_and_keep_their_bits()
     a = run_gpu(shape, w, st, assign, 2, taps=False)
     b = run_gpu(shape, w, st, assign, 2, taps=False, max_batch=2048)
     assert np.array_equal(a[0], b[0]) and np.array_equal(a[1], b[1]) and np.array_equal(a[2], b[2])
+
+
+@pytest.mark.parametrize("hkv,g", [(1, 8), (2, 1), (4, 3), (8, 2), (1, 1)])
+def test_large_path_head_layouts(hkv, g):
+    """The chunk-prefill kernel packs T = 128 // G tokens x G query heads into the 128 rows of its MMA tile and stages one
+    kv head per work item: every kv-head count the library takes and GQA groups 1, 2, 3 and 8 (T = 128, 64, 42, 16; G = 3
+    leaves two rows of the tile unused), chunk lengths that are not multiples of T, kv lengths that end on and next to the
+    64-token kv tile and the 16-token page boundaries, a 2-token chunk."""
+    shape = I.LayerShape(f"mixh{hkv}g{g}", 256, hkv * g, hkv, 128, 512, 1e-5, 10000.0, 8, 0, 400)
+    rng = np.random.default_rng(40 + hkv * 10 + g)
+    chunks = [(0, 64), (63, 130), (1, 2), (128, 191)]            # ends at kv 64, 193, 3, 319
+    st, assign = mixed_step(shape, 40 + hkv * 10 + g, chunks, rng.integers(0, 200, 20), 2)
+    assert st.hidden.shape[0] > 256
+    w = I.make_weights(shape, 1700 + hkv * 10 + g)
+    ref = oracle.layer_forward(shape, w, st.hidden, st.k_pool, st.v_pool, st.block_table, st.seq_lens, assign, 2, taps=True)
+    out, kp, vp, gt, grouping = run_gpu(shape, w, st, assign, 2)
+    check(shape, st, assign, 2, ref, out, kp, vp, gt, grouping)
+
+
+def test_too_many_decode_rows_are_reported_not_faulted():
+    """A large step may hold at most 256 rows outside prompt chunks: 300 lone rows set CC_DEVERR_TOO_MANY_DECODE (the
+    surplus rows' attention is skipped), nothing faults, and the first 256 decode rows are still right."""
+    import torch
+    from paper_2607_04181_b200 import binding as B
+    from paper_2607_04181_b200.harness import DeviceStep, Session
+
+    shape = MID
+    rng = np.random.default_rng(9)
+    st, assign = mixed_step(shape, 9, [], rng.integers(0, 120, 300), 2)
+    w = I.make_weights(shape, 1501)
+    ref = oracle.layer_forward(shape, w, st.hidden, st.k_pool, st.v_pool, st.block_table, st.seq_lens, assign, 2, taps=True)
+    with Session(shape, w, max_batch=300, max_blocks=st.block_table.shape[1], max_position=st.block_table.shape[1] * shape.page) as S:
+        S.scale(2)
+        step = DeviceStep(st, assign)
+        S.forward(step)
+        torch.cuda.synchronize()
+        assert B.cc_poll_device_error(S.ctx) == B.CC_DEVERR_TOO_MANY_DECODE
+        o = S.tap(B.CC_TAP_O, 300)
+    within(o[:256], ref["taps"]["o"][:256], "attention output of the first 256 decode rows")
