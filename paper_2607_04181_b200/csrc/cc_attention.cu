@@ -2,7 +2,7 @@
 // partitioning the paper relies on: PAPER.md:103, 391, 476).
 //
 // HBM-bound: every cached K/V byte of a request is read exactly once per step.  What was measured on
-// the way here (DESIGN.md section 10b): per-(page, head) 4 KiB requests from four warps
+// the way here (DESIGN.md section 9b): per-(page, head) 4 KiB requests from four warps
 // per CTA, by per-lane cp.async or by small TMA boxes alike, stream at 4.7 TB/s even with the math
 // removed, and the ragged end of a 256-token work list costs another ~9 us; whole pages (all kv
 // heads, 2 x 32 KiB contiguous) staged by one producer warp stream at 5.3 TB/s, 6.1 TB/s with an L2

@@ -656,6 +656,24 @@ k_gemm_cl(CcGemmGeo G, const uint8_t* __restrict__ act, CcEpi E, CcDims D, CcWor
         if (warp == 1) tmem_dealloc<kTmemCols>(tmem_base);
         return;
     }
+    // The first items of this warp's epilogue are known already (my columns, the row tables): issue their global loads
+    // (residual rows, gains, RoPE table, h1) now, so that their latency runs under the exchange.
+    constexpr int kWarps = kGemmThreads / 32;
+    const int c_lo = rank * cper, c_hi = min(n_pos, c_lo + cper);
+    const int n_items = max(0, c_hi - c_lo) * CC_G;
+    EpiPre pre[2];
+    int pp[2], bb[2], tt[2];
+    auto setup = [&](int it0) {
+#pragma unroll
+        for (int u = 0; u < 2; ++u) {
+            const int it = it0 + u, cl = it / CC_G, j = it - cl * CC_G;
+            pp[u] = c_lo + cl;
+            tt[u] = st * CC_G + j;
+            bb[u] = it < n_items ? H->perm[pp[u]] : -1;
+            if (bb[u] >= 0) epi_pre<KIND>(pre[u], E, D, W, SmemTab{H}, tt[u], pp[u], bb[u], lane);
+        }
+    };
+    setup(warp * 2);
     cluster_sync_all();                                              // every ring of the cluster is dead: it becomes the exchange buffer
     // exchange buffer in CTA j: [sender rank][tile 0 | 1][column of j's range][128 features] fp32
     const uint32_t slot_bytes = (uint32_t)CC_G * (uint32_t)cper * 512u;
@@ -681,13 +699,23 @@ k_gemm_cl(CcGemmGeo G, const uint8_t* __restrict__ act, CcEpi E, CcDims D, CcWor
                                  : "r"(tmem_base + ((uint32_t)(q * 32) << 16) + (uint32_t)j * 256 + (uint32_t)c0)
                                  : "memory");
                 tmem_ld_wait();
+                if (owner == rank) {                                 // my own columns: plain shared-memory stores
 #pragma unroll
-                for (int j = 0; j < CC_G; ++j)
+                    for (int j = 0; j < CC_G; ++j)
 #pragma unroll
-                    for (int i = 0; i < 8; ++i)
-                        asm volatile("st.shared::cluster.b32 [%0], %1;" ::"r"(dst_owner + ((uint32_t)j * (uint32_t)cper + (uint32_t)(cl + i)) * 512u),
-                                     "r"(v[j][i])
-                                     : "memory");
+                        for (int i = 0; i < 8; ++i)
+                            asm volatile("st.shared.b32 [%0], %1;" ::"r"(my_buf + (uint32_t)f * 4u + ((uint32_t)j * (uint32_t)cper + (uint32_t)(cl + i)) * 512u),
+                                         "r"(v[j][i])
+                                         : "memory");
+                } else {
+#pragma unroll
+                    for (int j = 0; j < CC_G; ++j)
+#pragma unroll
+                        for (int i = 0; i < 8; ++i)
+                            asm volatile("st.shared::cluster.b32 [%0], %1;" ::"r"(dst_owner + ((uint32_t)j * (uint32_t)cper + (uint32_t)(cl + i)) * 512u),
+                                         "r"(v[j][i])
+                                         : "memory");
+                }
             }
         }
     }
@@ -697,24 +725,16 @@ k_gemm_cl(CcGemmGeo G, const uint8_t* __restrict__ act, CcEpi E, CcDims D, CcWor
     if (threadIdx.x == 0) CC_TP(W, 2 + KIND, 4);
     // ---- my columns: add the S slots in rank order, fused epilogue; one warp per (column, tile) item ----
     {
-        constexpr int kWarps = kGemmThreads / 32;
-        const int c_lo = rank * cper, c_hi = min(n_pos, c_lo + cper);
-        const int n_items = max(0, c_hi - c_lo) * CC_G;
         const float* buf = reinterpret_cast<const float*>(stage0);
         const size_t slot_f = slot_bytes / 4;
         for (int it0 = warp * 2; it0 < n_items; it0 += kWarps * 2) {
-            EpiPre pre[2];
-            int pp[2], bb[2], tt[2];
+            if (it0 != warp * 2) setup(it0);
             float4 acc[2];
 #pragma unroll
             for (int u = 0; u < 2; ++u) {
                 const int it = it0 + u, cl = it / CC_G, j = it - cl * CC_G;
-                pp[u] = c_lo + cl;
-                tt[u] = st * CC_G + j;
-                bb[u] = it < n_items ? H->perm[pp[u]] : -1;
                 acc[u] = make_float4(0.f, 0.f, 0.f, 0.f);
                 if (bb[u] >= 0) {
-                    epi_pre<KIND>(pre[u], E, D, W, SmemTab{H}, tt[u], pp[u], bb[u], lane);
                     const float* src = buf + ((size_t)j * cper + cl) * 128 + 4 * lane;
                     for (int sdr = 0; sdr < S; ++sdr) {               // rank order: fixed
                         const float4 v = *reinterpret_cast<const float4*>(src + (size_t)sdr * slot_f);
