@@ -140,8 +140,9 @@ cc_status cc_ctx_set_operand_format(cc_ctx *ctx, int format);
 /* Activation planes of the four GEMM operands (x: QKV input, o: O input, y: gate/up input, a: down input) of
  * CC_OPERAND_F16 layers, chosen per step: a step of at most `rows` rows takes planes_upto_rows[4], a larger one
  * planes_above[4]; each entry 1 (one fp16 plane, 11 significand bits) or 2 (hi + lo fp16 planes, twice the tensor
- * work of that projection).  Steps of up to 64 rows are HBM-bound, so two planes cost them nothing: the default is
- * {2,2,2,2} up to 64 rows and {2,1,1,1} above (DESIGN.md "Precision" has the measured errors of every choice).  The choice depends on the step's
+ * work of that projection, and a larger activation slab per pipeline stage).  The default is {2,1,1,1} for every step
+ * size (rows = 64): the QKV input is the operand whose rounding shows (DESIGN.md "Precision" has the measured errors of
+ * every choice).  The choice depends on the step's
  * row count only, never on replica_assign, so outputs stay bit-identical across replica counts.  The environment
  * variable CC_PLANES="xoya,xoya[,rows]" sets the same at cc_ctx_create.  BF16X2 layers always use two planes. */
 cc_status cc_ctx_set_operand_planes(cc_ctx *ctx, int rows, const int *planes_upto_rows, const int *planes_above);

@@ -150,11 +150,12 @@ struct cc_ctx {
     bool cluster_gemm = true;                  // small steps run QKV / O / down as cluster split-K (CC_CLUSTER_GEMM=0: stream-K everywhere)
     int operand_format = CC_OPERAND_AUTO;      // layers created from now on (cc_ctx_set_operand_format)
     // activation planes of the four GEMM operands (x, o, y, a) of an fp16 layer, per step: steps of at most
-    // `planes_rows` rows are HBM-bound and take planes_small (two planes cost nothing there); larger steps take
-    // planes_large (cc_ctx_set_operand_planes)
+    // `planes_rows` rows take planes_small, larger ones planes_large (cc_ctx_set_operand_planes).
+    // Both default to {2, 1, 1, 1}: the QKV input is the operand whose rounding shows (measured), and a second plane
+    // of the others costs ring depth even where the tensor work is free (4 instead of 5 stages at batch 64: +4 us)
     int planes_rows = 64;
-    int planes_small[4] = {2, 2, 2, 2};
-    int planes_large[4] = {2, 1, 1, 1};        // measured: the QKV input is the operand whose rounding shows (short contexts)
+    int planes_small[4] = {2, 1, 1, 1};
+    int planes_large[4] = {2, 1, 1, 1};
     std::vector<Zombie> zombies;
 };
 

@@ -25,12 +25,14 @@
 //     the projection (RoPE + KV append | residual + norm statistics + operand packing | SwiGLU |
 //     residual + write-back in request order), so no separate reduce kernel runs between GEMMs.
 #include "cc_epilogue.cuh"
+#include <cstdio>
+#include <cstdlib>
 
 namespace {
 
 constexpr int kGemmThreads = 512;         // warp 0 producer, 1 MMA, 2..5 TMEM epilogue, 6..15 row tables; all 16 in the fixup
 constexpr int kHdrBytes = 8192;           // barriers + per-row tables in front of the stage ring
-constexpr int kMaxStages = 4;            // deeper rings do not stream faster (measured again in round 2: 5 stages no change, 6 stages slower at R = 4)
+constexpr int kMaxStages = 5;            // deeper rings do not stream faster (measured again in round 2: 5 stages no change, 6 stages slower at R = 4)
 constexpr int kGemmSmem = 225 * 1024;     // dynamic shared memory per CTA
 constexpr int kTmemCols = 512;
 constexpr uint32_t kWStage = CC_G * CC_A_TILE_BYTES;   // weight bytes per stage (32 KiB)
@@ -805,6 +807,7 @@ int cc_gemm_cl_cluster_size(int which, const CcGemmGeo& g, int n_sms) {
             cudaGetLastError();
             continue;
         }
+        if (getenv("CC_DEBUG_CLUSTERS")) fprintf(stderr, "k_gemm_cl<%d>: ST %d, cluster size %d -> %d active clusters\n", which, g.ST, S, n);
         if (n >= g.ST) best = S;
     }
     if (best && (long long)g.ST * best * 10 < (long long)g.P * 6) best = 0;
