@@ -659,15 +659,16 @@ k_gemm_cl(CcGemmGeo G, const uint8_t* __restrict__ act, CcEpi E, CcDims D, CcWor
         return;
     }
     // The first items of this warp's epilogue are known already (my columns, the row tables): issue their global loads
-    // (residual rows, gains, RoPE table, h1) now, so that their latency runs under the exchange.
-    constexpr int kWarps = kGemmThreads / 32;
+    // (residual rows, gains, RoPE table, h1) now, so that their latency runs under the exchange.  (kNI = 4 items per warp
+    // iteration measured 2.5 us SLOWER per step than 2; 1 the same as 2.)
+    constexpr int kWarps = kGemmThreads / 32, kNI = 2;
     const int c_lo = rank * cper, c_hi = min(n_pos, c_lo + cper);
     const int n_items = max(0, c_hi - c_lo) * CC_G;
-    EpiPre pre[2];
-    int pp[2], bb[2], tt[2];
+    EpiPre pre[kNI];
+    int pp[kNI], bb[kNI], tt[kNI];
     auto setup = [&](int it0) {
 #pragma unroll
-        for (int u = 0; u < 2; ++u) {
+        for (int u = 0; u < kNI; ++u) {
             const int it = it0 + u, cl = it / CC_G, j = it - cl * CC_G;
             pp[u] = c_lo + cl;
             tt[u] = st * CC_G + j;
@@ -675,7 +676,7 @@ k_gemm_cl(CcGemmGeo G, const uint8_t* __restrict__ act, CcEpi E, CcDims D, CcWor
             if (bb[u] >= 0) epi_pre<KIND>(pre[u], E, D, W, SmemTab{H}, tt[u], pp[u], bb[u], lane);
         }
     };
-    setup(warp * 2);
+    setup(warp * kNI);
     cluster_sync_all();                                              // every ring of the cluster is dead: it becomes the exchange buffer
     // exchange buffer in CTA j: [sender rank][tile 0 | 1][column of j's range][128 features] fp32
     const uint32_t slot_bytes = (uint32_t)CC_G * (uint32_t)cper * 512u;
@@ -729,11 +730,11 @@ k_gemm_cl(CcGemmGeo G, const uint8_t* __restrict__ act, CcEpi E, CcDims D, CcWor
     {
         const float* buf = reinterpret_cast<const float*>(stage0);
         const size_t slot_f = slot_bytes / 4;
-        for (int it0 = warp * 2; it0 < n_items; it0 += kWarps * 2) {
-            if (it0 != warp * 2) setup(it0);
-            float4 acc[2];
+        for (int it0 = warp * kNI; it0 < n_items; it0 += kWarps * kNI) {
+            if (it0 != warp * kNI) setup(it0);
+            float4 acc[kNI];
 #pragma unroll
-            for (int u = 0; u < 2; ++u) {
+            for (int u = 0; u < kNI; ++u) {
                 const int it = it0 + u, cl = it / CC_G, j = it - cl * CC_G;
                 acc[u] = make_float4(0.f, 0.f, 0.f, 0.f);
                 if (bb[u] >= 0) {
@@ -745,7 +746,7 @@ k_gemm_cl(CcGemmGeo G, const uint8_t* __restrict__ act, CcEpi E, CcDims D, CcWor
                 }
             }
 #pragma unroll
-            for (int u = 0; u < 2; ++u)
+            for (int u = 0; u < kNI; ++u)
                 if (bb[u] >= 0) epi_fin<KIND>(pre[u], E, D, W, SmemTab{H}, tt[u], pp[u], bb[u], acc[u], lane);
         }
     }
@@ -807,7 +808,6 @@ int cc_gemm_cl_cluster_size(int which, const CcGemmGeo& g, int n_sms) {
             cudaGetLastError();
             continue;
         }
-        if (getenv("CC_DEBUG_CLUSTERS")) fprintf(stderr, "k_gemm_cl<%d>: ST %d, cluster size %d -> %d active clusters\n", which, g.ST, S, n);
         if (n >= g.ST) best = S;
     }
     if (best && (long long)g.ST * best * 10 < (long long)g.P * 6) best = 0;
