@@ -472,10 +472,10 @@ cc_status cc_create_layer(cc_ctx* ctx, const cc_layer_desc* desc, const cc_layer
     D.off_g2 = blob.take((size_t)D.d * 2);
     L->blob_bytes = blob.take(0);
     if (ctx->cluster_gemm) {
-        D.qkv.S = cc_gemm_cl_cluster_size(0, D.qkv, ctx->n_sms);
-        D.o.S = cc_gemm_cl_cluster_size(1, D.o, ctx->n_sms);
-        D.gu.S = cc_gemm_cl_cluster_size(2, D.gu, ctx->n_sms);
-        D.dn.S = cc_gemm_cl_cluster_size(3, D.dn, ctx->n_sms);
+        cc_gemm_cl_geometry(0, D.qkv, ctx->n_sms);
+        cc_gemm_cl_geometry(1, D.o, ctx->n_sms);
+        cc_gemm_cl_geometry(2, D.gu, ctx->n_sms);
+        cc_gemm_cl_geometry(3, D.dn, ctx->n_sms);
     }
     if (D.qkv.ST > CC_FLAG_STRIDE || D.o.ST > CC_FLAG_STRIDE || D.gu.ST > CC_FLAG_STRIDE || D.dn.ST > CC_FLAG_STRIDE ||
         D.Mpart > CC_MAX_MPAD) {
@@ -1015,7 +1015,7 @@ cc_status cc_layer_gemm_grids(const cc_layer* L, int* ctas, int* cluster) {
     const CcGemmGeo* g[4] = {&L->D.qkv, &L->D.o, &L->D.gu, &L->D.dn};
     for (int i = 0; i < 4; ++i) {
         cluster[i] = g[i]->S;
-        ctas[i] = g[i]->S ? g[i]->ST * g[i]->S : g[i]->P;
+        ctas[i] = g[i]->S ? g[i]->ST * CC_G / g[i]->cl_tiles * g[i]->S : g[i]->P;
     }
     return CC_OK;
 }

@@ -64,6 +64,8 @@ struct CcGemmGeo {
     int KB;       // k-blocks of 64 per tile
     int P;        // CTAs (ranges)
     int S;        // cluster size of the small-step cluster split-K kernel (k_gemm_cl), 0 = stream-K only
+    int cl_tiles; // tiles of 128 output features per cluster of that kernel: 2 (a super tile) or 1
+    int pad_;
     size_t w_off; // byte offset of the packed matrix inside a replica blob
 };
 // Range of CTA i: units [cc_range_begin(i), cc_range_begin(i+1)).

@@ -38,8 +38,8 @@ constexpr int kTmemCols = 512;
 constexpr uint32_t kWStage = CC_G * CC_A_TILE_BYTES;   // weight bytes per stage (32 KiB)
 
 struct GemmSmemHdr {                      // lives at the start of dynamic smem
-    uint64_t full[kMaxStages];
-    uint64_t empty[kMaxStages];
+    uint64_t full[12];                    // kMaxStages (k_gemm, two-tile k_gemm_cl) or kClMaxStages (one-tile k_gemm_cl) in use
+    uint64_t empty[12];
     uint64_t tmem_full[2];
     uint64_t tmem_empty[2];
     uint32_t tmem_base;
@@ -457,8 +457,9 @@ k_gemm(CcGemmGeo G, const uint8_t* __restrict__ act, float* __restrict__ part, i
 // this kernel from the step's ROW COUNT only, so the choice cannot differ between replica counts either.
 constexpr int kClRows = 192;                  // grouped rows (n_pos) the two accumulators and the exchange buffers are sized for
 constexpr int kClMaxS = 8;
+constexpr int kClMaxStages = 8;              // ring depth of the one-tile variant (24 KiB stages at batch 64; 12 measured slower)
 
-template <int KIND>
+template <int KIND, int TILES>
 __global__ void __launch_bounds__(kGemmThreads, 1)
 k_gemm_cl(CcGemmGeo G, const uint8_t* __restrict__ act, CcEpi E, CcDims D, CcWork W, const CcLayerTable* __restrict__ tab, int S) {
     const int planes = D.pl[KIND];
@@ -468,11 +469,16 @@ k_gemm_cl(CcGemmGeo G, const uint8_t* __restrict__ act, CcEpi E, CcDims D, CcWor
     GemmSmemHdr* H = reinterpret_cast<GemmSmemHdr*>(smem_raw);
     const int warp = uniform((int)(threadIdx.x >> 5)), lane = threadIdx.x & 31;
     const int rank = (int)cluster_ctarank();
-    const int st = (int)blockIdx.x / S;                              // the cluster's super tile
+    // TILES = 2: the cluster owns a super tile (two adjacent tiles, one 32 KiB copy per k-block); TILES = 1: ONE tile of
+    // 128 output features (a 16 KiB atom per k-block, every other atom of its super tile): twice the clusters, half the
+    // exchange, for the projections whose super tiles are too few to fill the GPU with co-resident clusters (O, down)
+    const int unit = (int)blockIdx.x / S;                            // the cluster's super tile (TILES = 2) or tile (TILES = 1)
+    const int st = TILES == 2 ? unit : unit / CC_G, tile0 = TILES == 2 ? unit * CC_G : unit;
+    constexpr uint32_t kWBytes = (uint32_t)TILES * CC_A_TILE_BYTES;   // weight bytes per stage
 
     if (threadIdx.x == 0) CC_TP(W, 2 + KIND, 0);
     if (threadIdx.x == 0) {
-        for (int i = 0; i < kMaxStages; ++i) {
+        for (int i = 0; i < kClMaxStages; ++i) {
             mbar_init(&H->full[i], 1);
             mbar_init(&H->empty[i], 1);
         }
@@ -526,10 +532,10 @@ k_gemm_cl(CcGemmGeo G, const uint8_t* __restrict__ act, CcEpi E, CcDims D, CcWor
     }
     nmax = uniform(nmax);
     n_pos = uniform(n_pos);
-    const uint32_t stage_bytes = kWStage + (uint32_t)planes * (uint32_t)nmax * 128u;
+    const uint32_t stage_bytes = kWBytes + (uint32_t)planes * (uint32_t)nmax * 128u;
     uint8_t* stage0 = smem_raw + kHdrBytes;
     int n_stages = (kGemmSmem - kHdrBytes) / (int)stage_bytes;
-    if (n_stages > kMaxStages) n_stages = kMaxStages;
+    if (n_stages > (TILES == 2 ? kMaxStages : kClMaxStages)) n_stages = TILES == 2 ? kMaxStages : kClMaxStages;
     const int kb0 = (int)((long long)rank * G.KB / S), kb1 = (int)((long long)(rank + 1) * G.KB / S);
     const uint32_t tmem_base = uniform(H->tmem_base);
     // columns (grouped rows) CTA j owns in the reduction: [j * cper, (j + 1) * cper)
@@ -552,8 +558,9 @@ k_gemm_cl(CcGemmGeo G, const uint8_t* __restrict__ act, CcEpi E, CcDims D, CcWor
                     const int cnt = uniform(H->cnt[r]);
                     if (cnt == 0) continue;
                     const uint32_t nb = (uint32_t)((cnt + 15) & ~15) * 128u * (uint32_t)planes;
-                    const uint32_t tx = kWStage + nb;
-                    const uint8_t* wsrc = uniform(H->blob[r]) + G.w_off + ((size_t)st * G.KB + kb0) * kWStage;
+                    const uint32_t tx = kWBytes + nb;
+                    const uint8_t* wsrc = uniform(H->blob[r]) + G.w_off + ((size_t)st * G.KB + kb0) * kWStage +
+                                          (TILES == 2 ? 0 : (size_t)(unit % CC_G) * CC_A_TILE_BYTES);
                     const uint8_t* asrc = act + (size_t)(uniform(H->goff[r]) >> 3) * planes * 1024 + (size_t)kb0 * kb_stride;
                     for (int kb = kb0; kb < kb1; ++kb, ++idx) {
                         if (mode == 0 && idx >= n_pre) return;
@@ -562,9 +569,9 @@ k_gemm_cl(CcGemmGeo G, const uint8_t* __restrict__ act, CcEpi E, CcDims D, CcWor
                         if (elect_one()) {
                             if (mode == 0 || !pre) {
                                 mbar_expect_tx(&H->full[stage], tx);
-                                bulk_g2s_hint(sW, wsrc, kWStage, &H->full[stage], pol_w);
+                                bulk_g2s_hint(sW, wsrc, kWBytes, &H->full[stage], pol_w);
                             }
-                            if (mode == 1) bulk_g2s_hint(sW + kWStage, asrc, nb, &H->full[stage], pol_a);
+                            if (mode == 1) bulk_g2s_hint(sW + kWBytes, asrc, nb, &H->full[stage], pol_a);
                         }
                         wsrc += kWStage;
                         asrc += kb_stride;
@@ -588,7 +595,7 @@ k_gemm_cl(CcGemmGeo G, const uint8_t* __restrict__ act, CcEpi E, CcDims D, CcWor
             const uint32_t a_hi = (uint32_t)(umma_desc_sw128(0) >> 32);
             const uint32_t b_hi = (uint32_t)(umma_desc_sw128(0, (uint32_t)planes * 1024u) >> 32);
             const uint32_t desc_lo0 = (uint32_t)umma_desc_sw128(smem_u32(stage0));
-            const uint32_t dstage = stage_bytes >> 4, dact = kWStage >> 4;
+            const uint32_t dstage = stage_bytes >> 4, dact = kWBytes >> 4;
             uint32_t da = desc_lo0;
             for (int r = 0; r < CC_MAXR; ++r) {
                 const int cnt = uniform(H->cnt[r]);
@@ -601,7 +608,7 @@ k_gemm_cl(CcGemmGeo G, const uint8_t* __restrict__ act, CcEpi E, CcDims D, CcWor
                     if (elect_one()) {
                         const uint32_t db = da + dact;
 #pragma unroll
-                        for (int j = 0; j < CC_G; ++j) {
+                        for (int j = 0; j < TILES; ++j) {
                             const uint32_t d_tmem = tmem_base + (uint32_t)j * 256 + col0;
                             const uint32_t daj = da + (uint32_t)j * (CC_A_TILE_BYTES >> 4);
 #pragma unroll
@@ -663,15 +670,15 @@ k_gemm_cl(CcGemmGeo G, const uint8_t* __restrict__ act, CcEpi E, CcDims D, CcWor
     // iteration measured 2.5 us SLOWER per step than 2; 1 the same as 2.)
     constexpr int kWarps = kGemmThreads / 32, kNI = 2;
     const int c_lo = rank * cper, c_hi = min(n_pos, c_lo + cper);
-    const int n_items = max(0, c_hi - c_lo) * CC_G;
+    const int n_items = max(0, c_hi - c_lo) * TILES;
     EpiPre pre[kNI];
     int pp[kNI], bb[kNI], tt[kNI];
     auto setup = [&](int it0) {
 #pragma unroll
         for (int u = 0; u < kNI; ++u) {
-            const int it = it0 + u, cl = it / CC_G, j = it - cl * CC_G;
+            const int it = it0 + u, cl = it / TILES, j = it - cl * TILES;
             pp[u] = c_lo + cl;
-            tt[u] = st * CC_G + j;
+            tt[u] = tile0 + j;
             bb[u] = it < n_items ? H->perm[pp[u]] : -1;
             if (bb[u] >= 0) epi_pre<KIND>(pre[u], E, D, W, SmemTab{H}, tt[u], pp[u], bb[u], lane);
         }
@@ -679,7 +686,7 @@ k_gemm_cl(CcGemmGeo G, const uint8_t* __restrict__ act, CcEpi E, CcDims D, CcWor
     setup(warp * kNI);
     cluster_sync_all();                                              // every ring of the cluster is dead: it becomes the exchange buffer
     // exchange buffer in CTA j: [sender rank][tile 0 | 1][column of j's range][128 features] fp32
-    const uint32_t slot_bytes = (uint32_t)CC_G * (uint32_t)cper * 512u;
+    const uint32_t slot_bytes = (uint32_t)TILES * (uint32_t)cper * 512u;
     if (warp >= 2 && warp < 14) {                                    // three warps per TMEM lane quarter share the chunks
         const int q = warp & 3, f = q * 32 + lane, grp = (warp - 2) >> 2;   // lane quarter; output feature within the tile
         const uint32_t my_buf = smem_u32(stage0) + (uint32_t)rank * slot_bytes;
@@ -693,9 +700,9 @@ k_gemm_cl(CcGemmGeo G, const uint8_t* __restrict__ act, CcEpi E, CcDims D, CcWor
                 const int c0 = owner * cper + cl;
                 if (c0 >= n_pos) break;
                 if (chunk++ % 3 != grp) continue;
-                uint32_t v[CC_G][8];
+                uint32_t v[TILES][8];
 #pragma unroll
-                for (int j = 0; j < CC_G; ++j)
+                for (int j = 0; j < TILES; ++j)
                     asm volatile("tcgen05.ld.sync.aligned.32x32b.x8.b32 {%0, %1, %2, %3, %4, %5, %6, %7}, [%8];"
                                  : "=r"(v[j][0]), "=r"(v[j][1]), "=r"(v[j][2]), "=r"(v[j][3]), "=r"(v[j][4]), "=r"(v[j][5]), "=r"(v[j][6]),
                                    "=r"(v[j][7])
@@ -704,7 +711,7 @@ k_gemm_cl(CcGemmGeo G, const uint8_t* __restrict__ act, CcEpi E, CcDims D, CcWor
                 tmem_ld_wait();
                 if (owner == rank) {                                 // my own columns: plain shared-memory stores
 #pragma unroll
-                    for (int j = 0; j < CC_G; ++j)
+                    for (int j = 0; j < TILES; ++j)
 #pragma unroll
                         for (int i = 0; i < 8; ++i)
                             asm volatile("st.shared.b32 [%0], %1;" ::"r"(my_buf + (uint32_t)f * 4u + ((uint32_t)j * (uint32_t)cper + (uint32_t)(cl + i)) * 512u),
@@ -712,7 +719,7 @@ k_gemm_cl(CcGemmGeo G, const uint8_t* __restrict__ act, CcEpi E, CcDims D, CcWor
                                          : "memory");
                 } else {
 #pragma unroll
-                    for (int j = 0; j < CC_G; ++j)
+                    for (int j = 0; j < TILES; ++j)
 #pragma unroll
                         for (int i = 0; i < 8; ++i)
                             asm volatile("st.shared::cluster.b32 [%0], %1;" ::"r"(dst_owner + ((uint32_t)j * (uint32_t)cper + (uint32_t)(cl + i)) * 512u),
@@ -735,7 +742,7 @@ k_gemm_cl(CcGemmGeo G, const uint8_t* __restrict__ act, CcEpi E, CcDims D, CcWor
             float4 acc[kNI];
 #pragma unroll
             for (int u = 0; u < kNI; ++u) {
-                const int it = it0 + u, cl = it / CC_G, j = it - cl * CC_G;
+                const int it = it0 + u, cl = it / TILES, j = it - cl * TILES;
                 acc[u] = make_float4(0.f, 0.f, 0.f, 0.f);
                 if (bb[u] >= 0) {
                     const float* src = buf + ((size_t)j * cper + cl) * 128 + 4 * lane;
@@ -758,27 +765,30 @@ k_gemm_cl(CcGemmGeo G, const uint8_t* __restrict__ act, CcEpi E, CcDims D, CcWor
 
 }  // namespace
 
+// ---- cluster split-K variant (k_gemm_cl): the four projections of small steps --------------------------------------
+typedef void (*ClKernel)(CcGemmGeo, const uint8_t*, CcEpi, CcDims, CcWork, const CcLayerTable*, int);
+static ClKernel cl_kernel(int which, int tiles) {
+    if (tiles == 2)
+        return which == 0 ? (ClKernel)k_gemm_cl<EPI_QKV, 2> : which == 1 ? (ClKernel)k_gemm_cl<EPI_O, 2>
+               : which == 2 ? (ClKernel)k_gemm_cl<EPI_GU, 2> : (ClKernel)k_gemm_cl<EPI_DN, 2>;
+    return which == 0 ? (ClKernel)k_gemm_cl<EPI_QKV, 1> : which == 1 ? (ClKernel)k_gemm_cl<EPI_O, 1>
+           : which == 2 ? (ClKernel)k_gemm_cl<EPI_GU, 1> : (ClKernel)k_gemm_cl<EPI_DN, 1>;
+}
+
 cudaError_t cc_gemm_configure() {
     cudaError_t e = cudaFuncSetAttribute(k_gemm<EPI_QKV>, cudaFuncAttributeMaxDynamicSharedMemorySize, kGemmSmem);
     if (e == cudaSuccess) e = cudaFuncSetAttribute(k_gemm<EPI_O>, cudaFuncAttributeMaxDynamicSharedMemorySize, kGemmSmem);
     if (e == cudaSuccess) e = cudaFuncSetAttribute(k_gemm<EPI_GU>, cudaFuncAttributeMaxDynamicSharedMemorySize, kGemmSmem);
     if (e == cudaSuccess) e = cudaFuncSetAttribute(k_gemm<EPI_DN>, cudaFuncAttributeMaxDynamicSharedMemorySize, kGemmSmem);
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_gemm_cl<EPI_QKV>, cudaFuncAttributeMaxDynamicSharedMemorySize, kGemmSmem);
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_gemm_cl<EPI_O>, cudaFuncAttributeMaxDynamicSharedMemorySize, kGemmSmem);
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_gemm_cl<EPI_DN>, cudaFuncAttributeMaxDynamicSharedMemorySize, kGemmSmem);
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_gemm_cl<EPI_GU>, cudaFuncAttributeMaxDynamicSharedMemorySize, kGemmSmem);
+    for (int which = 0; which < 4 && e == cudaSuccess; ++which)
+        for (int tiles = 1; tiles <= 2 && e == cudaSuccess; ++tiles)
+            e = cudaFuncSetAttribute((const void*)cl_kernel(which, tiles), cudaFuncAttributeMaxDynamicSharedMemorySize, kGemmSmem);
     return e;
 }
 
-// ---- cluster split-K variant (k_gemm_cl): small steps of the QKV, O and down projections --------------------------
-typedef void (*ClKernel)(CcGemmGeo, const uint8_t*, CcEpi, CcDims, CcWork, const CcLayerTable*, int);
-static ClKernel cl_kernel(int which) {
-    return which == 0 ? (ClKernel)k_gemm_cl<EPI_QKV> : which == 1 ? (ClKernel)k_gemm_cl<EPI_O>
-           : which == 2 ? (ClKernel)k_gemm_cl<EPI_GU> : (ClKernel)k_gemm_cl<EPI_DN>;
-}
-static void cl_config(cudaLaunchConfig_t& cfg, cudaLaunchAttribute* attr, int ST, int S, cudaStream_t st, bool pdl) {
+static void cl_config(cudaLaunchConfig_t& cfg, cudaLaunchAttribute* attr, int n_clusters, int S, cudaStream_t st, bool pdl) {
     cfg = cudaLaunchConfig_t{};
-    cfg.gridDim = dim3((unsigned)(ST * S));
+    cfg.gridDim = dim3((unsigned)(n_clusters * S));
     cfg.blockDim = dim3(kGemmThreads);
     cfg.dynamicSmemBytes = kGemmSmem;
     cfg.stream = st;
@@ -791,27 +801,35 @@ static void cl_config(cudaLaunchConfig_t& cfg, cudaLaunchAttribute* attr, int ST
     cfg.attrs = attr;
     cfg.numAttrs = pdl ? 2 : 1;
 }
-// Largest cluster size S <= 8 for which all ST clusters of S CTAs are co-resident (one wave) and every CTA gets at
-// least one k-block; 0 = the projection stays on the stream-K kernel -- also when the clusters would use fewer than 60 %
-// of the CTAs stream-K would (too few SMs pulling on HBM).  A function of the layer shape and the device.  At cfg2 on a
-// B200: QKV 24 x 5 = 120 CTAs, O and down 16 x 6 = 96, gate/up 112 x 1 = 112 (no split at all: one CTA streams the whole
-// K of its super tile and runs the epilogue straight from its accumulators).
-int cc_gemm_cl_cluster_size(int which, const CcGemmGeo& g, int n_sms) {
-    int best = 0;
-    for (int S = 1; S <= kClMaxS; ++S) {
-        if (S > g.KB || g.ST * S > n_sms) continue;
-        cudaLaunchConfig_t cfg;
-        cudaLaunchAttribute attr[2];
-        cl_config(cfg, attr, g.ST, S, nullptr, false);
-        int n = 0;
-        if (cudaOccupancyMaxActiveClusters(&n, (void*)cl_kernel(which), &cfg) != cudaSuccess) {
-            cudaGetLastError();
-            continue;
+// Cluster geometry of projection `which` for small steps: g.cl_tiles in {1, 2} tiles per cluster and the largest cluster
+// size g.S <= 8 for which all clusters are co-resident (one wave) and every CTA gets at least one k-block -- whichever of
+// the two puts more CTAs on the GPU (two tiles on a tie: one 32 KiB copy per k-block).  g.S = 0 keeps the projection on
+// the stream-K kernel: no co-resident geometry, or one that would use fewer than 60 % of the CTAs stream-K would.  A
+// function of the layer shape and the device.
+void cc_gemm_cl_geometry(int which, CcGemmGeo& g, int n_sms) {
+    g.S = 0;
+    g.cl_tiles = 2;
+    int best_ctas = 0;
+    for (int tiles = 2; tiles >= 1; --tiles) {
+        const int n_clusters = g.ST * CC_G / tiles;
+        for (int S = 1; S <= kClMaxS; ++S) {
+            if (S > g.KB || n_clusters * S > n_sms) continue;
+            cudaLaunchConfig_t cfg;
+            cudaLaunchAttribute attr[2];
+            cl_config(cfg, attr, n_clusters, S, nullptr, false);
+            int n = 0;
+            if (cudaOccupancyMaxActiveClusters(&n, (void*)cl_kernel(which, tiles), &cfg) != cudaSuccess) {
+                cudaGetLastError();
+                continue;
+            }
+            if (n >= n_clusters && n_clusters * S > best_ctas) {
+                best_ctas = n_clusters * S;
+                g.S = S;
+                g.cl_tiles = tiles;
+            }
         }
-        if (n >= g.ST) best = S;
     }
-    if (best && (long long)g.ST * best * 10 < (long long)g.P * 6) best = 0;
-    return best;
+    if ((long long)best_ctas * 10 < (long long)g.P * 6) g.S = 0;
 }
 int cc_gemm_cl_max_rows() { return kClRows; }
 
@@ -822,8 +840,8 @@ cudaError_t cc_launch_gemm_cl(int which, const CcDims& D, const CcLayerTable* ta
     const uint8_t* act = which == 0 ? W.x_act : which == 1 ? W.o_act : which == 2 ? W.y_act : W.a_act;
     cudaLaunchConfig_t cfg;
     cudaLaunchAttribute attr[2];
-    cl_config(cfg, attr, g.ST, g.S, L.st, L.pdl);
-    return cudaLaunchKernelEx(&cfg, cl_kernel(which), g, act, E, D, W, tab, g.S);
+    cl_config(cfg, attr, g.ST * CC_G / g.cl_tiles, g.S, L.st, L.pdl);
+    return cudaLaunchKernelEx(&cfg, cl_kernel(which, g.cl_tiles), g, act, E, D, W, tab, g.S);
 }
 
 // which: 0 = QKV, 1 = O, 2 = gate/up, 3 = down

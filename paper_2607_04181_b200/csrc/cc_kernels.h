@@ -111,7 +111,7 @@ cudaError_t cc_launch_gemm(int which, const CcDims& D, const CcLayerTable* tab, 
 // small steps (at most cc_gemm_cl_max_rows() grouped rows) of QKV / O / down as a cluster split-K (cc_gemm.cu: k_gemm_cl)
 cudaError_t cc_launch_gemm_cl(int which, const CcDims& D, const CcLayerTable* tab, const CcWork& W, const int* seq_lens,
                               const int* assign, int batch, const CcKv& kv, __nv_bfloat16* hidden, const CcLaunch& L);
-int cc_gemm_cl_cluster_size(int which, const CcGemmGeo& g, int n_sms);
+void cc_gemm_cl_geometry(int which, CcGemmGeo& g, int n_sms);   // sets g.S and g.cl_tiles
 int cc_gemm_cl_max_rows();
 cudaError_t cc_launch_attention(const int* seq_lens, const CcKv& kv, const CcDims& D, const CcLayerTable* tab,
                                 const CcWork& W, const CcLaunch& L, const int* rowmap = nullptr);

@@ -30,7 +30,7 @@ __device__ __forceinline__ float block_sum(float v, float* red) {
 }
 
 // ---------------------------------------------------------------------------------------------
-// a0 + a1 in one kernel, one block per request row.
+// a0 + a1 in one kernel, one block per request row (+ two blocks for the tables).
 // a0: grouping.  Every block repeats it (256 rows: a few ballots), thread b owns row b.  Stable partition
 // by replica, groups start at multiples of 16 rows; page prefix of the attention work
 // split.  Block 0 publishes the tables; each block learns the grouped position of its own row.
@@ -51,8 +51,12 @@ __global__ void __launch_bounds__(kNormThreads) k_prologue(const int* __restrict
     __shared__ signed char s_rep[256];       // replica that serves row b (scan block only)
     __shared__ float red[kNormThreads / 32];
     const int b = threadIdx.x, warp = b >> 5, lane = b & 31;
-    const bool pub = blockIdx.x == 0;      // this block writes the tables
+    // grid = batch + 2: block b < batch normalises row b; the two extra blocks only publish the tables and look for the
+    // rows that share a request, so that no row's block carries that work on top of its own (it was the slowest block
+    // of the kernel by ~3 us, and the QKV GEMM waits for the last one)
+    const bool pub = blockIdx.x == gridDim.x - 2;    // this block writes the tables
     const bool scan = blockIdx.x == gridDim.x - 1;   // this one finds the rows that share a request (prompt chunks)
+    const bool has_row = (int)blockIdx.x < batch;
     if (b == 0) CC_TP(W, 0, 0);
     pdl_wait();
     if (b == 0) CC_TP(W, 0, 1);
@@ -66,7 +70,7 @@ __global__ void __launch_bounds__(kNormThreads) k_prologue(const int* __restrict
 #pragma unroll
         for (int j = 0; j < kNormVec; ++j) {
             const int c = threadIdx.x + j * kNormThreads;
-            v[j] = c < nchunk ? row[c] : make_uint4(0, 0, 0, 0);
+            v[j] = (has_row && c < nchunk) ? row[c] : make_uint4(0, 0, 0, 0);
         }
     }
     int rep = -1, pos = -1;
@@ -250,7 +254,7 @@ __global__ void __launch_bounds__(256) k_tap(const void* __restrict__ src, int w
 cudaError_t cc_launch_prologue(const int* assign, const int* seq_lens, const int* block_table, int batch,
                                const __nv_bfloat16* hidden, const CcDims& D, const CcLayerTable* tab, const CcWork& W,
                                const CcLaunch& L, const CcStageOut& so) {
-    return cc_launch_kernel(k_prologue, dim3(batch), dim3(kNormThreads), 0, L, assign, seq_lens, block_table, batch, hidden, D, tab,
+    return cc_launch_kernel(k_prologue, dim3(batch + 2), dim3(kNormThreads), 0, L, assign, seq_lens, block_table, batch, hidden, D, tab,
                             W, so);
 }
 cudaError_t cc_launch_tap(const void* src, int which, int planes, int dim, const CcDims& D, const CcWork& W,
