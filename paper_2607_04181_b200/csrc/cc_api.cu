@@ -156,6 +156,10 @@ struct cc_ctx {
     int planes_rows = 64;
     int planes_small[4] = {2, 1, 1, 1};
     int planes_large[4] = {2, 1, 1, 1};
+    // L2 weight prefetch of the small-step cluster GEMMs (CcDims::pf_next / pf_self; env CC_PREFETCH="next,self" for
+    // experiments).  Measured at cfg2: 3 / 4 stages take 2-3 us off the step at every replica count; 6 / 8
+    // gain nothing, 12 / 16 and more LOSE 5-10 us
+    int pf_next = 3, pf_self = 4;
     std::vector<Zombie> zombies;
 };
 
@@ -265,6 +269,8 @@ cc_status cc_ctx_create(int device, cc_ctx** out) {
     if (env && env[0] == '0') ctx->pdl = false;
     env = getenv("CC_CLUSTER_GEMM");
     if (env && env[0] == '0') ctx->cluster_gemm = false;
+    env = getenv("CC_PREFETCH");                // "next,self": weight stages prefetched into L2 across / inside the small-step GEMMs
+    if (env) sscanf(env, "%d,%d", &ctx->pf_next, &ctx->pf_self);
     env = getenv("CC_PLANES");                  // "xoya,xoya[,rows]": planes of small and large steps, e.g. 2222,1212,64
     if (env && std::strlen(env) >= 9 && env[4] == ',') {
         bool ok = true;
@@ -456,6 +462,7 @@ cc_status cc_create_layer(cc_ctx* ctx, const cc_layer_desc* desc, const cc_layer
     const bool big = d.max_batch > 256;                       // the layer also takes steps of more than 256 rows
     D.fmt = ctx->operand_format == CC_OPERAND_BF16X2 ? CC_FMT_BF16X2 : CC_FMT_F16;   // AUTO: fp16 unless a weight overflows it (below)
     for (int i = 0; i < 4; ++i) D.pl[i] = 2;                                           // per step: step_dims()
+    D.pf_next = D.pf_self = 0;
     D.eps = d.rms_eps;
     D.qk_scale_log2 = (float)(1.4426950408889634 / std::sqrt((double)D.Dh));
     // blob layout: [QKV tiles][O tiles][gate/up tiles][down tiles][g1][g2]
@@ -885,7 +892,7 @@ cudaError_t enqueue_forward(cc_layer* L, __nv_bfloat16* hidden, const CcKv& kv, 
                             int batch, cudaStream_t st, cudaEvent_t* ev = nullptr, __nv_bfloat16* hidden_host_alias = nullptr) {
     if (batch > 256) return enqueue_big(L, hidden, kv, seq_lens, assign, batch, st, ev);
     cc_ctx* ctx = L->ctx;
-    const CcDims D = step_dims(L, batch);
+    CcDims D = step_dims(L, batch);
     const CcWork& W = L->W;
     const CcLayerTable* tab = ctx->table_dev + L->row;
     CcLaunch Ln{st, ctx->n_sms, ctx->pdl && ev == nullptr};
@@ -904,6 +911,8 @@ cudaError_t enqueue_forward(cc_layer* L, __nv_bfloat16* hidden, const CcKv& kv, 
     // the three short projections of a SMALL step run as cluster split-K (k_gemm_cl): decided by the row count alone --
     // the worst-case grouped size of `batch` rows over CC_MAX_REPLICAS groups -- so it cannot differ between replica counts
     const bool cl = (batch + 15) / 16 * 16 + 16 * (CC_MAX_REPLICAS - 1) <= cc_gemm_cl_max_rows();
+    D.pf_next = cl ? ctx->pf_next : 0;
+    D.pf_self = cl ? ctx->pf_self : 0;
     for (int stage = 0; stage < kForwardLaunches && e == cudaSuccess; ++stage) {
         if (ev && (e = cudaEventRecord(ev[stage], st)) != cudaSuccess) break;
         switch (stage) {

@@ -182,6 +182,14 @@ k_attn(const int* __restrict__ seq_lens, CcKv kv, CcDims D, CcWork W, const CcLa
             p = r0 + q1;
             ++b;
         }
+        // my pages are on their way; the consumers still work on them: the first weight stages of the O projection's CTAs go
+        // to L2 meanwhile (small steps on the cluster GEMMs only: D.pf_next)
+        if (D.pf_next > 0) {
+            const uint8_t* blobs[CC_MAXR];
+#pragma unroll
+            for (int r = 0; r < CC_MAXR; ++r) blobs[r] = tab->rep[r].blob;
+            cc_prefetch_weights(D.o, blobs, W.sched->cnt, (int)blockIdx.x, (int)gridDim.x, 0, D.pf_next, lane);
+        }
         // end marker for the consumers
         if (!waited) pdl_wait();
         mbar_wait(&empty[stage], ph ^ 1);

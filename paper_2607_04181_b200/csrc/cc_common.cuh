@@ -104,6 +104,9 @@ struct CcDims {
     int max_batch, max_blocks, max_position;
     float eps;
     float qk_scale_log2;        // log2(e) / sqrt(Dh)
+    int pf_next, pf_self;       // small steps on the cluster GEMMs: weight stages a kernel prefetches into L2 for every CTA of the
+                                // NEXT projection once its own copies are issued / of its own range while it waits for its
+                                // predecessor (cc_prefetch_weights); 0 = off; set per step by the host
     CcGemmGeo qkv, o, gu, dn;   // the four projections
     size_t off_g1, off_g2;      // gains inside the blob (bf16 [d])
 };
@@ -309,6 +312,36 @@ __device__ __forceinline__ void tma_load_2d_hint(uint32_t dst_smem, const void* 
             "r"(dst_smem),
         "l"(tmap), "r"(c0), "r"(c1), "r"(bar_smem), "l"(policy)
         : "memory");
+}
+// L2 prefetch of a contiguous global range (16-byte granules): no shared memory, no barrier, fire and forget.
+__device__ __forceinline__ void bulk_prefetch_l2(const void* src_gmem, uint32_t bytes) {
+    asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(src_gmem), "r"(bytes) : "memory");
+}
+// CTA c' = (cluster unit, rank) of the small-step cluster GEMM with geometry N (k_gemm_cl) copies, for every replica that has
+// rows, the weight stages of k-blocks [rank KB / S, (rank + 1) KB / S) of its (super) tile, in that order.  This prefetches
+// stages [skip, skip + n) of that sequence into L2 for the CTAs c' = c, c + step, ... of N.  Called by one whole warp: the
+// kernel BEFORE N calls it once its own copies are issued (its exchange and epilogue would leave HBM idle otherwise, and
+// N's CTAs cannot start on an SM whose shared memory the predecessor still holds), N itself while it waits for that kernel.
+__device__ __forceinline__ void cc_prefetch_weights(const CcGemmGeo& N, const uint8_t* const* blob, const int* cnt, int c,
+                                                    int step, int skip, int n, int lane) {
+    if (N.S <= 0 || n <= 0) return;
+    const int n_cta = N.ST * CC_G / N.cl_tiles * N.S;
+    const uint32_t wbytes = (uint32_t)N.cl_tiles * CC_A_TILE_BYTES;
+    const size_t wstage = (size_t)CC_G * CC_A_TILE_BYTES;
+    for (int cc = c; cc < n_cta; cc += step) {
+        const int unit = cc / N.S, rank = cc % N.S;
+        const int st = N.cl_tiles == 2 ? unit : unit / CC_G;
+        const int kb0 = (int)((long long)rank * N.KB / N.S), len = (int)((long long)(rank + 1) * N.KB / N.S) - kb0;
+        const size_t off = N.w_off + ((size_t)st * N.KB + kb0) * wstage + (N.cl_tiles == 2 ? 0 : (size_t)(unit % CC_G) * CC_A_TILE_BYTES);
+        for (int i = skip + lane; i < skip + n; i += 32) {
+            int ri = i / len;
+            const int kb = i - ri * len;
+            int r = 0;
+            for (; r < CC_MAXR; ++r)
+                if (cnt[r] > 0 && ri-- == 0) break;                // the ri-th replica that has rows
+            if (r < CC_MAXR) bulk_prefetch_l2(blob[r] + off + (size_t)kb * wstage, wbytes);
+        }
+    }
 }
 __device__ __forceinline__ uint64_t policy_evict_first() {
     uint64_t p;

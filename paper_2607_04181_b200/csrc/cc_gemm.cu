@@ -581,11 +581,17 @@ k_gemm_cl(CcGemmGeo G, const uint8_t* __restrict__ act, CcEpi E, CcDims D, CcWor
                 }
             };
             run(0);
+            // the ring is full and the predecessor still runs: the next stages of my range go to L2 meanwhile
+            cc_prefetch_weights(G, H->blob, H->cnt, (int)blockIdx.x, (int)gridDim.x, n_pre, D.pf_self, lane);
             pdl_wait();
             if (lane == 0) CC_TP(W, 2 + KIND, 1);
             __syncwarp();
             if (elect_one()) pdl_launch_dependents();
             run(1);
+            // my copies are issued; the exchange and the epilogue follow: the first weight stages of the NEXT projection's CTAs
+            // go to L2 meanwhile (gate/up behind O, down behind gate/up)
+            if (KIND == EPI_O) cc_prefetch_weights(D.gu, H->blob, H->cnt, (int)blockIdx.x, (int)gridDim.x, 0, D.pf_next, lane);
+            if (KIND == EPI_GU) cc_prefetch_weights(D.dn, H->blob, H->cnt, (int)blockIdx.x, (int)gridDim.x, 0, D.pf_next, lane);
             if (lane == 0) CC_TP(W, 2 + KIND, 2);
             __syncwarp();
         } else if (warp == 1) {
@@ -810,7 +816,8 @@ void cc_gemm_cl_geometry(int which, CcGemmGeo& g, int n_sms) {
     g.S = 0;
     g.cl_tiles = 2;
     int best_ctas = 0;
-    for (int tiles = 2; tiles >= 1; --tiles) {
+    static const int min_tiles = getenv("CC_CL_MIN_TILES") ? atoi(getenv("CC_CL_MIN_TILES")) : 1;   // experiments
+    for (int tiles = 2; tiles >= min_tiles; --tiles) {
         const int n_clusters = g.ST * CC_G / tiles;
         for (int S = 1; S <= kClMaxS; ++S) {
             if (S > g.KB || n_clusters * S > n_sms) continue;
