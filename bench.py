@@ -689,6 +689,22 @@ def run_cfg3(args):
     assert B.cc_poll_device_error(S.ctx) == 0 and graph.exec_handle == exec_handle and graph.same_exec() and captures == 1
     ms = np.array([a.elapsed_time(b) for a, b in ev])
     flip_ms = {"scale_up_step_ms": float(ms[up]), "scale_down_step_ms": float(ms[down])}
+    # end to end: per step the input rows come from pinned host memory, the result rows go back to it and the host
+    # waits for them (it would sample the next tokens from them); host clock around the loop, contexts start over
+    e2e_steps = min(steps, 100)
+    h_in = torch.empty((batch, d), dtype=torch.bfloat16).pin_memory()
+    h_in.copy_(hidden.cpu())
+    h_out = torch.empty((batch, d), dtype=torch.bfloat16).pin_memory()
+    sl.copy_(torch.from_numpy(seq0))
+    torch.cuda.synchronize()
+    t0 = time.perf_counter()
+    for _ in range(e2e_steps):
+        hidden.copy_(h_in, non_blocking=True)
+        graph.replay()
+        h_out.copy_(hidden, non_blocking=True)
+        stream.synchronize()
+    e2e_ms = (time.perf_counter() - t0) * 1e3 / e2e_steps
+    assert B.cc_poll_device_error(S.ctx) == 0
     def summ(x):
         return {"mean_ms": round(float(x.mean()), 4), "p50_ms": round(float(np.percentile(x, 50)), 4),
                 "p99_ms": round(float(np.percentile(x, 99)), 4), "max_ms": round(float(x.max()), 4)}
@@ -713,6 +729,10 @@ def run_cfg3(args):
         "step_roofline": {"algorithmic_bytes_mid_run": int(bytes_step), "achieved_GBps": round(bytes_step / (mean_ms * 1e-3) / 1e9, 1),
                           "frac_of_measured_peak": round(bytes_step / (mean_ms * 1e-3) / 1e9 / peak, 4), "peak_source": peak_src},
         "gpu_launches": int(B.cc_forward_launch_count(S.layers[0])) * n_layers * steps,
+        "e2e": {"value": batch / (e2e_ms * 1e-3), "unit": UNIT, "ms_per_step": e2e_ms, "steps": e2e_steps,
+                "h2d_bytes_per_step": int(h_in.numel() * 2), "d2h_bytes_per_step": int(h_out.numel() * 2),
+                "how": "per step: the hidden rows copied from pinned host memory, one replay of the 32-layer graph, the result rows "
+                       "copied back, one stream synchronisation; host clock; all layers at 1 replica"},
     }
     print(json.dumps(line), flush=True)
     S.close()

@@ -26,7 +26,6 @@
 //     residual + write-back in request order), so no separate reduce kernel runs between GEMMs.
 #include "cc_epilogue.cuh"
 #include <cstdio>
-#include <cstdlib>
 
 namespace {
 
@@ -816,8 +815,7 @@ void cc_gemm_cl_geometry(int which, CcGemmGeo& g, int n_sms) {
     g.S = 0;
     g.cl_tiles = 2;
     int best_ctas = 0;
-    static const int min_tiles = getenv("CC_CL_MIN_TILES") ? atoi(getenv("CC_CL_MIN_TILES")) : 1;   // experiments
-    for (int tiles = 2; tiles >= min_tiles; --tiles) {
+    for (int tiles = 2; tiles >= 1; --tiles) {
         const int n_clusters = g.ST * CC_G / tiles;
         for (int S = 1; S <= kClMaxS; ++S) {
             if (S > g.KB || n_clusters * S > n_sms) continue;

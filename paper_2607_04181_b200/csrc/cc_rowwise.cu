@@ -110,20 +110,28 @@ __global__ void __launch_bounds__(kNormThreads) k_prologue(const int* __restrict
         s_goff[CC_MAXR] = off;
     }
     __syncthreads();
-    if (scan && b < batch && rep >= 0) {
+    if (scan) {
         // The attention kernel streams a row's pages before this step's appends are finished, up to the first page
         // some row of the step writes.  For a lone decode row that is its last page; for the rows of a prompt chunk
-        // (one request, consecutive positions) it is the lowest page any of them appends to.
-        const int key = s_key[b];
-        int m = s_wpg[b];
-        bool split = false;
-        for (int j = 0; j < batch; ++j)
-            if (s_key[j] == key) {
-                m = min(m, s_wpg[j]);
-                split |= s_rep[j] != rep;
+        // (one request, consecutive positions) it is the lowest page any of them appends to.  One warp per row, the
+        // lanes share the comparisons (a thread per row walking all rows took 3 us at batch 64, and the QKV GEMM
+        // waits for this block).
+        for (int rb = warp; rb < batch; rb += kNormThreads / 32) {
+            const int key = s_key[rb], rrep = s_rep[rb];
+            int m = 0x7fffffff;
+            bool split = false;
+            for (int j = lane; j < batch; j += 32)
+                if (s_key[j] == key) {
+                    m = min(m, s_wpg[j]);
+                    split |= s_rep[j] != rrep;
+                }
+            m = __reduce_min_sync(0xffffffffu, m);
+            split = __any_sync(0xffffffffu, split);
+            if (lane == 0 && rrep >= 0) {
+                W.first_wr[rb] = m;
+                if (split) atomicOr(W.err, CC_DEVERR_SPLIT_REQUEST);   // one request served by two replicas
             }
-        W.first_wr[b] = m;
-        if (split) atomicOr(W.err, CC_DEVERR_SPLIT_REQUEST);   // one request served by two replicas
+        }
     }
     if (b < 256) {
         // rank of this row among the rows of its replica: ballot of its warp + the warps before it
@@ -176,7 +184,10 @@ __global__ void __launch_bounds__(kNormThreads) k_prologue(const int* __restrict
     }
     __syncthreads();
     const int mypos = s_mypos;
-    if (mypos < 0) return;                 // block-uniform: padding row
+    if (mypos < 0) {                       // block-uniform: padding row, or one of the two table blocks
+        if (b == 0 && (pub || scan)) CC_TP(W, 0, 2);
+        return;
+    }
     const uint4* g = reinterpret_cast<const uint4*>(tab->rep[s_myrep].blob + D.off_g1);
     uint4 gv[kNormVec];
     float ss = 0.f;

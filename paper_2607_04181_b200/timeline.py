@@ -59,7 +59,7 @@ def main() -> None:
         print(f"{name:13s}", " | ".join(f"{t[k, pt, 0]:7.2f}..{t[k, pt, 1]:7.2f}" for pt in range(npt)))
     print("GEMM points: entry | dependency wait done (producer) | producer issued its last copy | mainloop drained, partials "
           "stored | first fixup wait done | end")
-    print("prologue: entry | dependency wait done | end;  attention: entry | dependency wait done (consumers) | consumers saw "
+    print("prologue: entry | dependency wait done | end (row blocks and the two table blocks);  attention: entry | dependency wait done (consumers) | consumers saw "
           "the end marker")
     for kind, name in enumerate(("gemm_qkv", "gemm_o", "gemm_gate_up", "gemm_down")):
         d, a = raw[8 + kind], raw[12 + kind]
