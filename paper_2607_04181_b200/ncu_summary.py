@@ -32,9 +32,9 @@ METRICS = [
     "sm__warps_active.avg.pct_of_peak_sustained_active",
 ]
 # kernel-name pattern -> the stage name bench.py uses
-STAGES = [(r"k_prologue", "prologue"), (r"k_gemm(_cl)?<(\(int\))?0>", "gemm_qkv"), (r"k_attn", "attention"),
-          (r"k_gemm(_cl)?<(\(int\))?1>", "gemm_o"), (r"k_gemm(_cl)?<(\(int\))?2>", "gemm_gate_up"),
-          (r"k_gemm(_cl)?<(\(int\))?3>", "gemm_down"),
+STAGES = [(r"k_prologue", "prologue"), (r"k_gemm(_cl)?<(\(int\))?0[,>]", "gemm_qkv"), (r"k_attn", "attention"),
+          (r"k_gemm(_cl)?<(\(int\))?1[,>]", "gemm_o"), (r"k_gemm(_cl)?<(\(int\))?2[,>]", "gemm_gate_up"),
+          (r"k_gemm(_cl)?<(\(int\))?3[,>]", "gemm_down"),
           (r"k_big_gemm<(\(int\))?0", "big_gemm_qkv"), (r"k_big_gemm<(\(int\))?1", "big_gemm_o"),
           (r"k_big_gemm<(\(int\))?2", "big_gemm_gate_up"), (r"k_big_gemm<(\(int\))?3", "big_gemm_down"),
           (r"k_prefill_attn", "prefill_attention"), (r"k_copy", "replica_copy")]
