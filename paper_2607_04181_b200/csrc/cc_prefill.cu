@@ -27,15 +27,16 @@ constexpr int kKvTile = 64;                  // kv tokens per tile (4 pages)
 constexpr int kKvStages = 3;
 constexpr int kQBytes = 2 * 2 * 128 * 128;   // Q: [hi | lo][half of Dh][128 rows][128 B]
 constexpr int kKvStageBytes = 2 * 2 * kKvTile * 128;   // [K | V][half of Dh][64 tokens][128 B]
-constexpr int kPBytes = 2 * 128 * 128;       // P: [hi | lo][128 rows][64 kv = 128 B]
+constexpr int kPBytes = 2 * 128 * 128;       // P: [hi | lo][128 rows][64 kv = 128 B]; two such buffers (tile parity)
 constexpr int kPfHdr = 1024;
-constexpr int kPfSmem = kPfHdr + kQBytes + kKvStages * kKvStageBytes + kPBytes;
+constexpr int kPfSmem = kPfHdr + kQBytes + kKvStages * kKvStageBytes + 2 * kPBytes;
+constexpr float kLazyLog2 = 8.f;             // O and l are rescaled only when a row maximum has grown by more than 2^8
 constexpr uint32_t kColS = 0, kColO = 128;   // TMEM columns: S buffers at 0 and 64, O at 128..255
 
 struct PfHdr {
     uint64_t kv_full[kKvStages], kv_empty[kKvStages];
     uint64_t s_full[2], s_free[2];
-    uint64_t p_full, pv_done, q_ready;
+    uint64_t p_full[2], pv_done[2], q_ready;      // [P buffer = kv tile parity]
     uint32_t tmem_base;
 };
 
@@ -108,8 +109,10 @@ k_prefill_attn(const int* __restrict__ seq_lens, CcKv kv, CcDims D, CcWork W, co
             mbar_init(&H->s_full[i], 1);
             mbar_init(&H->s_free[i], 4);
         }
-        mbar_init(&H->p_full, 4);
-        mbar_init(&H->pv_done, 1);
+        for (int i = 0; i < 2; ++i) {
+            mbar_init(&H->p_full[i], 4);
+            mbar_init(&H->pv_done[i], 1);
+        }
         mbar_init(&H->q_ready, 4);
         fence_mbar_init();
     }
@@ -167,24 +170,26 @@ k_prefill_attn(const int* __restrict__ seq_lens, CcKv kv, CcDims D, CcWork W, co
         // ===================== MMA issuer =====================
         const uint32_t idesc_s = idesc_bf16(kKvTile, false), idesc_o = idesc_bf16(128, true);
         const uint32_t q_lo = (uint32_t)umma_desc_sw128(smem_u32(sQ)), k_hi32 = (uint32_t)(umma_desc_sw128(0) >> 32);
-        const uint32_t p_lo = (uint32_t)umma_desc_sw128(smem_u32(sP));
+        const uint32_t p_lo0 = (uint32_t)umma_desc_sw128(smem_u32(sP));
         const uint64_t v_d0 = umma_desc_sw128_lbo(smem_u32(sKV) + 16384u, 8192u, 1024u);
         const uint32_t v_hi32 = (uint32_t)(v_d0 >> 32);
         uint32_t g = 0, n_pv = 0, n_item = 0;
         Item it;
         auto issue_pv = [&](uint32_t gt, bool first) {
             const int stage = (int)(gt % kKvStages);
-            mbar_wait(&H->p_full, n_pv & 1);
+            const uint32_t pb = n_pv & 1;
+            mbar_wait(&H->p_full[pb], (n_pv >> 1) & 1);
             tc_fence_after();
             if (elect_one()) {
                 const uint32_t v_lo = (uint32_t)v_d0 + (((uint32_t)stage * kKvStageBytes) >> 4);
+                const uint32_t p_lo = p_lo0 + pb * (kPBytes >> 4);
 #pragma unroll
                 for (int ks = 0; ks < kKvTile / 16; ++ks) {
                     // A: P plane (K-major, 16 kv = 32 B per step); B: V, MN-major, 16 kv rows = 2 KiB per step
                     umma_bf16_lo(tmem_base + kColO, p_lo + 2 * ks, v_lo + ks * 128, k_hi32, v_hi32, idesc_o, (first && ks == 0) ? 0u : 1u);
                     umma_bf16_lo(tmem_base + kColO, p_lo + 1024 + 2 * ks, v_lo + ks * 128, k_hi32, v_hi32, idesc_o, 1u);
                 }
-                umma_commit(&H->pv_done);
+                umma_commit(&H->pv_done[pb]);
                 umma_commit(&H->kv_empty[stage]);
             }
             __syncwarp();
@@ -225,22 +230,39 @@ k_prefill_attn(const int* __restrict__ seq_lens, CcKv kv, CcDims D, CcWork W, co
         Item it;
         for (int id = blockIdx.x; item_at(W, D, seq_lens, id, it); id += gridDim.x) {
             // ---- Q of the item: q_rot rows (fp32, post-RoPE) x log2(e)/sqrt(Dh) -> bf16 hi + lo operand planes ----
-            for (int r = (warp - 2); r < 128; r += 4) {                // one row per warp iteration, 512 B coalesced
-                const int tl = r / G, gq = r - tl * G;
-                float4 x = make_float4(0.f, 0.f, 0.f, 0.f);
-                if (tl < it.n_tok) {
-                    const int pos = W.pos_of[it.row0 + tl];
-                    x = *reinterpret_cast<const float4*>(W.q_rot + (size_t)pos * D.QD + (size_t)(it.h * G + gq) * 128 + 4 * lane);
+            // one row per warp iteration, 512 B coalesced; sixteen rows' loads in flight together (one at a time, the two
+            // dependent global loads of every row cost the item ~20 us during which the tensor pipe has nothing to do)
+            constexpr int kQB = 16;
+#pragma unroll 1
+            for (int rb = 0; rb < 32; rb += kQB) {
+                float4 x[kQB];
+                int pos[kQB];
+#pragma unroll
+                for (int u = 0; u < kQB; ++u) {
+                    const int r = (warp - 2) + 4 * (rb + u), tl = r / G;
+                    pos[u] = tl < it.n_tok ? W.pos_of[it.row0 + tl] : -1;
                 }
-                x.x *= D.qk_scale_log2; x.y *= D.qk_scale_log2; x.z *= D.qk_scale_log2; x.w *= D.qk_scale_log2;
-                uint32_t h0, l0, h1, l1;
-                split_hilo(x.x, x.y, h0, l0);
-                split_hilo(x.z, x.w, h1, l1);
-                // dims 4 lane .. 4 lane + 3: half = lane / 16, 16-byte chunk (lane % 16) / 2, byte (lane & 1) * 8 inside it
-                const uint32_t off = (uint32_t)(lane >> 4) * 16384u + (uint32_t)(r >> 3) * 1024u + (uint32_t)(r & 7) * 128u +
-                                     (uint32_t)((((lane & 15) >> 1) ^ (r & 7)) << 4) + (uint32_t)(lane & 1) * 8u;
-                *reinterpret_cast<uint2*>(sQ + off) = make_uint2(h0, h1);
-                *reinterpret_cast<uint2*>(sQ + 32768u + off) = make_uint2(l0, l1);
+#pragma unroll
+                for (int u = 0; u < kQB; ++u) {
+                    const int r = (warp - 2) + 4 * (rb + u), tl = r / G, gq = r - tl * G;
+                    x[u] = make_float4(0.f, 0.f, 0.f, 0.f);
+                    if (pos[u] >= 0)
+                        x[u] = *reinterpret_cast<const float4*>(W.q_rot + (size_t)pos[u] * D.QD + (size_t)(it.h * G + gq) * 128 + 4 * lane);
+                }
+#pragma unroll
+                for (int u = 0; u < kQB; ++u) {
+                    const int r = (warp - 2) + 4 * (rb + u);
+                    float4 v = x[u];
+                    v.x *= D.qk_scale_log2; v.y *= D.qk_scale_log2; v.z *= D.qk_scale_log2; v.w *= D.qk_scale_log2;
+                    uint32_t h0, l0, h1, l1;
+                    split_hilo(v.x, v.y, h0, l0);
+                    split_hilo(v.z, v.w, h1, l1);
+                    // dims 4 lane .. 4 lane + 3: half = lane / 16, 16-byte chunk (lane % 16) / 2, byte (lane & 1) * 8 inside it
+                    const uint32_t off = (uint32_t)(lane >> 4) * 16384u + (uint32_t)(r >> 3) * 1024u + (uint32_t)(r & 7) * 128u +
+                                         (uint32_t)((((lane & 15) >> 1) ^ (r & 7)) << 4) + (uint32_t)(lane & 1) * 8u;
+                    *reinterpret_cast<uint2*>(sQ + off) = make_uint2(h0, h1);
+                    *reinterpret_cast<uint2*>(sQ + 32768u + off) = make_uint2(l0, l1);
+                }
             }
             fence_proxy_async_smem();
             __syncwarp();
@@ -262,32 +284,49 @@ k_prefill_attn(const int* __restrict__ seq_lens, CcKv kv, CcDims D, CcWork W, co
                 if (lane == 0) mbar_arrive(&H->s_free[sb]);
                 float mx = -INFINITY;
                 const int lim = p_row - kv0;                           // columns 0 .. lim are visible
+                if (__all_sync(0xffffffffu, lim >= kKvTile - 1)) {     // not a diagonal tile of this warp's rows: no mask
 #pragma unroll
-                for (int u = 0; u < 2; ++u)
+                    for (int u = 0; u < 2; ++u)
 #pragma unroll
-                    for (int i = 0; i < 32; ++i) {
-                        const float v = (u * 32 + i <= lim) ? __uint_as_float(sv[u][i]) : -INFINITY;
-                        sv[u][i] = __float_as_uint(v);
-                        mx = fmaxf(mx, v);
-                    }
-                const float m_new = fmaxf(m_run, mx);                  // finite from tile 0 on: position 0 is visible to every row
-                const float alpha = exp2f(m_run - m_new);              // first tile: exp2(-inf) = 0, l_run = 0 anyway
-                if (j > 0) {
-                    mbar_wait(&H->pv_done, (n_pv - 1) & 1);            // P is free again and O holds tiles 0 .. j-1
-                    tc_fence_after();
-                    if (__any_sync(0xffffffffu, m_new > m_run)) {      // rescale this warp's 32 rows of O
-#pragma unroll 1
-                        for (int c = 0; c < 128; c += 32) {
-                            uint32_t ov[32];
-                            tmem_ld_32x32b_x32(lane_addr + kColO + c, ov);
-                            tmem_ld_wait();
+                        for (int i = 0; i < 32; ++i) mx = fmaxf(mx, __uint_as_float(sv[u][i]));
+                } else {
 #pragma unroll
-                            for (int i = 0; i < 32; ++i) ov[i] = __float_as_uint(__uint_as_float(ov[i]) * alpha);
-                            tmem_st_32x32b_x32(lane_addr + kColO + c, ov);
+                    for (int u = 0; u < 2; ++u)
+#pragma unroll
+                        for (int i = 0; i < 32; ++i) {
+                            const float v = (u * 32 + i <= lim) ? __uint_as_float(sv[u][i]) : -INFINITY;
+                            sv[u][i] = __float_as_uint(v);
+                            mx = fmaxf(mx, v);
                         }
-                        tmem_st_wait();
-                    }
                 }
+                // Lazy rescale: the probabilities are taken against a reference m_run that follows the running maximum only
+                // when that has grown by more than 2^kLazyLog2 in some row of the warp (p <= 2^8: harmless in fp32 / bf16
+                // hi + lo).  Then O (the warp's 32 TMEM lanes) and l are rescaled, which needs every P V product issued so
+                // far to be complete; otherwise this tile's probabilities go into the other P buffer while the previous
+                // product still runs.  A function of the data only.
+                const float m_seen = fmaxf(m_run, mx);                 // finite from tile 0 on: position 0 is visible to every row
+                float alpha = 1.f;
+                if (j == 0) {
+                    m_run = m_seen;                                    // first tile: O is overwritten, l_run = 0
+                } else if (__any_sync(0xffffffffu, m_seen > m_run + kLazyLog2)) {
+                    mbar_wait(&H->pv_done[(n_pv - 1) & 1], ((n_pv - 1) >> 1) & 1);   // O holds tiles 0 .. j-1
+                    tc_fence_after();
+                    alpha = exp2f(m_run - m_seen);
+                    m_run = m_seen;
+#pragma unroll 1
+                    for (int c = 0; c < 128; c += 32) {
+                        uint32_t ov[32];
+                        tmem_ld_32x32b_x32(lane_addr + kColO + c, ov);
+                        tmem_ld_wait();
+#pragma unroll
+                        for (int i = 0; i < 32; ++i) ov[i] = __float_as_uint(__uint_as_float(ov[i]) * alpha);
+                        tmem_st_32x32b_x32(lane_addr + kColO + c, ov);
+                    }
+                    tmem_st_wait();
+                }
+                const float m_new = m_run;
+                const uint32_t pb = n_pv & 1;
+                if (n_pv >= 2) mbar_wait(&H->pv_done[pb], ((n_pv - 2) >> 1) & 1);    // the product that read this P buffer is done
                 if (j == it.n_tiles - 1 && it.s_last < kv0 + kKvTile) {
                     // ragged last tile: V rows past the last position hold other data (or nothing): p = 0 must meet 0
                     mbar_wait(&H->kv_full[g % kKvStages], (g / kKvStages) & 1);
@@ -299,7 +338,7 @@ k_prefill_attn(const int* __restrict__ seq_lens, CcKv kv, CcDims D, CcWork W, co
                     }
                 }
                 float lsum = 0.f;
-                uint8_t* prow = sP + (uint32_t)(m >> 3) * 1024u + (uint32_t)(m & 7) * 128u;
+                uint8_t* prow = sP + pb * (uint32_t)kPBytes + (uint32_t)(m >> 3) * 1024u + (uint32_t)(m & 7) * 128u;
 #pragma unroll
                 for (int u = 0; u < 2; ++u)
 #pragma unroll
@@ -317,15 +356,14 @@ k_prefill_attn(const int* __restrict__ seq_lens, CcKv kv, CcDims D, CcWork W, co
                         *reinterpret_cast<uint4*>(prow + 16384u + ch) = make_uint4(lo[0], lo[1], lo[2], lo[3]);
                     }
                 l_run = l_run * alpha + lsum;
-                m_run = m_new;
                 fence_proxy_async_smem();
                 tc_fence_before();
                 __syncwarp();
-                if (lane == 0) mbar_arrive(&H->p_full);
+                if (lane == 0) mbar_arrive(&H->p_full[pb]);
                 ++n_pv;
             }
             // ---- the item's rows: O / l -> the O-projection operand ----
-            mbar_wait(&H->pv_done, (n_pv - 1) & 1);
+            mbar_wait(&H->pv_done[(n_pv - 1) & 1], ((n_pv - 1) >> 1) & 1);
             tc_fence_after();
             const int tlr = m / G, gq = m - tlr * G;
             const bool live = tlr < it.n_tok;
