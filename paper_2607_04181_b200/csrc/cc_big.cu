@@ -14,25 +14,32 @@ namespace {
 
 constexpr int kGroupThreads = 1024;
 
-// exclusive prefix of v over the block (all threads call); *total = sum
-__device__ __forceinline__ int block_scan_excl(int v, int* s_w, int* total) {
+// exclusive prefix of v over the block (all threads call); *total = sum.  v may pack several counters in bit fields
+// that cannot carry into one another.  Two levels of shuffles: the warps' totals are scanned by warp 0.
+__device__ __forceinline__ unsigned long long block_scan_excl(unsigned long long v, unsigned long long* s_w, unsigned long long* total) {
     const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
-    int inc = v;
+    unsigned long long inc = v;
 #pragma unroll
     for (int o = 1; o < 32; o <<= 1) {
-        const int t = __shfl_up_sync(0xffffffffu, inc, o);
+        const unsigned long long t = __shfl_up_sync(0xffffffffu, inc, o);
         if (lane >= o) inc += t;
     }
-    __syncthreads();
+    __syncthreads();                                                   // the previous call's readers are done with s_w
     if (lane == 31) s_w[w] = inc;
     __syncthreads();
-    int base = 0, tot = 0;
-    for (int i = 0; i < kGroupThreads / 32; ++i) {
-        if (i < w) base += s_w[i];
-        tot += s_w[i];
+    if (w == 0) {
+        static_assert(kGroupThreads == 1024, "one warp total per lane");
+        unsigned long long x = s_w[lane];
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            const unsigned long long t = __shfl_up_sync(0xffffffffu, x, o);
+            if (lane >= o) x += t;
+        }
+        s_w[lane] = x;
     }
-    *total = tot;
-    return base + inc - v;
+    __syncthreads();
+    *total = s_w[kGroupThreads / 32 - 1];
+    return (w ? s_w[w - 1] : 0ull) + inc - v;
 }
 
 __global__ void __launch_bounds__(kGroupThreads) k_big_group(const int* __restrict__ assign, const int* __restrict__ seq_lens,
@@ -40,9 +47,9 @@ __global__ void __launch_bounds__(kGroupThreads) k_big_group(const int* __restri
                                                              const CcLayerTable* __restrict__ tab, CcWork W) {
     __shared__ signed char s_rep[CC_BIG_MAX_ROWS];
     __shared__ unsigned char s_cont[CC_BIG_MAX_ROWS + 1];     // row b continues the chunk of row b - 1
-    __shared__ int s_w[kGroupThreads / 32];
-    __shared__ int s_cnt[CC_MAXR], s_goff[CC_MAXR + 1], s_run[CC_MAXR];
-    __shared__ int s_ndec, s_nchunk, s_ntail, s_pages, s_pages_dec;
+    __shared__ unsigned long long s_w[kGroupThreads / 32];
+    __shared__ int s_cnt[CC_MAXR], s_goff[CC_MAXR + 1];
+    __shared__ int s_pages_dec;
     __shared__ int s_head[CC_BIG_MAX_CHUNKS], s_tail[CC_BIG_MAX_CHUNKS], s_ntile[CC_BIG_MAX_CHUNKS];
     const int tid = threadIdx.x;
     const uint32_t mask = tab->active_mask;
@@ -54,19 +61,45 @@ __global__ void __launch_bounds__(kGroupThreads) k_big_group(const int* __restri
         W.row_page[i] = -1;
     }
     __syncthreads();
-    // ---- pass 1: the replica of every row, chunk continuation flags, rows per replica ----
-    for (int b0 = 0; b0 < batch; b0 += kGroupThreads) {
-        const int b = b0 + tid;
-        int rep = -1;
-        if (b < batch) rep = cc_row_replica(assign, seq_lens, b, batch, D, mask, err);
-        if (b < batch) s_rep[b] = (signed char)rep;
-        bool cont = false;
-        if (b < batch && b > 0 && rep >= 0) {
-            uint32_t e2 = 0;                                           // (row b - 1 reports its own errors)
-            cont = cc_row_replica(assign, seq_lens, b - 1, batch, D, mask, e2) >= 0 && seq_lens[b] == seq_lens[b - 1] + 1 &&
-                   block_table[(size_t)b * D.max_blocks] == block_table[(size_t)(b - 1) * D.max_blocks];
+    // Every global read of the grouping is issued up front, eight rows per thread (a row at a time, the dependent reads of the
+    // three passes cost ~30 memory latencies: 60-90 us of a step): the row's and its predecessor's seq_len, replica and
+    // first page id now, the page its token is appended to once the seq_len is there.
+    constexpr int kIt = CC_BIG_MAX_ROWS / kGroupThreads;
+    int seqv[kIt], repv[kIt], lpv[kIt];
+    bool contv[kIt];
+    {
+        int asg[kIt], fpv[kIt], seqp[kIt], asgp[kIt], fpp[kIt];
+#pragma unroll
+        for (int k = 0; k < kIt; ++k) {
+            const int b = k * kGroupThreads + tid;
+            const bool in = b < batch, inp = in && b > 0;
+            seqv[k] = in ? seq_lens[b] : 0;
+            asg[k] = in ? assign[b] : 0;
+            fpv[k] = in ? block_table[(size_t)b * D.max_blocks] : -1;
+            seqp[k] = inp ? seq_lens[b - 1] : 0;
+            asgp[k] = inp ? assign[b - 1] : 0;
+            fpp[k] = inp ? block_table[(size_t)(b - 1) * D.max_blocks] : -2;
         }
-        if (b < batch) s_cont[b] = cont ? 1 : 0;
+#pragma unroll
+        for (int k = 0; k < kIt; ++k) {
+            const int b = k * kGroupThreads + tid;
+            repv[k] = b < batch ? cc_row_replica_of(seqv[k], asg[k], D, mask, err) : -1;
+            uint32_t e2 = 0;                                           // (row b - 1 reports its own errors)
+            contv[k] = repv[k] >= 0 && b > 0 && cc_row_replica_of(seqp[k], asgp[k], D, mask, e2) >= 0 && seqv[k] == seqp[k] + 1 &&
+                       fpv[k] == fpp[k];
+            lpv[k] = repv[k] >= 0 ? block_table[(size_t)b * D.max_blocks + (seqv[k] - 1) / CC_PAGE] : -1;
+        }
+    }
+    // ---- pass 1: the replica of every row, chunk continuation flags, rows per replica ----
+#pragma unroll
+    for (int k = 0; k < kIt; ++k) {
+        const int b = k * kGroupThreads + tid;
+        if (k * kGroupThreads >= batch) break;
+        const int rep = repv[k];
+        if (b < batch) {
+            s_rep[b] = (signed char)rep;
+            s_cont[b] = contv[k] ? 1 : 0;
+        }
 #pragma unroll
         for (int r = 0; r < CC_MAXR; ++r) {
             const uint32_t bal = __ballot_sync(0xffffffffu, rep == r);
@@ -79,86 +112,78 @@ __global__ void __launch_bounds__(kGroupThreads) k_big_group(const int* __restri
         int off = 0;
         for (int r = 0; r < CC_MAXR; ++r) {
             s_goff[r] = off;
-            s_run[r] = 0;
             off += (s_cnt[r] + CC_ROW_ALIGN - 1) / CC_ROW_ALIGN * CC_ROW_ALIGN;
         }
         s_goff[CC_MAXR] = off;
-        s_ndec = 0;
-        s_nchunk = 0;
-        s_ntail = 0;
-        s_pages = 0;
         s_pages_dec = 0;
     }
     __syncthreads();
     // ---- pass 2: grouped positions (stable), per-row tables, decode-row list with its page prefix ----
-    for (int b0 = 0; b0 < batch; b0 += kGroupThreads) {
-        const int b = b0 + tid;
-        const int rep = b < batch ? s_rep[b] : -1;
-        int pos = -1;
+    // (every thread keeps the running totals: the scans hand the iteration's totals to all)
+    int run[CC_MAXR] = {0, 0, 0, 0}, n_dec_run = 0, pages_run = 0;
 #pragma unroll
-        for (int r = 0; r < CC_MAXR; ++r) {
-            int tot;
-            const int ex = block_scan_excl(rep == r ? 1 : 0, s_w, &tot);
-            if (rep == r) pos = s_goff[r] + s_run[r] + ex;
-            __syncthreads();
-            if (tid == 0) s_run[r] += tot;
+    for (int k = 0; k < kIt; ++k) {
+        if (k * kGroupThreads >= batch) break;
+        const int b = k * kGroupThreads + tid;
+        const int rep = repv[k];
+        int pos = -1;
+        {   // rank among the rows of the same replica: the four counters of an iteration (<= 1024 each) in 16-bit fields
+            unsigned long long tot;
+            const unsigned long long ex = block_scan_excl(rep >= 0 ? 1ull << (16 * rep) : 0ull, s_w, &tot);
+            if (rep >= 0) pos = s_goff[rep] + run[rep] + (int)((ex >> (16 * rep)) & 0xffffull);
+#pragma unroll
+            for (int r = 0; r < CC_MAXR; ++r) run[r] += (int)((tot >> (16 * r)) & 0xffffull);
         }
         if (b < batch) {
             W.pos_of[b] = pos;
             if (pos >= 0) {
-                const int p = seq_lens[b] - 1;
+                const int p = seqv[k] - 1;
                 W.perm[pos] = b;
                 W.row_pos[pos] = p;
-                W.row_page[pos] = block_table[(size_t)b * D.max_blocks + p / CC_PAGE];
+                W.row_page[pos] = lpv[k];
                 W.first_wr[b] = p / CC_PAGE;
                 if (s_cont[b] && s_rep[b - 1] != rep) err |= CC_DEVERR_SPLIT_REQUEST;   // one request, two replicas
             }
         }
-        // decode rows: live rows that neither continue a chunk nor start one
+        // decode rows: live rows that neither continue a chunk nor start one; their count (low 16 bits) and pages together
         const bool dec = rep >= 0 && !s_cont[b] && !s_cont[b + 1];
-        const int npg = dec ? (seq_lens[b] + CC_PAGE - 1) / CC_PAGE : 0;
-        int n_here, pg_here;
-        const int di = block_scan_excl(dec ? 1 : 0, s_w, &n_here);
-        const int pg = block_scan_excl(npg, s_w, &pg_here);
+        const int npg = dec ? (seqv[k] + CC_PAGE - 1) / CC_PAGE : 0;
+        unsigned long long dtot;
+        const unsigned long long dex = block_scan_excl((dec ? 1ull : 0ull) | ((unsigned long long)npg << 16), s_w, &dtot);
+        const int di = (int)(dex & 0xffffull), pg = (int)(dex >> 16), n_here = (int)(dtot & 0xffffull);
         if (dec) {
-            const int i = s_ndec + di;
+            const int i = n_dec_run + di;
             if (i < CC_BIG_MAX_DEC) {
                 W.dec_rows[i] = b;
-                W.pg_prefix[i] = s_pages + pg;
-                if (i == CC_BIG_MAX_DEC - 1 || (di == n_here - 1)) atomicMax(&s_pages_dec, s_pages + pg + npg);   // end of the list so far
+                W.pg_prefix[i] = pages_run + pg;
+                if (i == CC_BIG_MAX_DEC - 1 || (di == n_here - 1)) atomicMax(&s_pages_dec, pages_run + pg + npg);   // end of the list so far
             } else {
                 err |= CC_DEVERR_TOO_MANY_DECODE;
             }
         }
-        __syncthreads();
-        if (tid == 0) {
-            s_ndec += n_here;
-            s_pages += pg_here;
-        }
-        __syncthreads();
+        n_dec_run += n_here;
+        pages_run += (int)(dtot >> 16);
     }
     // chunks: a head is a live row that does not continue a chunk but whose successor does; a tail is a row that
     // continues one and whose successor does not.  Runs are disjoint and ordered, so head c pairs with tail c.
+    int n_chunk_run = 0, n_tail_run = 0;
     for (int b0 = 0; b0 < batch; b0 += kGroupThreads) {
         const int b = b0 + tid;
         const bool head = b < batch && s_rep[b] >= 0 && !s_cont[b] && s_cont[b + 1];
         const bool tail = b < batch && s_cont[b] && !s_cont[b + 1];
-        int n_here, t_here;
-        const int ci = block_scan_excl(head ? 1 : 0, s_w, &n_here);
-        const int ti = block_scan_excl(tail ? 1 : 0, s_w, &t_here);
+        unsigned long long tot;
+        const unsigned long long ex = block_scan_excl((head ? 1ull : 0ull) | (tail ? 1ull << 16 : 0ull), s_w, &tot);
+        const int ci = (int)(ex & 0xffffull), ti = (int)(ex >> 16);
         if (head) {
-            if (s_nchunk + ci < CC_BIG_MAX_CHUNKS) s_head[s_nchunk + ci] = b; else err |= CC_DEVERR_TOO_MANY_DECODE;
+            if (n_chunk_run + ci < CC_BIG_MAX_CHUNKS) s_head[n_chunk_run + ci] = b; else err |= CC_DEVERR_TOO_MANY_DECODE;
         }
-        if (tail && s_ntail + ti < CC_BIG_MAX_CHUNKS) s_tail[s_ntail + ti] = b;
-        __syncthreads();
-        if (tid == 0) {
-            s_nchunk += n_here;
-            s_ntail += t_here;
-        }
-        __syncthreads();
+        if (tail && n_tail_run + ti < CC_BIG_MAX_CHUNKS) s_tail[n_tail_run + ti] = b;
+        n_chunk_run += (int)(tot & 0xffffull);
+        n_tail_run += (int)(tot >> 16);
     }
+    __syncthreads();
     if (err) atomicOr(W.err, err);
-    const int n_chunks = min(s_nchunk, CC_BIG_MAX_CHUNKS);
+    const int n_chunks = min(n_chunk_run, CC_BIG_MAX_CHUNKS);
     const int T = 128 / D.G;                                           // tokens of a query tile
     if (tid < n_chunks) {
         const int len = s_tail[tid] - s_head[tid] + 1;
@@ -177,8 +202,9 @@ __global__ void __launch_bounds__(kGroupThreads) k_big_group(const int* __restri
         int cntj = 0;
         if (j >= 0)
             for (int c = 0; c < n_chunks; ++c) cntj += s_ntile[c] > j;
-        int here;
-        int at = n_items_tot + block_scan_excl(cntj, s_w, &here);
+        unsigned long long here64;
+        int at = n_items_tot + (int)block_scan_excl((unsigned long long)cntj, s_w, &here64);
+        const int here = (int)here64;
         if (j >= 0)
             for (int c = 0; c < n_chunks; ++c)
                 if (s_ntile[c] > j) {
@@ -193,7 +219,7 @@ __global__ void __launch_bounds__(kGroupThreads) k_big_group(const int* __restri
     }
     if (n_items_tot > CC_BIG_MAX_ITEMS && tid == 0) atomicOr(W.err, CC_DEVERR_TOO_MANY_DECODE);
     if (tid == 0) {
-        const int n_dec = min(s_ndec, CC_BIG_MAX_DEC);
+        const int n_dec = min(n_dec_run, CC_BIG_MAX_DEC);
         const int n_items = min(n_items_tot, CC_BIG_MAX_ITEMS);
         // the page prefix of the unused decode slots = the total (k_attn reads CC_BIG_MAX_DEC + 1 entries)
         const int total = s_pages_dec;

@@ -124,21 +124,24 @@ struct CcSched {
 // Replica that serves row b, or -1 for a row that does not run (padding, bad seq_len); `err` collects the
 // CC_DEVERR_* bits.  The ONE statement of the row-validity rules: the grouping kernel and the QKV GEMM
 // (which counts the groups itself, because it starts before the grouping kernel has finished) both use it.
-__device__ __forceinline__ int cc_row_replica(const int* __restrict__ assign, const int* __restrict__ seq_lens, int b,
-                                              int batch, const CcDims& D, uint32_t active_mask, uint32_t& err) {
-    if (b >= batch) return -1;
-    const int s = seq_lens[b];
+__device__ __forceinline__ int cc_row_replica_of(int s, int rep, const CcDims& D, uint32_t active_mask, uint32_t& err) {
     if (s <= 0) return -1;
     if (s > D.max_position || (s + CC_PAGE - 1) / CC_PAGE > D.max_blocks) {
         err |= CC_DEVERR_BAD_SEQLEN;
         return -1;
     }
-    int rep = assign[b];
     if (rep < 0 || rep >= CC_MAXR || !((active_mask >> rep) & 1u)) {
         err |= CC_DEVERR_BAD_REPLICA;
         rep = 0;
     }
     return rep;
+}
+__device__ __forceinline__ int cc_row_replica(const int* __restrict__ assign, const int* __restrict__ seq_lens, int b,
+                                              int batch, const CcDims& D, uint32_t active_mask, uint32_t& err) {
+    if (b >= batch) return -1;
+    const int s = seq_lens[b];
+    if (s <= 0) return -1;
+    return cc_row_replica_of(s, assign[b], D, active_mask, err);
 }
 
 // Replica group that holds grouped position `pos` (groups are laid out in replica order).

@@ -11,9 +11,12 @@
 //     by TMA (boxes of 16 rows x 128 B, 128-byte swizzle, straight into the operand layout), ring of three stages;
 //   * S = Q K^T (M 128, N 64, K 128) and O += P V (M 128, N 128, K 64) are tcgen05.mma into TMEM (S double
 //     buffered, O resident); K is the K-major B operand, V the MN-major one (no transpose anywhere);
-//   * four softmax warps own one row per thread (TMEM lane = row): tcgen05.ld of the scores, causal mask on the
-//     diagonal tiles only, online softmax in log2 units, O rescaled in TMEM only when a row maximum of the warp
-//     moved, probabilities written to shared memory as the A operand of the P V product;
+//   * eight softmax warps, one query row per thread (TMEM lane = row) and two warps per lane quarter that share a tile's 64
+//     columns (row maxima and sums meet through shared memory, one named barrier per pair and tile): tcgen05.ld of the
+//     scores, causal mask on the diagonal tiles only, online softmax in log2 units against a reference maximum that
+//     follows the running one only when that grew by more than 2^8 (then O is rescaled in TMEM), probabilities written
+//     to one of two shared-memory buffers as the A operand of the P V product, so the softmax of tile j + 1 runs while
+//     the product of tile j does;
 //   * q and the probabilities enter as bf16 hi + lo planes (two MMAs each) like in the decode kernel: the K/V are
 //     bf16 by definition, and a single bf16 plane of q or p costs 2e-3 on the attention output;
 //   * items are dealt round-robin in decreasing cost; every row is finished by one item in one fixed order, so the
@@ -22,14 +25,19 @@
 
 namespace {
 
-constexpr int kPfThreads = 192;              // warp 0 producer, warp 1 MMA issuer, warps 2..5 softmax (TMEM lane quarter = warp % 4)
+constexpr int kSmWarps = 8;                  // softmax warps: two per TMEM lane quarter, each takes half of a tile's columns
+constexpr int kPfThreads = (2 + kSmWarps) * 32;   // warp 0 producer, warp 1 MMA issuer, warps 2..9 softmax (TMEM lane quarter = warp % 4)
 constexpr int kKvTile = 64;                  // kv tokens per tile (4 pages)
-constexpr int kKvStages = 3;
+#ifndef CC_PF_KV_STAGES
+#define CC_PF_KV_STAGES 4
+#endif
+constexpr int kKvStages = CC_PF_KV_STAGES;
+constexpr int kPBufs = 5 - kKvStages;        // probability buffers: what the K/V ring leaves of the 227 KiB
 constexpr int kQBytes = 2 * 2 * 128 * 128;   // Q: [hi | lo][half of Dh][128 rows][128 B]
 constexpr int kKvStageBytes = 2 * 2 * kKvTile * 128;   // [K | V][half of Dh][64 tokens][128 B]
 constexpr int kPBytes = 2 * 128 * 128;       // P: [hi | lo][128 rows][64 kv = 128 B]; two such buffers (tile parity)
-constexpr int kPfHdr = 1024;
-constexpr int kPfSmem = kPfHdr + kQBytes + kKvStages * kKvStageBytes + 2 * kPBytes;
+constexpr int kPfHdr = 3072;                 // barriers (1 KiB) + the softmax pairs' exchange of row maxima / sums (2 KiB)
+constexpr int kPfSmem = kPfHdr + kQBytes + kKvStages * kKvStageBytes + kPBufs * kPBytes;
 constexpr float kLazyLog2 = 8.f;             // O and l are rescaled only when a row maximum has grown by more than 2^8
 constexpr uint32_t kColS = 0, kColO = 128;   // TMEM columns: S buffers at 0 and 64, O at 128..255
 
@@ -77,6 +85,11 @@ struct Item {                 // one (chunk, query tile, kv head)
 };
 __device__ __forceinline__ bool item_at(const CcWork& W, const CcDims& D, const int* __restrict__ seq_lens, int id, Item& it) {
     const int n = W.bs->n_items * D.Hkv;
+    {   // rounds of gridDim.x items in decreasing cost, dealt forwards and backwards in turn: dealt forwards only, block 0
+        // would get the dearest item of every round and the last block the cheapest (11 % apart at cfg4)
+        const int grid = (int)gridDim.x, round = id / grid, idx = id - round * grid;
+        if (round & 1) id = round * grid + (grid - 1 - idx);
+    }
     if (id >= n) return false;
     const int k = id / D.Hkv, T = 128 / D.G;
     const int c = W.item_chunk[k], j = W.item_tile[k];
@@ -107,13 +120,13 @@ k_prefill_attn(const int* __restrict__ seq_lens, CcKv kv, CcDims D, CcWork W, co
         }
         for (int i = 0; i < 2; ++i) {
             mbar_init(&H->s_full[i], 1);
-            mbar_init(&H->s_free[i], 4);
+            mbar_init(&H->s_free[i], kSmWarps);
         }
         for (int i = 0; i < 2; ++i) {
-            mbar_init(&H->p_full[i], 4);
+            mbar_init(&H->p_full[i], kSmWarps);
             mbar_init(&H->pv_done[i], 1);
         }
-        mbar_init(&H->q_ready, 4);
+        mbar_init(&H->q_ready, kSmWarps);
         fence_mbar_init();
     }
     if (warp == 1) tmem_alloc<256>(&H->tmem_base);
@@ -177,8 +190,8 @@ k_prefill_attn(const int* __restrict__ seq_lens, CcKv kv, CcDims D, CcWork W, co
         Item it;
         auto issue_pv = [&](uint32_t gt, bool first) {
             const int stage = (int)(gt % kKvStages);
-            const uint32_t pb = n_pv & 1;
-            mbar_wait(&H->p_full[pb], (n_pv >> 1) & 1);
+            const uint32_t pb = n_pv % kPBufs;
+            mbar_wait(&H->p_full[pb], (n_pv / kPBufs) & 1);
             tc_fence_after();
             if (elect_one()) {
                 const uint32_t v_lo = (uint32_t)v_d0 + (((uint32_t)stage * kKvStageBytes) >> 4);
@@ -189,7 +202,7 @@ k_prefill_attn(const int* __restrict__ seq_lens, CcKv kv, CcDims D, CcWork W, co
                     umma_bf16_lo(tmem_base + kColO, p_lo + 2 * ks, v_lo + ks * 128, k_hi32, v_hi32, idesc_o, (first && ks == 0) ? 0u : 1u);
                     umma_bf16_lo(tmem_base + kColO, p_lo + 1024 + 2 * ks, v_lo + ks * 128, k_hi32, v_hi32, idesc_o, 1u);
                 }
-                umma_commit(&H->pv_done[pb]);
+                umma_commit(&H->pv_done[n_pv & 1]);
                 umma_commit(&H->kv_empty[stage]);
             }
             __syncwarp();
@@ -222,46 +235,46 @@ k_prefill_attn(const int* __restrict__ seq_lens, CcKv kv, CcDims D, CcWork W, co
             issue_pv(g - 1, it.n_tiles == 1);
         }
     } else {
-        // ===================== softmax warps: one query row per thread =====================
-        const int q4 = warp & 3;                                       // TMEM lane quarter of this warp
+        // ===================== softmax warps: one query row per thread, the tile's 64 columns shared by two warps =====================
+        const int q4 = warp & 3;                                       // TMEM lane quarter of this warp (fixed by the hardware: warp % 4)
+        const int half = (warp - 2) >> 2;                              // columns 32 half .. 32 half + 31 of every score tile, 64 half .. of O
         const int m = q4 * 32 + lane;                                  // row of the tile: token m / G, q head m % G
         const uint32_t lane_addr = tmem_base + ((uint32_t)(q4 * 32) << 16);
+        float* xch = reinterpret_cast<float*>(smem_raw + 1024);        // [tile parity][half][128 rows]: the pair's row maxima (and row sums)
         uint32_t g = 0, n_pv = 0;
         Item it;
         for (int id = blockIdx.x; item_at(W, D, seq_lens, id, it); id += gridDim.x) {
             // ---- Q of the item: q_rot rows (fp32, post-RoPE) x log2(e)/sqrt(Dh) -> bf16 hi + lo operand planes ----
-            // one row per warp iteration, 512 B coalesced; sixteen rows' loads in flight together (one at a time, the two
-            // dependent global loads of every row cost the item ~20 us during which the tensor pipe has nothing to do)
-            constexpr int kQB = 16;
+            // One row per warp iteration, 512 B coalesced, eight rows' loads in flight.  The rows of a chunk are consecutive
+            // in their replica group (stable partition), so one table read gives all their grouped positions.
+            {
+                const int pos0 = W.pos_of[it.row0];
+                constexpr int kQB = 8;
 #pragma unroll 1
-            for (int rb = 0; rb < 32; rb += kQB) {
-                float4 x[kQB];
-                int pos[kQB];
+                for (int rb = 0; rb < 128 / kSmWarps; rb += kQB) {
+                    float4 x[kQB];
 #pragma unroll
-                for (int u = 0; u < kQB; ++u) {
-                    const int r = (warp - 2) + 4 * (rb + u), tl = r / G;
-                    pos[u] = tl < it.n_tok ? W.pos_of[it.row0 + tl] : -1;
-                }
+                    for (int u = 0; u < kQB; ++u) {
+                        const int r = (warp - 2) + kSmWarps * (rb + u), tl = r / G, gq = r - tl * G;
+                        x[u] = make_float4(0.f, 0.f, 0.f, 0.f);
+                        if (tl < it.n_tok)
+                            x[u] = *reinterpret_cast<const float4*>(W.q_rot + (size_t)min(pos0 + tl, D.Mpad - 1) * D.QD +
+                                                                    (size_t)(it.h * G + gq) * 128 + 4 * lane);
+                    }
 #pragma unroll
-                for (int u = 0; u < kQB; ++u) {
-                    const int r = (warp - 2) + 4 * (rb + u), tl = r / G, gq = r - tl * G;
-                    x[u] = make_float4(0.f, 0.f, 0.f, 0.f);
-                    if (pos[u] >= 0)
-                        x[u] = *reinterpret_cast<const float4*>(W.q_rot + (size_t)pos[u] * D.QD + (size_t)(it.h * G + gq) * 128 + 4 * lane);
-                }
-#pragma unroll
-                for (int u = 0; u < kQB; ++u) {
-                    const int r = (warp - 2) + 4 * (rb + u);
-                    float4 v = x[u];
-                    v.x *= D.qk_scale_log2; v.y *= D.qk_scale_log2; v.z *= D.qk_scale_log2; v.w *= D.qk_scale_log2;
-                    uint32_t h0, l0, h1, l1;
-                    split_hilo(v.x, v.y, h0, l0);
-                    split_hilo(v.z, v.w, h1, l1);
-                    // dims 4 lane .. 4 lane + 3: half = lane / 16, 16-byte chunk (lane % 16) / 2, byte (lane & 1) * 8 inside it
-                    const uint32_t off = (uint32_t)(lane >> 4) * 16384u + (uint32_t)(r >> 3) * 1024u + (uint32_t)(r & 7) * 128u +
-                                         (uint32_t)((((lane & 15) >> 1) ^ (r & 7)) << 4) + (uint32_t)(lane & 1) * 8u;
-                    *reinterpret_cast<uint2*>(sQ + off) = make_uint2(h0, h1);
-                    *reinterpret_cast<uint2*>(sQ + 32768u + off) = make_uint2(l0, l1);
+                    for (int u = 0; u < kQB; ++u) {
+                        const int r = (warp - 2) + kSmWarps * (rb + u);
+                        float4 v = x[u];
+                        v.x *= D.qk_scale_log2; v.y *= D.qk_scale_log2; v.z *= D.qk_scale_log2; v.w *= D.qk_scale_log2;
+                        uint32_t h0, l0, h1, l1;
+                        split_hilo(v.x, v.y, h0, l0);
+                        split_hilo(v.z, v.w, h1, l1);
+                        // dims 4 lane .. 4 lane + 3: half = lane / 16, 16-byte chunk (lane % 16) / 2, byte (lane & 1) * 8 inside it
+                        const uint32_t off = (uint32_t)(lane >> 4) * 16384u + (uint32_t)(r >> 3) * 1024u + (uint32_t)(r & 7) * 128u +
+                                             (uint32_t)((((lane & 15) >> 1) ^ (r & 7)) << 4) + (uint32_t)(lane & 1) * 8u;
+                        *reinterpret_cast<uint2*>(sQ + off) = make_uint2(h0, h1);
+                        *reinterpret_cast<uint2*>(sQ + 32768u + off) = make_uint2(l0, l1);
+                    }
                 }
             }
             fence_proxy_async_smem();
@@ -269,41 +282,42 @@ k_prefill_attn(const int* __restrict__ seq_lens, CcKv kv, CcDims D, CcWork W, co
             if (lane == 0) mbar_arrive(&H->q_ready);
             const int tl = min(m / G, it.n_tok - 1);                   // padding rows take the last token's mask
             const int p_row = seq_lens[it.row0 + tl] - 1;              // kv positions 0 .. p_row are visible
-            float m_run = -INFINITY, l_run = 0.f;
+            float m_run = -INFINITY, l_run = 0.f;                      // l_run: the sum over THIS warp's columns
             for (int j = 0; j < it.n_tiles; ++j, ++g) {
                 const uint32_t sb = g & 1;
-                const int kv0 = j * kKvTile;
+                const int kv0 = j * kKvTile + half * 32;               // kv position of this warp's first column
                 mbar_wait(&H->s_full[sb], (g >> 1) & 1);
                 tc_fence_after();
-                uint32_t sv[2][32];
-                tmem_ld_32x32b_x32(lane_addr + kColS + sb * kKvTile, sv[0]);
-                tmem_ld_32x32b_x32(lane_addr + kColS + sb * kKvTile + 32, sv[1]);
+                uint32_t sv[32];
+                tmem_ld_32x32b_x32(lane_addr + kColS + sb * kKvTile + half * 32, sv);
                 tmem_ld_wait();
                 tc_fence_before();
                 __syncwarp();
                 if (lane == 0) mbar_arrive(&H->s_free[sb]);
                 float mx = -INFINITY;
-                const int lim = p_row - kv0;                           // columns 0 .. lim are visible
-                if (__all_sync(0xffffffffu, lim >= kKvTile - 1)) {     // not a diagonal tile of this warp's rows: no mask
+                const int lim = p_row - kv0;                           // columns 0 .. lim (of this warp's 32) are visible
+                if (__all_sync(0xffffffffu, lim >= 31)) {              // not on the diagonal for this warp's rows: no mask
 #pragma unroll
-                    for (int u = 0; u < 2; ++u)
-#pragma unroll
-                        for (int i = 0; i < 32; ++i) mx = fmaxf(mx, __uint_as_float(sv[u][i]));
+                    for (int i = 0; i < 32; ++i) mx = fmaxf(mx, __uint_as_float(sv[i]));
                 } else {
 #pragma unroll
-                    for (int u = 0; u < 2; ++u)
-#pragma unroll
-                        for (int i = 0; i < 32; ++i) {
-                            const float v = (u * 32 + i <= lim) ? __uint_as_float(sv[u][i]) : -INFINITY;
-                            sv[u][i] = __float_as_uint(v);
-                            mx = fmaxf(mx, v);
-                        }
+                    for (int i = 0; i < 32; ++i) {
+                        const float v = (i <= lim) ? __uint_as_float(sv[i]) : -INFINITY;
+                        sv[i] = __float_as_uint(v);
+                        mx = fmaxf(mx, v);
+                    }
                 }
+                // the row maximum over both halves: through shared memory, one named barrier per pair of warps and tile
+                float* xm = xch + (g & 1) * 256;
+                xm[half * 128 + m] = mx;
+                named_bar_sync(1 + q4, 64);
+                mx = fmaxf(mx, xm[(half ^ 1) * 128 + m]);
                 // Lazy rescale: the probabilities are taken against a reference m_run that follows the running maximum only
                 // when that has grown by more than 2^kLazyLog2 in some row of the warp (p <= 2^8: harmless in fp32 / bf16
-                // hi + lo).  Then O (the warp's 32 TMEM lanes) and l are rescaled, which needs every P V product issued so
-                // far to be complete; otherwise this tile's probabilities go into the other P buffer while the previous
-                // product still runs.  A function of the data only.
+                // hi + lo).  Then O (this warp's half of the columns of its 32 TMEM lanes) and l are rescaled, which needs
+                // every P V product issued so far to be complete; otherwise this tile's probabilities go into the other P
+                // buffer while the previous product still runs.  Both warps of a pair see the same maxima, hence take the
+                // same decision; it is a function of the data only.
                 const float m_seen = fmaxf(m_run, mx);                 // finite from tile 0 on: position 0 is visible to every row
                 float alpha = 1.f;
                 if (j == 0) {
@@ -314,7 +328,7 @@ k_prefill_attn(const int* __restrict__ seq_lens, CcKv kv, CcDims D, CcWork W, co
                     alpha = exp2f(m_run - m_seen);
                     m_run = m_seen;
 #pragma unroll 1
-                    for (int c = 0; c < 128; c += 32) {
+                    for (int c = half * 64; c < half * 64 + 64; c += 32) {
                         uint32_t ov[32];
                         tmem_ld_32x32b_x32(lane_addr + kColO + c, ov);
                         tmem_ld_wait();
@@ -325,14 +339,15 @@ k_prefill_attn(const int* __restrict__ seq_lens, CcKv kv, CcDims D, CcWork W, co
                     tmem_st_wait();
                 }
                 const float m_new = m_run;
-                const uint32_t pb = n_pv & 1;
-                if (n_pv >= 2) mbar_wait(&H->pv_done[pb], ((n_pv - 2) >> 1) & 1);    // the product that read this P buffer is done
-                if (j == it.n_tiles - 1 && it.s_last < kv0 + kKvTile) {
+                const uint32_t pb = n_pv % kPBufs;
+                if (n_pv >= (uint32_t)kPBufs)                          // the product that read this P buffer is done
+                    mbar_wait(&H->pv_done[(n_pv - kPBufs) & 1], ((n_pv - kPBufs) >> 1) & 1);
+                if (j == it.n_tiles - 1 && it.s_last < j * kKvTile + kKvTile) {
                     // ragged last tile: V rows past the last position hold other data (or nothing): p = 0 must meet 0
                     mbar_wait(&H->kv_full[g % kKvStages], (g / kKvStages) & 1);
                     uint8_t* sV = sKV + (size_t)(g % kKvStages) * kKvStageBytes + 16384;
-                    const int first = it.s_last - kv0;
-                    for (int q = (warp - 2) * 32 + lane; q < (kKvTile - first) * 16; q += 128) {
+                    const int first = it.s_last - j * kKvTile;
+                    for (int q = (warp - 2) * 32 + lane; q < (kKvTile - first) * 16; q += kSmWarps * 32) {
                         const int r = first + (q >> 4), c = q & 15;    // row r, 16-byte chunk c of its 256 bytes
                         *reinterpret_cast<uint4*>(sV + (c >> 3) * 8192 + r * 128 + ((c & 7) << 4)) = make_uint4(0, 0, 0, 0);
                     }
@@ -340,21 +355,19 @@ k_prefill_attn(const int* __restrict__ seq_lens, CcKv kv, CcDims D, CcWork W, co
                 float lsum = 0.f;
                 uint8_t* prow = sP + pb * (uint32_t)kPBytes + (uint32_t)(m >> 3) * 1024u + (uint32_t)(m & 7) * 128u;
 #pragma unroll
-                for (int u = 0; u < 2; ++u)
+                for (int c8 = 0; c8 < 4; ++c8) {                       // 8 probabilities = one 16-byte chunk per plane
+                    uint32_t hi[4], lo[4];
 #pragma unroll
-                    for (int c8 = 0; c8 < 4; ++c8) {                   // 8 probabilities = one 16-byte chunk per plane
-                        uint32_t hi[4], lo[4];
-#pragma unroll
-                        for (int i = 0; i < 4; ++i) {
-                            const float p0 = exp2f(__uint_as_float(sv[u][c8 * 8 + 2 * i]) - m_new);
-                            const float p1 = exp2f(__uint_as_float(sv[u][c8 * 8 + 2 * i + 1]) - m_new);
-                            lsum += p0 + p1;
-                            split_hilo(p0, p1, hi[i], lo[i]);
-                        }
-                        const uint32_t ch = (uint32_t)(((u * 4 + c8) ^ (m & 7)) << 4);
-                        *reinterpret_cast<uint4*>(prow + ch) = make_uint4(hi[0], hi[1], hi[2], hi[3]);
-                        *reinterpret_cast<uint4*>(prow + 16384u + ch) = make_uint4(lo[0], lo[1], lo[2], lo[3]);
+                    for (int i = 0; i < 4; ++i) {
+                        const float p0 = exp2f(__uint_as_float(sv[c8 * 8 + 2 * i]) - m_new);
+                        const float p1 = exp2f(__uint_as_float(sv[c8 * 8 + 2 * i + 1]) - m_new);
+                        lsum += p0 + p1;
+                        split_hilo(p0, p1, hi[i], lo[i]);
                     }
+                    const uint32_t ch = (uint32_t)(((half * 4 + c8) ^ (m & 7)) << 4);
+                    *reinterpret_cast<uint4*>(prow + ch) = make_uint4(hi[0], hi[1], hi[2], hi[3]);
+                    *reinterpret_cast<uint4*>(prow + 16384u + ch) = make_uint4(lo[0], lo[1], lo[2], lo[3]);
+                }
                 l_run = l_run * alpha + lsum;
                 fence_proxy_async_smem();
                 tc_fence_before();
@@ -362,7 +375,14 @@ k_prefill_attn(const int* __restrict__ seq_lens, CcKv kv, CcDims D, CcWork W, co
                 if (lane == 0) mbar_arrive(&H->p_full[pb]);
                 ++n_pv;
             }
-            // ---- the item's rows: O / l -> the O-projection operand ----
+            // ---- the item's rows: O / l -> the O-projection operand; this warp writes its 64 columns ----
+            {
+                // the row sums of the two halves, added in half order; the parity buffer the last tile did not use
+                float* xl = xch + (g & 1) * 256;
+                xl[half * 128 + m] = l_run;
+                named_bar_sync(1 + q4, 64);
+                l_run = xl[m] + xl[128 + m];
+            }
             mbar_wait(&H->pv_done[(n_pv - 1) & 1], ((n_pv - 1) >> 1) & 1);
             tc_fence_after();
             const int tlr = m / G, gq = m - tlr * G;
@@ -370,7 +390,7 @@ k_prefill_attn(const int* __restrict__ seq_lens, CcKv kv, CcDims D, CcWork W, co
             const int pos = live ? W.pos_of[it.row0 + tlr] : 0;
             const float inv = 1.f / l_run;
 #pragma unroll 1
-            for (int c = 0; c < 128; c += 32) {
+            for (int c = half * 64; c < half * 64 + 64; c += 32) {
                 uint32_t ov[32];
                 tmem_ld_32x32b_x32(lane_addr + kColO + c, ov);
                 tmem_ld_wait();
