@@ -8,15 +8,16 @@
 //   * work item = (chunk, query tile of T = 128 / G tokens, kv head): the G query heads of the T tokens are the 128
 //     rows of the MMA (row m = token m / G, head m % G), so one K/V read serves the GQA group and T tokens;
 //   * the kv axis is walked in tiles of 64 tokens (4 pages): a producer warp stages the head's K and V of each page
-//     by TMA (boxes of 16 rows x 128 B, 128-byte swizzle, straight into the operand layout), ring of three stages;
+//     by TMA (boxes of 16 rows x 128 B, 128-byte swizzle, straight into the operand layout), ring of five stages;
 //   * S = Q K^T (M 128, N 64, K 128) and O += P V (M 128, N 128, K 64) are tcgen05.mma into TMEM (S double
 //     buffered, O resident); K is the K-major B operand, V the MN-major one (no transpose anywhere);
 //   * eight softmax warps, one query row per thread (TMEM lane = row) and two warps per lane quarter that share a tile's 64
 //     columns (row maxima and sums meet through shared memory, one named barrier per pair and tile): tcgen05.ld of the
 //     scores, causal mask on the diagonal tiles only, online softmax in log2 units against a reference maximum that
-//     follows the running one only when that grew by more than 2^8 (then O is rescaled in TMEM), probabilities written
-//     to one of two shared-memory buffers as the A operand of the P V product, so the softmax of tile j + 1 runs while
-//     the product of tile j does;
+//     follows the running one only when that grew by more than 2^8 (then O is rescaled in TMEM); the probabilities
+//     OVERWRITE the tile's scores in tensor memory (tcgen05.st, bf16 pairs) and are the A operand of the P V product
+//     from there (no shared memory, no proxy fence), so the softmax of tile j + 1 runs while the product of tile j does;
+//   * the Q rows of the next item are requested before the epilogue of the current one;
 //   * q and the probabilities enter as bf16 hi + lo planes (two MMAs each) like in the decode kernel: the K/V are
 //     bf16 by definition, and a single bf16 plane of q or p costs 2e-3 on the attention output;
 //   * items are dealt round-robin in decreasing cost; every row is finished by one item in one fixed order, so the
@@ -28,23 +29,19 @@ namespace {
 constexpr int kSmWarps = 8;                  // softmax warps: two per TMEM lane quarter, each takes half of a tile's columns
 constexpr int kPfThreads = (2 + kSmWarps) * 32;   // warp 0 producer, warp 1 MMA issuer, warps 2..9 softmax (TMEM lane quarter = warp % 4)
 constexpr int kKvTile = 64;                  // kv tokens per tile (4 pages)
-#ifndef CC_PF_KV_STAGES
-#define CC_PF_KV_STAGES 4
-#endif
-constexpr int kKvStages = CC_PF_KV_STAGES;
-constexpr int kPBufs = 5 - kKvStages;        // probability buffers: what the K/V ring leaves of the 227 KiB
+constexpr int kKvStages = 5;                 // what Q leaves of the 227 KiB (the probabilities live in TMEM)
 constexpr int kQBytes = 2 * 2 * 128 * 128;   // Q: [hi | lo][half of Dh][128 rows][128 B]
 constexpr int kKvStageBytes = 2 * 2 * kKvTile * 128;   // [K | V][half of Dh][64 tokens][128 B]
-constexpr int kPBytes = 2 * 128 * 128;       // P: [hi | lo][128 rows][64 kv = 128 B]; two such buffers (tile parity)
 constexpr int kPfHdr = 3072;                 // barriers (1 KiB) + the softmax pairs' exchange of row maxima / sums (2 KiB)
-constexpr int kPfSmem = kPfHdr + kQBytes + kKvStages * kKvStageBytes + kPBufs * kPBytes;
+constexpr int kPfSmem = kPfHdr + kQBytes + kKvStages * kKvStageBytes;
 constexpr float kLazyLog2 = 8.f;             // O and l are rescaled only when a row maximum has grown by more than 2^8
-constexpr uint32_t kColS = 0, kColO = 128;   // TMEM columns: S buffers at 0 and 64, O at 128..255
+constexpr uint32_t kColS = 0, kColO = 128;   // TMEM columns: S buffers at 0 and 64, O at 128..255.  The probabilities of a tile
+                                             // overwrite its scores: bf16 pairs, hi plane in columns 0..31 of the buffer, lo in 32..63
 
 struct PfHdr {
     uint64_t kv_full[kKvStages], kv_empty[kKvStages];
     uint64_t s_full[2], s_free[2];
-    uint64_t p_full[2], pv_done[2], q_ready;      // [P buffer = kv tile parity]
+    uint64_t p_full[2], pv_done[2], q_ready;      // [kv tile parity]
     uint32_t tmem_base;
 };
 
@@ -73,7 +70,33 @@ __device__ __forceinline__ void tmem_st_32x32b_x32(uint32_t taddr, const uint32_
         "r"(r[31])
         : "memory");
 }
+// 2^x by the special-function unit alone (exp2f adds a range fix-up of three instructions per value; what it would fix --
+// results below 2^-126 -- is zero against a row sum of at least 1 here)
+__device__ __forceinline__ float ex2_ftz(float x) {
+    float y;
+    asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+    return y;
+}
 __device__ __forceinline__ void tmem_st_wait() { asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory"); }
+__device__ __forceinline__ void tmem_st_32x32b_x16(uint32_t taddr, const uint32_t (&r)[16]) {
+    asm volatile(
+        "tcgen05.st.sync.aligned.32x32b.x16.b32 [%0], {%1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15, %16};" ::"r"(taddr),
+        "r"(r[0]), "r"(r[1]), "r"(r[2]), "r"(r[3]), "r"(r[4]), "r"(r[5]), "r"(r[6]), "r"(r[7]), "r"(r[8]), "r"(r[9]), "r"(r[10]),
+        "r"(r[11]), "r"(r[12]), "r"(r[13]), "r"(r[14]), "r"(r[15])
+        : "memory");
+}
+// D += A B with the A operand in TENSOR MEMORY (lane = row, 32-bit column c = the bf16 pair k = 2c, 2c + 1 of the row: 8 columns
+// per MMA of K = 16) and B through a shared-memory descriptor: no shared-memory read for A, no proxy fence for its writer.
+__device__ __forceinline__ void umma_bf16_ts(uint32_t d_tmem, uint32_t a_tmem, uint32_t b_lo, uint32_t b_hi, uint32_t idesc,
+                                             uint32_t accumulate) {
+    asm volatile(
+        "{\n\t.reg .pred p;\n\t.reg .b64 db;\n\t"
+        "setp.ne.b32 p, %5, 0;\n\t"
+        "mov.b64 db, {%2, %3};\n\t"
+        "tcgen05.mma.cta_group::1.kind::f16 [%0], [%1], db, %4, p;\n\t}" ::"r"(d_tmem),
+        "r"(a_tmem), "r"(b_lo), "r"(b_hi), "r"(idesc), "r"(accumulate)
+        : "memory");
+}
 
 struct Item {                 // one (chunk, query tile, kv head)
     int row0;                 // original row of the tile's first token
@@ -109,7 +132,6 @@ k_prefill_attn(const int* __restrict__ seq_lens, CcKv kv, CcDims D, CcWork W, co
     PfHdr* H = reinterpret_cast<PfHdr*>(smem_raw);
     uint8_t* sQ = smem_raw + kPfHdr;
     uint8_t* sKV = sQ + kQBytes;
-    uint8_t* sP = sKV + kKvStages * kKvStageBytes;
     const int warp = uniform((int)(threadIdx.x >> 5)), lane = threadIdx.x & 31;
     const int G = D.G;
 
@@ -183,24 +205,23 @@ k_prefill_attn(const int* __restrict__ seq_lens, CcKv kv, CcDims D, CcWork W, co
         // ===================== MMA issuer =====================
         const uint32_t idesc_s = idesc_bf16(kKvTile, false), idesc_o = idesc_bf16(128, true);
         const uint32_t q_lo = (uint32_t)umma_desc_sw128(smem_u32(sQ)), k_hi32 = (uint32_t)(umma_desc_sw128(0) >> 32);
-        const uint32_t p_lo0 = (uint32_t)umma_desc_sw128(smem_u32(sP));
         const uint64_t v_d0 = umma_desc_sw128_lbo(smem_u32(sKV) + 16384u, 8192u, 1024u);
         const uint32_t v_hi32 = (uint32_t)(v_d0 >> 32);
         uint32_t g = 0, n_pv = 0, n_item = 0;
         Item it;
         auto issue_pv = [&](uint32_t gt, bool first) {
             const int stage = (int)(gt % kKvStages);
-            const uint32_t pb = n_pv % kPBufs;
-            mbar_wait(&H->p_full[pb], (n_pv / kPBufs) & 1);
+            const uint32_t pb = n_pv & 1;                              // = the tile's score buffer
+            mbar_wait(&H->p_full[pb], (n_pv >> 1) & 1);
             tc_fence_after();
             if (elect_one()) {
                 const uint32_t v_lo = (uint32_t)v_d0 + (((uint32_t)stage * kKvStageBytes) >> 4);
-                const uint32_t p_lo = p_lo0 + pb * (kPBytes >> 4);
+                const uint32_t p_t = tmem_base + kColS + pb * kKvTile;   // hi pairs at + 0, lo pairs at + 32
 #pragma unroll
                 for (int ks = 0; ks < kKvTile / 16; ++ks) {
-                    // A: P plane (K-major, 16 kv = 32 B per step); B: V, MN-major, 16 kv rows = 2 KiB per step
-                    umma_bf16_lo(tmem_base + kColO, p_lo + 2 * ks, v_lo + ks * 128, k_hi32, v_hi32, idesc_o, (first && ks == 0) ? 0u : 1u);
-                    umma_bf16_lo(tmem_base + kColO, p_lo + 1024 + 2 * ks, v_lo + ks * 128, k_hi32, v_hi32, idesc_o, 1u);
+                    // A: P plane in TMEM (16 kv = 8 columns per step); B: V, MN-major, 16 kv rows = 2 KiB per step
+                    umma_bf16_ts(tmem_base + kColO, p_t + 8 * ks, v_lo + ks * 128, v_hi32, idesc_o, (first && ks == 0) ? 0u : 1u);
+                    umma_bf16_ts(tmem_base + kColO, p_t + 32 + 8 * ks, v_lo + ks * 128, v_hi32, idesc_o, 1u);
                 }
                 umma_commit(&H->pv_done[n_pv & 1]);
                 umma_commit(&H->kv_empty[stage]);
@@ -243,39 +264,42 @@ k_prefill_attn(const int* __restrict__ seq_lens, CcKv kv, CcDims D, CcWork W, co
         float* xch = reinterpret_cast<float*>(smem_raw + 1024);        // [tile parity][half][128 rows]: the pair's row maxima (and row sums)
         uint32_t g = 0, n_pv = 0;
         Item it;
-        for (int id = blockIdx.x; item_at(W, D, seq_lens, id, it); id += gridDim.x) {
-            // ---- Q of the item: q_rot rows (fp32, post-RoPE) x log2(e)/sqrt(Dh) -> bf16 hi + lo operand planes ----
-            // One row per warp iteration, 512 B coalesced, eight rows' loads in flight.  The rows of a chunk are consecutive
-            // in their replica group (stable partition), so one table read gives all their grouped positions.
-            {
-                const int pos0 = W.pos_of[it.row0];
-                constexpr int kQB = 8;
-#pragma unroll 1
-                for (int rb = 0; rb < 128 / kSmWarps; rb += kQB) {
-                    float4 x[kQB];
+        // The sixteen Q rows this warp stages per item (q_rot, fp32, post-RoPE) are requested one item ahead: the loads of
+        // item i + 1 are issued before the epilogue of item i and used after it (one row at a time they cost an item ~20 us,
+        // in two batches after the epilogue still ~4 us during which the tensor pipe has nothing to do).  The rows of a
+        // chunk are consecutive in their replica group (stable partition), so one table read gives all their positions.
+        constexpr int kQR = 128 / kSmWarps;
+        float4 xq[kQR];
+        auto load_q = [&](const Item& t) {
+            const int pos0 = W.pos_of[t.row0];
 #pragma unroll
-                    for (int u = 0; u < kQB; ++u) {
-                        const int r = (warp - 2) + kSmWarps * (rb + u), tl = r / G, gq = r - tl * G;
-                        x[u] = make_float4(0.f, 0.f, 0.f, 0.f);
-                        if (tl < it.n_tok)
-                            x[u] = *reinterpret_cast<const float4*>(W.q_rot + (size_t)min(pos0 + tl, D.Mpad - 1) * D.QD +
-                                                                    (size_t)(it.h * G + gq) * 128 + 4 * lane);
-                    }
+            for (int u = 0; u < kQR; ++u) {
+                const int r = (warp - 2) + kSmWarps * u, tl = r / G, gq = r - tl * G;
+                xq[u] = make_float4(0.f, 0.f, 0.f, 0.f);
+                if (tl < t.n_tok)
+                    xq[u] = *reinterpret_cast<const float4*>(W.q_rot + (size_t)min(pos0 + tl, D.Mpad - 1) * D.QD +
+                                                             (size_t)(t.h * G + gq) * 128 + 4 * lane);
+            }
+        };
+        Item nx;
+        int id = blockIdx.x;
+        bool have = item_at(W, D, seq_lens, id, it);
+        if (have) load_q(it);
+        for (; have; id += gridDim.x, it = nx) {
+            // ---- Q of the item: x log2(e)/sqrt(Dh) -> bf16 hi + lo operand planes ----
 #pragma unroll
-                    for (int u = 0; u < kQB; ++u) {
-                        const int r = (warp - 2) + kSmWarps * (rb + u);
-                        float4 v = x[u];
-                        v.x *= D.qk_scale_log2; v.y *= D.qk_scale_log2; v.z *= D.qk_scale_log2; v.w *= D.qk_scale_log2;
-                        uint32_t h0, l0, h1, l1;
-                        split_hilo(v.x, v.y, h0, l0);
-                        split_hilo(v.z, v.w, h1, l1);
-                        // dims 4 lane .. 4 lane + 3: half = lane / 16, 16-byte chunk (lane % 16) / 2, byte (lane & 1) * 8 inside it
-                        const uint32_t off = (uint32_t)(lane >> 4) * 16384u + (uint32_t)(r >> 3) * 1024u + (uint32_t)(r & 7) * 128u +
-                                             (uint32_t)((((lane & 15) >> 1) ^ (r & 7)) << 4) + (uint32_t)(lane & 1) * 8u;
-                        *reinterpret_cast<uint2*>(sQ + off) = make_uint2(h0, h1);
-                        *reinterpret_cast<uint2*>(sQ + 32768u + off) = make_uint2(l0, l1);
-                    }
-                }
+            for (int u = 0; u < kQR; ++u) {
+                const int r = (warp - 2) + kSmWarps * u;
+                float4 v = xq[u];
+                v.x *= D.qk_scale_log2; v.y *= D.qk_scale_log2; v.z *= D.qk_scale_log2; v.w *= D.qk_scale_log2;
+                uint32_t h0, l0, h1, l1;
+                split_hilo(v.x, v.y, h0, l0);
+                split_hilo(v.z, v.w, h1, l1);
+                // dims 4 lane .. 4 lane + 3: half = lane / 16, 16-byte chunk (lane % 16) / 2, byte (lane & 1) * 8 inside it
+                const uint32_t off = (uint32_t)(lane >> 4) * 16384u + (uint32_t)(r >> 3) * 1024u + (uint32_t)(r & 7) * 128u +
+                                     (uint32_t)((((lane & 15) >> 1) ^ (r & 7)) << 4) + (uint32_t)(lane & 1) * 8u;
+                *reinterpret_cast<uint2*>(sQ + off) = make_uint2(h0, h1);
+                *reinterpret_cast<uint2*>(sQ + 32768u + off) = make_uint2(l0, l1);
             }
             fence_proxy_async_smem();
             __syncwarp();
@@ -339,9 +363,8 @@ k_prefill_attn(const int* __restrict__ seq_lens, CcKv kv, CcDims D, CcWork W, co
                     tmem_st_wait();
                 }
                 const float m_new = m_run;
-                const uint32_t pb = n_pv % kPBufs;
-                if (n_pv >= (uint32_t)kPBufs)                          // the product that read this P buffer is done
-                    mbar_wait(&H->pv_done[(n_pv - kPBufs) & 1], ((n_pv - kPBufs) >> 1) & 1);
+                const uint32_t pb = n_pv & 1;                          // == sb: the probabilities replace the tile's scores (both
+                                                                       // warps of the pair have theirs in registers: the barrier above)
                 if (j == it.n_tiles - 1 && it.s_last < j * kKvTile + kKvTile) {
                     // ragged last tile: V rows past the last position hold other data (or nothing): p = 0 must meet 0
                     mbar_wait(&H->kv_full[g % kKvStages], (g / kKvStages) & 1);
@@ -353,28 +376,26 @@ k_prefill_attn(const int* __restrict__ seq_lens, CcKv kv, CcDims D, CcWork W, co
                     }
                 }
                 float lsum = 0.f;
-                uint8_t* prow = sP + pb * (uint32_t)kPBytes + (uint32_t)(m >> 3) * 1024u + (uint32_t)(m & 7) * 128u;
+                uint32_t hi[16], lo[16];                               // this warp's 32 kv columns as bf16 pairs
 #pragma unroll
-                for (int c8 = 0; c8 < 4; ++c8) {                       // 8 probabilities = one 16-byte chunk per plane
-                    uint32_t hi[4], lo[4];
-#pragma unroll
-                    for (int i = 0; i < 4; ++i) {
-                        const float p0 = exp2f(__uint_as_float(sv[c8 * 8 + 2 * i]) - m_new);
-                        const float p1 = exp2f(__uint_as_float(sv[c8 * 8 + 2 * i + 1]) - m_new);
-                        lsum += p0 + p1;
-                        split_hilo(p0, p1, hi[i], lo[i]);
-                    }
-                    const uint32_t ch = (uint32_t)(((half * 4 + c8) ^ (m & 7)) << 4);
-                    *reinterpret_cast<uint4*>(prow + ch) = make_uint4(hi[0], hi[1], hi[2], hi[3]);
-                    *reinterpret_cast<uint4*>(prow + 16384u + ch) = make_uint4(lo[0], lo[1], lo[2], lo[3]);
+                for (int i = 0; i < 16; ++i) {
+                    const float p0 = ex2_ftz(__uint_as_float(sv[2 * i]) - m_new);
+                    const float p1 = ex2_ftz(__uint_as_float(sv[2 * i + 1]) - m_new);
+                    lsum += p0 + p1;
+                    split_hilo(p0, p1, hi[i], lo[i]);
                 }
+                tmem_st_32x32b_x16(lane_addr + kColS + pb * kKvTile + half * 16, hi);
+                tmem_st_32x32b_x16(lane_addr + kColS + pb * kKvTile + 32 + half * 16, lo);
+                tmem_st_wait();
                 l_run = l_run * alpha + lsum;
-                fence_proxy_async_smem();
+                if (j == it.n_tiles - 1 && it.s_last < j * kKvTile + kKvTile) fence_proxy_async_smem();   // the zeroed V rows
                 tc_fence_before();
                 __syncwarp();
                 if (lane == 0) mbar_arrive(&H->p_full[pb]);
                 ++n_pv;
             }
+            have = item_at(W, D, seq_lens, id + (int)gridDim.x, nx);
+            if (have) load_q(nx);                                      // in flight during the epilogue below
             // ---- the item's rows: O / l -> the O-projection operand; this warp writes its 64 columns ----
             {
                 // the row sums of the two halves, added in half order; the parity buffer the last tile did not use
