@@ -9,8 +9,8 @@
 //     rows of the MMA (row m = token m / G, head m % G), so one K/V read serves the GQA group and T tokens;
 //   * the kv axis is walked in tiles of 64 tokens (4 pages): a producer warp stages the head's K and V of each page
 //     by TMA (boxes of 16 rows x 128 B, 128-byte swizzle, straight into the operand layout), ring of five stages;
-//   * S = Q K^T (M 128, N 64, K 128) and O += P V (M 128, N 128, K 64) are tcgen05.mma into TMEM (S double
-//     buffered, O resident); K is the K-major B operand, V the MN-major one (no transpose anywhere);
+//   * S = Q K^T (M 128, N 64, K 128) and O += P V (M 128, N 128, K 64) are tcgen05.mma into TMEM (three S
+//     buffers: the scores run two tiles ahead of the products; O resident); K is the K-major B operand, V the MN-major one (no transpose anywhere);
 //   * eight softmax warps, one query row per thread (TMEM lane = row) and two warps per lane quarter that share a tile's 64
 //     columns (row maxima and sums meet through shared memory, one named barrier per pair and tile): tcgen05.ld of the
 //     scores, causal mask on the diagonal tiles only, online softmax in log2 units against a reference maximum that
@@ -35,13 +35,14 @@ constexpr int kKvStageBytes = 2 * 2 * kKvTile * 128;   // [K | V][half of Dh][64
 constexpr int kPfHdr = 3072;                 // barriers (1 KiB) + the softmax pairs' exchange of row maxima / sums (2 KiB)
 constexpr int kPfSmem = kPfHdr + kQBytes + kKvStages * kKvStageBytes;
 constexpr float kLazyLog2 = 8.f;             // O and l are rescaled only when a row maximum has grown by more than 2^8
-constexpr uint32_t kColS = 0, kColO = 128;   // TMEM columns: S buffers at 0 and 64, O at 128..255.  The probabilities of a tile
+constexpr int kSBufs = 3;                    // score / probability buffers: Q K^T runs two tiles ahead of P V
+constexpr uint32_t kColS = 0, kColO = 192;   // TMEM columns: S buffers at 0, 64, 128, O at 192..319.  The probabilities of a tile
                                              // overwrite its scores: bf16 pairs, hi plane in columns 0..31 of the buffer, lo in 32..63
 
 struct PfHdr {
     uint64_t kv_full[kKvStages], kv_empty[kKvStages];
-    uint64_t s_full[2], s_free[2];
-    uint64_t p_full[2], pv_done[2], q_ready;      // [kv tile parity]
+    uint64_t s_full[kSBufs], p_full[kSBufs];      // [score buffer = kv tile % 3]
+    uint64_t pv_done[2], q_ready;                 // pv_done: [kv tile parity]
     uint32_t tmem_base;
 };
 
@@ -140,18 +141,15 @@ k_prefill_attn(const int* __restrict__ seq_lens, CcKv kv, CcDims D, CcWork W, co
             mbar_init(&H->kv_full[i], 1);
             mbar_init(&H->kv_empty[i], 1);
         }
-        for (int i = 0; i < 2; ++i) {
+        for (int i = 0; i < kSBufs; ++i) {
             mbar_init(&H->s_full[i], 1);
-            mbar_init(&H->s_free[i], kSmWarps);
-        }
-        for (int i = 0; i < 2; ++i) {
             mbar_init(&H->p_full[i], kSmWarps);
-            mbar_init(&H->pv_done[i], 1);
         }
+        for (int i = 0; i < 2; ++i) mbar_init(&H->pv_done[i], 1);
         mbar_init(&H->q_ready, kSmWarps);
         fence_mbar_init();
     }
-    if (warp == 1) tmem_alloc<256>(&H->tmem_base);
+    if (warp == 1) tmem_alloc<512>(&H->tmem_base);
     tc_fence_before();
     __syncthreads();
     tc_fence_after();
@@ -207,53 +205,60 @@ k_prefill_attn(const int* __restrict__ seq_lens, CcKv kv, CcDims D, CcWork W, co
         const uint32_t q_lo = (uint32_t)umma_desc_sw128(smem_u32(sQ)), k_hi32 = (uint32_t)(umma_desc_sw128(0) >> 32);
         const uint64_t v_d0 = umma_desc_sw128_lbo(smem_u32(sKV) + 16384u, 8192u, 1024u);
         const uint32_t v_hi32 = (uint32_t)(v_d0 >> 32);
-        uint32_t g = 0, n_pv = 0, n_item = 0;
+        uint32_t g = 0, n_item = 0;                                    // g: kv tiles of the items before this one
         Item it;
+        // The tensor pipe executes in issue order, and the order below is S(0) S(1) | PV(0) S(2) | PV(1) S(3) | ...: the scores of a
+        // tile are ready two softmax periods before they are needed, and S(j + 2), which overwrites the buffer of P(j - 1), is
+        // issued behind PV(j - 1) -- no "buffer free" barrier.
+        auto issue_s = [&](uint32_t gt) {
+            const int stage = (int)(gt % kKvStages);
+            const uint32_t sb = gt % kSBufs;
+            mbar_wait(&H->kv_full[stage], (gt / kKvStages) & 1);
+            tc_fence_after();
+            if (elect_one()) {
+                const uint32_t k_lo = (uint32_t)umma_desc_sw128(smem_u32(sKV) + (uint32_t)stage * kKvStageBytes);
+                const uint32_t d = tmem_base + kColS + sb * kKvTile;
+#pragma unroll
+                for (int ks = 0; ks < 8; ++ks) {
+                    // Q: [plane][half][128 rows][128 B] -> half = ks / 4 at + 16 KiB, 32 B per step; K: halves 8 KiB apart
+                    const uint32_t qa = q_lo + (uint32_t)(ks >> 2) * 1024 + 2 * (ks & 3);
+                    const uint32_t kb = k_lo + (uint32_t)(ks >> 2) * 512 + 2 * (ks & 3);
+                    umma_bf16_lo(d, qa, kb, k_hi32, k_hi32, idesc_s, ks == 0 ? 0u : 1u);
+                    umma_bf16_lo(d, qa + 2048, kb, k_hi32, k_hi32, idesc_s, 1u);       // the lo plane of q, 32 KiB further
+                }
+                umma_commit(&H->s_full[sb]);
+            }
+            __syncwarp();
+        };
         auto issue_pv = [&](uint32_t gt, bool first) {
             const int stage = (int)(gt % kKvStages);
-            const uint32_t pb = n_pv & 1;                              // = the tile's score buffer
-            mbar_wait(&H->p_full[pb], (n_pv >> 1) & 1);
+            const uint32_t sb = gt % kSBufs;                           // the probabilities replaced the tile's scores
+            mbar_wait(&H->p_full[sb], (gt / kSBufs) & 1);
             tc_fence_after();
             if (elect_one()) {
                 const uint32_t v_lo = (uint32_t)v_d0 + (((uint32_t)stage * kKvStageBytes) >> 4);
-                const uint32_t p_t = tmem_base + kColS + pb * kKvTile;   // hi pairs at + 0, lo pairs at + 32
+                const uint32_t p_t = tmem_base + kColS + sb * kKvTile;   // hi pairs at + 0, lo pairs at + 32
 #pragma unroll
                 for (int ks = 0; ks < kKvTile / 16; ++ks) {
                     // A: P plane in TMEM (16 kv = 8 columns per step); B: V, MN-major, 16 kv rows = 2 KiB per step
                     umma_bf16_ts(tmem_base + kColO, p_t + 8 * ks, v_lo + ks * 128, v_hi32, idesc_o, (first && ks == 0) ? 0u : 1u);
                     umma_bf16_ts(tmem_base + kColO, p_t + 32 + 8 * ks, v_lo + ks * 128, v_hi32, idesc_o, 1u);
                 }
-                umma_commit(&H->pv_done[n_pv & 1]);
+                umma_commit(&H->pv_done[gt & 1]);
                 umma_commit(&H->kv_empty[stage]);
             }
             __syncwarp();
-            ++n_pv;
         };
         for (int id = blockIdx.x; item_at(W, D, seq_lens, id, it); id += gridDim.x, ++n_item) {
             mbar_wait(&H->q_ready, n_item & 1);
-            for (int j = 0; j < it.n_tiles; ++j, ++g) {
-                const int stage = (int)(g % kKvStages);
-                const uint32_t sb = g & 1;
-                mbar_wait(&H->kv_full[stage], (g / kKvStages) & 1);
-                mbar_wait(&H->s_free[sb], ((g >> 1) & 1) ^ 1);
-                tc_fence_after();
-                if (elect_one()) {
-                    const uint32_t k_lo = (uint32_t)umma_desc_sw128(smem_u32(sKV) + (uint32_t)stage * kKvStageBytes);
-                    const uint32_t d = tmem_base + kColS + sb * kKvTile;
-#pragma unroll
-                    for (int ks = 0; ks < 8; ++ks) {
-                        // Q: [plane][half][128 rows][128 B] -> half = ks / 4 at + 16 KiB, 32 B per step; K: halves 8 KiB apart
-                        const uint32_t qa = q_lo + (uint32_t)(ks >> 2) * 1024 + 2 * (ks & 3);
-                        const uint32_t kb = k_lo + (uint32_t)(ks >> 2) * 512 + 2 * (ks & 3);
-                        umma_bf16_lo(d, qa, kb, k_hi32, k_hi32, idesc_s, ks == 0 ? 0u : 1u);
-                        umma_bf16_lo(d, qa + 2048, kb, k_hi32, k_hi32, idesc_s, 1u);       // the lo plane of q, 32 KiB further
-                    }
-                    umma_commit(&H->s_full[sb]);
-                }
-                __syncwarp();
-                if (j > 0) issue_pv(g - 1, j == 1);
+            const uint32_t n = (uint32_t)it.n_tiles;
+            issue_s(g);
+            if (n > 1) issue_s(g + 1);
+            for (uint32_t j = 0; j < n; ++j) {
+                issue_pv(g + j, j == 0);
+                if (j + 2 < n) issue_s(g + j + 2);
             }
-            issue_pv(g - 1, it.n_tiles == 1);
+            g += n;
         }
     } else {
         // ===================== softmax warps: one query row per thread, the tile's 64 columns shared by two warps =====================
@@ -308,16 +313,13 @@ k_prefill_attn(const int* __restrict__ seq_lens, CcKv kv, CcDims D, CcWork W, co
             const int p_row = seq_lens[it.row0 + tl] - 1;              // kv positions 0 .. p_row are visible
             float m_run = -INFINITY, l_run = 0.f;                      // l_run: the sum over THIS warp's columns
             for (int j = 0; j < it.n_tiles; ++j, ++g) {
-                const uint32_t sb = g & 1;
+                const uint32_t sb = g % kSBufs;
                 const int kv0 = j * kKvTile + half * 32;               // kv position of this warp's first column
-                mbar_wait(&H->s_full[sb], (g >> 1) & 1);
+                mbar_wait(&H->s_full[sb], (g / kSBufs) & 1);
                 tc_fence_after();
                 uint32_t sv[32];
                 tmem_ld_32x32b_x32(lane_addr + kColS + sb * kKvTile + half * 32, sv);
                 tmem_ld_wait();
-                tc_fence_before();
-                __syncwarp();
-                if (lane == 0) mbar_arrive(&H->s_free[sb]);
                 float mx = -INFINITY;
                 const int lim = p_row - kv0;                           // columns 0 .. lim (of this warp's 32) are visible
                 if (__all_sync(0xffffffffu, lim >= 31)) {              // not on the diagonal for this warp's rows: no mask
@@ -363,8 +365,7 @@ k_prefill_attn(const int* __restrict__ seq_lens, CcKv kv, CcDims D, CcWork W, co
                     tmem_st_wait();
                 }
                 const float m_new = m_run;
-                const uint32_t pb = n_pv & 1;                          // == sb: the probabilities replace the tile's scores (both
-                                                                       // warps of the pair have theirs in registers: the barrier above)
+                // the probabilities replace the tile's scores: both warps of the pair have theirs in registers (the barrier above)
                 if (j == it.n_tiles - 1 && it.s_last < j * kKvTile + kKvTile) {
                     // ragged last tile: V rows past the last position hold other data (or nothing): p = 0 must meet 0
                     mbar_wait(&H->kv_full[g % kKvStages], (g / kKvStages) & 1);
@@ -384,14 +385,14 @@ k_prefill_attn(const int* __restrict__ seq_lens, CcKv kv, CcDims D, CcWork W, co
                     lsum += p0 + p1;
                     split_hilo(p0, p1, hi[i], lo[i]);
                 }
-                tmem_st_32x32b_x16(lane_addr + kColS + pb * kKvTile + half * 16, hi);
-                tmem_st_32x32b_x16(lane_addr + kColS + pb * kKvTile + 32 + half * 16, lo);
+                tmem_st_32x32b_x16(lane_addr + kColS + sb * kKvTile + half * 16, hi);
+                tmem_st_32x32b_x16(lane_addr + kColS + sb * kKvTile + 32 + half * 16, lo);
                 tmem_st_wait();
                 l_run = l_run * alpha + lsum;
                 if (j == it.n_tiles - 1 && it.s_last < j * kKvTile + kKvTile) fence_proxy_async_smem();   // the zeroed V rows
                 tc_fence_before();
                 __syncwarp();
-                if (lane == 0) mbar_arrive(&H->p_full[pb]);
+                if (lane == 0) mbar_arrive(&H->p_full[sb]);
                 ++n_pv;
             }
             have = item_at(W, D, seq_lens, id + (int)gridDim.x, nx);
@@ -430,7 +431,7 @@ k_prefill_attn(const int* __restrict__ seq_lens, CcKv kv, CcDims D, CcWork W, co
     }
     tc_fence_before();
     __syncthreads();
-    if (warp == 1) tmem_dealloc<256>(tmem_base);
+    if (warp == 1) tmem_dealloc<512>(tmem_base);
 }
 
 }  // namespace
