@@ -407,6 +407,32 @@ cc_status cc_slotalloc_alloc(cc_slotalloc *a, uint64_t bytes, uint64_t *addr); /
 cc_status cc_slotalloc_free(cc_slotalloc *a, uint64_t addr);
 uint64_t cc_slotalloc_free_bytes(const cc_slotalloc *a);
 
+/* ---- an entry point that allocates nothing ---------------------------------------------------------------------
+ * Paged GQA decode attention as a stand-alone call for callers that cannot
+ * allocate device memory: it needs no cc_ctx and no layer and calls no cudaMalloc / cudaFree / allocating library
+ * routine.  Its split-KV partial results live in ONE file-scope device array of CC_STATIC_SCRATCH_BYTES that every GPU
+ * which loads the library holds until the process exits (cc_forward keeps the same partials in the layer workspace that
+ * cc_create_layer allocates, and is the fast path: TMA page boxes, one CTA per SM).
+ *   q           device, fp32 [batch][n_q_heads][head_dim], post-RoPE, unscaled (the 1/sqrt(head_dim) is applied here)
+ *   k_pool,     device, bf16 [n_pages][n_kv_heads][16][head_dim] (the layout of cc_forward's pools), read only
+ *   v_pool
+ *   block_table device, int32 [batch][max_blocks]; entries below ceil(seq_len / 16) must be valid page ids (an id
+ *               outside [0, n_pages) is read as page 0, never out of bounds)
+ *   seq_lens    device, int32 [batch]; row b attends positions 0 .. seq_lens[b] - 1; a row with seq_lens[b] <= 0 gives zeros
+ *   out         device, fp32 [batch][n_q_heads][head_dim], written
+ *   stream      a cudaStream_t of the CURRENT device (NULL = the default stream); the call only enqueues
+ * head_dim 64 or 128; n_q_heads a multiple of n_kv_heads, at most 16 times it.  Sizes whose partial results do not fit
+ * the array even with one range per row (64 KiB + batch * n_q_heads * (head_dim + 2) * 4 bytes > CC_STATIC_SCRATCH_BYTES,
+ * or batch * n_kv_heads > 16384) are rejected with CC_ERR_INVALID and a message naming the limit.  The first call on a
+ * device takes the array's address (cudaGetSymbolAddress with that device current): make it outside a stream capture.
+ * Every call on a device shares the array: calls that OVERLAP on the GPU race -- use one stream, or order them with
+ * events.  The result does not depend on which block finishes last (ranges are merged in range order). */
+#define CC_STATIC_SCRATCH_BYTES ((size_t)8 << 20)
+size_t cc_static_scratch_bytes(void);
+cc_status cc_attention_decode_static(const float *q, const void *k_pool, const void *v_pool, const int32_t *block_table,
+                                     const int32_t *seq_lens, float *out, int batch, int n_q_heads, int n_kv_heads,
+                                     int head_dim, int max_blocks, int n_pages, void *stream);
+
 const char *cc_last_error(void);
 const char *cc_version(void);
 

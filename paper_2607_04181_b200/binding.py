@@ -34,6 +34,7 @@ EXPORTS = (
     "cc_forward_host", "cc_forward_host_async", "cc_forward_profiled", "cc_forward_launch_count", "cc_layer_gemm_grids", "cc_replica_copy", "cc_kv_plan_migration", "cc_kv_plan_catchup", "cc_kv_migrate", "cc_debug_tap", "cc_debug_grouping", "cc_debug_trace",
     "cc_slotalloc_create", "cc_slotalloc_destroy", "cc_slotalloc_donate", "cc_slotalloc_reclaim",
     "cc_slotalloc_alloc", "cc_slotalloc_free", "cc_slotalloc_free_bytes", "cc_last_error", "cc_version",
+    "cc_static_scratch_bytes", "cc_attention_decode_static",
     "cc_ctl_mem_bytes", "cc_ctl_flops", "cc_ctl_comm_seconds", "cc_ctl_speedup", "cc_ctl_speedup_vec", "cc_ctl_distance",
     "cc_ctl_candidate_count", "cc_ctl_decide", "cc_ctl_place",
 )
@@ -274,6 +275,22 @@ def cc_forward_launch_count(layer) -> int:
     n = C.c_int()
     _check(_lib.cc_forward_launch_count(layer, C.byref(n)))
     return n.value
+
+
+# ---- the entry point that allocates nothing (include/cocoscale.h) -------------------------------------
+_lib.cc_static_scratch_bytes.restype = C.c_size_t
+
+
+def cc_static_scratch_bytes() -> int:
+    return int(_lib.cc_static_scratch_bytes())
+
+
+def cc_attention_decode_static(q, k_pool, v_pool, block_table, seq_lens, out, batch: int, n_q_heads: int, n_kv_heads: int,
+                               head_dim: int, max_blocks: int, n_pages: int, stream=None) -> None:
+    """Device pointers / torch CUDA tensors in, `out` written on the device; needs no context or layer."""
+    _check(_lib.cc_attention_decode_static(_ptr(q), _ptr(k_pool), _ptr(v_pool), _ptr(block_table), _ptr(seq_lens), _ptr(out),
+                                           C.c_int(batch), C.c_int(n_q_heads), C.c_int(n_kv_heads), C.c_int(head_dim),
+                                           C.c_int(max_blocks), C.c_int(n_pages), _stream(stream)))
 
 
 def cc_replica_copy(ctx, dst, src, nbytes: int, chunk_bytes: int = 0, stream=None) -> None:

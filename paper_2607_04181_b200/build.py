@@ -17,7 +17,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libcocoscale.so")
 SOURCES = ["cc_api.cu", "cc_kernels.cu", "cc_rowwise.cu", "cc_gemm.cu", "cc_attention.cu", "cc_control.cu", "cc_big.cu", "cc_big_gemm.cu",
-           "cc_prefill.cu"]
+           "cc_prefill.cu", "cc_noalloc.cu"]
 HEADERS = ["cc_common.cuh", "cc_kernels.h", "cc_epilogue.cuh", os.path.join("..", "..", "include", "cocoscale.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-Xcompiler", "-fPIC,-fvisibility=hidden", "--threads", "4"]

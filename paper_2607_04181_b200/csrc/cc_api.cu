@@ -31,6 +31,10 @@ cc_status fail(cc_status st, const char* fmt, ...) {
     g_err = buf;
     return st;
 }
+}  // namespace
+// for the other translation units of the library (cc_noalloc.cu): what cc_last_error() returns on this thread
+void cc_internal_set_error(const char* msg) { g_err = msg ? msg : ""; }
+namespace {
 #define CC_CUDA(expr)                                                                              \
     do {                                                                                           \
         cudaError_t e_ = (expr);                                                                   \
