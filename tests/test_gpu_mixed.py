@@ -220,3 +220,78 @@ def test_too_many_decode_rows_are_reported_not_faulted():
         assert B.cc_poll_device_error(S.ctx) == B.CC_DEVERR_TOO_MANY_DECODE
         o = S.tap(B.CC_TAP_O, 300)
     within(o[:256], ref["taps"]["o"][:256], "attention output of the first 256 decode rows")
+
+
+def test_cfg4_full_size_mixed_step_on_sampled_oracle_rows():
+    """BASELINE.json configs[3] at FULL size, the step `bench.py --workload cfg4` times: the 14B-class layer, two
+    2048-token prompt chunks from position 0 and 256 decode rows with contexts U{256..4096} = 4352 rows in one cc_forward,
+    two replicas (prompt r on replica r % 2, decode rows alternate).  The oracle cannot run 4352 rows of this layer in a
+    test's time, so: (1) the K/V every row of the step appends -- the oracle's own a1-a4 (rmsnorm, matmul_wt, rope, bf16
+    round: oracle/cc_oracle.c orc_sub_batch) over ALL rows -- against the GPU's cache, slot by slot, every other slot
+    bit-identical to the input; (2) with those K/V in the cache, oracle.layer_forward on SAMPLED rows one by one: the
+    first, second, tile-boundary (G = 5: 25 tokens per query tile; kv tiles of 64), middle and last tokens of both chunks,
+    the decode rows with the shortest and the longest context and six more -- layer output and the taps q, o, h1."""
+    import torch
+    from paper_2607_04181_b200 import binding as B
+    from paper_2607_04181_b200.harness import DeviceStep, Session
+
+    shape = I.LayerShape("cfg4full", 5120, 40, 8, 128, 17408, 1e-5, 500000.0, 256, 256, 4096)
+    Hkv, Dh, page = shape.n_kv_heads, shape.head_dim, shape.page
+    rng = np.random.default_rng(44)
+    dec_ctx = rng.integers(256, 4097, 256)
+    dec_ctx[0], dec_ctx[1] = 4096, 256
+    st, assign = mixed_step(shape, 44, [(0, 2048), (0, 2048)], dec_ctx, 2)
+    batch = st.hidden.shape[0]
+    assert batch == 4352
+    w = I.make_weights(shape, 1004)
+    with Session(shape, w, max_batch=batch, max_blocks=st.block_table.shape[1],
+                 max_position=st.block_table.shape[1] * page) as S:
+        S.scale(2)
+        step = DeviceStep(st, assign)
+        S.forward(step)
+        torch.cuda.synchronize()
+        assert B.cc_poll_device_error(S.ctx) == 0
+        out, (kp, vp) = step.out_bits(), step.pools_bits()
+        gt = {n: S.tap(t, batch) for n, t in (("q", B.CC_TAP_Q), ("o", B.CC_TAP_O), ("h1", B.CC_TAP_H1))}
+        del step
+    # (1) the appended K/V of all rows
+    seq = st.seq_lens.astype(np.int64)
+    x = oracle.rmsnorm(I.bf16_bits_to_f32(st.hidden), w["g1"], shape.rms_eps)
+    k, v = oracle.matmul_wt(x, w["wk"]), oracle.matmul_wt(x, w["wv"])
+    for b in range(batch):
+        k[b] = oracle.rope(k[b], Hkv, Dh, int(seq[b]) - 1, shape.rope_base)
+    kb = I.f32_to_bf16_bits(k).reshape(batch, Hkv, Dh)
+    vb = I.f32_to_bf16_bits(v).reshape(batch, Hkv, Dh)
+    pg = st.block_table[np.arange(batch), (seq - 1) // page]
+    sl = (seq - 1) % page
+    rel_k = within(I.bf16_bits_to_f32(kp[pg, :, sl, :]), I.bf16_bits_to_f32(kb), "appended K of all 4352 rows")
+    rel_v = within(I.bf16_bits_to_f32(vp[pg, :, sl, :]), I.bf16_bits_to_f32(vb), "appended V of all 4352 rows")
+    for mine, theirs in ((st.k_pool, kp), (st.v_pool, vp)):          # nothing else in the cache changed
+        tmp = mine.copy()
+        tmp[pg, :, sl, :] = theirs[pg, :, sl, :]
+        assert np.array_equal(tmp, theirs)
+        del tmp
+    # (2) sampled rows through the whole layer
+    kin, vin = st.k_pool.copy(), st.v_pool.copy()
+    kin[pg, :, sl, :] = kb
+    vin[pg, :, sl, :] = vb
+    starts = np.nonzero(seq == 1)[0]
+    assert len(starts) == 2
+    in_chunk = np.zeros(batch, bool)
+    sample = []
+    for s0 in starts:
+        assert np.array_equal(seq[s0:s0 + 2048], np.arange(1, 2049))
+        in_chunk[s0:s0 + 2048] = True
+        sample += [s0 + t for t in (0, 1, 24, 25, 63, 64, 1023, 2047)]
+    dec = np.nonzero(~in_chunk)[0]
+    assert len(dec) == 256
+    sample += [int(dec[np.argmax(seq[dec])]), int(dec[np.argmin(seq[dec])])] + [int(b) for b in rng.choice(dec, 6, replace=False)]
+    sample = np.array(sorted(set(sample)))
+    ref = oracle.layer_forward(shape, w, st.hidden[sample], kin, vin, st.block_table[sample], st.seq_lens[sample], assign[sample],
+                               2, taps=True)
+    rel = {"k": rel_k, "v": rel_v}
+    for n in ("q", "o", "h1"):
+        rel[n] = within(gt[n][sample], ref["taps"][n], f"tap {n} of the sampled rows")
+    rel["out"] = within(I.bf16_bits_to_f32(out[sample]), I.bf16_bits_to_f32(ref["out"]), "layer output of the sampled rows")
+    print("cfg4 full size, sampled rows, normalised rms error per stage:", {a: round(b, 5) for a, b in rel.items()})
+    assert max(rel.values()) < 1e-2, rel
