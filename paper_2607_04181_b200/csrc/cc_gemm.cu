@@ -458,6 +458,8 @@ constexpr int kClRows = 192;                  // grouped rows (n_pos) the two ac
 constexpr int kClMaxS = 8;
 constexpr int kClMaxStages = 8;              // ring depth of the one-tile variant (24 KiB stages at batch 64; 12 measured slower)
 
+__device__ __forceinline__ bool planes_out_one(const CcDims& D) { return D.pl[CC_OP_A] == 1; }
+
 template <int KIND, int TILES>
 __global__ void __launch_bounds__(kGemmThreads, 1)
 k_gemm_cl(CcGemmGeo G, const uint8_t* __restrict__ act, CcEpi E, CcDims D, CcWork W, const CcLayerTable* __restrict__ tab, int S) {
@@ -668,6 +670,73 @@ k_gemm_cl(CcGemmGeo G, const uint8_t* __restrict__ act, CcEpi E, CcDims D, CcWor
     if (nmax == 0) {                                                 // nothing runs this step (the same in every CTA of the cluster)
         pdl_wait();
         if (warp == 1) tmem_dealloc<kTmemCols>(tmem_base);
+        return;
+    }
+    if (KIND == EPI_GU && S == 1 && D.fmt == CC_FMT_F16 && planes_out_one(D)) {
+        // ---- gate/up alone on its super tile (no split-K, no exchange): SwiGLU straight from tensor memory ----
+        // The generic tail below moves the fp32 accumulators through shared memory and then runs one warp per (column, tile)
+        // item: 250 instructions per two items, four passes per warp at batch 64 = 4.5 us in which HBM idles and the down
+        // projection waits.  Here the warps pair gate (even TMEM lane) with up (odd lane) by one shuffle,
+        // apply the row scale and SiLU in registers, and drop the fp16 results into an image of the operand rows in the
+        // (dead) ring -- [tile][column][128 B], 16-byte chunks swizzled as in a_act; then all threads copy the image out
+        // in 16-byte chunks.
+        uint8_t* img = stage0;
+        const int kb_end = D.dn.KB;                                  // tiles at or beyond it are padding of the last super tile
+        {
+            // all sixteen warps (the producer, the issuer and the helpers are done): four per TMEM lane quarter share the
+            // 8-column chunks
+            const int q = warp & 3, grp = warp >> 2, odd = lane & 1;
+            const int jo = q * 16 + (lane >> 1);                     // output (= down-projection k) index within the tile's 64
+            tc_fence_after();
+            for (int c0 = grp * 8; c0 < n_pos; c0 += 32) {
+                uint32_t v[TILES][8];
+#pragma unroll
+                for (int j = 0; j < TILES; ++j)
+                    asm volatile("tcgen05.ld.sync.aligned.32x32b.x8.b32 {%0, %1, %2, %3, %4, %5, %6, %7}, [%8];"
+                                 : "=r"(v[j][0]), "=r"(v[j][1]), "=r"(v[j][2]), "=r"(v[j][3]), "=r"(v[j][4]), "=r"(v[j][5]), "=r"(v[j][6]),
+                                   "=r"(v[j][7])
+                                 : "r"(tmem_base + ((uint32_t)(q * 32) << 16) + (uint32_t)j * 256 + (uint32_t)c0)
+                                 : "memory");
+                tmem_ld_wait();
+                // the even lane (gate) finishes columns c0 .. c0 + 3, the odd lane (up) columns c0 + 4 .. c0 + 7
+#pragma unroll
+                for (int i = 0; i < 4; ++i) {
+                    const int col = c0 + 4 * odd + i;
+                    const bool live = col < n_pos && H->perm[min(col, n_pos - 1)] >= 0;
+                    const float inv = __int_as_float(H->aux[min(col, n_pos - 1)]);
+                    uint8_t* dst = img + (size_t)col * 128 + (((jo >> 3) ^ (col & 7)) << 4) + (jo & 7) * 2;
+#pragma unroll
+                    for (int j = 0; j < TILES; ++j) {
+                        const uint32_t mine = odd ? v[j][4 + i] : v[j][i];
+                        const uint32_t send = odd ? v[j][i] : v[j][4 + i];
+                        const uint32_t recv = __shfl_xor_sync(0xffffffffu, send, 1);
+                        const float g0 = __uint_as_float(odd ? recv : mine) * inv, u0 = __uint_as_float(odd ? mine : recv) * inv;
+                        // silu(g) u with the special-function unit's 2^x and 1/x (a few ulp from the IEEE division of the
+                        // generic tail; g -> -inf gives -0, g -> +inf gives g)
+                        float ex;
+                        asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(ex) : "f"(g0 * -1.4426950408889634f));
+                        float a = g0 * __frcp_rn(1.f + ex) * u0;
+                        a = fminf(fmaxf(a, -65504.f), 65504.f);
+                        if (live && tile0 + j < kb_end) *reinterpret_cast<__half*>(dst + (size_t)j * n_pos * 128) = __float2half_rn(a);
+                    }
+                }
+            }
+        }
+        tc_fence_before();
+        __syncthreads();
+        if (warp == 1) tmem_dealloc<kTmemCols>(tmem_base);
+        if (threadIdx.x == 0) CC_TP(W, 2 + KIND, 4);
+        for (int id = (int)threadIdx.x; id < TILES * n_pos * 8; id += kGemmThreads) {
+            const int j = id / (n_pos * 8), rem = id - j * n_pos * 8, col = rem >> 3, c = rem & 7;
+            if (tile0 + j >= kb_end || H->perm[col] < 0) continue;
+            const uint4 val = *reinterpret_cast<const uint4*>(img + ((size_t)j * n_pos + col) * 128 + c * 16);
+            // physical chunk c of the row holds the values k = kb * 64 + (c ^ (col & 7)) * 8 ..
+            *reinterpret_cast<uint4*>(W.a_act + act_chunk_off(col, (tile0 + j) * 64 + ((c ^ (col & 7)) << 3), D.Mpad, 1, 0)) = val;
+        }
+#ifdef CC_TRACE
+        __syncthreads();
+        if (threadIdx.x == 0) CC_TP(W, 2 + KIND, 5);
+#endif
         return;
     }
     // The first items of this warp's epilogue are known already (my columns, the row tables): issue their global loads
