@@ -29,13 +29,15 @@ def main() -> None:
     ap = argparse.ArgumentParser()
     ap.add_argument("--replicas", type=int, default=1)
     ap.add_argument("--replays", type=int, default=7)
+    ap.add_argument("--batch", type=int, default=0, help="decode rows (default: the cfg2 batch, 64)")
     args = ap.parse_args()
     shape = I.CFG2
+    batch = args.batch or shape.batch
     w = I.make_weights(shape, 1002)
-    st = I.make_step_inputs(shape, 2002, 3002)
-    S = Session(shape, w, max_batch=shape.batch, n_slots=3)
+    st = I.make_step_inputs(shape, 2002, 3002, batch=batch)
+    S = Session(shape, w, max_batch=batch, n_slots=3)
     S.scale(args.replicas)
-    step = DeviceStep(st, I.even_split(shape.batch, args.replicas))
+    step = DeviceStep(st, I.even_split(batch, args.replicas))
     for _ in range(3):
         S.forward(step)
     torch.cuda.synchronize()
@@ -53,7 +55,7 @@ def main() -> None:
         raw = B.cc_debug_trace(S.ctx, reset=True).astype(np.float64)
         rel.append((raw - raw[0, 0, 0]) / 1e3)
     t = np.median(np.stack(rel), axis=0)
-    print(f"cfg2 layer, R={args.replicas}, graph replay with PDL; us relative to the prologue's entry, median of {args.replays} "
+    print(f"cfg2 layer, batch {batch}, R={args.replicas}, graph replay with PDL; us relative to the prologue's entry, median of {args.replays} "
           f"replays; each point: min..max over the CTAs")
     for k, name, npt in KERNELS:
         print(f"{name:13s}", " | ".join(f"{t[k, pt, 0]:7.2f}..{t[k, pt, 1]:7.2f}" for pt in range(npt)))
