@@ -58,6 +58,8 @@ struct GlobalTab {
 struct TileIter {                             // walks this pair's tiles: (replica group r, super tile st, row block rb)
     int r, st, rb, row0, rows;                // row0: first grouped row of the block; rows: live rows in it
 };
+// MMA N of a row block: its rows rounded up to 32 (each CTA of the pair stages half of them, a multiple of 16)
+__device__ __forceinline__ int tile_n(int rows) { return (rows + 31) & ~31; }
 __device__ __forceinline__ bool tile_at(const BigHdr* H, int ST, long long t, TileIter& it) {
 #pragma unroll
     for (int r = 0; r < CC_MAXR; ++r) {
@@ -87,7 +89,7 @@ k_big_gemm(CcGemmGeo G, const uint8_t* __restrict__ act, CcEpi E, CcDims D, CcWo
     const uint32_t rank = cluster_ctarank();
     const int pair = blockIdx.x >> 1, n_pairs = gridDim.x >> 1;
     const int planes = D.pl[KIND];
-    const uint32_t b_bytes = 128u * 128u * (uint32_t)planes;          // this CTA's 128 rows of one k-block
+    const uint32_t b_bytes = 128u * 128u * (uint32_t)planes;          // this CTA's rows of one k-block, at most 128
     const uint32_t stage_bytes = CC_A_TILE_BYTES + b_bytes;
     const int n_stages = planes == 1 ? 6 : 4;
     uint8_t* stage0 = smem_raw + kBigHdrBytes;
@@ -134,14 +136,17 @@ k_big_gemm(CcGemmGeo G, const uint8_t* __restrict__ act, CcEpi E, CcDims D, CcWo
         TileIter it;
         for (long long t = pair; tile_at(H, G.ST, t, it); t += n_pairs) {
             const uint8_t* wsrc = uniform(H->blob[it.r]) + G.w_off + cc_atom_off(G.KB, it.st * CC_G + (int)rank, 0);
-            const uint8_t* asrc = act + (size_t)((it.row0 + (int)rank * 128) >> 3) * planes * 1024;
+            // a ragged last row block of a replica group is an MMA of N = its rows rounded up to 32 (half from each CTA), not 256
+            const int half = tile_n(it.rows) >> 1;
+            const uint32_t bt_bytes = (uint32_t)half * 128u * (uint32_t)planes;
+            const uint8_t* asrc = act + (size_t)((it.row0 + (int)rank * half) >> 3) * planes * 1024;
             for (int kb = 0; kb < G.KB; ++kb) {
                 mbar_wait(&H->empty[stage], ph ^ 1);
                 if (elect_one()) {
                     uint8_t* s = stage0 + (size_t)stage * stage_bytes;
-                    mbar_expect_tx(&H->full[stage], stage_bytes);
+                    mbar_expect_tx(&H->full[stage], CC_A_TILE_BYTES + bt_bytes);
                     bulk_g2s(s, wsrc, CC_A_TILE_BYTES, &H->full[stage]);
-                    bulk_g2s_hint(s + CC_A_TILE_BYTES, asrc, b_bytes, &H->full[stage], pol_a);
+                    bulk_g2s_hint(s + CC_A_TILE_BYTES, asrc, bt_bytes, &H->full[stage], pol_a);
                 }
                 wsrc += (size_t)CC_G * CC_A_TILE_BYTES;
                 asrc += kb_stride;
@@ -169,13 +174,13 @@ k_big_gemm(CcGemmGeo G, const uint8_t* __restrict__ act, CcEpi E, CcDims D, CcWo
         const uint32_t b_hi = (uint32_t)(umma_desc_sw128(0, (uint32_t)planes * 1024u) >> 32);
         const uint32_t desc_lo0 = (uint32_t)umma_desc_sw128(smem_u32(stage0));
         const uint32_t dstage = stage_bytes >> 4, dact = CC_A_TILE_BYTES >> 4;
-        const uint32_t idesc = umma_idesc_pair_m256(kBlockRows, D.fmt);
         TileIter it;
         for (long long t = pair; tile_at(H, G.ST, t, it); t += n_pairs, ++pc) {
             const uint32_t buf = pc & 1;
             mbar_wait(&H->tmem_empty[buf], ((pc >> 1) & 1) ^ 1);
             tc_fence_after();
             const uint32_t d_tmem = tmem_base + buf * 256;
+            const uint32_t idesc = umma_idesc_pair_m256((uint32_t)tile_n(it.rows), D.fmt);
             for (int kb = 0; kb < G.KB; ++kb) {
                 mbar_wait(&H->full[stage], ph);
                 mbar_wait(&H->peer_full[stage], ph);
